@@ -1,0 +1,380 @@
+"""Pins for oracle/sphere.py and oracle/direct_sums.c (CPU only).
+
+Every check compares the oracle with something other than itself: closed forms,
+Wigner's explicit factorial sum evaluated in mpmath, scipy's special functions,
+orthogonality by Gauss-Legendre quadrature, the literal sum of Eq. 16, least
+squares, high-precision mpmath quadrature, and the cited fixtures of tests/golden/.
+"""
+import math
+import os
+
+import mpmath as mp
+import numpy as np
+import pytest
+import scipy.special as sc
+
+from oracle import sphere as S
+from paper_2402_01282_b200 import inputs as I
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+LD = np.longdouble
+
+
+def wigner_d_explicit(l, m, n, beta):
+    """Wigner's factorial sum for d^l_{mn}(beta) = <l m|exp(-i beta J_y)|l n> (Varshalovich et al. 1989,
+    cited PAPER.md:434), evaluated in 40-digit mpmath."""
+    mp.mp.dps = 40
+    b = mp.mpf(beta)
+    c, s = mp.cos(b / 2), mp.sin(b / 2)
+    pre = mp.sqrt(mp.factorial(l + n) * mp.factorial(l - n) * mp.factorial(l + m) * mp.factorial(l - m))
+    tot = mp.mpf(0)
+    for k in range(max(0, n - m), min(l + n, l - m) + 1):
+        den = (mp.factorial(l + n - k) * mp.factorial(k) * mp.factorial(l - k - m) * mp.factorial(k - n + m))
+        tot += (-1) ** (k - n + m) * c ** (2 * l - 2 * k + n - m) * s ** (2 * k - n + m) / den
+    return pre * tot
+
+
+def random_flm(L, seed, real=False):
+    return (I.flm_real(L, seed, 1, "white") if real else I.flm_complex(L, seed, 1, "white"))[0]
+
+
+# ------------------------------------------------------------------ Wigner d
+@pytest.mark.parametrize("beta", [0.3, 1.1, 2.5, 3.0])
+def test_wigner_d_closed_forms(beta):
+    b = LD(beta)
+    c, s = np.cos(b), np.sin(b)
+    tol = 5e-18
+    assert abs(S.wigner_d(3, 1, 1, b)[1] - (1 + c) / 2) < tol
+    assert abs(S.wigner_d(3, 1, 0, b)[1] - (-s / np.sqrt(LD(2)))) < tol
+    assert abs(S.wigner_d(3, 1, -1, b)[1] - (1 - c) / 2) < tol
+    assert abs(S.wigner_d(3, 2, 0, b)[2] - np.sqrt(LD(6)) / 4 * s * s) < tol
+    assert abs(S.wigner_d(3, 2, 1, b)[2] - (-(1 + c) * s / 2)) < tol
+    assert abs(S.wigner_d(3, 0, 0, b)[2] - (3 * c * c - 1) / 2) < tol
+
+
+def test_wigner_d_matches_explicit_factorial_sum():
+    L = 10
+    for beta in (0.4, 1.7, 2.9):
+        for m in range(-(L - 1), L):
+            for n in range(-4, 5):
+                d = S.wigner_d(L, m, n, LD(beta))
+                for l in range(L):
+                    ref = 0.0 if l < max(abs(m), abs(n)) else float(wigner_d_explicit(l, m, n, beta))
+                    assert abs(float(d[l]) - ref) < 2e-15, (l, m, n, beta)
+
+
+def test_wigner_d_symmetries_and_end_values():
+    L, beta = 14, LD(0.9)
+    pi = S.pi("f80")
+    for m in range(-6, 7):
+        for n in range(-4, 5):
+            d = S.wigner_d(L, m, n, beta)
+            assert np.abs(d - (-1) ** (m - n) * S.wigner_d(L, n, m, beta)).max() < 1e-17
+            assert np.abs(d - S.wigner_d(L, -n, -m, beta)).max() < 1e-17
+            sign = np.array([(-1) ** (l + m) for l in range(L)], dtype=LD)
+            assert np.abs(S.wigner_d(L, m, -n, beta) - sign * S.wigner_d(L, m, n, pi - beta)).max() < 1e-16
+            l0 = max(abs(m), abs(n))
+            d0, dpi = S.wigner_d(L, m, n, LD(0)), S.wigner_d(L, m, n, pi)
+            for l in range(l0, L):
+                assert abs(d0[l] - (1 if m == n else 0)) < 1e-17
+                assert abs(dpi[l] - ((-1) ** (l - n) if m == -n else 0)) < 1e-15
+
+
+def test_wigner_d_orthogonality_by_gauss_legendre():
+    L = 24
+    x, w = np.polynomial.legendre.leggauss(64)
+    for (m, n) in ((0, 0), (3, 0), (5, 2), (-7, 4), (2, -2)):
+        D = np.array([S.wigner_d(L, m, n, LD(np.arccos(xi))).astype(float) for xi in x])  # [node][l]
+        G = np.einsum("i,il,ik->lk", w, D, D)
+        l0 = max(abs(m), abs(n))
+        expect = np.diag([2.0 / (2 * l + 1) if l >= l0 else 0.0 for l in range(L)])
+        assert np.abs(G - expect).max() < 1e-13
+
+
+@pytest.mark.parametrize("prec,L,tol", [("f80", 96, 1e-15), ("f64", 96, 1e-12), ("f64", 700, 1e-11)])
+def test_wigner_d_unitarity(prec, L, tol):
+    """sum_m (d^l_{mn})^2 = 1 at MW rings, for l up to L-1: catches a lost seed or a wrong coefficient."""
+    th = S.mw_thetas(L, prec)
+    for t in (0, L // 3, L // 2, L - 2):
+        for n in (0, 2):
+            tot = np.zeros(L, dtype=S.REAL[prec])
+            for m in range(-(L - 1), L):
+                tot += S.wigner_d(L, m, n, th[t], prec) ** 2
+            assert np.abs(tot[n:] - 1).max() < tol
+
+
+def test_wigner_d_legendre_and_jacobi():
+    L, beta = 40, 1.234
+    d = S.wigner_d(L, 0, 0, LD(beta)).astype(float)
+    assert np.abs(d - sc.eval_legendre(np.arange(L), np.cos(beta))).max() < 1e-14
+    # d^l_{mn} = (-1)^{m-n} sqrt((l+m)!(l-m)!/((l+n)!(l-n)!)) sin^{m-n}(b/2) cos^{m+n}(b/2) P^{(m-n,m+n)}_{l-m}(cos b), m>=|n|
+    for (m, n) in ((3, 1), (4, -2), (2, 2)):
+        d = S.wigner_d(L, m, n, LD(beta)).astype(float)
+        for l in range(m, 20):
+            pre = math.sqrt(math.factorial(l + m) * math.factorial(l - m) / (math.factorial(l + n) * math.factorial(l - n)))
+            ref = ((-1) ** (m - n) * pre * math.sin(beta / 2) ** (m - n) * math.cos(beta / 2) ** (m + n)
+                   * sc.eval_jacobi(l - m, m - n, m + n, math.cos(beta)))
+            assert abs(d[l] - ref) < 1e-13 * max(1, abs(ref))
+
+
+# ------------------------------------------------------------------ Y_lm, SHT
+def _mw_grid(L):
+    th = S.mw_thetas(L).astype(float)
+    ph = S.mw_phis(L).astype(float)
+    return np.meshgrid(th, ph, indexing="ij")
+
+
+def test_spherical_harmonics_closed_forms_and_scipy():
+    L = 6
+    TH, PH = _mw_grid(L)
+    closed = {
+        (0, 0): np.full_like(TH, 1 / math.sqrt(4 * math.pi)) + 0j,
+        (1, 0): math.sqrt(3 / (4 * math.pi)) * np.cos(TH) + 0j,
+        (1, 1): -math.sqrt(3 / (8 * math.pi)) * np.sin(TH) * np.exp(1j * PH),
+        (2, 0): math.sqrt(5 / (16 * math.pi)) * (3 * np.cos(TH) ** 2 - 1) + 0j,
+    }
+    for l in range(L):
+        for m in range(-l, l + 1):
+            flm = np.zeros((L, 2 * L - 1), dtype=complex)
+            flm[l, m + L - 1] = 1
+            Y = S.sht_inverse(flm, L).astype(complex)
+            assert np.abs(Y - sc.sph_harm_y(l, m, TH, PH)).max() < 1e-14
+            if (l, m) in closed:
+                assert np.abs(Y - closed[(l, m)]).max() < 1e-15
+
+
+@pytest.mark.parametrize("L", [1, 2, 5, 9, 16])
+def test_sht_forward_is_least_squares_inverse_of_independent_synthesis(L):
+    """Build the synthesis matrix from scipy's Y_lm (independent of the oracle), synthesise a random
+    band-limited signal with it, and require sht_forward to return the coefficients (Eq. 2, exact MW, R3)."""
+    TH, PH = _mw_grid(L)
+    flm = random_flm(L, 11 + L)
+    f = np.zeros_like(TH, dtype=complex)
+    cols, idx = [], []
+    for l in range(L):
+        for m in range(-l, l + 1):
+            Y = sc.sph_harm_y(l, m, TH, PH)
+            f += flm[l, m + L - 1] * Y
+            cols.append(Y.ravel())
+            idx.append((l, m + L - 1))
+    got = S.sht_forward(f, L).astype(complex)
+    assert np.abs(got - flm).max() < 2e-14
+    sol = np.linalg.lstsq(np.array(cols).T, f.ravel(), rcond=None)[0]
+    for (l, mi), v in zip(idx, sol):
+        assert abs(got[l, mi] - v) < 1e-12
+    assert np.abs(S.sht_inverse(flm, L).astype(complex) - f).max() < 1e-13
+
+
+def test_sht_round_trip_and_integral():
+    L = 33
+    flm = random_flm(L, 5)
+    f = S.sht_inverse(flm, L)
+    assert np.abs(S.sht_forward(f, L) - flm).max() < 1e-16
+    # int cos^2(theta) dOmega = 4pi/3 = sqrt(4pi) f_00
+    TH, _ = _mw_grid(L)
+    f00 = S.sht_forward(np.cos(TH) ** 2, L)[0, L - 1]
+    assert abs(complex(f00) * math.sqrt(4 * math.pi) - 4 * math.pi / 3) < 1e-14
+
+
+def test_f64_instance_agrees_with_f80():
+    L = 20
+    flm = random_flm(L, 9)
+    f80 = S.sht_inverse(flm, L, "f80")
+    f64 = S.sht_inverse(flm, L, "f64")
+    assert np.abs(f80 - f64).max() < 1e-13
+    assert np.abs(S.sht_forward(f64, L, "f64") - flm).max() < 1e-13
+
+
+# ------------------------------------------------------------------ Wigner transform
+def test_wigner_inverse_matches_literal_eq16_sum():
+    """W(alpha,beta,gamma) = sum_{l,m,n} X_{nlm} d^l_{mn}(beta) e^{i(m alpha + n gamma)}  (Eqs. 5, 16, 47)
+    with d from the explicit factorial sum, at a handful of samples."""
+    L, N = 5, 3
+    rng = np.random.default_rng(3)
+    X = np.zeros((2 * N - 1, L, 2 * L - 1), dtype=complex)
+    for n in range(-(N - 1), N):
+        for l in range(abs(n), L):
+            for m in range(-l, l + 1):
+                X[n + N - 1, l, m + L - 1] = rng.standard_normal() + 1j * rng.standard_normal()
+    W = S.wigner_inverse(X, L, N).astype(complex)
+    th, ph = S.mw_thetas(L).astype(float), S.mw_phis(L).astype(float)
+    for (g, t, a) in ((0, 0, 0), (1, 2, 3), (4, 4, 8), (2, 3, 5), (3, 1, 7)):
+        gam = 2 * math.pi * g / (2 * N - 1)
+        ref = 0
+        for n in range(-(N - 1), N):
+            for l in range(abs(n), L):
+                for m in range(-l, l + 1):
+                    ref += (X[n + N - 1, l, m + L - 1] * float(wigner_d_explicit(l, m, n, th[t]))
+                            * np.exp(1j * (m * ph[a] + n * gam)))
+        assert abs(W[g, t, a] - ref) < 1e-13
+
+
+@pytest.mark.parametrize("L,N", [(7, 3), (8, 4), (12, 1), (3, 3)])
+def test_wigner_forward_inverts_wigner_inverse(L, N):
+    rng = np.random.default_rng(L * 10 + N)
+    X = np.zeros((2 * N - 1, L, 2 * L - 1), dtype=complex)
+    for n in range(-(N - 1), N):
+        for l in range(abs(n), L):
+            for m in range(-l, l + 1):
+                X[n + N - 1, l, m + L - 1] = rng.standard_normal() + 1j * rng.standard_normal()
+    W = S.wigner_inverse(X, L, N)
+    back = S.wigner_forward(W, L, N)
+    # Eq. 5 carries (2l+1)/(8pi^2); wigner_inverse takes X = that factor times f^l_{mn}
+    ell = np.arange(L)
+    assert np.abs(back * ((2 * ell + 1) / (8 * math.pi ** 2))[None, :, None] - X).max() < 1e-15
+
+
+def test_wigner_transform_with_N1_reduces_to_sht():
+    L = 10
+    flm = random_flm(L, 2)
+    ell = np.arange(L).astype(LD)
+    c_l = np.sqrt((2 * ell + 1) / (4 * S.pi("f80")))
+    W = S.wigner_inverse((c_l[:, None] * flm)[None], L, 1)
+    assert np.abs(W[0] - S.sht_inverse(flm, L)).max() < 1e-17
+
+
+# ------------------------------------------------------------------ filters
+def _golden(name):
+    rows = []
+    with open(os.path.join(GOLDEN, name)) as fh:
+        for line in fh:
+            line = line.split("#")[0].strip()
+            if line:
+                rows.append(line.split())
+    return rows
+
+
+def test_zeta_worked_values_and_normalisation():
+    for row in _golden("zeta_worked_values.txt"):
+        N, l, m, val = int(row[0]), int(row[1]), int(row[2]), row[3]
+        z = S.zeta(l + 1, N)
+        assert abs(complex(z[l, m + N - 1]) - complex(eval(val, {"sqrt": math.sqrt, "j": 1j}))) < 3e-16
+    for N in (1, 2, 3, 4, 5, 6):
+        z = S.zeta(20, N)
+        tot = np.sum(np.abs(z) ** 2, axis=1).astype(float)
+        assert np.abs(tot[1:] - 1).max() < 1e-15
+        assert abs(tot[0] - (1 if N % 2 == 1 else 0)) < 1e-15
+        # real wavelet: zeta_{l,-m} = (-1)^m conj(zeta_{lm})   (O7)
+        for m in range(-(N - 1), N):
+            assert np.abs(z[:, -m + N - 1] - (-1) ** m * np.conj(z[:, m + N - 1])).max() == 0
+
+
+def test_k_lambda_against_mpmath_quadrature_and_golden():
+    mp.mp.dps = 30
+
+    def k_ref(t, lam):
+        def s2(u):  # s_lambda(u)^2 / u  (Eqs. A2-A3)
+            x = 2 * lam / (lam - 1) * (u - 1 / lam) - 1
+            return mp.exp(-2 / (1 - x ** 2)) / u if abs(x) < 1 else mp.mpf(0)
+        return mp.quad(s2, mp.linspace(t, 1, 9)) / mp.quad(s2, mp.linspace(mp.mpf(1) / lam, 1, 9))
+
+    for lam in (2, 3, 1.5):
+        for t in (0.55, 0.7, 0.9, 0.99):
+            if t <= 1 / lam:
+                continue
+            got = S.k_lambda(np.array([t], dtype=LD), lam)[0]
+            assert abs(float(got) - float(k_ref(mp.mpf(t), mp.mpf(lam)))) < 2e-16
+    for row in _golden("k_lambda_reference.txt"):
+        lam, t, val = float(row[0]), float(row[1]), float(row[2])
+        assert abs(float(S.k_lambda(np.array([t], dtype=LD), lam)[0]) - val) < 5e-16
+    k = S.k_lambda(np.linspace(0, 1.2, 200).astype(LD), 2)
+    assert k[0] == 1 and k[-1] == 0 and np.all(np.diff(k) <= 0)
+    assert S.k_lambda(np.array([0.5], dtype=LD), 2)[0] == 1 and S.k_lambda(np.array([1.0], dtype=LD), 2)[0] == 0
+
+
+@pytest.mark.parametrize("L,N,lam,J0", [(32, 1, 2, 0), (64, 3, 2, 2), (40, 4, 3, 1), (17, 2, 2, 0), (100, 5, 1.7, 3)])
+def test_admissibility_identity(L, N, lam, J0):
+    """Eq. 30: 4pi/(2l+1)|Phi_l0|^2 + 8pi^2/(2l+1) sum_{j,n} |Psi^j_ln|^2 = 1 for every l."""
+    psi, phi, J = S.filters(L, N, lam, J0)
+    ell = np.arange(L).astype(LD)
+    pi = S.pi("f80")
+    tot = 4 * pi / (2 * ell + 1) * phi ** 2 + 8 * pi ** 2 / (2 * ell + 1) * np.sum(np.abs(psi) ** 2, axis=(0, 2))
+    assert np.abs(tot - 1).max() < 1e-17
+
+
+def test_scale_supports_match_survey_table():
+    """First/last non-zero l per scale at L=1024, lam=2, J0=2 (R1c; SURVEY.md 8(c) pins)."""
+    kap, _ = S.kappa(1024, 2, 2, "f64")
+    got = []
+    for j in range(kap.shape[0]):
+        nz = np.nonzero(kap[j] > 0)[0]
+        got.append((int(nz[0]), int(nz[-1])))
+    rows = [(int(r[1]), int(r[2])) for r in _golden("scale_supports_L1024.txt")]
+    assert got == rows
+    for j, (lo, hi) in enumerate(got):
+        assert hi < S.bandlimit_of_scale(j + 2, 1024, 2, True)
+
+
+# ------------------------------------------------------------------ whole transform
+@pytest.mark.parametrize("L,N,lam,J0,mr,real", [
+    (16, 3, 2, 0, True, False), (16, 5, 2, 2, True, True), (12, 1, 2, 0, False, True),
+    (9, 2, 2, 0, True, True), (20, 4, 3, 1, True, False), (8, 3, 2, 0, False, False)])
+def test_wavelet_round_trip_energy_and_reality(L, N, lam, J0, mr, real):
+    flm = random_flm(L, 100 + L + N, real)
+    f = S.sht_inverse(flm, L)
+    if real:
+        assert np.abs(f.imag).max() < 1e-17
+    W_phi, W_psi = S.analysis(f, L, N, lam, J0, mr)
+    if real:
+        assert np.abs(W_phi.imag).max() < 1e-17
+        assert max(np.abs(w.imag).max() for w in W_psi.values()) < 1e-17
+    f2 = S.synthesis(W_phi, W_psi, L, N, lam, J0, mr)
+    assert np.abs(f2 - f).max() / np.abs(f).max() < 1e-16
+    # tight-frame energy identity on coefficients (Eq. 30 x |f_lm|^2)
+    psi, phi, J = S.filters(L, N, lam, J0)
+    ell = np.arange(L).astype(LD)
+    pi = S.pi("f80")
+    lhs = np.sum(np.abs(flm) ** 2)
+    rhs = np.sum(4 * pi / (2 * ell + 1) * phi ** 2 * np.sum(np.abs(flm) ** 2, axis=1))
+    for j in range(J0, J + 1):
+        Lj = S.bandlimit_of_scale(j, L, lam, mr)
+        what = S.wigner_forward(W_psi[j], Lj, N)           # = 8pi^2/(2l+1) f_lm Psi*_ln  (Eq. 27)
+        ellj = np.arange(Lj).astype(LD)
+        rhs += np.sum((2 * ellj + 1)[None, :, None] / (8 * pi ** 2) * np.abs(what) ** 2)
+    assert abs(lhs - rhs) / lhs < 1e-16
+
+
+def test_multiresolution_on_off_agree_in_harmonic_space():
+    L, N, lam, J0 = 16, 3, 2, 1
+    flm = random_flm(L, 77)
+    f = S.sht_inverse(flm, L)
+    _, W_on = S.analysis(f, L, N, lam, J0, True)
+    _, W_off = S.analysis(f, L, N, lam, J0, False)
+    for j in W_on:
+        Lj = S.bandlimit_of_scale(j, L, lam, True)
+        a = S.wigner_forward(W_on[j], Lj, N)
+        b = S._crop_lm(S.wigner_forward(W_off[j], L, N), L, Lj)
+        assert np.abs(a - b).max() < 1e-16
+
+
+def test_analysis_matches_literal_directional_convolution():
+    """W^{Psi j}(rho) = sum_{l,m,n} f_lm Psi^{j*}_ln D^{l*}_mn(rho)  (Eq. 16 with g = Psi^j; Eq. 26),
+    d from the explicit factorial sum, filters from the oracle; W^Phi = sum sqrt(4pi/(2l+1)) f_lm Phi_l0 Y_lm."""
+    L, N, lam, J0 = 8, 3, 2, 0
+    flm = random_flm(L, 21)
+    f = S.sht_inverse(flm, L)
+    W_phi, W_psi = S.analysis(f, L, N, lam, J0, True)
+    psi, phi, J = S.filters(L, N, lam, J0)
+    for j, (g, t, a) in ((3, (1, 5, 9)), (2, (4, 2, 11)), (1, (0, 3, 6)), (3, (2, 7, 14))):
+        Lj = S.bandlimit_of_scale(j, L, lam, True)
+        th, ph = S.mw_thetas(Lj).astype(float), S.mw_phis(Lj).astype(float)
+        gam = 2 * math.pi * g / (2 * N - 1)
+        ref = 0
+        for l in range(Lj):
+            for m in range(-l, l + 1):
+                for n in range(-min(l, N - 1), min(l, N - 1) + 1):
+                    ref += (complex(flm[l, m + L - 1]) * np.conj(complex(psi[j - J0, l, n + N - 1]))
+                            * float(wigner_d_explicit(l, m, n, th[t])) * np.exp(1j * (m * ph[a] + n * gam)))
+        assert abs(complex(W_psi[j][g, t, a]) - ref) < 1e-13
+    assert W_phi.shape == (1, 1)
+    assert abs(complex(W_phi[0, 0]) - complex(flm[0, L - 1]) * float(phi[0]) * math.sqrt(4 * math.pi)
+               / math.sqrt(4 * math.pi)) < 1e-15
+
+
+def test_input_recipes_are_stable():
+    """SHA-256 of the seeded coefficient arrays (detects a change of numpy's random stream)."""
+    for row in _golden("input_sha256.txt"):
+        name, digest = row[0], row[1]
+        if name in ("C3", "C4", "C5"):
+            continue  # large; checked in the gpu tests
+        assert I.sha256(I.config_coefficients(name)) == digest
