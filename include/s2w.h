@@ -1,0 +1,139 @@
+/* s2w.h -- C ABI of the B200-native scale-discretised directional wavelet transform
+ * on the sphere S^2 and the ball B^3 (hot path of arXiv:2402.01282).
+ *
+ * "P:n" = line n of PAPER.md (the paper text this library was written from).
+ * Every transform entry point runs hand-written sm_100a CUDA kernels in fp64; there is
+ * no CPU fallback.  Calls that need a device fail with S2W_ECUDA when none is present;
+ * the kernel-build calls (s2wav_kernels, s2ball_kernels, s2ball_radial_nodes) are pure
+ * host code and work without a GPU.
+ *
+ * Conventions:
+ *   MW sampling at band-limit L: theta_t = pi(2t+1)/(2L-1), t = 0..L-1;
+ *   phi_p = 2 pi p/(2L-1), p = 0..2L-2; gamma_g = 2 pi g/(2N-1), g = 0..2N-2.
+ *   Y_lm = sqrt((2l+1)/4pi) d^l_{m0}(theta) e^{i m phi};  D^l_mn = e^{-i m alpha} d^l_mn(beta) e^{-i n gamma}
+ *   (Eq. 47), d^l_mn(beta) = <l m| exp(-i beta J_y) |l n>.
+ *   Scales j = J0..J, J = smallest integer with lambda^J >= L; kappa^j(l) = kappa_lambda(l / lambda^j)
+ *   (Eq. A5); L_j = min(ceil(lambda^{j+1}), L) with multiresolution (Eq. 38), else L;
+ *   scaling band-limit L_s = min(ceil(lambda^{J0}), L) with multiresolution, else L.
+ *
+ * Layouts: C row-major.  Signals [batch][theta][phi]; sphere coefficients per signal: the scaling block
+ * [L_s][2L_s-1] first, then the scales ascending, each [2N-1 gamma][L_j beta][2L_j-1 alpha]
+ * (s2w_plan_scale_shape gives shapes and offsets); consecutive signals of a batch are
+ * s2w_plan_coeff_elems() apart.  With S2W_REAL elements are double, otherwise interleaved
+ * complex128 (re, im).  Ball: signal [P shells][L][2L-1]; coefficients: scaling block [P][L][2L-1],
+ * then scales ordered j' (radial) outer, j (angular) inner, each [P_j'][2N-1][L_j][2L_j-1].
+ *
+ * Ownership: the caller owns every signal, coefficient and workspace buffer (device memory);
+ * a plan owns only its own tables and is immutable after creation.
+ * Errors: every call returns 0 (S2W_OK) or a negative code; nothing throws across the ABI;
+ * s2w_last_error() returns a thread-local message.
+ */
+#ifndef S2W_H
+#define S2W_H
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct s2w_plan s2w_plan;
+
+enum { S2W_OK = 0, S2W_EINVAL = -1, S2W_ENOMEM = -2, S2W_ECUDA = -3, S2W_EUNSUPPORTED = -4 };
+enum { S2W_REAL = 1, S2W_PRECOMPUTE = 2 };
+
+/* ---- kernel-build calls (host only; Appendix A; "calculated and cached") ---- */
+
+/* Number of wavelet scales: writes J (top scale index) for band-limit L and dilation lambda. */
+int s2w_scale_count(int L, double lambda, int *J);
+
+/* Sphere filters.  psi: host [J-J0+1][L][2N-1] complex (re,im interleaved), Psi^j_{l n} at
+ * [j-J0][l][n+N-1] = sqrt((2l+1)/8pi^2) kappa^j(l) zeta_{l n} (Eq. A9 without p; zeta: Eq. A6);
+ * phi: host [L], Phi_{l 0} = sqrt((2l+1)/4pi) sqrt(k_lambda(l/lambda^J0)) (Eq. A10).
+ * Either pointer may be NULL.  EINVAL if L<1, N<1, N>L, lambda<=1, J0<0 or J0>J. */
+int s2wav_kernels(double *psi, double *phi, int L, int N, double lambda, int J0);
+
+/* Ball filters, stored separably (Eq. A9): kappa_l [J-J0+1][L] = kappa^j(l), kappa_p [J'-J0+1][P] =
+ * kappa^{j'}(p) = kappa_nu(p/nu^{j'}), zeta [L][2N-1] complex, phi [P][L] = Phi_{l 0 p} =
+ * sqrt((2l+1)/4pi) sqrt(a+b-ab), a = k_lambda(l/lambda^J0), b = k_nu(p/nu^J0)  (Eq. A10; reading R9).
+ * J0 is used for both the angular and the radial lowest scale (reading R10). */
+int s2ball_kernels(double *kappa_l, double *kappa_p, double *zeta, double *phi,
+                   int L, int P, int N, double lambda_l, double lambda_p, int J0);
+
+/* Gauss-Laguerre radial nodes (generalised, alpha = 2, reading R8): r [P] = tau x_i with L_P^(2)(x_i) = 0,
+ * and q [P] = tau^3 w_i e^{x_i}, the weight that multiplies f(r_i) K_p(r_i) in the quadrature of Eq. 7. */
+int s2ball_radial_nodes(double *r, double *q, int P, double tau);
+
+/* ---- plans: the cached precomputed components ---- */
+
+/* flags: S2W_REAL (signal and coefficients real), S2W_PRECOMPUTE (reserved: returns S2W_EUNSUPPORTED).
+ * batch = number of independent signals per call (>= 1).  device = CUDA device ordinal.
+ * Creation allocates device tables, runs set-up kernels and synchronises. */
+int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int multiresolution,
+                      int flags, int batch, int device);
+int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, double lambda_p, int J0,
+                       double tau, int flags, int device);
+int s2w_plan_destroy(s2w_plan *plan);
+
+/* Scale ranges: angular j = J0..J and (ball) radial j' = J0p..Jp (sphere: J0p = Jp = 0). */
+int s2w_plan_scales(const s2w_plan *plan, int *J0, int *J, int *J0p, int *Jp);
+/* Shape and element offset (within one signal's coefficient block) of scale (j, jp); j = -1 is the scaling block
+ * (n_gamma = 1).  n_r is the number of radial shells (1 on the sphere). */
+int s2w_plan_scale_shape(const s2w_plan *plan, int j, int jp, int *n_r, int *n_gamma, int *n_theta, int *n_phi,
+                         size_t *offset_elems);
+/* Elements (double or complex128) of one signal's coefficient block / of one signal. */
+size_t s2w_plan_coeff_elems(const s2w_plan *plan);
+size_t s2w_plan_signal_elems(const s2w_plan *plan);
+/* Bytes of device scratch the plan-level transforms need (caller allocates, 256-byte aligned). */
+size_t s2w_plan_workspace_bytes(const s2w_plan *plan);
+
+/* ---- transforms on an explicit plan: asynchronous on `stream`, no allocation, no host sync ---- */
+/* Analysis, Alg. 1 / Alg. 2: in = signal(s), out = coefficients. */
+int s2w_plan_forward(const s2w_plan *plan, const void *in_dev, void *out_dev, void *work_dev, void *stream);
+/* Synthesis, Alg. 1 / Alg. 2: in = coefficients, out = signal(s). */
+int s2w_plan_inverse(const s2w_plan *plan, const void *in_dev, void *out_dev, void *work_dev, void *stream);
+
+/* Harmonic-space taps used by the parity tests: forward spherical harmonic transform of the plan's signal(s)
+ * (steps a1-a3 of DESIGN.md) writing flm [batch][L][2L-1] complex128 at [l][m+L-1] (ball: [P][L][2L-1], after the
+ * radial transform: f_{lmp}), and its inverse. */
+int s2w_plan_harmonic_forward(const s2w_plan *plan, const void *f_dev, void *flm_dev, void *work_dev, void *stream);
+int s2w_plan_harmonic_inverse(const s2w_plan *plan, const void *flm_dev, void *f_dev, void *work_dev, void *stream);
+
+/* ---- the transforms named by the problem statement: explicit arguments, device pointers.
+ * The plan and its workspace are looked up in an internal cache keyed on the arguments (the first call builds them
+ * and synchronises; later calls are asynchronous on `stream`). ---- */
+int s2wav_forward(const void *f_dev, void *w_dev, int L, int N, double lambda, int J0, int multiresolution,
+                  int flags, int batch, void *stream);
+int s2wav_inverse(const void *w_dev, void *f_dev, int L, int N, double lambda, int J0, int multiresolution,
+                  int flags, int batch, void *stream);
+int s2ball_forward(const void *f_dev, void *w_dev, int L, int P, int N, double lambda_l, double lambda_p,
+                   int J0, double tau, int flags, void *stream);
+int s2ball_inverse(const void *w_dev, void *f_dev, int L, int P, int N, double lambda_l, double lambda_p,
+                   int J0, double tau, int flags, void *stream);
+
+/* Same, with HOST buffers: copies in, transforms, copies out, synchronises (the end-to-end path bench.py times). */
+int s2wav_forward_host(const void *f_host, void *w_host, int L, int N, double lambda, int J0, int multiresolution,
+                       int flags, int batch);
+int s2wav_inverse_host(const void *w_host, void *f_host, int L, int N, double lambda, int J0, int multiresolution,
+                       int flags, int batch);
+
+int s2ball_forward_host(const void *f_host, void *w_host, int L, int P, int N, double lambda_l, double lambda_p,
+                        int J0, double tau, int flags);
+int s2ball_inverse_host(const void *w_host, void *f_host, int L, int P, int N, double lambda_l, double lambda_p,
+                        int J0, double tau, int flags);
+
+/* Drop every cached plan and workspace. */
+int s2w_cache_clear(void);
+
+/* FP64 pipe probe: runs a register-resident DFMA chain (kind 0) or an mma.sync m8n8k4 f64 chain (kind 1) on
+ * `device` and writes the achieved TFLOP/s.  Used by bench.py to report the measured ALU peak. */
+int s2w_probe_fp64(int kind, int device, double *tflops);
+
+/* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
+unsigned long long s2w_launch_count(void);
+
+const char *s2w_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,45 @@
+// common.cuh -- shared declarations of the CUDA path (sm_100a, fp64).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <string>
+
+namespace s2w {
+
+typedef double2 cplx;  // complex128: x = re, y = im
+
+__host__ __device__ __forceinline__ cplx cmake(double r, double i) { return make_double2(r, i); }
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cplx csub(cplx a, cplx b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ cplx cmul(cplx a, cplx b)
+{
+    return make_double2(fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x));
+}
+__device__ __forceinline__ cplx cmulc(cplx a, cplx b)  // a * conj(b)
+{
+    return make_double2(fma(a.x, b.x, a.y * b.y), fma(a.y, b.x, -a.x * b.y));
+}
+__device__ __forceinline__ cplx cconj(cplx a) { return make_double2(a.x, -a.y); }
+__device__ __forceinline__ cplx cscale(cplx a, double s) { return make_double2(a.x * s, a.y * s); }
+
+void set_error(const std::string &msg);
+void count_launch();
+
+#define S2W_CUDA_CHECK(expr)                                                                       \
+    do {                                                                                           \
+        cudaError_t _e = (expr);                                                                   \
+        if (_e != cudaSuccess) {                                                                   \
+            s2w::set_error(std::string(#expr) + ": " + cudaGetErrorString(_e));                    \
+            return S2W_ECUDA;                                                                      \
+        }                                                                                          \
+    } while (0)
+
+// launch + count (every kernel of this library goes through this macro)
+#define S2W_LAUNCH(kernel, grid, block, smem, stream, ...)                                         \
+    do {                                                                                           \
+        kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);                                \
+        s2w::count_launch();                                                                       \
+    } while (0)
+
+}  // namespace s2w

@@ -1,0 +1,200 @@
+// fft_core.cuh -- block-cooperative power-of-two complex128 FFT in shared memory.
+//
+// The MW grids have 2L-1 = 2^k - 1 samples per ring (never a power of two), so every DFT on the path is done as a
+// Bluestein chirp convolution of length M = 2^q >= 2n-1.  A convolution needs FFT -> pointwise multiply -> inverse
+// FFT, which lets us drop all reordering passes: the forward transform is decimation-in-frequency (natural in,
+// digit-reversed out), the kernel spectrum is stored in that same digit-reversed order, and the inverse transform is
+// decimation-in-time (digit-reversed in, natural out).  Both run in place on one padded shared-memory buffer with
+// radix-8 register butterflies; the innermost pass is fused with the pointwise multiply.
+#pragma once
+#include "common.cuh"
+
+namespace s2w {
+
+// one 16-byte pad slot after every 8 elements: stride-8 accesses of the small-stride passes become conflict-free
+#define S2W_PAD(e) ((e) + ((e) >> 3))
+__host__ __device__ inline int fft_padded_len(int M) { return M + (M >> 3) + 1; }
+
+struct FftTab {
+    int n;              // DFT length (2L-1)
+    int L;              // band-limit of the grid
+    int logM, M;        // Bluestein length
+    int twmul;          // twiddle table stride: W_M^k = tw[k * twmul]
+    int twmask;         // table length - 1
+    const cplx *tw;     // exp(-2 pi i k / Mtab)
+    const cplx *chirp;  // [n]  exp(-i pi j^2 / n)
+    const cplx *bhat_m; // [M]  digit-reversed FFT of the wrapped exp(+i pi d^2/n), times 1/M   (forward DFT, sign -)
+    const cplx *bhat_p; // [M]  same for exp(-i pi d^2/n)                                       (inverse DFT, sign +)
+    const cplx *what;   // [M]  digit-reversed FFT of the wrapped quadrature kernel w(q), times 1/M   (reweighting)
+    const cplx *rw_in1, *rw_out1, *rw_in3, *rw_out3;  // [n] each: reweighting phase tables (ring_fft.cu)
+};
+
+template <bool INV>
+__device__ __forceinline__ cplx mul_mi(cplx a)  // times -i (forward) or +i (inverse)
+{
+    return INV ? cmake(-a.y, a.x) : cmake(a.y, -a.x);
+}
+
+template <bool INV>
+__device__ __forceinline__ void bfly4(cplx &x0, cplx &x1, cplx &x2, cplx &x3)
+{
+    cplx t0 = cadd(x0, x2), t1 = csub(x0, x2), t2 = cadd(x1, x3), t3 = mul_mi<INV>(csub(x1, x3));
+    x0 = cadd(t0, t2);
+    x1 = cadd(t1, t3);
+    x2 = csub(t0, t2);
+    x3 = csub(t1, t3);
+}
+
+template <int R, bool INV>
+struct Bfly;
+
+template <bool INV>
+struct Bfly<2, INV> {
+    static __device__ __forceinline__ void run(cplx (&v)[2])
+    {
+        cplx a = v[0];
+        v[0] = cadd(a, v[1]);
+        v[1] = csub(a, v[1]);
+    }
+};
+template <bool INV>
+struct Bfly<4, INV> {
+    static __device__ __forceinline__ void run(cplx (&v)[4]) { bfly4<INV>(v[0], v[1], v[2], v[3]); }
+};
+template <bool INV>
+struct Bfly<8, INV> {
+    static __device__ __forceinline__ void run(cplx (&v)[8])
+    {
+        const double h = 0.70710678118654752440;
+        cplx a0 = v[0], a1 = v[2], a2 = v[4], a3 = v[6];
+        cplx b0 = v[1], b1 = v[3], b2 = v[5], b3 = v[7];
+        bfly4<INV>(a0, a1, a2, a3);
+        bfly4<INV>(b0, b1, b2, b3);
+        // w^k b_k with w = exp(-+ i pi/4)
+        cplx c1, c3;
+        if (INV) {
+            c1 = cmake((b1.x - b1.y) * h, (b1.x + b1.y) * h);
+            c3 = cmake((-b3.x - b3.y) * h, (b3.x - b3.y) * h);
+        } else {
+            c1 = cmake((b1.x + b1.y) * h, (b1.y - b1.x) * h);
+            c3 = cmake((b3.y - b3.x) * h, (-b3.x - b3.y) * h);
+        }
+        cplx c2 = mul_mi<INV>(b2);
+        v[0] = cadd(a0, b0);
+        v[4] = csub(a0, b0);
+        v[1] = cadd(a1, c1);
+        v[5] = csub(a1, c1);
+        v[2] = cadd(a2, c2);
+        v[6] = csub(a2, c2);
+        v[3] = cadd(a3, c3);
+        v[7] = csub(a3, c3);
+    }
+};
+
+// One decimation-in-frequency pass on sub-transforms of size S (radix R): butterflies, then twiddles W_S^{i j}.
+template <int R>
+__device__ __forceinline__ void dif_pass(cplx *buf, int M, int logS, const FftTab &T)
+{
+    const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
+    const int s = 1 << logs;
+    const int twm = T.twmul << (T.logM - logS);  // W_S^k = W_M^{k M/S}
+    for (int idx = threadIdx.x; idx < (M / R); idx += blockDim.x) {
+        int i = idx & (s - 1);
+        int base = ((idx >> logs) << logS) + i;
+        cplx v[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[k] = buf[S2W_PAD(base + (k << logs))];
+        Bfly<R, false>::run(v);
+#pragma unroll
+        for (int j = 1; j < R; ++j) v[j] = cmul(v[j], __ldg(&T.tw[(i * j * twm) & T.twmask]));
+#pragma unroll
+        for (int k = 0; k < R; ++k) buf[S2W_PAD(base + (k << logs))] = v[k];
+    }
+}
+
+// The matching decimation-in-time inverse pass: conjugate twiddles, then inverse butterflies.
+template <int R>
+__device__ __forceinline__ void dit_pass(cplx *buf, int M, int logS, const FftTab &T)
+{
+    const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
+    const int s = 1 << logs;
+    const int twm = T.twmul << (T.logM - logS);
+    for (int idx = threadIdx.x; idx < (M / R); idx += blockDim.x) {
+        int i = idx & (s - 1);
+        int base = ((idx >> logs) << logS) + i;
+        cplx v[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[k] = buf[S2W_PAD(base + (k << logs))];
+#pragma unroll
+        for (int j = 1; j < R; ++j) v[j] = cmulc(v[j], __ldg(&T.tw[(i * j * twm) & T.twmask]));
+        Bfly<R, true>::run(v);
+#pragma unroll
+        for (int k = 0; k < R; ++k) buf[S2W_PAD(base + (k << logs))] = v[k];
+    }
+}
+
+// Innermost pass of both transforms fused with the pointwise product: groups of R consecutive elements.
+template <int R>
+__device__ __forceinline__ void mid_pass(cplx *buf, int M, const cplx *__restrict__ khat)
+{
+    for (int g = threadIdx.x; g < (M / R); g += blockDim.x) {
+        cplx v[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[k] = buf[S2W_PAD(g * R + k)];
+        Bfly<R, false>::run(v);
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[k] = cmul(v[k], __ldg(&khat[g * R + k]));
+        Bfly<R, true>::run(v);
+#pragma unroll
+        for (int k = 0; k < R; ++k) buf[S2W_PAD(g * R + k)] = v[k];
+    }
+}
+
+// Forward transform only (used once per table at plan creation): natural in, digit-reversed out.
+__device__ inline void fft_dif_full(cplx *buf, const FftTab &T)
+{
+    const int M = T.M;
+    int logS = T.logM;
+    while (logS >= 3) {
+        dif_pass<8>(buf, M, logS, T);
+        __syncthreads();
+        logS -= 3;
+    }
+    if (logS == 2) {
+        dif_pass<4>(buf, M, 2, T);
+        __syncthreads();
+    } else if (logS == 1) {
+        dif_pass<2>(buf, M, 1, T);
+        __syncthreads();
+    }
+}
+
+// buf <- circular convolution (length M) of buf with the kernel whose digit-reversed, 1/M-scaled spectrum is khat.
+// Ends with a __syncthreads().  Requires a __syncthreads() after the caller's writes to buf.
+__device__ inline void fft_convolve(cplx *buf, const FftTab &T, const cplx *__restrict__ khat)
+{
+    const int M = T.M;
+    const int r = T.logM % 3;
+    const int logMid = (r == 0) ? 3 : r;  // innermost group: 8, 2 or 4 elements
+    int logS = T.logM;
+    while (logS > logMid) {
+        dif_pass<8>(buf, M, logS, T);
+        __syncthreads();
+        logS -= 3;
+    }
+    if (logMid == 3)
+        mid_pass<8>(buf, M, khat);
+    else if (logMid == 2)
+        mid_pass<4>(buf, M, khat);
+    else
+        mid_pass<2>(buf, M, khat);
+    __syncthreads();
+    logS = logMid + 3;
+    while (logS <= T.logM) {
+        dit_pass<8>(buf, M, logS, T);
+        __syncthreads();
+        logS += 3;
+    }
+}
+
+}  // namespace s2w

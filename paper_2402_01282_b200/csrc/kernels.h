@@ -1,0 +1,78 @@
+// kernels.h -- host-callable launchers of the CUDA kernels (ring_fft.cu, wigner.cu, radial.cu).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "../../include/s2w.h"
+#include "common.cuh"
+
+namespace s2w {
+
+#define S2W_MAX_N 32                 // directionality limit: 2N-1 <= 63 gamma samples
+#define S2W_MAX_ROWS (2 * S2W_MAX_N)  // rows n handled by one launch
+
+struct FftTab;
+
+// rows (values of n) one SO(3) FFT launch works on
+struct So3Args {
+    int N;                       // directionality: 2N-1 gamma samples
+    int nn;                      // number of rows
+    int nrows;                   // rows per signal in the F array
+    int n_val[S2W_MAX_ROWS];     // n
+    int n_row[S2W_MAX_ROWS];     // row index of n in F
+    int n_rowm[S2W_MAX_ROWS];    // row index of -n in F
+};
+
+struct RwArgs {
+    int nn, nrows, Md, isReal;
+    int n_val[S2W_MAX_ROWS];
+    int n_row[S2W_MAX_ROWS];
+};
+
+// one launch of the on-the-fly Wigner contraction (steps a3, a5, a6, a7)
+struct WigArgs {
+    int Lg;        // band-limit of the theta grid (rings t = 0..Lg-1, |m| < Lg, l < Lg)
+    int Lfull;     // band-limit of the plan (l-stride of flmT, extent of the coefficient table)
+    int B;         // signals
+    int isReal;    // harmonic arrays hold m >= 0 only
+    int nn;        // number of n values
+    int nrows;     // rows per signal in F
+    int lmin;      // first l with a non-zero filter entry
+    int n_val[S2W_MAX_ROWS], n_tab[S2W_MAX_ROWS], n_row[S2W_MAX_ROWS], n_rowm[S2W_MAX_ROWS], n_filtm[S2W_MAX_ROWS];
+    size_t tri;                 // entries per n in the coefficient table: Lfull (Lfull+1)/2
+    const double *coef;         // [ntab][tri][3]: (alpha, beta, gamma) of the step l -> l+1 at packed (m, l)
+    const int *lstart;          // [ntab][Lg][Lg] (n, m, t): first l at which ring t is active
+    const double2 *dseed;       // [ntab][Lg][Lg]: (d^{lstart}, d^{lstart-1})
+    const double *xcos;         // [Lg] cos(beta_t)
+    const cplx *filt;           // [nn][Lg] filter applied to row q at degree l
+    cplx *flmT;                 // [B][Mfull][Lfull]  f_{l m} stored m-major; Mfull = Lfull (real) or 2 Lfull - 1
+    cplx *F;                    // [B][nrows][Lg][Md], Md = Lg (real) or 2 Lg - 1
+};
+
+void set_error(const std::string &msg);
+
+int launch_twiddles(cplx *tw, int Mtab, cudaStream_t st);
+int launch_fft_tables(const FftTab &T, cplx *chirp, cplx *rw_in1, cplx *rw_out1, cplx *rw_in3, cplx *rw_out3,
+                      cplx *bhat_m, cplx *bhat_p, cplx *what, cudaStream_t st);
+// pixel-side arrays: signal b starts sig_stride elements after signal b-1; rows of Lg rings each
+int launch_ring_fwd(bool real, const void *in, cplx *out, int B, int Lg, size_t sig_stride, const FftTab &T,
+                    cudaStream_t st);
+int launch_ring_inv(bool real, const cplx *in, void *out, int B, int Lg, size_t sig_stride, const FftTab &T,
+                    cudaStream_t st);
+int launch_so3_inv(bool real, const cplx *F, void *W, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
+                   cudaStream_t st);
+int launch_so3_fwd(bool real, const void *W, size_t sig_stride, cplx *F, const So3Args &A, int batch, const FftTab &T,
+                   cudaStream_t st);
+int launch_reweight(cplx *F, const RwArgs &A, int batch, const FftTab &T, cudaStream_t st);
+
+int launch_wigner_coef(double *coef, int Lfull, const int *n_vals, int ntab, cudaStream_t st);
+int launch_wigner_ramp(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg,
+                       const int *n_vals, int ntab, const double *xcos, int *lstart, double2 *dseed, cudaStream_t st);
+int launch_wigner_inverse(const WigArgs &A, cudaStream_t st);   // harmonic -> rings   (a5, a7)
+int launch_wigner_forward(const WigArgs &A, cudaStream_t st);   // rings -> harmonic   (a3, a6), accumulates
+
+int launch_flm_pack(const cplx *flm_user, cplx *flmT, int B, int L, bool real, cudaStream_t st);
+int launch_flm_unpack(const cplx *flmT, cplx *flm_user, int B, int L, bool real, cudaStream_t st);
+
+int probe_fp64(int kind, double *tflops);
+
+}  // namespace s2w

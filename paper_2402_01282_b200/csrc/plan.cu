@@ -1,0 +1,1016 @@
+// plan.cu -- plans (cached tables) and the transform drivers behind the C ABI of include/s2w.h.
+//
+// Sphere analysis (Alg. 1), with the step names of DESIGN.md:
+//   a1 ring DFT -> a2 reweight -> a3 forward SHT contraction  (f_lm, kept m-major on the device)
+//   scaling: a7-type contraction at L_s with filter Phi_l0 -> a1 inverse                   (Eq. 29/41)
+//   each j : a4+a5 filter x inverse Wigner contraction at L_j -> a8 (alpha, gamma) DFT       (Eq. 27/40)
+// Sphere synthesis (Alg. 1) runs the mirror image and accumulates into f_lm     (Eq. 42).
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <map>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "fft_core.cuh"
+#include "host_math.h"
+#include "kernels.h"
+
+namespace s2w {
+
+static thread_local std::string g_err;
+static unsigned long long g_launches = 0;
+void set_error(const std::string &msg) { g_err = msg; }
+void count_launch() { ++g_launches; }
+
+namespace {
+
+typedef long double ld;
+const ld PI_L = 3.14159265358979323846264338327950288419716939937510L;
+
+struct DevPool {  // owns device allocations of a plan
+    std::vector<void *> ptrs;
+    template <typename T>
+    int alloc(T **p, size_t count)
+    {
+        void *q = 0;
+        cudaError_t e = cudaMalloc(&q, std::max<size_t>(count, 1) * sizeof(T));
+        if (e != cudaSuccess) {
+            set_error(std::string("cudaMalloc: ") + cudaGetErrorString(e));
+            cudaGetLastError();
+            return e == cudaErrorMemoryAllocation ? S2W_ENOMEM : S2W_ECUDA;
+        }
+        ptrs.push_back(q);
+        *p = (T *)q;
+        return S2W_OK;
+    }
+    template <typename T>
+    int upload(T **p, const std::vector<T> &h)
+    {
+        int rc = alloc(p, h.size());
+        if (rc) return rc;
+        if (!h.empty()) S2W_CUDA_CHECK(cudaMemcpy(*p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+        return S2W_OK;
+    }
+    void release()
+    {
+        for (void *p : ptrs) cudaFree(p);
+        ptrs.clear();
+    }
+};
+
+struct GridTab {  // everything that depends on the theta/phi grid of band-limit Lg
+    int Lg;
+    FftTab fft;
+    double *xcos;
+    int *lstart;
+    double2 *dseed;
+};
+
+struct Stage {  // one Wigner contraction launch: rows, filters
+    int grid;   // index into plan->grids
+    int Lg;
+    int lmin;
+    int nn, nrows;
+    int n_val[S2W_MAX_ROWS], n_tab[S2W_MAX_ROWS], n_row[S2W_MAX_ROWS], n_rowm[S2W_MAX_ROWS], n_filtm[S2W_MAX_ROWS];
+    cplx *filt_ana;  // [nn][Lg]  harmonic -> rings
+    cplx *filt_syn;  // [nn][Lg]  rings -> harmonic
+};
+
+struct Scale {
+    int j, jp;
+    int Lj, Pj;
+    size_t offset;  // element offset in one signal's coefficient block
+    Stage st;
+    double *Kinv;   // ball: [Pj nodes][Pj p]   K_p(r_i) kappa^{j'}(p) on the Pj-node grid       (analysis)
+    double *Kfwd;   // ball: [Pj p][Pj nodes]   q_i K_p(r_i) kappa^{j'}(p)                       (synthesis)
+};
+
+}  // namespace
+}  // namespace s2w
+
+using namespace s2w;
+
+struct s2w_plan {
+    int kind;  // 0 sphere, 1 ball
+    int L, N, P, J0, J, J0p, Jp, multires, flags, batch, device;
+    double lambda, nu, tau;
+    bool real;
+    DevPool pool;
+    std::vector<GridTab> grids;
+    std::vector<int> tabn;  // table values of n: script-N united with {0}
+    double *coef;
+    size_t tri;
+    cplx *tw;
+    int Mtab;
+    Stage sht;       // plain spherical harmonic transform at L (filters c_l and (2 pi/n) c_l)
+    Stage scaling;   // scaling coefficients at L_s
+    int Ls;
+    size_t scaling_offset;
+    std::vector<Scale> scales;
+    size_t coeff_elems, signal_elems;
+    size_t ws_flm_elems, ws_F_elems, ws_bytes;
+    // ball
+    double *Kfull_fwd;  // [P p][P nodes]  q_i K_p(r_i)
+    double *Kfull_inv;  // [P nodes][P p]  K_p(r_i)
+    cplx *phi_ball;     // [P][L] sqrt(4pi/(2l+1)) Phi_{l0p}
+};
+
+namespace s2w {
+namespace {
+
+int find_tab(const s2w_plan *p, int n)
+{
+    for (size_t i = 0; i < p->tabn.size(); ++i)
+        if (p->tabn[i] == n) return (int)i;
+    return -1;
+}
+
+int grid_index(s2w_plan *p, int Lg)
+{
+    for (size_t i = 0; i < p->grids.size(); ++i)
+        if (p->grids[i].Lg == Lg) return (int)i;
+    return -1;
+}
+
+int ceil_log2(int v)
+{
+    int l = 0;
+    while ((1 << l) < v) ++l;
+    return l;
+}
+
+// Range-extended seeds d^{l0}_{mn}(beta_t), l0 = max(m,|n|), m >= 0, as mantissa * 2^expo (long double arithmetic):
+//   d^m_{mn} = sqrt((2m)!/((m+n)!(m-n)!)) cos^{m+n}(beta/2) (-sin(beta/2))^{m-n}   for m >= |n|,
+// built by the one-term recursion in m, and for m < |n| from d^l_{mn} = (-1)^{m-n} d^l_{nm} = d^l_{-n,-m}.
+void host_seeds(int Lg, const std::vector<int> &tabn, std::vector<double> &mant, std::vector<int> &expo,
+                std::vector<double> &xcos)
+{
+    const size_t per = (size_t)Lg * Lg;
+    mant.assign(tabn.size() * per, 0.0);
+    expo.assign(tabn.size() * per, 0);
+    xcos.assign(Lg, 0.0);
+    std::vector<ld> ch(Lg), sh(Lg);
+    for (int t = 0; t < Lg; ++t) {
+        ld beta = PI_L * (ld)(2 * t + 1) / (ld)(2 * Lg - 1);
+        xcos[t] = (double)cosl(beta);
+        ch[t] = cosl(beta / 2);
+        sh[t] = sinl(beta / 2);
+    }
+    auto put = [&](size_t idx, ld v) {
+        int e = 0;
+        ld mnt = frexpl(v, &e);
+        mant[idx] = (double)mnt;
+        expo[idx] = e;
+    };
+    // S(l0, q) at ring t by direct product (only used for l0 = |n| <= N-1)
+    auto S_direct = [&](int l0, int q, int t) -> ld {
+        int a = l0 + q, b = l0 - q;
+        ld v = 1;
+        for (int i = 1; i <= b; ++i) v *= sqrtl((ld)(a + i) / (ld)i) * (-sh[t]);
+        for (int i = 1; i <= a; ++i) v *= ch[t];
+        return v;
+    };
+    std::vector<ld> ratio(Lg + 1);
+    for (size_t tab = 0; tab < tabn.size(); ++tab) {
+        const int n = tabn[tab], an = n < 0 ? -n : n;
+        if (an >= Lg) continue;
+        for (int m = an; m + 1 < Lg; ++m)
+            ratio[m] = sqrtl((ld)(2 * m + 2) * (ld)(2 * m + 1) / ((ld)(m + 1 + n) * (ld)(m + 1 - n)));
+        for (int t = 0; t < Lg; ++t) {
+            // m < |n|
+            for (int m = 0; m < an; ++m) {
+                ld v;
+                if (n > 0)
+                    v = (((an - m) & 1) ? -1 : 1) * S_direct(an, m, t);
+                else
+                    v = S_direct(an, -m, t);
+                put((tab * Lg + m) * (size_t)Lg + t, v);
+            }
+            // m >= |n|
+            ld s = 1;
+            if (n >= 0)
+                for (int i = 0; i < 2 * an; ++i) s *= ch[t];
+            else
+                for (int i = 0; i < 2 * an; ++i) s *= sh[t];
+            const ld cs = -ch[t] * sh[t];
+            for (int m = an; m < Lg; ++m) {
+                put((tab * Lg + m) * (size_t)Lg + t, s);
+                if (m + 1 < Lg) s *= ratio[m] * cs;
+            }
+        }
+    }
+}
+
+int build_grid(s2w_plan *p, int Lg)
+{
+    if (grid_index(p, Lg) >= 0) return S2W_OK;
+    GridTab g;
+    memset(&g, 0, sizeof(g));
+    g.Lg = Lg;
+    FftTab &T = g.fft;
+    T.n = 2 * Lg - 1;
+    T.L = Lg;
+    T.logM = std::max(1, ceil_log2(2 * T.n - 1));
+    T.M = 1 << T.logM;
+    T.tw = p->tw;
+    T.twmul = p->Mtab / T.M;
+    T.twmask = p->Mtab - 1;
+    cplx *chirp, *i1, *o1, *i3, *o3, *bm, *bp, *wh;
+    int rc;
+    if ((rc = p->pool.alloc(&chirp, T.n))) return rc;
+    if ((rc = p->pool.alloc(&i1, T.n))) return rc;
+    if ((rc = p->pool.alloc(&o1, T.n))) return rc;
+    if ((rc = p->pool.alloc(&i3, T.n))) return rc;
+    if ((rc = p->pool.alloc(&o3, T.n))) return rc;
+    if ((rc = p->pool.alloc(&bm, T.M))) return rc;
+    if ((rc = p->pool.alloc(&bp, T.M))) return rc;
+    if ((rc = p->pool.alloc(&wh, T.M))) return rc;
+    T.chirp = chirp;
+    T.rw_in1 = i1;
+    T.rw_out1 = o1;
+    T.rw_in3 = i3;
+    T.rw_out3 = o3;
+    T.bhat_m = bm;
+    T.bhat_p = bp;
+    T.what = wh;
+    if ((rc = launch_fft_tables(T, chirp, i1, o1, i3, o3, bm, bp, wh, 0))) return rc;
+
+    std::vector<double> mant, xcos;
+    std::vector<int> expo;
+    host_seeds(Lg, p->tabn, mant, expo, xcos);
+    double *dmant;
+    int *dexpo;
+    if ((rc = p->pool.upload(&g.xcos, xcos))) return rc;
+    // temporaries (freed after the ramp kernel)
+    const size_t cnt = mant.size();
+    S2W_CUDA_CHECK(cudaMalloc((void **)&dmant, std::max<size_t>(cnt, 1) * sizeof(double)));
+    S2W_CUDA_CHECK(cudaMalloc((void **)&dexpo, std::max<size_t>(cnt, 1) * sizeof(int)));
+    S2W_CUDA_CHECK(cudaMemcpy(dmant, mant.data(), cnt * sizeof(double), cudaMemcpyHostToDevice));
+    S2W_CUDA_CHECK(cudaMemcpy(dexpo, expo.data(), cnt * sizeof(int), cudaMemcpyHostToDevice));
+    if ((rc = p->pool.alloc(&g.lstart, cnt))) return rc;
+    if ((rc = p->pool.alloc(&g.dseed, cnt))) return rc;
+    rc = launch_wigner_ramp(dmant, dexpo, p->coef, p->tri, p->L, Lg, p->tabn.data(), (int)p->tabn.size(), g.xcos,
+                            g.lstart, g.dseed, 0);
+    cudaError_t e = cudaDeviceSynchronize();
+    cudaFree(dmant);
+    cudaFree(dexpo);
+    if (rc) return rc;
+    if (e != cudaSuccess) {
+        set_error(std::string("plan set-up kernels: ") + cudaGetErrorString(e));
+        return S2W_ECUDA;
+    }
+    p->grids.push_back(g);
+    return S2W_OK;
+}
+
+// rows of a stage from a list of n values (all |n| < Lg), in the F layout with `nrows` rows per signal where row(n) is
+// given by row_of(n)
+int fill_stage_rows(s2w_plan *p, Stage &st, const std::vector<int> &ns, const std::vector<int> &rows, int nrows)
+{
+    st.nn = (int)ns.size();
+    st.nrows = nrows;
+    if (st.nn > S2W_MAX_ROWS) return S2W_EINVAL;
+    for (int q = 0; q < st.nn; ++q) {
+        st.n_val[q] = ns[q];
+        st.n_tab[q] = find_tab(p, ns[q]);
+        st.n_row[q] = rows[q];
+        st.n_rowm[q] = rows[q];
+        st.n_filtm[q] = q;
+        for (int q2 = 0; q2 < st.nn; ++q2)
+            if (ns[q2] == -ns[q]) {
+                st.n_rowm[q] = rows[q2];
+                st.n_filtm[q] = q2;
+            }
+        if (st.n_tab[q] < 0) return S2W_EINVAL;
+    }
+    return S2W_OK;
+}
+
+void fill_wig_args(const s2w_plan *p, const Stage &st, bool synthesis, int B, cplx *flmT, cplx *F, WigArgs &A)
+{
+    const GridTab &g = p->grids[st.grid];
+    A.Lg = st.Lg;
+    A.Lfull = p->L;
+    A.B = B;
+    A.isReal = p->real ? 1 : 0;
+    A.nn = st.nn;
+    A.nrows = st.nrows;
+    A.lmin = st.lmin;
+    for (int q = 0; q < st.nn; ++q) {
+        A.n_val[q] = st.n_val[q];
+        A.n_tab[q] = st.n_tab[q];
+        A.n_row[q] = st.n_row[q];
+        A.n_rowm[q] = st.n_rowm[q];
+        A.n_filtm[q] = st.n_filtm[q];
+    }
+    A.tri = p->tri;
+    A.coef = p->coef;
+    A.lstart = g.lstart;
+    A.dseed = g.dseed;
+    A.xcos = g.xcos;
+    A.filt = synthesis ? st.filt_syn : st.filt_ana;
+    A.flmT = flmT;
+    A.F = F;
+}
+
+void fill_so3_args(const s2w_plan *p, const Stage &st, So3Args &A)
+{
+    A.N = p->N;
+    A.nn = st.nn;
+    A.nrows = st.nrows;
+    for (int q = 0; q < st.nn; ++q) {
+        A.n_val[q] = st.n_val[q];
+        A.n_row[q] = st.n_row[q];
+        A.n_rowm[q] = st.n_rowm[q];
+    }
+}
+
+void fill_rw_args(const s2w_plan *p, const Stage &st, RwArgs &A)
+{
+    A.nn = st.nn;
+    A.nrows = st.nrows;
+    A.isReal = p->real ? 1 : 0;
+    A.Md = p->real ? st.Lg : 2 * st.Lg - 1;
+    for (int q = 0; q < st.nn; ++q) {
+        A.n_val[q] = st.n_val[q];
+        A.n_row[q] = st.n_row[q];
+    }
+}
+
+int check_params(int L, int N, double lambda, int J0)
+{
+    if (L < 1 || N < 1 || N > L || !(lambda > 1.0) || J0 < 0) {
+        set_error("invalid argument: need L >= 1, 1 <= N <= L, lambda > 1, J0 >= 0");
+        return S2W_EINVAL;
+    }
+    if (N > S2W_MAX_N) {
+        set_error("N above S2W_MAX_N");
+        return S2W_EUNSUPPORTED;
+    }
+    if (J0 > scale_count(L, lambda)) {
+        set_error("invalid argument: J0 > J");
+        return S2W_EINVAL;
+    }
+    return S2W_OK;
+}
+
+// common part of plan creation: tables that depend on (L, N) only
+int plan_common(s2w_plan *p)
+{
+    int rc;
+    p->tabn.clear();
+    for (int n = -(p->N - 1); n <= p->N - 1; n += 2) p->tabn.push_back(n);
+    if (find_tab(p, 0) < 0) p->tabn.push_back(0);
+    p->tri = (size_t)p->L * (p->L + 1) / 2;
+    if ((rc = p->pool.alloc(&p->coef, p->tabn.size() * p->tri * 3))) return rc;
+    if ((rc = launch_wigner_coef(p->coef, p->L, p->tabn.data(), (int)p->tabn.size(), 0))) return rc;
+    p->Mtab = 1 << std::max(1, ceil_log2(2 * (2 * p->L - 1) - 1));
+    if ((rc = p->pool.alloc(&p->tw, p->Mtab))) return rc;
+    if ((rc = launch_twiddles(p->tw, p->Mtab, 0))) return rc;
+    S2W_CUDA_CHECK(cudaDeviceSynchronize());
+    return S2W_OK;
+}
+
+int make_stage_filters(s2w_plan *p, Stage &st, const std::vector<cplx> &ana, const std::vector<cplx> &syn)
+{
+    int rc;
+    if ((rc = p->pool.upload(&st.filt_ana, ana))) return rc;
+    if ((rc = p->pool.upload(&st.filt_syn, syn))) return rc;
+    return S2W_OK;
+}
+
+// SHT stage at band-limit Lg with analysis-direction filter a(l) (harmonic -> rings) and synthesis filter s(l)
+int make_n0_stage(s2w_plan *p, Stage &st, int Lg, const std::vector<double> &a, const std::vector<double> &s)
+{
+    int rc;
+    if ((rc = build_grid(p, Lg))) return rc;
+    memset(&st, 0, sizeof(st));
+    st.grid = grid_index(p, Lg);
+    st.Lg = Lg;
+    st.lmin = 0;
+    std::vector<int> ns(1, 0), rows(1, 0);
+    if ((rc = fill_stage_rows(p, st, ns, rows, 1))) return rc;
+    std::vector<cplx> fa(Lg), fs(Lg);
+    for (int l = 0; l < Lg; ++l) {
+        fa[l] = cmake(a[l], 0.0);
+        fs[l] = cmake(s[l], 0.0);
+    }
+    return make_stage_filters(p, st, fa, fs);
+}
+
+}  // namespace
+
+// ---- transform drivers (sphere) ---------------------------------------------------------------------------------
+
+struct Work {
+    cplx *flmT;
+    cplx *F;
+};
+
+static Work carve(const s2w_plan *p, void *work)
+{
+    Work w;
+    w.flmT = (cplx *)work;
+    w.F = w.flmT + ((p->ws_flm_elems + 15) / 16) * 16;
+    return w;
+}
+
+// pixels [B][L][2L-1] -> flmT
+static int sht_forward_dev(const s2w_plan *p, const Stage &st, const void *f, size_t sig_stride, int B, const Work &w,
+                           bool zero_first, cudaStream_t s)
+{
+    const GridTab &g = p->grids[st.grid];
+    int rc;
+    if ((rc = launch_ring_fwd(p->real, f, w.F, B, st.Lg, sig_stride, g.fft, s))) return rc;
+    RwArgs R;
+    fill_rw_args(p, st, R);
+    if ((rc = launch_reweight(w.F, R, B, g.fft, s))) return rc;
+    if (zero_first) {
+        const size_t Mfull = p->real ? p->L : 2 * p->L - 1;
+        S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * Mfull * p->L * sizeof(cplx), s));
+    }
+    WigArgs A;
+    fill_wig_args(p, st, true, B, w.flmT, w.F, A);
+    return launch_wigner_forward(A, s);
+}
+
+// flmT -> pixels
+static int sht_inverse_dev(const s2w_plan *p, const Stage &st, void *f, size_t sig_stride, int B, const Work &w,
+                           cudaStream_t s)
+{
+    const GridTab &g = p->grids[st.grid];
+    WigArgs A;
+    fill_wig_args(p, st, false, B, w.flmT, w.F, A);
+    int rc;
+    if ((rc = launch_wigner_inverse(A, s))) return rc;
+    return launch_ring_inv(p->real, w.F, f, B, st.Lg, sig_stride, g.fft, s);
+}
+
+static int sphere_forward(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s)
+{
+    const Work w = carve(p, work);
+    const int B = p->batch;
+    const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
+    int rc;
+    if ((rc = sht_forward_dev(p, p->sht, in, p->signal_elems, B, w, true, s))) return rc;
+    // scaling coefficients
+    if ((rc = sht_inverse_dev(p, p->scaling, (char *)out + p->scaling_offset * esz, p->coeff_elems, B, w, s)))
+        return rc;
+    for (size_t i = 0; i < p->scales.size(); ++i) {
+        const Scale &sc = p->scales[i];
+        void *dst = (char *)out + sc.offset * esz;
+        if (sc.st.nn == 0) {
+            for (int b = 0; b < B; ++b)
+                S2W_CUDA_CHECK(cudaMemsetAsync((char *)dst + (size_t)b * p->coeff_elems * esz, 0,
+                                               (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1) * esz, s));
+            continue;
+        }
+        WigArgs A;
+        fill_wig_args(p, sc.st, false, B, w.flmT, w.F, A);
+        if ((rc = launch_wigner_inverse(A, s))) return rc;
+        So3Args S;
+        fill_so3_args(p, sc.st, S);
+        if ((rc = launch_so3_inv(p->real, w.F, dst, p->coeff_elems, S, B, p->grids[sc.st.grid].fft, s))) return rc;
+    }
+    S2W_CUDA_CHECK(cudaPeekAtLastError());
+    return S2W_OK;
+}
+
+static int sphere_inverse(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s)
+{
+    const Work w = carve(p, work);
+    const int B = p->batch;
+    const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
+    int rc;
+    if ((rc = sht_forward_dev(p, p->scaling, (const char *)in + p->scaling_offset * esz, p->coeff_elems, B, w, true,
+                              s)))
+        return rc;
+    for (size_t i = 0; i < p->scales.size(); ++i) {
+        const Scale &sc = p->scales[i];
+        if (sc.st.nn == 0) continue;
+        const void *src = (const char *)in + sc.offset * esz;
+        const GridTab &g = p->grids[sc.st.grid];
+        So3Args S;
+        fill_so3_args(p, sc.st, S);
+        if ((rc = launch_so3_fwd(p->real, src, p->coeff_elems, w.F, S, B, g.fft, s))) return rc;
+        RwArgs R;
+        fill_rw_args(p, sc.st, R);
+        if ((rc = launch_reweight(w.F, R, B, g.fft, s))) return rc;
+        WigArgs A;
+        fill_wig_args(p, sc.st, true, B, w.flmT, w.F, A);
+        if ((rc = launch_wigner_forward(A, s))) return rc;
+    }
+    if ((rc = sht_inverse_dev(p, p->sht, out, p->signal_elems, B, w, s))) return rc;
+    S2W_CUDA_CHECK(cudaPeekAtLastError());
+    return S2W_OK;
+}
+
+}  // namespace s2w
+
+// =================================================================================================================
+// C ABI
+// =================================================================================================================
+extern "C" {
+
+const char *s2w_last_error(void) { return g_err.c_str(); }
+unsigned long long s2w_launch_count(void) { return g_launches; }
+
+int s2w_scale_count(int L, double lambda, int *J)
+{
+    if (L < 1 || !(lambda > 1.0) || !J) {
+        set_error("invalid argument");
+        return S2W_EINVAL;
+    }
+    *J = scale_count(L, lambda);
+    return S2W_OK;
+}
+
+int s2wav_kernels(double *psi, double *phi, int L, int N, double lambda, int J0)
+{
+    int rc = check_params(L, N, lambda, J0);
+    if (rc) return rc;
+    const int J = scale_count(L, lambda);
+    std::vector<double> kappa, ksc, zeta;
+    kappa_profiles(L, lambda, J0, J, kappa, ksc);
+    zeta_tiling(L, N, zeta);
+    const double pi = pi_d();
+    const int nn = 2 * N - 1;
+    if (psi)
+        for (int j = J0; j <= J; ++j)
+            for (int l = 0; l < L; ++l) {
+                const double pre = std::sqrt((2.0 * l + 1.0) / (8.0 * pi * pi)) * kappa[(size_t)(j - J0) * L + l];
+                for (int ni = 0; ni < nn; ++ni) {
+                    const size_t o = (((size_t)(j - J0) * L + l) * nn + ni) * 2;
+                    psi[o] = pre * zeta[((size_t)l * nn + ni) * 2];
+                    psi[o + 1] = pre * zeta[((size_t)l * nn + ni) * 2 + 1];
+                }
+            }
+    if (phi)
+        for (int l = 0; l < L; ++l) phi[l] = std::sqrt((2.0 * l + 1.0) / (4.0 * pi)) * std::sqrt(ksc[l]);
+    return S2W_OK;
+}
+
+int s2ball_kernels(double *kappa_l, double *kappa_p, double *zeta, double *phi, int L, int P, int N, double lambda_l,
+                   double lambda_p, int J0)
+{
+    int rc = check_params(L, N, lambda_l, J0);
+    if (rc) return rc;
+    if (P < 1 || !(lambda_p > 1.0) || J0 > scale_count(P, lambda_p)) {
+        set_error("invalid argument: need P >= 1, lambda_p > 1, J0 <= J'");
+        return S2W_EINVAL;
+    }
+    const int J = scale_count(L, lambda_l), Jp = scale_count(P, lambda_p);
+    std::vector<double> kl, kscl, kp, kscp, z;
+    kappa_profiles(L, lambda_l, J0, J, kl, kscl);
+    kappa_profiles(P, lambda_p, J0, Jp, kp, kscp);
+    zeta_tiling(L, N, z);
+    if (kappa_l) std::copy(kl.begin(), kl.end(), kappa_l);
+    if (kappa_p) std::copy(kp.begin(), kp.end(), kappa_p);
+    if (zeta) std::copy(z.begin(), z.end(), zeta);
+    const double pi = pi_d();
+    if (phi)
+        for (int p = 0; p < P; ++p)
+            for (int l = 0; l < L; ++l) {
+                const double a = kscl[l], b = kscp[p];
+                phi[(size_t)p * L + l] = std::sqrt((2.0 * l + 1.0) / (4.0 * pi)) * std::sqrt(a + b - a * b);
+            }
+    return S2W_OK;
+}
+
+int s2ball_radial_nodes(double *r, double *q, int P, double tau)
+{
+    if (P < 1 || !(tau > 0.0) || !r || !q) {
+        set_error("invalid argument: need P >= 1, tau > 0");
+        return S2W_EINVAL;
+    }
+    std::vector<double> x, w;
+    gauss_laguerre2(P, x, w);
+    if ((int)x.size() != P) {
+        set_error("Gauss-Laguerre root search failed");
+        return S2W_EUNSUPPORTED;
+    }
+    for (int i = 0; i < P; ++i) {
+        r[i] = tau * x[i];
+        q[i] = tau * tau * tau * w[i];
+    }
+    return S2W_OK;
+}
+
+int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int multiresolution, int flags, int batch,
+                      int device)
+{
+    if (!out) {
+        set_error("null plan pointer");
+        return S2W_EINVAL;
+    }
+    *out = 0;
+    int rc = check_params(L, N, lambda, J0);
+    if (rc) return rc;
+    if (batch < 1) {
+        set_error("invalid argument: batch < 1");
+        return S2W_EINVAL;
+    }
+    if (flags & S2W_PRECOMPUTE) {
+        set_error("S2W_PRECOMPUTE is not implemented yet");
+        return S2W_EUNSUPPORTED;
+    }
+    if (L > 2048) {
+        set_error("L > 2048 is not supported");
+        return S2W_EUNSUPPORTED;
+    }
+    S2W_CUDA_CHECK(cudaSetDevice(device));
+    s2w_plan *p = new s2w_plan();
+    p->kind = 0;
+    p->L = L;
+    p->N = N;
+    p->P = 1;
+    p->lambda = lambda;
+    p->nu = 0;
+    p->tau = 1;
+    p->J0 = J0;
+    p->J = scale_count(L, lambda);
+    p->J0p = p->Jp = 0;
+    p->multires = multiresolution ? 1 : 0;
+    p->flags = flags;
+    p->batch = batch;
+    p->device = device;
+    p->real = (flags & S2W_REAL) != 0;
+    p->Kfull_fwd = p->Kfull_inv = 0;
+    p->phi_ball = 0;
+#define S2W_PLAN_TRY(expr)          \
+    do {                            \
+        rc = (expr);                \
+        if (rc) {                   \
+            s2w_plan_destroy(p);    \
+            return rc;              \
+        }                           \
+    } while (0)
+    S2W_PLAN_TRY(plan_common(p));
+
+    const double pi = pi_d();
+    std::vector<double> kappa, ksc, zeta;
+    kappa_profiles(L, lambda, J0, p->J, kappa, ksc);
+    zeta_tiling(L, N, zeta);
+    const int nn = 2 * N - 1;
+
+    // plain SHT at L: harmonic -> rings uses c_l, rings -> harmonic uses (2 pi / n) c_l   (Eqs. 2-3)
+    {
+        std::vector<double> a(L), s(L);
+        for (int l = 0; l < L; ++l) {
+            a[l] = std::sqrt((2.0 * l + 1.0) / (4.0 * pi));
+            s[l] = a[l] * 2.0 * pi / (2.0 * L - 1.0);
+        }
+        S2W_PLAN_TRY(make_n0_stage(p, p->sht, L, a, s));
+    }
+    // scaling coefficients at L_s: c_l sqrt(4pi/(2l+1)) Phi_l0 = Phi_l0   (Eq. 29)
+    p->Ls = scaling_bandlimit(L, lambda, J0, p->multires);
+    {
+        std::vector<double> a(p->Ls), s(p->Ls);
+        for (int l = 0; l < p->Ls; ++l) {
+            a[l] = std::sqrt((2.0 * l + 1.0) / (4.0 * pi)) * std::sqrt(ksc[l]);
+            s[l] = a[l] * 2.0 * pi / (2.0 * p->Ls - 1.0);
+        }
+        S2W_PLAN_TRY(make_n0_stage(p, p->scaling, p->Ls, a, s));
+    }
+    size_t off = 0;
+    p->scaling_offset = 0;
+    off += (size_t)p->Ls * (2 * p->Ls - 1);
+    size_t maxF = (size_t)L * (p->real ? L : 2 * L - 1);
+    for (int j = J0; j <= p->J; ++j) {
+        Scale sc;
+        memset(&sc, 0, sizeof(sc));
+        sc.j = j;
+        sc.jp = 0;
+        sc.Pj = 1;
+        sc.Lj = scale_bandlimit(j, L, lambda, p->multires);
+        sc.offset = off;
+        off += (size_t)nn * sc.Lj * (2 * sc.Lj - 1);
+        S2W_PLAN_TRY(build_grid(p, sc.Lj));
+        Stage &st = sc.st;
+        st.grid = grid_index(p, sc.Lj);
+        st.Lg = sc.Lj;
+        const double *kj = &kappa[(size_t)(j - J0) * L];
+        st.lmin = sc.Lj;
+        for (int l = 0; l < sc.Lj; ++l)
+            if (kj[l] != 0.0) {
+                st.lmin = l;
+                break;
+            }
+        std::vector<int> ns, rows;
+        for (int ni = 0; ni < N; ++ni) {
+            int n = -(N - 1) + 2 * ni;
+            if (std::abs(n) < sc.Lj) {
+                ns.push_back(n);
+                rows.push_back(ni);
+            }
+        }
+        S2W_PLAN_TRY(fill_stage_rows(p, st, ns, rows, N));
+        std::vector<cplx> fa((size_t)st.nn * sc.Lj), fs((size_t)st.nn * sc.Lj);
+        const double syn_norm = 4.0 * pi * pi / (2.0 * sc.Lj - 1.0);
+        for (int q = 0; q < st.nn; ++q)
+            for (int l = 0; l < sc.Lj; ++l) {
+                const double pre = std::sqrt((2.0 * l + 1.0) / (8.0 * pi * pi)) * kj[l];
+                const size_t zo = ((size_t)l * nn + (st.n_val[q] + N - 1)) * 2;
+                const double re = pre * zeta[zo], im = pre * zeta[zo + 1];
+                fa[(size_t)q * sc.Lj + l] = cmake(re, -im);                        // conj(Psi)   (Eq. 40)
+                fs[(size_t)q * sc.Lj + l] = cmake(re * syn_norm, im * syn_norm);   // Psi (2pi)^2/n_a  (Eq. 42)
+            }
+        S2W_PLAN_TRY(make_stage_filters(p, st, fa, fs));
+        maxF = std::max(maxF, (size_t)N * sc.Lj * (p->real ? sc.Lj : 2 * sc.Lj - 1));
+        p->scales.push_back(sc);
+    }
+    p->coeff_elems = off;
+    p->signal_elems = (size_t)L * (2 * L - 1);
+    p->ws_flm_elems = (size_t)batch * (p->real ? L : 2 * L - 1) * L;
+    p->ws_F_elems = (size_t)batch * maxF;
+    p->ws_bytes = (((p->ws_flm_elems + 15) / 16) * 16 + p->ws_F_elems) * sizeof(cplx) + 256;
+    S2W_PLAN_TRY(cudaDeviceSynchronize() == cudaSuccess ? S2W_OK : S2W_ECUDA);
+    *out = p;
+    return S2W_OK;
+}
+
+int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, double lambda_p, int J0, double tau,
+                       int flags, int device)
+{
+    (void)out; (void)L; (void)P; (void)N; (void)lambda_l; (void)lambda_p; (void)J0; (void)tau; (void)flags; (void)device;
+    set_error("ball plans are not implemented yet");
+    return S2W_EUNSUPPORTED;
+}
+
+int s2w_plan_destroy(s2w_plan *p)
+{
+    if (!p) return S2W_OK;
+    p->pool.release();
+    delete p;
+    return S2W_OK;
+}
+
+int s2w_plan_scales(const s2w_plan *p, int *J0, int *J, int *J0p, int *Jp)
+{
+    if (!p) return S2W_EINVAL;
+    if (J0) *J0 = p->J0;
+    if (J) *J = p->J;
+    if (J0p) *J0p = p->J0p;
+    if (Jp) *Jp = p->Jp;
+    return S2W_OK;
+}
+
+int s2w_plan_scale_shape(const s2w_plan *p, int j, int jp, int *n_r, int *n_gamma, int *n_theta, int *n_phi,
+                         size_t *offset_elems)
+{
+    if (!p) return S2W_EINVAL;
+    int nr = 1, ngam = 1, nt = 0, np = 0;
+    size_t off = 0;
+    if (j < 0) {
+        nr = p->kind == 1 ? p->P : 1;
+        nt = p->Ls;
+        np = 2 * p->Ls - 1;
+        off = p->scaling_offset;
+    } else {
+        const Scale *sc = 0;
+        for (size_t i = 0; i < p->scales.size(); ++i)
+            if (p->scales[i].j == j && p->scales[i].jp == jp) sc = &p->scales[i];
+        if (!sc) {
+            set_error("no such scale");
+            return S2W_EINVAL;
+        }
+        nr = sc->Pj;
+        ngam = 2 * p->N - 1;
+        nt = sc->Lj;
+        np = 2 * sc->Lj - 1;
+        off = sc->offset;
+    }
+    if (n_r) *n_r = nr;
+    if (n_gamma) *n_gamma = ngam;
+    if (n_theta) *n_theta = nt;
+    if (n_phi) *n_phi = np;
+    if (offset_elems) *offset_elems = off;
+    return S2W_OK;
+}
+
+size_t s2w_plan_coeff_elems(const s2w_plan *p) { return p ? p->coeff_elems : 0; }
+size_t s2w_plan_signal_elems(const s2w_plan *p) { return p ? p->signal_elems : 0; }
+size_t s2w_plan_workspace_bytes(const s2w_plan *p) { return p ? p->ws_bytes : 0; }
+
+static void *align256(void *p) { return (void *)(((uintptr_t)p + 255) & ~(uintptr_t)255); }
+
+int s2w_plan_forward(const s2w_plan *p, const void *in, void *out, void *work, void *stream)
+{
+    if (!p || !in || !out || !work) {
+        set_error("null pointer");
+        return S2W_EINVAL;
+    }
+    if (p->kind != 0) return S2W_EUNSUPPORTED;
+    return sphere_forward(p, in, out, align256(work), (cudaStream_t)stream);
+}
+
+int s2w_plan_inverse(const s2w_plan *p, const void *in, void *out, void *work, void *stream)
+{
+    if (!p || !in || !out || !work) {
+        set_error("null pointer");
+        return S2W_EINVAL;
+    }
+    if (p->kind != 0) return S2W_EUNSUPPORTED;
+    return sphere_inverse(p, in, out, align256(work), (cudaStream_t)stream);
+}
+
+int s2w_plan_harmonic_forward(const s2w_plan *p, const void *f, void *flm, void *work, void *stream)
+{
+    if (!p || !f || !flm || !work) {
+        set_error("null pointer");
+        return S2W_EINVAL;
+    }
+    if (p->kind != 0) return S2W_EUNSUPPORTED;
+    const Work w = carve(p, align256(work));
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = sht_forward_dev(p, p->sht, f, p->signal_elems, p->batch, w, true, s);
+    if (rc) return rc;
+    rc = launch_flm_unpack(w.flmT, (cplx *)flm, p->batch, p->L, p->real, s);
+    if (rc) return rc;
+    S2W_CUDA_CHECK(cudaPeekAtLastError());
+    return S2W_OK;
+}
+
+int s2w_plan_harmonic_inverse(const s2w_plan *p, const void *flm, void *f, void *work, void *stream)
+{
+    if (!p || !f || !flm || !work) {
+        set_error("null pointer");
+        return S2W_EINVAL;
+    }
+    if (p->kind != 0) return S2W_EUNSUPPORTED;
+    const Work w = carve(p, align256(work));
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = launch_flm_pack((const cplx *)flm, w.flmT, p->batch, p->L, p->real, s);
+    if (rc) return rc;
+    rc = sht_inverse_dev(p, p->sht, f, p->signal_elems, p->batch, w, s);
+    if (rc) return rc;
+    S2W_CUDA_CHECK(cudaPeekAtLastError());
+    return S2W_OK;
+}
+
+// ---- plan cache behind the argument-style entry points ----
+namespace {
+struct CacheKey {
+    int kind, L, P, N, J0, multires, flags, batch, device;
+    double lam, nu, tau;
+    bool operator<(const CacheKey &o) const
+    {
+        return std::memcmp(this, &o, sizeof(CacheKey)) < 0;
+    }
+};
+struct CacheEntry {
+    s2w_plan *plan;
+    void *work;
+};
+std::map<CacheKey, CacheEntry> g_cache;
+std::mutex g_cache_mu;
+
+int cached_sphere(int L, int N, double lambda, int J0, int multires, int flags, int batch, CacheEntry *e)
+{
+    int device = 0;
+    S2W_CUDA_CHECK(cudaGetDevice(&device));
+    CacheKey k;
+    std::memset(&k, 0, sizeof(k));
+    k.kind = 0;
+    k.L = L;
+    k.N = N;
+    k.J0 = J0;
+    k.multires = multires ? 1 : 0;
+    k.flags = flags;
+    k.batch = batch;
+    k.device = device;
+    k.lam = lambda;
+    std::lock_guard<std::mutex> lock(g_cache_mu);
+    auto it = g_cache.find(k);
+    if (it == g_cache.end()) {
+        CacheEntry ne;
+        ne.plan = 0;
+        ne.work = 0;
+        int rc = s2wav_plan_create(&ne.plan, L, N, lambda, J0, multires, flags, batch, device);
+        if (rc) return rc;
+        cudaError_t ce = cudaMalloc(&ne.work, s2w_plan_workspace_bytes(ne.plan));
+        if (ce != cudaSuccess) {
+            s2w_plan_destroy(ne.plan);
+            set_error(std::string("cudaMalloc(workspace): ") + cudaGetErrorString(ce));
+            cudaGetLastError();
+            return S2W_ENOMEM;
+        }
+        it = g_cache.insert(std::make_pair(k, ne)).first;
+    }
+    *e = it->second;
+    return S2W_OK;
+}
+}  // namespace
+
+int s2wav_forward(const void *f, void *w, int L, int N, double lambda, int J0, int multires, int flags, int batch,
+                  void *stream)
+{
+    CacheEntry e;
+    int rc = cached_sphere(L, N, lambda, J0, multires, flags, batch, &e);
+    if (rc) return rc;
+    return s2w_plan_forward(e.plan, f, w, e.work, stream);
+}
+
+int s2wav_inverse(const void *w, void *f, int L, int N, double lambda, int J0, int multires, int flags, int batch,
+                  void *stream)
+{
+    CacheEntry e;
+    int rc = cached_sphere(L, N, lambda, J0, multires, flags, batch, &e);
+    if (rc) return rc;
+    return s2w_plan_inverse(e.plan, w, f, e.work, stream);
+}
+
+static int host_roundtrip(bool fwd, const void *in_h, void *out_h, int L, int N, double lambda, int J0, int multires,
+                          int flags, int batch)
+{
+    if (!in_h || !out_h) {
+        set_error("null pointer");
+        return S2W_EINVAL;
+    }
+    CacheEntry e;
+    int rc = cached_sphere(L, N, lambda, J0, multires, flags, batch, &e);
+    if (rc) return rc;
+    const size_t esz = (flags & S2W_REAL) ? sizeof(double) : sizeof(cplx);
+    const size_t sig = e.plan->signal_elems * batch * esz, cof = e.plan->coeff_elems * batch * esz;
+    void *d_in = 0, *d_out = 0;
+    S2W_CUDA_CHECK(cudaMalloc(&d_in, fwd ? sig : cof));
+    cudaError_t ce = cudaMalloc(&d_out, fwd ? cof : sig);
+    if (ce != cudaSuccess) {
+        cudaFree(d_in);
+        set_error("cudaMalloc failed");
+        return S2W_ENOMEM;
+    }
+    rc = S2W_OK;
+    if (cudaMemcpyAsync(d_in, in_h, fwd ? sig : cof, cudaMemcpyHostToDevice, 0) != cudaSuccess) rc = S2W_ECUDA;
+    if (!rc) rc = fwd ? s2w_plan_forward(e.plan, d_in, d_out, e.work, 0) : s2w_plan_inverse(e.plan, d_in, d_out, e.work, 0);
+    if (!rc && cudaMemcpyAsync(out_h, d_out, fwd ? cof : sig, cudaMemcpyDeviceToHost, 0) != cudaSuccess) rc = S2W_ECUDA;
+    if (cudaStreamSynchronize(0) != cudaSuccess && !rc) {
+        set_error(std::string("stream sync: ") + cudaGetErrorString(cudaGetLastError()));
+        rc = S2W_ECUDA;
+    }
+    cudaFree(d_in);
+    cudaFree(d_out);
+    return rc;
+}
+
+int s2wav_forward_host(const void *f, void *w, int L, int N, double lambda, int J0, int multires, int flags, int batch)
+{
+    return host_roundtrip(true, f, w, L, N, lambda, J0, multires, flags, batch);
+}
+int s2wav_inverse_host(const void *w, void *f, int L, int N, double lambda, int J0, int multires, int flags, int batch)
+{
+    return host_roundtrip(false, w, f, L, N, lambda, J0, multires, flags, batch);
+}
+
+int s2ball_forward(const void *f, void *w, int L, int P, int N, double lambda_l, double lambda_p, int J0, double tau,
+                   int flags, void *stream)
+{
+    (void)f; (void)w; (void)L; (void)P; (void)N; (void)lambda_l; (void)lambda_p; (void)J0; (void)tau; (void)flags; (void)stream;
+    set_error("ball transforms are not implemented yet");
+    return S2W_EUNSUPPORTED;
+}
+int s2ball_inverse(const void *w, void *f, int L, int P, int N, double lambda_l, double lambda_p, int J0, double tau,
+                   int flags, void *stream)
+{
+    (void)f; (void)w; (void)L; (void)P; (void)N; (void)lambda_l; (void)lambda_p; (void)J0; (void)tau; (void)flags; (void)stream;
+    set_error("ball transforms are not implemented yet");
+    return S2W_EUNSUPPORTED;
+}
+
+int s2ball_forward_host(const void *f, void *w, int L, int P, int N, double lambda_l, double lambda_p, int J0,
+                        double tau, int flags)
+{
+    (void)f; (void)w; (void)L; (void)P; (void)N; (void)lambda_l; (void)lambda_p; (void)J0; (void)tau; (void)flags;
+    set_error("ball transforms are not implemented yet");
+    return S2W_EUNSUPPORTED;
+}
+int s2ball_inverse_host(const void *w, void *f, int L, int P, int N, double lambda_l, double lambda_p, int J0,
+                        double tau, int flags)
+{
+    (void)f; (void)w; (void)L; (void)P; (void)N; (void)lambda_l; (void)lambda_p; (void)J0; (void)tau; (void)flags;
+    set_error("ball transforms are not implemented yet");
+    return S2W_EUNSUPPORTED;
+}
+
+int s2w_cache_clear(void)
+{
+    std::lock_guard<std::mutex> lock(g_cache_mu);
+    for (auto &kv : g_cache) {
+        cudaFree(kv.second.work);
+        s2w_plan_destroy(kv.second.plan);
+    }
+    g_cache.clear();
+    return S2W_OK;
+}
+
+int s2w_probe_fp64(int kind, int device, double *tflops)
+{
+    if (!tflops || kind < 0 || kind > 1) return S2W_EINVAL;
+    S2W_CUDA_CHECK(cudaSetDevice(device));
+    return probe_fp64(kind, tflops);
+}
+
+}  // extern "C"

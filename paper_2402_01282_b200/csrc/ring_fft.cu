@@ -1,0 +1,494 @@
+// ring_fft.cu -- batched odd-length fp64 DFTs along phi / alpha (steps a1 and a8 of DESIGN.md) and the MW
+// theta-quadrature reweighting (step a2), all as Bluestein chirp convolutions on fft_core.cuh.
+//
+//   a1  F_m(theta_t) = (1/n) sum_p f(theta_t, phi_p) e^{-i m phi_p},  n = 2L-1                      (Eq. 2)
+//   a8  W(gamma_g, beta_t, alpha_a) = sum_{m,n} F_mn(beta_t) e^{i(m alpha_a + n gamma_g)}            (Eq. 5/47)
+//       F_mn(beta_t) = 1/(n_a n_g) sum_{a,g} W e^{-i(m alpha_a + n gamma_g)}                         (Eq. 48)
+//   a2  h = fold(DFT^-1(w * DFT(extend(F))))  per (m,n) column along theta                          (R3)
+//
+// Real signals: W real  <=>  F_{-m,-n} = conj(F_mn).  The harmonic-side arrays then hold m = 0..L-1 only, two real
+// rings share one complex DFT in a1, and a8 transforms only the rows n >= 0.
+#include "fft_core.cuh"
+#include "kernels.h"
+
+namespace s2w {
+
+namespace {
+
+__device__ __forceinline__ cplx cis_2pi_frac(int num, int den)  // exp(2 pi i num/den), num reduced mod den
+{
+    int r = num % den;
+    if (r < 0) r += den;
+    double s, c;
+    sincospi(2.0 * (double)r / (double)den, &s, &c);
+    return cmake(c, s);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a1 forward: pixels -> F_m.  Real: one block per pair of rows, out[row][m], m = 0..L-1.
+//                              Complex: one block per row, out[row][m+L-1].
+// ---------------------------------------------------------------------------------------------------------------
+template <bool REAL>
+__global__ void __launch_bounds__(256) ring_fwd_kernel(const void *__restrict__ in, cplx *__restrict__ out, int nrows,
+                                                      size_t sig_stride, FftTab T)
+{
+    extern __shared__ cplx buf[];
+    const int n = T.n, L = T.L, M = T.M;
+    const double inv_n = 1.0 / (double)n;
+    if (REAL) {
+        const int r0 = 2 * blockIdx.x, r1 = r0 + 1;
+        const bool has1 = r1 < nrows;
+        const double *x0 = (const double *)in + (size_t)(r0 / L) * sig_stride + (size_t)(r0 % L) * n;
+        const double *x1 = (const double *)in + (size_t)(r1 / L) * sig_stride + (size_t)(r1 % L) * n;
+        for (int p = threadIdx.x; p < M; p += blockDim.x) {
+            cplx v = cmake(0.0, 0.0);
+            if (p < n) v = cmul(cmake(x0[p], has1 ? x1[p] : 0.0), __ldg(&T.chirp[p]));
+            buf[S2W_PAD(p)] = v;
+        }
+        __syncthreads();
+        fft_convolve(buf, T, T.bhat_m);
+        for (int k = threadIdx.x; k < n; k += blockDim.x) buf[S2W_PAD(k)] = cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k]));
+        __syncthreads();
+        for (int m = threadIdx.x; m < L; m += blockDim.x) {
+            cplx a = buf[S2W_PAD(m)], b = cconj(buf[S2W_PAD(m == 0 ? 0 : n - m)]);
+            cplx s = cadd(a, b), d = csub(a, b);
+            out[(size_t)r0 * L + m] = cscale(s, 0.5 * inv_n);
+            if (has1) out[(size_t)r1 * L + m] = cmake(0.5 * inv_n * d.y, -0.5 * inv_n * d.x);
+        }
+    } else {
+        const int r0 = blockIdx.x;
+        const cplx *x0 = (const cplx *)in + (size_t)(r0 / L) * sig_stride + (size_t)(r0 % L) * n;
+        for (int p = threadIdx.x; p < M; p += blockDim.x) {
+            cplx v = cmake(0.0, 0.0);
+            if (p < n) v = cmul(x0[p], __ldg(&T.chirp[p]));
+            buf[S2W_PAD(p)] = v;
+        }
+        __syncthreads();
+        fft_convolve(buf, T, T.bhat_m);
+        for (int mi = threadIdx.x; mi < n; mi += blockDim.x) {
+            int m = mi - (L - 1);
+            int k = m < 0 ? m + n : m;
+            out[(size_t)r0 * n + mi] = cscale(cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k])), inv_n);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a1 inverse: F_m -> pixels, f = sum_m F_m e^{i m phi_p}.
+// ---------------------------------------------------------------------------------------------------------------
+template <bool REAL>
+__global__ void __launch_bounds__(256) ring_inv_kernel(const cplx *__restrict__ in, void *__restrict__ out, int nrows,
+                                                      size_t sig_stride, FftTab T)
+{
+    extern __shared__ cplx buf[];
+    const int n = T.n, L = T.L, M = T.M;
+    if (REAL) {
+        const int r0 = 2 * blockIdx.x, r1 = r0 + 1;
+        const bool has1 = r1 < nrows;
+        const cplx *X0 = in + (size_t)r0 * L;
+        const cplx *X1 = in + (size_t)r1 * L;
+        for (int k = threadIdx.x; k < M; k += blockDim.x) {
+            cplx v = cmake(0.0, 0.0);
+            if (k < n) {
+                int m = k < L ? k : n - k;  // |m|
+                cplx a = X0[m], b = has1 ? X1[m] : cmake(0.0, 0.0);
+                if (k >= L) {
+                    a = cconj(a);
+                    b = cconj(b);
+                }
+                // Z_k = A_k + i B_k
+                v = cmulc(cmake(a.x - b.y, a.y + b.x), __ldg(&T.chirp[k]));
+            }
+            buf[S2W_PAD(k)] = v;
+        }
+        __syncthreads();
+        fft_convolve(buf, T, T.bhat_p);
+        double *y0 = (double *)out + (size_t)(r0 / L) * sig_stride + (size_t)(r0 % L) * n;
+        double *y1 = (double *)out + (size_t)(r1 / L) * sig_stride + (size_t)(r1 % L) * n;
+        for (int p = threadIdx.x; p < n; p += blockDim.x) {
+            cplx z = cmulc(buf[S2W_PAD(p)], __ldg(&T.chirp[p]));
+            y0[p] = z.x;
+            if (has1) y1[p] = z.y;
+        }
+    } else {
+        const int r0 = blockIdx.x;
+        const cplx *X0 = in + (size_t)r0 * n;
+        for (int k = threadIdx.x; k < M; k += blockDim.x) {
+            cplx v = cmake(0.0, 0.0);
+            if (k < n) {
+                int m = k < L ? k : k - n;
+                v = cmulc(X0[m + L - 1], __ldg(&T.chirp[k]));
+            }
+            buf[S2W_PAD(k)] = v;
+        }
+        __syncthreads();
+        fft_convolve(buf, T, T.bhat_p);
+        cplx *y0 = (cplx *)out + (size_t)(r0 / L) * sig_stride + (size_t)(r0 % L) * n;
+        for (int p = threadIdx.x; p < n; p += blockDim.x) y0[p] = cmulc(buf[S2W_PAD(p)], __ldg(&T.chirp[p]));
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a8 analysis: F[b][row][t][mi] -> W[b][g][t][a].  One block per (b, t); loops over the rows n of the scale.
+// Real: rows n >= 0 only: V_n(a) = sum_m F_mn e^{i m alpha_a} with F_{-m,n} = conj(F_{m,-n});
+//       W = sum_{n>=0} c_n Re(e^{i n gamma_g} V_n), c_0 = 1, c_n = 2.
+// ---------------------------------------------------------------------------------------------------------------
+template <bool REAL>
+__global__ void __launch_bounds__(256) so3_inv_kernel(const cplx *__restrict__ F, void *__restrict__ W, size_t sig_stride,
+                                                     So3Args A, FftTab T)
+{
+    extern __shared__ cplx buf[];
+    const int n = T.n, L = T.L, M = T.M;
+    const int t = blockIdx.x, b = blockIdx.y;
+    const int Md = REAL ? L : n;
+    const int ng = 2 * A.N - 1;
+    const cplx *Fb = F + (size_t)b * A.nrows * L * Md;
+    __shared__ cplx gph[2 * S2W_MAX_N];
+    bool first = true;
+    for (int q = 0; q < A.nn; ++q) {
+        const int nv = A.n_val[q];
+        if (REAL && nv < 0) continue;
+        if (threadIdx.x < ng) gph[threadIdx.x] = cis_2pi_frac(nv * (int)threadIdx.x, ng);
+        const cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * Md;   // row of n
+        const cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * Md;  // row of -n
+        for (int k = threadIdx.x; k < M; k += blockDim.x) {
+            cplx v = cmake(0.0, 0.0);
+            if (k < n) {
+                if (REAL) {
+                    v = k < L ? Fp[k] : cconj(Fm[n - k]);
+                } else {
+                    int m = k < L ? k : k - n;
+                    v = Fp[m + L - 1];
+                }
+                v = cmulc(v, __ldg(&T.chirp[k]));
+            }
+            buf[S2W_PAD(k)] = v;
+        }
+        __syncthreads();
+        fft_convolve(buf, T, T.bhat_p);
+        for (int g = 0; g < ng; ++g) {
+            cplx ph = gph[g];
+            if (REAL) {
+                double *Wr = (double *)W + (size_t)b * sig_stride + ((size_t)g * L + t) * n;
+                const double cn = nv == 0 ? 1.0 : 2.0;
+                for (int a = threadIdx.x; a < n; a += blockDim.x) {
+                    cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
+                    double val = cn * (ph.x * v.x - ph.y * v.y);
+                    Wr[a] = first ? val : Wr[a] + val;
+                }
+            } else {
+                cplx *Wc = (cplx *)W + (size_t)b * sig_stride + ((size_t)g * L + t) * n;
+                for (int a = threadIdx.x; a < n; a += blockDim.x) {
+                    cplx v = cmul(ph, cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a])));
+                    Wc[a] = first ? v : cadd(Wc[a], v);
+                }
+            }
+        }
+        first = false;
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a8 synthesis: W[b][g][t][a] -> F[b][row][t][mi], F_mn = 1/(n_a n_g) sum_{a,g} W e^{-i(m alpha_a + n gamma_g)}.
+// The gamma sum is done first in pixel space, V_n(a) = (1/n_g) sum_g e^{-i n gamma_g} W(g,t,a), then one DFT per row.
+// Real: rows n >= 0; the row of -n follows from F_{m,-n} = conj(F_{-m,n}).
+// ---------------------------------------------------------------------------------------------------------------
+template <bool REAL>
+__global__ void __launch_bounds__(256) so3_fwd_kernel(const void *__restrict__ W, cplx *__restrict__ F, size_t sig_stride,
+                                                     So3Args A, FftTab T)
+{
+    extern __shared__ cplx buf[];
+    const int n = T.n, L = T.L, M = T.M;
+    const int t = blockIdx.x, b = blockIdx.y;
+    const int Md = REAL ? L : n;
+    const int ng = 2 * A.N - 1;
+    const double inv_ng = 1.0 / (double)ng, inv_n = 1.0 / (double)n;
+    cplx *Fb = F + (size_t)b * A.nrows * L * Md;
+    __shared__ cplx gph[2 * S2W_MAX_N];
+    for (int q = 0; q < A.nn; ++q) {
+        const int nv = A.n_val[q];
+        if (REAL && nv < 0) continue;
+        if (threadIdx.x < ng) gph[threadIdx.x] = cis_2pi_frac(-nv * (int)threadIdx.x, ng);
+        __syncthreads();
+        for (int a = threadIdx.x; a < M; a += blockDim.x) {
+            cplx v = cmake(0.0, 0.0);
+            if (a < n) {
+                for (int g = 0; g < ng; ++g) {
+                    cplx ph = gph[g];
+                    if (REAL) {
+                        double w = ((const double *)W)[(size_t)b * sig_stride + ((size_t)g * L + t) * n + a];
+                        v.x = fma(ph.x, w, v.x);
+                        v.y = fma(ph.y, w, v.y);
+                    } else {
+                        cplx w = ((const cplx *)W)[(size_t)b * sig_stride + ((size_t)g * L + t) * n + a];
+                        v = cadd(v, cmul(ph, w));
+                    }
+                }
+                v = cmul(cscale(v, inv_ng), __ldg(&T.chirp[a]));
+            }
+            buf[S2W_PAD(a)] = v;
+        }
+        __syncthreads();
+        fft_convolve(buf, T, T.bhat_m);
+        cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * Md;
+        cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * Md;
+        if (REAL) {
+            for (int m = threadIdx.x; m < L; m += blockDim.x) {
+                Fp[m] = cscale(cmul(buf[S2W_PAD(m)], __ldg(&T.chirp[m])), inv_n);
+                if (nv != 0) {
+                    int k = m == 0 ? 0 : n - m;
+                    Fm[m] = cscale(cconj(cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k]))), inv_n);
+                }
+            }
+        } else {
+            for (int mi = threadIdx.x; mi < n; mi += blockDim.x) {
+                int m = mi - (L - 1);
+                int k = m < 0 ? m + n : m;
+                Fp[mi] = cscale(cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k])), inv_n);
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a2 reweighting of one theta-column F[.][t][mi] (stride Md) of parity sigma = (-1)^{m+n}, in place (R3):
+//   (ii)  extend to n = 2L-1 rings by F(theta_{n-1-t}) = sigma F(theta_t)
+//   (iii) Fh(k) = 1/n sum_t F(theta_t) e^{-i k theta_t},  theta_t = pi(2t+1)/n,  |k| <= L-1
+//   (iv)  G(k') = sum_k Fh(k) w(k + k')
+//   (v)   g(theta_t) = sum_k' G(k') e^{-i k' theta_t}
+//   (vi)  h(theta_t) = g(theta_t) + sigma g(theta_{n-1-t}),  t < L-1;   h(theta_{L-1}) = g(theta_{L-1})
+// Three chained chirp convolutions with no reordering in between: (iii) is evaluated at k = L-1-i, i = 0..n-1, as a
+// sign(+) DFT of the modulated column, which makes (iv) a plain convolution xr * w landing at slot i' = k' + L-1, and
+// (v) a sign(-) DFT over i' with an output modulation; the four phase tables rw_* absorb chirps and modulations.
+// One block per column.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) reweight_kernel(cplx *__restrict__ F, RwArgs A, FftTab T)
+{
+    extern __shared__ cplx buf[];
+    const int n = T.n, L = T.L, M = T.M;
+    const int mi = blockIdx.x, q = blockIdx.y, b = blockIdx.z;
+    const int m = A.isReal ? mi : mi - (L - 1);
+    const int nv = A.n_val[q];
+    const double sigma = ((m + nv) & 1) ? -1.0 : 1.0;
+    cplx *col = F + ((size_t)b * A.nrows + A.n_row[q]) * (size_t)L * A.Md + mi;
+    for (int t = threadIdx.x; t < M; t += blockDim.x) {
+        cplx v = cmake(0.0, 0.0);
+        if (t < n) {
+            v = t < L ? col[(size_t)t * A.Md] : cscale(col[(size_t)(n - 1 - t) * A.Md], sigma);
+            v = cmul(v, __ldg(&T.rw_in1[t]));
+        }
+        buf[S2W_PAD(t)] = v;
+    }
+    __syncthreads();
+    fft_convolve(buf, T, T.bhat_p);
+    for (int i = threadIdx.x; i < M; i += blockDim.x)
+        buf[S2W_PAD(i)] = i < n ? cmul(buf[S2W_PAD(i)], __ldg(&T.rw_out1[i])) : cmake(0.0, 0.0);
+    __syncthreads();
+    fft_convolve(buf, T, T.what);
+    for (int i = threadIdx.x; i < M; i += blockDim.x)
+        buf[S2W_PAD(i)] = i < n ? cmul(buf[S2W_PAD(i)], __ldg(&T.rw_in3[i])) : cmake(0.0, 0.0);
+    __syncthreads();
+    fft_convolve(buf, T, T.bhat_m);
+    for (int t = threadIdx.x; t < L; t += blockDim.x) {
+        cplx g0 = cmul(buf[S2W_PAD(t)], __ldg(&T.rw_out3[t]));
+        if (t < L - 1) {
+            int tb = n - 1 - t;
+            cplx g1 = cmul(buf[S2W_PAD(tb)], __ldg(&T.rw_out3[tb]));
+            g0 = cmake(fma(sigma, g1.x, g0.x), fma(sigma, g1.y, g0.y));
+        }
+        col[(size_t)t * A.Md] = g0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// plan-time table kernels
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void twiddle_kernel(cplx *tw, int Mtab)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < Mtab) {
+        double s, c;
+        sincospi(-2.0 * (double)k / (double)Mtab, &s, &c);
+        tw[k] = cmake(c, s);
+    }
+}
+
+// exp(i pi num/n) with the integer num reduced mod 2n exactly
+__device__ __forceinline__ cplx cis_pi_frac(long long num, int n)
+{
+    long long r = num % (2LL * n);
+    if (r < 0) r += 2LL * n;
+    double s, c;
+    sincospi((double)r / (double)n, &s, &c);
+    return cmake(c, s);
+}
+
+// chirp[j] = exp(-i pi j^2/n); reweighting phase tables (see reweight_kernel):
+//   rw_in1[t]  = exp(i pi [t^2 - (L-1)(2t+1)]/n)       rw_out1[i] = exp(i pi (i + i^2)/n) / n
+//   rw_in3[i]  = exp(-i pi (i + i^2)/n)                rw_out3[t] = exp(i pi [(L-1)(2t+1) - t^2]/n)
+__global__ void chirp_kernel(cplx *chirp, cplx *rw_in1, cplx *rw_out1, cplx *rw_in3, cplx *rw_out3, int n, int L)
+{
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    long long jj = (long long)j * j, mod = (long long)(L - 1) * (2 * j + 1);
+    chirp[j] = cis_pi_frac(-jj, n);
+    rw_in1[j] = cis_pi_frac(jj - mod, n);
+    rw_out1[j] = cscale(cis_pi_frac(j + jj, n), 1.0 / (double)n);
+    rw_in3[j] = cis_pi_frac(-(j + jj), n);
+    rw_out3[j] = cis_pi_frac(mod - jj, n);
+}
+
+// kind 0: b[d mod M] = exp(+i pi d^2/n)/M, |d| < n   (forward DFT);  kind 1: conjugate (inverse DFT);
+// kind 2: w(q)/M, |q| < n:  2/(1-q^2) for even q, +-i pi/2 for q = +-1, 0 otherwise   (R3 (iv)).
+// One block; transforms in place (digit-reversed output) and writes khat[M].
+__global__ void __launch_bounds__(256) kernel_spectrum_kernel(cplx *khat, int kind, FftTab T)
+{
+    extern __shared__ cplx buf[];
+    const int n = T.n, M = T.M;
+    const double invM = 1.0 / (double)M;
+    for (int e = threadIdx.x; e < M; e += blockDim.x) buf[S2W_PAD(e)] = cmake(0.0, 0.0);
+    __syncthreads();
+    for (int e = threadIdx.x; e < 2 * n - 1; e += blockDim.x) {
+        int d = e - (n - 1);
+        cplx v;
+        if (kind == 2) {
+            if ((d & 1) == 0)
+                v = cmake(2.0 / (1.0 - (double)d * (double)d), 0.0);
+            else if (d == 1)
+                v = cmake(0.0, 1.5707963267948966192);
+            else if (d == -1)
+                v = cmake(0.0, -1.5707963267948966192);
+            else
+                v = cmake(0.0, 0.0);
+        } else {
+            long long r = ((long long)d * d) % (2LL * n);
+            double s, c;
+            sincospi((double)r / (double)n, &s, &c);
+            v = cmake(c, kind == 0 ? s : -s);
+        }
+        int slot = d < 0 ? d + M : d;
+        buf[S2W_PAD(slot)] = cscale(v, invM);
+    }
+    __syncthreads();
+    fft_dif_full(buf, T);
+    for (int e = threadIdx.x; e < M; e += blockDim.x) khat[e] = buf[S2W_PAD(e)];
+}
+
+size_t fft_smem_bytes(const FftTab &T) { return (size_t)fft_padded_len(T.M) * sizeof(cplx); }
+
+template <typename K>
+int set_smem(K kernel, size_t bytes)
+{
+    if (bytes > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        if (e != cudaSuccess) {
+            set_error(std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
+            return S2W_ECUDA;
+        }
+    }
+    return S2W_OK;
+}
+
+}  // namespace
+
+// ---- host launchers -------------------------------------------------------------------------------------------
+
+int launch_twiddles(cplx *tw, int Mtab, cudaStream_t st)
+{
+    S2W_LAUNCH(twiddle_kernel, (Mtab + 255) / 256, 256, 0, st, tw, Mtab);
+    return S2W_OK;
+}
+
+int launch_fft_tables(const FftTab &T, cplx *chirp, cplx *rw_in1, cplx *rw_out1, cplx *rw_in3, cplx *rw_out3,
+                      cplx *bhat_m, cplx *bhat_p, cplx *what, cudaStream_t st)
+{
+    S2W_LAUNCH(chirp_kernel, (T.n + 255) / 256, 256, 0, st, chirp, rw_in1, rw_out1, rw_in3, rw_out3, T.n, T.L);
+    size_t sm = fft_smem_bytes(T);
+    int rc = set_smem(kernel_spectrum_kernel, sm);
+    if (rc) return rc;
+    S2W_LAUNCH(kernel_spectrum_kernel, 1, 256, sm, st, bhat_m, 0, T);
+    S2W_LAUNCH(kernel_spectrum_kernel, 1, 256, sm, st, bhat_p, 1, T);
+    S2W_LAUNCH(kernel_spectrum_kernel, 1, 256, sm, st, what, 2, T);
+    return S2W_OK;
+}
+
+int launch_ring_fwd(bool real, const void *in, cplx *out, int B, int Lg, size_t sig_stride, const FftTab &T,
+                    cudaStream_t st)
+{
+    const int nrows = B * Lg;
+    if (nrows <= 0) return S2W_OK;
+    size_t sm = fft_smem_bytes(T);
+    int rc;
+    if (real) {
+        if ((rc = set_smem(ring_fwd_kernel<true>, sm))) return rc;
+        S2W_LAUNCH(ring_fwd_kernel<true>, (nrows + 1) / 2, 256, sm, st, in, out, nrows, sig_stride, T);
+    } else {
+        if ((rc = set_smem(ring_fwd_kernel<false>, sm))) return rc;
+        S2W_LAUNCH(ring_fwd_kernel<false>, nrows, 256, sm, st, in, out, nrows, sig_stride, T);
+    }
+    return S2W_OK;
+}
+
+int launch_ring_inv(bool real, const cplx *in, void *out, int B, int Lg, size_t sig_stride, const FftTab &T,
+                    cudaStream_t st)
+{
+    const int nrows = B * Lg;
+    if (nrows <= 0) return S2W_OK;
+    size_t sm = fft_smem_bytes(T);
+    int rc;
+    if (real) {
+        if ((rc = set_smem(ring_inv_kernel<true>, sm))) return rc;
+        S2W_LAUNCH(ring_inv_kernel<true>, (nrows + 1) / 2, 256, sm, st, in, out, nrows, sig_stride, T);
+    } else {
+        if ((rc = set_smem(ring_inv_kernel<false>, sm))) return rc;
+        S2W_LAUNCH(ring_inv_kernel<false>, nrows, 256, sm, st, in, out, nrows, sig_stride, T);
+    }
+    return S2W_OK;
+}
+
+int launch_so3_inv(bool real, const cplx *F, void *W, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
+                   cudaStream_t st)
+{
+    size_t sm = fft_smem_bytes(T);
+    dim3 grid(T.L, batch);
+    int rc;
+    if (real) {
+        if ((rc = set_smem(so3_inv_kernel<true>, sm))) return rc;
+        S2W_LAUNCH(so3_inv_kernel<true>, grid, 256, sm, st, F, W, sig_stride, A, T);
+    } else {
+        if ((rc = set_smem(so3_inv_kernel<false>, sm))) return rc;
+        S2W_LAUNCH(so3_inv_kernel<false>, grid, 256, sm, st, F, W, sig_stride, A, T);
+    }
+    return S2W_OK;
+}
+
+int launch_so3_fwd(bool real, const void *W, size_t sig_stride, cplx *F, const So3Args &A, int batch, const FftTab &T,
+                   cudaStream_t st)
+{
+    size_t sm = fft_smem_bytes(T);
+    dim3 grid(T.L, batch);
+    int rc;
+    if (real) {
+        if ((rc = set_smem(so3_fwd_kernel<true>, sm))) return rc;
+        S2W_LAUNCH(so3_fwd_kernel<true>, grid, 256, sm, st, W, F, sig_stride, A, T);
+    } else {
+        if ((rc = set_smem(so3_fwd_kernel<false>, sm))) return rc;
+        S2W_LAUNCH(so3_fwd_kernel<false>, grid, 256, sm, st, W, F, sig_stride, A, T);
+    }
+    return S2W_OK;
+}
+
+int launch_reweight(cplx *F, const RwArgs &A, int batch, const FftTab &T, cudaStream_t st)
+{
+    if (A.nn <= 0) return S2W_OK;
+    size_t sm = fft_smem_bytes(T);
+    int rc = set_smem(reweight_kernel, sm);
+    if (rc) return rc;
+    dim3 grid(A.Md, A.nn, batch);
+    S2W_LAUNCH(reweight_kernel, grid, 256, sm, st, F, A, T);
+    return S2W_OK;
+}
+
+}  // namespace s2w

@@ -1,0 +1,157 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via paper_2402_01282_b200.api) against the CPU oracle,
+element by element on the same seeded inputs.  Tolerances are BASELINE.json's: forward coefficients within
+1e-11 relative max error per scale block, round trip within 1e-12 relative max error (reading R12)."""
+import numpy as np
+import pytest
+
+from oracle import sphere as S
+from paper_2402_01282_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+FWD_TOL = 1e-11
+RT_TOL = 1e-12
+
+
+def _api():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2402_01282_b200 import api
+    return torch, api
+
+
+def _signals(L, seed, real, batch, spectrum="l^-2"):
+    """(flm [batch][L][2L-1], pixels [batch][L][2L-1]) -- pixels by the oracle's inverse SHT in long double."""
+    gen = inputs.flm_real if real else inputs.flm_complex
+    flm = gen(L, seed, batch, spectrum)
+    f = np.stack([S.sht_inverse(flm[b], L, "f80") for b in range(batch)])
+    if real:
+        assert np.abs(f.imag).max() < 1e-14 * max(1.0, np.abs(f).max())
+        return flm, np.ascontiguousarray(f.real.astype(np.float64))
+    return flm, np.ascontiguousarray(f.astype(np.complex128))
+
+
+def _relmax(a, b):
+    den = np.abs(b).max()
+    num = np.abs(a - b).max()
+    return num if den == 0 else num / den
+
+
+@pytest.mark.parametrize("L,real,batch", [(1, False, 1), (2, True, 1), (5, False, 2), (16, True, 3), (33, False, 1),
+                                          (64, True, 1), (100, False, 1)])
+def test_harmonic_transforms_match_oracle(L, real, batch):
+    torch, api = _api()
+    flm, f = _signals(L, 11 + L, real, batch)
+    plan = api.s2wav_plan_create(L, 1, 2.0, 0, True, real, batch)
+    fd = torch.from_numpy(f).cuda()
+    got = plan.harmonic_forward(fd, L * (2 * L - 1)).cpu().numpy().reshape(batch, L, 2 * L - 1)
+    for b in range(batch):
+        ref = S.sht_forward(f[b], L, "f80").astype(np.complex128)
+        assert _relmax(got[b], ref) < FWD_TOL
+        assert _relmax(got[b], flm[b]) < FWD_TOL
+    back = plan.harmonic_inverse(torch.from_numpy(flm).cuda()).cpu().numpy().reshape(batch, L, 2 * L - 1)
+    assert _relmax(back, f) < RT_TOL
+    plan.close()
+
+
+CASES = [
+    # L, N, lam, J0, multires, real, batch
+    (32, 1, 2.0, 0, False, True, 1),      # BASELINE config 1
+    (16, 3, 2.0, 0, True, False, 1),
+    (24, 4, 2.0, 1, True, True, 2),       # even N: imaginary zeta
+    (20, 5, 3.0, 1, True, False, 1),
+    (9, 2, 2.0, 0, True, True, 1),        # L_0 = 2 with N = 2
+    (12, 3, 2.0, 0, True, False, 3),      # L_0 = 2 < N
+    (40, 3, 1.7, 2, True, True, 5),       # non-integer lambda, batch > 4 (two column chunks)
+    (64, 5, 2.0, 2, False, False, 1),     # no multiresolution
+    (7, 7, 2.0, 0, True, True, 1),        # N = L
+    (1, 1, 2.0, 0, True, False, 1),       # degenerate L = 1
+]
+
+
+@pytest.mark.parametrize("L,N,lam,J0,mr,real,batch", CASES)
+def test_forward_inverse_parity_small(L, N, lam, J0, mr, real, batch):
+    torch, api = _api()
+    spectrum = "white" if L == 32 and N == 1 else "l^-2"
+    flm, f = _signals(L, 100 + L + N, real, batch, spectrum)
+    plan = api.s2wav_plan_create(L, N, lam, J0, mr, real, batch)
+    w = plan.forward(torch.from_numpy(f).cuda())
+    scal, scales = plan.split(w)
+    filt = S.filters(L, N, lam, J0, "f80")
+    worst = 0.0
+    for b in range(batch):
+        o_phi, o_psi = S.analysis(f[b], L, N, lam, J0, mr, "f80", filt)
+        e = _relmax(scal[b].cpu().numpy(), o_phi.astype(np.complex128) if not real else o_phi.real.astype(np.float64))
+        worst = max(worst, e)
+        for j in range(plan.J0, plan.J + 1):
+            ref = o_psi[j]
+            if real:
+                assert np.abs(ref.imag).max() <= 1e-13 * max(np.abs(ref).max(), 1e-300)
+                ref = ref.real.astype(np.float64)
+            else:
+                ref = ref.astype(np.complex128)
+            got = scales[(j, 0)][b].cpu().numpy()
+            assert got.shape == ref.shape
+            worst = max(worst, _relmax(got, ref))
+    assert worst < FWD_TOL, worst
+    # round trip on the GPU
+    back = plan.inverse(w).cpu().numpy().reshape(f.shape)
+    assert _relmax(back, f) < RT_TOL
+    # synthesis parity: oracle coefficients in, compare with the oracle's synthesis
+    o_phi, o_psi = S.analysis(f[0], L, N, lam, J0, mr, "f80", filt)
+    o_f = S.synthesis(o_phi, o_psi, L, N, lam, J0, mr, "f80", filt)
+    packed = np.zeros((batch, plan.coeff_elems), dtype=f.dtype)
+    cast = (lambda a: a.real.astype(np.float64)) if real else (lambda a: a.astype(np.complex128))
+    nr, ng, nt, npx, off = plan.scale_shape(-1)
+    packed[0, off:off + nt * npx] = cast(o_phi).ravel()
+    for j in range(plan.J0, plan.J + 1):
+        nr, ng, nt, npx, off = plan.scale_shape(j)
+        packed[0, off:off + ng * nt * npx] = cast(o_psi[j]).ravel()
+    back = plan.inverse(torch.from_numpy(packed).cuda()).cpu().numpy().reshape(f.shape)
+    assert _relmax(back[0], cast(o_f)) < FWD_TOL
+    plan.close()
+
+
+def test_config2_full_parity():
+    """BASELINE config 2: L = 256, N = 3, lambda = 2, J0 = 2, multiresolution, complex signal, seed 1."""
+    torch, api = _api()
+    c = inputs.CONFIGS["C2"]
+    L, N, lam, J0 = c["L"], c["N"], c["lam"], c["J0"]
+    flm = inputs.config_coefficients("C2")
+    f = np.ascontiguousarray(S.sht_inverse(flm[0], L, "f80").astype(np.complex128))[None]
+    plan = api.s2wav_plan_create(L, N, lam, J0, True, False, 1)
+    w = plan.forward(torch.from_numpy(f).cuda())
+    scal, scales = plan.split(w)
+    filt = S.filters(L, N, lam, J0, "f80")
+    o_phi, o_psi = S.analysis_from_flm(S.sht_forward(f[0], L, "f80"), L, N, lam, J0, True, "f80", filt)
+    assert _relmax(scal[0].cpu().numpy(), o_phi.astype(np.complex128)) < FWD_TOL
+    for j in range(plan.J0, plan.J + 1):
+        assert _relmax(scales[(j, 0)][0].cpu().numpy(), o_psi[j].astype(np.complex128)) < FWD_TOL, j
+    back = plan.inverse(w).cpu().numpy().reshape(f.shape)
+    assert _relmax(back, f) < RT_TOL
+    plan.close()
+
+
+def test_argument_style_entry_points_and_host_path():
+    torch, api = _api()
+    L, N, lam, J0 = 16, 3, 2.0, 1
+    flm, f = _signals(L, 5, True, 2)
+    fd = torch.from_numpy(f).cuda()
+    w = api.s2wav_forward(fd, L, N, lam, J0, True)
+    back = api.s2wav_inverse(w, L, N, lam, J0, True)
+    assert _relmax(back.cpu().numpy(), f) < RT_TOL
+    wh = api.s2wav_forward_host(f, L, N, lam, J0, True)
+    assert np.array_equal(wh, w.cpu().numpy())
+    fh = api.s2wav_inverse_host(wh, L, N, lam, J0, True)
+    assert _relmax(fh, f) < RT_TOL
+    assert api.launch_count() > 0
+
+
+def test_error_codes():
+    torch, api = _api()
+    with pytest.raises(api.S2WError):
+        api.s2wav_plan_create(8, 9, 2.0, 0)          # N > L
+    with pytest.raises(api.S2WError):
+        api.s2wav_plan_create(8, 2, 1.0, 0)          # lambda <= 1
+    with pytest.raises(api.S2WError):
+        api.s2wav_plan_create(8, 2, 2.0, 7)          # J0 > J
