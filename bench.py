@@ -1,0 +1,408 @@
+"""bench.py -- throughput of the fp64 directional wavelet transform (forward + inverse) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C3|C2|C1|C4]
+
+One "step" = one forward + one inverse transform of one batch of the workload (all hot-path steps a1-a8 of DESIGN.md).
+The default workload is BASELINE.json's metric configuration: L = 1024, N = 5, lambda = 2, J0 = 2, multiresolution,
+real fp64 signals, batch of 4 (configs[2]) -> 4 transforms per step.  Prints ONE JSON line (rank 0).
+
+`value`  : transforms/s with inputs resident in HBM (plan-level C-ABI calls, CUDA events, max over ranks).
+`e2e`    : the same metric through the host-buffer C-ABI calls (s2wav_forward_host / s2wav_inverse_host), pinned
+           host memory, H2D and D2H copies inside the timed region.
+`roofline`: dominant kernel class (on-the-fly Wigner contraction), bound "alu": algorithmic FP64 flops per launch
+           / device time per launch measured with cudaEvents inside the library (s2w_timing_*), against the
+           nominal DFMA peak 148 SMs x 64 lanes x 2 x sm_max_mhz.
+`cpu_baseline`: the oracle (oracle/, double instance, OpenMP) timed on a bounded sample of the same workload.
+N > 1: replicas only: every rank transforms its own batch, no data-path collective, scaling "weak".
+`--impl reference` times the oracle itself (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 wavelet fwd+inv transforms/sec"
+UNIT = "transforms/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md recipe)
+# ---------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            p = [x.strip() for x in r.split(",")]
+            if len(p) < 7:
+                continue
+            try:
+                sm.append(float(p[0]))
+                smax.append(float(p[1]))
+                power.append(float(p[2]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if p[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "reasons": sorted(reasons),
+                "power_w_max": float(max(power)), "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# workload description and algorithmic work (tuples and flops per launch class)
+# ---------------------------------------------------------------------------------------------------------------
+def stage_tuples(Lg, n_list, lmin, real):
+    """(t, m, l, n) tuples of one Wigner contraction launch: all Lg rings, l in [max(|m|,|n|,lmin), Lg),
+    m >= 0 (the (-m,-n) column shares the recursion: d^l_{-m,-n} = (-1)^{m+n} d^l_{mn})."""
+    m = np.arange(Lg)
+    tot = 0
+    for n in n_list:
+        lo = np.maximum(np.maximum(m, abs(n)), lmin)
+        tot += int(np.clip(Lg - lo, 0, None).sum()) * Lg
+    return tot
+
+
+def workload_stages(cfg, api):
+    """[(Lg, n_list, lmin)] for the contraction launches of ONE direction of one transform pair: the set is the same
+    for the inverse-type kernel (a7 at L_s, a5 per scale, a7 at L) and the forward-type kernel (a3, a6, a3)."""
+    L, N, lam, J0, mr = cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"]
+    psi, phi = api.s2wav_kernels(L, N, lam, J0)
+    J = api.s2w_scale_count(L, lam)
+
+    def bl(e):
+        return L if not mr else int(min(int(np.ceil(lam ** e - 1e-9)), L))
+    stages = [(L, [0], 0), (bl(J0), [0], 0)]
+    for j in range(J0, J + 1):
+        Lj = bl(j + 1)
+        a = np.abs(psi[j - J0][:Lj])
+        ns = [n for n in range(-(N - 1), N, 2) if abs(n) < Lj and a[:, n + N - 1].any()]
+        nz = np.nonzero(a.any(axis=1))[0]
+        if len(ns) and len(nz):
+            stages.append((Lj, ns, int(nz[0])))
+    return stages
+
+
+def contraction_flops_per_step(cfg, api):
+    """Algorithmic FP64 flops of the Wigner contraction kernels in one step, per kernel class:
+    per tuple 5 flops for the recursion step (shared by all columns) + 4 flops per complex column
+    (2 DFMA: d * (re, im)); columns = batch (real) or 2 * batch (complex: (m,n) and (-m,-n))."""
+    cols = cfg["batch"] * (1 if cfg["real"] else 2)
+    tup = sum(stage_tuples(Lg, ns, lmin, cfg["real"]) for (Lg, ns, lmin) in workload_stages(cfg, api))
+    return tup, tup * (5.0 + 4.0 * cols)
+
+
+def make_signals(cfg, api, torch, device, seed_offset=0):
+    """Band-limited synthetic signals of the workload, resident on `device`: coefficients from the seeded recipe of
+    paper_2402_01282_b200.inputs, synthesised to MW pixels by the library's own inverse
+    harmonic transform (set-up, outside every timed region)."""
+    from paper_2402_01282_b200 import inputs
+    L, B, real = cfg["L"], cfg["batch"], cfg["real"]
+    gen = inputs.flm_real if real else inputs.flm_complex
+    flm = gen(L, cfg["seed"] + 1000 * seed_offset, B, cfg["spectrum"])
+    plan = api.s2wav_plan_create(L, 1, cfg["lam"], 0, True, real, B, device.index or 0)
+    f = plan.harmonic_inverse(torch.from_numpy(flm).to(device))
+    torch.cuda.synchronize()
+    plan.close()
+    return f.reshape(B, L, 2 * L - 1)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# CPU baseline: the oracle as it stands (double instance, OpenMP), on a bounded sample of the workload
+# ---------------------------------------------------------------------------------------------------------------
+def oracle_sample(cfg, nrings=None):
+    """Times the oracle's analysis of ONE signal restricted to the top wavelet scale and to `nrings` of its beta
+    rings (same sums, fewer outputs: oracle.sphere.analysis_from_flm(scales=, rings=)), and scales the time to one
+    full forward + inverse transform by the tuple counts of DESIGN.md (forward and inverse visit the same tuples).
+    Returns (transforms/s, cores, description, seconds)."""
+    from oracle import sphere as S
+    from paper_2402_01282_b200 import inputs
+    L, N, lam, J0, mr, real = cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"], cfg["real"]
+    gen = inputs.flm_real if real else inputs.flm_complex
+    flm = gen(L, cfg["seed"], 1, cfg["spectrum"])[0]
+    filt = S.filters(L, N, lam, J0, "f64")
+    psi, phi, J = filt
+    Lj = S.bandlimit_of_scale(J, L, lam, mr)
+    if nrings is None:
+        nrings = max(1, min(Lj, int(round(6.0e9 / (N * float(Lj) ** 2 * 4.0)))))  # ~10-30 s of CPU work
+    rings = np.unique(np.linspace(0, Lj - 1, nrings).astype(int))
+    S.wigner_d(8, 1, 0, 0.3, "f64")  # loads / builds the library outside the timed region
+    t0 = time.perf_counter()
+    S.analysis_from_flm(flm, L, N, lam, J0, mr, "f64", filt, scales=[J], rings={J: rings})
+    dt = time.perf_counter() - t0
+    # tuples of the sample (complex oracle: both signs of m) vs tuples of a full forward + inverse transform
+    a = np.abs(psi[J - J0][:Lj])
+    ns = [n for n in range(-(N - 1), N, 2) if abs(n) < Lj and a[:, n + N - 1].any()]
+    lmin = int(np.nonzero(a.any(axis=1))[0][0])
+    per_ring = 0
+    for n in ns:
+        m = np.abs(np.arange(-(Lj - 1), Lj))
+        per_ring += int(np.clip(Lj - np.maximum(np.maximum(m, abs(n)), lmin), 0, None).sum())
+    sample_tuples = per_ring * len(rings)
+    return dt, sample_tuples, S.num_threads("f64"), ("oracle analysis of 1 signal, top scale j=%d (L_j=%d), %d of %d "
+                                                    "beta rings; scaled by (t,m,l,n) tuple count" % (J, Lj, len(rings), Lj))
+
+
+def full_tuples_complex(cfg, api_or_none=None):
+    """(t, m, l, n) tuples of one forward + inverse transform as the oracle visits them (all m of both signs)."""
+    from oracle import sphere as S
+    L, N, lam, J0, mr = cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"]
+    psi, phi, J = S.filters(L, N, lam, J0, "f64")
+    tot = 0
+
+    def add(Lg, ns, lmin):
+        t = 0
+        m = np.abs(np.arange(-(Lg - 1), Lg))
+        for n in ns:
+            t += int(np.clip(Lg - np.maximum(np.maximum(m, abs(n)), lmin), 0, None).sum()) * Lg
+        return t
+    tot += add(L, [0], 0) + add(S.bandlimit_of_scaling(L, lam, J0, mr), [0], 0)
+    for j in range(J0, J + 1):
+        Lj = S.bandlimit_of_scale(j, L, lam, mr)
+        a = np.abs(np.asarray(psi[j - J0][:Lj], dtype=np.complex128))
+        ns = [n for n in range(-(N - 1), N, 2) if abs(n) < Lj and a[:, n + N - 1].any()]
+        nz = np.nonzero(a.any(axis=1))[0]
+        if len(ns) and len(nz):
+            tot += add(Lj, ns, int(nz[0]))
+    return 2 * tot  # analysis + synthesis
+
+
+def cpu_baseline(cfg):
+    dt, sample_tuples, cores, desc = oracle_sample(cfg)
+    full = full_tuples_complex(cfg)
+    est_seconds = dt * full / max(sample_tuples, 1)
+    return {"value": 1.0 / est_seconds, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "%s; sample %.1f s = %.3g of the %.3g tuples of one fwd+inv transform (extrapolated)"
+                      % (desc, dt, sample_tuples / full, full)}
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle as it stands on the host cores; each step is one bounded sample."""
+    vals, base = [], None
+    for i in range(args.warmup + args.steps):
+        base = cpu_baseline(cfg)
+        if i >= args.warmup:
+            vals.append(base["value"])
+    v = float(np.mean(vals))
+    base["value"] = v
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * cfg["batch"] / v,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(cfg, args), "cpu_baseline": base,
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def workload_config(cfg, args):
+    return {"workload": "%s: sphere L=%d N=%d lambda=%g J0=%d multires=%s %s fp64 batch=%d, forward+inverse"
+                        % (cfg["name"], cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"],
+                           "real" if cfg["real"] else "complex", cfg["batch"]),
+            "L": cfg["L"], "N": cfg["N"], "lambda": cfg["lam"], "J0": cfg["J0"], "multiresolution": cfg["multires"],
+            "batch_per_gpu": cfg["batch"], "mode": "on-the-fly Wigner recursion",
+            "parallelism": "replicas x%d (no data-path collective)" % args.gpus,
+            "l2": "coefficient block per step (%.2f GB) exceeds the 126 MB L2; no explicit flush" % cfg.get("coeff_gb", 0.0)}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------------------------
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_2402_01282_b200 import api
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    L, N, lam, J0, mr, real, B = cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"], cfg["real"], cfg["batch"]
+    f = make_signals(cfg, api, torch, device, seed_offset=rank)     # independent signals per replica
+    plan = api.s2wav_plan_create(L, N, lam, J0, mr, real, B, local)
+    cfg["coeff_gb"] = plan.coeff_elems * B * (8 if real else 16) / 1e9
+    w = torch.empty((B, plan.coeff_elems), dtype=plan.dtype, device=device)
+    back = torch.empty((B, plan.signal_elems), dtype=plan.dtype, device=device)
+
+    def step():
+        plan.forward(f, out=w)
+        plan.inverse(w, out=back)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    rt_err = float((back.view_as(f) - f).abs().max() / f.abs().max())
+
+    # ---- device-resident timing: exactly K steps, CUDA events on the launching (current) stream ----
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = api.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = api.launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+
+    # ---- per-class kernel times (same steps, event pairs around every launch; a separate pass so that the
+    #      event records do not sit inside the headline number) ----
+    api.timing_enable(True)
+    api.timing_read()
+    ksteps = max(2, min(args.steps, 5))
+    for _ in range(ksteps):
+        step()
+    torch.cuda.synchronize()
+    classes = api.timing_read()
+    api.timing_enable(False)
+
+    # ---- end to end through the host-buffer C ABI calls (pinned memory; H2D + D2H inside) ----
+    e2e = None
+    if not args.no_e2e:
+        fh = torch.empty(f.shape, dtype=f.dtype, pin_memory=True)
+        fh.copy_(f)
+        fh_np = fh.numpy()
+        api.s2wav_inverse_host(api.s2wav_forward_host(fh_np, L, N, lam, J0, mr), L, N, lam, J0, mr)  # warm-up
+        barrier()
+        nrep = max(1, min(args.steps, 3))
+        t0 = time.perf_counter()
+        for _ in range(nrep):
+            wh = api.s2wav_forward_host(fh_np, L, N, lam, J0, mr)
+            fb = api.s2wav_inverse_host(wh, L, N, lam, J0, mr)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        esz = 8 if real else 16
+        sig_b, cof_b = plan.signal_elems * B * esz, plan.coeff_elems * B * esz
+        e2e = {"dt": dt / nrep, "h2d": sig_b + cof_b, "d2h": sig_b + cof_b,
+               "rt_err": float(np.abs(fb - fh_np).max() / np.abs(fh_np).max())}
+
+    # ---- max over ranks ----
+    tmax = torch.tensor([ms, e2e["dt"] if e2e else 0.0], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms, e2e_dt = float(tmax[0]), float(tmax[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    value = world * B * args.steps / (ms * 1e-3)
+    tup, flops = contraction_flops_per_step(cfg, api)   # per class per step
+    dom = max(("wigner_inverse", "wigner_forward"), key=lambda k: classes[k][0])
+    dom_ms, dom_n = classes[dom]
+    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+    peak = 148 * 64 * 2 * sm_max * 1e6 / 1e12          # nominal DFMA peak, TFLOP/s
+    achieved = flops * ksteps / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+    try:
+        probe = {"dfma_tflops": api.probe_fp64(0, local), "dmma_tflops": api.probe_fp64(1, local)}
+    except Exception as e:  # noqa: BLE001
+        probe = {"error": str(e)}
+    total_kms = sum(v[0] for v in classes.values())
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, args),
+        "clocks": clocks, "gpu_launches": int(launches),
+        "roundtrip_rel_err": rt_err,
+        "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                     "frac": achieved / peak if peak else None, "traffic": None,
+                     "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x sm_max_mhz (DESIGN.md); "
+                                    "measured DFMA-chain probe beside it",
+                     "probe": probe, "tuples_per_step": tup, "flops_per_step": flops,
+                     "launches_per_step": dom_n / ksteps, "ms_per_step": dom_ms / ksteps},
+        "kernel_ms_per_step": {k: round(v[0] / ksteps, 4) for k, v in classes.items()},
+        "kernel_share": {k: round(v[0] / total_kms, 4) for k, v in classes.items()} if total_kms else None,
+    }
+    if e2e:
+        line["e2e"] = {"value": world * B / e2e_dt, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"],
+                       "d2h_bytes_per_step": e2e["d2h"], "roundtrip_rel_err": e2e["rt_err"]}
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(cfg)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    from paper_2402_01282_b200 import inputs
+    cfg = dict(inputs.CONFIGS[args.workload])
+    cfg["name"] = args.workload
+    cfg["multires"] = cfg["multires"]
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_reference(args, cfg)
+        return
+    run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

@@ -128,6 +128,17 @@ int s2w_cache_clear(void);
  * `device` and writes the achieved TFLOP/s.  Used by bench.py to report the measured ALU peak. */
 int s2w_probe_fp64(int kind, int device, double *tflops);
 
+/* Per-class device timers (bench.py's roofline and step breakdown).  While enabled, every kernel launch of the
+ * library is bracketed by a cudaEvent pair on its stream (no host synchronisation is added).  s2w_timing_read
+ * synchronises on the recorded events, writes the summed device milliseconds and the launch count of each class
+ * since the previous read into ms[nclass] / launches[nclass] (host arrays), and clears the record.  Classes:
+ * 0 inverse Wigner contraction (a5, a7), 1 forward Wigner contraction (a3, a6), 2 ring FFT (a1), 3 (alpha, gamma)
+ * FFT (a8), 4 theta reweighting (a2), 5 radial Laguerre contraction (a10), 6 everything else; classes >= nclass
+ * are folded into the last one. */
+#define S2W_TIMING_CLASSES 7
+int s2w_timing_enable(int on);
+int s2w_timing_read(double *ms, unsigned long long *launches, int nclass);
+
 /* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
 unsigned long long s2w_launch_count(void);
 

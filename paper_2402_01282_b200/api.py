@@ -48,6 +48,8 @@ SIGNATURES = {
     "s2ball_inverse_host": (_c_int, [_c_vp, _c_vp, _c_int, _c_int, _c_int, _c_dbl, _c_dbl, _c_int, _c_dbl, _c_int]),
     "s2w_cache_clear": (_c_int, []),
     "s2w_probe_fp64": (_c_int, [_c_int, _c_int, ctypes.POINTER(_c_dbl)]),
+    "s2w_timing_enable": (_c_int, [_c_int]),
+    "s2w_timing_read": (_c_int, [_c_vp, _c_vp, _c_int]),
     "s2w_launch_count": (ctypes.c_ulonglong, []),
     "s2w_last_error": (ctypes.c_char_p, []),
 }
@@ -336,6 +338,21 @@ def probe_fp64(kind, device=0):
     v = _c_dbl(0.0)
     _check(lib().s2w_probe_fp64(int(kind), int(device), ctypes.byref(v)))
     return v.value
+
+
+TIMING_CLASSES = ("wigner_inverse", "wigner_forward", "ring_fft", "so3_fft", "reweight", "radial", "other")
+
+
+def timing_enable(on):
+    _check(lib().s2w_timing_enable(int(bool(on))))
+
+
+def timing_read():
+    """{class name: (device ms, launches)} since the previous read (synchronises on the recorded events)."""
+    ms = np.zeros(len(TIMING_CLASSES))
+    cnt = np.zeros(len(TIMING_CLASSES), dtype=np.uint64)
+    _check(lib().s2w_timing_read(_np_ptr(ms), _np_ptr(cnt), len(TIMING_CLASSES)))
+    return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(TIMING_CLASSES)}
 
 
 def launch_count():

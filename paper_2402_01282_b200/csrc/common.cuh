@@ -35,11 +35,21 @@ void count_launch();
         }                                                                                          \
     } while (0)
 
-// launch + count (every kernel of this library goes through this macro)
-#define S2W_LAUNCH(kernel, grid, block, smem, stream, ...)                                         \
+// kernel classes of the per-class device timers (s2w_timing_*; bench.py's roofline and step breakdown)
+enum { S2W_K_WIGNER_INV = 0, S2W_K_WIGNER_FWD = 1, S2W_K_RING_FFT = 2, S2W_K_SO3_FFT = 3, S2W_K_REWEIGHT = 4,
+       S2W_K_RADIAL = 5, S2W_K_OTHER = 6, S2W_K_NCLASS = 7 };
+void timing_begin(int cls, cudaStream_t st);  // no-ops unless s2w_timing_enable(1)
+void timing_end(cudaStream_t st);
+
+// launch + count (every kernel of this library goes through these macros)
+#define S2W_LAUNCH_C(cls, kernel, grid, block, smem, stream, ...)                                  \
     do {                                                                                           \
+        s2w::timing_begin((cls), (stream));                                                        \
         kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);                                \
+        s2w::timing_end((stream));                                                                 \
         s2w::count_launch();                                                                       \
     } while (0)
+#define S2W_LAUNCH(kernel, grid, block, smem, stream, ...)                                         \
+    S2W_LAUNCH_C(s2w::S2W_K_OTHER, kernel, grid, block, smem, stream, __VA_ARGS__)
 
 }  // namespace s2w

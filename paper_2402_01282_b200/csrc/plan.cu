@@ -25,6 +25,39 @@ static unsigned long long g_launches = 0;
 void set_error(const std::string &msg) { g_err = msg; }
 void count_launch() { ++g_launches; }
 
+// ---- per-class device timers: cudaEvent pairs around every launch while enabled (s2w_timing_enable/read) ----
+namespace {
+struct TimedLaunch {
+    cudaEvent_t a, b;
+    int cls;
+};
+bool g_timing = false;
+std::vector<TimedLaunch> g_timed;     // recorded since the last read
+std::vector<TimedLaunch> g_ev_free;   // recycled event pairs
+std::mutex g_timing_mu;
+}  // namespace
+void timing_begin(int cls, cudaStream_t st)
+{
+    if (!g_timing) return;
+    std::lock_guard<std::mutex> lock(g_timing_mu);
+    TimedLaunch t;
+    if (!g_ev_free.empty()) {
+        t = g_ev_free.back();
+        g_ev_free.pop_back();
+    } else {
+        if (cudaEventCreate(&t.a) != cudaSuccess || cudaEventCreate(&t.b) != cudaSuccess) return;
+    }
+    t.cls = cls;
+    cudaEventRecord(t.a, st);
+    g_timed.push_back(t);
+}
+void timing_end(cudaStream_t st)
+{
+    if (!g_timing) return;
+    std::lock_guard<std::mutex> lock(g_timing_mu);
+    if (!g_timed.empty()) cudaEventRecord(g_timed.back().b, st);
+}
+
 namespace {
 
 typedef long double ld;
@@ -1004,6 +1037,42 @@ int s2w_cache_clear(void)
     }
     g_cache.clear();
     return S2W_OK;
+}
+
+int s2w_timing_enable(int on)
+{
+    std::lock_guard<std::mutex> lock(g_timing_mu);
+    g_timing = on != 0;
+    return S2W_OK;
+}
+
+int s2w_timing_read(double *ms, unsigned long long *launches, int nclass)
+{
+    if (!ms || !launches || nclass < 1) {
+        set_error("invalid argument");
+        return S2W_EINVAL;
+    }
+    std::lock_guard<std::mutex> lock(g_timing_mu);
+    for (int c = 0; c < nclass; ++c) {
+        ms[c] = 0.0;
+        launches[c] = 0;
+    }
+    int rc = S2W_OK;
+    for (size_t i = 0; i < g_timed.size(); ++i) {
+        float t = 0.f;
+        if (cudaEventSynchronize(g_timed[i].b) != cudaSuccess ||
+            cudaEventElapsedTime(&t, g_timed[i].a, g_timed[i].b) != cudaSuccess) {
+            set_error(std::string("timing events: ") + cudaGetErrorString(cudaGetLastError()));
+            rc = S2W_ECUDA;
+        } else {
+            const int c = g_timed[i].cls < nclass ? g_timed[i].cls : nclass - 1;
+            ms[c] += (double)t;
+            launches[c] += 1;
+        }
+        g_ev_free.push_back(g_timed[i]);
+    }
+    g_timed.clear();
+    return rc;
 }
 
 int s2w_probe_fp64(int kind, int device, double *tflops)

@@ -423,10 +423,10 @@ int launch_ring_fwd(bool real, const void *in, cplx *out, int B, int Lg, size_t 
     int rc;
     if (real) {
         if ((rc = set_smem(ring_fwd_kernel<true>, sm))) return rc;
-        S2W_LAUNCH(ring_fwd_kernel<true>, (nrows + 1) / 2, 256, sm, st, in, out, nrows, sig_stride, T);
+        S2W_LAUNCH_C(S2W_K_RING_FFT, ring_fwd_kernel<true>, (nrows + 1) / 2, 256, sm, st, in, out, nrows, sig_stride, T);
     } else {
         if ((rc = set_smem(ring_fwd_kernel<false>, sm))) return rc;
-        S2W_LAUNCH(ring_fwd_kernel<false>, nrows, 256, sm, st, in, out, nrows, sig_stride, T);
+        S2W_LAUNCH_C(S2W_K_RING_FFT, ring_fwd_kernel<false>, nrows, 256, sm, st, in, out, nrows, sig_stride, T);
     }
     return S2W_OK;
 }
@@ -440,10 +440,10 @@ int launch_ring_inv(bool real, const cplx *in, void *out, int B, int Lg, size_t 
     int rc;
     if (real) {
         if ((rc = set_smem(ring_inv_kernel<true>, sm))) return rc;
-        S2W_LAUNCH(ring_inv_kernel<true>, (nrows + 1) / 2, 256, sm, st, in, out, nrows, sig_stride, T);
+        S2W_LAUNCH_C(S2W_K_RING_FFT, ring_inv_kernel<true>, (nrows + 1) / 2, 256, sm, st, in, out, nrows, sig_stride, T);
     } else {
         if ((rc = set_smem(ring_inv_kernel<false>, sm))) return rc;
-        S2W_LAUNCH(ring_inv_kernel<false>, nrows, 256, sm, st, in, out, nrows, sig_stride, T);
+        S2W_LAUNCH_C(S2W_K_RING_FFT, ring_inv_kernel<false>, nrows, 256, sm, st, in, out, nrows, sig_stride, T);
     }
     return S2W_OK;
 }
@@ -456,10 +456,10 @@ int launch_so3_inv(bool real, const cplx *F, void *W, size_t sig_stride, const S
     int rc;
     if (real) {
         if ((rc = set_smem(so3_inv_kernel<true>, sm))) return rc;
-        S2W_LAUNCH(so3_inv_kernel<true>, grid, 256, sm, st, F, W, sig_stride, A, T);
+        S2W_LAUNCH_C(S2W_K_SO3_FFT, so3_inv_kernel<true>, grid, 256, sm, st, F, W, sig_stride, A, T);
     } else {
         if ((rc = set_smem(so3_inv_kernel<false>, sm))) return rc;
-        S2W_LAUNCH(so3_inv_kernel<false>, grid, 256, sm, st, F, W, sig_stride, A, T);
+        S2W_LAUNCH_C(S2W_K_SO3_FFT, so3_inv_kernel<false>, grid, 256, sm, st, F, W, sig_stride, A, T);
     }
     return S2W_OK;
 }
@@ -472,10 +472,10 @@ int launch_so3_fwd(bool real, const void *W, size_t sig_stride, cplx *F, const S
     int rc;
     if (real) {
         if ((rc = set_smem(so3_fwd_kernel<true>, sm))) return rc;
-        S2W_LAUNCH(so3_fwd_kernel<true>, grid, 256, sm, st, W, F, sig_stride, A, T);
+        S2W_LAUNCH_C(S2W_K_SO3_FFT, so3_fwd_kernel<true>, grid, 256, sm, st, W, F, sig_stride, A, T);
     } else {
         if ((rc = set_smem(so3_fwd_kernel<false>, sm))) return rc;
-        S2W_LAUNCH(so3_fwd_kernel<false>, grid, 256, sm, st, W, F, sig_stride, A, T);
+        S2W_LAUNCH_C(S2W_K_SO3_FFT, so3_fwd_kernel<false>, grid, 256, sm, st, W, F, sig_stride, A, T);
     }
     return S2W_OK;
 }
@@ -487,7 +487,7 @@ int launch_reweight(cplx *F, const RwArgs &A, int batch, const FftTab &T, cudaSt
     int rc = set_smem(reweight_kernel, sm);
     if (rc) return rc;
     dim3 grid(A.Md, A.nn, batch);
-    S2W_LAUNCH(reweight_kernel, grid, 256, sm, st, F, A, T);
+    S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight_kernel, grid, 256, sm, st, F, A, T);
     return S2W_OK;
 }
 
