@@ -333,6 +333,62 @@ def s2wav_inverse_host(w, L, N, lam, J0, multiresolution=True):
     return f
 
 
+def _coeff_elems_ball(L, P, N, lam_l, lam_p, J0):
+    key = ("ball", L, P, N, float(lam_l), float(lam_p), J0)
+    if key not in _SIZE_CACHE:
+        J, Jp = s2w_scale_count(L, lam_l), s2w_scale_count(P, lam_p)
+
+        def bl(lam, e, cap):
+            return int(min(int(np.ceil(float(lam) ** e - 1e-9)), cap))
+        tot = P * L * (2 * L - 1)
+        for jp in range(J0, Jp + 1):
+            Pj = bl(lam_p, jp + 1, P)
+            for j in range(J0, J + 1):
+                Lj = bl(lam_l, j + 1, L)
+                tot += Pj * (2 * N - 1) * Lj * (2 * Lj - 1)
+        _SIZE_CACHE[key] = tot
+    return _SIZE_CACHE[key]
+
+
+def s2ball_forward(f, L, P, N, lam_l, lam_p, J0, tau=1.0):
+    """f: CUDA tensor [P, L, 2L-1] on the Gauss-Laguerre shells -> packed coefficients [K]."""
+    torch = _torch()
+    f = f.contiguous()
+    real = f.dtype == torch.float64
+    w = torch.empty(_coeff_elems_ball(L, P, N, lam_l, lam_p, J0), dtype=f.dtype, device=f.device)
+    _check(lib().s2ball_forward(f.data_ptr(), w.data_ptr(), int(L), int(P), int(N), float(lam_l), float(lam_p),
+                                int(J0), float(tau), S2W_REAL if real else 0, _stream_ptr()))
+    return w
+
+
+def s2ball_inverse(w, L, P, N, lam_l, lam_p, J0, tau=1.0):
+    torch = _torch()
+    w = w.contiguous()
+    real = w.dtype == torch.float64
+    f = torch.empty((P, L, 2 * L - 1), dtype=w.dtype, device=w.device)
+    _check(lib().s2ball_inverse(w.data_ptr(), f.data_ptr(), int(L), int(P), int(N), float(lam_l), float(lam_p),
+                                int(J0), float(tau), S2W_REAL if real else 0, _stream_ptr()))
+    return f
+
+
+def s2ball_forward_host(f, L, P, N, lam_l, lam_p, J0, tau=1.0):
+    f = np.ascontiguousarray(f)
+    real = f.dtype == np.float64
+    w = np.empty(_coeff_elems_ball(L, P, N, lam_l, lam_p, J0), dtype=f.dtype)
+    _check(lib().s2ball_forward_host(_np_ptr(f), _np_ptr(w), int(L), int(P), int(N), float(lam_l), float(lam_p),
+                                     int(J0), float(tau), S2W_REAL if real else 0))
+    return w
+
+
+def s2ball_inverse_host(w, L, P, N, lam_l, lam_p, J0, tau=1.0):
+    w = np.ascontiguousarray(w)
+    real = w.dtype == np.float64
+    f = np.empty((P, L, 2 * L - 1), dtype=w.dtype)
+    _check(lib().s2ball_inverse_host(_np_ptr(w), _np_ptr(f), int(L), int(P), int(N), float(lam_l), float(lam_p),
+                                     int(J0), float(tau), S2W_REAL if real else 0))
+    return f
+
+
 def probe_fp64(kind, device=0):
     """Measured TFLOP/s of a DFMA chain (kind 0) or an fp64 mma.sync chain (kind 1)."""
     v = _c_dbl(0.0)

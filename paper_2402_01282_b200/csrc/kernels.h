@@ -29,6 +29,10 @@ struct RwArgs {
 };
 
 // one launch of the on-the-fly Wigner contraction (steps a3, a5, a6, a7)
+//
+// Rings are handled in GROUPS of 32 (one warp lane each): the rings of each hemisphere are sorted by |cos beta|
+// (equator first); group 2j holds north rings 32j..32j+31 of that order, group 2j+1 the south ones.  All rings of a
+// group start the recursion at the same degree gstart (monotone non-decreasing in j), with seeds stored at that degree.
 struct WigArgs {
     int Lg;        // band-limit of the theta grid (rings t = 0..Lg-1, |m| < Lg, l < Lg)
     int Lfull;     // band-limit of the plan (l-stride of flmT, extent of the coefficient table)
@@ -37,12 +41,14 @@ struct WigArgs {
     int nn;        // number of n values
     int nrows;     // rows per signal in F
     int lmin;      // first l with a non-zero filter entry
+    int G;         // ring groups (even)
     int n_val[S2W_MAX_ROWS], n_tab[S2W_MAX_ROWS], n_row[S2W_MAX_ROWS], n_rowm[S2W_MAX_ROWS], n_filtm[S2W_MAX_ROWS];
     size_t tri;                 // entries per n in the coefficient table: Lfull (Lfull+1)/2
-    const double *coef;         // [ntab][tri][3]: (alpha, beta, gamma) of the step l -> l+1 at packed (m, l)
-    const int *lstart;          // [ntab][Lg][Lg] (n, m, t): first l at which ring t is active
-    const double2 *dseed;       // [ntab][Lg][Lg]: (d^{lstart}, d^{lstart-1})
-    const double *xcos;         // [Lg] cos(beta_t)
+    const double *coef;         // [ntab][tri][4]: (alpha, gamma, e_N, e_S) of the step l -> l+1 at packed (m, l)
+    const int *gstart;          // [ntab][Lg (m)][G]: first degree at which group g is active
+    const double2 *dseed;       // [ntab][Lg (m)][32 G]: (d~^{gstart}, u~_{gstart-1}) per ring slot
+    const double *yv;           // [32 G] 1 - |cos beta| per ring slot (0 for empty slots)
+    const int *ring;            // [32 G] ring index t of the slot, -1 if empty
     const cplx *filt;           // [nn][Lg] filter applied to row q at degree l
     cplx *flmT;                 // [B][Mfull][Lfull]  f_{l m} stored m-major; Mfull = Lfull (real) or 2 Lfull - 1
     cplx *F;                    // [B][nrows][Lg][Md], Md = Lg (real) or 2 Lg - 1
@@ -64,9 +70,12 @@ int launch_so3_fwd(bool real, const void *W, size_t sig_stride, cplx *F, const S
                    cudaStream_t st);
 int launch_reweight(cplx *F, const RwArgs &A, int batch, const FftTab &T, cudaStream_t st);
 
-int launch_wigner_coef(double *coef, int Lfull, const int *n_vals, int ntab, cudaStream_t st);
-int launch_wigner_ramp(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg,
-                       const int *n_vals, int ntab, const double *xcos, int *lstart, double2 *dseed, cudaStream_t st);
+// plan-time: group start degrees and seeds from the range-extended values d^{l0}_{mn}(beta_t) = mant 2^expo ([ntab][Lg m][Lg t])
+int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int G,
+                        const int *n_vals, int ntab, const double *yv, const int *ring, int *gstart, double2 *dseed,
+                        cudaStream_t st);
+int launch_radial(const double *A, int R, int K, const cplx *in, cplx *out, size_t cols, int Lfull, const double *win,
+                  const double *wout, bool accumulate, cudaStream_t st);
 int launch_wigner_inverse(const WigArgs &A, cudaStream_t st);   // harmonic -> rings   (a5, a7)
 int launch_wigner_forward(const WigArgs &A, cudaStream_t st);   // rings -> harmonic   (a3, a6), accumulates
 

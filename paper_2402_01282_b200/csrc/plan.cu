@@ -97,9 +97,11 @@ struct DevPool {  // owns device allocations of a plan
 struct GridTab {  // everything that depends on the theta/phi grid of band-limit Lg
     int Lg;
     FftTab fft;
-    double *xcos;
-    int *lstart;
-    double2 *dseed;
+    int G;           // ring groups of 32 (even): 2j north, 2j+1 south, each hemisphere sorted by |cos beta|
+    double *yv;      // [32 G] 1 - |cos beta_t| of the ring in each slot
+    int *ring;       // [32 G] ring index t, -1 for an empty slot
+    int *gstart;     // [ntab][Lg][G]
+    double2 *dseed;  // [ntab][Lg][32 G]
 };
 
 struct Stage {  // one Wigner contraction launch: rows, filters
@@ -148,7 +150,8 @@ struct s2w_plan {
     // ball
     double *Kfull_fwd;  // [P p][P nodes]  q_i K_p(r_i)
     double *Kfull_inv;  // [P nodes][P p]  K_p(r_i)
-    cplx *phi_ball;     // [P][L] sqrt(4pi/(2l+1)) Phi_{l0p}
+    double *phi_ball;   // [P][L] sqrt(4pi/(2l+1)) Phi_{l0p}
+    size_t ws_shell_elems;  // ball: elements of one [P][Mfull][L] harmonic array
 };
 
 namespace s2w {
@@ -179,19 +182,34 @@ int ceil_log2(int v)
 //   d^m_{mn} = sqrt((2m)!/((m+n)!(m-n)!)) cos^{m+n}(beta/2) (-sin(beta/2))^{m-n}   for m >= |n|,
 // built by the one-term recursion in m, and for m < |n| from d^l_{mn} = (-1)^{m-n} d^l_{nm} = d^l_{-n,-m}.
 void host_seeds(int Lg, const std::vector<int> &tabn, std::vector<double> &mant, std::vector<int> &expo,
-                std::vector<double> &xcos)
+                std::vector<double> &yv, std::vector<int> &ring, int &G)
 {
     const size_t per = (size_t)Lg * Lg;
     mant.assign(tabn.size() * per, 0.0);
     expo.assign(tabn.size() * per, 0);
-    xcos.assign(Lg, 0.0);
     std::vector<ld> ch(Lg), sh(Lg);
+    // ring groups: each hemisphere sorted by |cos beta| ascending, y = 1 - |cos beta| = 2 sin^2(beta/2) or 2 cos^2(beta/2)
+    std::vector<std::pair<ld, int> > hemi[2];
     for (int t = 0; t < Lg; ++t) {
         ld beta = PI_L * (ld)(2 * t + 1) / (ld)(2 * Lg - 1);
-        xcos[t] = (double)cosl(beta);
         ch[t] = cosl(beta / 2);
         sh[t] = sinl(beta / 2);
+        const bool south = 4 * t + 2 > 2 * Lg - 1;  // beta > pi/2
+        const ld y = south ? 2 * ch[t] * ch[t] : 2 * sh[t] * sh[t];
+        hemi[south ? 1 : 0].push_back(std::make_pair(-y, t));  // |cos| ascending = y descending
     }
+    std::sort(hemi[0].begin(), hemi[0].end());
+    std::sort(hemi[1].begin(), hemi[1].end());
+    const size_t most = std::max(hemi[0].size(), hemi[1].size());
+    G = 2 * (int)std::max<size_t>(1, (most + 31) / 32);
+    yv.assign((size_t)32 * G, 0.0);
+    ring.assign((size_t)32 * G, -1);
+    for (int h = 0; h < 2; ++h)
+        for (size_t i = 0; i < hemi[h].size(); ++i) {
+            const size_t slot = ((i / 32) * 2 + h) * 32 + i % 32;
+            yv[slot] = (double)(-hemi[h][i].first);
+            ring[slot] = hemi[h][i].second;
+        }
     auto put = [&](size_t idx, ld v) {
         int e = 0;
         ld mnt = frexpl(v, &e);
@@ -237,6 +255,34 @@ void host_seeds(int Lg, const std::vector<int> &tabn, std::vector<double> &mant,
     }
 }
 
+// Recursion coefficients of the step l -> l+1 in difference form (wigner.cu), packed rows l = m..L-1 for every m >= 0
+// and every table value of n: (alpha_l, gamma_l, e_N, e_S), e_N/S = alpha_l - gamma_l - 1 -/+ beta_l, formed in long
+// double so that the cancellation in e leaves a correctly rounded double.  Entries with l < |n| are zero.
+void host_coef(int L, const std::vector<int> &tabn, std::vector<double> &coef)
+{
+    const size_t tri = (size_t)L * (L + 1) / 2;
+    coef.assign(tabn.size() * tri * 4, 0.0);
+    for (size_t tab = 0; tab < tabn.size(); ++tab) {
+        const int n = tabn[tab], an = n < 0 ? -n : n;
+        size_t o = tab * tri * 4;
+        for (int m = 0; m < L; ++m)
+            for (int l = m; l < L; ++l, o += 4) {
+                if (l < an) continue;
+                ld a = 1, b = 0, g = 0;
+                if (l > 0) {
+                    const ld lp = l + 1, lq = l, md = m, nd = n;
+                    a = lp * (2 * lq + 1) / sqrtl((lp * lp - md * md) * (lp * lp - nd * nd));
+                    b = a * md * nd / (lq * lp);
+                    g = a * sqrtl((lq * lq - md * md) * (lq * lq - nd * nd)) / (lq * (2 * lq + 1));
+                }
+                coef[o] = (double)a;
+                coef[o + 1] = (double)g;
+                coef[o + 2] = (double)(a - g - 1 - b);
+                coef[o + 3] = (double)(a - g - 1 + b);
+            }
+    }
+}
+
 int build_grid(s2w_plan *p, int Lg)
 {
     if (grid_index(p, Lg) >= 0) return S2W_OK;
@@ -271,22 +317,24 @@ int build_grid(s2w_plan *p, int Lg)
     T.what = wh;
     if ((rc = launch_fft_tables(T, chirp, i1, o1, i3, o3, bm, bp, wh, 0))) return rc;
 
-    std::vector<double> mant, xcos;
-    std::vector<int> expo;
-    host_seeds(Lg, p->tabn, mant, expo, xcos);
+    std::vector<double> mant, yv;
+    std::vector<int> expo, ring;
+    host_seeds(Lg, p->tabn, mant, expo, yv, ring, g.G);
     double *dmant;
     int *dexpo;
-    if ((rc = p->pool.upload(&g.xcos, xcos))) return rc;
-    // temporaries (freed after the ramp kernel)
+    if ((rc = p->pool.upload(&g.yv, yv))) return rc;
+    if ((rc = p->pool.upload(&g.ring, ring))) return rc;
+    // temporaries (freed after the seed kernels)
     const size_t cnt = mant.size();
+    const size_t ntab = p->tabn.size();
     S2W_CUDA_CHECK(cudaMalloc((void **)&dmant, std::max<size_t>(cnt, 1) * sizeof(double)));
     S2W_CUDA_CHECK(cudaMalloc((void **)&dexpo, std::max<size_t>(cnt, 1) * sizeof(int)));
     S2W_CUDA_CHECK(cudaMemcpy(dmant, mant.data(), cnt * sizeof(double), cudaMemcpyHostToDevice));
     S2W_CUDA_CHECK(cudaMemcpy(dexpo, expo.data(), cnt * sizeof(int), cudaMemcpyHostToDevice));
-    if ((rc = p->pool.alloc(&g.lstart, cnt))) return rc;
-    if ((rc = p->pool.alloc(&g.dseed, cnt))) return rc;
-    rc = launch_wigner_ramp(dmant, dexpo, p->coef, p->tri, p->L, Lg, p->tabn.data(), (int)p->tabn.size(), g.xcos,
-                            g.lstart, g.dseed, 0);
+    if ((rc = p->pool.alloc(&g.gstart, ntab * Lg * g.G))) return rc;
+    if ((rc = p->pool.alloc(&g.dseed, ntab * Lg * (size_t)32 * g.G))) return rc;
+    rc = launch_wigner_seeds(dmant, dexpo, p->coef, p->tri, p->L, Lg, g.G, p->tabn.data(), (int)ntab, g.yv, g.ring,
+                             g.gstart, g.dseed, 0);
     cudaError_t e = cudaDeviceSynchronize();
     cudaFree(dmant);
     cudaFree(dexpo);
@@ -341,9 +389,11 @@ void fill_wig_args(const s2w_plan *p, const Stage &st, bool synthesis, int B, cp
     }
     A.tri = p->tri;
     A.coef = p->coef;
-    A.lstart = g.lstart;
+    A.G = g.G;
+    A.gstart = g.gstart;
     A.dseed = g.dseed;
-    A.xcos = g.xcos;
+    A.yv = g.yv;
+    A.ring = g.ring;
     A.filt = synthesis ? st.filt_syn : st.filt_ana;
     A.flmT = flmT;
     A.F = F;
@@ -398,8 +448,11 @@ int plan_common(s2w_plan *p)
     for (int n = -(p->N - 1); n <= p->N - 1; n += 2) p->tabn.push_back(n);
     if (find_tab(p, 0) < 0) p->tabn.push_back(0);
     p->tri = (size_t)p->L * (p->L + 1) / 2;
-    if ((rc = p->pool.alloc(&p->coef, p->tabn.size() * p->tri * 3))) return rc;
-    if ((rc = launch_wigner_coef(p->coef, p->L, p->tabn.data(), (int)p->tabn.size(), 0))) return rc;
+    {
+        std::vector<double> coef;
+        host_coef(p->L, p->tabn, coef);
+        if ((rc = p->pool.upload(&p->coef, coef))) return rc;
+    }
     p->Mtab = 1 << std::max(1, ceil_log2(2 * (2 * p->L - 1) - 1));
     if ((rc = p->pool.alloc(&p->tw, p->Mtab))) return rc;
     if ((rc = launch_twiddles(p->tw, p->Mtab, 0))) return rc;
@@ -431,6 +484,47 @@ int make_n0_stage(s2w_plan *p, Stage &st, int Lg, const std::vector<double> &a, 
         fa[l] = cmake(a[l], 0.0);
         fs[l] = cmake(s[l], 0.0);
     }
+    return make_stage_filters(p, st, fa, fs);
+}
+
+// wavelet stage of angular scale j at band-limit sc.Lj: rows n of script-N inside the band-limit, filters
+// conj(Psi^j_{ln}) (analysis, Eq. 40) and Psi^j_{ln} (2pi)^2/(2L_j-1) (synthesis, Eq. 42), with
+// Psi^j_{ln} = sqrt((2l+1)/8pi^2) kappa^j(l) zeta_{ln} (Eq. A9).  kj = kappa^j(l), l < L.
+int make_scale_stage(s2w_plan *p, Scale &sc, const double *kj, const std::vector<double> &zeta)
+{
+    const int N = p->N, nn = 2 * N - 1;
+    const double pi = pi_d();
+    int rc;
+    if ((rc = build_grid(p, sc.Lj))) return rc;
+    Stage &st = sc.st;
+    st.grid = grid_index(p, sc.Lj);
+    st.Lg = sc.Lj;
+    st.lmin = sc.Lj;
+    for (int l = 0; l < sc.Lj; ++l)
+        if (kj[l] != 0.0) {
+            st.lmin = l;
+            break;
+        }
+    std::vector<int> ns, rows;
+    if (st.lmin < sc.Lj)
+        for (int ni = 0; ni < N; ++ni) {
+            int n = -(N - 1) + 2 * ni;
+            if (std::abs(n) < sc.Lj) {
+                ns.push_back(n);
+                rows.push_back(ni);
+            }
+        }
+    if ((rc = fill_stage_rows(p, st, ns, rows, N))) return rc;
+    std::vector<cplx> fa((size_t)st.nn * sc.Lj), fs((size_t)st.nn * sc.Lj);
+    const double syn_norm = 4.0 * pi * pi / (2.0 * sc.Lj - 1.0);
+    for (int q = 0; q < st.nn; ++q)
+        for (int l = 0; l < sc.Lj; ++l) {
+            const double pre = std::sqrt((2.0 * l + 1.0) / (8.0 * pi * pi)) * kj[l];
+            const size_t zo = ((size_t)l * nn + (st.n_val[q] + N - 1)) * 2;
+            const double re = pre * zeta[zo], im = pre * zeta[zo + 1];
+            fa[(size_t)q * sc.Lj + l] = cmake(re, -im);
+            fs[(size_t)q * sc.Lj + l] = cmake(re * syn_norm, im * syn_norm);
+        }
     return make_stage_filters(p, st, fa, fs);
 }
 
@@ -482,6 +576,45 @@ static int sht_inverse_dev(const s2w_plan *p, const Stage &st, void *f, size_t s
     return launch_ring_inv(p->real, w.F, f, B, st.Lg, sig_stride, g.fft, s);
 }
 
+// a4 + a5 + a8 for one scale: filter x inverse Wigner contraction at L_j, then the (alpha, gamma) DFT.  B signals whose
+// coefficient blocks are sig_stride elements apart.
+static int scale_analysis(const s2w_plan *p, const Scale &sc, int B, const Work &w, void *dst, size_t sig_stride,
+                          cudaStream_t s)
+{
+    const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
+    if (sc.st.nn == 0) {
+        for (int b = 0; b < B; ++b)
+            S2W_CUDA_CHECK(cudaMemsetAsync((char *)dst + (size_t)b * sig_stride * esz, 0,
+                                           (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1) * esz, s));
+        return S2W_OK;
+    }
+    int rc;
+    WigArgs A;
+    fill_wig_args(p, sc.st, false, B, w.flmT, w.F, A);
+    if ((rc = launch_wigner_inverse(A, s))) return rc;
+    So3Args S;
+    fill_so3_args(p, sc.st, S);
+    return launch_so3_inv(p->real, w.F, dst, sig_stride, S, B, p->grids[sc.st.grid].fft, s);
+}
+
+// a8 + a2 + a6 + a4 for one scale: (alpha, gamma) DFT, reweighting, forward Wigner contraction accumulating into flmT.
+static int scale_synthesis(const s2w_plan *p, const Scale &sc, int B, const Work &w, const void *src, size_t sig_stride,
+                           cudaStream_t s)
+{
+    if (sc.st.nn == 0) return S2W_OK;
+    const GridTab &g = p->grids[sc.st.grid];
+    int rc;
+    So3Args S;
+    fill_so3_args(p, sc.st, S);
+    if ((rc = launch_so3_fwd(p->real, src, sig_stride, w.F, S, B, g.fft, s))) return rc;
+    RwArgs R;
+    fill_rw_args(p, sc.st, R);
+    if ((rc = launch_reweight(w.F, R, B, g.fft, s))) return rc;
+    WigArgs A;
+    fill_wig_args(p, sc.st, true, B, w.flmT, w.F, A);
+    return launch_wigner_forward(A, s);
+}
+
 static int sphere_forward(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s)
 {
     const Work w = carve(p, work);
@@ -494,19 +627,7 @@ static int sphere_forward(const s2w_plan *p, const void *in, void *out, void *wo
         return rc;
     for (size_t i = 0; i < p->scales.size(); ++i) {
         const Scale &sc = p->scales[i];
-        void *dst = (char *)out + sc.offset * esz;
-        if (sc.st.nn == 0) {
-            for (int b = 0; b < B; ++b)
-                S2W_CUDA_CHECK(cudaMemsetAsync((char *)dst + (size_t)b * p->coeff_elems * esz, 0,
-                                               (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1) * esz, s));
-            continue;
-        }
-        WigArgs A;
-        fill_wig_args(p, sc.st, false, B, w.flmT, w.F, A);
-        if ((rc = launch_wigner_inverse(A, s))) return rc;
-        So3Args S;
-        fill_so3_args(p, sc.st, S);
-        if ((rc = launch_so3_inv(p->real, w.F, dst, p->coeff_elems, S, B, p->grids[sc.st.grid].fft, s))) return rc;
+        if ((rc = scale_analysis(p, sc, B, w, (char *)out + sc.offset * esz, p->coeff_elems, s))) return rc;
     }
     S2W_CUDA_CHECK(cudaPeekAtLastError());
     return S2W_OK;
@@ -523,20 +644,91 @@ static int sphere_inverse(const s2w_plan *p, const void *in, void *out, void *wo
         return rc;
     for (size_t i = 0; i < p->scales.size(); ++i) {
         const Scale &sc = p->scales[i];
-        if (sc.st.nn == 0) continue;
-        const void *src = (const char *)in + sc.offset * esz;
-        const GridTab &g = p->grids[sc.st.grid];
-        So3Args S;
-        fill_so3_args(p, sc.st, S);
-        if ((rc = launch_so3_fwd(p->real, src, p->coeff_elems, w.F, S, B, g.fft, s))) return rc;
-        RwArgs R;
-        fill_rw_args(p, sc.st, R);
-        if ((rc = launch_reweight(w.F, R, B, g.fft, s))) return rc;
-        WigArgs A;
-        fill_wig_args(p, sc.st, true, B, w.flmT, w.F, A);
-        if ((rc = launch_wigner_forward(A, s))) return rc;
+        if ((rc = scale_synthesis(p, sc, B, w, (const char *)in + sc.offset * esz, p->coeff_elems, s))) return rc;
     }
     if ((rc = sht_inverse_dev(p, p->sht, out, p->signal_elems, B, w, s))) return rc;
+    S2W_CUDA_CHECK(cudaPeekAtLastError());
+    return S2W_OK;
+}
+
+// ---- transform drivers (ball, Alg. 2) -----------------------------------------------------------------
+// workspace: flm_sh [P][Mfull][L] (per-shell harmonic coefficients), flmp [P][Mfull][L] (f_{lmp}), F.
+struct BallWork {
+    cplx *flm_sh, *flmp, *F;
+};
+static BallWork carve_ball(const s2w_plan *p, void *work)
+{
+    BallWork w;
+    const size_t sh = ((p->ws_shell_elems + 15) / 16) * 16;
+    w.flm_sh = (cplx *)work;
+    w.flmp = w.flm_sh + sh;
+    w.F = w.flmp + sh;
+    return w;
+}
+
+static int ball_forward(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s)
+{
+    const BallWork bw = carve_ball(p, work);
+    Work w;
+    w.flmT = bw.flm_sh;
+    w.F = bw.F;
+    const int P = p->P, L = p->L;
+    const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
+    const size_t cols = (size_t)(p->real ? L : 2 * L - 1) * L;
+    const size_t shell = (size_t)L * (2 * L - 1);
+    int rc;
+    // Z: per-shell spherical harmonic transform, then the radial quadrature (Eq. 10)
+    if ((rc = sht_forward_dev(p, p->sht, in, shell, P, w, true, s))) return rc;
+    if ((rc = launch_radial(p->Kfull_fwd, P, P, bw.flm_sh, bw.flmp, cols, L, 0, 0, false, s))) return rc;
+    // scaling coefficients: Phi f, Z^-1 at full resolution (Eq. 35; R9)
+    if ((rc = launch_radial(p->Kfull_inv, P, P, bw.flmp, bw.flm_sh, cols, L, p->phi_ball, 0, false, s))) return rc;
+    if ((rc = sht_inverse_dev(p, p->sht, (char *)out + p->scaling_offset * esz, shell, P, w, s))) return rc;
+    // wavelet coefficients: per radial scale j' one inverse Laguerre contraction onto the P_j' grid, then the sphere's
+    // scale stage on each of its shells for every angular scale j (Eqs. 33, 43-44)
+    size_t i = 0;
+    while (i < p->scales.size()) {
+        const Scale &first = p->scales[i];
+        if ((rc = launch_radial(first.Kinv, first.Pj, first.Pj, bw.flmp, bw.flm_sh, cols, L, 0, 0, false, s))) return rc;
+        for (; i < p->scales.size() && p->scales[i].jp == first.jp; ++i) {
+            const Scale &sc = p->scales[i];
+            const size_t stride = (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1);
+            if ((rc = scale_analysis(p, sc, sc.Pj, w, (char *)out + sc.offset * esz, stride, s))) return rc;
+        }
+    }
+    S2W_CUDA_CHECK(cudaPeekAtLastError());
+    return S2W_OK;
+}
+
+static int ball_inverse(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s)
+{
+    const BallWork bw = carve_ball(p, work);
+    Work w;
+    w.flmT = bw.flm_sh;
+    w.F = bw.F;
+    const int P = p->P, L = p->L;
+    const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
+    const size_t Mfull = p->real ? L : 2 * L - 1;
+    const size_t cols = Mfull * L;
+    const size_t shell = (size_t)L * (2 * L - 1);
+    int rc;
+    // scaling part: Z W^Phi, times Phi (Eq. 46)
+    if ((rc = sht_forward_dev(p, p->sht, (const char *)in + p->scaling_offset * esz, shell, P, w, true, s))) return rc;
+    if ((rc = launch_radial(p->Kfull_fwd, P, P, bw.flm_sh, bw.flmp, cols, L, 0, p->phi_ball, false, s))) return rc;
+    // wavelet part: per j' sum the angular scales shell by shell, then the radial quadrature on the P_j' grid
+    size_t i = 0;
+    while (i < p->scales.size()) {
+        const Scale &first = p->scales[i];
+        S2W_CUDA_CHECK(cudaMemsetAsync(bw.flm_sh, 0, (size_t)first.Pj * cols * sizeof(cplx), s));
+        for (; i < p->scales.size() && p->scales[i].jp == first.jp; ++i) {
+            const Scale &sc = p->scales[i];
+            const size_t stride = (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1);
+            if ((rc = scale_synthesis(p, sc, sc.Pj, w, (const char *)in + sc.offset * esz, stride, s))) return rc;
+        }
+        if ((rc = launch_radial(first.Kfwd, first.Pj, first.Pj, bw.flm_sh, bw.flmp, cols, L, 0, 0, true, s))) return rc;
+    }
+    // Z^-1
+    if ((rc = launch_radial(p->Kfull_inv, P, P, bw.flmp, bw.flm_sh, cols, L, 0, 0, false, s))) return rc;
+    if ((rc = sht_inverse_dev(p, p->sht, out, shell, P, w, s))) return rc;
     S2W_CUDA_CHECK(cudaPeekAtLastError());
     return S2W_OK;
 }
@@ -721,37 +913,7 @@ int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int m
         sc.Lj = scale_bandlimit(j, L, lambda, p->multires);
         sc.offset = off;
         off += (size_t)nn * sc.Lj * (2 * sc.Lj - 1);
-        S2W_PLAN_TRY(build_grid(p, sc.Lj));
-        Stage &st = sc.st;
-        st.grid = grid_index(p, sc.Lj);
-        st.Lg = sc.Lj;
-        const double *kj = &kappa[(size_t)(j - J0) * L];
-        st.lmin = sc.Lj;
-        for (int l = 0; l < sc.Lj; ++l)
-            if (kj[l] != 0.0) {
-                st.lmin = l;
-                break;
-            }
-        std::vector<int> ns, rows;
-        for (int ni = 0; ni < N; ++ni) {
-            int n = -(N - 1) + 2 * ni;
-            if (std::abs(n) < sc.Lj) {
-                ns.push_back(n);
-                rows.push_back(ni);
-            }
-        }
-        S2W_PLAN_TRY(fill_stage_rows(p, st, ns, rows, N));
-        std::vector<cplx> fa((size_t)st.nn * sc.Lj), fs((size_t)st.nn * sc.Lj);
-        const double syn_norm = 4.0 * pi * pi / (2.0 * sc.Lj - 1.0);
-        for (int q = 0; q < st.nn; ++q)
-            for (int l = 0; l < sc.Lj; ++l) {
-                const double pre = std::sqrt((2.0 * l + 1.0) / (8.0 * pi * pi)) * kj[l];
-                const size_t zo = ((size_t)l * nn + (st.n_val[q] + N - 1)) * 2;
-                const double re = pre * zeta[zo], im = pre * zeta[zo + 1];
-                fa[(size_t)q * sc.Lj + l] = cmake(re, -im);                        // conj(Psi)   (Eq. 40)
-                fs[(size_t)q * sc.Lj + l] = cmake(re * syn_norm, im * syn_norm);   // Psi (2pi)^2/n_a  (Eq. 42)
-            }
-        S2W_PLAN_TRY(make_stage_filters(p, st, fa, fs));
+        S2W_PLAN_TRY(make_scale_stage(p, sc, &kappa[(size_t)(j - J0) * L], zeta));
         maxF = std::max(maxF, (size_t)N * sc.Lj * (p->real ? sc.Lj : 2 * sc.Lj - 1));
         p->scales.push_back(sc);
     }
@@ -768,9 +930,145 @@ int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int m
 int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, double lambda_p, int J0, double tau,
                        int flags, int device)
 {
-    (void)out; (void)L; (void)P; (void)N; (void)lambda_l; (void)lambda_p; (void)J0; (void)tau; (void)flags; (void)device;
-    set_error("ball plans are not implemented yet");
-    return S2W_EUNSUPPORTED;
+    if (!out) {
+        set_error("null plan pointer");
+        return S2W_EINVAL;
+    }
+    *out = 0;
+    int rc = check_params(L, N, lambda_l, J0);
+    if (rc) return rc;
+    if (P < 1 || !(lambda_p > 1.0) || !(tau > 0.0) || J0 > scale_count(P, lambda_p)) {
+        set_error("invalid argument: need P >= 1, lambda_p > 1, tau > 0, J0 <= J'");
+        return S2W_EINVAL;
+    }
+    if (flags & S2W_PRECOMPUTE) {
+        set_error("S2W_PRECOMPUTE is not available for ball plans");
+        return S2W_EUNSUPPORTED;
+    }
+    if (L > 2048) {
+        set_error("L > 2048 is not supported");
+        return S2W_EUNSUPPORTED;
+    }
+    S2W_CUDA_CHECK(cudaSetDevice(device));
+    s2w_plan *p = new s2w_plan();
+    p->kind = 1;
+    p->L = L;
+    p->N = N;
+    p->P = P;
+    p->lambda = lambda_l;
+    p->nu = lambda_p;
+    p->tau = tau;
+    p->J0 = J0;
+    p->J = scale_count(L, lambda_l);
+    p->J0p = J0;
+    p->Jp = scale_count(P, lambda_p);
+    p->multires = 1;
+    p->flags = flags;
+    p->batch = 1;
+    p->device = device;
+    p->real = (flags & S2W_REAL) != 0;
+    p->Kfull_fwd = p->Kfull_inv = 0;
+    p->phi_ball = 0;
+    S2W_PLAN_TRY(plan_common(p));
+
+    const double pi = pi_d();
+    std::vector<double> kl, kscl, kp, kscp, zeta;
+    kappa_profiles(L, lambda_l, J0, p->J, kl, kscl);
+    kappa_profiles(P, lambda_p, J0, p->Jp, kp, kscp);
+    zeta_tiling(L, N, zeta);
+    const int nn = 2 * N - 1;
+    {
+        std::vector<double> a(L), s(L);
+        for (int l = 0; l < L; ++l) {
+            a[l] = std::sqrt((2.0 * l + 1.0) / (4.0 * pi));
+            s[l] = a[l] * 2.0 * pi / (2.0 * L - 1.0);
+        }
+        S2W_PLAN_TRY(make_n0_stage(p, p->sht, L, a, s));
+    }
+    p->scaling = p->sht;
+    p->Ls = L;  // the scaling function is non-zero on the cross {l small} u {p small}: full resolution (R9)
+    // radial matrices on the full P-node grid
+    {
+        std::vector<double> x, qw, K;
+        gauss_laguerre2(P, x, qw);
+        if ((int)x.size() != P) {
+            set_error("Gauss-Laguerre root search failed");
+            s2w_plan_destroy(p);
+            return S2W_EUNSUPPORTED;
+        }
+        laguerre_basis(P, x, tau, K);  // K[p][i]
+        const double t3 = tau * tau * tau;
+        std::vector<double> fwd((size_t)P * P), inv((size_t)P * P), phi((size_t)P * L);
+        for (int pp = 0; pp < P; ++pp)
+            for (int i = 0; i < P; ++i) {
+                fwd[(size_t)pp * P + i] = t3 * qw[i] * K[(size_t)pp * P + i];
+                inv[(size_t)i * P + pp] = K[(size_t)pp * P + i];
+            }
+        for (int pp = 0; pp < P; ++pp)
+            for (int l = 0; l < L; ++l) {
+                const double a = kscl[l], b = kscp[pp];
+                phi[(size_t)pp * L + l] = std::sqrt(a + b - a * b);  // sqrt(4pi/(2l+1)) Phi_{l0p}
+            }
+        S2W_PLAN_TRY(p->pool.upload(&p->Kfull_fwd, fwd));
+        S2W_PLAN_TRY(p->pool.upload(&p->Kfull_inv, inv));
+        S2W_PLAN_TRY(p->pool.upload(&p->phi_ball, phi));
+    }
+    size_t off = 0;
+    p->scaling_offset = 0;
+    off += (size_t)P * L * (2 * L - 1);
+    size_t maxF = (size_t)L * (p->real ? L : 2 * L - 1);
+    // angular stages, one per j (shared by all j')
+    std::vector<Scale> ang;
+    for (int j = J0; j <= p->J; ++j) {
+        Scale sc;
+        memset(&sc, 0, sizeof(sc));
+        sc.j = j;
+        sc.Lj = scale_bandlimit(j, L, lambda_l, true);
+        S2W_PLAN_TRY(make_scale_stage(p, sc, &kl[(size_t)(j - J0) * L], zeta));
+        maxF = std::max(maxF, (size_t)N * sc.Lj * (p->real ? sc.Lj : 2 * sc.Lj - 1));
+        ang.push_back(sc);
+    }
+    for (int jp = p->J0p; jp <= p->Jp; ++jp) {
+        const int Pj = scale_bandlimit(jp, P, lambda_p, true);
+        std::vector<double> x, qw, K;
+        gauss_laguerre2(Pj, x, qw);
+        if ((int)x.size() != Pj) {
+            set_error("Gauss-Laguerre root search failed");
+            s2w_plan_destroy(p);
+            return S2W_EUNSUPPORTED;
+        }
+        laguerre_basis(Pj, x, tau, K);  // K[p][i], p < Pj, on the Pj-node grid
+        const double t3 = tau * tau * tau;
+        const double *kj = &kp[(size_t)(jp - p->J0p) * P];
+        std::vector<double> kinv((size_t)Pj * Pj), kfwd((size_t)Pj * Pj);
+        for (int pp = 0; pp < Pj; ++pp)
+            for (int i = 0; i < Pj; ++i) {
+                kinv[(size_t)i * Pj + pp] = K[(size_t)pp * Pj + i] * kj[pp];
+                kfwd[(size_t)pp * Pj + i] = t3 * qw[i] * K[(size_t)pp * Pj + i] * kj[pp];
+            }
+        double *dKinv, *dKfwd;
+        S2W_PLAN_TRY(p->pool.upload(&dKinv, kinv));
+        S2W_PLAN_TRY(p->pool.upload(&dKfwd, kfwd));
+        for (size_t a = 0; a < ang.size(); ++a) {
+            Scale sc = ang[a];
+            sc.jp = jp;
+            sc.Pj = Pj;
+            sc.Kinv = dKinv;
+            sc.Kfwd = dKfwd;
+            sc.offset = off;
+            off += (size_t)Pj * nn * sc.Lj * (2 * sc.Lj - 1);
+            p->scales.push_back(sc);
+        }
+    }
+    p->coeff_elems = off;
+    p->signal_elems = (size_t)P * L * (2 * L - 1);
+    p->ws_shell_elems = (size_t)P * (p->real ? L : 2 * L - 1) * L;
+    p->ws_flm_elems = 2 * (((p->ws_shell_elems + 15) / 16) * 16);
+    p->ws_F_elems = (size_t)P * maxF;
+    p->ws_bytes = (p->ws_flm_elems + p->ws_F_elems) * sizeof(cplx) + 256;
+    S2W_PLAN_TRY(cudaDeviceSynchronize() == cudaSuccess ? S2W_OK : S2W_ECUDA);
+    *out = p;
+    return S2W_OK;
 }
 
 int s2w_plan_destroy(s2w_plan *p)
@@ -836,7 +1134,7 @@ int s2w_plan_forward(const s2w_plan *p, const void *in, void *out, void *work, v
         set_error("null pointer");
         return S2W_EINVAL;
     }
-    if (p->kind != 0) return S2W_EUNSUPPORTED;
+    if (p->kind == 1) return ball_forward(p, in, out, align256(work), (cudaStream_t)stream);
     return sphere_forward(p, in, out, align256(work), (cudaStream_t)stream);
 }
 
@@ -846,7 +1144,7 @@ int s2w_plan_inverse(const s2w_plan *p, const void *in, void *out, void *work, v
         set_error("null pointer");
         return S2W_EINVAL;
     }
-    if (p->kind != 0) return S2W_EUNSUPPORTED;
+    if (p->kind == 1) return ball_inverse(p, in, out, align256(work), (cudaStream_t)stream);
     return sphere_inverse(p, in, out, align256(work), (cudaStream_t)stream);
 }
 
@@ -856,13 +1154,22 @@ int s2w_plan_harmonic_forward(const s2w_plan *p, const void *f, void *flm, void 
         set_error("null pointer");
         return S2W_EINVAL;
     }
-    if (p->kind != 0) return S2W_EUNSUPPORTED;
-    const Work w = carve(p, align256(work));
     cudaStream_t s = (cudaStream_t)stream;
-    int rc = sht_forward_dev(p, p->sht, f, p->signal_elems, p->batch, w, true, s);
-    if (rc) return rc;
-    rc = launch_flm_unpack(w.flmT, (cplx *)flm, p->batch, p->L, p->real, s);
-    if (rc) return rc;
+    int rc;
+    if (p->kind == 1) {
+        const BallWork bw = carve_ball(p, align256(work));
+        Work w;
+        w.flmT = bw.flm_sh;
+        w.F = bw.F;
+        const size_t cols = (size_t)(p->real ? p->L : 2 * p->L - 1) * p->L;
+        if ((rc = sht_forward_dev(p, p->sht, f, (size_t)p->L * (2 * p->L - 1), p->P, w, true, s))) return rc;
+        if ((rc = launch_radial(p->Kfull_fwd, p->P, p->P, bw.flm_sh, bw.flmp, cols, p->L, 0, 0, false, s))) return rc;
+        if ((rc = launch_flm_unpack(bw.flmp, (cplx *)flm, p->P, p->L, p->real, s))) return rc;
+    } else {
+        const Work w = carve(p, align256(work));
+        if ((rc = sht_forward_dev(p, p->sht, f, p->signal_elems, p->batch, w, true, s))) return rc;
+        if ((rc = launch_flm_unpack(w.flmT, (cplx *)flm, p->batch, p->L, p->real, s))) return rc;
+    }
     S2W_CUDA_CHECK(cudaPeekAtLastError());
     return S2W_OK;
 }
@@ -873,13 +1180,22 @@ int s2w_plan_harmonic_inverse(const s2w_plan *p, const void *flm, void *f, void 
         set_error("null pointer");
         return S2W_EINVAL;
     }
-    if (p->kind != 0) return S2W_EUNSUPPORTED;
-    const Work w = carve(p, align256(work));
     cudaStream_t s = (cudaStream_t)stream;
-    int rc = launch_flm_pack((const cplx *)flm, w.flmT, p->batch, p->L, p->real, s);
-    if (rc) return rc;
-    rc = sht_inverse_dev(p, p->sht, f, p->signal_elems, p->batch, w, s);
-    if (rc) return rc;
+    int rc;
+    if (p->kind == 1) {
+        const BallWork bw = carve_ball(p, align256(work));
+        Work w;
+        w.flmT = bw.flm_sh;
+        w.F = bw.F;
+        const size_t cols = (size_t)(p->real ? p->L : 2 * p->L - 1) * p->L;
+        if ((rc = launch_flm_pack((const cplx *)flm, bw.flmp, p->P, p->L, p->real, s))) return rc;
+        if ((rc = launch_radial(p->Kfull_inv, p->P, p->P, bw.flmp, bw.flm_sh, cols, p->L, 0, 0, false, s))) return rc;
+        if ((rc = sht_inverse_dev(p, p->sht, f, (size_t)p->L * (2 * p->L - 1), p->P, w, s))) return rc;
+    } else {
+        const Work w = carve(p, align256(work));
+        if ((rc = launch_flm_pack((const cplx *)flm, w.flmT, p->batch, p->L, p->real, s))) return rc;
+        if ((rc = sht_inverse_dev(p, p->sht, f, p->signal_elems, p->batch, w, s))) return rc;
+    }
     S2W_CUDA_CHECK(cudaPeekAtLastError());
     return S2W_OK;
 }
@@ -901,14 +1217,16 @@ struct CacheEntry {
 std::map<CacheKey, CacheEntry> g_cache;
 std::mutex g_cache_mu;
 
-int cached_sphere(int L, int N, double lambda, int J0, int multires, int flags, int batch, CacheEntry *e)
+int cached_plan(int kind, int L, int P, int N, double lambda, double nu, double tau, int J0, int multires, int flags,
+                int batch, CacheEntry *e)
 {
     int device = 0;
     S2W_CUDA_CHECK(cudaGetDevice(&device));
     CacheKey k;
     std::memset(&k, 0, sizeof(k));
-    k.kind = 0;
+    k.kind = kind;
     k.L = L;
+    k.P = P;
     k.N = N;
     k.J0 = J0;
     k.multires = multires ? 1 : 0;
@@ -916,13 +1234,16 @@ int cached_sphere(int L, int N, double lambda, int J0, int multires, int flags, 
     k.batch = batch;
     k.device = device;
     k.lam = lambda;
+    k.nu = nu;
+    k.tau = tau;
     std::lock_guard<std::mutex> lock(g_cache_mu);
     auto it = g_cache.find(k);
     if (it == g_cache.end()) {
         CacheEntry ne;
         ne.plan = 0;
         ne.work = 0;
-        int rc = s2wav_plan_create(&ne.plan, L, N, lambda, J0, multires, flags, batch, device);
+        int rc = kind == 0 ? s2wav_plan_create(&ne.plan, L, N, lambda, J0, multires, flags, batch, device)
+                           : s2ball_plan_create(&ne.plan, L, P, N, lambda, nu, J0, tau, flags, device);
         if (rc) return rc;
         cudaError_t ce = cudaMalloc(&ne.work, s2w_plan_workspace_bytes(ne.plan));
         if (ce != cudaSuccess) {
@@ -936,38 +1257,16 @@ int cached_sphere(int L, int N, double lambda, int J0, int multires, int flags, 
     *e = it->second;
     return S2W_OK;
 }
-}  // namespace
 
-int s2wav_forward(const void *f, void *w, int L, int N, double lambda, int J0, int multires, int flags, int batch,
-                  void *stream)
-{
-    CacheEntry e;
-    int rc = cached_sphere(L, N, lambda, J0, multires, flags, batch, &e);
-    if (rc) return rc;
-    return s2w_plan_forward(e.plan, f, w, e.work, stream);
-}
-
-int s2wav_inverse(const void *w, void *f, int L, int N, double lambda, int J0, int multires, int flags, int batch,
-                  void *stream)
-{
-    CacheEntry e;
-    int rc = cached_sphere(L, N, lambda, J0, multires, flags, batch, &e);
-    if (rc) return rc;
-    return s2w_plan_inverse(e.plan, w, f, e.work, stream);
-}
-
-static int host_roundtrip(bool fwd, const void *in_h, void *out_h, int L, int N, double lambda, int J0, int multires,
-                          int flags, int batch)
+// host-buffer variant of a cached transform: copy in, transform, copy out, synchronise
+int host_transform(bool fwd, const CacheEntry &e, const void *in_h, void *out_h)
 {
     if (!in_h || !out_h) {
         set_error("null pointer");
         return S2W_EINVAL;
     }
-    CacheEntry e;
-    int rc = cached_sphere(L, N, lambda, J0, multires, flags, batch, &e);
-    if (rc) return rc;
-    const size_t esz = (flags & S2W_REAL) ? sizeof(double) : sizeof(cplx);
-    const size_t sig = e.plan->signal_elems * batch * esz, cof = e.plan->coeff_elems * batch * esz;
+    const size_t esz = e.plan->real ? sizeof(double) : sizeof(cplx);
+    const size_t sig = e.plan->signal_elems * e.plan->batch * esz, cof = e.plan->coeff_elems * e.plan->batch * esz;
     void *d_in = 0, *d_out = 0;
     S2W_CUDA_CHECK(cudaMalloc(&d_in, fwd ? sig : cof));
     cudaError_t ce = cudaMalloc(&d_out, fwd ? cof : sig);
@@ -976,7 +1275,7 @@ static int host_roundtrip(bool fwd, const void *in_h, void *out_h, int L, int N,
         set_error("cudaMalloc failed");
         return S2W_ENOMEM;
     }
-    rc = S2W_OK;
+    int rc = S2W_OK;
     if (cudaMemcpyAsync(d_in, in_h, fwd ? sig : cof, cudaMemcpyHostToDevice, 0) != cudaSuccess) rc = S2W_ECUDA;
     if (!rc) rc = fwd ? s2w_plan_forward(e.plan, d_in, d_out, e.work, 0) : s2w_plan_inverse(e.plan, d_in, d_out, e.work, 0);
     if (!rc && cudaMemcpyAsync(out_h, d_out, fwd ? cof : sig, cudaMemcpyDeviceToHost, 0) != cudaSuccess) rc = S2W_ECUDA;
@@ -988,44 +1287,73 @@ static int host_roundtrip(bool fwd, const void *in_h, void *out_h, int L, int N,
     cudaFree(d_out);
     return rc;
 }
+}  // namespace
+
+int s2wav_forward(const void *f, void *w, int L, int N, double lambda, int J0, int multires, int flags, int batch,
+                  void *stream)
+{
+    CacheEntry e;
+    int rc = cached_plan(0, L, 1, N, lambda, 0.0, 1.0, J0, multires, flags, batch, &e);
+    if (rc) return rc;
+    return s2w_plan_forward(e.plan, f, w, e.work, stream);
+}
+
+int s2wav_inverse(const void *w, void *f, int L, int N, double lambda, int J0, int multires, int flags, int batch,
+                  void *stream)
+{
+    CacheEntry e;
+    int rc = cached_plan(0, L, 1, N, lambda, 0.0, 1.0, J0, multires, flags, batch, &e);
+    if (rc) return rc;
+    return s2w_plan_inverse(e.plan, w, f, e.work, stream);
+}
 
 int s2wav_forward_host(const void *f, void *w, int L, int N, double lambda, int J0, int multires, int flags, int batch)
 {
-    return host_roundtrip(true, f, w, L, N, lambda, J0, multires, flags, batch);
+    CacheEntry e;
+    int rc = cached_plan(0, L, 1, N, lambda, 0.0, 1.0, J0, multires, flags, batch, &e);
+    if (rc) return rc;
+    return host_transform(true, e, f, w);
 }
 int s2wav_inverse_host(const void *w, void *f, int L, int N, double lambda, int J0, int multires, int flags, int batch)
 {
-    return host_roundtrip(false, w, f, L, N, lambda, J0, multires, flags, batch);
+    CacheEntry e;
+    int rc = cached_plan(0, L, 1, N, lambda, 0.0, 1.0, J0, multires, flags, batch, &e);
+    if (rc) return rc;
+    return host_transform(false, e, w, f);
 }
 
 int s2ball_forward(const void *f, void *w, int L, int P, int N, double lambda_l, double lambda_p, int J0, double tau,
                    int flags, void *stream)
 {
-    (void)f; (void)w; (void)L; (void)P; (void)N; (void)lambda_l; (void)lambda_p; (void)J0; (void)tau; (void)flags; (void)stream;
-    set_error("ball transforms are not implemented yet");
-    return S2W_EUNSUPPORTED;
+    CacheEntry e;
+    int rc = cached_plan(1, L, P, N, lambda_l, lambda_p, tau, J0, 1, flags, 1, &e);
+    if (rc) return rc;
+    return s2w_plan_forward(e.plan, f, w, e.work, stream);
 }
 int s2ball_inverse(const void *w, void *f, int L, int P, int N, double lambda_l, double lambda_p, int J0, double tau,
                    int flags, void *stream)
 {
-    (void)f; (void)w; (void)L; (void)P; (void)N; (void)lambda_l; (void)lambda_p; (void)J0; (void)tau; (void)flags; (void)stream;
-    set_error("ball transforms are not implemented yet");
-    return S2W_EUNSUPPORTED;
+    CacheEntry e;
+    int rc = cached_plan(1, L, P, N, lambda_l, lambda_p, tau, J0, 1, flags, 1, &e);
+    if (rc) return rc;
+    return s2w_plan_inverse(e.plan, w, f, e.work, stream);
 }
 
 int s2ball_forward_host(const void *f, void *w, int L, int P, int N, double lambda_l, double lambda_p, int J0,
                         double tau, int flags)
 {
-    (void)f; (void)w; (void)L; (void)P; (void)N; (void)lambda_l; (void)lambda_p; (void)J0; (void)tau; (void)flags;
-    set_error("ball transforms are not implemented yet");
-    return S2W_EUNSUPPORTED;
+    CacheEntry e;
+    int rc = cached_plan(1, L, P, N, lambda_l, lambda_p, tau, J0, 1, flags, 1, &e);
+    if (rc) return rc;
+    return host_transform(true, e, f, w);
 }
 int s2ball_inverse_host(const void *w, void *f, int L, int P, int N, double lambda_l, double lambda_p, int J0,
                         double tau, int flags)
 {
-    (void)f; (void)w; (void)L; (void)P; (void)N; (void)lambda_l; (void)lambda_p; (void)J0; (void)tau; (void)flags;
-    set_error("ball transforms are not implemented yet");
-    return S2W_EUNSUPPORTED;
+    CacheEntry e;
+    int rc = cached_plan(1, L, P, N, lambda_l, lambda_p, tau, J0, 1, flags, 1, &e);
+    if (rc) return rc;
+    return host_transform(false, e, w, f);
 }
 
 int s2w_cache_clear(void)

@@ -4,17 +4,28 @@
 //   inverse direction (a5, a7):  F_mn(beta_t) = sum_l d^l_mn(beta_t) G_n(l) f_lm                     (Eq. 5/47)
 //   forward direction (a3, a6):  f_lm += G'_n(l) sum_t d^l_mn(beta_t) h_mn(beta_t)                   (Eq. 4/48)
 //
-// d^l_mn(beta) is generated by the three-term recursion in l (Varshalovich et al., cited P:434)
+// d^l_mn(beta) follows the three-term recursion in l (Varshalovich et al., cited P:434)
 //   d^{l+1} = (alpha_l cos(beta) - beta_l) d^l - gamma_l d^{l-1},
 //   alpha_l = (l+1)(2l+1)/sqrt(((l+1)^2-m^2)((l+1)^2-n^2)),  beta_l = alpha_l m n/(l(l+1)),
 //   gamma_l = alpha_l sqrt((l^2-m^2)(l^2-n^2))/(l(2l+1)),
-// with one thread owning R theta rings: the recursion state never leaves registers, the coefficients of the current
-// l-tile are broadcast from shared memory, and one recursion step is shared by all NC real columns (signals x
-// re/im x {(m,n), (-m,-n)}) of the block: d^l_{-m,-n} = (-1)^{m+n} d^l_{mn}.
+// evaluated in DIFFERENCE FORM.  Near the poles consecutive d^l are nearly equal (north) or nearly opposite (south),
+// and the plain recursion doubles-integrates its rounding errors (error ~ l^1.5 eps: 1e-11 at l = 1000).
+// With y = 1 - |cos beta| and, for southern rings, the mirrored sequence d~^l = (-1)^l d^l (which obeys the same
+// recursion with cos(beta) -> -cos(beta), beta_l -> -beta_l):
+//   u_l = gamma_l u_{l-1} + (e - alpha_l y) d~^l,      d~^{l+1} = d~^l + u_l,
+//   e = e_N = alpha_l - gamma_l - 1 - beta_l (north),  e = e_S = alpha_l - gamma_l - 1 + beta_l (south),
+// where e_N, e_S are tabulated from long double (they vanish exactly where d is constant in l) and y carries the
+// angle with full relative precision.  4 FP64 operations per step, shared by all columns of the block.
 //
-// Rings start late: `lstart` holds, per (n, m, t), the first l at which |d^l_mn(beta_t)| has grown to 2^-90 and
-// `dseed` the pair (d^{lstart}, d^{lstart-1}) there (computed once per plan by wigner_ramp_kernel in range-extended
-// arithmetic), so the exponentially small start of the recursion is neither computed nor able to underflow.
+// Rings are processed in groups of 32 (a warp, one lane per ring): each hemisphere's rings sorted by |cos beta|,
+// group 2j = north rings 32j.., group 2j+1 = south rings 32j...  A group starts at the first degree at which any of
+// its rings has reached |d| >= 2^-90 (the exponentially small start of the recursion is neither computed nor able to
+// underflow); the start is warp-uniform and monotone in j, so a warp that owns groups j0 < j1 < ... runs phases with
+// 1, 2, ... active groups and no per-step checks.  Even warps own north groups, odd warps south groups.
+//
+// Inverse direction: DFMA, accumulators in registers.  Forward direction: the sum over rings is done by the FP64
+// tensor pipe (mma.sync.m8n8k4.f64: D[col][l] += h^T[col][ring] d[ring][l]), the d values of an l-octet passing
+// through a warp-private shared-memory transpose.
 #include <climits>
 
 #include "kernels.h"
@@ -29,80 +40,91 @@ namespace {
 
 __device__ __forceinline__ size_t tri_off(int m, int Lfull) { return (size_t)m * Lfull - ((size_t)m * (m - 1)) / 2 - m; }
 
-// ---------------------------------------------------------------------------------------------------------------
-// plan-time: recursion coefficients, packed rows l = m..L-1 for every m >= 0 and every table value of n
-// ---------------------------------------------------------------------------------------------------------------
 struct NList {
     int v[S2W_MAX_ROWS];
 };
 
-__global__ void wigner_coef_kernel(double *coef, int L, size_t tri, NList nl)
+// one recursion step l -> l+1 (see the header): ag = (alpha_l, gamma_l), e = e_N or e_S
+__device__ __forceinline__ void wig_step(double &d, double &u, double y, double alpha, double gamma, double e)
 {
-    const int m = blockIdx.y, n = nl.v[blockIdx.z];
-    const int l = m + blockIdx.x * blockDim.x + threadIdx.x;
-    if (l >= L) return;
-    double *o = coef + ((size_t)blockIdx.z * tri + tri_off(m, L) + l) * 3;
-    const int an = n < 0 ? -n : n;
-    double a = 0.0, b = 0.0, g = 0.0;
-    if (l >= an) {
-        if (l == 0) {
-            a = 1.0;
-        } else {
-            const double lp = (double)(l + 1), ld = (double)l, md = (double)m, nd = (double)n;
-            a = lp * (2.0 * ld + 1.0) / sqrt((lp * lp - md * md) * (lp * lp - nd * nd));
-            b = a * md * nd / (ld * lp);
-            g = a * sqrt((ld * ld - md * md) * (ld * ld - nd * nd)) / (ld * (2.0 * ld + 1.0));
-        }
-    }
-    o[0] = a;
-    o[1] = b;
-    o[2] = g;
+    const double eps = fma(-alpha, y, e);
+    u = fma(gamma, u, eps * d);
+    d += u;
 }
 
-// plan-time: from the range-extended seed d^{l0}_{mn}(beta_t) = mant * 2^expo run the recursion until the value reaches
-// 2^RAMP_THRESHOLD_EXP; store that degree and the two values there.  One thread per (n, m, t).
-__global__ void wigner_ramp_kernel(const double *__restrict__ mant, const int *__restrict__ expo,
-                                   const double *__restrict__ coef, size_t tri, int Lfull, int Lg, NList nl,
-                                   const double *__restrict__ xcos, int *__restrict__ lstart,
-                                   double2 *__restrict__ dseed)
+// ---------------------------------------------------------------------------------------------------------------
+// plan-time: group start degrees and seeds.  One warp per (group, m, table n); lane = ring slot.
+//   pass 0: every ring runs the range-extended recursion from its seed d^{l0} = mant 2^expo until |d| >= 2^-90;
+//           the group start is the minimum over the warp.
+//   fix   : suffix minimum over the groups of a hemisphere (monotone starts).
+//   pass 1: every ring runs to the group start and stores (d~, u~) there.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(32) wigner_seed_kernel(const double *__restrict__ mant, const int *__restrict__ expo,
+                                                        const double *__restrict__ coef, size_t tri, int Lfull, int Lg,
+                                                        int G, NList nl, const double *__restrict__ yv,
+                                                        const int *__restrict__ ring, int *__restrict__ gstart,
+                                                        double2 *__restrict__ dseed, int pass)
 {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    const int m = blockIdx.y, tab = blockIdx.z;
-    if (t >= Lg) return;
+    const int g = blockIdx.x, m = blockIdx.y, tab = blockIdx.z, lane = threadIdx.x;
+    const int k = g * 32 + lane;
+    const int t = ring[k];
     const int n = nl.v[tab], an = n < 0 ? -n : n;
     const int l0 = m > an ? m : an;
-    const size_t idx = ((size_t)tab * Lg + m) * Lg + t;
-    if (l0 >= Lg) {
-        lstart[idx] = Lg;
-        dseed[idx] = make_double2(0.0, 0.0);
-        return;
+    const bool south = (g & 1) != 0;
+    const size_t gidx = ((size_t)tab * Lg + m) * G + g;
+    const int target = pass == 0 ? Lg : gstart[gidx];
+    double d = 0.0, u = 0.0;
+    int e = 0, l = l0;
+    if (t >= 0 && l0 < Lg) {
+        const size_t idx = ((size_t)tab * Lg + m) * Lg + t;
+        d = mant[idx];
+        if (south && (l0 & 1)) d = -d;
+        u = d;
+        e = expo[idx];
     }
-    const double *c = coef + ((size_t)tab * tri + tri_off(m, Lfull)) * 3;
-    const double x = xcos[t];
-    double d0 = mant[idx], dm1 = 0.0;
-    int e = expo[idx];
-    int l = l0;
-    if (d0 == 0.0) l = Lg;
-    while (l < Lg) {
-        if (e + ilogb(d0) >= RAMP_THRESHOLD_EXP) break;
-        double a = c[3 * (size_t)l], b = c[3 * (size_t)l + 1], g = c[3 * (size_t)l + 2];
-        double dn = fma(a, x, -b) * d0;
-        dn = fma(-g, dm1, dn);
-        dm1 = d0;
-        d0 = dn;
-        ++l;
-        if (fabs(d0) > 0x1p300) {
-            d0 *= 0x1p-300;
-            dm1 *= 0x1p-300;
-            e += 300;
+    int ls = Lg;
+    if (d != 0.0) {
+        const double *c = coef + ((size_t)tab * tri + tri_off(m, Lfull)) * 4;
+        const double y = yv[k];
+        while (l < target) {
+            if (pass == 0 && e + ilogb(d) >= RAMP_THRESHOLD_EXP) break;
+            const double4 q = *reinterpret_cast<const double4 *>(c + 4 * (size_t)l);
+            wig_step(d, u, y, q.x, q.y, south ? q.w : q.z);
+            ++l;
+            if (fabs(d) > 0x1p300 || fabs(u) > 0x1p300) {
+                d *= 0x1p-300;
+                u *= 0x1p-300;
+                e += 300;
+            }
         }
+        if (d != 0.0) ls = l;
     }
-    if (l >= Lg) {
-        lstart[idx] = Lg;
-        dseed[idx] = make_double2(0.0, 0.0);
+    if (pass == 0) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const int other = __shfl_xor_sync(0xffffffffu, ls, o);
+            ls = other < ls ? other : ls;
+        }
+        if (lane == 0) gstart[gidx] = ls;
     } else {
-        lstart[idx] = l;
-        dseed[idx] = make_double2(ldexp(d0, e), ldexp(dm1, e));
+        double2 s = make_double2(0.0, 0.0);
+        if (target < Lg && d != 0.0) s = make_double2(ldexp(d, e), ldexp(u, e));
+        dseed[((size_t)tab * Lg + m) * (size_t)(32 * G) + k] = s;
+    }
+}
+
+__global__ void wigner_start_fix_kernel(int *__restrict__ gstart, int G, int count)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    int *gs = gstart + (size_t)i * G;
+    for (int hemi = 0; hemi < 2; ++hemi) {
+        int run = INT_MAX;
+        for (int j = G / 2 - 1; j >= 0; --j) {
+            const int v = gs[2 * j + hemi];
+            run = v < run ? v : run;
+            gs[2 * j + hemi] = run;
+        }
     }
 }
 
@@ -124,28 +146,82 @@ __device__ __forceinline__ ColInfo col_info(const WigArgs &A, int cc)
     return c;
 }
 
+// stage the recursion coefficients of degrees lt..lt+TL-1 of row (m, tab): s_ag = (alpha, gamma), s_e = (e_N, e_S)
+template <int TL>
+__device__ __forceinline__ void stage_coef(const double *__restrict__ crow, int lt, int l0, int Lg, double2 *s_ag,
+                                           double2 *s_e)
+{
+    for (int i = threadIdx.x; i < TL; i += blockDim.x) {
+        const int l = lt + i;
+        double4 q = make_double4(0.0, 0.0, 0.0, 0.0);
+        if (l >= l0 && l < Lg) q = *reinterpret_cast<const double4 *>(crow + 4 * (size_t)l);
+        s_ag[i] = make_double2(q.x, q.y);
+        s_e[i] = make_double2(q.z, q.w);
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------------
-// inverse direction: one block per (m >= 0, column chunk); thread owns R rings; loops over the n of the launch
+// inverse direction: one block per (m >= 0, column chunk) covering all rings; warp w owns groups w, w+W, w+2W, ...
+// (slot r = group r W + w), lane = ring.  Loops over the n of the launch.
 // ---------------------------------------------------------------------------------------------------------------
+template <int NC, int R, int RA, bool ACC>
+__device__ __forceinline__ void inv_range(int la, int lb, int lt, int hemi, const double2 *s_ag, const double2 *s_e,
+                                          const double *s_X, const double (&y)[R], double (&d)[R], double (&u)[R],
+                                          double (&acc)[R][NC])
+{
+    const double *se = reinterpret_cast<const double *>(s_e) + hemi;
+    for (int l = la; l < lb; ++l) {
+        const int i = l - lt;
+        const double2 ag = s_ag[i];
+        const double e = se[2 * i];
+        double xv[NC];
+        if (ACC) {
+#pragma unroll
+            for (int c = 0; c < NC; ++c) xv[c] = s_X[i * NC + c];
+        }
+#pragma unroll
+        for (int r = 0; r < RA; ++r) {
+            if (ACC) {
+#pragma unroll
+                for (int c = 0; c < NC; ++c) acc[r][c] = fma(d[r], xv[c], acc[r][c]);
+            }
+            wig_step(d[r], u[r], y[r], ag.x, ag.y, e);
+        }
+    }
+}
+
+template <int NC, int R, bool ACC>
+__device__ __forceinline__ void inv_dispatch(int ra, int la, int lb, int lt, int hemi, const double2 *s_ag,
+                                             const double2 *s_e, const double *s_X, const double (&y)[R],
+                                             double (&d)[R], double (&u)[R], double (&acc)[R][NC])
+{
+    if (R >= 4 && ra == 4) return inv_range<NC, R, (R >= 4 ? 4 : R), ACC>(la, lb, lt, hemi, s_ag, s_e, s_X, y, d, u, acc);
+    if (R >= 3 && ra == 3) return inv_range<NC, R, (R >= 3 ? 3 : R), ACC>(la, lb, lt, hemi, s_ag, s_e, s_X, y, d, u, acc);
+    if (R >= 2 && ra == 2) return inv_range<NC, R, (R >= 2 ? 2 : R), ACC>(la, lb, lt, hemi, s_ag, s_e, s_X, y, d, u, acc);
+    if (ra >= 1) return inv_range<NC, R, 1, ACC>(la, lb, lt, hemi, s_ag, s_e, s_X, y, d, u, acc);
+}
+
 template <int NC, int R, int MAXT>
 __global__ void __launch_bounds__(MAXT) wigner_inverse_kernel(WigArgs A)
 {
-    __shared__ double2 s_ab[WIG_TL];
-    __shared__ double s_g[WIG_TL];
-    __shared__ double s_X[WIG_TL * NC];
+    __shared__ double2 s_ag[WIG_TL];
+    __shared__ double2 s_e[WIG_TL];
+    __shared__ double s_X[2][WIG_TL * NC];  // [0]: X_l, [1]: (-1)^l X_l (southern warps)
 
     const int m = blockIdx.x, chunk = blockIdx.y;
-    const int Lg = A.Lg, Lfull = A.Lfull;
+    const int Lg = A.Lg, Lfull = A.Lfull, G = A.G;
     const int Md = A.isReal ? Lg : 2 * Lg - 1;
     const int Mfull = A.isReal ? Lfull : 2 * Lfull - 1;
-    const int T = blockDim.x;
+    const int T = blockDim.x, W = T >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, hemi = warp & 1;
 
     int tr[R];
-    double x[R];
+    double y[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        tr[r] = threadIdx.x + r * T;
-        x[r] = tr[r] < Lg ? A.xcos[tr[r]] : 0.0;
+        const int g = r * W + warp;
+        tr[r] = g < G ? A.ring[g * 32 + lane] : -1;
+        y[r] = g < G ? A.yv[g * 32 + lane] : 0.0;
     }
 
     for (int q = 0; q < A.nn; ++q) {
@@ -153,108 +229,81 @@ __global__ void __launch_bounds__(MAXT) wigner_inverse_kernel(WigArgs A)
         const int l0 = m > an ? m : an;
         if (l0 >= Lg) continue;
         const int tab = A.n_tab[q];
-        const double *crow = A.coef + ((size_t)tab * A.tri + tri_off(m, Lfull)) * 3;
-        const size_t sbase = ((size_t)tab * Lg + m) * Lg;
+        const double *crow = A.coef + ((size_t)tab * A.tri + tri_off(m, Lfull)) * 4;
+        const int *gsrow = A.gstart + ((size_t)tab * Lg + m) * G;
+        const double2 *seedrow = A.dseed + ((size_t)tab * Lg + m) * (size_t)(32 * G);
         const double sgn = ((m + n) & 1) ? -1.0 : 1.0;
         const int lacc = l0 > A.lmin ? l0 : A.lmin;  // first l that contributes
 
-        int ls[R];
-        int wls = INT_MAX;
-        double d0[R], dm1[R], acc[R][NC];
+        int gs[R + 1];
+        double d[R], u[R], acc[R][NC];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            ls[r] = tr[r] < Lg ? A.lstart[sbase + tr[r]] : INT_MAX;
-            wls = ls[r] < wls ? ls[r] : wls;
-            d0[r] = 0.0;
-            dm1[r] = 0.0;
+            const int g = r * W + warp;
+            gs[r] = g < G ? gsrow[g] : INT_MAX;
+            d[r] = 0.0;
+            u[r] = 0.0;
 #pragma unroll
             for (int c = 0; c < NC; ++c) acc[r][c] = 0.0;
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            int other = __shfl_xor_sync(0xffffffffu, wls, o);
-            wls = other < wls ? other : wls;
-        }
+        gs[R] = INT_MAX;
+        // first degree any group of the block needs: groups 0 and 1 start first
+        int bmin = gsrow[0];
+        if (G > 1 && gsrow[1] < bmin) bmin = gsrow[1];
+        if (bmin < l0) bmin = l0;
 
-        for (int lt = l0 & ~(WIG_TL - 1); lt < Lg; lt += WIG_TL) {
+        for (int lt = bmin & ~(WIG_TL - 1); lt < Lg; lt += WIG_TL) {
             __syncthreads();
-            for (int i = threadIdx.x; i < WIG_TL; i += T) {
-                const int l = lt + i;
-                double2 ab = make_double2(0.0, 0.0);
-                double g = 0.0;
-                if (l >= l0 && l < Lg) {
-                    ab = make_double2(crow[3 * (size_t)l], crow[3 * (size_t)l + 1]);
-                    g = crow[3 * (size_t)l + 2];
-                }
-                s_ab[i] = ab;
-                s_g[i] = g;
-            }
+            stage_coef<WIG_TL>(crow, lt, l0, Lg, s_ag, s_e);
             for (int i = threadIdx.x; i < WIG_TL * (NC / 2); i += T) {
-                const int ll = i / (NC / 2), k = i % (NC / 2);
+                const int k = i / WIG_TL, ll = i % WIG_TL;  // consecutive threads -> consecutive l (coalesced)
                 const int l = lt + ll;
                 const ColInfo ci = col_info(A, chunk * (NC / 2) + k);
                 cplx X = cmake(0.0, 0.0);
                 if (l >= lacc && l < Lg && ci.valid) {
                     const int mi = A.isReal ? m : (ci.minus ? Lfull - 1 - m : Lfull - 1 + m);
                     const cplx f = A.flmT[((size_t)ci.b * Mfull + mi) * Lfull + l];
-                    const cplx G = A.filt[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
-                    X = cmul(G, f);
+                    const cplx Gf = A.filt[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
+                    X = cmul(Gf, f);
                     if (ci.minus) X = cscale(X, sgn);
                 }
-                s_X[ll * NC + 2 * k] = X.x;
-                s_X[ll * NC + 2 * k + 1] = X.y;
+                const double alt = (l & 1) ? -1.0 : 1.0;
+                s_X[0][ll * NC + 2 * k] = X.x;
+                s_X[0][ll * NC + 2 * k + 1] = X.y;
+                s_X[1][ll * NC + 2 * k] = alt * X.x;
+                s_X[1][ll * NC + 2 * k + 1] = alt * X.y;
             }
             __syncthreads();
 
-            int la = lt > wls ? lt : wls;
             const int lb = (lt + WIG_TL) < Lg ? (lt + WIG_TL) : Lg;
-            int lmid = lacc > la ? lacc : la;
-            lmid = lmid < lb ? lmid : lb;
-            // recursion only (no filter support yet)
-            for (int l = la; l < lmid; ++l) {
-                const double2 ab = s_ab[l - lt];
-                const double g = s_g[l - lt];
+            int l = lt > gs[0] ? lt : gs[0];
+            while (l < lb) {
+                int ra = 0;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    if (l == ls[r]) {
-                        const double2 s = A.dseed[sbase + tr[r]];
-                        d0[r] = s.x;
-                        dm1[r] = s.y;
+                    if (gs[r] <= l) ++ra;
+                    if (gs[r] == l) {  // group r starts here (warp-uniform)
+                        const double2 s = seedrow[(r * W + warp) * 32 + lane];
+                        d[r] = s.x;
+                        u[r] = s.y;
                     }
-                    double dn = fma(ab.x, x[r], -ab.y) * d0[r];
-                    dn = fma(-g, dm1[r], dn);
-                    dm1[r] = d0[r];
-                    d0[r] = dn;
                 }
-            }
-            // accumulate + recursion
-            for (int l = lmid; l < lb; ++l) {
-                const double2 ab = s_ab[l - lt];
-                const double g = s_g[l - lt];
-                double xv[NC];
+                int le = lb;
 #pragma unroll
-                for (int c = 0; c < NC; ++c) xv[c] = s_X[(l - lt) * NC + c];
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    if (l == ls[r]) {
-                        const double2 s = A.dseed[sbase + tr[r]];
-                        d0[r] = s.x;
-                        dm1[r] = s.y;
-                    }
-#pragma unroll
-                    for (int c = 0; c < NC; ++c) acc[r][c] = fma(d0[r], xv[c], acc[r][c]);
-                    double dn = fma(ab.x, x[r], -ab.y) * d0[r];
-                    dn = fma(-g, dm1[r], dn);
-                    dm1[r] = d0[r];
-                    d0[r] = dn;
-                }
+                for (int r = 0; r < R; ++r)
+                    if (gs[r] > l && gs[r] < le) le = gs[r];
+                // recursion only below the filter support, then accumulate + recursion
+                const int lmid = lacc < l ? l : (lacc < le ? lacc : le);
+                if (l < lmid) inv_dispatch<NC, R, false>(ra, l, lmid, lt, hemi, s_ag, s_e, s_X[hemi], y, d, u, acc);
+                if (lmid < le) inv_dispatch<NC, R, true>(ra, lmid, le, lt, hemi, s_ag, s_e, s_X[hemi], y, d, u, acc);
+                l = le;
             }
         }
 
         // store F_{m,n}(t) and (complex signals) F_{-m,-n}(t)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            if (tr[r] >= Lg) continue;
+            if (tr[r] < 0) continue;
 #pragma unroll
             for (int k = 0; k < NC / 2; ++k) {
                 const ColInfo ci = col_info(A, chunk * (NC / 2) + k);
@@ -269,218 +318,179 @@ __global__ void __launch_bounds__(MAXT) wigner_inverse_kernel(WigArgs A)
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// forward direction: one block per (m >= 0, column chunk) covering ALL rings; per l the partial sums over a thread's
-// rings are reduced over the warp with a halving shuffle, over the warps through shared memory, then multiplied by
-// the output filter and added to f_lm.
+// forward direction: one block per (m >= 0, chunk of 4 complex = 8 real columns) covering ALL rings.
+// Per l-octet every active group (warp, slot) runs 8 recursion steps, writing d~ into a warp-private shared-memory
+// tile laid out as eight 4-ring x 8-degree B-fragments; the tensor pipe then accumulates
+//     D[col][l] += sum_{ring} hT[col][ring] d~[ring][l]          (mma.sync.m8n8k4.f64, 8 per group and octet)
+// with hT (the ring data, constant over l) held in registers as A-fragments.  Per l-tile the warps' partial sums meet
+// in shared memory (southern warps with the sign (-1)^l that turns d~ back into d), are multiplied by the output
+// filter and added to f_lm with one red.global.add.f64 per value (each address is touched once per launch).
 // ---------------------------------------------------------------------------------------------------------------
-// column whose warp total ends up in `lane` after warp_reduce_cols (lanes with (lane & (32/NC - 1)) == 0 write)
-template <int NC>
-__device__ __forceinline__ int lane_col(int lane)
+#define FWD_QS 36                 // doubles per 4-ring fragment row block (32 + 4 pad: conflict-free transposed stores)
+#define FWD_GT (8 * FWD_QS)       // doubles per group tile
+
+__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b)
 {
-    if (NC == 8) return ((lane & 16) ? 4 : 0) + ((lane & 8) ? 2 : 0) + ((lane & 4) ? 1 : 0);
-    if (NC == 4) return ((lane & 16) ? 2 : 0) + ((lane & 8) ? 1 : 0);
-    return (lane & 16) ? 1 : 0;
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
 }
 
-template <int NC>
-__device__ __forceinline__ double warp_reduce_cols(double (&p)[NC], int lane, int &col)
-{
-    double v;
-    if (NC == 8) {
-        bool hi = (lane & 16) != 0;
-        double q4[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            double send = hi ? p[i] : p[i + 4], keep = hi ? p[i + 4] : p[i];
-            q4[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-        }
-        hi = (lane & 8) != 0;
-        double q2[2];
-#pragma unroll
-        for (int i = 0; i < 2; ++i) {
-            double send = hi ? q4[i] : q4[i + 2], keep = hi ? q4[i + 2] : q4[i];
-            q2[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-        }
-        hi = (lane & 4) != 0;
-        double send = hi ? q2[0] : q2[1], keep = hi ? q2[1] : q2[0];
-        v = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-        v += __shfl_xor_sync(0xffffffffu, v, 2);
-        v += __shfl_xor_sync(0xffffffffu, v, 1);
-    } else if (NC == 4) {
-        bool hi = (lane & 16) != 0;
-        double q2[2];
-#pragma unroll
-        for (int i = 0; i < 2; ++i) {
-            double send = hi ? p[i] : p[i + 2], keep = hi ? p[i + 2] : p[i];
-            q2[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-        }
-        hi = (lane & 8) != 0;
-        double send = hi ? q2[0] : q2[1], keep = hi ? q2[1] : q2[0];
-        v = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-        v += __shfl_xor_sync(0xffffffffu, v, 4);
-        v += __shfl_xor_sync(0xffffffffu, v, 2);
-        v += __shfl_xor_sync(0xffffffffu, v, 1);
-    } else {
-        bool hi = (lane & 16) != 0;
-        double send = hi ? p[0] : p[1], keep = hi ? p[1] : p[0];
-        v = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-        v += __shfl_xor_sync(0xffffffffu, v, 8);
-        v += __shfl_xor_sync(0xffffffffu, v, 4);
-        v += __shfl_xor_sync(0xffffffffu, v, 2);
-        v += __shfl_xor_sync(0xffffffffu, v, 1);
-    }
-    col = lane_col<NC>(lane);
-    return v;
-}
-
-template <int NC, int R, int MAXT>
+template <int R, int MAXT>
 __global__ void __launch_bounds__(MAXT) wigner_forward_kernel(WigArgs A)
 {
+    constexpr int NC = 8;
     constexpr int NW = MAXT / 32;
-    constexpr int WRITER_MASK = 32 / NC - 1;
-    __shared__ double2 s_ab[WIG_TLF];
-    __shared__ double s_g[WIG_TLF];
-    __shared__ double s_red[WIG_TLF][NW][NC];
+    __shared__ double2 s_ag[WIG_TLF];
+    __shared__ double2 s_e[WIG_TLF];
+    __shared__ double s_red[NW][WIG_TLF][NC];
+    extern __shared__ double s_dt[];  // [W][R][FWD_GT]
 
     const int m = blockIdx.x, chunk = blockIdx.y;
-    const int Lg = A.Lg, Lfull = A.Lfull;
+    const int Lg = A.Lg, Lfull = A.Lfull, G = A.G;
     const int Md = A.isReal ? Lg : 2 * Lg - 1;
     const int Mfull = A.isReal ? Lfull : 2 * Lfull - 1;
-    const int T = blockDim.x;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = T >> 5;
+    const int T = blockDim.x, W = T >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, hemi = warp & 1;
+    double *dt = s_dt + (size_t)warp * R * FWD_GT;
+    const int wr_off = (lane >> 2) * FWD_QS + (lane & 3);  // + 4 * (l & 7): store slot of this lane's ring
 
-    int tr[R];
-    double x[R];
+    double y[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        tr[r] = threadIdx.x + r * T;
-        x[r] = tr[r] < Lg ? A.xcos[tr[r]] : 0.0;
+        const int g = r * W + warp;
+        y[r] = g < G ? A.yv[g * 32 + lane] : 0.0;
     }
+    // A-fragment coordinates of this lane: column c = lane / 4, ring quad member lane % 4
+    const int fc = lane >> 2, fk = lane & 3;
+    const ColInfo fci = col_info(A, chunk * (NC / 2) + (fc >> 1));
 
     for (int q = 0; q < A.nn; ++q) {
         const int n = A.n_val[q], an = n < 0 ? -n : n;
         const int l0 = m > an ? m : an;
         if (l0 >= Lg) continue;
         const int tab = A.n_tab[q];
-        const double *crow = A.coef + ((size_t)tab * A.tri + tri_off(m, Lfull)) * 3;
-        const size_t sbase = ((size_t)tab * Lg + m) * Lg;
+        const double *crow = A.coef + ((size_t)tab * A.tri + tri_off(m, Lfull)) * 4;
+        const int *gsrow = A.gstart + ((size_t)tab * Lg + m) * G;
+        const double2 *seedrow = A.dseed + ((size_t)tab * Lg + m) * (size_t)(32 * G);
         const double sgn = ((m + n) & 1) ? -1.0 : 1.0;
         const int lacc = l0 > A.lmin ? l0 : A.lmin;
 
-        int ls[R];
-        int wls = INT_MAX;
-        double d0[R], dm1[R], h[R][NC];
+        // ring data as A-fragments: hA[r][quad] = h[ring (r, quad, fk)][column fc]
+        int gs[R];
+        double d[R], u[R], hA[R][8];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            ls[r] = tr[r] < Lg ? A.lstart[sbase + tr[r]] : INT_MAX;
-            wls = ls[r] < wls ? ls[r] : wls;
-            d0[r] = 0.0;
-            dm1[r] = 0.0;
+            const int g = r * W + warp;
+            gs[r] = g < G ? gsrow[g] : INT_MAX;
+            d[r] = 0.0;
+            u[r] = 0.0;
 #pragma unroll
-            for (int k = 0; k < NC / 2; ++k) {
-                const ColInfo ci = col_info(A, chunk * (NC / 2) + k);
-                cplx v = cmake(0.0, 0.0);
-                if (ci.valid && tr[r] < Lg) {
-                    const int row = ci.minus ? A.n_rowm[q] : A.n_row[q];
-                    const int mi = A.isReal ? m : (ci.minus ? Lg - 1 - m : Lg - 1 + m);
-                    v = A.F[(((size_t)ci.b * A.nrows + row) * Lg + tr[r]) * Md + mi];
-                    if (ci.minus) v = cscale(v, sgn);
+            for (int qd = 0; qd < 8; ++qd) {
+                double v = 0.0;
+                const int t = g < G ? A.ring[g * 32 + qd * 4 + fk] : -1;
+                if (t >= 0 && fci.valid) {
+                    const int row = fci.minus ? A.n_rowm[q] : A.n_row[q];
+                    const int mi = A.isReal ? m : (fci.minus ? Lg - 1 - m : Lg - 1 + m);
+                    const cplx hv = A.F[(((size_t)fci.b * A.nrows + row) * Lg + t) * Md + mi];
+                    v = (fc & 1) ? hv.y : hv.x;
+                    if (fci.minus) v *= sgn;
                 }
-                h[r][2 * k] = v.x;
-                h[r][2 * k + 1] = v.y;
+                hA[r][qd] = v;
             }
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            int other = __shfl_xor_sync(0xffffffffu, wls, o);
-            wls = other < wls ? other : wls;
-        }
+        // tiles start at the first group start; tiles wholly below the filter support run the recursion only
+        int first = gsrow[0];
+        if (G > 1 && gsrow[1] < first) first = gsrow[1];
+        if (first < l0) first = l0;
 
-        for (int lt = l0 & ~(WIG_TLF - 1); lt < Lg; lt += WIG_TLF) {
+        for (int lt = first & ~(WIG_TLF - 1); lt < Lg; lt += WIG_TLF) {
             __syncthreads();
-            for (int i = threadIdx.x; i < WIG_TLF; i += T) {
-                const int l = lt + i;
-                double2 ab = make_double2(0.0, 0.0);
-                double g = 0.0;
-                if (l >= l0 && l < Lg) {
-                    ab = make_double2(crow[3 * (size_t)l], crow[3 * (size_t)l + 1]);
-                    g = crow[3 * (size_t)l + 2];
-                }
-                s_ab[i] = ab;
-                s_g[i] = g;
-            }
+            stage_coef<WIG_TLF>(crow, lt, l0, Lg, s_ag, s_e);
             __syncthreads();
-
-            const int lb = (lt + WIG_TLF) < Lg ? (lt + WIG_TLF) : Lg;
-            int la = lt > wls ? lt : wls;
-            la = la < lb ? la : lb;
-            int lmid = lacc > la ? lacc : la;
-            lmid = lmid < lb ? lmid : lb;
-            // degrees of this tile that need an output but at which this warp is still inactive: contribute zero
-            if ((lane & WRITER_MASK) == 0) {
-                const int wcol = lane_col<NC>(lane);
-                const int lz0 = lacc > lt ? lacc : lt;
-                for (int l = lz0; l < la; ++l) s_red[l - lt][warp][wcol] = 0.0;
-            }
-            for (int l = la; l < lmid; ++l) {
-                const double2 ab = s_ab[l - lt];
-                const double g = s_g[l - lt];
+            const bool want = lt + WIG_TLF > lacc;  // this tile has outputs
+            const double *se = reinterpret_cast<const double *>(s_e) + hemi;
+#pragma unroll 1
+            for (int oc = 0; oc < WIG_TLF / 8; ++oc) {
+                const int lo = lt + 8 * oc;
+                double c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
+                if (gs[0] < lo + 8 && lo < Lg) {
+                    const bool mm = want && (lo + 8 > lacc);
 #pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    if (l == ls[r]) {
-                        const double2 s = A.dseed[sbase + tr[r]];
-                        d0[r] = s.x;
-                        dm1[r] = s.y;
+                    for (int r = 0; r < R; ++r) {
+                        if (gs[r] >= lo + 8) continue;  // warp-uniform
+                        double *dst = dt + r * FWD_GT + wr_off;
+                        if (gs[r] >= lo) {  // the group starts inside this octet
+#pragma unroll
+                            for (int s = 0; s < 8; ++s) {
+                                if (gs[r] == lo + s) {
+                                    const double2 sd = seedrow[(r * W + warp) * 32 + lane];
+                                    d[r] = sd.x;
+                                    u[r] = sd.y;
+                                }
+                                dst[4 * s] = d[r];
+                                const double2 ag = s_ag[8 * oc + s];
+                                wig_step(d[r], u[r], y[r], ag.x, ag.y, se[2 * (8 * oc + s)]);
+                            }
+                        } else {
+#pragma unroll
+                            for (int s = 0; s < 8; ++s) {
+                                dst[4 * s] = d[r];
+                                const double2 ag = s_ag[8 * oc + s];
+                                wig_step(d[r], u[r], y[r], ag.x, ag.y, se[2 * (8 * oc + s)]);
+                            }
+                        }
                     }
-                    double dn = fma(ab.x, x[r], -ab.y) * d0[r];
-                    dn = fma(-g, dm1[r], dn);
-                    dm1[r] = d0[r];
-                    d0[r] = dn;
+                    if (mm) {
+                        __syncwarp();
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            if (gs[r] >= lo + 8) continue;
+                            const double *src = dt + r * FWD_GT + lane;
+#pragma unroll
+                            for (int qd = 0; qd < 8; qd += 2) {
+                                dmma884(c0, c1, hA[r][qd], src[qd * FWD_QS]);
+                                dmma884(c2, c3, hA[r][qd + 1], src[(qd + 1) * FWD_QS]);
+                            }
+                        }
+                        __syncwarp();
+                    }
+                }
+                // D fragment: row (column index) lane / 4, degrees 2 (lane % 4) + {0, 1} of the octet
+                if (want) {
+                    s_red[warp][8 * oc + 2 * fk][fc] = c0 + c2;
+                    s_red[warp][8 * oc + 2 * fk + 1][fc] = c1 + c3;
                 }
             }
-            for (int l = lmid; l < lb; ++l) {
-                const double2 ab = s_ab[l - lt];
-                const double g = s_g[l - lt];
-                double p[NC];
-#pragma unroll
-                for (int c = 0; c < NC; ++c) p[c] = 0.0;
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    if (l == ls[r]) {
-                        const double2 s = A.dseed[sbase + tr[r]];
-                        d0[r] = s.x;
-                        dm1[r] = s.y;
-                    }
-#pragma unroll
-                    for (int c = 0; c < NC; ++c) p[c] = fma(d0[r], h[r][c], p[c]);
-                    double dn = fma(ab.x, x[r], -ab.y) * d0[r];
-                    dn = fma(-g, dm1[r], dn);
-                    dm1[r] = d0[r];
-                    d0[r] = dn;
-                }
-                int col;
-                const double v = warp_reduce_cols<NC>(p, lane, col);
-                if ((lane & WRITER_MASK) == 0) s_red[l - lt][warp][col] = v;
-            }
+            if (!want) continue;
             __syncthreads();
             // cross-warp sum, output filter, accumulate into f_lm
             for (int i = threadIdx.x; i < WIG_TLF * (NC / 2); i += T) {
-                const int ll = i / (NC / 2), k = i % (NC / 2);
+                const int k = i / WIG_TLF, ll = i % WIG_TLF;
                 const int l = lt + ll;
                 const ColInfo ci = col_info(A, chunk * (NC / 2) + k);
                 if (l < lacc || l >= Lg || !ci.valid) continue;
                 if (ci.minus && m == 0) continue;
-                double re = 0.0, im = 0.0;
-                for (int w = 0; w < nw; ++w) {
-                    re += s_red[ll][w][2 * k];
-                    im += s_red[ll][w][2 * k + 1];
+                double re = 0.0, im = 0.0, reS = 0.0, imS = 0.0;
+                for (int w = 0; w < W; w += 2) {
+                    re += s_red[w][ll][2 * k];
+                    im += s_red[w][ll][2 * k + 1];
+                    reS += s_red[w + 1][ll][2 * k];
+                    imS += s_red[w + 1][ll][2 * k + 1];
                 }
-                const cplx G = A.filt[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
-                const cplx val = cmul(G, cmake(re, im));
+                if (l & 1) {
+                    re -= reS;
+                    im -= imS;
+                } else {
+                    re += reS;
+                    im += imS;
+                }
+                const cplx Gf = A.filt[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
+                const cplx val = cmul(Gf, cmake(re, im));
                 const int mi = A.isReal ? m : (ci.minus ? Lfull - 1 - m : Lfull - 1 + m);
-                cplx *dst = &A.flmT[((size_t)ci.b * Mfull + mi) * Lfull + l];
-                const cplx old = *dst;
-                *dst = cadd(old, val);
+                double *dst = reinterpret_cast<double *>(&A.flmT[((size_t)ci.b * Mfull + mi) * Lfull + l]);
+                atomicAdd(dst, val.x);
+                atomicAdd(dst + 1, val.y);
             }
         }
     }
@@ -551,16 +561,25 @@ __global__ void __launch_bounds__(256) dmma_probe_kernel(double *out, int iters,
     double fa = a + threadIdx.x * 1e-9, fb = b;
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                         : "+d"(c[i][0]), "+d"(c[i][1])
-                         : "d"(fa), "d"(fb));
-        }
+        for (int i = 0; i < 4; ++i) dmma884(c[i][0], c[i][1], fa, fb);
     }
     double s = 0.0;
 #pragma unroll
     for (int i = 0; i < 4; ++i) s += c[i][0] + c[i][1];
     if (s == 123.456) out[0] = s;
+}
+
+// block shape for a grid with G ring groups: W warps (even), R groups per warp
+struct WigCfg {
+    int R, W, MAXT;
+};
+bool wig_cfg(int G, WigCfg &c)
+{
+    if (G < 2 || (G & 1) || G > 64) return false;
+    c.W = G <= 8 ? G : (G <= 32 ? 8 : 16);
+    c.R = (G + c.W - 1) / c.W;
+    c.MAXT = c.W <= 8 ? 256 : 512;
+    return c.R <= 4;
 }
 
 template <int NC, int R, int MAXT>
@@ -569,58 +588,53 @@ void launch_inv_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
     dim3 grid(A.Lg, chunks);
     S2W_LAUNCH_C(S2W_K_WIGNER_INV, (wigner_inverse_kernel<NC, R, MAXT>), grid, T, 0, st, A);
 }
-template <int NC, int R, int MAXT>
-void launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
-{
-    dim3 grid(A.Lg, chunks);
-    S2W_LAUNCH_C(S2W_K_WIGNER_FWD, (wigner_forward_kernel<NC, R, MAXT>), grid, T, 0, st, A);
-}
 
-struct WigCfg {
-    int R, T, MAXT;
-};
-WigCfg wig_cfg(int Lg)
+template <int R, int MAXT>
+int launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
 {
-    WigCfg c;
-    if (Lg <= 256) {
-        c.R = 1;
-        c.T = ((Lg + 31) / 32) * 32;
-        c.MAXT = 256;
-    } else if (Lg <= 512) {
-        c.R = 2;
-        c.T = 256;
-        c.MAXT = 256;
-    } else if (Lg <= 1024) {
-        c.R = 4;
-        c.T = 256;
-        c.MAXT = 256;
-    } else {
-        c.R = 4;
-        c.T = 512;
-        c.MAXT = 512;
+    const size_t smem = (size_t)(T / 32) * R * FWD_GT * sizeof(double);
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(wigner_forward_kernel<R, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)((size_t)(MAXT / 32) * R * FWD_GT * sizeof(double)));
+        if (e != cudaSuccess) {
+            set_error(std::string("cudaFuncSetAttribute(wigner_forward_kernel): ") + cudaGetErrorString(e));
+            return S2W_ECUDA;
+        }
+        configured = true;
     }
-    return c;
+    dim3 grid(A.Lg, chunks);
+    S2W_LAUNCH_C(S2W_K_WIGNER_FWD, (wigner_forward_kernel<R, MAXT>), grid, T, smem, st, A);
+    return S2W_OK;
 }
 
 template <int NC>
-int dispatch(bool fwd, const WigArgs &A, int chunks, cudaStream_t st)
+int dispatch_inv(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t st)
 {
-    const WigCfg c = wig_cfg(A.Lg);
-    if (A.Lg > 2048) {
-        set_error("band-limits above 2048 are not supported by the on-the-fly Wigner kernels");
-        return S2W_EUNSUPPORTED;
-    }
-#define S2W_WIG_CASE(RR, MT)                                        \
-    if (c.R == RR && c.MAXT == MT) {                                \
-        if (fwd)                                                    \
-            launch_fwd_t<NC, RR, MT>(A, c.T, chunks, st);           \
-        else                                                        \
-            launch_inv_t<NC, RR, MT>(A, c.T, chunks, st);           \
-        return S2W_OK;                                              \
+#define S2W_WIG_CASE(RR, MT)                              \
+    if (c.R == RR && c.MAXT == MT) {                      \
+        launch_inv_t<NC, RR, MT>(A, 32 * c.W, chunks, st); \
+        return S2W_OK;                                    \
     }
     S2W_WIG_CASE(1, 256)
     S2W_WIG_CASE(2, 256)
+    S2W_WIG_CASE(3, 256)
     S2W_WIG_CASE(4, 256)
+    S2W_WIG_CASE(3, 512)
+    S2W_WIG_CASE(4, 512)
+#undef S2W_WIG_CASE
+    return S2W_EINVAL;
+}
+
+int dispatch_fwd(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t st)
+{
+#define S2W_WIG_CASE(RR, MT) \
+    if (c.R == RR && c.MAXT == MT) return launch_fwd_t<RR, MT>(A, 32 * c.W, chunks, st);
+    S2W_WIG_CASE(1, 256)
+    S2W_WIG_CASE(2, 256)
+    S2W_WIG_CASE(3, 256)
+    S2W_WIG_CASE(4, 256)
+    S2W_WIG_CASE(3, 512)
     S2W_WIG_CASE(4, 512)
 #undef S2W_WIG_CASE
     return S2W_EINVAL;
@@ -629,31 +643,31 @@ int dispatch(bool fwd, const WigArgs &A, int chunks, cudaStream_t st)
 int launch_wigner(bool fwd, const WigArgs &A, cudaStream_t st)
 {
     if (A.nn <= 0 || A.Lg <= 0) return S2W_OK;
+    WigCfg c;
+    if (!wig_cfg(A.G, c)) {
+        set_error("band-limits above 2048 are not supported by the on-the-fly Wigner kernels");
+        return S2W_EUNSUPPORTED;
+    }
     const int CT = A.isReal ? A.B : 2 * A.B;
-    if (CT >= 3) return dispatch<8>(fwd, A, (CT + 3) / 4, st);
-    if (CT == 2) return dispatch<4>(fwd, A, 1, st);
-    return dispatch<2>(fwd, A, 1, st);
+    if (fwd) return dispatch_fwd(A, c, (CT + 3) / 4, st);
+    if (CT >= 3) return dispatch_inv<8>(A, c, (CT + 3) / 4, st);
+    if (CT == 2) return dispatch_inv<4>(A, c, 1, st);
+    return dispatch_inv<2>(A, c, 1, st);
 }
 
 }  // namespace
 
-int launch_wigner_coef(double *coef, int Lfull, const int *n_vals, int ntab, cudaStream_t st)
+int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int G,
+                        const int *n_vals, int ntab, const double *yv, const int *ring, int *gstart, double2 *dseed,
+                        cudaStream_t st)
 {
     NList nl;
     for (int i = 0; i < ntab; ++i) nl.v[i] = n_vals[i];
-    const size_t tri = (size_t)Lfull * (Lfull + 1) / 2;
-    dim3 grid((Lfull + 127) / 128, Lfull, ntab);
-    S2W_LAUNCH(wigner_coef_kernel, grid, 128, 0, st, coef, Lfull, tri, nl);
-    return S2W_OK;
-}
-
-int launch_wigner_ramp(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg,
-                       const int *n_vals, int ntab, const double *xcos, int *lstart, double2 *dseed, cudaStream_t st)
-{
-    NList nl;
-    for (int i = 0; i < ntab; ++i) nl.v[i] = n_vals[i];
-    dim3 grid((Lg + 127) / 128, Lg, ntab);
-    S2W_LAUNCH(wigner_ramp_kernel, grid, 128, 0, st, mant, expo, coef, tri, Lfull, Lg, nl, xcos, lstart, dseed);
+    dim3 grid(G, Lg, ntab);
+    S2W_LAUNCH(wigner_seed_kernel, grid, 32, 0, st, mant, expo, coef, tri, Lfull, Lg, G, nl, yv, ring, gstart, dseed, 0);
+    const int count = Lg * ntab;
+    S2W_LAUNCH(wigner_start_fix_kernel, (count + 127) / 128, 128, 0, st, gstart, G, count);
+    S2W_LAUNCH(wigner_seed_kernel, grid, 32, 0, st, mant, expo, coef, tri, Lfull, Lg, G, nl, yv, ring, gstart, dseed, 1);
     return S2W_OK;
 }
 

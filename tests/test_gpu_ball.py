@@ -1,0 +1,122 @@
+"""GPU parity tests of the ball (Fourier-Laguerre) wavelet transform: the CUDA path through the C ABI against the CPU
+oracle (oracle/ball.py), element by element on the same seeded inputs.  Tolerances: forward coefficients 1e-11
+relative max error per scale block, round trip 1e-12 (BASELINE.json, reading R12)."""
+import numpy as np
+import pytest
+
+from oracle import ball as OB
+from paper_2402_01282_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+FWD_TOL = 1e-11
+RT_TOL = 1e-12
+
+
+def _api():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2402_01282_b200 import api
+    return torch, api
+
+
+def _relmax(a, b):
+    den = np.abs(b).max()
+    num = np.abs(a - b).max()
+    return num if den == 0 else num / den
+
+
+def _voxels(L, P, tau, seed):
+    flmp = inputs.flmp_complex(L, P, seed)
+    f = OB.z_inverse(flmp, L, P, tau, "f80")
+    return flmp, np.ascontiguousarray(f.astype(np.complex128))
+
+
+@pytest.mark.parametrize("L,P,tau", [(8, 8, 1.0), (12, 5, 2.0), (33, 16, 1.0)])
+def test_spherical_laguerre_transform_matches_oracle(L, P, tau):
+    """Z and Z^-1 (Eqs. 10-11): per-shell SHT + radial Laguerre contraction (a10)."""
+    torch, api = _api()
+    flmp, f = _voxels(L, P, tau, 40 + L)
+    plan = api.s2ball_plan_create(L, P, 1, 2.0, 2.0, 0, tau)
+    got = plan.harmonic_forward(torch.from_numpy(f).cuda().reshape(1, -1), P * L * (2 * L - 1))
+    got = got.cpu().numpy().reshape(P, L, 2 * L - 1)
+    ref = OB.z_forward(f, L, P, tau, "f80").astype(np.complex128)
+    assert _relmax(got, ref) < FWD_TOL
+    assert _relmax(got, flmp) < FWD_TOL
+    back = plan.harmonic_inverse(torch.from_numpy(flmp).cuda().reshape(1, -1)).cpu().numpy().reshape(P, L, 2 * L - 1)
+    assert _relmax(back, f) < RT_TOL
+    plan.close()
+
+
+CASES = [
+    # L, P, N, lam_l, lam_p, J0, tau
+    (8, 8, 1, 2.0, 2.0, 0, 1.0),
+    (12, 8, 3, 2.0, 2.0, 0, 1.0),
+    (16, 6, 2, 2.0, 3.0, 1, 0.5),     # even N, P not a power of the dilation, J0 = 1, tau != 1
+    (20, 16, 3, 2.0, 2.0, 0, 1.0),
+]
+
+
+@pytest.mark.parametrize("L,P,N,lam,nu,J0,tau", CASES)
+def test_ball_forward_inverse_parity(L, P, N, lam, nu, J0, tau):
+    torch, api = _api()
+    flmp, f = _voxels(L, P, tau, 70 + L + N)
+    plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau)
+    fd = torch.from_numpy(f).cuda().reshape(1, -1)
+    w = plan.forward(fd)
+    scal, scales = plan.split(w)
+    filt = OB.filters(L, P, N, lam, nu, J0, J0, "f80")
+    o_phi, o_psi = OB.analysis(f, L, P, N, lam, nu, J0, J0, tau, "f80", filt)
+    assert _relmax(scal[0].cpu().numpy(), o_phi.astype(np.complex128)) < FWD_TOL
+    assert set(scales.keys()) == set(o_psi.keys())
+    for key, ref in o_psi.items():
+        got = scales[key][0].cpu().numpy()
+        assert got.shape == ref.shape, key
+        assert _relmax(got, ref.astype(np.complex128)) < FWD_TOL, key
+    back = plan.inverse(w).cpu().numpy().reshape(f.shape)
+    assert _relmax(back, f) < RT_TOL
+    # synthesis parity on the oracle's coefficients
+    o_f = OB.synthesis(o_phi, o_psi, L, P, N, lam, nu, J0, J0, tau, "f80", filt)
+    packed = np.zeros((1, plan.coeff_elems), dtype=np.complex128)
+    nr, ng, nt, npx, off = plan.scale_shape(-1)
+    packed[0, off:off + nr * nt * npx] = o_phi.astype(np.complex128).ravel()
+    for (j, jp), ref in o_psi.items():
+        nr, ng, nt, npx, off = plan.scale_shape(j, jp)
+        packed[0, off:off + nr * ng * nt * npx] = ref.astype(np.complex128).ravel()
+    back2 = plan.inverse(torch.from_numpy(packed).cuda()).cpu().numpy().reshape(f.shape)
+    assert _relmax(back2, o_f.astype(np.complex128)) < FWD_TOL
+    plan.close()
+
+
+def test_ball_argument_style_entry_points_and_host_path():
+    torch, api = _api()
+    L, P, N, lam, nu, J0, tau = 10, 4, 2, 2.0, 2.0, 0, 1.0
+    flmp, f = _voxels(L, P, tau, 9)
+    fd = torch.from_numpy(f).cuda()
+    w = api.s2ball_forward(fd, L, P, N, lam, nu, J0, tau)
+    back = api.s2ball_inverse(w, L, P, N, lam, nu, J0, tau)
+    assert _relmax(back.cpu().numpy(), f) < RT_TOL
+    wh = api.s2ball_forward_host(f, L, P, N, lam, nu, J0, tau)
+    assert np.allclose(wh, w.cpu().numpy(), rtol=0, atol=1e-13 * np.abs(wh).max())
+    fh = api.s2ball_inverse_host(wh, L, P, N, lam, nu, J0, tau)
+    assert _relmax(fh, f) < RT_TOL
+
+
+def test_ball_real_signal_gives_real_coefficients():
+    """A real field on the ball: S2W_REAL path (m >= 0 only) against the complex path."""
+    torch, api = _api()
+    L, P, N, lam, nu, J0, tau = 12, 6, 3, 2.0, 2.0, 0, 1.0
+    flm = np.stack([inputs.flm_real(L, 200 + p, 1)[0] / np.sqrt(p + 1.0) for p in range(P)])
+    f = OB.z_inverse(flm, L, P, tau, "f80")
+    assert np.abs(f.imag).max() < 1e-14 * np.abs(f).max()
+    fr = np.ascontiguousarray(f.real.astype(np.float64))
+    pr = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau, real=True)
+    pc = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau, real=False)
+    wr = pr.forward(torch.from_numpy(fr).cuda().reshape(1, -1)).cpu().numpy()
+    wc = pc.forward(torch.from_numpy(fr.astype(np.complex128)).cuda().reshape(1, -1)).cpu().numpy()
+    assert np.abs(wc.imag).max() < 1e-12 * np.abs(wc).max()
+    assert _relmax(wr, wc.real) < FWD_TOL
+    back = pr.inverse(torch.from_numpy(wr).cuda()).cpu().numpy().reshape(fr.shape)
+    assert _relmax(back, fr) < RT_TOL
+    pr.close()
+    pc.close()
