@@ -259,6 +259,30 @@ def workload_config(cfg, args):
 
 
 # ---------------------------------------------------------------------------------------------------------------
+# multi-GPU bookkeeping: replicas only -- every rank transforms its own batch of signals, there is
+# no data-path collective; the only exchange is this MAX over the ranks' device times.
+# ---------------------------------------------------------------------------------------------------------------
+def replica_seed_offset(rank):
+    """Rank r draws its signals from seed + 1000 r: independent signals per replica."""
+    return int(rank)
+
+
+def max_over_ranks(values, world, device):
+    """Element-wise MAX of a list of floats over all ranks (identity for world == 1)."""
+    import torch
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_value(world, batch_per_rank, steps, ms_max):
+    """transforms/s of the whole job: the units ALL ranks processed over the slowest rank's device time."""
+    return world * batch_per_rank * steps / (ms_max * 1e-3)
+
+
+# ---------------------------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------------------------
 def run_ours(args, cfg):
@@ -282,7 +306,7 @@ def run_ours(args, cfg):
         torch.cuda.synchronize()
 
     L, N, lam, J0, mr, real, B = cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"], cfg["real"], cfg["batch"]
-    f = make_signals(cfg, api, torch, device, seed_offset=rank)     # independent signals per replica
+    f = make_signals(cfg, api, torch, device, seed_offset=replica_seed_offset(rank))     # independent signals per replica
     plan = api.s2wav_plan_create(L, N, lam, J0, mr, real, B, local)
     cfg["coeff_gb"] = plan.coeff_elems * B * (8 if real else 16) / 1e9
     w = torch.empty((B, plan.coeff_elems), dtype=plan.dtype, device=device)
@@ -345,16 +369,13 @@ def run_ours(args, cfg):
                "rt_err": float(np.abs(fb - fh_np).max() / np.abs(fh_np).max())}
 
     # ---- max over ranks ----
-    tmax = torch.tensor([ms, e2e["dt"] if e2e else 0.0], dtype=torch.float64, device=device)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms, e2e_dt = float(tmax[0]), float(tmax[1])
+    ms, e2e_dt = max_over_ranks([ms, e2e["dt"] if e2e else 0.0], world, device)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    value = world * B * args.steps / (ms * 1e-3)
+    value = whole_job_value(world, B, args.steps, ms)
     tup, flops = contraction_flops_per_step(cfg, api)   # per class per step
     dom = max(("wigner_inverse", "wigner_forward"), key=lambda k: classes[k][0])
     dom_ms, dom_n = classes[dom]

@@ -65,7 +65,10 @@ int s2ball_radial_nodes(double *r, double *q, int P, double tau);
 
 /* ---- plans: the cached precomputed components ---- */
 
-/* flags: S2W_REAL (signal and coefficients real), S2W_PRECOMPUTE (reserved: returns S2W_EUNSUPPORTED).
+/* flags: S2W_REAL (signal and coefficients real); S2W_PRECOMPUTE: the Wigner-d values of every theta grid of the plan
+ * are tabulated in device memory at creation ("simply precomputed"; 8 B per (ring, m >= 0, l, n): 21.5 GB at
+ * L = 1024, N = 5) and the contractions stream that table through the FP64 tensor pipe instead of running the
+ * recursion; S2W_ENOMEM if the table does not fit.
  * batch = number of independent signals per call (>= 1).  device = CUDA device ordinal.
  * Creation allocates device tables, runs set-up kernels and synchronises. */
 int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int multiresolution,

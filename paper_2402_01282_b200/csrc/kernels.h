@@ -49,6 +49,8 @@ struct WigArgs {
     const double2 *dseed;       // [ntab][Lg (m)][32 G]: (d~^{gstart}, u~_{gstart-1}) per ring slot
     const double *yv;           // [32 G] 1 - |cos beta| per ring slot (0 for empty slots)
     const int *ring;            // [32 G] ring index t of the slot, -1 if empty
+    const double *dtab;         // precomputed-kernel variant: [ntab][tri_g][32 G] d^l_mn(beta) per ring slot, else null
+    size_t tri_g;               // Lg (Lg + 1) / 2
     const cplx *filt;           // [nn][Lg] filter applied to row q at degree l
     cplx *flmT;                 // [B][Mfull][Lfull]  f_{l m} stored m-major; Mfull = Lfull (real) or 2 Lfull - 1
     cplx *F;                    // [B][nrows][Lg][Md], Md = Lg (real) or 2 Lg - 1
@@ -73,6 +75,9 @@ int launch_reweight(cplx *F, const RwArgs &A, int batch, const FftTab &T, cudaSt
 // plan-time: group start degrees and seeds from the range-extended values d^{l0}_{mn}(beta_t) = mant 2^expo ([ntab][Lg m][Lg t])
 int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int G,
                         const int *n_vals, int ntab, const double *yv, const int *ring, int *gstart, double2 *dseed,
+                        cudaStream_t st);
+int launch_wigner_table(const double *coef, size_t tri, int Lfull, int Lg, int G, const int *n_vals, int ntab,
+                        const double *yv, const int *gstart, const double2 *dseed, double *dtab, size_t tri_g,
                         cudaStream_t st);
 int launch_radial(const double *A, int R, int K, const cplx *in, cplx *out, size_t cols, int Lfull, const double *win,
                   const double *wout, bool accumulate, cudaStream_t st);

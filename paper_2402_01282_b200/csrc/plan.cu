@@ -102,6 +102,7 @@ struct GridTab {  // everything that depends on the theta/phi grid of band-limit
     int *ring;       // [32 G] ring index t, -1 for an empty slot
     int *gstart;     // [ntab][Lg][G]
     double2 *dseed;  // [ntab][Lg][32 G]
+    double *dtab;    // S2W_PRECOMPUTE: [ntab][Lg (Lg+1)/2][32 G] d^l_mn(beta) per ring slot (else null)
 };
 
 struct Stage {  // one Wigner contraction launch: rows, filters
@@ -343,6 +344,19 @@ int build_grid(s2w_plan *p, int Lg)
         set_error(std::string("plan set-up kernels: ") + cudaGetErrorString(e));
         return S2W_ECUDA;
     }
+    if (p->flags & S2W_PRECOMPUTE) {
+        const size_t tri_g = (size_t)Lg * (Lg + 1) / 2;
+        const size_t elems = ntab * tri_g * (size_t)32 * g.G;
+        if ((rc = p->pool.alloc(&g.dtab, elems))) {
+            if (rc == S2W_ENOMEM) set_error("the precomputed Wigner-d table does not fit in device memory");
+            return rc;
+        }
+        S2W_CUDA_CHECK(cudaMemsetAsync(g.dtab, 0, elems * sizeof(double), 0));
+        if ((rc = launch_wigner_table(p->coef, p->tri, p->L, Lg, g.G, p->tabn.data(), (int)ntab, g.yv, g.gstart, g.dseed,
+                                      g.dtab, tri_g, 0)))
+            return rc;
+        S2W_CUDA_CHECK(cudaDeviceSynchronize());
+    }
     p->grids.push_back(g);
     return S2W_OK;
 }
@@ -394,6 +408,8 @@ void fill_wig_args(const s2w_plan *p, const Stage &st, bool synthesis, int B, cp
     A.dseed = g.dseed;
     A.yv = g.yv;
     A.ring = g.ring;
+    A.dtab = g.dtab;
+    A.tri_g = (size_t)st.Lg * (st.Lg + 1) / 2;
     A.filt = synthesis ? st.filt_syn : st.filt_ana;
     A.flmT = flmT;
     A.F = F;
@@ -838,10 +854,6 @@ int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int m
         set_error("invalid argument: batch < 1");
         return S2W_EINVAL;
     }
-    if (flags & S2W_PRECOMPUTE) {
-        set_error("S2W_PRECOMPUTE is not implemented yet");
-        return S2W_EUNSUPPORTED;
-    }
     if (L > 2048) {
         set_error("L > 2048 is not supported");
         return S2W_EUNSUPPORTED;
@@ -940,10 +952,6 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
     if (P < 1 || !(lambda_p > 1.0) || !(tau > 0.0) || J0 > scale_count(P, lambda_p)) {
         set_error("invalid argument: need P >= 1, lambda_p > 1, tau > 0, J0 <= J'");
         return S2W_EINVAL;
-    }
-    if (flags & S2W_PRECOMPUTE) {
-        set_error("S2W_PRECOMPUTE is not available for ball plans");
-        return S2W_EUNSUPPORTED;
     }
     if (L > 2048) {
         set_error("L > 2048 is not supported");

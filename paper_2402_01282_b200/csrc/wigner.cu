@@ -336,7 +336,7 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
                  : "d"(a), "d"(b));
 }
 
-template <int R, int MAXT>
+template <int R, int MAXT, bool PRE>
 __global__ void __launch_bounds__(MAXT) wigner_forward_kernel(WigArgs A)
 {
     constexpr int NC = 8;
@@ -406,15 +406,38 @@ __global__ void __launch_bounds__(MAXT) wigner_forward_kernel(WigArgs A)
 
         for (int lt = first & ~(WIG_TLF - 1); lt < Lg; lt += WIG_TLF) {
             __syncthreads();
-            stage_coef<WIG_TLF>(crow, lt, l0, Lg, s_ag, s_e);
-            __syncthreads();
+            if (!PRE) {
+                stage_coef<WIG_TLF>(crow, lt, l0, Lg, s_ag, s_e);
+                __syncthreads();
+            }
             const bool want = lt + WIG_TLF > lacc;  // this tile has outputs
             const double *se = reinterpret_cast<const double *>(s_e) + hemi;
 #pragma unroll 1
             for (int oc = 0; oc < WIG_TLF / 8; ++oc) {
                 const int lo = lt + 8 * oc;
                 double c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
-                if (gs[0] < lo + 8 && lo < Lg) {
+                if (PRE) {
+                    // precomputed-kernel variant (a9): B-fragments straight from the d-table in HBM
+                    if (gs[0] < lo + 8 && lo < Lg && want && lo + 8 > lacc) {
+                        const int lrow = lo + (lane >> 2);
+                        const bool ok = lrow >= l0 && lrow < Lg;
+                        const double *trow = A.dtab + ((size_t)tab * A.tri_g + tri_off(m, Lg) + (ok ? lrow : l0)) *
+                                                          (size_t)(32 * G) + (lane & 3);
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            if (gs[r] >= lo + 8) continue;
+                            const double *src = trow + (r * W + warp) * 32;
+                            double bv[8];
+#pragma unroll
+                            for (int qd = 0; qd < 8; ++qd) bv[qd] = ok ? __ldg(src + 4 * qd) : 0.0;
+#pragma unroll
+                            for (int qd = 0; qd < 8; qd += 2) {
+                                dmma884(c0, c1, hA[r][qd], bv[qd]);
+                                dmma884(c2, c3, hA[r][qd + 1], bv[qd + 1]);
+                            }
+                        }
+                    }
+                } else if (gs[0] < lo + 8 && lo < Lg) {
                     const bool mm = want && (lo + 8 > lacc);
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
@@ -478,7 +501,7 @@ __global__ void __launch_bounds__(MAXT) wigner_forward_kernel(WigArgs A)
                     reS += s_red[w + 1][ll][2 * k];
                     imS += s_red[w + 1][ll][2 * k + 1];
                 }
-                if (l & 1) {
+                if (!PRE && (l & 1)) {
                     re -= reS;
                     im -= imS;
                 } else {
@@ -491,6 +514,134 @@ __global__ void __launch_bounds__(MAXT) wigner_forward_kernel(WigArgs A)
                 double *dst = reinterpret_cast<double *>(&A.flmT[((size_t)ci.b * Mfull + mi) * Lfull + l]);
                 atomicAdd(dst, val.x);
                 atomicAdd(dst + 1, val.y);
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// precomputed-kernel variant (step a9; "simply precomputed"; O(N L^3) memory)
+//
+// dtab[tab][packed (m, l >= m) of the grid][32 G ring slots] holds d^l_mn(beta) itself (southern rings with their true
+// sign), zero below the group start.  One warp per (group, m, n) fills its rows by the recursion above.  The
+// contraction kernels then only stream the table: both directions are batched small-N GEMMs on the FP64 tensor pipe
+// (mma.sync.m8n8k4.f64), HBM-bound at 8 B per (ring, m, l, n) tuple for up to 4 complex columns.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(32) wigner_table_kernel(const double *__restrict__ coef, size_t tri, int Lfull, int Lg,
+                                                         int G, NList nl, const double *__restrict__ yv,
+                                                         const int *__restrict__ gstart,
+                                                         const double2 *__restrict__ dseed, double *__restrict__ dtab,
+                                                         size_t tri_g)
+{
+    const int g = blockIdx.x, m = blockIdx.y, tab = blockIdx.z, lane = threadIdx.x;
+    const int k = g * 32 + lane;
+    const bool south = (g & 1) != 0;
+    const int gs = gstart[((size_t)tab * Lg + m) * G + g];
+    if (gs >= Lg) return;
+    const double2 sd = dseed[((size_t)tab * Lg + m) * (size_t)(32 * G) + k];
+    double d = sd.x, u = sd.y;
+    const double y = yv[k];
+    const double *c = coef + ((size_t)tab * tri + tri_off(m, Lfull)) * 4;
+    double *out = dtab + ((size_t)tab * tri_g + tri_off(m, Lg)) * (size_t)(32 * G) + k;
+    for (int l = gs; l < Lg; ++l) {
+        out[(size_t)l * (32 * G)] = (south && (l & 1)) ? -d : d;
+        const double4 q = *reinterpret_cast<const double4 *>(c + 4 * (size_t)l);
+        wig_step(d, u, y, q.x, q.y, south ? q.w : q.z);
+    }
+}
+
+// inverse direction from the table: D[ring][col] += A[ring][l] B[l][col], A-fragments (8 rings x 4 degrees) gathered
+// from the table, B = filter x f_lm from shared memory, accumulators 8 rings x 8 columns per ring octet.
+template <int R, int MAXT>
+__global__ void __launch_bounds__(MAXT) precomp_inverse_kernel(WigArgs A)
+{
+    constexpr int NC = 8;
+    __shared__ double s_X[WIG_TL * NC];
+
+    const int m = blockIdx.x, chunk = blockIdx.y;
+    const int Lg = A.Lg, Lfull = A.Lfull, G = A.G;
+    const int Md = A.isReal ? Lg : 2 * Lg - 1;
+    const int Mfull = A.isReal ? Lfull : 2 * Lfull - 1;
+    const int T = blockDim.x, W = T >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int fr = lane >> 2, fk = lane & 3;  // A: ring fr of the octet, degree fk of the quad; B: degree fk, column fr
+
+    for (int q = 0; q < A.nn; ++q) {
+        const int n = A.n_val[q], an = n < 0 ? -n : n;
+        const int l0 = m > an ? m : an;
+        if (l0 >= Lg) continue;
+        const int tab = A.n_tab[q];
+        const int *gsrow = A.gstart + ((size_t)tab * Lg + m) * G;
+        const double sgn = ((m + n) & 1) ? -1.0 : 1.0;
+        const int lacc = l0 > A.lmin ? l0 : A.lmin;
+        const double *tbase = A.dtab + ((size_t)tab * A.tri_g + tri_off(m, Lg)) * (size_t)(32 * G);
+
+        int gs[R];
+        double acc[R][4][2];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int g = r * W + warp;
+            gs[r] = g < G ? gsrow[g] : INT_MAX;
+#pragma unroll
+            for (int o = 0; o < 4; ++o) acc[r][o][0] = acc[r][o][1] = 0.0;
+        }
+        int first = gsrow[0];
+        if (G > 1 && gsrow[1] < first) first = gsrow[1];
+        if (first < lacc) first = lacc;
+
+        for (int lt = first & ~(WIG_TL - 1); lt < Lg; lt += WIG_TL) {
+            __syncthreads();
+            for (int i = threadIdx.x; i < WIG_TL * (NC / 2); i += T) {
+                const int k = i / WIG_TL, ll = i % WIG_TL;
+                const int l = lt + ll;
+                const ColInfo ci = col_info(A, chunk * (NC / 2) + k);
+                cplx X = cmake(0.0, 0.0);
+                if (l >= lacc && l < Lg && ci.valid) {
+                    const int mi = A.isReal ? m : (ci.minus ? Lfull - 1 - m : Lfull - 1 + m);
+                    const cplx f = A.flmT[((size_t)ci.b * Mfull + mi) * Lfull + l];
+                    const cplx Gf = A.filt[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
+                    X = cmul(Gf, f);
+                    if (ci.minus) X = cscale(X, sgn);
+                }
+                s_X[ll * NC + 2 * k] = X.x;
+                s_X[ll * NC + 2 * k + 1] = X.y;
+            }
+            __syncthreads();
+#pragma unroll 2
+            for (int lq = 0; lq < WIG_TL; lq += 4) {
+                const int lo = lt + lq;
+                if (lo + 4 <= lacc || lo >= Lg || gs[0] >= lo + 4) continue;
+                const double bv = s_X[(lq + fk) * NC + fr];
+                const int lrow = lo + fk;
+                const bool ok = lrow >= l0 && lrow < Lg;
+                const double *trow = tbase + (size_t)(ok ? lrow : l0) * (32 * G) + fr;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    if (gs[r] >= lo + 4) continue;
+                    const double *src = trow + (r * W + warp) * 32;
+                    double av[4];
+#pragma unroll
+                    for (int o = 0; o < 4; ++o) av[o] = ok ? __ldg(src + 8 * o) : 0.0;
+#pragma unroll
+                    for (int o = 0; o < 4; ++o) dmma884(acc[r][o][0], acc[r][o][1], av[o], bv);
+                }
+            }
+        }
+
+        // D fragment: ring lane / 4 of the octet, real columns 2 (lane % 4) + {0, 1} = complex column lane % 4
+        const ColInfo ci = col_info(A, chunk * (NC / 2) + fk);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int g = r * W + warp;
+            if (g >= G || !ci.valid) continue;
+            if (ci.minus && m == 0) continue;
+            const int row = ci.minus ? A.n_rowm[q] : A.n_row[q];
+            const int mi = A.isReal ? m : (ci.minus ? Lg - 1 - m : Lg - 1 + m);
+#pragma unroll
+            for (int o = 0; o < 4; ++o) {
+                const int t = A.ring[g * 32 + o * 8 + fr];
+                if (t < 0) continue;
+                A.F[(((size_t)ci.b * A.nrows + row) * Lg + t) * Md + mi] = cmake(acc[r][o][0], acc[r][o][1]);
             }
         }
     }
@@ -589,13 +740,13 @@ void launch_inv_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
     S2W_LAUNCH_C(S2W_K_WIGNER_INV, (wigner_inverse_kernel<NC, R, MAXT>), grid, T, 0, st, A);
 }
 
-template <int R, int MAXT>
+template <int R, int MAXT, bool PRE>
 int launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
 {
-    const size_t smem = (size_t)(T / 32) * R * FWD_GT * sizeof(double);
+    const size_t smem = PRE ? 0 : (size_t)(T / 32) * R * FWD_GT * sizeof(double);
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(wigner_forward_kernel<R, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(wigner_forward_kernel<R, MAXT, PRE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)((size_t)(MAXT / 32) * R * FWD_GT * sizeof(double)));
         if (e != cudaSuccess) {
             set_error(std::string("cudaFuncSetAttribute(wigner_forward_kernel): ") + cudaGetErrorString(e));
@@ -604,7 +755,7 @@ int launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
         configured = true;
     }
     dim3 grid(A.Lg, chunks);
-    S2W_LAUNCH_C(S2W_K_WIGNER_FWD, (wigner_forward_kernel<R, MAXT>), grid, T, smem, st, A);
+    S2W_LAUNCH_C(S2W_K_WIGNER_FWD, (wigner_forward_kernel<R, MAXT, PRE>), grid, T, smem, st, A);
     return S2W_OK;
 }
 
@@ -628,8 +779,28 @@ int dispatch_inv(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t st)
 
 int dispatch_fwd(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t st)
 {
-#define S2W_WIG_CASE(RR, MT) \
-    if (c.R == RR && c.MAXT == MT) return launch_fwd_t<RR, MT>(A, 32 * c.W, chunks, st);
+#define S2W_WIG_CASE(RR, MT)                                                              \
+    if (c.R == RR && c.MAXT == MT)                                                        \
+        return A.dtab ? launch_fwd_t<RR, MT, true>(A, 32 * c.W, chunks, st)               \
+                      : launch_fwd_t<RR, MT, false>(A, 32 * c.W, chunks, st);
+    S2W_WIG_CASE(1, 256)
+    S2W_WIG_CASE(2, 256)
+    S2W_WIG_CASE(3, 256)
+    S2W_WIG_CASE(4, 256)
+    S2W_WIG_CASE(3, 512)
+    S2W_WIG_CASE(4, 512)
+#undef S2W_WIG_CASE
+    return S2W_EINVAL;
+}
+
+int dispatch_inv_pre(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t st)
+{
+#define S2W_WIG_CASE(RR, MT)                                                                                  \
+    if (c.R == RR && c.MAXT == MT) {                                                                          \
+        dim3 grid(A.Lg, chunks);                                                                              \
+        S2W_LAUNCH_C(S2W_K_WIGNER_INV, (precomp_inverse_kernel<RR, MT>), grid, 32 * c.W, 0, st, A);            \
+        return S2W_OK;                                                                                        \
+    }
     S2W_WIG_CASE(1, 256)
     S2W_WIG_CASE(2, 256)
     S2W_WIG_CASE(3, 256)
@@ -650,6 +821,7 @@ int launch_wigner(bool fwd, const WigArgs &A, cudaStream_t st)
     }
     const int CT = A.isReal ? A.B : 2 * A.B;
     if (fwd) return dispatch_fwd(A, c, (CT + 3) / 4, st);
+    if (A.dtab) return dispatch_inv_pre(A, c, (CT + 3) / 4, st);
     if (CT >= 3) return dispatch_inv<8>(A, c, (CT + 3) / 4, st);
     if (CT == 2) return dispatch_inv<4>(A, c, 1, st);
     return dispatch_inv<2>(A, c, 1, st);
@@ -668,6 +840,17 @@ int launch_wigner_seeds(const double *mant, const int *expo, const double *coef,
     const int count = Lg * ntab;
     S2W_LAUNCH(wigner_start_fix_kernel, (count + 127) / 128, 128, 0, st, gstart, G, count);
     S2W_LAUNCH(wigner_seed_kernel, grid, 32, 0, st, mant, expo, coef, tri, Lfull, Lg, G, nl, yv, ring, gstart, dseed, 1);
+    return S2W_OK;
+}
+
+int launch_wigner_table(const double *coef, size_t tri, int Lfull, int Lg, int G, const int *n_vals, int ntab,
+                        const double *yv, const int *gstart, const double2 *dseed, double *dtab, size_t tri_g,
+                        cudaStream_t st)
+{
+    NList nl;
+    for (int i = 0; i < ntab; ++i) nl.v[i] = n_vals[i];
+    dim3 grid(G, Lg, ntab);
+    S2W_LAUNCH(wigner_table_kernel, grid, 32, 0, st, coef, tri, Lfull, Lg, G, nl, yv, gstart, dseed, dtab, tri_g);
     return S2W_OK;
 }
 

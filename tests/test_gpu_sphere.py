@@ -155,3 +155,68 @@ def test_error_codes():
         api.s2wav_plan_create(8, 2, 1.0, 0)          # lambda <= 1
     with pytest.raises(api.S2WError):
         api.s2wav_plan_create(8, 2, 2.0, 7)          # J0 > J
+
+
+PRE_CASES = [
+    # L, N, lam, J0, multires, real, batch
+    (24, 4, 2.0, 1, True, True, 2),
+    (20, 5, 3.0, 1, True, False, 1),
+    (40, 3, 1.7, 2, True, True, 5),
+    (64, 5, 2.0, 2, False, False, 1),
+    (130, 3, 2.0, 3, True, True, 4),      # several ring groups per hemisphere, ragged last group
+]
+
+
+@pytest.mark.parametrize("L,N,lam,J0,mr,real,batch", PRE_CASES)
+def test_precomputed_kernel_variant_parity(L, N, lam, J0, mr, real, batch):
+    """S2W_PRECOMPUTE (step a9): the table-streaming DMMA contraction against the oracle and the on-the-fly path."""
+    torch, api = _api()
+    flm, f = _signals(L, 300 + L + N, real, batch)
+    plan = api.s2wav_plan_create(L, N, lam, J0, mr, real, batch, flags=api.S2W_PRECOMPUTE)
+    otf = api.s2wav_plan_create(L, N, lam, J0, mr, real, batch)
+    fd = torch.from_numpy(f).cuda()
+    w = plan.forward(fd)
+    w2 = otf.forward(fd)
+    scale = float(w2.abs().max())
+    assert float((w - w2).abs().max()) < 1e-12 * scale
+    scal, scales = plan.split(w)
+    filt = S.filters(L, N, lam, J0, "f80")
+    cast = (lambda a: a.real.astype(np.float64)) if real else (lambda a: a.astype(np.complex128))
+    o_phi, o_psi = S.analysis(f[0], L, N, lam, J0, mr, "f80", filt)
+    assert _relmax(scal[0].cpu().numpy(), cast(o_phi)) < FWD_TOL
+    for j in range(plan.J0, plan.J + 1):
+        assert _relmax(scales[(j, 0)][0].cpu().numpy(), cast(o_psi[j])) < FWD_TOL, j
+    back = plan.inverse(w).cpu().numpy().reshape(f.shape)
+    assert _relmax(back, f) < RT_TOL
+    plan.close()
+    otf.close()
+
+
+def test_config3_full_size_sampled_parity():
+    """BASELINE config 3 at full size (L = 1024, N = 5, batch 4, real) in the launch configuration bench.py times:
+    round trip on all pixels, and forward coefficients of the top scale on sampled beta rings against the oracle
+    (which evaluates single rings: oracle.sphere.analysis_from_flm(scales=, rings=))."""
+    torch, api = _api()
+    c = inputs.CONFIGS["C3"]
+    L, N, lam, J0, B = c["L"], c["N"], c["lam"], c["J0"], c["batch"]
+    flm = inputs.config_coefficients("C3")
+    plan = api.s2wav_plan_create(L, N, lam, J0, True, True, B)
+    f = plan.harmonic_inverse(torch.from_numpy(flm).cuda())
+    w = plan.forward(f)
+    back = plan.inverse(w)
+    rt = float((back - f).abs().max() / f.abs().max())
+    assert rt < RT_TOL, rt
+    # harmonic coefficients recovered from the pixels (forward SHT, steps a1-a3) against the seeded truth
+    got_flm = plan.harmonic_forward(f, L * (2 * L - 1)).cpu().numpy().reshape(B, L, 2 * L - 1)
+    assert _relmax(got_flm, flm) < FWD_TOL
+    # sampled rings of the two top scales and of a middle scale, signal 1
+    scal, scales = plan.split(w)
+    filt = S.filters(L, N, lam, J0, "f80")
+    for j, rings in [(plan.J, [0, 1, 357, 1022, 1023]), (plan.J - 1, [3, 511, 1020]), (plan.J - 3, [0, 64, 127])]:
+        _, o_psi = S.analysis_from_flm(flm[1], L, N, lam, J0, True, "f80", filt, scales=[j],
+                                       rings={j: np.array(rings)})
+        ref = o_psi[j].real.astype(np.float64)                      # [2N-1][len(rings)][2L_j-1]
+        got = scales[(j, 0)][1][:, rings, :].cpu().numpy()
+        den = float(scales[(j, 0)][1].abs().max())
+        assert np.abs(got - ref).max() / den < FWD_TOL, j
+    plan.close()

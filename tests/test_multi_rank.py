@@ -1,0 +1,66 @@
+"""World-size-2 test of bench.py's multi-GPU bookkeeping on CPU (gloo): the path shards as independent replicas with
+no data-path collective; the only exchange is the MAX over ranks of the device time, and the reported
+value is the units all ranks processed over that time."""
+import os
+import socket
+import sys
+
+import numpy as np
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    return port
+
+
+def _worker(rank, world, port, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    from paper_2402_01282_b200 import inputs
+    ms_local = [10.0, 14.5][rank]          # this rank's "device time" for 5 steps
+    e2e_local = [0.30, 0.20][rank]
+    ms, e2e = bench.max_over_ranks([ms_local, e2e_local], world, torch.device("cpu"))
+    value = bench.whole_job_value(world, 4, 5, ms)
+    # independent signals per replica: different seeds, same recipe
+    flm = inputs.flm_real(16, 2 + 1000 * bench.replica_seed_offset(rank), 1)
+    digest = torch.tensor([float(np.abs(flm).sum())], dtype=torch.float64)
+    both = [torch.zeros_like(digest) for _ in range(world)]
+    dist.all_gather(both, digest)
+    out.put((rank, ms, e2e, value, [float(b) for b in both]))
+    dist.destroy_process_group()
+
+
+def test_replicas_max_over_ranks_world2():
+    world = 2
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(out.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, ms, e2e, value, digests in res:
+        assert ms == 14.5 and e2e == 0.30                      # MAX over ranks, identical on every rank
+        assert abs(value - 2 * 4 * 5 / 14.5e-3) < 1e-9          # whole-job units over the slowest rank's time
+        assert digests[0] != digests[1]                          # replicas transform different signals
+
+
+def test_single_rank_is_identity():
+    import bench
+    assert bench.max_over_ranks([3.0, 1.0], 1, torch.device("cpu")) == [3.0, 1.0]
+    assert bench.whole_job_value(1, 4, 10, 50.0) == 4 * 10 / 50e-3
