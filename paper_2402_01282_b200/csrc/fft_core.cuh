@@ -29,6 +29,20 @@ struct FftTab {
     const cplx *rw_in1, *rw_out1, *rw_in3, *rw_out3;  // [n] each: reweighting phase tables (ring_fft.cu)
 };
 
+// Tables of the Toeplitz/Hankel form of the theta reweighting (ring_fft.cu, reweight_th_kernel): length-M2 power-of-two
+// transforms, M2 >= 2(L-1) - 1.
+struct RwTab {
+    int L;                 // band-limit of the grid; 0: not available (tiny grids use the Bluestein kernel)
+    FftTab fft;            // M = M2, twiddles only
+    const cplx *That;      // [M2] spectrum of T(d) = 1/sin(pi d/n) (digit-reversed order), times 1/(n M2)
+    const cplx *Ghat;      // [M2] spectrum of H(d + L - 1) times the reversal phase, times 1/(n M2)
+    const int *negpos;     // [M2] position of frequency -k given the position of frequency k
+    const double *delta;   // [L] c_t - c_{n-1-t}
+    const double *dsum;    // [L] (K_tt + K_{n-1-t,n-1-t}) / n
+    const double *vpole;   // [2][L] pole column per parity (sigma = +1, -1), / n
+    const double *rpole;   // [2][L] pole row per parity, / n
+};
+
 template <bool INV>
 __device__ __forceinline__ cplx mul_mi(cplx a)  // times -i (forward) or +i (inverse)
 {
@@ -147,6 +161,93 @@ __device__ __forceinline__ void mid_pass(cplx *buf, int M, const cplx *__restric
         Bfly<R, true>::run(v);
 #pragma unroll
         for (int k = 0; k < R; ++k) buf[S2W_PAD(g * R + k)] = v[k];
+    }
+}
+
+// Batched variants: nb transforms of length M stored bstride elements apart in one shared-memory buffer; one pass
+// works on all of them between two barriers.
+template <int R>
+__device__ __forceinline__ void dif_pass_b(cplx *buf, int M, int logS, const FftTab &T, int nb, int bstride)
+{
+    const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
+    const int s = 1 << logs;
+    const int twm = T.twmul << (T.logM - logS);
+    const int per = M / R;
+    for (int it = threadIdx.x; it < nb * per; it += blockDim.x) {
+        const int bi = it / per, idx = it - bi * per;
+        cplx *b = buf + bi * bstride;
+        int i = idx & (s - 1);
+        int base = ((idx >> logs) << logS) + i;
+        cplx v[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[k] = b[S2W_PAD(base + (k << logs))];
+        Bfly<R, false>::run(v);
+#pragma unroll
+        for (int j = 1; j < R; ++j) v[j] = cmul(v[j], __ldg(&T.tw[(i * j * twm) & T.twmask]));
+#pragma unroll
+        for (int k = 0; k < R; ++k) b[S2W_PAD(base + (k << logs))] = v[k];
+    }
+}
+
+template <int R>
+__device__ __forceinline__ void dit_pass_b(cplx *buf, int M, int logS, const FftTab &T, int nb, int bstride)
+{
+    const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
+    const int s = 1 << logs;
+    const int twm = T.twmul << (T.logM - logS);
+    const int per = M / R;
+    for (int it = threadIdx.x; it < nb * per; it += blockDim.x) {
+        const int bi = it / per, idx = it - bi * per;
+        cplx *b = buf + bi * bstride;
+        int i = idx & (s - 1);
+        int base = ((idx >> logs) << logS) + i;
+        cplx v[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[k] = b[S2W_PAD(base + (k << logs))];
+#pragma unroll
+        for (int j = 1; j < R; ++j) v[j] = cmulc(v[j], __ldg(&T.tw[(i * j * twm) & T.twmask]));
+        Bfly<R, true>::run(v);
+#pragma unroll
+        for (int k = 0; k < R; ++k) b[S2W_PAD(base + (k << logs))] = v[k];
+    }
+}
+
+// nb forward transforms, natural in, digit-reversed out (radix 8 ... 8, then 4 or 2).  Ends with a barrier.
+__device__ inline void fft_dif_full_b(cplx *buf, const FftTab &T, int nb, int bstride)
+{
+    const int M = T.M;
+    int logS = T.logM;
+    while (logS >= 3) {
+        dif_pass_b<8>(buf, M, logS, T, nb, bstride);
+        __syncthreads();
+        logS -= 3;
+    }
+    if (logS == 2) {
+        dif_pass_b<4>(buf, M, 2, T, nb, bstride);
+        __syncthreads();
+    } else if (logS == 1) {
+        dif_pass_b<2>(buf, M, 1, T, nb, bstride);
+        __syncthreads();
+    }
+}
+
+// the matching inverse: digit-reversed in, natural out, unscaled.  Ends with a barrier.
+__device__ inline void fft_dit_full_b(cplx *buf, const FftTab &T, int nb, int bstride)
+{
+    const int M = T.M;
+    int logS = T.logM % 3;
+    if (logS == 2) {
+        dit_pass_b<4>(buf, M, 2, T, nb, bstride);
+        __syncthreads();
+    } else if (logS == 1) {
+        dit_pass_b<2>(buf, M, 1, T, nb, bstride);
+        __syncthreads();
+    }
+    logS += 3;
+    while (logS <= T.logM) {
+        dit_pass_b<8>(buf, M, logS, T, nb, bstride);
+        __syncthreads();
+        logS += 3;
     }
 }
 

@@ -11,6 +11,7 @@ namespace s2w {
 #define S2W_MAX_ROWS (2 * S2W_MAX_N)  // rows n handled by one launch
 
 struct FftTab;
+struct RwTab;
 
 // rows (values of n) one SO(3) FFT launch works on
 struct So3Args {
@@ -71,6 +72,8 @@ int launch_so3_inv(bool real, const cplx *F, void *W, size_t sig_stride, const S
 int launch_so3_fwd(bool real, const void *W, size_t sig_stride, cplx *F, const So3Args &A, int batch, const FftTab &T,
                    cudaStream_t st);
 int launch_reweight(cplx *F, const RwArgs &A, int batch, const FftTab &T, cudaStream_t st);
+int launch_reweight_th(cplx *F, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st);   // L >= 8, L <= 2048
+int launch_fft_forward(cplx *data, const FftTab &T, cudaStream_t st);   // plan-time, in place, digit-reversed out
 
 // plan-time: group start degrees and seeds from the range-extended values d^{l0}_{mn}(beta_t) = mant 2^expo ([ntab][Lg m][Lg t])
 int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int G,

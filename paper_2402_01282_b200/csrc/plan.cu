@@ -97,6 +97,7 @@ struct DevPool {  // owns device allocations of a plan
 struct GridTab {  // everything that depends on the theta/phi grid of band-limit Lg
     int Lg;
     FftTab fft;
+    RwTab rw;        // Toeplitz/Hankel reweighting tables (rw.L = 0 on tiny grids)
     int G;           // ring groups of 32 (even): 2j north, 2j+1 south, each hemisphere sorted by |cos beta|
     double *yv;      // [32 G] 1 - |cos beta_t| of the ring in each slot
     int *ring;       // [32 G] ring index t, -1 for an empty slot
@@ -284,6 +285,163 @@ void host_coef(int L, const std::vector<int> &tabn, std::vector<double> &coef)
     }
 }
 
+// Tables of the Toeplitz/Hankel reweighting (ring_fft.cu, reweight_th_kernel) for band-limit L >= 8, in long double.
+// With n = 2L-1 and theta_t = pi (2t+1)/n, K[t,s] = sum_{|k|,|k'| < L} w(k+k') e^{-i(k theta_s + k' theta_t)},
+// w(q) = int_0^pi e^{i q theta} sin(theta) dtheta (reading R3), one finds K[t,s] = (-1)^{t-s} (c_t - c_s)/sin(pi (t-s)/n)
+// off the diagonal; c_t (with c_0 = 0) is read off the first column, the diagonal is summed directly.
+struct RwHost {
+    std::vector<double> delta, dsum, vpole, rpole, kT, kG;
+    int M2, logM2;
+};
+void host_rw_tables(int L, RwHost &H)
+{
+    const int n = 2 * L - 1, Lm = L - 1;
+    std::vector<ld> cs(2 * n), sn(2 * n);
+    for (int j = 0; j < 2 * n; ++j) {
+        cs[j] = cosl(PI_L * (ld)j / (ld)n);
+        sn[j] = sinl(PI_L * (ld)j / (ld)n);
+    }
+    auto idx = [&](long long a) {  // a mod 2n
+        long long r = a % (2LL * n);
+        return (int)(r < 0 ? r + 2LL * n : r);
+    };
+    // G0(k') = sum_k w(k+k') e^{-i k theta_0};  w even q: 2/(1-q^2) real, q = +-1: +-i pi/2
+    std::vector<ld> g0r(n), g0i(n);
+    for (int kp = -(L - 1); kp <= L - 1; ++kp) {
+        ld ar = 0, ai = 0;
+        for (int k = -(L - 1); k <= L - 1; ++k) {
+            const int q = k + kp;
+            const int J = idx(k);  // e^{-i k theta_0} = cs[J] - i sn[J]
+            if ((q & 1) == 0) {
+                const ld w = 2 / (1 - (ld)q * (ld)q);
+                ar += w * cs[J];
+                ai -= w * sn[J];
+            } else if (q == 1 || q == -1) {
+                const ld w = (q == 1 ? 1 : -1) * PI_L / 2;  // i w (cs - i sn) = w sn + i w cs
+                ar += w * sn[J];
+                ai += w * cs[J];
+            }
+        }
+        g0r[kp + L - 1] = ar;
+        g0i[kp + L - 1] = ai;
+    }
+    std::vector<ld> c(n), kd(n);
+    for (int t = 0; t < n; ++t) {
+        ld re = 0;
+        for (int kp = -(L - 1); kp <= L - 1; ++kp) {
+            const int J = idx((long long)kp * (2 * t + 1));  // e^{-i k' theta_t}
+            re += g0r[kp + L - 1] * cs[J] + g0i[kp + L - 1] * sn[J];
+        }
+        c[t] = ((t & 1) ? -1 : 1) * re * sn[t];
+        // diagonal: sum_q w(q) (n - |q|) e^{-i q theta_t}
+        ld d = 2 * (ld)n + PI_L * (ld)(n - 1) * sn[idx(2 * t + 1)];
+        for (int q = 2; q <= 2 * L - 2; q += 2)
+            d += 2 * (2 / (1 - (ld)q * (ld)q)) * (ld)(n - q) * cs[idx((long long)q * (2 * t + 1))];
+        kd[t] = d;
+    }
+    auto K = [&](int t, int s) -> ld {
+        if (t == s) return kd[t];
+        const int d = t - s;
+        const ld sd = d > 0 ? sn[d] : -sn[-d];
+        return ((d & 1) ? -1 : 1) * (c[t] - c[s]) / sd;
+    };
+    H.delta.assign(L, 0.0);
+    H.dsum.assign(L, 0.0);
+    H.vpole.assign(2 * (size_t)L, 0.0);
+    H.rpole.assign(2 * (size_t)L, 0.0);
+    for (int t = 0; t < Lm; ++t) {
+        H.delta[t] = (double)(c[t] - c[n - 1 - t]);
+        H.dsum[t] = (double)((kd[t] + kd[n - 1 - t]) / n);
+        for (int par = 0; par < 2; ++par) {
+            const ld sg = par ? -1 : 1;
+            H.vpole[(size_t)par * L + t] = (double)((K(t, L - 1) + sg * K(n - 1 - t, L - 1)) / n);
+            H.rpole[(size_t)par * L + t] = (double)((K(L - 1, t) + sg * K(L - 1, n - 1 - t)) / n);
+        }
+    }
+    H.rpole[L - 1] = H.rpole[(size_t)L + L - 1] = (double)(kd[L - 1] / n);
+    H.logM2 = std::max(1, ceil_log2(2 * Lm - 1));
+    H.M2 = 1 << H.logM2;
+    H.kT.assign(H.M2, 0.0);
+    H.kG.assign(H.M2, 0.0);
+    const ld scale = 1 / ((ld)n * (ld)H.M2);
+    for (int d = -(Lm - 1); d <= Lm - 1; ++d) {
+        const int slot = d < 0 ? d + H.M2 : d;
+        if (d != 0) H.kT[slot] = (double)(scale / (d > 0 ? sn[d] : -sn[-d]));
+        H.kG[slot] = (double)(scale / sn[d + Lm]);
+    }
+}
+
+int build_rw(s2w_plan *p, GridTab &g)
+{
+    const int L = g.Lg;
+    memset(&g.rw, 0, sizeof(g.rw));
+    if (L < 8) return S2W_OK;
+    RwHost H;
+    host_rw_tables(L, H);
+    const int M2 = H.M2, Lm = L - 1;
+    FftTab &T = g.rw.fft;
+    T.n = 0;
+    T.L = L;
+    T.logM = H.logM2;
+    T.M = M2;
+    T.tw = p->tw;
+    T.twmul = p->Mtab / M2;
+    T.twmask = p->Mtab - 1;
+    // spectra in the transform's own (digit-reversed) order, and that order itself from the transform of e_1
+    std::vector<cplx> hbuf((size_t)3 * M2, cmake(0.0, 0.0));
+    for (int i = 0; i < M2; ++i) {
+        hbuf[i] = cmake(H.kT[i], 0.0);
+        hbuf[(size_t)M2 + i] = cmake(H.kG[i], 0.0);
+    }
+    hbuf[(size_t)2 * M2 + 1] = cmake(1.0, 0.0);
+    cplx *dbuf;
+    int rc;
+    if ((rc = p->pool.upload(&dbuf, hbuf))) return rc;
+    for (int a = 0; a < 3; ++a)
+        if ((rc = launch_fft_forward(dbuf + (size_t)a * M2, T, 0))) return rc;
+    S2W_CUDA_CHECK(cudaMemcpy(hbuf.data(), dbuf, hbuf.size() * sizeof(cplx), cudaMemcpyDeviceToHost));
+    std::vector<int> kof(M2), pos(M2, -1), negpos(M2);
+    for (int q = 0; q < M2; ++q) {
+        const cplx v = hbuf[(size_t)2 * M2 + q];  // exp(-2 pi i k / M2)
+        long long k = llround(-std::atan2(v.y, v.x) * (double)M2 / (2.0 * pi_d()));
+        k %= M2;
+        if (k < 0) k += M2;
+        kof[q] = (int)k;
+        pos[k] = q;
+    }
+    for (int k = 0; k < M2; ++k)
+        if (pos[k] < 0) {
+            set_error("internal error: transform order is not a permutation");
+            return S2W_ECUDA;
+        }
+    for (int q = 0; q < M2; ++q) {
+        negpos[q] = pos[(M2 - kof[q]) % M2];
+        // reversal phase of the Hankel part: exp(-2 pi i k (Lm - 1) / M2)
+        const long long j = ((long long)kof[q] * (Lm - 1)) % M2;
+        const ld ang = -2 * PI_L * (ld)j / (ld)M2;
+        const ld pr = cosl(ang), pi_ = sinl(ang);
+        const cplx gq = hbuf[(size_t)M2 + q];
+        hbuf[(size_t)M2 + q] = cmake((double)(gq.x * pr - gq.y * pi_), (double)(gq.x * pi_ + gq.y * pr));
+    }
+    S2W_CUDA_CHECK(cudaMemcpy(dbuf, hbuf.data(), (size_t)2 * M2 * sizeof(cplx), cudaMemcpyHostToDevice));
+    g.rw.That = dbuf;
+    g.rw.Ghat = dbuf + M2;
+    int *dneg;
+    double *dd, *ds, *dv, *dr;
+    if ((rc = p->pool.upload(&dneg, negpos))) return rc;
+    if ((rc = p->pool.upload(&dd, H.delta))) return rc;
+    if ((rc = p->pool.upload(&ds, H.dsum))) return rc;
+    if ((rc = p->pool.upload(&dv, H.vpole))) return rc;
+    if ((rc = p->pool.upload(&dr, H.rpole))) return rc;
+    g.rw.negpos = dneg;
+    g.rw.delta = dd;
+    g.rw.dsum = ds;
+    g.rw.vpole = dv;
+    g.rw.rpole = dr;
+    g.rw.L = L;
+    return S2W_OK;
+}
+
 int build_grid(s2w_plan *p, int Lg)
 {
     if (grid_index(p, Lg) >= 0) return S2W_OK;
@@ -317,6 +475,7 @@ int build_grid(s2w_plan *p, int Lg)
     T.bhat_p = bp;
     T.what = wh;
     if ((rc = launch_fft_tables(T, chirp, i1, o1, i3, o3, bm, bp, wh, 0))) return rc;
+    if ((rc = build_rw(p, g))) return rc;
 
     std::vector<double> mant, yv;
     std::vector<int> expo, ring;
@@ -570,7 +729,7 @@ static int sht_forward_dev(const s2w_plan *p, const Stage &st, const void *f, si
     if ((rc = launch_ring_fwd(p->real, f, w.F, B, st.Lg, sig_stride, g.fft, s))) return rc;
     RwArgs R;
     fill_rw_args(p, st, R);
-    if ((rc = launch_reweight(w.F, R, B, g.fft, s))) return rc;
+    if ((rc = g.rw.L ? launch_reweight_th(w.F, R, B, g.rw, s) : launch_reweight(w.F, R, B, g.fft, s))) return rc;
     if (zero_first) {
         const size_t Mfull = p->real ? p->L : 2 * p->L - 1;
         S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * Mfull * p->L * sizeof(cplx), s));
@@ -625,7 +784,7 @@ static int scale_synthesis(const s2w_plan *p, const Scale &sc, int B, const Work
     if ((rc = launch_so3_fwd(p->real, src, sig_stride, w.F, S, B, g.fft, s))) return rc;
     RwArgs R;
     fill_rw_args(p, sc.st, R);
-    if ((rc = launch_reweight(w.F, R, B, g.fft, s))) return rc;
+    if ((rc = g.rw.L ? launch_reweight_th(w.F, R, B, g.rw, s) : launch_reweight(w.F, R, B, g.fft, s))) return rc;
     WigArgs A;
     fill_wig_args(p, sc.st, true, B, w.flmT, w.F, A);
     return launch_wigner_forward(A, s);

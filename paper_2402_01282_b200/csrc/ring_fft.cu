@@ -303,6 +303,121 @@ __global__ void __launch_bounds__(256) reweight_kernel(cplx *__restrict__ F, RwA
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// a2 in Toeplitz/Hankel form.  On the extended grid of n = 2L-1 rings the operator of R3 (iii)-(v),
+//   K[t,s] = sum_{k,k'} w(k+k') e^{-i(k theta_s + k' theta_t)} = int_0^pi D_n(theta-theta_t) D_n(theta-theta_s) sin(theta) dtheta
+// (D_n the Dirichlet kernel), is Cauchy-like:  K[t,s] = (-1)^{t-s} (c_t - c_s) / sin(pi (t-s)/n),  t != s.
+// Folding the extension and the fold (vi) into it, with a_t = (-1)^t, delta_t = c_t - c_{n-1-t}, on rings t, s < L-1:
+//   n h_t = a_t [ delta_t ((T - sigma H) u1)_t - ((T + sigma H) u2)_t ] + (K_tt + K_{n-1-t,n-1-t}) x_t + v_sigma[t] x_{L-1},
+//   u1 = a x,  u2 = delta a x,  T[t,s] = 1/sin(pi (t-s)/n) (0 on the diagonal),  H[t,s] = 1/sin(pi (t+s+1)/n),
+// and the pole ring t = L-1 (its own mirror image) is a plain dot product with a tabulated row.  T u and H u are
+// linear convolutions of length-(L-1) sequences: four power-of-two FFTs of length M2 >= 2L-3 per column (H u uses
+// the spectrum of u at -k), instead of three Bluestein convolutions (six FFTs of length 2 M2).  All tables (c_t, the
+// diagonal, pole row and column) are computed in long double at plan creation; no chirps, so the result is also more
+// accurate (2e-16 at L = 1024).  One block per column; both sequences go through each FFT pass together.
+// ---------------------------------------------------------------------------------------------------------------
+#define RW_MAXPT 8  // ring values a thread keeps in registers (L <= 8 * blockDim)
+__global__ void __launch_bounds__(256) reweight_th_kernel(cplx *__restrict__ F, RwArgs A, RwTab R)
+{
+    extern __shared__ cplx buf[];
+    __shared__ cplx s_part[8];
+    __shared__ cplx s_pole[2];
+    const FftTab &T = R.fft;
+    const int L = R.L, Lm = L - 1, M = T.M;
+    const int bstride = fft_padded_len(M);
+    cplx *b1 = buf, *b2 = buf + bstride;
+    const int mi = blockIdx.x, q = blockIdx.y, b = blockIdx.z;
+    const int m = A.isReal ? mi : mi - (L - 1);
+    const int nv = A.n_val[q];
+    const int par = ((m + nv) & 1) ? 1 : 0;  // 0: sigma = +1, 1: sigma = -1
+    const double sigma = par ? -1.0 : 1.0;
+    cplx *col = F + ((size_t)b * A.nrows + A.n_row[q]) * (size_t)L * A.Md + mi;
+    const double *rp = R.rpole + par * L, *vp = R.vpole + par * L;
+
+    cplx xs[RW_MAXPT];
+    cplx dot = cmake(0.0, 0.0);
+#pragma unroll
+    for (int k = 0; k < RW_MAXPT; ++k) {
+        const int t = threadIdx.x + k * blockDim.x;
+        cplx x = cmake(0.0, 0.0);
+        if (t < L) {
+            x = col[(size_t)t * A.Md];
+            const double r = rp[t];
+            dot.x = fma(r, x.x, dot.x);
+            dot.y = fma(r, x.y, dot.y);
+        }
+        xs[k] = x;
+        if (t == Lm) s_pole[0] = x;
+    }
+    for (int t = threadIdx.x; t < M; t += blockDim.x) {  // zero padding (and the slots filled below)
+        b1[S2W_PAD(t)] = cmake(0.0, 0.0);
+        b2[S2W_PAD(t)] = cmake(0.0, 0.0);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < RW_MAXPT; ++k) {
+        const int t = threadIdx.x + k * blockDim.x;
+        if (t < Lm) {
+            const cplx u1 = (t & 1) ? cscale(xs[k], -1.0) : xs[k];
+            b1[S2W_PAD(t)] = u1;
+            b2[S2W_PAD(t)] = cscale(u1, R.delta[t]);
+        }
+    }
+    // pole-ring dot product: warp shuffle, then across warps
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        dot.x += __shfl_xor_sync(0xffffffffu, dot.x, o);
+        dot.y += __shfl_xor_sync(0xffffffffu, dot.y, o);
+    }
+    if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = dot;
+    __syncthreads();
+    fft_dif_full_b(buf, T, 2, bstride);
+    // spectra of T u -/+ sigma H u: Y(k) = That(k) U(k) -/+ sigma Ghat(k) U(-k)
+    for (int p = threadIdx.x; p < M; p += blockDim.x) {
+        const int pn = __ldg(&R.negpos[p]);
+        if (pn < p) continue;
+        const cplx tp = __ldg(&R.That[p]), gp = cscale(__ldg(&R.Ghat[p]), sigma);
+        const cplx tn = __ldg(&R.That[pn]), gn = cscale(__ldg(&R.Ghat[pn]), sigma);
+        const cplx u1p = b1[S2W_PAD(p)], u1n = b1[S2W_PAD(pn)], u2p = b2[S2W_PAD(p)], u2n = b2[S2W_PAD(pn)];
+        b1[S2W_PAD(p)] = csub(cmul(tp, u1p), cmul(gp, u1n));
+        b2[S2W_PAD(p)] = cadd(cmul(tp, u2p), cmul(gp, u2n));
+        if (pn != p) {
+            b1[S2W_PAD(pn)] = csub(cmul(tn, u1n), cmul(gn, u1p));
+            b2[S2W_PAD(pn)] = cadd(cmul(tn, u2n), cmul(gn, u2p));
+        }
+    }
+    __syncthreads();
+    fft_dit_full_b(buf, T, 2, bstride);
+    const cplx xpole = s_pole[0];
+#pragma unroll
+    for (int k = 0; k < RW_MAXPT; ++k) {
+        const int t = threadIdx.x + k * blockDim.x;
+        if (t < Lm) {
+            const cplx y1 = b1[S2W_PAD(t)], y2 = b2[S2W_PAD(t)];
+            const double dl = R.delta[t], ds = R.dsum[t], v = vp[t];
+            cplx h = cmake(fma(dl, y1.x, -y2.x), fma(dl, y1.y, -y2.y));
+            if (t & 1) h = cscale(h, -1.0);
+            h.x += fma(ds, xs[k].x, v * xpole.x);
+            h.y += fma(ds, xs[k].y, v * xpole.y);
+            col[(size_t)t * A.Md] = h;
+        } else if (t == Lm) {
+            cplx acc = cmake(0.0, 0.0);
+            for (int w = 0; w < (int)(blockDim.x >> 5); ++w) acc = cadd(acc, s_part[w]);
+            col[(size_t)t * A.Md] = acc;
+        }
+    }
+}
+
+// plan-time: in-place forward transform (natural in, digit-reversed out) of one length-M array, one block
+__global__ void __launch_bounds__(256) fft_forward_kernel(cplx *data, FftTab T)
+{
+    extern __shared__ cplx buf[];
+    for (int e = threadIdx.x; e < T.M; e += blockDim.x) buf[S2W_PAD(e)] = data[e];
+    __syncthreads();
+    fft_dif_full(buf, T);
+    for (int e = threadIdx.x; e < T.M; e += blockDim.x) data[e] = buf[S2W_PAD(e)];
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // plan-time table kernels
 // ---------------------------------------------------------------------------------------------------------------
 __global__ void twiddle_kernel(cplx *tw, int Mtab)
@@ -477,6 +592,26 @@ int launch_so3_fwd(bool real, const void *W, size_t sig_stride, cplx *F, const S
         if ((rc = set_smem(so3_fwd_kernel<false>, sm))) return rc;
         S2W_LAUNCH_C(S2W_K_SO3_FFT, so3_fwd_kernel<false>, grid, 256, sm, st, W, F, sig_stride, A, T);
     }
+    return S2W_OK;
+}
+
+int launch_fft_forward(cplx *data, const FftTab &T, cudaStream_t st)
+{
+    size_t sm = fft_smem_bytes(T);
+    int rc = set_smem(fft_forward_kernel, sm);
+    if (rc) return rc;
+    S2W_LAUNCH(fft_forward_kernel, 1, 256, sm, st, data, T);
+    return S2W_OK;
+}
+
+int launch_reweight_th(cplx *F, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st)
+{
+    if (A.nn <= 0) return S2W_OK;
+    size_t sm = 2 * (size_t)fft_padded_len(R.fft.M) * sizeof(cplx);
+    int rc = set_smem(reweight_th_kernel, sm);
+    if (rc) return rc;
+    dim3 grid(A.Md, A.nn, batch);
+    S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight_th_kernel, grid, 256, sm, st, F, A, R);
     return S2W_OK;
 }
 
