@@ -105,6 +105,25 @@ struct Bfly<8, INV> {
     }
 };
 
+// Twiddles W^j, j = 1..R-1, from one table entry W = W_S^i: powers by repeated complex multiplication (at most three
+// multiplications deep, error <= ~4 ulp).  One 16-byte table load per butterfly instead of R-1 scattered ones: the
+// table does not fit beside three blocks' shared memory in L1, and scattered 16-byte loads cost a wavefront each.
+template <int R>
+__device__ __forceinline__ void twiddle_powers(cplx w1, cplx (&w)[R])
+{
+    w[1 % R] = w1;
+    if (R >= 4) {
+        w[2] = cmul(w1, w1);
+        w[3] = cmul(w[2], w1);
+    }
+    if (R >= 8) {
+        w[4] = cmul(w[2], w[2]);
+        w[5] = cmul(w[4], w1);
+        w[6] = cmul(w[3], w[3]);
+        w[7] = cmul(w[4], w[3]);
+    }
+}
+
 // One decimation-in-frequency pass on sub-transforms of size S (radix R): butterflies, then twiddles W_S^{i j}.
 template <int R>
 __device__ __forceinline__ void dif_pass(cplx *buf, int M, int logS, const FftTab &T)
@@ -119,8 +138,10 @@ __device__ __forceinline__ void dif_pass(cplx *buf, int M, int logS, const FftTa
 #pragma unroll
         for (int k = 0; k < R; ++k) v[k] = buf[S2W_PAD(base + (k << logs))];
         Bfly<R, false>::run(v);
+        cplx w[R];
+        twiddle_powers<R>(__ldg(&T.tw[(i * twm) & T.twmask]), w);
 #pragma unroll
-        for (int j = 1; j < R; ++j) v[j] = cmul(v[j], __ldg(&T.tw[(i * j * twm) & T.twmask]));
+        for (int j = 1; j < R; ++j) v[j] = cmul(v[j], w[j]);
 #pragma unroll
         for (int k = 0; k < R; ++k) buf[S2W_PAD(base + (k << logs))] = v[k];
     }
@@ -139,8 +160,10 @@ __device__ __forceinline__ void dit_pass(cplx *buf, int M, int logS, const FftTa
         cplx v[R];
 #pragma unroll
         for (int k = 0; k < R; ++k) v[k] = buf[S2W_PAD(base + (k << logs))];
+        cplx w[R];
+        twiddle_powers<R>(__ldg(&T.tw[(i * twm) & T.twmask]), w);
 #pragma unroll
-        for (int j = 1; j < R; ++j) v[j] = cmulc(v[j], __ldg(&T.tw[(i * j * twm) & T.twmask]));
+        for (int j = 1; j < R; ++j) v[j] = cmulc(v[j], w[j]);
         Bfly<R, true>::run(v);
 #pragma unroll
         for (int k = 0; k < R; ++k) buf[S2W_PAD(base + (k << logs))] = v[k];
@@ -182,8 +205,10 @@ __device__ __forceinline__ void dif_pass_b(cplx *buf, int M, int logS, const Fft
 #pragma unroll
         for (int k = 0; k < R; ++k) v[k] = b[S2W_PAD(base + (k << logs))];
         Bfly<R, false>::run(v);
+        cplx w[R];
+        twiddle_powers<R>(__ldg(&T.tw[(i * twm) & T.twmask]), w);
 #pragma unroll
-        for (int j = 1; j < R; ++j) v[j] = cmul(v[j], __ldg(&T.tw[(i * j * twm) & T.twmask]));
+        for (int j = 1; j < R; ++j) v[j] = cmul(v[j], w[j]);
 #pragma unroll
         for (int k = 0; k < R; ++k) b[S2W_PAD(base + (k << logs))] = v[k];
     }
@@ -204,8 +229,10 @@ __device__ __forceinline__ void dit_pass_b(cplx *buf, int M, int logS, const Fft
         cplx v[R];
 #pragma unroll
         for (int k = 0; k < R; ++k) v[k] = b[S2W_PAD(base + (k << logs))];
+        cplx w[R];
+        twiddle_powers<R>(__ldg(&T.tw[(i * twm) & T.twmask]), w);
 #pragma unroll
-        for (int j = 1; j < R; ++j) v[j] = cmulc(v[j], __ldg(&T.tw[(i * j * twm) & T.twmask]));
+        for (int j = 1; j < R; ++j) v[j] = cmulc(v[j], w[j]);
         Bfly<R, true>::run(v);
 #pragma unroll
         for (int k = 0; k < R; ++k) b[S2W_PAD(base + (k << logs))] = v[k];

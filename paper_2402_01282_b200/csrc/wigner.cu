@@ -202,7 +202,7 @@ __device__ __forceinline__ void inv_dispatch(int ra, int la, int lb, int lt, int
 }
 
 template <int NC, int R, int MAXT>
-__global__ void __launch_bounds__(MAXT) wigner_inverse_kernel(WigArgs A)
+__global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_inverse_kernel(WigArgs A)
 {
     __shared__ double2 s_ag[WIG_TL];
     __shared__ double2 s_e[WIG_TL];
@@ -337,7 +337,7 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
 }
 
 template <int R, int MAXT, bool PRE>
-__global__ void __launch_bounds__(MAXT) wigner_forward_kernel(WigArgs A)
+__global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_kernel(WigArgs A)
 {
     constexpr int NC = 8;
     constexpr int NW = MAXT / 32;
@@ -439,28 +439,46 @@ __global__ void __launch_bounds__(MAXT) wigner_forward_kernel(WigArgs A)
                     }
                 } else if (gs[0] < lo + 8 && lo < Lg) {
                     const bool mm = want && (lo + 8 > lacc);
+                    int ra = 0;
+                    bool starting = false;
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
-                        if (gs[r] >= lo + 8) continue;  // warp-uniform
-                        double *dst = dt + r * FWD_GT + wr_off;
-                        if (gs[r] >= lo) {  // the group starts inside this octet
+                        if (gs[r] < lo + 8) {
+                            ++ra;
+                            if (gs[r] >= lo) starting = true;
+                        }
+                    }
+                    double *dst = dt + wr_off;
+                    if (!starting) {
+                        // all active groups started before this octet: R independent chains, step by step
 #pragma unroll
-                            for (int s = 0; s < 8; ++s) {
-                                if (gs[r] == lo + s) {
-                                    const double2 sd = seedrow[(r * W + warp) * 32 + lane];
-                                    d[r] = sd.x;
-                                    u[r] = sd.y;
+                        for (int s = 0; s < 8; ++s) {
+                            const double2 ag = s_ag[8 * oc + s];
+                            const double e = se[2 * (8 * oc + s)];
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                if (r < ra) {
+                                    dst[r * FWD_GT + 4 * s] = d[r];
+                                    wig_step(d[r], u[r], y[r], ag.x, ag.y, e);
                                 }
-                                dst[4 * s] = d[r];
-                                const double2 ag = s_ag[8 * oc + s];
-                                wig_step(d[r], u[r], y[r], ag.x, ag.y, se[2 * (8 * oc + s)]);
                             }
-                        } else {
+                        }
+                    } else {
+#pragma unroll 1
+                        for (int s = 0; s < 8; ++s) {
+                            const double2 ag = s_ag[8 * oc + s];
+                            const double e = se[2 * (8 * oc + s)];
 #pragma unroll
-                            for (int s = 0; s < 8; ++s) {
-                                dst[4 * s] = d[r];
-                                const double2 ag = s_ag[8 * oc + s];
-                                wig_step(d[r], u[r], y[r], ag.x, ag.y, se[2 * (8 * oc + s)]);
+                            for (int r = 0; r < R; ++r) {
+                                if (r < ra) {
+                                    if (gs[r] == lo + s) {  // the group starts here (warp-uniform)
+                                        const double2 sd = seedrow[(r * W + warp) * 32 + lane];
+                                        d[r] = sd.x;
+                                        u[r] = sd.y;
+                                    }
+                                    dst[r * FWD_GT + 4 * s] = d[r];
+                                    wig_step(d[r], u[r], y[r], ag.x, ag.y, e);
+                                }
                             }
                         }
                     }
