@@ -35,7 +35,7 @@ namespace s2w {
 namespace {
 
 #define WIG_TL 64   // l-tile of the inverse kernel
-#define WIG_TLF 32  // l-tile of the forward kernel
+#define WIG_TLF 64  // l-tile of the forward kernel
 #define RAMP_THRESHOLD_EXP (-90)
 
 __device__ __forceinline__ size_t tri_off(int m, int Lfull) { return (size_t)m * Lfull - ((size_t)m * (m - 1)) / 2 - m; }
@@ -336,6 +336,37 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
                  : "d"(a), "d"(b));
 }
 
+// one l-octet of RA active groups (all started before the octet): 8 recursion steps of RA independent chains with the
+// d~ values stored as B-fragments, then (if the octet has outputs) 8 RA tensor-pipe accumulations.
+template <int R, int RA>
+__device__ __forceinline__ void fwd_octet(const double2 *s_ag8, const double *se8, double *dst, const double *src,
+                                          bool mm, const double (&y)[R], double (&d)[R], double (&u)[R],
+                                          const double (&hA)[R][8], double &c0, double &c1, double &c2, double &c3)
+{
+#pragma unroll
+    for (int s = 0; s < 8; ++s) {
+        const double2 ag = s_ag8[s];
+        const double e = se8[2 * s];
+#pragma unroll
+        for (int r = 0; r < RA; ++r) {
+            dst[r * FWD_GT + 4 * s] = d[r];
+            wig_step(d[r], u[r], y[r], ag.x, ag.y, e);
+        }
+    }
+    if (mm) {
+        __syncwarp();
+#pragma unroll
+        for (int r = 0; r < RA; ++r) {
+#pragma unroll
+            for (int qd = 0; qd < 8; qd += 2) {
+                dmma884(c0, c1, hA[r][qd], src[r * FWD_GT + qd * FWD_QS]);
+                dmma884(c2, c3, hA[r][qd + 1], src[r * FWD_GT + (qd + 1) * FWD_QS]);
+            }
+        }
+        __syncwarp();
+    }
+}
+
 template <int R, int MAXT, bool PRE>
 __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_kernel(WigArgs A)
 {
@@ -343,8 +374,9 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
     constexpr int NW = MAXT / 32;
     __shared__ double2 s_ag[WIG_TLF];
     __shared__ double2 s_e[WIG_TLF];
-    __shared__ double s_red[NW][WIG_TLF][NC];
-    extern __shared__ double s_dt[];  // [W][R][FWD_GT]
+    extern __shared__ double s_dyn[];  // s_red [NW][WIG_TLF][NC], then the B-fragment tiles [W][R][FWD_GT]
+    double (*s_red)[WIG_TLF][NC] = reinterpret_cast<double (*)[WIG_TLF][NC]>(s_dyn);
+    double *s_dt = s_dyn + NW * WIG_TLF * NC;
 
     const int m = blockIdx.x, chunk = blockIdx.y;
     const int Lg = A.Lg, Lfull = A.Lfull, G = A.G;
@@ -449,20 +481,18 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                         }
                     }
                     double *dst = dt + wr_off;
+                    const double *src = dt + lane;
                     if (!starting) {
-                        // all active groups started before this octet: R independent chains, step by step
-#pragma unroll
-                        for (int s = 0; s < 8; ++s) {
-                            const double2 ag = s_ag[8 * oc + s];
-                            const double e = se[2 * (8 * oc + s)];
-#pragma unroll
-                            for (int r = 0; r < R; ++r) {
-                                if (r < ra) {
-                                    dst[r * FWD_GT + 4 * s] = d[r];
-                                    wig_step(d[r], u[r], y[r], ag.x, ag.y, e);
-                                }
-                            }
-                        }
+                        const double2 *ag8 = s_ag + 8 * oc;
+                        const double *se8 = se + 16 * oc;
+                        if (R >= 4 && ra == 4)
+                            fwd_octet<R, (R >= 4 ? 4 : R)>(ag8, se8, dst, src, mm, y, d, u, hA, c0, c1, c2, c3);
+                        else if (R >= 3 && ra == 3)
+                            fwd_octet<R, (R >= 3 ? 3 : R)>(ag8, se8, dst, src, mm, y, d, u, hA, c0, c1, c2, c3);
+                        else if (R >= 2 && ra == 2)
+                            fwd_octet<R, (R >= 2 ? 2 : R)>(ag8, se8, dst, src, mm, y, d, u, hA, c0, c1, c2, c3);
+                        else
+                            fwd_octet<R, 1>(ag8, se8, dst, src, mm, y, d, u, hA, c0, c1, c2, c3);
                     } else {
 #pragma unroll 1
                         for (int s = 0; s < 8; ++s) {
@@ -481,20 +511,19 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                                 }
                             }
                         }
-                    }
-                    if (mm) {
-                        __syncwarp();
+                        if (mm) {
+                            __syncwarp();
 #pragma unroll
-                        for (int r = 0; r < R; ++r) {
-                            if (gs[r] >= lo + 8) continue;
-                            const double *src = dt + r * FWD_GT + lane;
+                            for (int r = 0; r < R; ++r) {
+                                if (r >= ra) continue;
 #pragma unroll
-                            for (int qd = 0; qd < 8; qd += 2) {
-                                dmma884(c0, c1, hA[r][qd], src[qd * FWD_QS]);
-                                dmma884(c2, c3, hA[r][qd + 1], src[(qd + 1) * FWD_QS]);
+                                for (int qd = 0; qd < 8; qd += 2) {
+                                    dmma884(c0, c1, hA[r][qd], src[r * FWD_GT + qd * FWD_QS]);
+                                    dmma884(c2, c3, hA[r][qd + 1], src[r * FWD_GT + (qd + 1) * FWD_QS]);
+                                }
                             }
+                            __syncwarp();
                         }
-                        __syncwarp();
                     }
                 }
                 // D fragment: row (column index) lane / 4, degrees 2 (lane % 4) + {0, 1} of the octet
@@ -761,11 +790,12 @@ void launch_inv_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
 template <int R, int MAXT, bool PRE>
 int launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
 {
-    const size_t smem = PRE ? 0 : (size_t)(T / 32) * R * FWD_GT * sizeof(double);
+    const size_t red = (size_t)(MAXT / 32) * WIG_TLF * 8 * sizeof(double);
+    const size_t smem = red + (PRE ? 0 : (size_t)(T / 32) * R * FWD_GT * sizeof(double));
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(wigner_forward_kernel<R, MAXT, PRE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)((size_t)(MAXT / 32) * R * FWD_GT * sizeof(double)));
+                                             (int)(red + (size_t)(MAXT / 32) * R * FWD_GT * sizeof(double)));
         if (e != cudaSuccess) {
             set_error(std::string("cudaFuncSetAttribute(wigner_forward_kernel): ") + cudaGetErrorString(e));
             return S2W_ECUDA;
