@@ -21,6 +21,7 @@ struct FftTab {
     int logM, M;        // Bluestein length
     int twmul;          // twiddle table stride: W_M^k = tw[k * twmul]
     int twmask;         // table length - 1
+    int twlo;           // low bits of the two-level twiddle split (min(6, log2 table length))
     const cplx *tw;     // exp(-2 pi i k / Mtab)
     const cplx *chirp;  // [n]  exp(-i pi j^2 / n)
     const cplx *bhat_m; // [M]  digit-reversed FFT of the wrapped exp(+i pi d^2/n), times 1/M   (forward DFT, sign -)
@@ -34,9 +35,10 @@ struct FftTab {
 struct RwTab {
     int L;                 // band-limit of the grid; 0: not available (tiny grids use the Bluestein kernel)
     FftTab fft;            // M = M2, twiddles only
-    const cplx *That;      // [M2] spectrum of T(d) = 1/sin(pi d/n) (digit-reversed order), times 1/(n M2)
-    const cplx *Ghat;      // [M2] spectrum of H(d + L - 1) times the reversal phase, times 1/(n M2)
-    const int *negpos;     // [M2] position of frequency -k given the position of frequency k
+    int npairs;            // M2/2 + 1 pairs of positions (p, p') holding frequencies (k, -k) in the transform's order
+    const int2 *pairs;     // [npairs]
+    const cplx *TG;        // [npairs][4]: That(p), Ghat(p), That(p'), Ghat(p') -- spectra of T(d) = 1/sin(pi d/n) and of
+                           // H(d + L - 1) times the reversal phase, both times 1/(n M2)
     const double *delta;   // [L] c_t - c_{n-1-t}
     const double *dsum;    // [L] (K_tt + K_{n-1-t,n-1-t}) / n
     const double *vpole;   // [2][L] pole column per parity (sigma = +1, -1), / n
@@ -124,9 +126,24 @@ __device__ __forceinline__ void twiddle_powers(cplx w1, cplx (&w)[R])
     }
 }
 
+// Two-level twiddle table in shared memory: W^k = W^{(k >> twlo) << twlo} W^{k & (2^twlo - 1)}, at most 128 + 64 entries
+// (3 KB) copied from the global table at kernel start, so no pass waits on a global load.
+#define S2W_TW_SMEM 192
+__device__ __forceinline__ void tw_stage(cplx *stw, const FftTab &T)
+{
+    const int nh = (T.twmask + 1) >> T.twlo, nl = 1 << T.twlo;
+    for (int i = threadIdx.x; i < nh; i += blockDim.x) stw[i] = T.tw[i << T.twlo];
+    for (int i = threadIdx.x; i < nl; i += blockDim.x) stw[nh + i] = T.tw[i];
+}
+__device__ __forceinline__ cplx tw_lookup(const cplx *stw, const FftTab &T, int k)
+{
+    const int nh = (T.twmask + 1) >> T.twlo;
+    return cmul(stw[k >> T.twlo], stw[nh + (k & ((1 << T.twlo) - 1))]);
+}
+
 // One decimation-in-frequency pass on sub-transforms of size S (radix R): butterflies, then twiddles W_S^{i j}.
 template <int R>
-__device__ __forceinline__ void dif_pass(cplx *buf, int M, int logS, const FftTab &T)
+__device__ __forceinline__ void dif_pass(cplx *buf, int M, int logS, const FftTab &T, const cplx *stw)
 {
     const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
     const int s = 1 << logs;
@@ -139,7 +156,7 @@ __device__ __forceinline__ void dif_pass(cplx *buf, int M, int logS, const FftTa
         for (int k = 0; k < R; ++k) v[k] = buf[S2W_PAD(base + (k << logs))];
         Bfly<R, false>::run(v);
         cplx w[R];
-        twiddle_powers<R>(__ldg(&T.tw[(i * twm) & T.twmask]), w);
+        twiddle_powers<R>(tw_lookup(stw, T, (i * twm) & T.twmask), w);
 #pragma unroll
         for (int j = 1; j < R; ++j) v[j] = cmul(v[j], w[j]);
 #pragma unroll
@@ -149,7 +166,7 @@ __device__ __forceinline__ void dif_pass(cplx *buf, int M, int logS, const FftTa
 
 // The matching decimation-in-time inverse pass: conjugate twiddles, then inverse butterflies.
 template <int R>
-__device__ __forceinline__ void dit_pass(cplx *buf, int M, int logS, const FftTab &T)
+__device__ __forceinline__ void dit_pass(cplx *buf, int M, int logS, const FftTab &T, const cplx *stw)
 {
     const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
     const int s = 1 << logs;
@@ -161,7 +178,7 @@ __device__ __forceinline__ void dit_pass(cplx *buf, int M, int logS, const FftTa
 #pragma unroll
         for (int k = 0; k < R; ++k) v[k] = buf[S2W_PAD(base + (k << logs))];
         cplx w[R];
-        twiddle_powers<R>(__ldg(&T.tw[(i * twm) & T.twmask]), w);
+        twiddle_powers<R>(tw_lookup(stw, T, (i * twm) & T.twmask), w);
 #pragma unroll
         for (int j = 1; j < R; ++j) v[j] = cmulc(v[j], w[j]);
         Bfly<R, true>::run(v);
@@ -190,7 +207,7 @@ __device__ __forceinline__ void mid_pass(cplx *buf, int M, const cplx *__restric
 // Batched variants: nb transforms of length M stored bstride elements apart in one shared-memory buffer; one pass
 // works on all of them between two barriers.
 template <int R>
-__device__ __forceinline__ void dif_pass_b(cplx *buf, int M, int logS, const FftTab &T, int nb, int bstride)
+__device__ __forceinline__ void dif_pass_b(cplx *buf, int M, int logS, const FftTab &T, const cplx *stw, int nb, int bstride)
 {
     const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
     const int s = 1 << logs;
@@ -206,7 +223,7 @@ __device__ __forceinline__ void dif_pass_b(cplx *buf, int M, int logS, const Fft
         for (int k = 0; k < R; ++k) v[k] = b[S2W_PAD(base + (k << logs))];
         Bfly<R, false>::run(v);
         cplx w[R];
-        twiddle_powers<R>(__ldg(&T.tw[(i * twm) & T.twmask]), w);
+        twiddle_powers<R>(tw_lookup(stw, T, (i * twm) & T.twmask), w);
 #pragma unroll
         for (int j = 1; j < R; ++j) v[j] = cmul(v[j], w[j]);
 #pragma unroll
@@ -215,7 +232,7 @@ __device__ __forceinline__ void dif_pass_b(cplx *buf, int M, int logS, const Fft
 }
 
 template <int R>
-__device__ __forceinline__ void dit_pass_b(cplx *buf, int M, int logS, const FftTab &T, int nb, int bstride)
+__device__ __forceinline__ void dit_pass_b(cplx *buf, int M, int logS, const FftTab &T, const cplx *stw, int nb, int bstride)
 {
     const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
     const int s = 1 << logs;
@@ -230,7 +247,7 @@ __device__ __forceinline__ void dit_pass_b(cplx *buf, int M, int logS, const Fft
 #pragma unroll
         for (int k = 0; k < R; ++k) v[k] = b[S2W_PAD(base + (k << logs))];
         cplx w[R];
-        twiddle_powers<R>(__ldg(&T.tw[(i * twm) & T.twmask]), w);
+        twiddle_powers<R>(tw_lookup(stw, T, (i * twm) & T.twmask), w);
 #pragma unroll
         for (int j = 1; j < R; ++j) v[j] = cmulc(v[j], w[j]);
         Bfly<R, true>::run(v);
@@ -240,73 +257,73 @@ __device__ __forceinline__ void dit_pass_b(cplx *buf, int M, int logS, const Fft
 }
 
 // nb forward transforms, natural in, digit-reversed out (radix 8 ... 8, then 4 or 2).  Ends with a barrier.
-__device__ inline void fft_dif_full_b(cplx *buf, const FftTab &T, int nb, int bstride)
+__device__ inline void fft_dif_full_b(cplx *buf, const FftTab &T, const cplx *stw, int nb, int bstride)
 {
     const int M = T.M;
     int logS = T.logM;
     while (logS >= 3) {
-        dif_pass_b<8>(buf, M, logS, T, nb, bstride);
+        dif_pass_b<8>(buf, M, logS, T, stw, nb, bstride);
         __syncthreads();
         logS -= 3;
     }
     if (logS == 2) {
-        dif_pass_b<4>(buf, M, 2, T, nb, bstride);
+        dif_pass_b<4>(buf, M, 2, T, stw, nb, bstride);
         __syncthreads();
     } else if (logS == 1) {
-        dif_pass_b<2>(buf, M, 1, T, nb, bstride);
+        dif_pass_b<2>(buf, M, 1, T, stw, nb, bstride);
         __syncthreads();
     }
 }
 
 // the matching inverse: digit-reversed in, natural out, unscaled.  Ends with a barrier.
-__device__ inline void fft_dit_full_b(cplx *buf, const FftTab &T, int nb, int bstride)
+__device__ inline void fft_dit_full_b(cplx *buf, const FftTab &T, const cplx *stw, int nb, int bstride)
 {
     const int M = T.M;
     int logS = T.logM % 3;
     if (logS == 2) {
-        dit_pass_b<4>(buf, M, 2, T, nb, bstride);
+        dit_pass_b<4>(buf, M, 2, T, stw, nb, bstride);
         __syncthreads();
     } else if (logS == 1) {
-        dit_pass_b<2>(buf, M, 1, T, nb, bstride);
+        dit_pass_b<2>(buf, M, 1, T, stw, nb, bstride);
         __syncthreads();
     }
     logS += 3;
     while (logS <= T.logM) {
-        dit_pass_b<8>(buf, M, logS, T, nb, bstride);
+        dit_pass_b<8>(buf, M, logS, T, stw, nb, bstride);
         __syncthreads();
         logS += 3;
     }
 }
 
 // Forward transform only (used once per table at plan creation): natural in, digit-reversed out.
-__device__ inline void fft_dif_full(cplx *buf, const FftTab &T)
+__device__ inline void fft_dif_full(cplx *buf, const FftTab &T, const cplx *stw)
 {
     const int M = T.M;
     int logS = T.logM;
     while (logS >= 3) {
-        dif_pass<8>(buf, M, logS, T);
+        dif_pass<8>(buf, M, logS, T, stw);
         __syncthreads();
         logS -= 3;
     }
     if (logS == 2) {
-        dif_pass<4>(buf, M, 2, T);
+        dif_pass<4>(buf, M, 2, T, stw);
         __syncthreads();
     } else if (logS == 1) {
-        dif_pass<2>(buf, M, 1, T);
+        dif_pass<2>(buf, M, 1, T, stw);
         __syncthreads();
     }
 }
 
 // buf <- circular convolution (length M) of buf with the kernel whose digit-reversed, 1/M-scaled spectrum is khat.
 // Ends with a __syncthreads().  Requires a __syncthreads() after the caller's writes to buf.
-__device__ inline void fft_convolve(cplx *buf, const FftTab &T, const cplx *__restrict__ khat)
+__device__ inline void fft_convolve(cplx *buf, const FftTab &T, const cplx *stw, const cplx *__restrict__ khat)
 {
     const int M = T.M;
     const int r = T.logM % 3;
     const int logMid = (r == 0) ? 3 : r;  // innermost group: 8, 2 or 4 elements
     int logS = T.logM;
     while (logS > logMid) {
-        dif_pass<8>(buf, M, logS, T);
+        dif_pass<8>(buf, M, logS, T, stw);
         __syncthreads();
         logS -= 3;
     }
@@ -319,7 +336,7 @@ __device__ inline void fft_convolve(cplx *buf, const FftTab &T, const cplx *__re
     __syncthreads();
     logS = logMid + 3;
     while (logS <= T.logM) {
-        dit_pass<8>(buf, M, logS, T);
+        dit_pass<8>(buf, M, logS, T, stw);
         __syncthreads();
         logS += 3;
     }

@@ -387,6 +387,7 @@ int build_rw(s2w_plan *p, GridTab &g)
     T.tw = p->tw;
     T.twmul = p->Mtab / M2;
     T.twmask = p->Mtab - 1;
+    T.twlo = std::min(6, ceil_log2(p->Mtab));
     // spectra in the transform's own (digit-reversed) order, and that order itself from the transform of e_1
     std::vector<cplx> hbuf((size_t)3 * M2, cmake(0.0, 0.0));
     for (int i = 0; i < M2; ++i) {
@@ -423,17 +424,29 @@ int build_rw(s2w_plan *p, GridTab &g)
         const cplx gq = hbuf[(size_t)M2 + q];
         hbuf[(size_t)M2 + q] = cmake((double)(gq.x * pr - gq.y * pi_), (double)(gq.x * pi_ + gq.y * pr));
     }
-    S2W_CUDA_CHECK(cudaMemcpy(dbuf, hbuf.data(), (size_t)2 * M2 * sizeof(cplx), cudaMemcpyHostToDevice));
-    g.rw.That = dbuf;
-    g.rw.Ghat = dbuf + M2;
-    int *dneg;
+    std::vector<int2> pairs;
+    std::vector<cplx> tg;
+    for (int q = 0; q < M2; ++q) {
+        const int qn = negpos[q];
+        if (qn < q) continue;
+        pairs.push_back(make_int2(q, qn));
+        tg.push_back(hbuf[q]);
+        tg.push_back(hbuf[(size_t)M2 + q]);
+        tg.push_back(hbuf[qn]);
+        tg.push_back(hbuf[(size_t)M2 + qn]);
+    }
+    int2 *dpairs;
+    cplx *dtg;
     double *dd, *ds, *dv, *dr;
-    if ((rc = p->pool.upload(&dneg, negpos))) return rc;
+    if ((rc = p->pool.upload(&dpairs, pairs))) return rc;
+    if ((rc = p->pool.upload(&dtg, tg))) return rc;
+    g.rw.npairs = (int)pairs.size();
+    g.rw.pairs = dpairs;
+    g.rw.TG = dtg;
     if ((rc = p->pool.upload(&dd, H.delta))) return rc;
     if ((rc = p->pool.upload(&ds, H.dsum))) return rc;
     if ((rc = p->pool.upload(&dv, H.vpole))) return rc;
     if ((rc = p->pool.upload(&dr, H.rpole))) return rc;
-    g.rw.negpos = dneg;
     g.rw.delta = dd;
     g.rw.dsum = ds;
     g.rw.vpole = dv;
@@ -456,6 +469,7 @@ int build_grid(s2w_plan *p, int Lg)
     T.tw = p->tw;
     T.twmul = p->Mtab / T.M;
     T.twmask = p->Mtab - 1;
+    T.twlo = std::min(6, ceil_log2(p->Mtab));
     cplx *chirp, *i1, *o1, *i3, *o3, *bm, *bp, *wh;
     int rc;
     if ((rc = p->pool.alloc(&chirp, T.n))) return rc;

@@ -29,10 +29,12 @@ __device__ __forceinline__ cplx cis_2pi_frac(int num, int den)  // exp(2 pi i nu
 //                              Complex: one block per row, out[row][m+L-1].
 // ---------------------------------------------------------------------------------------------------------------
 template <bool REAL>
-__global__ void __launch_bounds__(256) ring_fwd_kernel(const void *__restrict__ in, cplx *__restrict__ out, int nrows,
+__global__ void __launch_bounds__(256, 3) ring_fwd_kernel(const void *__restrict__ in, cplx *__restrict__ out, int nrows,
                                                       size_t sig_stride, FftTab T)
 {
     extern __shared__ cplx buf[];
+    __shared__ cplx s_tw[S2W_TW_SMEM];
+    tw_stage(s_tw, T);
     const int n = T.n, L = T.L, M = T.M;
     const double inv_n = 1.0 / (double)n;
     if (REAL) {
@@ -46,7 +48,7 @@ __global__ void __launch_bounds__(256) ring_fwd_kernel(const void *__restrict__ 
             buf[S2W_PAD(p)] = v;
         }
         __syncthreads();
-        fft_convolve(buf, T, T.bhat_m);
+        fft_convolve(buf, T, s_tw, T.bhat_m);
         for (int k = threadIdx.x; k < n; k += blockDim.x) buf[S2W_PAD(k)] = cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k]));
         __syncthreads();
         for (int m = threadIdx.x; m < L; m += blockDim.x) {
@@ -64,7 +66,7 @@ __global__ void __launch_bounds__(256) ring_fwd_kernel(const void *__restrict__ 
             buf[S2W_PAD(p)] = v;
         }
         __syncthreads();
-        fft_convolve(buf, T, T.bhat_m);
+        fft_convolve(buf, T, s_tw, T.bhat_m);
         for (int mi = threadIdx.x; mi < n; mi += blockDim.x) {
             int m = mi - (L - 1);
             int k = m < 0 ? m + n : m;
@@ -77,10 +79,12 @@ __global__ void __launch_bounds__(256) ring_fwd_kernel(const void *__restrict__ 
 // a1 inverse: F_m -> pixels, f = sum_m F_m e^{i m phi_p}.
 // ---------------------------------------------------------------------------------------------------------------
 template <bool REAL>
-__global__ void __launch_bounds__(256) ring_inv_kernel(const cplx *__restrict__ in, void *__restrict__ out, int nrows,
+__global__ void __launch_bounds__(256, 3) ring_inv_kernel(const cplx *__restrict__ in, void *__restrict__ out, int nrows,
                                                       size_t sig_stride, FftTab T)
 {
     extern __shared__ cplx buf[];
+    __shared__ cplx s_tw[S2W_TW_SMEM];
+    tw_stage(s_tw, T);
     const int n = T.n, L = T.L, M = T.M;
     if (REAL) {
         const int r0 = 2 * blockIdx.x, r1 = r0 + 1;
@@ -102,7 +106,7 @@ __global__ void __launch_bounds__(256) ring_inv_kernel(const cplx *__restrict__ 
             buf[S2W_PAD(k)] = v;
         }
         __syncthreads();
-        fft_convolve(buf, T, T.bhat_p);
+        fft_convolve(buf, T, s_tw, T.bhat_p);
         double *y0 = (double *)out + (size_t)(r0 / L) * sig_stride + (size_t)(r0 % L) * n;
         double *y1 = (double *)out + (size_t)(r1 / L) * sig_stride + (size_t)(r1 % L) * n;
         for (int p = threadIdx.x; p < n; p += blockDim.x) {
@@ -122,7 +126,7 @@ __global__ void __launch_bounds__(256) ring_inv_kernel(const cplx *__restrict__ 
             buf[S2W_PAD(k)] = v;
         }
         __syncthreads();
-        fft_convolve(buf, T, T.bhat_p);
+        fft_convolve(buf, T, s_tw, T.bhat_p);
         cplx *y0 = (cplx *)out + (size_t)(r0 / L) * sig_stride + (size_t)(r0 % L) * n;
         for (int p = threadIdx.x; p < n; p += blockDim.x) y0[p] = cmulc(buf[S2W_PAD(p)], __ldg(&T.chirp[p]));
     }
@@ -134,10 +138,12 @@ __global__ void __launch_bounds__(256) ring_inv_kernel(const cplx *__restrict__ 
 //       W = sum_{n>=0} c_n Re(e^{i n gamma_g} V_n), c_0 = 1, c_n = 2.
 // ---------------------------------------------------------------------------------------------------------------
 template <bool REAL>
-__global__ void __launch_bounds__(256) so3_inv_kernel(const cplx *__restrict__ F, void *__restrict__ W, size_t sig_stride,
+__global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict__ F, void *__restrict__ W, size_t sig_stride,
                                                      So3Args A, FftTab T)
 {
     extern __shared__ cplx buf[];
+    __shared__ cplx s_tw[S2W_TW_SMEM];
+    tw_stage(s_tw, T);
     const int n = T.n, L = T.L, M = T.M;
     const int t = blockIdx.x, b = blockIdx.y;
     const int Md = REAL ? L : n;
@@ -165,22 +171,36 @@ __global__ void __launch_bounds__(256) so3_inv_kernel(const cplx *__restrict__ F
             buf[S2W_PAD(k)] = v;
         }
         __syncthreads();
-        fft_convolve(buf, T, T.bhat_p);
-        for (int g = 0; g < ng; ++g) {
-            cplx ph = gph[g];
+        fft_convolve(buf, T, s_tw, T.bhat_p);
+        // one pass over alpha: the chirp product once, then all gamma planes with their loads issued together
+        for (int a = threadIdx.x; a < n; a += blockDim.x) {
+            const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
             if (REAL) {
-                double *Wr = (double *)W + (size_t)b * sig_stride + ((size_t)g * L + t) * n;
+                double *Wr = (double *)W + (size_t)b * sig_stride + (size_t)t * n + a;
                 const double cn = nv == 0 ? 1.0 : 2.0;
-                for (int a = threadIdx.x; a < n; a += blockDim.x) {
-                    cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
-                    double val = cn * (ph.x * v.x - ph.y * v.y);
-                    Wr[a] = first ? val : Wr[a] + val;
+                const double vx = cn * v.x, vy = cn * v.y;
+                for (int g0 = 0; g0 < ng; g0 += 9) {
+                    double old[9];
+#pragma unroll
+                    for (int k = 0; k < 9; ++k)
+                        old[k] = (!first && g0 + k < ng) ? Wr[(size_t)(g0 + k) * L * n] : 0.0;
+#pragma unroll
+                    for (int k = 0; k < 9; ++k)
+                        if (g0 + k < ng) {
+                            const cplx ph = gph[g0 + k];
+                            Wr[(size_t)(g0 + k) * L * n] = old[k] + (ph.x * vx - ph.y * vy);
+                        }
                 }
             } else {
-                cplx *Wc = (cplx *)W + (size_t)b * sig_stride + ((size_t)g * L + t) * n;
-                for (int a = threadIdx.x; a < n; a += blockDim.x) {
-                    cplx v = cmul(ph, cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a])));
-                    Wc[a] = first ? v : cadd(Wc[a], v);
+                cplx *Wc = (cplx *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+                for (int g0 = 0; g0 < ng; g0 += 5) {
+                    cplx old[5];
+#pragma unroll
+                    for (int k = 0; k < 5; ++k)
+                        old[k] = (!first && g0 + k < ng) ? Wc[(size_t)(g0 + k) * L * n] : cmake(0.0, 0.0);
+#pragma unroll
+                    for (int k = 0; k < 5; ++k)
+                        if (g0 + k < ng) Wc[(size_t)(g0 + k) * L * n] = cadd(old[k], cmul(gph[g0 + k], v));
                 }
             }
         }
@@ -195,10 +215,12 @@ __global__ void __launch_bounds__(256) so3_inv_kernel(const cplx *__restrict__ F
 // Real: rows n >= 0; the row of -n follows from F_{m,-n} = conj(F_{-m,n}).
 // ---------------------------------------------------------------------------------------------------------------
 template <bool REAL>
-__global__ void __launch_bounds__(256) so3_fwd_kernel(const void *__restrict__ W, cplx *__restrict__ F, size_t sig_stride,
+__global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict__ W, cplx *__restrict__ F, size_t sig_stride,
                                                      So3Args A, FftTab T)
 {
     extern __shared__ cplx buf[];
+    __shared__ cplx s_tw[S2W_TW_SMEM];
+    tw_stage(s_tw, T);
     const int n = T.n, L = T.L, M = T.M;
     const int t = blockIdx.x, b = blockIdx.y;
     const int Md = REAL ? L : n;
@@ -214,15 +236,30 @@ __global__ void __launch_bounds__(256) so3_fwd_kernel(const void *__restrict__ W
         for (int a = threadIdx.x; a < M; a += blockDim.x) {
             cplx v = cmake(0.0, 0.0);
             if (a < n) {
-                for (int g = 0; g < ng; ++g) {
-                    cplx ph = gph[g];
-                    if (REAL) {
-                        double w = ((const double *)W)[(size_t)b * sig_stride + ((size_t)g * L + t) * n + a];
-                        v.x = fma(ph.x, w, v.x);
-                        v.y = fma(ph.y, w, v.y);
-                    } else {
-                        cplx w = ((const cplx *)W)[(size_t)b * sig_stride + ((size_t)g * L + t) * n + a];
-                        v = cadd(v, cmul(ph, w));
+                if (REAL) {
+                    const double *Wr = (const double *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+                    for (int g0 = 0; g0 < ng; g0 += 9) {
+                        double wv[9];
+#pragma unroll
+                        for (int k = 0; k < 9; ++k) wv[k] = g0 + k < ng ? Wr[(size_t)(g0 + k) * L * n] : 0.0;
+#pragma unroll
+                        for (int k = 0; k < 9; ++k)
+                            if (g0 + k < ng) {
+                                const cplx ph = gph[g0 + k];
+                                v.x = fma(ph.x, wv[k], v.x);
+                                v.y = fma(ph.y, wv[k], v.y);
+                            }
+                    }
+                } else {
+                    const cplx *Wc = (const cplx *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+                    for (int g0 = 0; g0 < ng; g0 += 5) {
+                        cplx wv[5];
+#pragma unroll
+                        for (int k = 0; k < 5; ++k)
+                            wv[k] = g0 + k < ng ? Wc[(size_t)(g0 + k) * L * n] : cmake(0.0, 0.0);
+#pragma unroll
+                        for (int k = 0; k < 5; ++k)
+                            if (g0 + k < ng) v = cadd(v, cmul(gph[g0 + k], wv[k]));
                     }
                 }
                 v = cmul(cscale(v, inv_ng), __ldg(&T.chirp[a]));
@@ -230,7 +267,7 @@ __global__ void __launch_bounds__(256) so3_fwd_kernel(const void *__restrict__ W
             buf[S2W_PAD(a)] = v;
         }
         __syncthreads();
-        fft_convolve(buf, T, T.bhat_m);
+        fft_convolve(buf, T, s_tw, T.bhat_m);
         cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * Md;
         cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * Md;
         if (REAL) {
@@ -267,6 +304,8 @@ __global__ void __launch_bounds__(256) so3_fwd_kernel(const void *__restrict__ W
 __global__ void __launch_bounds__(256) reweight_kernel(cplx *__restrict__ F, RwArgs A, FftTab T)
 {
     extern __shared__ cplx buf[];
+    __shared__ cplx s_tw[S2W_TW_SMEM];
+    tw_stage(s_tw, T);
     const int n = T.n, L = T.L, M = T.M;
     const int mi = blockIdx.x, q = blockIdx.y, b = blockIdx.z;
     const int m = A.isReal ? mi : mi - (L - 1);
@@ -282,15 +321,15 @@ __global__ void __launch_bounds__(256) reweight_kernel(cplx *__restrict__ F, RwA
         buf[S2W_PAD(t)] = v;
     }
     __syncthreads();
-    fft_convolve(buf, T, T.bhat_p);
+    fft_convolve(buf, T, s_tw, T.bhat_p);
     for (int i = threadIdx.x; i < M; i += blockDim.x)
         buf[S2W_PAD(i)] = i < n ? cmul(buf[S2W_PAD(i)], __ldg(&T.rw_out1[i])) : cmake(0.0, 0.0);
     __syncthreads();
-    fft_convolve(buf, T, T.what);
+    fft_convolve(buf, T, s_tw, T.what);
     for (int i = threadIdx.x; i < M; i += blockDim.x)
         buf[S2W_PAD(i)] = i < n ? cmul(buf[S2W_PAD(i)], __ldg(&T.rw_in3[i])) : cmake(0.0, 0.0);
     __syncthreads();
-    fft_convolve(buf, T, T.bhat_m);
+    fft_convolve(buf, T, s_tw, T.bhat_m);
     for (int t = threadIdx.x; t < L; t += blockDim.x) {
         cplx g0 = cmul(buf[S2W_PAD(t)], __ldg(&T.rw_out3[t]));
         if (t < L - 1) {
@@ -316,9 +355,11 @@ __global__ void __launch_bounds__(256) reweight_kernel(cplx *__restrict__ F, RwA
 // accurate (2e-16 at L = 1024).  One block per column; both sequences go through each FFT pass together.
 // ---------------------------------------------------------------------------------------------------------------
 #define RW_MAXPT 8  // ring values a thread keeps in registers (L <= 8 * blockDim)
-__global__ void __launch_bounds__(256) reweight_th_kernel(cplx *__restrict__ F, RwArgs A, RwTab R)
+__global__ void __launch_bounds__(256, 3) reweight_th_kernel(cplx *__restrict__ F, RwArgs A, RwTab R)
 {
     extern __shared__ cplx buf[];
+    __shared__ cplx s_tw[S2W_TW_SMEM];
+    tw_stage(s_tw, R.fft);
     __shared__ cplx s_part[8];
     __shared__ cplx s_pole[2];
     const FftTab &T = R.fft;
@@ -370,13 +411,13 @@ __global__ void __launch_bounds__(256) reweight_th_kernel(cplx *__restrict__ F, 
     }
     if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = dot;
     __syncthreads();
-    fft_dif_full_b(buf, T, 2, bstride);
+    fft_dif_full_b(buf, T, s_tw, 2, bstride);
     // spectra of T u -/+ sigma H u: Y(k) = That(k) U(k) -/+ sigma Ghat(k) U(-k)
-    for (int p = threadIdx.x; p < M; p += blockDim.x) {
-        const int pn = __ldg(&R.negpos[p]);
-        if (pn < p) continue;
-        const cplx tp = __ldg(&R.That[p]), gp = cscale(__ldg(&R.Ghat[p]), sigma);
-        const cplx tn = __ldg(&R.That[pn]), gn = cscale(__ldg(&R.Ghat[pn]), sigma);
+    for (int i = threadIdx.x; i < R.npairs; i += blockDim.x) {
+        const int2 pp = __ldg(&R.pairs[i]);
+        const int p = pp.x, pn = pp.y;
+        const cplx tp = __ldg(&R.TG[4 * i]), gp = cscale(__ldg(&R.TG[4 * i + 1]), sigma);
+        const cplx tn = __ldg(&R.TG[4 * i + 2]), gn = cscale(__ldg(&R.TG[4 * i + 3]), sigma);
         const cplx u1p = b1[S2W_PAD(p)], u1n = b1[S2W_PAD(pn)], u2p = b2[S2W_PAD(p)], u2n = b2[S2W_PAD(pn)];
         b1[S2W_PAD(p)] = csub(cmul(tp, u1p), cmul(gp, u1n));
         b2[S2W_PAD(p)] = cadd(cmul(tp, u2p), cmul(gp, u2n));
@@ -386,7 +427,7 @@ __global__ void __launch_bounds__(256) reweight_th_kernel(cplx *__restrict__ F, 
         }
     }
     __syncthreads();
-    fft_dit_full_b(buf, T, 2, bstride);
+    fft_dit_full_b(buf, T, s_tw, 2, bstride);
     const cplx xpole = s_pole[0];
 #pragma unroll
     for (int k = 0; k < RW_MAXPT; ++k) {
@@ -411,9 +452,11 @@ __global__ void __launch_bounds__(256) reweight_th_kernel(cplx *__restrict__ F, 
 __global__ void __launch_bounds__(256) fft_forward_kernel(cplx *data, FftTab T)
 {
     extern __shared__ cplx buf[];
+    __shared__ cplx s_tw[S2W_TW_SMEM];
+    tw_stage(s_tw, T);
     for (int e = threadIdx.x; e < T.M; e += blockDim.x) buf[S2W_PAD(e)] = data[e];
     __syncthreads();
-    fft_dif_full(buf, T);
+    fft_dif_full(buf, T, s_tw);
     for (int e = threadIdx.x; e < T.M; e += blockDim.x) data[e] = buf[S2W_PAD(e)];
 }
 
@@ -461,6 +504,8 @@ __global__ void chirp_kernel(cplx *chirp, cplx *rw_in1, cplx *rw_out1, cplx *rw_
 __global__ void __launch_bounds__(256) kernel_spectrum_kernel(cplx *khat, int kind, FftTab T)
 {
     extern __shared__ cplx buf[];
+    __shared__ cplx s_tw[S2W_TW_SMEM];
+    tw_stage(s_tw, T);
     const int n = T.n, M = T.M;
     const double invM = 1.0 / (double)M;
     for (int e = threadIdx.x; e < M; e += blockDim.x) buf[S2W_PAD(e)] = cmake(0.0, 0.0);
@@ -487,7 +532,7 @@ __global__ void __launch_bounds__(256) kernel_spectrum_kernel(cplx *khat, int ki
         buf[S2W_PAD(slot)] = cscale(v, invM);
     }
     __syncthreads();
-    fft_dif_full(buf, T);
+    fft_dif_full(buf, T, s_tw);
     for (int e = threadIdx.x; e < M; e += blockDim.x) khat[e] = buf[S2W_PAD(e)];
 }
 
