@@ -40,7 +40,9 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4"])
+    ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--precompute", action="store_true",
+                    help="sphere workloads: the precomputed-kernel variant (S2W_PRECOMPUTE, step a9)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -253,7 +255,8 @@ def workload_config(cfg, args):
                         % (cfg["name"], cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"],
                            "real" if cfg["real"] else "complex", cfg["batch"]),
             "L": cfg["L"], "N": cfg["N"], "lambda": cfg["lam"], "J0": cfg["J0"], "multiresolution": cfg["multires"],
-            "batch_per_gpu": cfg["batch"], "mode": "on-the-fly Wigner recursion",
+            "batch_per_gpu": cfg["batch"],
+            "mode": "precomputed Wigner-d table (DMMA)" if getattr(args, "precompute", False) else "on-the-fly Wigner recursion",
             "parallelism": "replicas x%d (no data-path collective)" % args.gpus,
             "l2": "coefficient block per step (%.2f GB) exceeds the 126 MB L2; no explicit flush" % cfg.get("coeff_gb", 0.0)}
 
@@ -307,7 +310,8 @@ def run_ours(args, cfg):
 
     L, N, lam, J0, mr, real, B = cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"], cfg["real"], cfg["batch"]
     f = make_signals(cfg, api, torch, device, seed_offset=replica_seed_offset(rank))     # independent signals per replica
-    plan = api.s2wav_plan_create(L, N, lam, J0, mr, real, B, local)
+    plan = api.s2wav_plan_create(L, N, lam, J0, mr, real, B, local,
+                                 flags=api.S2W_PRECOMPUTE if args.precompute else 0)
     cfg["coeff_gb"] = plan.coeff_elems * B * (8 if real else 16) / 1e9
     w = torch.empty((B, plan.coeff_elems), dtype=plan.dtype, device=device)
     back = torch.empty((B, plan.signal_elems), dtype=plan.dtype, device=device)
@@ -350,17 +354,21 @@ def run_ours(args, cfg):
 
     # ---- end to end through the host-buffer C ABI calls (pinned memory; H2D + D2H inside) ----
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not args.precompute:
+        # pinned host buffers for the signals, the coefficients and the reconstruction
         fh = torch.empty(f.shape, dtype=f.dtype, pin_memory=True)
         fh.copy_(f)
         fh_np = fh.numpy()
-        api.s2wav_inverse_host(api.s2wav_forward_host(fh_np, L, N, lam, J0, mr), L, N, lam, J0, mr)  # warm-up
+        wh_np = torch.empty((B, plan.coeff_elems), dtype=f.dtype, pin_memory=True).numpy()
+        fb_np = torch.empty(f.shape, dtype=f.dtype, pin_memory=True).numpy()
+        api.s2wav_inverse_host(api.s2wav_forward_host(fh_np, L, N, lam, J0, mr, out=wh_np), L, N, lam, J0, mr,
+                               out=fb_np)  # warm-up (builds the cached plan and its staging buffers)
         barrier()
         nrep = max(1, min(args.steps, 3))
         t0 = time.perf_counter()
         for _ in range(nrep):
-            wh = api.s2wav_forward_host(fh_np, L, N, lam, J0, mr)
-            fb = api.s2wav_inverse_host(wh, L, N, lam, J0, mr)
+            wh = api.s2wav_forward_host(fh_np, L, N, lam, J0, mr, out=wh_np)
+            fb = api.s2wav_inverse_host(wh, L, N, lam, J0, mr, out=fb_np)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
         esz = 8 if real else 16
@@ -412,12 +420,135 @@ def run_ours(args, cfg):
         dist.destroy_process_group()
 
 
+# ---------------------------------------------------------------------------------------------------------------
+# ball workload (C5): one step = forward + inverse Fourier-Laguerre wavelet transform of one [P][L][2L-1] field
+# ---------------------------------------------------------------------------------------------------------------
+def ball_stages(cfg, api):
+    """[(Lg, n_list, lmin, shells)] of the contraction launches of one direction (Alg. 2): Z at (L, P), the scaling
+    part at (L, P), then every (j', j) with P_j' shells."""
+    L, P, N, lam, nu, J0 = cfg["L"], cfg["P"], cfg["N"], cfg["lam"], cfg["nu"], cfg["J0"]
+    kl = api.s2ball_kernels(L, P, N, lam, nu, J0)["kappa_l"]
+    J, Jp = api.s2w_scale_count(L, lam), api.s2w_scale_count(P, nu)
+
+    def bl(base, e, cap):
+        return int(min(int(np.ceil(base ** e - 1e-9)), cap))
+    stages = [(L, [0], 0, P), (L, [0], 0, P)]
+    for jp in range(J0, Jp + 1):
+        Pj = bl(nu, jp + 1, P)
+        for j in range(J0, J + 1):
+            Lj = bl(lam, j + 1, L)
+            k = np.abs(kl[j - J0][:Lj])
+            nz = np.nonzero(k)[0]
+            ns = [n for n in range(-(N - 1), N, 2) if abs(n) < Lj]
+            if len(nz) and len(ns):
+                stages.append((Lj, ns, int(nz[0]), Pj))
+    return stages
+
+
+def run_ball(args, cfg):
+    import torch
+    from paper_2402_01282_b200 import api, inputs
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (there is no CPU fallback)")
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise RuntimeError("the ball workload is single-GPU (replicas only); run it with --gpus 1")
+    torch.cuda.set_device(0)
+    device = torch.device("cuda", 0)
+    L, P, N, lam, nu, J0, tau = cfg["L"], cfg["P"], cfg["N"], cfg["lam"], cfg["nu"], cfg["J0"], cfg["tau"]
+    plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau)
+    flmp = inputs.config_coefficients("C5")
+    f = plan.harmonic_inverse(torch.from_numpy(flmp).to(device).reshape(1, -1))
+    w = torch.empty((1, plan.coeff_elems), dtype=plan.dtype, device=device)
+    back = torch.empty((1, plan.signal_elems), dtype=plan.dtype, device=device)
+
+    def step():
+        plan.forward(f, out=w)
+        plan.inverse(w, out=back)
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    rt_err = float((back - f).abs().max() / f.abs().max())
+    sampler = ClockSampler(0)
+    sampler.start()
+    l0 = api.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    launches = api.launch_count() - l0
+    clocks = sampler.stop()
+    api.timing_enable(True)
+    api.timing_read()
+    ksteps = max(2, min(args.steps, 5))
+    for _ in range(ksteps):
+        step()
+    torch.cuda.synchronize()
+    classes = api.timing_read()
+    api.timing_enable(False)
+    # algorithmic flops of one contraction class: 5 per tuple (recursion) + 4 per tuple and complex column; a complex
+    # shell is 2 columns ((m,n) and (-m,-n))
+    flops = 0.0
+    for (Lg, ns, lmin, shells) in ball_stages(cfg, api):
+        flops += stage_tuples(Lg, ns, lmin, False) * (5.0 + 4.0 * 2 * shells)
+    dom = max(("wigner_inverse", "wigner_forward"), key=lambda k: classes[k][0])
+    dom_ms = classes[dom][0]
+    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+    peak = 148 * 64 * 2 * sm_max * 1e6 / 1e12
+    achieved = flops * ksteps / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+    e2e = None
+    if not args.no_e2e:
+        fh = torch.empty((P, L, 2 * L - 1), dtype=f.dtype, pin_memory=True)
+        fh.copy_(f.reshape(P, L, 2 * L - 1))
+        fh_np = fh.numpy()
+        wh_np = torch.empty(plan.coeff_elems, dtype=f.dtype, pin_memory=True).numpy()
+        fb_np = torch.empty((P, L, 2 * L - 1), dtype=f.dtype, pin_memory=True).numpy()
+        api.s2ball_inverse_host(api.s2ball_forward_host(fh_np, L, P, N, lam, nu, J0, tau, out=wh_np), L, P, N, lam, nu,
+                                J0, tau, out=fb_np)
+        t0 = time.perf_counter()
+        wh = api.s2ball_forward_host(fh_np, L, P, N, lam, nu, J0, tau, out=wh_np)
+        fb = api.s2ball_inverse_host(wh, L, P, N, lam, nu, J0, tau, out=fb_np)
+        dt = time.perf_counter() - t0
+        nbytes = (plan.signal_elems + plan.coeff_elems) * 16
+        e2e = {"value": 1.0 / dt, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+               "roundtrip_rel_err": float(np.abs(fb - fh_np).max() / np.abs(fh_np).max())}
+    total_kms = sum(v[0] for v in classes.values())
+    line = {
+        "metric": METRIC, "value": args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "C5: ball L=%d P=%d N=%d lambda_l=%g lambda_p=%g J0=%d tau=%g complex fp64, "
+                               "forward+inverse" % (L, P, N, lam, nu, J0, tau),
+                   "L": L, "P": P, "N": N, "parallelism": "replicas x1 (no data-path collective)",
+                   "l2": "coefficient block per step (%.2f GB) exceeds the 126 MB L2; no explicit flush"
+                         % (plan.coeff_elems * 16 / 1e9)},
+        "clocks": clocks, "gpu_launches": int(launches), "roundtrip_rel_err": rt_err,
+        "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                     "frac": achieved / peak if peak else None, "traffic": None,
+                     "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x sm_max_mhz (DESIGN.md)",
+                     "flops_per_step": flops, "ms_per_step": dom_ms / ksteps},
+        "kernel_ms_per_step": {k: round(v[0] / ksteps, 4) for k, v in classes.items()},
+        "kernel_share": {k: round(v[0] / total_kms, 4) for k, v in classes.items()} if total_kms else None,
+    }
+    if e2e:
+        line["e2e"] = e2e
+    print(json.dumps(line))
+
+
+
 def main():
     args = parse_args()
     from paper_2402_01282_b200 import inputs
     cfg = dict(inputs.CONFIGS[args.workload])
     cfg["name"] = args.workload
-    cfg["multires"] = cfg["multires"]
+    if cfg.get("kind") == "ball":
+        if args.impl == "reference":
+            raise SystemExit("--impl reference times the sphere workloads (the metric configuration is C3)")
+        run_ball(args, cfg)
+        return
     if args.impl == "reference":
         if int(os.environ.get("RANK", "0")) == 0:
             run_reference(args, cfg)

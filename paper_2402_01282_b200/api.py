@@ -310,24 +310,33 @@ def s2wav_inverse(w, L, N, lam, J0, multiresolution=True):
     return f
 
 
-def s2wav_forward_host(f, L, N, lam, J0, multiresolution=True):
+def _host_out(out, shape, dtype):
+    """Caller-provided output (e.g. a view of pinned memory: copies are then asynchronous DMA) or a fresh array."""
+    if out is None:
+        return np.empty(shape, dtype=dtype)
+    if out.dtype != dtype or out.size != int(np.prod(shape)) or not out.flags["C_CONTIGUOUS"]:
+        raise ValueError("out must be a C-contiguous %s array of %d elements" % (dtype, int(np.prod(shape))))
+    return out.reshape(shape)
+
+
+def s2wav_forward_host(f, L, N, lam, J0, multiresolution=True, out=None):
     """numpy in, numpy out; host<->device copies happen inside the library call."""
     f = np.ascontiguousarray(f)
     real = f.dtype == np.float64
     batch = f.size // (L * (2 * L - 1))
     K = _coeff_elems_sphere(L, N, lam, J0, multiresolution)
-    w = np.empty((batch, K), dtype=f.dtype)
+    w = _host_out(out, (batch, K), f.dtype)
     _check(lib().s2wav_forward_host(_np_ptr(f), _np_ptr(w), int(L), int(N), float(lam), int(J0),
                                     int(bool(multiresolution)), S2W_REAL if real else 0, batch))
     return w
 
 
-def s2wav_inverse_host(w, L, N, lam, J0, multiresolution=True):
+def s2wav_inverse_host(w, L, N, lam, J0, multiresolution=True, out=None):
     w = np.ascontiguousarray(w)
     real = w.dtype == np.float64
     K = _coeff_elems_sphere(L, N, lam, J0, multiresolution)
     batch = w.size // K
-    f = np.empty((batch, L, 2 * L - 1), dtype=w.dtype)
+    f = _host_out(out, (batch, L, 2 * L - 1), w.dtype)
     _check(lib().s2wav_inverse_host(_np_ptr(w), _np_ptr(f), int(L), int(N), float(lam), int(J0),
                                     int(bool(multiresolution)), S2W_REAL if real else 0, batch))
     return f
@@ -371,19 +380,19 @@ def s2ball_inverse(w, L, P, N, lam_l, lam_p, J0, tau=1.0):
     return f
 
 
-def s2ball_forward_host(f, L, P, N, lam_l, lam_p, J0, tau=1.0):
+def s2ball_forward_host(f, L, P, N, lam_l, lam_p, J0, tau=1.0, out=None):
     f = np.ascontiguousarray(f)
     real = f.dtype == np.float64
-    w = np.empty(_coeff_elems_ball(L, P, N, lam_l, lam_p, J0), dtype=f.dtype)
+    w = _host_out(out, (_coeff_elems_ball(L, P, N, lam_l, lam_p, J0),), f.dtype)
     _check(lib().s2ball_forward_host(_np_ptr(f), _np_ptr(w), int(L), int(P), int(N), float(lam_l), float(lam_p),
                                      int(J0), float(tau), S2W_REAL if real else 0))
     return w
 
 
-def s2ball_inverse_host(w, L, P, N, lam_l, lam_p, J0, tau=1.0):
+def s2ball_inverse_host(w, L, P, N, lam_l, lam_p, J0, tau=1.0, out=None):
     w = np.ascontiguousarray(w)
     real = w.dtype == np.float64
-    f = np.empty((P, L, 2 * L - 1), dtype=w.dtype)
+    f = _host_out(out, (P, L, 2 * L - 1), w.dtype)
     _check(lib().s2ball_inverse_host(_np_ptr(w), _np_ptr(f), int(L), int(P), int(N), float(lam_l), float(lam_p),
                                      int(J0), float(tau), S2W_REAL if real else 0))
     return f

@@ -1394,6 +1394,7 @@ struct CacheKey {
 struct CacheEntry {
     s2w_plan *plan;
     void *work;
+    void *d_sig, *d_cof;  // device staging buffers of the host-buffer entry points (allocated on first use)
 };
 std::map<CacheKey, CacheEntry> g_cache;
 std::mutex g_cache_mu;
@@ -1423,6 +1424,7 @@ int cached_plan(int kind, int L, int P, int N, double lambda, double nu, double 
         CacheEntry ne;
         ne.plan = 0;
         ne.work = 0;
+        ne.d_sig = ne.d_cof = 0;
         int rc = kind == 0 ? s2wav_plan_create(&ne.plan, L, N, lambda, J0, multires, flags, batch, device)
                            : s2ball_plan_create(&ne.plan, L, P, N, lambda, nu, J0, tau, flags, device);
         if (rc) return rc;
@@ -1439,7 +1441,32 @@ int cached_plan(int kind, int L, int P, int N, double lambda, double nu, double 
     return S2W_OK;
 }
 
-// host-buffer variant of a cached transform: copy in, transform, copy out, synchronise
+// as cached_plan, and makes sure the entry owns device staging buffers for one signal batch and one coefficient batch
+int cached_plan_staged(int kind, int L, int P, int N, double lambda, double nu, double tau, int J0, int multires,
+                       int flags, int batch, CacheEntry *e)
+{
+    int rc = cached_plan(kind, L, P, N, lambda, nu, tau, J0, multires, flags, batch, e);
+    if (rc || e->d_sig) return rc;
+    std::lock_guard<std::mutex> lock(g_cache_mu);
+    for (auto &kv : g_cache) {
+        if (kv.second.plan != e->plan) continue;
+        const size_t esz = e->plan->real ? sizeof(double) : sizeof(cplx);
+        const size_t sig = e->plan->signal_elems * e->plan->batch * esz, cof = e->plan->coeff_elems * e->plan->batch * esz;
+        if (cudaMalloc(&kv.second.d_sig, sig) != cudaSuccess || cudaMalloc(&kv.second.d_cof, cof) != cudaSuccess) {
+            cudaFree(kv.second.d_sig);
+            kv.second.d_sig = kv.second.d_cof = 0;
+            cudaGetLastError();
+            set_error("cudaMalloc(staging buffers) failed");
+            return S2W_ENOMEM;
+        }
+        *e = kv.second;
+        return S2W_OK;
+    }
+    return S2W_EINVAL;
+}
+
+// host-buffer variant of a cached transform: copy in, transform, copy out, synchronise.  Copies are asynchronous when
+// the host buffers are pinned (cudaHostAlloc / cudaHostRegister / torch pin_memory) and staged by the driver otherwise.
 int host_transform(bool fwd, const CacheEntry &e, const void *in_h, void *out_h)
 {
     if (!in_h || !out_h) {
@@ -1448,14 +1475,7 @@ int host_transform(bool fwd, const CacheEntry &e, const void *in_h, void *out_h)
     }
     const size_t esz = e.plan->real ? sizeof(double) : sizeof(cplx);
     const size_t sig = e.plan->signal_elems * e.plan->batch * esz, cof = e.plan->coeff_elems * e.plan->batch * esz;
-    void *d_in = 0, *d_out = 0;
-    S2W_CUDA_CHECK(cudaMalloc(&d_in, fwd ? sig : cof));
-    cudaError_t ce = cudaMalloc(&d_out, fwd ? cof : sig);
-    if (ce != cudaSuccess) {
-        cudaFree(d_in);
-        set_error("cudaMalloc failed");
-        return S2W_ENOMEM;
-    }
+    void *d_in = fwd ? e.d_sig : e.d_cof, *d_out = fwd ? e.d_cof : e.d_sig;
     int rc = S2W_OK;
     if (cudaMemcpyAsync(d_in, in_h, fwd ? sig : cof, cudaMemcpyHostToDevice, 0) != cudaSuccess) rc = S2W_ECUDA;
     if (!rc) rc = fwd ? s2w_plan_forward(e.plan, d_in, d_out, e.work, 0) : s2w_plan_inverse(e.plan, d_in, d_out, e.work, 0);
@@ -1464,8 +1484,6 @@ int host_transform(bool fwd, const CacheEntry &e, const void *in_h, void *out_h)
         set_error(std::string("stream sync: ") + cudaGetErrorString(cudaGetLastError()));
         rc = S2W_ECUDA;
     }
-    cudaFree(d_in);
-    cudaFree(d_out);
     return rc;
 }
 }  // namespace
@@ -1491,14 +1509,14 @@ int s2wav_inverse(const void *w, void *f, int L, int N, double lambda, int J0, i
 int s2wav_forward_host(const void *f, void *w, int L, int N, double lambda, int J0, int multires, int flags, int batch)
 {
     CacheEntry e;
-    int rc = cached_plan(0, L, 1, N, lambda, 0.0, 1.0, J0, multires, flags, batch, &e);
+    int rc = cached_plan_staged(0, L, 1, N, lambda, 0.0, 1.0, J0, multires, flags, batch, &e);
     if (rc) return rc;
     return host_transform(true, e, f, w);
 }
 int s2wav_inverse_host(const void *w, void *f, int L, int N, double lambda, int J0, int multires, int flags, int batch)
 {
     CacheEntry e;
-    int rc = cached_plan(0, L, 1, N, lambda, 0.0, 1.0, J0, multires, flags, batch, &e);
+    int rc = cached_plan_staged(0, L, 1, N, lambda, 0.0, 1.0, J0, multires, flags, batch, &e);
     if (rc) return rc;
     return host_transform(false, e, w, f);
 }
@@ -1524,7 +1542,7 @@ int s2ball_forward_host(const void *f, void *w, int L, int P, int N, double lamb
                         double tau, int flags)
 {
     CacheEntry e;
-    int rc = cached_plan(1, L, P, N, lambda_l, lambda_p, tau, J0, 1, flags, 1, &e);
+    int rc = cached_plan_staged(1, L, P, N, lambda_l, lambda_p, tau, J0, 1, flags, 1, &e);
     if (rc) return rc;
     return host_transform(true, e, f, w);
 }
@@ -1532,7 +1550,7 @@ int s2ball_inverse_host(const void *w, void *f, int L, int P, int N, double lamb
                         double tau, int flags)
 {
     CacheEntry e;
-    int rc = cached_plan(1, L, P, N, lambda_l, lambda_p, tau, J0, 1, flags, 1, &e);
+    int rc = cached_plan_staged(1, L, P, N, lambda_l, lambda_p, tau, J0, 1, flags, 1, &e);
     if (rc) return rc;
     return host_transform(false, e, w, f);
 }
@@ -1542,6 +1560,8 @@ int s2w_cache_clear(void)
     std::lock_guard<std::mutex> lock(g_cache_mu);
     for (auto &kv : g_cache) {
         cudaFree(kv.second.work);
+        cudaFree(kv.second.d_sig);
+        cudaFree(kv.second.d_cof);
         s2w_plan_destroy(kv.second.plan);
     }
     g_cache.clear();
