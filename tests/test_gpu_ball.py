@@ -120,3 +120,29 @@ def test_ball_real_signal_gives_real_coefficients():
     assert _relmax(back, fr) < RT_TOL
     pr.close()
     pc.close()
+
+
+def test_config5_full_size():
+    """BASELINE config 5 at full size (L = P = 128, N = 3, complex, 64 (j, j') scales): round trip on all voxels,
+    recovered f_lmp against the seeded truth, and two whole (j, j') coefficient blocks against the oracle."""
+    torch, api = _api()
+    c = inputs.CONFIGS["C5"]
+    L, P, N, lam, nu, J0, tau = c["L"], c["P"], c["N"], c["lam"], c["nu"], c["J0"], c["tau"]
+    flmp = inputs.config_coefficients("C5")
+    plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau)
+    f = plan.harmonic_inverse(torch.from_numpy(flmp).cuda().reshape(1, -1))
+    got = plan.harmonic_forward(f, P * L * (2 * L - 1)).cpu().numpy().reshape(P, L, 2 * L - 1)
+    assert _relmax(got, flmp) < FWD_TOL
+    w = plan.forward(f)
+    back = plan.inverse(w)
+    assert float((back - f).abs().max() / f.abs().max()) < RT_TOL
+    scal, scales = plan.split(w)
+    filt = OB.filters(L, P, N, lam, nu, J0, J0, "f80")
+    keys = [(4, 5), (6, 3)]
+    _, o_psi = OB.analysis_from_flmp(flmp, L, P, N, lam, nu, J0, J0, tau, "f80", filt, scales=keys)
+    for key in keys:
+        ref = o_psi[key].astype(np.complex128)
+        got = scales[key][0].cpu().numpy()
+        assert got.shape == ref.shape
+        assert _relmax(got, ref) < FWD_TOL, key
+    plan.close()

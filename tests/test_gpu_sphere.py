@@ -220,3 +220,27 @@ def test_config3_full_size_sampled_parity():
         den = float(scales[(j, 0)][1].abs().max())
         assert np.abs(got - ref).max() / den < FWD_TOL, j
     plan.close()
+
+
+def test_config4_band_limit_2048_seeds_and_sampled_rings():
+    """BASELINE config 4 grid (L = 2048, real): beyond L ~ 1930 the plain recursion seed underflows fp64,
+    so this exercises the range-extended group seeds.  Harmonic transforms: recovered f_lm against the seeded truth,
+    pixels of sampled rings (poles, mid-latitudes, the rings whose seeds underflow) against the long-double oracle,
+    and the wavelet round trip at N = 3, J0 = 4."""
+    torch, api = _api()
+    c = inputs.CONFIGS["C4"]
+    L, N, lam, J0 = c["L"], c["N"], c["lam"], c["J0"]
+    flm = inputs.config_coefficients("C4")
+    plan = api.s2wav_plan_create(L, N, lam, J0, True, True, 1)
+    f = plan.harmonic_inverse(torch.from_numpy(flm).cuda())
+    got_flm = plan.harmonic_forward(f, L * (2 * L - 1)).cpu().numpy().reshape(1, L, 2 * L - 1)
+    assert _relmax(got_flm, flm) < FWD_TOL
+    rings = [0, 1, 2, 156, 480, 1023, 1024, 1890, 2045, 2046, 2047]
+    th = S.mw_thetas(L, "f80")
+    ref = S.sht_inverse(flm[0], L, "f80", thetas=th[rings]).real.astype(np.float64)
+    fn = f.cpu().numpy().reshape(L, 2 * L - 1)
+    assert np.abs(fn[rings] - ref).max() / np.abs(fn).max() < RT_TOL
+    w = plan.forward(f)
+    back = plan.inverse(w)
+    assert float((back - f).abs().max() / f.abs().max()) < RT_TOL
+    plan.close()
