@@ -54,7 +54,8 @@ struct WigArgs {
     size_t tri_g;               // Lg (Lg + 1) / 2
     const cplx *filt;           // [nn][Lg] filter applied to row q at degree l
     cplx *flmT;                 // [B][Mfull][Lfull]  f_{l m} stored m-major; Mfull = Lfull (real) or 2 Lfull - 1
-    cplx *F;                    // [B][nrows][Lg][Md], Md = Lg (real) or 2 Lg - 1
+    cplx *F;                    // inverse direction: output [B][nrows][Lg][Md], Md = Lg (real) or 2 Lg - 1;
+                                // forward direction: input, transposed [B][nrows][Md][Lg]
 };
 
 void set_error(const std::string &msg);
@@ -71,8 +72,10 @@ int launch_so3_inv(bool real, const cplx *F, void *W, size_t sig_stride, const S
                    cudaStream_t st);
 int launch_so3_fwd(bool real, const void *W, size_t sig_stride, cplx *F, const So3Args &A, int batch, const FftTab &T,
                    cudaStream_t st);
-int launch_reweight(cplx *F, const RwArgs &A, int batch, const FftTab &T, cudaStream_t st);
-int launch_reweight_th(cplx *F, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st);   // L >= 8, L <= 2048
+// a2: reads F[b][row][t][mi], writes the reweighted columns TRANSPOSED, Ft[b][row][mi][t] (what the forward Wigner
+// contraction reads: ring data of one m contiguous)
+int launch_reweight(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const FftTab &T, cudaStream_t st);
+int launch_reweight_th(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st);   // L >= 8, L <= 2048
 int launch_fft_forward(cplx *data, const FftTab &T, cudaStream_t st);   // plan-time, in place, digit-reversed out
 
 // plan-time: group start degrees and seeds from the range-extended values d^{l0}_{mn}(beta_t) = mant 2^expo ([ntab][Lg m][Lg t])

@@ -723,7 +723,8 @@ int make_scale_stage(s2w_plan *p, Scale &sc, const double *kj, const std::vector
 
 struct Work {
     cplx *flmT;
-    cplx *F;
+    cplx *F;   // [B][n][t][m]
+    cplx *Ft;  // [B][n][m][t]: reweighted columns, input of the forward contraction
 };
 
 static Work carve(const s2w_plan *p, void *work)
@@ -731,6 +732,7 @@ static Work carve(const s2w_plan *p, void *work)
     Work w;
     w.flmT = (cplx *)work;
     w.F = w.flmT + ((p->ws_flm_elems + 15) / 16) * 16;
+    w.Ft = w.F + ((p->ws_F_elems + 15) / 16) * 16;
     return w;
 }
 
@@ -743,13 +745,13 @@ static int sht_forward_dev(const s2w_plan *p, const Stage &st, const void *f, si
     if ((rc = launch_ring_fwd(p->real, f, w.F, B, st.Lg, sig_stride, g.fft, s))) return rc;
     RwArgs R;
     fill_rw_args(p, st, R);
-    if ((rc = g.rw.L ? launch_reweight_th(w.F, R, B, g.rw, s) : launch_reweight(w.F, R, B, g.fft, s))) return rc;
+    if ((rc = g.rw.L ? launch_reweight_th(w.F, w.Ft, R, B, g.rw, s) : launch_reweight(w.F, w.Ft, R, B, g.fft, s))) return rc;
     if (zero_first) {
         const size_t Mfull = p->real ? p->L : 2 * p->L - 1;
         S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * Mfull * p->L * sizeof(cplx), s));
     }
     WigArgs A;
-    fill_wig_args(p, st, true, B, w.flmT, w.F, A);
+    fill_wig_args(p, st, true, B, w.flmT, w.Ft, A);
     return launch_wigner_forward(A, s);
 }
 
@@ -798,9 +800,9 @@ static int scale_synthesis(const s2w_plan *p, const Scale &sc, int B, const Work
     if ((rc = launch_so3_fwd(p->real, src, sig_stride, w.F, S, B, g.fft, s))) return rc;
     RwArgs R;
     fill_rw_args(p, sc.st, R);
-    if ((rc = g.rw.L ? launch_reweight_th(w.F, R, B, g.rw, s) : launch_reweight(w.F, R, B, g.fft, s))) return rc;
+    if ((rc = g.rw.L ? launch_reweight_th(w.F, w.Ft, R, B, g.rw, s) : launch_reweight(w.F, w.Ft, R, B, g.fft, s))) return rc;
     WigArgs A;
-    fill_wig_args(p, sc.st, true, B, w.flmT, w.F, A);
+    fill_wig_args(p, sc.st, true, B, w.flmT, w.Ft, A);
     return launch_wigner_forward(A, s);
 }
 
@@ -843,7 +845,7 @@ static int sphere_inverse(const s2w_plan *p, const void *in, void *out, void *wo
 // ---- transform drivers (ball, Alg. 2) -----------------------------------------------------------------
 // workspace: flm_sh [P][Mfull][L] (per-shell harmonic coefficients), flmp [P][Mfull][L] (f_{lmp}), F.
 struct BallWork {
-    cplx *flm_sh, *flmp, *F;
+    cplx *flm_sh, *flmp, *F, *Ft;
 };
 static BallWork carve_ball(const s2w_plan *p, void *work)
 {
@@ -852,6 +854,7 @@ static BallWork carve_ball(const s2w_plan *p, void *work)
     w.flm_sh = (cplx *)work;
     w.flmp = w.flm_sh + sh;
     w.F = w.flmp + sh;
+    w.Ft = w.F + ((p->ws_F_elems + 15) / 16) * 16;
     return w;
 }
 
@@ -861,6 +864,7 @@ static int ball_forward(const s2w_plan *p, const void *in, void *out, void *work
     Work w;
     w.flmT = bw.flm_sh;
     w.F = bw.F;
+    w.Ft = bw.Ft;
     const int P = p->P, L = p->L;
     const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
     const size_t cols = (size_t)(p->real ? L : 2 * L - 1) * L;
@@ -894,6 +898,7 @@ static int ball_inverse(const s2w_plan *p, const void *in, void *out, void *work
     Work w;
     w.flmT = bw.flm_sh;
     w.F = bw.F;
+    w.Ft = bw.Ft;
     const int P = p->P, L = p->L;
     const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
     const size_t Mfull = p->real ? L : 2 * L - 1;
@@ -1106,7 +1111,7 @@ int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int m
     p->signal_elems = (size_t)L * (2 * L - 1);
     p->ws_flm_elems = (size_t)batch * (p->real ? L : 2 * L - 1) * L;
     p->ws_F_elems = (size_t)batch * maxF;
-    p->ws_bytes = (((p->ws_flm_elems + 15) / 16) * 16 + p->ws_F_elems) * sizeof(cplx) + 256;
+    p->ws_bytes = (((p->ws_flm_elems + 15) / 16) * 16 + 2 * (((p->ws_F_elems + 15) / 16) * 16)) * sizeof(cplx) + 256;
     S2W_PLAN_TRY(cudaDeviceSynchronize() == cudaSuccess ? S2W_OK : S2W_ECUDA);
     *out = p;
     return S2W_OK;
@@ -1246,7 +1251,7 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
     p->ws_shell_elems = (size_t)P * (p->real ? L : 2 * L - 1) * L;
     p->ws_flm_elems = 2 * (((p->ws_shell_elems + 15) / 16) * 16);
     p->ws_F_elems = (size_t)P * maxF;
-    p->ws_bytes = (p->ws_flm_elems + p->ws_F_elems) * sizeof(cplx) + 256;
+    p->ws_bytes = (p->ws_flm_elems + 2 * (((p->ws_F_elems + 15) / 16) * 16)) * sizeof(cplx) + 256;
     S2W_PLAN_TRY(cudaDeviceSynchronize() == cudaSuccess ? S2W_OK : S2W_ECUDA);
     *out = p;
     return S2W_OK;
@@ -1342,6 +1347,7 @@ int s2w_plan_harmonic_forward(const s2w_plan *p, const void *f, void *flm, void 
         Work w;
         w.flmT = bw.flm_sh;
         w.F = bw.F;
+        w.Ft = bw.Ft;
         const size_t cols = (size_t)(p->real ? p->L : 2 * p->L - 1) * p->L;
         if ((rc = sht_forward_dev(p, p->sht, f, (size_t)p->L * (2 * p->L - 1), p->P, w, true, s))) return rc;
         if ((rc = launch_radial(p->Kfull_fwd, p->P, p->P, bw.flm_sh, bw.flmp, cols, p->L, 0, 0, false, s))) return rc;
@@ -1368,6 +1374,7 @@ int s2w_plan_harmonic_inverse(const s2w_plan *p, const void *flm, void *f, void 
         Work w;
         w.flmT = bw.flm_sh;
         w.F = bw.F;
+        w.Ft = bw.Ft;
         const size_t cols = (size_t)(p->real ? p->L : 2 * p->L - 1) * p->L;
         if ((rc = launch_flm_pack((const cplx *)flm, bw.flmp, p->P, p->L, p->real, s))) return rc;
         if ((rc = launch_radial(p->Kfull_inv, p->P, p->P, bw.flmp, bw.flm_sh, cols, p->L, 0, 0, false, s))) return rc;

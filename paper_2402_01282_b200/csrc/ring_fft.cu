@@ -301,7 +301,7 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
 // (v) a sign(-) DFT over i' with an output modulation; the four phase tables rw_* absorb chirps and modulations.
 // One block per column.
 // ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) reweight_kernel(cplx *__restrict__ F, RwArgs A, FftTab T)
+__global__ void __launch_bounds__(256) reweight_kernel(const cplx *__restrict__ F, cplx *__restrict__ Ft, RwArgs A, FftTab T)
 {
     extern __shared__ cplx buf[];
     __shared__ cplx s_tw[S2W_TW_SMEM];
@@ -311,7 +311,8 @@ __global__ void __launch_bounds__(256) reweight_kernel(cplx *__restrict__ F, RwA
     const int m = A.isReal ? mi : mi - (L - 1);
     const int nv = A.n_val[q];
     const double sigma = ((m + nv) & 1) ? -1.0 : 1.0;
-    cplx *col = F + ((size_t)b * A.nrows + A.n_row[q]) * (size_t)L * A.Md + mi;
+    const cplx *col = F + ((size_t)b * A.nrows + A.n_row[q]) * (size_t)L * A.Md + mi;
+    cplx *colT = Ft + (((size_t)b * A.nrows + A.n_row[q]) * A.Md + mi) * (size_t)L;  // [b][row][mi][t]: t contiguous
     for (int t = threadIdx.x; t < M; t += blockDim.x) {
         cplx v = cmake(0.0, 0.0);
         if (t < n) {
@@ -337,7 +338,7 @@ __global__ void __launch_bounds__(256) reweight_kernel(cplx *__restrict__ F, RwA
             cplx g1 = cmul(buf[S2W_PAD(tb)], __ldg(&T.rw_out3[tb]));
             g0 = cmake(fma(sigma, g1.x, g0.x), fma(sigma, g1.y, g0.y));
         }
-        col[(size_t)t * A.Md] = g0;
+        colT[t] = g0;
     }
 }
 
@@ -355,7 +356,8 @@ __global__ void __launch_bounds__(256) reweight_kernel(cplx *__restrict__ F, RwA
 // accurate (2e-16 at L = 1024).  One block per column; both sequences go through each FFT pass together.
 // ---------------------------------------------------------------------------------------------------------------
 #define RW_MAXPT 8  // ring values a thread keeps in registers (L <= 8 * blockDim)
-__global__ void __launch_bounds__(256, 3) reweight_th_kernel(cplx *__restrict__ F, RwArgs A, RwTab R)
+__global__ void __launch_bounds__(256, 3) reweight_th_kernel(const cplx *__restrict__ F, cplx *__restrict__ Ft, RwArgs A,
+                                                            RwTab R)
 {
     extern __shared__ cplx buf[];
     __shared__ cplx s_tw[S2W_TW_SMEM];
@@ -371,7 +373,8 @@ __global__ void __launch_bounds__(256, 3) reweight_th_kernel(cplx *__restrict__ 
     const int nv = A.n_val[q];
     const int par = ((m + nv) & 1) ? 1 : 0;  // 0: sigma = +1, 1: sigma = -1
     const double sigma = par ? -1.0 : 1.0;
-    cplx *col = F + ((size_t)b * A.nrows + A.n_row[q]) * (size_t)L * A.Md + mi;
+    const cplx *col = F + ((size_t)b * A.nrows + A.n_row[q]) * (size_t)L * A.Md + mi;
+    cplx *colT = Ft + (((size_t)b * A.nrows + A.n_row[q]) * A.Md + mi) * (size_t)L;  // [b][row][mi][t]: t contiguous
     const double *rp = R.rpole + par * L, *vp = R.vpole + par * L;
 
     cplx xs[RW_MAXPT];
@@ -439,11 +442,11 @@ __global__ void __launch_bounds__(256, 3) reweight_th_kernel(cplx *__restrict__ 
             if (t & 1) h = cscale(h, -1.0);
             h.x += fma(ds, xs[k].x, v * xpole.x);
             h.y += fma(ds, xs[k].y, v * xpole.y);
-            col[(size_t)t * A.Md] = h;
+            colT[t] = h;
         } else if (t == Lm) {
             cplx acc = cmake(0.0, 0.0);
             for (int w = 0; w < (int)(blockDim.x >> 5); ++w) acc = cadd(acc, s_part[w]);
-            col[(size_t)t * A.Md] = acc;
+            colT[t] = acc;
         }
     }
 }
@@ -649,25 +652,25 @@ int launch_fft_forward(cplx *data, const FftTab &T, cudaStream_t st)
     return S2W_OK;
 }
 
-int launch_reweight_th(cplx *F, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st)
+int launch_reweight_th(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st)
 {
     if (A.nn <= 0) return S2W_OK;
     size_t sm = 2 * (size_t)fft_padded_len(R.fft.M) * sizeof(cplx);
     int rc = set_smem(reweight_th_kernel, sm);
     if (rc) return rc;
     dim3 grid(A.Md, A.nn, batch);
-    S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight_th_kernel, grid, 256, sm, st, F, A, R);
+    S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight_th_kernel, grid, 256, sm, st, F, Ft, A, R);
     return S2W_OK;
 }
 
-int launch_reweight(cplx *F, const RwArgs &A, int batch, const FftTab &T, cudaStream_t st)
+int launch_reweight(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const FftTab &T, cudaStream_t st)
 {
     if (A.nn <= 0) return S2W_OK;
     size_t sm = fft_smem_bytes(T);
     int rc = set_smem(reweight_kernel, sm);
     if (rc) return rc;
     dim3 grid(A.Md, A.nn, batch);
-    S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight_kernel, grid, 256, sm, st, F, A, T);
+    S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight_kernel, grid, 256, sm, st, F, Ft, A, T);
     return S2W_OK;
 }
 

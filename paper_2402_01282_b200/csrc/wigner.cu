@@ -424,7 +424,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                 if (t >= 0 && fci.valid) {
                     const int row = fci.minus ? A.n_rowm[q] : A.n_row[q];
                     const int mi = A.isReal ? m : (fci.minus ? Lg - 1 - m : Lg - 1 + m);
-                    const cplx hv = A.F[(((size_t)fci.b * A.nrows + row) * Lg + t) * Md + mi];
+                    const cplx hv = A.F[(((size_t)fci.b * A.nrows + row) * Md + mi) * Lg + t];
                     v = (fc & 1) ? hv.y : hv.x;
                     if (fci.minus) v *= sgn;
                 }
