@@ -806,35 +806,94 @@ static int scale_synthesis(const s2w_plan *p, const Scale &sc, int B, const Work
     return launch_wigner_forward(A, s);
 }
 
-static int sphere_forward(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s)
+// Host-buffer pipelining of the sphere transforms (s2wav_*_host): coefficient blocks cross PCIe on a second stream while
+// other scales are being computed.  Analysis: each block is copied out as soon as its kernels are done; synthesis: all
+// blocks are copied in up front, in the order of use, and each scale waits only for its own block.  Blocks are visited
+// largest scale first, so that the copies of the two big top scales overlap the computation of the rest.
+struct HostPipe {
+    cudaStream_t copy;
+    char *host;   // coefficient buffer on the host, [batch][coeff_elems]
+    char *dev;    // the same on the device
+    size_t pitch; // bytes between consecutive signals
+    int B;
+    std::vector<cudaEvent_t> evs;
+    int next_event(cudaEvent_t *e)
+    {
+        cudaEvent_t ev;
+        if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) return S2W_ECUDA;
+        evs.push_back(ev);
+        *e = ev;
+        return S2W_OK;
+    }
+    int block_out(size_t off_bytes, size_t bytes, cudaStream_t s)  // computed on s -> host
+    {
+        cudaEvent_t ev;
+        if (next_event(&ev)) return S2W_ECUDA;
+        S2W_CUDA_CHECK(cudaEventRecord(ev, s));
+        S2W_CUDA_CHECK(cudaStreamWaitEvent(copy, ev, 0));
+        S2W_CUDA_CHECK(cudaMemcpy2DAsync(host + off_bytes, pitch, dev + off_bytes, pitch, bytes, B, cudaMemcpyDeviceToHost, copy));
+        return S2W_OK;
+    }
+    int block_in(size_t off_bytes, size_t bytes, cudaEvent_t *ready)  // host -> device, event when it has arrived
+    {
+        S2W_CUDA_CHECK(cudaMemcpy2DAsync(dev + off_bytes, pitch, host + off_bytes, pitch, bytes, B, cudaMemcpyHostToDevice, copy));
+        if (next_event(ready)) return S2W_ECUDA;
+        S2W_CUDA_CHECK(cudaEventRecord(*ready, copy));
+        return S2W_OK;
+    }
+    void release()
+    {
+        for (cudaEvent_t e : evs) cudaEventDestroy(e);
+        evs.clear();
+    }
+};
+
+static int sphere_forward(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s, HostPipe *hp = 0)
 {
     const Work w = carve(p, work);
     const int B = p->batch;
     const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
+    const size_t nn = 2 * p->N - 1;
     int rc;
     if ((rc = sht_forward_dev(p, p->sht, in, p->signal_elems, B, w, true, s))) return rc;
+    const int ns = (int)p->scales.size();
+    for (int k = 0; k < ns; ++k) {
+        const Scale &sc = p->scales[hp ? ns - 1 - k : k];
+        if ((rc = scale_analysis(p, sc, B, w, (char *)out + sc.offset * esz, p->coeff_elems, s))) return rc;
+        if (hp && (rc = hp->block_out(sc.offset * esz, nn * sc.Lj * (2 * sc.Lj - 1) * esz, s))) return rc;
+    }
     // scaling coefficients
     if ((rc = sht_inverse_dev(p, p->scaling, (char *)out + p->scaling_offset * esz, p->coeff_elems, B, w, s)))
         return rc;
-    for (size_t i = 0; i < p->scales.size(); ++i) {
-        const Scale &sc = p->scales[i];
-        if ((rc = scale_analysis(p, sc, B, w, (char *)out + sc.offset * esz, p->coeff_elems, s))) return rc;
-    }
+    if (hp && (rc = hp->block_out(p->scaling_offset * esz, (size_t)p->Ls * (2 * p->Ls - 1) * esz, s))) return rc;
     S2W_CUDA_CHECK(cudaPeekAtLastError());
     return S2W_OK;
 }
 
-static int sphere_inverse(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s)
+static int sphere_inverse(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s, HostPipe *hp = 0)
 {
     const Work w = carve(p, work);
     const int B = p->batch;
     const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
+    const size_t nn = 2 * p->N - 1;
+    const int ns = (int)p->scales.size();
     int rc;
+    std::vector<cudaEvent_t> ready(ns + 1);
+    if (hp) {
+        if ((rc = hp->block_in(p->scaling_offset * esz, (size_t)p->Ls * (2 * p->Ls - 1) * esz, &ready[ns]))) return rc;
+        for (int k = 0; k < ns; ++k) {
+            const Scale &sc = p->scales[ns - 1 - k];
+            if ((rc = hp->block_in(sc.offset * esz, nn * sc.Lj * (2 * sc.Lj - 1) * esz, &ready[ns - 1 - k]))) return rc;
+        }
+        S2W_CUDA_CHECK(cudaStreamWaitEvent(s, ready[ns], 0));
+    }
     if ((rc = sht_forward_dev(p, p->scaling, (const char *)in + p->scaling_offset * esz, p->coeff_elems, B, w, true,
                               s)))
         return rc;
-    for (size_t i = 0; i < p->scales.size(); ++i) {
+    for (int k = 0; k < ns; ++k) {
+        const int i = hp ? ns - 1 - k : k;
         const Scale &sc = p->scales[i];
+        if (hp) S2W_CUDA_CHECK(cudaStreamWaitEvent(s, ready[i], 0));
         if ((rc = scale_synthesis(p, sc, B, w, (const char *)in + sc.offset * esz, p->coeff_elems, s))) return rc;
     }
     if ((rc = sht_inverse_dev(p, p->sht, out, p->signal_elems, B, w, s))) return rc;
@@ -1480,10 +1539,37 @@ int host_transform(bool fwd, const CacheEntry &e, const void *in_h, void *out_h)
         set_error("null pointer");
         return S2W_EINVAL;
     }
-    const size_t esz = e.plan->real ? sizeof(double) : sizeof(cplx);
-    const size_t sig = e.plan->signal_elems * e.plan->batch * esz, cof = e.plan->coeff_elems * e.plan->batch * esz;
+    const s2w_plan *p = e.plan;
+    const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
+    const size_t sig = p->signal_elems * p->batch * esz, cof = p->coeff_elems * p->batch * esz;
     void *d_in = fwd ? e.d_sig : e.d_cof, *d_out = fwd ? e.d_cof : e.d_sig;
     int rc = S2W_OK;
+    if (p->kind == 0) {
+        // sphere: coefficient blocks pipelined over a second stream (see HostPipe)
+        static cudaStream_t copy_stream = 0;
+        if (!copy_stream) S2W_CUDA_CHECK(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+        HostPipe hp;
+        hp.copy = copy_stream;
+        hp.host = fwd ? (char *)out_h : (char *)const_cast<void *>(in_h);
+        hp.dev = (char *)e.d_cof;
+        hp.pitch = p->coeff_elems * esz;
+        hp.B = p->batch;
+        void *work = (void *)(((uintptr_t)e.work + 255) & ~(uintptr_t)255);
+        if (fwd) {
+            if (cudaMemcpyAsync(d_in, in_h, sig, cudaMemcpyHostToDevice, 0) != cudaSuccess) rc = S2W_ECUDA;
+            if (!rc) rc = sphere_forward(p, d_in, d_out, work, 0, &hp);
+        } else {
+            rc = sphere_inverse(p, d_in, d_out, work, 0, &hp);
+            if (!rc && cudaMemcpyAsync(out_h, d_out, sig, cudaMemcpyDeviceToHost, 0) != cudaSuccess) rc = S2W_ECUDA;
+        }
+        cudaError_t e1 = cudaStreamSynchronize(0), e2 = cudaStreamSynchronize(copy_stream);
+        hp.release();
+        if ((e1 != cudaSuccess || e2 != cudaSuccess) && !rc) {
+            set_error(std::string("stream sync: ") + cudaGetErrorString(e1 != cudaSuccess ? e1 : e2));
+            rc = S2W_ECUDA;
+        }
+        return rc;
+    }
     if (cudaMemcpyAsync(d_in, in_h, fwd ? sig : cof, cudaMemcpyHostToDevice, 0) != cudaSuccess) rc = S2W_ECUDA;
     if (!rc) rc = fwd ? s2w_plan_forward(e.plan, d_in, d_out, e.work, 0) : s2w_plan_inverse(e.plan, d_in, d_out, e.work, 0);
     if (!rc && cudaMemcpyAsync(out_h, d_out, fwd ? cof : sig, cudaMemcpyDeviceToHost, 0) != cudaSuccess) rc = S2W_ECUDA;
