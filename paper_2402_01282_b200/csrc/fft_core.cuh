@@ -295,6 +295,53 @@ __device__ inline void fft_dit_full_b(cplx *buf, const FftTab &T, const cplx *st
     }
 }
 
+template <int R>
+__device__ __forceinline__ void mid_pass_b(cplx *buf, int M, const cplx *__restrict__ khat, int nb, int bstride)
+{
+    const int per = M / R;
+    for (int it = threadIdx.x; it < nb * per; it += blockDim.x) {
+        const int bi = it / per, g = it - bi * per;
+        cplx *b = buf + bi * bstride;
+        cplx v[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[k] = b[S2W_PAD(g * R + k)];
+        Bfly<R, false>::run(v);
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[k] = cmul(v[k], __ldg(&khat[g * R + k]));
+        Bfly<R, true>::run(v);
+#pragma unroll
+        for (int k = 0; k < R; ++k) b[S2W_PAD(g * R + k)] = v[k];
+    }
+}
+
+// nb circular convolutions (sequences bstride apart) with the same kernel spectrum; see fft_convolve.
+__device__ inline void fft_convolve_b(cplx *buf, const FftTab &T, const cplx *stw, const cplx *__restrict__ khat,
+                                      int nb, int bstride)
+{
+    const int M = T.M;
+    const int r = T.logM % 3;
+    const int logMid = (r == 0) ? 3 : r;
+    int logS = T.logM;
+    while (logS > logMid) {
+        dif_pass_b<8>(buf, M, logS, T, stw, nb, bstride);
+        __syncthreads();
+        logS -= 3;
+    }
+    if (logMid == 3)
+        mid_pass_b<8>(buf, M, khat, nb, bstride);
+    else if (logMid == 2)
+        mid_pass_b<4>(buf, M, khat, nb, bstride);
+    else
+        mid_pass_b<2>(buf, M, khat, nb, bstride);
+    __syncthreads();
+    logS = logMid + 3;
+    while (logS <= T.logM) {
+        dit_pass_b<8>(buf, M, logS, T, stw, nb, bstride);
+        __syncthreads();
+        logS += 3;
+    }
+}
+
 // Forward transform only (used once per table at plan creation): natural in, digit-reversed out.
 __device__ inline void fft_dif_full(cplx *buf, const FftTab &T, const cplx *stw)
 {

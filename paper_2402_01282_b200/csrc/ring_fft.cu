@@ -137,15 +137,21 @@ __global__ void __launch_bounds__(256, 3) ring_inv_kernel(const cplx *__restrict
 // Real: rows n >= 0 only: V_n(a) = sum_m F_mn e^{i m alpha_a} with F_{-m,n} = conj(F_{m,-n});
 //       W = sum_{n>=0} c_n Re(e^{i n gamma_g} V_n), c_0 = 1, c_n = 2.
 // ---------------------------------------------------------------------------------------------------------------
-template <bool REAL>
+// MULTI: rpb rings per block (small grids), tpr = blockDim / rpb threads per ring; otherwise one ring per block.
+template <bool REAL, bool MULTI>
 __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict__ F, void *__restrict__ W, size_t sig_stride,
-                                                     So3Args A, FftTab T)
+                                                     So3Args A, FftTab T, int rpb)
 {
-    extern __shared__ cplx buf[];
+    extern __shared__ cplx buf0[];
     __shared__ cplx s_tw[S2W_TW_SMEM];
     tw_stage(s_tw, T);
     const int n = T.n, L = T.L, M = T.M;
-    const int t = blockIdx.x, b = blockIdx.y;
+    const int bstride = fft_padded_len(M);
+    const int tpr = MULTI ? blockDim.x / rpb : blockDim.x;
+    const int rl = MULTI ? threadIdx.x / tpr : 0, tl = MULTI ? threadIdx.x - rl * tpr : threadIdx.x;
+    cplx *buf = buf0 + (size_t)rl * bstride;
+    const int t = MULTI ? blockIdx.x * rpb + rl : blockIdx.x, b = blockIdx.y;
+    const bool has = MULTI ? t < L : true;
     const int Md = REAL ? L : n;
     const int ng = 2 * A.N - 1;
     const cplx *Fb = F + (size_t)b * A.nrows * L * Md;
@@ -157,9 +163,9 @@ __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict_
         if (threadIdx.x < ng) gph[threadIdx.x] = cis_2pi_frac(nv * (int)threadIdx.x, ng);
         const cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * Md;   // row of n
         const cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * Md;  // row of -n
-        for (int k = threadIdx.x; k < M; k += blockDim.x) {
+        for (int k = tl; k < M; k += tpr) {
             cplx v = cmake(0.0, 0.0);
-            if (k < n) {
+            if (k < n && has) {
                 if (REAL) {
                     v = k < L ? Fp[k] : cconj(Fm[n - k]);
                 } else {
@@ -171,9 +177,12 @@ __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict_
             buf[S2W_PAD(k)] = v;
         }
         __syncthreads();
-        fft_convolve(buf, T, s_tw, T.bhat_p);
+        if (MULTI)
+            fft_convolve_b(buf0, T, s_tw, T.bhat_p, rpb, bstride);
+        else
+            fft_convolve(buf, T, s_tw, T.bhat_p);
         // one pass over alpha: the chirp product once, then all gamma planes with their loads issued together
-        for (int a = threadIdx.x; a < n; a += blockDim.x) {
+        for (int a = tl; a < (has ? n : 0); a += tpr) {
             const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
             if (REAL) {
                 double *Wr = (double *)W + (size_t)b * sig_stride + (size_t)t * n + a;
@@ -214,15 +223,20 @@ __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict_
 // The gamma sum is done first in pixel space, V_n(a) = (1/n_g) sum_g e^{-i n gamma_g} W(g,t,a), then one DFT per row.
 // Real: rows n >= 0; the row of -n follows from F_{m,-n} = conj(F_{-m,n}).
 // ---------------------------------------------------------------------------------------------------------------
-template <bool REAL>
+template <bool REAL, bool MULTI>
 __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict__ W, cplx *__restrict__ F, size_t sig_stride,
-                                                     So3Args A, FftTab T)
+                                                     So3Args A, FftTab T, int rpb)
 {
-    extern __shared__ cplx buf[];
+    extern __shared__ cplx buf0[];
     __shared__ cplx s_tw[S2W_TW_SMEM];
     tw_stage(s_tw, T);
     const int n = T.n, L = T.L, M = T.M;
-    const int t = blockIdx.x, b = blockIdx.y;
+    const int bstride = fft_padded_len(M);
+    const int tpr = MULTI ? blockDim.x / rpb : blockDim.x;
+    const int rl = MULTI ? threadIdx.x / tpr : 0, tl = MULTI ? threadIdx.x - rl * tpr : threadIdx.x;
+    cplx *buf = buf0 + (size_t)rl * bstride;
+    const int t = MULTI ? blockIdx.x * rpb + rl : blockIdx.x, b = blockIdx.y;
+    const bool has = MULTI ? t < L : true;
     const int Md = REAL ? L : n;
     const int ng = 2 * A.N - 1;
     const double inv_ng = 1.0 / (double)ng, inv_n = 1.0 / (double)n;
@@ -233,9 +247,9 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
         if (REAL && nv < 0) continue;
         if (threadIdx.x < ng) gph[threadIdx.x] = cis_2pi_frac(-nv * (int)threadIdx.x, ng);
         __syncthreads();
-        for (int a = threadIdx.x; a < M; a += blockDim.x) {
+        for (int a = tl; a < M; a += tpr) {
             cplx v = cmake(0.0, 0.0);
-            if (a < n) {
+            if (a < n && has) {
                 if (REAL) {
                     const double *Wr = (const double *)W + (size_t)b * sig_stride + (size_t)t * n + a;
                     for (int g0 = 0; g0 < ng; g0 += 9) {
@@ -267,11 +281,14 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
             buf[S2W_PAD(a)] = v;
         }
         __syncthreads();
-        fft_convolve(buf, T, s_tw, T.bhat_m);
+        if (MULTI)
+            fft_convolve_b(buf0, T, s_tw, T.bhat_m, rpb, bstride);
+        else
+            fft_convolve(buf, T, s_tw, T.bhat_m);
         cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * Md;
         cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * Md;
         if (REAL) {
-            for (int m = threadIdx.x; m < L; m += blockDim.x) {
+            for (int m = tl; m < (has ? L : 0); m += tpr) {
                 Fp[m] = cscale(cmul(buf[S2W_PAD(m)], __ldg(&T.chirp[m])), inv_n);
                 if (nv != 0) {
                     int k = m == 0 ? 0 : n - m;
@@ -279,7 +296,7 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
                 }
             }
         } else {
-            for (int mi = threadIdx.x; mi < n; mi += blockDim.x) {
+            for (int mi = tl; mi < (has ? n : 0); mi += tpr) {
                 int m = mi - (L - 1);
                 int k = m < 0 ? m + n : m;
                 Fp[mi] = cscale(cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k])), inv_n);
@@ -451,6 +468,112 @@ __global__ void __launch_bounds__(256, 3) reweight_th_kernel(const cplx *__restr
     }
 }
 
+// The same for the small grids of the multiresolution / ball scale loops (M2 <= 1024): cpb = 2048 / M2 columns per block,
+// tpc = 256 / cpb threads per column, all 2 cpb sequences through each FFT pass together -- one column per block would
+// spend its time in per-block set-up and barriers there.
+#define RW_MAXCPB 128
+__global__ void __launch_bounds__(256, 2) reweight_th_multi_kernel(const cplx *__restrict__ F, cplx *__restrict__ Ft,
+                                                                  RwArgs A, RwTab R, int cpb, int ncolumns)
+{
+    extern __shared__ cplx buf[];
+    __shared__ cplx s_tw[S2W_TW_SMEM];
+    tw_stage(s_tw, R.fft);
+    __shared__ double s_dot[RW_MAXCPB][2];
+    __shared__ cplx s_pole[RW_MAXCPB];
+    const FftTab &T = R.fft;
+    const int L = R.L, Lm = L - 1, M = T.M;
+    const int bstride = fft_padded_len(M);
+    const int tpc = blockDim.x / cpb, cl = threadIdx.x / tpc, tl = threadIdx.x - cl * tpc;
+    cplx *b1 = buf + (size_t)(2 * cl) * bstride, *b2 = b1 + bstride;
+    const int colid = blockIdx.x * cpb + cl;
+    const bool has = colid < ncolumns;
+    const int mi = colid % A.Md, q = (colid / A.Md) % A.nn, b = colid / (A.Md * A.nn);
+    const int m = A.isReal ? mi : mi - (L - 1);
+    const int nv = has ? A.n_val[q] : 0;
+    const int par = ((m + nv) & 1) ? 1 : 0;
+    const double sigma = par ? -1.0 : 1.0;
+    const int row = has ? A.n_row[q] : 0;
+    const cplx *col = F + ((size_t)b * A.nrows + row) * (size_t)L * A.Md + mi;
+    cplx *colT = Ft + (((size_t)b * A.nrows + row) * A.Md + mi) * (size_t)L;
+    const double *rp = R.rpole + par * L, *vp = R.vpole + par * L;
+
+    if (threadIdx.x < cpb) s_dot[threadIdx.x][0] = s_dot[threadIdx.x][1] = 0.0;
+    cplx xs[RW_MAXPT];
+    cplx dot = cmake(0.0, 0.0);
+#pragma unroll
+    for (int k = 0; k < RW_MAXPT; ++k) {
+        const int t = tl + k * tpc;
+        cplx x = cmake(0.0, 0.0);
+        if (t < L && has) {
+            x = col[(size_t)t * A.Md];
+            const double r = rp[t];
+            dot.x = fma(r, x.x, dot.x);
+            dot.y = fma(r, x.y, dot.y);
+            if (t == Lm) s_pole[cl] = x;
+        }
+        xs[k] = x;
+    }
+    for (int t = tl; t < M; t += tpc) {
+        b1[S2W_PAD(t)] = cmake(0.0, 0.0);
+        b2[S2W_PAD(t)] = cmake(0.0, 0.0);
+    }
+    __syncthreads();  // zeroed buffers and s_dot are visible
+#pragma unroll
+    for (int k = 0; k < RW_MAXPT; ++k) {
+        const int t = tl + k * tpc;
+        if (t < Lm) {
+            const cplx u1 = (t & 1) ? cscale(xs[k], -1.0) : xs[k];
+            b1[S2W_PAD(t)] = u1;
+            b2[S2W_PAD(t)] = cscale(u1, R.delta[t]);
+        }
+    }
+    {   // pole-ring dot product: shuffle tree over the lanes of a column inside a warp, then shared atomics
+        const int w = tpc < 32 ? tpc : 32;  // a power of two; columns never straddle a w-lane group
+        for (int o = w >> 1; o > 0; o >>= 1) {
+            dot.x += __shfl_xor_sync(0xffffffffu, dot.x, o);
+            dot.y += __shfl_xor_sync(0xffffffffu, dot.y, o);
+        }
+        if ((threadIdx.x & (w - 1)) == 0) {
+            atomicAdd(&s_dot[cl][0], dot.x);
+            atomicAdd(&s_dot[cl][1], dot.y);
+        }
+    }
+    __syncthreads();
+    fft_dif_full_b(buf, T, s_tw, 2 * cpb, bstride);
+    for (int i = tl; i < R.npairs; i += tpc) {
+        const int2 pp = __ldg(&R.pairs[i]);
+        const int p = pp.x, pn = pp.y;
+        const cplx tp = __ldg(&R.TG[4 * i]), gp = cscale(__ldg(&R.TG[4 * i + 1]), sigma);
+        const cplx tn = __ldg(&R.TG[4 * i + 2]), gn = cscale(__ldg(&R.TG[4 * i + 3]), sigma);
+        const cplx u1p = b1[S2W_PAD(p)], u1n = b1[S2W_PAD(pn)], u2p = b2[S2W_PAD(p)], u2n = b2[S2W_PAD(pn)];
+        b1[S2W_PAD(p)] = csub(cmul(tp, u1p), cmul(gp, u1n));
+        b2[S2W_PAD(p)] = cadd(cmul(tp, u2p), cmul(gp, u2n));
+        if (pn != p) {
+            b1[S2W_PAD(pn)] = csub(cmul(tn, u1n), cmul(gn, u1p));
+            b2[S2W_PAD(pn)] = cadd(cmul(tn, u2n), cmul(gn, u2p));
+        }
+    }
+    __syncthreads();
+    fft_dit_full_b(buf, T, s_tw, 2 * cpb, bstride);
+    if (!has) return;
+    const cplx xpole = s_pole[cl];
+#pragma unroll
+    for (int k = 0; k < RW_MAXPT; ++k) {
+        const int t = tl + k * tpc;
+        if (t < Lm) {
+            const cplx y1 = b1[S2W_PAD(t)], y2 = b2[S2W_PAD(t)];
+            const double dl = R.delta[t], ds = R.dsum[t], v = vp[t];
+            cplx h = cmake(fma(dl, y1.x, -y2.x), fma(dl, y1.y, -y2.y));
+            if (t & 1) h = cscale(h, -1.0);
+            h.x += fma(ds, xs[k].x, v * xpole.x);
+            h.y += fma(ds, xs[k].y, v * xpole.y);
+            colT[t] = h;
+        } else if (t == Lm) {
+            colT[t] = cmake(s_dot[cl][0], s_dot[cl][1]);
+        }
+    }
+}
+
 // plan-time: in-place forward transform (natural in, digit-reversed out) of one length-M array, one block
 __global__ void __launch_bounds__(256) fft_forward_kernel(cplx *data, FftTab T)
 {
@@ -611,36 +734,48 @@ int launch_ring_inv(bool real, const cplx *in, void *out, int B, int Lg, size_t 
     return S2W_OK;
 }
 
+static int seqs_per_block(int fit, long long total, int cap);
+
+template <bool REAL, bool MULTI>
+static int so3_launch_t(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch,
+                        const FftTab &T, int rpb, cudaStream_t st)
+{
+    size_t sm = (size_t)rpb * fft_smem_bytes(T);
+    dim3 grid((T.L + rpb - 1) / rpb, batch);
+    int rc;
+    if (fwd) {
+        if ((rc = set_smem(so3_fwd_kernel<REAL, MULTI>, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_SO3_FFT, (so3_fwd_kernel<REAL, MULTI>), grid, 256, sm, st, in, (cplx *)out, sig_stride, A, T,
+                     rpb);
+    } else {
+        if ((rc = set_smem(so3_inv_kernel<REAL, MULTI>, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_SO3_FFT, (so3_inv_kernel<REAL, MULTI>), grid, 256, sm, st, (const cplx *)in, out, sig_stride, A,
+                     T, rpb);
+    }
+    return S2W_OK;
+}
+
+static int so3_launch(bool fwd, bool real, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch,
+                      const FftTab &T, cudaStream_t st)
+{
+    const int rpb = seqs_per_block(4096 / T.M, (long long)T.L * batch, 32);
+    if (rpb > 1)
+        return real ? so3_launch_t<true, true>(fwd, in, out, sig_stride, A, batch, T, rpb, st)
+                    : so3_launch_t<false, true>(fwd, in, out, sig_stride, A, batch, T, rpb, st);
+    return real ? so3_launch_t<true, false>(fwd, in, out, sig_stride, A, batch, T, 1, st)
+                : so3_launch_t<false, false>(fwd, in, out, sig_stride, A, batch, T, 1, st);
+}
+
 int launch_so3_inv(bool real, const cplx *F, void *W, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
                    cudaStream_t st)
 {
-    size_t sm = fft_smem_bytes(T);
-    dim3 grid(T.L, batch);
-    int rc;
-    if (real) {
-        if ((rc = set_smem(so3_inv_kernel<true>, sm))) return rc;
-        S2W_LAUNCH_C(S2W_K_SO3_FFT, so3_inv_kernel<true>, grid, 256, sm, st, F, W, sig_stride, A, T);
-    } else {
-        if ((rc = set_smem(so3_inv_kernel<false>, sm))) return rc;
-        S2W_LAUNCH_C(S2W_K_SO3_FFT, so3_inv_kernel<false>, grid, 256, sm, st, F, W, sig_stride, A, T);
-    }
-    return S2W_OK;
+    return so3_launch(false, real, F, W, sig_stride, A, batch, T, st);
 }
 
 int launch_so3_fwd(bool real, const void *W, size_t sig_stride, cplx *F, const So3Args &A, int batch, const FftTab &T,
                    cudaStream_t st)
 {
-    size_t sm = fft_smem_bytes(T);
-    dim3 grid(T.L, batch);
-    int rc;
-    if (real) {
-        if ((rc = set_smem(so3_fwd_kernel<true>, sm))) return rc;
-        S2W_LAUNCH_C(S2W_K_SO3_FFT, so3_fwd_kernel<true>, grid, 256, sm, st, W, F, sig_stride, A, T);
-    } else {
-        if ((rc = set_smem(so3_fwd_kernel<false>, sm))) return rc;
-        S2W_LAUNCH_C(S2W_K_SO3_FFT, so3_fwd_kernel<false>, grid, 256, sm, st, W, F, sig_stride, A, T);
-    }
-    return S2W_OK;
+    return so3_launch(true, real, W, F, sig_stride, A, batch, T, st);
 }
 
 int launch_fft_forward(cplx *data, const FftTab &T, cudaStream_t st)
@@ -652,12 +787,29 @@ int launch_fft_forward(cplx *data, const FftTab &T, cudaStream_t st)
     return S2W_OK;
 }
 
+// sequences per block on small grids: as many as fit the shared-memory budget of one full-size sequence, but never so
+// many that the launch drops below ~6 blocks per SM
+static int seqs_per_block(int fit, long long total, int cap)
+{
+    int s = fit < 1 ? 1 : (fit > cap ? cap : fit);
+    while (s > 1 && total / s < 900) s >>= 1;
+    return s;
+}
+
 int launch_reweight_th(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st)
 {
     if (A.nn <= 0) return S2W_OK;
-    size_t sm = 2 * (size_t)fft_padded_len(R.fft.M) * sizeof(cplx);
-    int rc = set_smem(reweight_th_kernel, sm);
-    if (rc) return rc;
+    const int ncol = A.Md * A.nn * batch;
+    const int cpb = seqs_per_block(2048 / R.fft.M, ncol, RW_MAXCPB);
+    size_t sm = 2 * (size_t)cpb * fft_padded_len(R.fft.M) * sizeof(cplx);
+    int rc;
+    if (cpb > 1) {
+        if ((rc = set_smem(reweight_th_multi_kernel, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight_th_multi_kernel, (ncol + cpb - 1) / cpb, 256, sm, st, F, Ft, A, R, cpb,
+                     ncol);
+        return S2W_OK;
+    }
+    if ((rc = set_smem(reweight_th_kernel, sm))) return rc;
     dim3 grid(A.Md, A.nn, batch);
     S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight_th_kernel, grid, 256, sm, st, F, Ft, A, R);
     return S2W_OK;
