@@ -307,6 +307,185 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// a8 for REAL signals on the large grids: one block per PAIR of rings.  The row n = 0 has a Hermitian spectrum
+// (F_{-m,0} = conj F_{m,0}) and a real transform, so the two rings share one complex DFT (ring t0 in the real part,
+// ring t0+1 in the imaginary part), as in a1; the rows n > 0 are done ring by ring.  5 instead of 6 convolutions per
+// ring pair at N = 5.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256, 3) so3_inv_pair_kernel(const cplx *__restrict__ F, double *__restrict__ W,
+                                                             size_t sig_stride, So3Args A, FftTab T)
+{
+    extern __shared__ cplx buf[];
+    __shared__ cplx s_tw[S2W_TW_SMEM];
+    __shared__ cplx gph[2 * S2W_MAX_N];
+    tw_stage(s_tw, T);
+    const int n = T.n, L = T.L, M = T.M;
+    const int t0 = 2 * blockIdx.x, b = blockIdx.y;
+    const bool has1 = t0 + 1 < L;
+    const int ng = 2 * A.N - 1;
+    const cplx *Fb = F + (size_t)b * A.nrows * L * L;
+    double *Wb = W + (size_t)b * sig_stride;
+    const size_t plane = (size_t)L * n;
+    bool first = true;
+    for (int q = 0; q < A.nn; ++q) {
+        const int nv = A.n_val[q];
+        if (nv < 0) continue;
+        if (nv == 0) {
+            const cplx *X0 = Fb + ((size_t)A.n_row[q] * L + t0) * L, *X1 = X0 + L;
+            for (int k = threadIdx.x; k < M; k += blockDim.x) {
+                cplx v = cmake(0.0, 0.0);
+                if (k < n) {
+                    const int m = k < L ? k : n - k;
+                    cplx a = X0[m], c = has1 ? X1[m] : cmake(0.0, 0.0);
+                    if (k >= L) {
+                        a = cconj(a);
+                        c = cconj(c);
+                    }
+                    v = cmulc(cmake(a.x - c.y, a.y + c.x), __ldg(&T.chirp[k]));
+                }
+                buf[S2W_PAD(k)] = v;
+            }
+            __syncthreads();
+            fft_convolve(buf, T, s_tw, T.bhat_p);
+            for (int a = threadIdx.x; a < n; a += blockDim.x) {
+                const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));  // V_0 of ring t0 + i V_0 of ring t0+1
+                double *Wr = Wb + (size_t)t0 * n + a;
+                for (int g = 0; g < ng; ++g) {
+                    Wr[g * plane] = first ? v.x : Wr[g * plane] + v.x;
+                    if (has1) Wr[g * plane + n] = first ? v.y : Wr[g * plane + n] + v.y;
+                }
+            }
+            first = false;
+            __syncthreads();
+            continue;
+        }
+        if (threadIdx.x < ng) gph[threadIdx.x] = cis_2pi_frac(nv * (int)threadIdx.x, ng);
+        for (int r = 0; r < (has1 ? 2 : 1); ++r) {
+            const int t = t0 + r;
+            const cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * L;
+            const cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * L;
+            for (int k = threadIdx.x; k < M; k += blockDim.x) {
+                cplx v = cmake(0.0, 0.0);
+                if (k < n) v = cmulc(k < L ? Fp[k] : cconj(Fm[n - k]), __ldg(&T.chirp[k]));
+                buf[S2W_PAD(k)] = v;
+            }
+            __syncthreads();
+            fft_convolve(buf, T, s_tw, T.bhat_p);
+            for (int a = threadIdx.x; a < n; a += blockDim.x) {
+                const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
+                double *Wr = Wb + (size_t)t * n + a;
+                const double vx = 2.0 * v.x, vy = 2.0 * v.y;
+                for (int g0 = 0; g0 < ng; g0 += 9) {
+                    double old[9];
+#pragma unroll
+                    for (int k = 0; k < 9; ++k) old[k] = (!first && g0 + k < ng) ? Wr[(g0 + k) * plane] : 0.0;
+#pragma unroll
+                    for (int k = 0; k < 9; ++k)
+                        if (g0 + k < ng) {
+                            const cplx ph = gph[g0 + k];
+                            Wr[(g0 + k) * plane] = old[k] + (ph.x * vx - ph.y * vy);
+                        }
+                }
+            }
+            __syncthreads();
+        }
+        first = false;
+    }
+}
+
+__global__ void __launch_bounds__(256, 3) so3_fwd_pair_kernel(const double *__restrict__ W, cplx *__restrict__ F,
+                                                             size_t sig_stride, So3Args A, FftTab T)
+{
+    extern __shared__ cplx buf[];
+    __shared__ cplx s_tw[S2W_TW_SMEM];
+    __shared__ cplx gph[2 * S2W_MAX_N];
+    tw_stage(s_tw, T);
+    const int n = T.n, L = T.L, M = T.M;
+    const int t0 = 2 * blockIdx.x, b = blockIdx.y;
+    const bool has1 = t0 + 1 < L;
+    const int ng = 2 * A.N - 1;
+    const double inv_ng = 1.0 / (double)ng, inv_n = 1.0 / (double)n;
+    cplx *Fb = F + (size_t)b * A.nrows * L * L;
+    const double *Wb = W + (size_t)b * sig_stride;
+    const size_t plane = (size_t)L * n;
+    for (int q = 0; q < A.nn; ++q) {
+        const int nv = A.n_val[q];
+        if (nv < 0) continue;
+        if (nv == 0) {
+            for (int a = threadIdx.x; a < M; a += blockDim.x) {
+                cplx v = cmake(0.0, 0.0);
+                if (a < n) {
+                    const double *Wr = Wb + (size_t)t0 * n + a;
+                    for (int g0 = 0; g0 < ng; g0 += 9) {
+                        double w0[9], w1[9];
+#pragma unroll
+                        for (int k = 0; k < 9; ++k) {
+                            w0[k] = g0 + k < ng ? Wr[(g0 + k) * plane] : 0.0;
+                            w1[k] = (has1 && g0 + k < ng) ? Wr[(g0 + k) * plane + n] : 0.0;
+                        }
+#pragma unroll
+                        for (int k = 0; k < 9; ++k) {
+                            v.x += w0[k];
+                            v.y += w1[k];
+                        }
+                    }
+                    v = cmul(cscale(v, inv_ng), __ldg(&T.chirp[a]));
+                }
+                buf[S2W_PAD(a)] = v;
+            }
+            __syncthreads();
+            fft_convolve(buf, T, s_tw, T.bhat_m);
+            for (int k = threadIdx.x; k < n; k += blockDim.x) buf[S2W_PAD(k)] = cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k]));
+            __syncthreads();
+            cplx *F0 = Fb + ((size_t)A.n_row[q] * L + t0) * L, *F1 = F0 + L;
+            for (int m = threadIdx.x; m < L; m += blockDim.x) {
+                const cplx a = buf[S2W_PAD(m)], c = cconj(buf[S2W_PAD(m == 0 ? 0 : n - m)]);
+                const cplx sm = cadd(a, c), df = csub(a, c);
+                F0[m] = cscale(sm, 0.5 * inv_n);
+                if (has1) F1[m] = cmake(0.5 * inv_n * df.y, -0.5 * inv_n * df.x);
+            }
+            __syncthreads();
+            continue;
+        }
+        if (threadIdx.x < ng) gph[threadIdx.x] = cis_2pi_frac(-nv * (int)threadIdx.x, ng);
+        __syncthreads();
+        for (int r = 0; r < (has1 ? 2 : 1); ++r) {
+            const int t = t0 + r;
+            for (int a = threadIdx.x; a < M; a += blockDim.x) {
+                cplx v = cmake(0.0, 0.0);
+                if (a < n) {
+                    const double *Wr = Wb + (size_t)t * n + a;
+                    for (int g0 = 0; g0 < ng; g0 += 9) {
+                        double wv[9];
+#pragma unroll
+                        for (int k = 0; k < 9; ++k) wv[k] = g0 + k < ng ? Wr[(g0 + k) * plane] : 0.0;
+#pragma unroll
+                        for (int k = 0; k < 9; ++k)
+                            if (g0 + k < ng) {
+                                const cplx ph = gph[g0 + k];
+                                v.x = fma(ph.x, wv[k], v.x);
+                                v.y = fma(ph.y, wv[k], v.y);
+                            }
+                    }
+                    v = cmul(cscale(v, inv_ng), __ldg(&T.chirp[a]));
+                }
+                buf[S2W_PAD(a)] = v;
+            }
+            __syncthreads();
+            fft_convolve(buf, T, s_tw, T.bhat_m);
+            cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * L;
+            cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * L;
+            for (int m = threadIdx.x; m < L; m += blockDim.x) {
+                Fp[m] = cscale(cmul(buf[S2W_PAD(m)], __ldg(&T.chirp[m])), inv_n);
+                const int k = m == 0 ? 0 : n - m;
+                Fm[m] = cscale(cconj(cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k]))), inv_n);
+            }
+            __syncthreads();
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // a2 reweighting of one theta-column F[.][t][mi] (stride Md) of parity sigma = (-1)^{m+n}, in place (R3):
 //   (ii)  extend to n = 2L-1 rings by F(theta_{n-1-t}) = sigma F(theta_t)
 //   (iii) Fh(k) = 1/n sum_t F(theta_t) e^{-i k theta_t},  theta_t = pi(2t+1)/n,  |k| <= L-1
@@ -759,6 +938,21 @@ static int so3_launch(bool fwd, bool real, const void *in, void *out, size_t sig
                       const FftTab &T, cudaStream_t st)
 {
     const int rpb = seqs_per_block(4096 / T.M, (long long)T.L * batch, 32);
+    if (rpb == 1 && real) {  // large grids, real signals: ring pairs (the n = 0 row shares one transform)
+        size_t sm = fft_smem_bytes(T);
+        dim3 grid((T.L + 1) / 2, batch);
+        int rc;
+        if (fwd) {
+            if ((rc = set_smem(so3_fwd_pair_kernel, sm))) return rc;
+            S2W_LAUNCH_C(S2W_K_SO3_FFT, so3_fwd_pair_kernel, grid, 256, sm, st, (const double *)in, (cplx *)out,
+                         sig_stride, A, T);
+        } else {
+            if ((rc = set_smem(so3_inv_pair_kernel, sm))) return rc;
+            S2W_LAUNCH_C(S2W_K_SO3_FFT, so3_inv_pair_kernel, grid, 256, sm, st, (const cplx *)in, (double *)out,
+                         sig_stride, A, T);
+        }
+        return S2W_OK;
+    }
     if (rpb > 1)
         return real ? so3_launch_t<true, true>(fwd, in, out, sig_stride, A, batch, T, rpb, st)
                     : so3_launch_t<false, true>(fwd, in, out, sig_stride, A, batch, T, rpb, st);
