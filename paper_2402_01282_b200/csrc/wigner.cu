@@ -19,7 +19,7 @@
 //
 // Rings are processed in groups of 32 (a warp, one lane per ring): each hemisphere's rings sorted by |cos beta|,
 // group 2j = north rings 32j.., group 2j+1 = south rings 32j...  A group starts at the first degree at which any of
-// its rings has reached |d| >= 2^-90 (the exponentially small start of the recursion is neither computed nor able to
+// its rings has reached |d| >= 2^-70 (the exponentially small start of the recursion is neither computed nor able to
 // underflow); the start is warp-uniform and monotone in j, so a warp that owns groups j0 < j1 < ... runs phases with
 // 1, 2, ... active groups and no per-step checks.  Even warps own north groups, odd warps south groups.
 //
@@ -36,7 +36,7 @@ namespace {
 
 #define WIG_TL 64   // l-tile of the inverse kernel
 #define WIG_TLF 64  // l-tile of the forward kernel
-#define RAMP_THRESHOLD_EXP (-90)
+#define RAMP_THRESHOLD_EXP (-70)
 
 __device__ __forceinline__ size_t tri_off(int m, int Lfull) { return (size_t)m * Lfull - ((size_t)m * (m - 1)) / 2 - m; }
 
@@ -54,7 +54,7 @@ __device__ __forceinline__ void wig_step(double &d, double &u, double y, double 
 
 // ---------------------------------------------------------------------------------------------------------------
 // plan-time: group start degrees and seeds.  One warp per (group, m, table n); lane = ring slot.
-//   pass 0: every ring runs the range-extended recursion from its seed d^{l0} = mant 2^expo until |d| >= 2^-90;
+//   pass 0: every ring runs the range-extended recursion from its seed d^{l0} = mant 2^expo until |d| >= 2^-70;
 //           the group start is the minimum over the warp.
 //   fix   : suffix minimum over the groups of a hemisphere (monotone starts).
 //   pass 1: every ring runs to the group start and stores (d~, u~) there.
