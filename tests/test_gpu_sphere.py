@@ -244,3 +244,63 @@ def test_config4_band_limit_2048_seeds_and_sampled_rings():
     back = plan.inverse(w)
     assert float((back - f).abs().max() / f.abs().max()) < RT_TOL
     plan.close()
+
+
+EDGE_CASES = [
+    # L, N, lam, J0, multires, real, batch
+    (2, 1, 2.0, 0, True, True, 1),        # smallest non-trivial grid: 2 rings x 3 samples
+    (3, 2, 2.0, 1, True, False, 2),
+    (16, 2, 2.0, 4, True, True, 1),       # J0 = J: a single wavelet scale plus the scaling part
+    (27, 3, 3.0, 0, True, True, 3),       # lambda = 3, L = lambda^3
+    (33, 5, 2.0, 2, False, True, 2),      # no multiresolution, N > 1, real, L = 2^k + 1 (empty top scale)
+    (48, 3, 2.0, 1, True, False, 7),      # 14 columns: four column chunks, the last one ragged
+    (96, 6, 2.0, 3, True, True, 1),       # even N (imaginary zeta), three ring groups per hemisphere
+]
+
+
+@pytest.mark.parametrize("L,N,lam,J0,mr,real,batch", EDGE_CASES)
+def test_forward_inverse_parity_edge_cases(L, N, lam, J0, mr, real, batch):
+    torch, api = _api()
+    flm, f = _signals(L, 500 + L + N, real, batch)
+    plan = api.s2wav_plan_create(L, N, lam, J0, mr, real, batch)
+    w = plan.forward(torch.from_numpy(f).cuda())
+    scal, scales = plan.split(w)
+    filt = S.filters(L, N, lam, J0, "f80")
+    cast = (lambda a: a.real.astype(np.float64)) if real else (lambda a: a.astype(np.complex128))
+    for b in sorted({0, batch - 1}):
+        o_phi, o_psi = S.analysis(f[b], L, N, lam, J0, mr, "f80", filt)
+        assert _relmax(scal[b].cpu().numpy(), cast(o_phi)) < FWD_TOL
+        for j in range(plan.J0, plan.J + 1):
+            ref = cast(o_psi[j])
+            got = scales[(j, 0)][b].cpu().numpy()
+            assert got.shape == ref.shape
+            if np.abs(ref).max() == 0.0:
+                assert np.abs(got).max() == 0.0          # empty scale: exactly zero
+            else:
+                assert _relmax(got, ref) < FWD_TOL, (b, j)
+    back = plan.inverse(w).cpu().numpy().reshape(f.shape)
+    assert _relmax(back, f) < RT_TOL
+    plan.close()
+
+
+def test_two_plans_and_a_side_stream():
+    """Plans are immutable and independent: two plans used alternately, one of them on a non-default stream."""
+    torch, api = _api()
+    flm_a, f_a = _signals(20, 900, True, 1)
+    flm_b, f_b = _signals(28, 901, False, 2)
+    pa = api.s2wav_plan_create(20, 3, 2.0, 1, True, True, 1)
+    pb = api.s2wav_plan_create(28, 2, 2.0, 0, True, False, 2)
+    fa, fb = torch.from_numpy(f_a).cuda(), torch.from_numpy(f_b).cuda()
+    ref_a, ref_b = pa.forward(fa).clone(), pb.forward(fb).clone()
+    side = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    for _ in range(3):
+        with torch.cuda.stream(side):
+            wa = pa.forward(fa)
+        wb = pb.forward(fb)
+        torch.cuda.synchronize()
+        assert torch.equal(wa, ref_a) and torch.equal(wb, ref_b)
+    back = pa.inverse(wa).cpu().numpy().reshape(f_a.shape)
+    assert _relmax(back, f_a) < RT_TOL
+    pa.close()
+    pb.close()
