@@ -53,6 +53,11 @@ struct WigArgs {
     const double *dtab;         // precomputed-kernel variant: [ntab][tri_g][32 G] d^l_mn(beta) per ring slot, else null
     size_t tri_g;               // Lg (Lg + 1) / 2
     const cplx *filt;           // [nn][Lg] filter applied to row q at degree l
+    // two scales sharing one recursion (same grid, same rows n; at most 2 complex columns): the second scale's filter,
+    // support start (>= lmin) and array; null / unused otherwise
+    const cplx *filt2;
+    int lmin2;
+    cplx *F2;
     cplx *flmT;                 // [B][Mfull][Lfull]  f_{l m} stored m-major; Mfull = Lfull (real) or 2 Lfull - 1
     cplx *F;                    // inverse direction: output [B][nrows][Lg][Md], Md = Lg (real) or 2 Lg - 1;
                                 // forward direction: input, transposed [B][nrows][Md][Lg]

@@ -584,6 +584,9 @@ void fill_wig_args(const s2w_plan *p, const Stage &st, bool synthesis, int B, cp
     A.dtab = g.dtab;
     A.tri_g = (size_t)st.Lg * (st.Lg + 1) / 2;
     A.filt = synthesis ? st.filt_syn : st.filt_ana;
+    A.filt2 = 0;
+    A.lmin2 = st.lmin;
+    A.F2 = 0;
     A.flmT = flmT;
     A.F = F;
 }
@@ -723,8 +726,9 @@ int make_scale_stage(s2w_plan *p, Scale &sc, const double *kj, const std::vector
 
 struct Work {
     cplx *flmT;
-    cplx *F;   // [B][n][t][m]
-    cplx *Ft;  // [B][n][m][t]: reweighted columns, input of the forward contraction
+    cplx *F;    // [B][n][t][m]
+    cplx *Ft;   // [B][n][m][t]: reweighted columns, input of the forward contraction
+    cplx *Ft2;  // the same for the second of two scales that share one recursion
 };
 
 static Work carve(const s2w_plan *p, void *work)
@@ -733,6 +737,7 @@ static Work carve(const s2w_plan *p, void *work)
     w.flmT = (cplx *)work;
     w.F = w.flmT + ((p->ws_flm_elems + 15) / 16) * 16;
     w.Ft = w.F + ((p->ws_F_elems + 15) / 16) * 16;
+    w.Ft2 = w.Ft + ((p->ws_F_elems + 15) / 16) * 16;
     return w;
 }
 
@@ -848,6 +853,60 @@ struct HostPipe {
     }
 };
 
+// Two scales can share one recursion (wigner.cu: NS = 2 inverse kernel, fused tile rows of the forward kernel) when
+// they live on the same grid with the same rows n and the batch has at most two complex columns; `a` is the one whose
+// filter support starts first.  On-the-fly plans only.
+static bool scales_fusable(const s2w_plan *p, const Scale &a, const Scale &b, int B)
+{
+    if ((p->flags & S2W_PRECOMPUTE) || (p->real ? B : 2 * B) > 2) return false;
+    if (a.st.grid != b.st.grid || a.st.nn != b.st.nn || a.st.nn == 0 || a.st.lmin > b.st.lmin) return false;
+    for (int q = 0; q < a.st.nn; ++q)
+        if (a.st.n_val[q] != b.st.n_val[q] || a.st.n_row[q] != b.st.n_row[q]) return false;
+    return true;
+}
+
+// a4 + a5 for two fusable scales in one launch (outputs w.F and w.Ft), then a8 for each
+static int scale_pair_analysis(const s2w_plan *p, const Scale &a, const Scale &b, int B, const Work &w, void *dst_a,
+                               void *dst_b, size_t sig_stride, cudaStream_t s)
+{
+    int rc;
+    WigArgs A;
+    fill_wig_args(p, a.st, false, B, w.flmT, w.F, A);
+    A.filt2 = b.st.filt_ana;
+    A.lmin2 = b.st.lmin;
+    A.F2 = w.Ft;
+    if ((rc = launch_wigner_inverse(A, s))) return rc;
+    So3Args S;
+    fill_so3_args(p, a.st, S);
+    const FftTab &T = p->grids[a.st.grid].fft;
+    if ((rc = launch_so3_inv(p->real, w.F, dst_a, sig_stride, S, B, T, s))) return rc;
+    return launch_so3_inv(p->real, w.Ft, dst_b, sig_stride, S, B, T, s);
+}
+
+// a8 + a2 for each of two fusable scales (into w.Ft and w.Ft2), then a6 + a4 for both in one launch
+static int scale_pair_synthesis(const s2w_plan *p, const Scale &a, const Scale &b, int B, const Work &w, const void *src_a,
+                                const void *src_b, size_t sig_stride, cudaStream_t s)
+{
+    const GridTab &g = p->grids[a.st.grid];
+    int rc;
+    So3Args S;
+    fill_so3_args(p, a.st, S);
+    RwArgs R;
+    fill_rw_args(p, a.st, R);
+    for (int k = 0; k < 2; ++k) {
+        cplx *Ft = k ? w.Ft2 : w.Ft;
+        if ((rc = launch_so3_fwd(p->real, k ? src_b : src_a, sig_stride, w.F, S, B, g.fft, s))) return rc;
+        if ((rc = g.rw.L ? launch_reweight_th(w.F, Ft, R, B, g.rw, s) : launch_reweight(w.F, Ft, R, B, g.fft, s)))
+            return rc;
+    }
+    WigArgs A;
+    fill_wig_args(p, a.st, true, B, w.flmT, w.Ft, A);
+    A.filt2 = b.st.filt_syn;
+    A.lmin2 = b.st.lmin;
+    A.F2 = w.Ft2;
+    return launch_wigner_forward(A, s);
+}
+
 static int sphere_forward(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s, HostPipe *hp = 0)
 {
     const Work w = carve(p, work);
@@ -857,8 +916,19 @@ static int sphere_forward(const s2w_plan *p, const void *in, void *out, void *wo
     int rc;
     if ((rc = sht_forward_dev(p, p->sht, in, p->signal_elems, B, w, true, s))) return rc;
     const int ns = (int)p->scales.size();
-    for (int k = 0; k < ns; ++k) {
-        const Scale &sc = p->scales[hp ? ns - 1 - k : k];
+    // the two top scales share one recursion when they can; they go first (their blocks are the big host copies)
+    int rest = ns;
+    if (ns >= 2 && scales_fusable(p, p->scales[ns - 2], p->scales[ns - 1], B)) {
+        const Scale &a = p->scales[ns - 2], &b = p->scales[ns - 1];
+        if ((rc = scale_pair_analysis(p, a, b, B, w, (char *)out + a.offset * esz, (char *)out + b.offset * esz,
+                                      p->coeff_elems, s)))
+            return rc;
+        if (hp && (rc = hp->block_out(b.offset * esz, nn * b.Lj * (2 * b.Lj - 1) * esz, s))) return rc;
+        if (hp && (rc = hp->block_out(a.offset * esz, nn * a.Lj * (2 * a.Lj - 1) * esz, s))) return rc;
+        rest = ns - 2;
+    }
+    for (int k = 0; k < rest; ++k) {
+        const Scale &sc = p->scales[hp ? rest - 1 - k : k];
         if ((rc = scale_analysis(p, sc, B, w, (char *)out + sc.offset * esz, p->coeff_elems, s))) return rc;
         if (hp && (rc = hp->block_out(sc.offset * esz, nn * sc.Lj * (2 * sc.Lj - 1) * esz, s))) return rc;
     }
@@ -890,8 +960,20 @@ static int sphere_inverse(const s2w_plan *p, const void *in, void *out, void *wo
     if ((rc = sht_forward_dev(p, p->scaling, (const char *)in + p->scaling_offset * esz, p->coeff_elems, B, w, true,
                               s)))
         return rc;
-    for (int k = 0; k < ns; ++k) {
-        const int i = hp ? ns - 1 - k : k;
+    int rest = ns;
+    if (ns >= 2 && scales_fusable(p, p->scales[ns - 2], p->scales[ns - 1], B)) {
+        const Scale &a = p->scales[ns - 2], &b = p->scales[ns - 1];
+        if (hp) {
+            S2W_CUDA_CHECK(cudaStreamWaitEvent(s, ready[ns - 1], 0));
+            S2W_CUDA_CHECK(cudaStreamWaitEvent(s, ready[ns - 2], 0));
+        }
+        if ((rc = scale_pair_synthesis(p, a, b, B, w, (const char *)in + a.offset * esz, (const char *)in + b.offset * esz,
+                                       p->coeff_elems, s)))
+            return rc;
+        rest = ns - 2;
+    }
+    for (int k = 0; k < rest; ++k) {
+        const int i = hp ? rest - 1 - k : k;
         const Scale &sc = p->scales[i];
         if (hp) S2W_CUDA_CHECK(cudaStreamWaitEvent(s, ready[i], 0));
         if ((rc = scale_synthesis(p, sc, B, w, (const char *)in + sc.offset * esz, p->coeff_elems, s))) return rc;
@@ -1170,7 +1252,7 @@ int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int m
     p->signal_elems = (size_t)L * (2 * L - 1);
     p->ws_flm_elems = (size_t)batch * (p->real ? L : 2 * L - 1) * L;
     p->ws_F_elems = (size_t)batch * maxF;
-    p->ws_bytes = (((p->ws_flm_elems + 15) / 16) * 16 + 2 * (((p->ws_F_elems + 15) / 16) * 16)) * sizeof(cplx) + 256;
+    p->ws_bytes = (((p->ws_flm_elems + 15) / 16) * 16 + 3 * (((p->ws_F_elems + 15) / 16) * 16)) * sizeof(cplx) + 256;
     S2W_PLAN_TRY(cudaDeviceSynchronize() == cudaSuccess ? S2W_OK : S2W_ECUDA);
     *out = p;
     return S2W_OK;

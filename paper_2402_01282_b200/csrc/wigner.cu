@@ -164,49 +164,51 @@ __device__ __forceinline__ void stage_coef(const double *__restrict__ crow, int 
 // inverse direction: one block per (m >= 0, column chunk) covering all rings; warp w owns groups w, w+W, w+2W, ...
 // (slot r = group r W + w), lane = ring.  Loops over the n of the launch.
 // ---------------------------------------------------------------------------------------------------------------
-template <int NC, int R, int RA, bool ACC>
+// NCT columns in shared memory per degree, the first NACC of them accumulated (0: recursion only)
+template <int NCT, int R, int RA, int NACC>
 __device__ __forceinline__ void inv_range(int la, int lb, int lt, int hemi, const double2 *s_ag, const double2 *s_e,
                                           const double *s_X, const double (&y)[R], double (&d)[R], double (&u)[R],
-                                          double (&acc)[R][NC])
+                                          double (&acc)[R][NCT])
 {
     const double *se = reinterpret_cast<const double *>(s_e) + hemi;
     for (int l = la; l < lb; ++l) {
         const int i = l - lt;
         const double2 ag = s_ag[i];
         const double e = se[2 * i];
-        double xv[NC];
-        if (ACC) {
+        double xv[NACC > 0 ? NACC : 1];
 #pragma unroll
-            for (int c = 0; c < NC; ++c) xv[c] = s_X[i * NC + c];
-        }
+        for (int c = 0; c < NACC; ++c) xv[c] = s_X[i * NCT + c];
 #pragma unroll
         for (int r = 0; r < RA; ++r) {
-            if (ACC) {
 #pragma unroll
-                for (int c = 0; c < NC; ++c) acc[r][c] = fma(d[r], xv[c], acc[r][c]);
-            }
+            for (int c = 0; c < NACC; ++c) acc[r][c] = fma(d[r], xv[c], acc[r][c]);
             wig_step(d[r], u[r], y[r], ag.x, ag.y, e);
         }
     }
 }
 
-template <int NC, int R, bool ACC>
+template <int NCT, int R, int NACC>
 __device__ __forceinline__ void inv_dispatch(int ra, int la, int lb, int lt, int hemi, const double2 *s_ag,
                                              const double2 *s_e, const double *s_X, const double (&y)[R],
-                                             double (&d)[R], double (&u)[R], double (&acc)[R][NC])
+                                             double (&d)[R], double (&u)[R], double (&acc)[R][NCT])
 {
-    if (R >= 4 && ra == 4) return inv_range<NC, R, (R >= 4 ? 4 : R), ACC>(la, lb, lt, hemi, s_ag, s_e, s_X, y, d, u, acc);
-    if (R >= 3 && ra == 3) return inv_range<NC, R, (R >= 3 ? 3 : R), ACC>(la, lb, lt, hemi, s_ag, s_e, s_X, y, d, u, acc);
-    if (R >= 2 && ra == 2) return inv_range<NC, R, (R >= 2 ? 2 : R), ACC>(la, lb, lt, hemi, s_ag, s_e, s_X, y, d, u, acc);
-    if (ra >= 1) return inv_range<NC, R, 1, ACC>(la, lb, lt, hemi, s_ag, s_e, s_X, y, d, u, acc);
+    if (R >= 4 && ra == 4) return inv_range<NCT, R, (R >= 4 ? 4 : R), NACC>(la, lb, lt, hemi, s_ag, s_e, s_X, y, d, u, acc);
+    if (R >= 3 && ra == 3) return inv_range<NCT, R, (R >= 3 ? 3 : R), NACC>(la, lb, lt, hemi, s_ag, s_e, s_X, y, d, u, acc);
+    if (R >= 2 && ra == 2) return inv_range<NCT, R, (R >= 2 ? 2 : R), NACC>(la, lb, lt, hemi, s_ag, s_e, s_X, y, d, u, acc);
+    if (ra >= 1) return inv_range<NCT, R, 1, NACC>(la, lb, lt, hemi, s_ag, s_e, s_X, y, d, u, acc);
 }
 
-template <int NC, int R, int MAXT>
+// NS = 2 (batches of at most 2 complex columns): two wavelet scales that live on the same theta grid with the same rows
+// n -- the two top scales of a multiresolution transform -- share ONE recursion: NC columns of scale A (filter A.filt,
+// support from A.lmin, output A.F) and NC columns of scale B (A.filt2, A.lmin2 >= A.lmin, A.F2).  With few columns the
+// recursion (4 FP64 instructions per step) outweighs the accumulation (NC), so sharing it is worth up to a third.
+template <int NC, int R, int MAXT, int NS>
 __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_inverse_kernel(WigArgs A)
 {
+    constexpr int NCT = NC * NS;
     __shared__ double2 s_ag[WIG_TL];
     __shared__ double2 s_e[WIG_TL];
-    __shared__ double s_X[2][WIG_TL * NC];  // [0]: X_l, [1]: (-1)^l X_l (southern warps)
+    __shared__ double s_X[2][WIG_TL * NCT];  // [0]: X_l, [1]: (-1)^l X_l (southern warps)
 
     const int m = blockIdx.x, chunk = blockIdx.y;
     const int Lg = A.Lg, Lfull = A.Lfull, G = A.G;
@@ -233,10 +235,11 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_inverse_ke
         const int *gsrow = A.gstart + ((size_t)tab * Lg + m) * G;
         const double2 *seedrow = A.dseed + ((size_t)tab * Lg + m) * (size_t)(32 * G);
         const double sgn = ((m + n) & 1) ? -1.0 : 1.0;
-        const int lacc = l0 > A.lmin ? l0 : A.lmin;  // first l that contributes
+        const int lacc = l0 > A.lmin ? l0 : A.lmin;                        // first l that contributes (scale A)
+        const int lacc2 = NS > 1 ? (l0 > A.lmin2 ? l0 : A.lmin2) : lacc;    // ... to scale B
 
         int gs[R + 1];
-        double d[R], u[R], acc[R][NC];
+        double d[R], u[R], acc[R][NCT];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int g = r * W + warp;
@@ -244,7 +247,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_inverse_ke
             d[r] = 0.0;
             u[r] = 0.0;
 #pragma unroll
-            for (int c = 0; c < NC; ++c) acc[r][c] = 0.0;
+            for (int c = 0; c < NCT; ++c) acc[r][c] = 0.0;
         }
         gs[R] = INT_MAX;
         // first degree any group of the block needs: groups 0 and 1 start first
@@ -255,23 +258,24 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_inverse_ke
         for (int lt = bmin & ~(WIG_TL - 1); lt < Lg; lt += WIG_TL) {
             __syncthreads();
             stage_coef<WIG_TL>(crow, lt, l0, Lg, s_ag, s_e);
-            for (int i = threadIdx.x; i < WIG_TL * (NC / 2); i += T) {
+            for (int i = threadIdx.x; i < WIG_TL * (NCT / 2); i += T) {
                 const int k = i / WIG_TL, ll = i % WIG_TL;  // consecutive threads -> consecutive l (coalesced)
+                const int sc = k / (NC / 2), kk = k - sc * (NC / 2);
                 const int l = lt + ll;
-                const ColInfo ci = col_info(A, chunk * (NC / 2) + k);
+                const ColInfo ci = col_info(A, chunk * (NC / 2) + kk);
                 cplx X = cmake(0.0, 0.0);
-                if (l >= lacc && l < Lg && ci.valid) {
+                if (l >= (sc ? lacc2 : lacc) && l < Lg && ci.valid) {
                     const int mi = A.isReal ? m : (ci.minus ? Lfull - 1 - m : Lfull - 1 + m);
                     const cplx f = A.flmT[((size_t)ci.b * Mfull + mi) * Lfull + l];
-                    const cplx Gf = A.filt[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
+                    const cplx Gf = (sc ? A.filt2 : A.filt)[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
                     X = cmul(Gf, f);
                     if (ci.minus) X = cscale(X, sgn);
                 }
                 const double alt = (l & 1) ? -1.0 : 1.0;
-                s_X[0][ll * NC + 2 * k] = X.x;
-                s_X[0][ll * NC + 2 * k + 1] = X.y;
-                s_X[1][ll * NC + 2 * k] = alt * X.x;
-                s_X[1][ll * NC + 2 * k + 1] = alt * X.y;
+                s_X[0][ll * NCT + 2 * k] = X.x;
+                s_X[0][ll * NCT + 2 * k + 1] = X.y;
+                s_X[1][ll * NCT + 2 * k] = alt * X.x;
+                s_X[1][ll * NCT + 2 * k + 1] = alt * X.y;
             }
             __syncthreads();
 
@@ -292,10 +296,15 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_inverse_ke
 #pragma unroll
                 for (int r = 0; r < R; ++r)
                     if (gs[r] > l && gs[r] < le) le = gs[r];
-                // recursion only below the filter support, then accumulate + recursion
-                const int lmid = lacc < l ? l : (lacc < le ? lacc : le);
-                if (l < lmid) inv_dispatch<NC, R, false>(ra, l, lmid, lt, hemi, s_ag, s_e, s_X[hemi], y, d, u, acc);
-                if (lmid < le) inv_dispatch<NC, R, true>(ra, lmid, le, lt, hemi, s_ag, s_e, s_X[hemi], y, d, u, acc);
+                // recursion only below the filter support of scale A, scale A alone up to the support of scale B
+                if (lacc > l && lacc < le) le = lacc;
+                if (lacc2 > l && lacc2 < le) le = lacc2;
+                if (l < lacc)
+                    inv_dispatch<NCT, R, 0>(ra, l, le, lt, hemi, s_ag, s_e, s_X[hemi], y, d, u, acc);
+                else if (NS > 1 && l < lacc2)
+                    inv_dispatch<NCT, R, NC>(ra, l, le, lt, hemi, s_ag, s_e, s_X[hemi], y, d, u, acc);
+                else
+                    inv_dispatch<NCT, R, NCT>(ra, l, le, lt, hemi, s_ag, s_e, s_X[hemi], y, d, u, acc);
                 l = le;
             }
         }
@@ -305,13 +314,15 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_inverse_ke
         for (int r = 0; r < R; ++r) {
             if (tr[r] < 0) continue;
 #pragma unroll
-            for (int k = 0; k < NC / 2; ++k) {
-                const ColInfo ci = col_info(A, chunk * (NC / 2) + k);
+            for (int k = 0; k < NCT / 2; ++k) {
+                const int sc = k / (NC / 2), kk = k - sc * (NC / 2);
+                const ColInfo ci = col_info(A, chunk * (NC / 2) + kk);
                 if (!ci.valid) continue;
                 if (ci.minus && m == 0) continue;  // (0,-n) is the plus column of another n
                 const int row = ci.minus ? A.n_rowm[q] : A.n_row[q];
                 const int mi = A.isReal ? m : (ci.minus ? Lg - 1 - m : Lg - 1 + m);
-                A.F[(((size_t)ci.b * A.nrows + row) * Lg + tr[r]) * Md + mi] = cmake(acc[r][2 * k], acc[r][2 * k + 1]);
+                (sc ? A.F2 : A.F)[(((size_t)ci.b * A.nrows + row) * Lg + tr[r]) * Md + mi] =
+                    cmake(acc[r][2 * k], acc[r][2 * k + 1]);
             }
         }
     }
@@ -395,7 +406,11 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
     }
     // A-fragment coordinates of this lane: column c = lane / 4, ring quad member lane % 4
     const int fc = lane >> 2, fk = lane & 3;
-    const ColInfo fci = col_info(A, chunk * (NC / 2) + (fc >> 1));
+    // A.F2 set (at most 2 complex columns): the tile rows 4..7, idle otherwise, carry a second scale that shares the
+    // recursion (same grid, same rows n): rows 0..3 = columns of scale A (A.F, A.filt), rows 4..7 = scale B (A.F2, A.filt2)
+    const bool fuse = A.F2 != nullptr;
+    const ColInfo fci = col_info(A, fuse ? ((fc & 3) >> 1) : chunk * (NC / 2) + (fc >> 1));
+    const cplx *Fsrc = (fuse && fc >= 4) ? A.F2 : A.F;
 
     for (int q = 0; q < A.nn; ++q) {
         const int n = A.n_val[q], an = n < 0 ? -n : n;
@@ -424,7 +439,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                 if (t >= 0 && fci.valid) {
                     const int row = fci.minus ? A.n_rowm[q] : A.n_row[q];
                     const int mi = A.isReal ? m : (fci.minus ? Lg - 1 - m : Lg - 1 + m);
-                    const cplx hv = A.F[(((size_t)fci.b * A.nrows + row) * Md + mi) * Lg + t];
+                    const cplx hv = Fsrc[(((size_t)fci.b * A.nrows + row) * Md + mi) * Lg + t];
                     v = (fc & 1) ? hv.y : hv.x;
                     if (fci.minus) v *= sgn;
                 }
@@ -538,25 +553,30 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
             for (int i = threadIdx.x; i < WIG_TLF * (NC / 2); i += T) {
                 const int k = i / WIG_TLF, ll = i % WIG_TLF;
                 const int l = lt + ll;
-                const ColInfo ci = col_info(A, chunk * (NC / 2) + k);
+                if (fuse && k >= 2) continue;  // fused: k = complex column, both scales summed below
+                const ColInfo ci = col_info(A, fuse ? k : chunk * (NC / 2) + k);
                 if (l < lacc || l >= Lg || !ci.valid) continue;
                 if (ci.minus && m == 0) continue;
-                double re = 0.0, im = 0.0, reS = 0.0, imS = 0.0;
-                for (int w = 0; w < W; w += 2) {
-                    re += s_red[w][ll][2 * k];
-                    im += s_red[w][ll][2 * k + 1];
-                    reS += s_red[w + 1][ll][2 * k];
-                    imS += s_red[w + 1][ll][2 * k + 1];
+                cplx val = cmake(0.0, 0.0);
+                for (int sc = 0; sc < (fuse ? 2 : 1); ++sc) {
+                    const int c0i = 2 * k + 4 * sc;
+                    double re = 0.0, im = 0.0, reS = 0.0, imS = 0.0;
+                    for (int w = 0; w < W; w += 2) {
+                        re += s_red[w][ll][c0i];
+                        im += s_red[w][ll][c0i + 1];
+                        reS += s_red[w + 1][ll][c0i];
+                        imS += s_red[w + 1][ll][c0i + 1];
+                    }
+                    if (!PRE && (l & 1)) {
+                        re -= reS;
+                        im -= imS;
+                    } else {
+                        re += reS;
+                        im += imS;
+                    }
+                    const cplx Gf = (sc ? A.filt2 : A.filt)[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
+                    val = cadd(val, cmul(Gf, cmake(re, im)));
                 }
-                if (!PRE && (l & 1)) {
-                    re -= reS;
-                    im -= imS;
-                } else {
-                    re += reS;
-                    im += imS;
-                }
-                const cplx Gf = A.filt[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
-                const cplx val = cmul(Gf, cmake(re, im));
                 const int mi = A.isReal ? m : (ci.minus ? Lfull - 1 - m : Lfull - 1 + m);
                 double *dst = reinterpret_cast<double *>(&A.flmT[((size_t)ci.b * Mfull + mi) * Lfull + l]);
                 atomicAdd(dst, val.x);
@@ -780,11 +800,11 @@ bool wig_cfg(int G, WigCfg &c)
     return c.R <= 4;
 }
 
-template <int NC, int R, int MAXT>
+template <int NC, int R, int MAXT, int NS>
 void launch_inv_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
 {
     dim3 grid(A.Lg, chunks);
-    S2W_LAUNCH_C(S2W_K_WIGNER_INV, (wigner_inverse_kernel<NC, R, MAXT>), grid, T, 0, st, A);
+    S2W_LAUNCH_C(S2W_K_WIGNER_INV, (wigner_inverse_kernel<NC, R, MAXT, NS>), grid, T, 0, st, A);
 }
 
 template <int R, int MAXT, bool PRE>
@@ -807,12 +827,12 @@ int launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
     return S2W_OK;
 }
 
-template <int NC>
+template <int NC, int NS>
 int dispatch_inv(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t st)
 {
 #define S2W_WIG_CASE(RR, MT)                              \
     if (c.R == RR && c.MAXT == MT) {                      \
-        launch_inv_t<NC, RR, MT>(A, 32 * c.W, chunks, st); \
+        launch_inv_t<NC, RR, MT, NS>(A, 32 * c.W, chunks, st); \
         return S2W_OK;                                    \
     }
     S2W_WIG_CASE(1, 256)
@@ -870,9 +890,13 @@ int launch_wigner(bool fwd, const WigArgs &A, cudaStream_t st)
     const int CT = A.isReal ? A.B : 2 * A.B;
     if (fwd) return dispatch_fwd(A, c, (CT + 3) / 4, st);
     if (A.dtab) return dispatch_inv_pre(A, c, (CT + 3) / 4, st);
-    if (CT >= 3) return dispatch_inv<8>(A, c, (CT + 3) / 4, st);
-    if (CT == 2) return dispatch_inv<4>(A, c, 1, st);
-    return dispatch_inv<2>(A, c, 1, st);
+    if (A.F2) {  // two scales, one recursion: batches of at most two complex columns
+        if (CT > 2) return S2W_EINVAL;
+        return CT == 2 ? dispatch_inv<4, 2>(A, c, 1, st) : dispatch_inv<2, 2>(A, c, 1, st);
+    }
+    if (CT >= 3) return dispatch_inv<8, 1>(A, c, (CT + 3) / 4, st);
+    if (CT == 2) return dispatch_inv<4, 1>(A, c, 1, st);
+    return dispatch_inv<2, 1>(A, c, 1, st);
 }
 
 }  // namespace
