@@ -395,18 +395,31 @@ def run_ours(args, cfg):
     except Exception as e:  # noqa: BLE001
         probe = {"error": str(e)}
     total_kms = sum(v[0] for v in classes.values())
+    roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "frac": achieved / peak if peak else None, "traffic": None,
+                "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x sm_max_mhz (DESIGN.md); "
+                               "measured DFMA-chain probe beside it",
+                "probe": probe, "tuples_per_step": tup, "flops_per_step": flops,
+                "launches_per_step": dom_n / ksteps, "ms_per_step": dom_ms / ksteps}
+    if args.precompute:
+        # the precomputed-kernel variant streams 8 B of Wigner-d table per (ring, m, l, n) tuple
+        hbm = None
+        try:
+            hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+            src = "measured copy bandwidth of MEASURED_PEAKS.json"
+        except Exception:  # noqa: BLE001
+            hbm, src = 6650.0, "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
+        gbs = 8.0 * tup * ksteps / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": gbs, "peak": hbm, "unit": "GB/s",
+                    "frac": gbs / hbm, "traffic": None, "peak_source": src, "tuples_per_step": tup,
+                    "bytes_per_step": 8.0 * tup, "launches_per_step": dom_n / ksteps, "ms_per_step": dom_ms / ksteps}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, args),
         "clocks": clocks, "gpu_launches": int(launches),
         "roundtrip_rel_err": rt_err,
-        "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                     "frac": achieved / peak if peak else None, "traffic": None,
-                     "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x sm_max_mhz (DESIGN.md); "
-                                    "measured DFMA-chain probe beside it",
-                     "probe": probe, "tuples_per_step": tup, "flops_per_step": flops,
-                     "launches_per_step": dom_n / ksteps, "ms_per_step": dom_ms / ksteps},
+        "roofline": roofline,
         "kernel_ms_per_step": {k: round(v[0] / ksteps, 4) for k, v in classes.items()},
         "kernel_share": {k: round(v[0] / total_kms, 4) for k, v in classes.items()} if total_kms else None,
     }

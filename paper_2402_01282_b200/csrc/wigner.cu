@@ -378,7 +378,7 @@ __device__ __forceinline__ void fwd_octet(const double2 *s_ag8, const double *se
     }
 }
 
-template <int R, int MAXT, bool PRE>
+template <int R, int MAXT, bool PRE, bool FUSE>
 __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_kernel(WigArgs A)
 {
     constexpr int NC = 8;
@@ -408,7 +408,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
     const int fc = lane >> 2, fk = lane & 3;
     // A.F2 set (at most 2 complex columns): the tile rows 4..7, idle otherwise, carry a second scale that shares the
     // recursion (same grid, same rows n): rows 0..3 = columns of scale A (A.F, A.filt), rows 4..7 = scale B (A.F2, A.filt2)
-    const bool fuse = A.F2 != nullptr;
+    constexpr bool fuse = FUSE;
     const ColInfo fci = col_info(A, fuse ? ((fc & 3) >> 1) : chunk * (NC / 2) + (fc >> 1));
     const cplx *Fsrc = (fuse && fc >= 4) ? A.F2 : A.F;
 
@@ -807,14 +807,14 @@ void launch_inv_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
     S2W_LAUNCH_C(S2W_K_WIGNER_INV, (wigner_inverse_kernel<NC, R, MAXT, NS>), grid, T, 0, st, A);
 }
 
-template <int R, int MAXT, bool PRE>
+template <int R, int MAXT, bool PRE, bool FUSE>
 int launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
 {
     const size_t red = (size_t)(MAXT / 32) * WIG_TLF * 8 * sizeof(double);
     const size_t smem = red + (PRE ? 0 : (size_t)(T / 32) * R * FWD_GT * sizeof(double));
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(wigner_forward_kernel<R, MAXT, PRE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(wigner_forward_kernel<R, MAXT, PRE, FUSE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)(red + (size_t)(MAXT / 32) * R * FWD_GT * sizeof(double)));
         if (e != cudaSuccess) {
             set_error(std::string("cudaFuncSetAttribute(wigner_forward_kernel): ") + cudaGetErrorString(e));
@@ -823,7 +823,7 @@ int launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
         configured = true;
     }
     dim3 grid(A.Lg, chunks);
-    S2W_LAUNCH_C(S2W_K_WIGNER_FWD, (wigner_forward_kernel<R, MAXT, PRE>), grid, T, smem, st, A);
+    S2W_LAUNCH_C(S2W_K_WIGNER_FWD, (wigner_forward_kernel<R, MAXT, PRE, FUSE>), grid, T, smem, st, A);
     return S2W_OK;
 }
 
@@ -849,8 +849,9 @@ int dispatch_fwd(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t st)
 {
 #define S2W_WIG_CASE(RR, MT)                                                              \
     if (c.R == RR && c.MAXT == MT)                                                        \
-        return A.dtab ? launch_fwd_t<RR, MT, true>(A, 32 * c.W, chunks, st)               \
-                      : launch_fwd_t<RR, MT, false>(A, 32 * c.W, chunks, st);
+        return A.dtab ? launch_fwd_t<RR, MT, true, false>(A, 32 * c.W, chunks, st)        \
+                      : (A.F2 ? launch_fwd_t<RR, MT, false, true>(A, 32 * c.W, chunks, st) \
+                              : launch_fwd_t<RR, MT, false, false>(A, 32 * c.W, chunks, st));
     S2W_WIG_CASE(1, 256)
     S2W_WIG_CASE(2, 256)
     S2W_WIG_CASE(3, 256)
