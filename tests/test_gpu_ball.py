@@ -146,3 +146,19 @@ def test_config5_full_size():
         assert got.shape == ref.shape
         assert _relmax(got, ref) < FWD_TOL, key
     plan.close()
+
+
+def test_ball_precomputed_kernel_variant_matches_on_the_fly():
+    """S2W_PRECOMPUTE on a ball plan: same coefficients as the recursion path, round trip within tolerance."""
+    torch, api = _api()
+    L, P, N, lam, nu, J0, tau = 20, 8, 3, 2.0, 2.0, 0, 1.0
+    flmp, f = _voxels(L, P, tau, 77)
+    fd = torch.from_numpy(f).cuda().reshape(1, -1)
+    otf = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau)
+    pre = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau, flags=api.S2W_PRECOMPUTE)
+    w0, w1 = otf.forward(fd), pre.forward(fd)
+    assert float((w0 - w1).abs().max()) < 1e-12 * float(w0.abs().max())
+    back = pre.inverse(w1).cpu().numpy().reshape(f.shape)
+    assert _relmax(back, f) < RT_TOL
+    otf.close()
+    pre.close()
