@@ -304,3 +304,25 @@ def test_two_plans_and_a_side_stream():
     assert _relmax(back, f_a) < RT_TOL
     pa.close()
     pb.close()
+
+
+@pytest.mark.parametrize("L,N,real", [(600, 3, True), (1100, 2, False)])
+def test_large_band_limits_that_are_not_powers_of_two(L, N, real):
+    """Ragged ring groups (20 and 36 groups of 32), three groups per warp, Bluestein lengths 4096 and 8192: recovered
+    f_lm against the seeded truth, sampled rings against the oracle, wavelet round trip."""
+    torch, api = _api()
+    gen = inputs.flm_real if real else inputs.flm_complex
+    flm = gen(L, 40 + L, 1)
+    plan = api.s2wav_plan_create(L, N, 2.0, 3, True, real, 1)
+    f = plan.harmonic_inverse(torch.from_numpy(flm).cuda())
+    got = plan.harmonic_forward(f, L * (2 * L - 1)).cpu().numpy().reshape(1, L, 2 * L - 1)
+    assert _relmax(got, flm) < FWD_TOL
+    rings = [0, 1, L // 3, L // 2, L - 2, L - 1]
+    ref = S.sht_inverse(flm[0], L, "f80", thetas=S.mw_thetas(L, "f80")[rings])
+    fn = f.cpu().numpy().reshape(L, 2 * L - 1)
+    ref = ref.real.astype(np.float64) if real else ref.astype(np.complex128)
+    assert np.abs(fn[rings] - ref).max() / np.abs(fn).max() < RT_TOL
+    w = plan.forward(f)
+    back = plan.inverse(w)
+    assert float((back - f).abs().max() / f.abs().max()) < RT_TOL
+    plan.close()
