@@ -8,6 +8,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <mutex>
@@ -154,6 +155,19 @@ struct s2w_plan {
     double *Kfull_inv;  // [P nodes][P p]  K_p(r_i)
     double *phi_ball;   // [P][L] sqrt(4pi/(2l+1)) Phi_{l0p}
     size_t ws_shell_elems;  // ball: elements of one [P][Mfull][L] harmonic array
+    // CUDA graphs of whole transforms (s2w_plan_forward / s2w_plan_inverse), keyed by direction and buffer addresses:
+    // a transform is 40 (sphere) to 900 (ball) small launches, replayed as one graph launch after its first call.
+    // The only mutable state of a plan; guarded by graph_mu.
+    struct GraphEntry {
+        int dir;
+        const void *in;
+        void *out, *work;
+        cudaGraphExec_t exec;
+        unsigned long long launches;
+    };
+    mutable std::vector<GraphEntry> graphs;
+    mutable cudaStream_t capture_stream;
+    mutable std::mutex graph_mu;
 };
 
 namespace s2w {
@@ -1180,6 +1194,7 @@ int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int m
     S2W_CUDA_CHECK(cudaSetDevice(device));
     s2w_plan *p = new s2w_plan();
     p->kind = 0;
+    p->capture_stream = 0;
     p->L = L;
     p->N = N;
     p->P = 1;
@@ -1279,6 +1294,7 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
     S2W_CUDA_CHECK(cudaSetDevice(device));
     s2w_plan *p = new s2w_plan();
     p->kind = 1;
+    p->capture_stream = 0;
     p->L = L;
     p->N = N;
     p->P = P;
@@ -1401,6 +1417,8 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
 int s2w_plan_destroy(s2w_plan *p)
 {
     if (!p) return S2W_OK;
+    for (auto &g : p->graphs) cudaGraphExecDestroy(g.exec);
+    if (p->capture_stream) cudaStreamDestroy(p->capture_stream);
     p->pool.release();
     delete p;
     return S2W_OK;
@@ -1455,14 +1473,67 @@ size_t s2w_plan_workspace_bytes(const s2w_plan *p) { return p ? p->ws_bytes : 0;
 
 static void *align256(void *p) { return (void *)(((uintptr_t)p + 255) & ~(uintptr_t)255); }
 
+// One whole transform, directly on `s` or -- unless the per-class timers are on or S2W_NO_GRAPH is set -- as a CUDA
+// graph: captured on the plan's private stream at the first call with a given (direction, in, out, work) and replayed
+// on the caller's stream afterwards (the legacy default stream cannot be captured, a private one can).
+static int run_transform(const s2w_plan *p, int dir, const void *in, void *out, void *work, cudaStream_t s)
+{
+    auto direct = [&](cudaStream_t st) {
+        if (p->kind == 1) return dir == 0 ? ball_forward(p, in, out, work, st) : ball_inverse(p, in, out, work, st);
+        return dir == 0 ? sphere_forward(p, in, out, work, st) : sphere_inverse(p, in, out, work, st);
+    };
+    static const bool no_graph = getenv("S2W_NO_GRAPH") != 0;
+    if (no_graph || g_timing) return direct(s);
+    std::lock_guard<std::mutex> lock(p->graph_mu);
+    for (auto &g : p->graphs)
+        if (g.dir == dir && g.in == in && g.out == out && g.work == work) {
+            S2W_CUDA_CHECK(cudaGraphLaunch(g.exec, s));
+            g_launches += g.launches;
+            return S2W_OK;
+        }
+    if (!p->capture_stream) S2W_CUDA_CHECK(cudaStreamCreateWithFlags(&p->capture_stream, cudaStreamNonBlocking));
+    const unsigned long long n0 = g_launches;
+    S2W_CUDA_CHECK(cudaStreamBeginCapture(p->capture_stream, cudaStreamCaptureModeThreadLocal));
+    const int rc = direct(p->capture_stream);
+    cudaGraph_t graph = 0;
+    const cudaError_t ce = cudaStreamEndCapture(p->capture_stream, &graph);
+    const unsigned long long nl = g_launches - n0;
+    g_launches = n0;
+    if (rc || ce != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        if (rc) return rc;
+        return direct(s);  // capture not possible here: run the launches directly
+    }
+    s2w_plan::GraphEntry e;
+    e.dir = dir;
+    e.in = in;
+    e.out = out;
+    e.work = work;
+    e.launches = nl;
+    const cudaError_t ci = cudaGraphInstantiate(&e.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ci != cudaSuccess) {
+        cudaGetLastError();
+        return direct(s);
+    }
+    if (p->graphs.size() >= 16) {  // bounded cache: drop the oldest
+        cudaGraphExecDestroy(p->graphs.front().exec);
+        p->graphs.erase(p->graphs.begin());
+    }
+    p->graphs.push_back(e);
+    S2W_CUDA_CHECK(cudaGraphLaunch(e.exec, s));
+    g_launches += nl;
+    return S2W_OK;
+}
+
 int s2w_plan_forward(const s2w_plan *p, const void *in, void *out, void *work, void *stream)
 {
     if (!p || !in || !out || !work) {
         set_error("null pointer");
         return S2W_EINVAL;
     }
-    if (p->kind == 1) return ball_forward(p, in, out, align256(work), (cudaStream_t)stream);
-    return sphere_forward(p, in, out, align256(work), (cudaStream_t)stream);
+    return run_transform(p, 0, in, out, align256(work), (cudaStream_t)stream);
 }
 
 int s2w_plan_inverse(const s2w_plan *p, const void *in, void *out, void *work, void *stream)
@@ -1471,8 +1542,7 @@ int s2w_plan_inverse(const s2w_plan *p, const void *in, void *out, void *work, v
         set_error("null pointer");
         return S2W_EINVAL;
     }
-    if (p->kind == 1) return ball_inverse(p, in, out, align256(work), (cudaStream_t)stream);
-    return sphere_inverse(p, in, out, align256(work), (cudaStream_t)stream);
+    return run_transform(p, 1, in, out, align256(work), (cudaStream_t)stream);
 }
 
 int s2w_plan_harmonic_forward(const s2w_plan *p, const void *f, void *flm, void *work, void *stream)
