@@ -8,80 +8,90 @@
 //   out[r][c] (+)= wout[r][l(c)] * sum_k A[r][k] * win[k][l(c)] * in[k][c],      l(c) = c mod Lfull,
 //
 // where the optional real weights win / wout carry the (p, l)-dependent scaling filter sqrt(4pi/(2l+1)) Phi_{l0p}
-// (Eq. 35; it is not separable, reading R9).  A dense fp64 contraction: 64 x 64 output tile per block,
-// 4 rows x 4 complex columns per thread, operands staged through shared memory in k-chunks of 16.
+// (Eq. 35; it is not separable, reading R9).  A dense fp64 contraction on the FP64 tensor pipe
+// (mma.sync.m8n8k4.f64): 64 rows x 64 complex columns per block, operands staged through shared memory.
 #include "kernels.h"
 
 namespace s2w {
 
 namespace {
 
-#define RAD_TR 64   // rows per block
-#define RAD_TC 64   // complex columns per block
-#define RAD_TK 16   // k-chunk
+#define RAD_TR 64    // rows per block
+#define RAD_TC 128   // real columns (64 complex) per block
+#define RAD_TK 16    // k-chunk
+#define RAD_SA 17    // row stride of the A tile (doubles)
+#define RAD_SB 132   // row stride of the B tile: 4 k-rows x 8 columns of a fragment land in distinct banks
 
+__device__ __forceinline__ void dmma884_r(double &c0, double &c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+// FP64 tensor pipe: D[row][col] += A[row][k] B[k][col] with the complex shell arrays read as 2 cols real columns.
+// Block = 64 rows x 128 real columns, 8 warps of 16 rows x 64 columns (2 x 8 accumulator fragments); operands staged
+// through shared memory in k-chunks of 16 (the input weight w_in is applied while staging B).
 __global__ void __launch_bounds__(256) radial_kernel(const double *__restrict__ A, int R, int K,
                                                     const cplx *__restrict__ in, cplx *__restrict__ out, size_t cols,
                                                     int Lfull, const double *__restrict__ win,
                                                     const double *__restrict__ wout, int accumulate)
 {
-    __shared__ double sA[RAD_TK][RAD_TR + 1];
-    __shared__ cplx sX[RAD_TK][RAD_TC];
-    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;  // tx: column group, ty: row group
-    const size_t c0 = (size_t)blockIdx.x * RAD_TC;
+    __shared__ double sA[RAD_TR * RAD_SA];
+    __shared__ double sB[RAD_TK * RAD_SB];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int fr = lane >> 2, fk = lane & 3;
+    const int wr0 = (warp & 3) * 16, wc0 = (warp >> 2) * 64;  // this warp's rows / real columns inside the block tile
+    const size_t dc0 = (size_t)blockIdx.x * RAD_TC;            // first real column of the block
     const int r0 = blockIdx.y * RAD_TR;
 
-    cplx acc[4][4];
+    double acc[2][8][2];
 #pragma unroll
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < 2; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] = cmake(0.0, 0.0);
+        for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
     for (int k0 = 0; k0 < K; k0 += RAD_TK) {
         __syncthreads();
-        for (int e = threadIdx.x; e < RAD_TK * RAD_TR; e += 256) {
+        for (int e = threadIdx.x; e < RAD_TR * RAD_TK; e += 256) {
             const int kk = e & (RAD_TK - 1), rr = e >> 4;
             const int r = r0 + rr, k = k0 + kk;
-            sA[kk][rr] = (r < R && k < K) ? A[(size_t)r * K + k] : 0.0;
+            sA[rr * RAD_SA + kk] = (r < R && k < K) ? A[(size_t)r * K + k] : 0.0;
         }
-        for (int e = threadIdx.x; e < RAD_TK * RAD_TC; e += 256) {
-            const int cc = e & (RAD_TC - 1), kk = e >> 6;
-            const size_t c = c0 + cc;
+        for (int e = threadIdx.x; e < RAD_TK * (RAD_TC / 2); e += 256) {
+            const int cc = e & (RAD_TC / 2 - 1), kk = e >> 6;  // complex column inside the tile, k inside the chunk
+            const size_t c = dc0 / 2 + cc;
             const int k = k0 + kk;
             cplx v = cmake(0.0, 0.0);
             if (c < cols && k < K) {
                 v = in[(size_t)k * cols + c];
                 if (win) v = cscale(v, win[(size_t)k * Lfull + (int)(c % (size_t)Lfull)]);
             }
-            sX[kk][cc] = v;
+            *reinterpret_cast<cplx *>(&sB[kk * RAD_SB + 2 * cc]) = v;
         }
         __syncthreads();
 #pragma unroll
-        for (int kk = 0; kk < RAD_TK; ++kk) {
-            double a[4];
-            cplx x[4];
+        for (int kq = 0; kq < RAD_TK; kq += 4) {
+            const double a0 = sA[(wr0 + fr) * RAD_SA + kq + fk], a1 = sA[(wr0 + 8 + fr) * RAD_SA + kq + fk];
+            const double *brow = sB + (kq + fk) * RAD_SB + wc0 + fr;
 #pragma unroll
-            for (int i = 0; i < 4; ++i) a[i] = sA[kk][ty * 4 + i];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) x[j] = sX[kk][tx + 16 * j];
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    acc[i][j].x = fma(a[i], x[j].x, acc[i][j].x);
-                    acc[i][j].y = fma(a[i], x[j].y, acc[i][j].y);
-                }
+            for (int j = 0; j < 8; ++j) {
+                const double b = brow[8 * j];
+                dmma884_r(acc[0][j][0], acc[0][j][1], a0, b);
+                dmma884_r(acc[1][j][0], acc[1][j][1], a1, b);
+            }
         }
     }
+    // D fragment: row fr of the octet, real columns 2 fk + {0, 1} = one complex element
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const int r = r0 + ty * 4 + i;
+    for (int i = 0; i < 2; ++i) {
+        const int r = r0 + wr0 + 8 * i + fr;
         if (r >= R) continue;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const size_t c = c0 + tx + 16 * j;
+        for (int j = 0; j < 8; ++j) {
+            const size_t c = (dc0 + wc0 + 8 * j) / 2 + fk;
             if (c >= cols) continue;
-            cplx v = acc[i][j];
+            cplx v = cmake(acc[i][j][0], acc[i][j][1]);
             if (wout) v = cscale(v, wout[(size_t)r * Lfull + (int)(c % (size_t)Lfull)]);
             cplx *dst = &out[(size_t)r * cols + c];
             if (accumulate) v = cadd(v, *dst);
@@ -96,7 +106,7 @@ int launch_radial(const double *A, int R, int K, const cplx *in, cplx *out, size
                   const double *wout, bool accumulate, cudaStream_t st)
 {
     if (R <= 0 || cols == 0) return S2W_OK;
-    dim3 grid((unsigned)((cols + RAD_TC - 1) / RAD_TC), (R + RAD_TR - 1) / RAD_TR);
+    dim3 grid((unsigned)((2 * cols + RAD_TC - 1) / RAD_TC), (R + RAD_TR - 1) / RAD_TR);
     S2W_LAUNCH_C(S2W_K_RADIAL, radial_kernel, grid, 256, 0, st, A, R, K, in, out, cols, Lfull, win, wout,
                  accumulate ? 1 : 0);
     return S2W_OK;
