@@ -34,7 +34,7 @@ namespace s2w {
 
 namespace {
 
-#define WIG_TL 64   // l-tile of the inverse kernel
+#define WIG_TL 64   // l-tile of the inverse kernels (the recursion kernel uses 256 on grids with several groups per warp)
 #define WIG_TLF 64  // l-tile of the forward kernel
 #define RAMP_THRESHOLD_EXP (-70)
 
@@ -206,9 +206,10 @@ template <int NC, int R, int MAXT, int NS>
 __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_inverse_kernel(WigArgs A)
 {
     constexpr int NCT = NC * NS;
-    __shared__ double2 s_ag[WIG_TL];
-    __shared__ double2 s_e[WIG_TL];
-    __shared__ double s_X[2][WIG_TL * NCT];  // [0]: X_l, [1]: (-1)^l X_l (southern warps)
+    constexpr int TL = R == 1 ? 64 : 256;  // l-tile: long tiles (fewer barriers) on the large grids, short on small ones
+    __shared__ double2 s_ag[TL];
+    __shared__ double2 s_e[TL];
+    __shared__ double s_X[2][TL * NCT];  // [0]: X_l, [1]: (-1)^l X_l (southern warps)
 
     const int m = blockIdx.x, chunk = blockIdx.y;
     const int Lg = A.Lg, Lfull = A.Lfull, G = A.G;
@@ -255,11 +256,11 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_inverse_ke
         if (G > 1 && gsrow[1] < bmin) bmin = gsrow[1];
         if (bmin < l0) bmin = l0;
 
-        for (int lt = bmin & ~(WIG_TL - 1); lt < Lg; lt += WIG_TL) {
+        for (int lt = bmin & ~(TL - 1); lt < Lg; lt += TL) {
             __syncthreads();
-            stage_coef<WIG_TL>(crow, lt, l0, Lg, s_ag, s_e);
-            for (int i = threadIdx.x; i < WIG_TL * (NCT / 2); i += T) {
-                const int k = i / WIG_TL, ll = i % WIG_TL;  // consecutive threads -> consecutive l (coalesced)
+            stage_coef<TL>(crow, lt, l0, Lg, s_ag, s_e);
+            for (int i = threadIdx.x; i < TL * (NCT / 2); i += T) {
+                const int k = i / TL, ll = i % TL;  // consecutive threads -> consecutive l (coalesced)
                 const int sc = k / (NC / 2), kk = k - sc * (NC / 2);
                 const int l = lt + ll;
                 const ColInfo ci = col_info(A, chunk * (NC / 2) + kk);
@@ -279,7 +280,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_inverse_ke
             }
             __syncthreads();
 
-            const int lb = (lt + WIG_TL) < Lg ? (lt + WIG_TL) : Lg;
+            const int lb = (lt + TL) < Lg ? (lt + TL) : Lg;
             int l = lt > gs[0] ? lt : gs[0];
             while (l < lb) {
                 int ra = 0;
