@@ -35,7 +35,7 @@ namespace s2w {
 namespace {
 
 #define WIG_TL 64   // l-tile of the inverse kernels (the recursion kernel uses 256 on grids with several groups per warp)
-#define WIG_TLF 64  // l-tile of the forward kernel
+#define FWD_TILE(R) ((R) == 1 ? 64 : 256)  // l-tile of the forward kernel: short on small grids, long on large ones
 #define RAMP_THRESHOLD_EXP (-70)
 
 __device__ __forceinline__ size_t tri_off(int m, int Lfull) { return (size_t)m * Lfull - ((size_t)m * (m - 1)) / 2 - m; }
@@ -383,12 +383,11 @@ template <int R, int MAXT, bool PRE, bool FUSE>
 __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_kernel(WigArgs A)
 {
     constexpr int NC = 8;
-    constexpr int NW = MAXT / 32;
-    __shared__ double2 s_ag[WIG_TLF];
-    __shared__ double2 s_e[WIG_TLF];
-    extern __shared__ double s_dyn[];  // s_red [NW][WIG_TLF][NC], then the B-fragment tiles [W][R][FWD_GT]
-    double (*s_red)[WIG_TLF][NC] = reinterpret_cast<double (*)[WIG_TLF][NC]>(s_dyn);
-    double *s_dt = s_dyn + NW * WIG_TLF * NC;
+    constexpr int TLF = FWD_TILE(R);
+    __shared__ double2 s_ag[TLF];
+    __shared__ double2 s_e[TLF];
+    __shared__ double s_red[TLF][NC];  // per-tile sums over all warps (shared-memory atomics), true sign
+    extern __shared__ double s_dt[];   // the B-fragment tiles [W][R][FWD_GT]
 
     const int m = blockIdx.x, chunk = blockIdx.y;
     const int Lg = A.Lg, Lfull = A.Lfull, G = A.G;
@@ -452,21 +451,22 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
         if (G > 1 && gsrow[1] < first) first = gsrow[1];
         if (first < l0) first = l0;
 
-        for (int lt = first & ~(WIG_TLF - 1); lt < Lg; lt += WIG_TLF) {
+        for (int lt = first & ~(TLF - 1); lt < Lg; lt += TLF) {
             __syncthreads();
-            if (!PRE) {
-                stage_coef<WIG_TLF>(crow, lt, l0, Lg, s_ag, s_e);
-                __syncthreads();
-            }
-            const bool want = lt + WIG_TLF > lacc;  // this tile has outputs
+            for (int i = threadIdx.x; i < TLF * NC; i += T) (&s_red[0][0])[i] = 0.0;
+            if (!PRE) stage_coef<TLF>(crow, lt, l0, Lg, s_ag, s_e);
+            __syncthreads();
+            const bool want = lt + TLF > lacc;  // this tile has outputs
             const double *se = reinterpret_cast<const double *>(s_e) + hemi;
 #pragma unroll 1
-            for (int oc = 0; oc < WIG_TLF / 8; ++oc) {
+            for (int oc = 0; oc < TLF / 8; ++oc) {
                 const int lo = lt + 8 * oc;
                 double c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
+                bool contributed = false;
                 if (PRE) {
                     // precomputed-kernel variant (a9): B-fragments straight from the d-table in HBM
                     if (gs[0] < lo + 8 && lo < Lg && want && lo + 8 > lacc) {
+                        contributed = true;
                         const int lrow = lo + (lane >> 2);
                         const bool ok = lrow >= l0 && lrow < Lg;
                         const double *trow = A.dtab + ((size_t)tab * A.tri_g + tri_off(m, Lg) + (ok ? lrow : l0)) *
@@ -487,6 +487,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                     }
                 } else if (gs[0] < lo + 8 && lo < Lg) {
                     const bool mm = want && (lo + 8 > lacc);
+                    contributed = mm;
                     int ra = 0;
                     bool starting = false;
 #pragma unroll
@@ -543,16 +544,18 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                     }
                 }
                 // D fragment: row (column index) lane / 4, degrees 2 (lane % 4) + {0, 1} of the octet
-                if (want) {
-                    s_red[warp][8 * oc + 2 * fk][fc] = c0 + c2;
-                    s_red[warp][8 * oc + 2 * fk + 1][fc] = c1 + c3;
+                // (southern warps: d = (-1)^l d~, and the octet starts at an even degree)
+                if (contributed) {
+                    const double v0 = c0 + c2, v1 = c1 + c3;
+                    atomicAdd(&s_red[8 * oc + 2 * fk][fc], v0);
+                    atomicAdd(&s_red[8 * oc + 2 * fk + 1][fc], (!PRE && hemi) ? -v1 : v1);
                 }
             }
             if (!want) continue;
             __syncthreads();
             // cross-warp sum, output filter, accumulate into f_lm
-            for (int i = threadIdx.x; i < WIG_TLF * (NC / 2); i += T) {
-                const int k = i / WIG_TLF, ll = i % WIG_TLF;
+            for (int i = threadIdx.x; i < TLF * (NC / 2); i += T) {
+                const int k = i / TLF, ll = i % TLF;
                 const int l = lt + ll;
                 if (fuse && k >= 2) continue;  // fused: k = complex column, both scales summed below
                 const ColInfo ci = col_info(A, fuse ? k : chunk * (NC / 2) + k);
@@ -561,20 +564,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                 cplx val = cmake(0.0, 0.0);
                 for (int sc = 0; sc < (fuse ? 2 : 1); ++sc) {
                     const int c0i = 2 * k + 4 * sc;
-                    double re = 0.0, im = 0.0, reS = 0.0, imS = 0.0;
-                    for (int w = 0; w < W; w += 2) {
-                        re += s_red[w][ll][c0i];
-                        im += s_red[w][ll][c0i + 1];
-                        reS += s_red[w + 1][ll][c0i];
-                        imS += s_red[w + 1][ll][c0i + 1];
-                    }
-                    if (!PRE && (l & 1)) {
-                        re -= reS;
-                        im -= imS;
-                    } else {
-                        re += reS;
-                        im += imS;
-                    }
+                    const double re = s_red[ll][c0i], im = s_red[ll][c0i + 1];
                     const cplx Gf = (sc ? A.filt2 : A.filt)[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
                     val = cadd(val, cmul(Gf, cmake(re, im)));
                 }
@@ -811,12 +801,11 @@ void launch_inv_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
 template <int R, int MAXT, bool PRE, bool FUSE>
 int launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
 {
-    const size_t red = (size_t)(MAXT / 32) * WIG_TLF * 8 * sizeof(double);
-    const size_t smem = red + (PRE ? 0 : (size_t)(T / 32) * R * FWD_GT * sizeof(double));
+    const size_t smem = PRE ? 0 : (size_t)(T / 32) * R * FWD_GT * sizeof(double);
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(wigner_forward_kernel<R, MAXT, PRE, FUSE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)(red + (size_t)(MAXT / 32) * R * FWD_GT * sizeof(double)));
+                                             (int)((size_t)(MAXT / 32) * R * FWD_GT * sizeof(double)));
         if (e != cudaSuccess) {
             set_error(std::string("cudaFuncSetAttribute(wigner_forward_kernel): ") + cudaGetErrorString(e));
             return S2W_ECUDA;
