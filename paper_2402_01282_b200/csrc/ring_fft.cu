@@ -312,6 +312,115 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
 // ring t0+1 in the imaginary part), as in a1; the rows n > 0 are done ring by ring.  5 instead of 6 convolutions per
 // ring pair at N = 5.
 // ---------------------------------------------------------------------------------------------------------------
+// The same for at most 9 gamma samples (N <= 5), without read-modify-write of the gamma planes: the rows are done
+// ring by ring, the transforms V_n(alpha) of all rows but the last are parked in the ring's own output planes (V_0 in
+// plane 0, row i in planes 2i+1, 2i+2: at most 2N-3 of the 2N-1 planes), and the pass of the last row reads them back
+// -- each thread its own alpha samples, so program order is all the ordering needed -- and writes every plane once:
+//   W(alpha, gamma_g) = V_0(alpha) + 2 Re sum_{n>0} e^{i n gamma_g} V_n(alpha).
+__device__ __forceinline__ void so3_inv_pair_few(const cplx *__restrict__ F, double *__restrict__ W, size_t sig_stride,
+                                                 const So3Args &A, const FftTab &T, cplx *buf, const cplx *s_tw,
+                                                 cplx *gph)
+{
+    const int n = T.n, L = T.L, M = T.M;
+    const int t0 = 2 * blockIdx.x, b = blockIdx.y;
+    const bool has1 = t0 + 1 < L;
+    const int ng = 2 * A.N - 1;
+    const cplx *Fb = F + (size_t)b * A.nrows * L * L;
+    double *Wb = W + (size_t)b * sig_stride;
+    const size_t plane = (size_t)L * n;
+    int q0 = -1, np = 0;  // the row n = 0 and the number of rows n > 0
+    for (int q = 0; q < A.nn; ++q) {
+        if (A.n_val[q] == 0) q0 = q;
+        if (A.n_val[q] > 0) {
+            for (int g = threadIdx.x; g < ng; g += blockDim.x) gph[np * ng + g] = cis_2pi_frac(A.n_val[q] * g, ng);
+            ++np;
+        }
+    }
+    if (q0 >= 0) {
+        const cplx *X0 = Fb + ((size_t)A.n_row[q0] * L + t0) * L, *X1 = X0 + L;
+        for (int k = threadIdx.x; k < M; k += blockDim.x) {
+            cplx v = cmake(0.0, 0.0);
+            if (k < n) {
+                const int m = k < L ? k : n - k;
+                cplx a = X0[m], c = has1 ? X1[m] : cmake(0.0, 0.0);
+                if (k >= L) {
+                    a = cconj(a);
+                    c = cconj(c);
+                }
+                v = cmulc(cmake(a.x - c.y, a.y + c.x), __ldg(&T.chirp[k]));
+            }
+            buf[S2W_PAD(k)] = v;
+        }
+        __syncthreads();
+        fft_convolve(buf, T, s_tw, T.bhat_p);
+        for (int a = threadIdx.x; a < n; a += blockDim.x) {
+            const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));  // V_0 of ring t0 + i V_0 of ring t0+1
+            double *Wr = Wb + (size_t)t0 * n + a;
+            for (int g = 0; g < (np ? 1 : ng); ++g) {
+                Wr[g * plane] = v.x;
+                if (has1) Wr[g * plane + n] = v.y;
+            }
+        }
+        __syncthreads();
+    }
+    for (int r = 0; r < (has1 ? 2 : 1); ++r) {
+        const int t = t0 + r;
+        int i = 0;
+        for (int q = 0; q < A.nn; ++q) {
+            if (A.n_val[q] <= 0) continue;
+            const cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * L;
+            const cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * L;
+            for (int k = threadIdx.x; k < M; k += blockDim.x) {
+                cplx v = cmake(0.0, 0.0);
+                if (k < n) v = cmulc(k < L ? Fp[k] : cconj(Fm[n - k]), __ldg(&T.chirp[k]));
+                buf[S2W_PAD(k)] = v;
+            }
+            __syncthreads();
+            fft_convolve(buf, T, s_tw, T.bhat_p);
+            if (i + 1 < np) {
+                for (int a = threadIdx.x; a < n; a += blockDim.x) {
+                    const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
+                    double *Wr = Wb + (size_t)t * n + a;
+                    Wr[(2 * i + 1) * plane] = v.x;
+                    Wr[(2 * i + 2) * plane] = v.y;
+                }
+            } else {
+                for (int a = threadIdx.x; a < n; a += blockDim.x) {
+                    const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
+                    double *Wr = Wb + (size_t)t * n + a;
+                    double sc[7];
+#pragma unroll
+                    for (int s = 0; s < 7; ++s) sc[s] = 0.0;
+                    if (q0 >= 0) sc[0] = Wr[0];
+#pragma unroll
+                    for (int s = 1; s < 7; ++s)
+                        if (s < 2 * np - 1) sc[s] = Wr[s * plane];
+                    double out[9];
+#pragma unroll
+                    for (int g = 0; g < 9; ++g) {
+                        const cplx ph = gph[(np - 1) * ng + (g < ng ? g : 0)];
+                        out[g] = fma(2.0, ph.x * v.x - ph.y * v.y, sc[0]);
+                    }
+#pragma unroll
+                    for (int j = 0; j < 3; ++j)
+                        if (j + 1 < np) {
+#pragma unroll
+                            for (int g = 0; g < 9; ++g) {
+                                const cplx ph = gph[j * ng + (g < ng ? g : 0)];
+                                out[g] = fma(2.0, ph.x * sc[2 * j + 1] - ph.y * sc[2 * j + 2], out[g]);
+                            }
+                        }
+#pragma unroll
+                    for (int g = 0; g < 9; ++g)
+                        if (g < ng) Wr[g * plane] = out[g];
+                }
+            }
+            __syncthreads();
+            ++i;
+        }
+    }
+}
+
 __global__ void __launch_bounds__(256, 3) so3_inv_pair_kernel(const cplx *__restrict__ F, double *__restrict__ W,
                                                              size_t sig_stride, So3Args A, FftTab T)
 {
@@ -326,6 +435,10 @@ __global__ void __launch_bounds__(256, 3) so3_inv_pair_kernel(const cplx *__rest
     const cplx *Fb = F + (size_t)b * A.nrows * L * L;
     double *Wb = W + (size_t)b * sig_stride;
     const size_t plane = (size_t)L * n;
+    if (ng <= 9) {
+        so3_inv_pair_few(F, W, sig_stride, A, T, buf, s_tw, gph);
+        return;
+    }
     bool first = true;
     for (int q = 0; q < A.nn; ++q) {
         const int nv = A.n_val[q];
@@ -843,11 +956,30 @@ __global__ void __launch_bounds__(256) kernel_spectrum_kernel(cplx *khat, int ki
 
 size_t fft_smem_bytes(const FftTab &T) { return (size_t)fft_padded_len(T.M) * sizeof(cplx); }
 
+// Kernels that may need more than 48 KB of dynamic shared memory are raised to the device's opt-in limit, never to
+// the size of one launch: the attribute belongs to the function, not to the launch, so a per-launch value would be
+// lowered again by the next (smaller) launch -- under a captured graph, or with two host threads, that is a race with
+// the launches that still need the larger size.
 template <typename K>
 int set_smem(K kernel, size_t bytes)
 {
     if (bytes > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        static int optin = 0;
+        if (!optin) {
+            int dev = 0;
+            cudaGetDevice(&dev);
+            if (cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) optin = 0;
+        }
+        cudaFuncAttributes fa;
+        if (cudaFuncGetAttributes(&fa, kernel) != cudaSuccess) fa.sharedSizeBytes = 0;
+        const int room = optin - (int)fa.sharedSizeBytes;  // the limit covers static + dynamic
+        if (room < 0 || (size_t)room < bytes) {
+            cudaGetLastError();
+            set_error("shared memory per block: the transform length needs more than the device offers");
+            return S2W_ECUDA;
+        }
+        if (fa.maxDynamicSharedSizeBytes == room) return S2W_OK;
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, room);
         if (e != cudaSuccess) {
             set_error(std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
             return S2W_ECUDA;
