@@ -326,3 +326,29 @@ def test_large_band_limits_that_are_not_powers_of_two(L, N, real):
     back = plan.inverse(w)
     assert float((back - f).abs().max() / f.abs().max()) < RT_TOL
     plan.close()
+
+
+@pytest.mark.parametrize("N", [1, 2, 4, 5, 6])
+def test_real_ring_pair_kernels_agree_with_the_complex_path_on_large_grids(N):
+    """Real signals on grids with Bluestein length >= 4096 take the ring-pair (alpha, gamma) kernels (a8): with and
+    without a row n = 0 (odd / even N), one or two rows n > 0 (parked in the output planes, no read-modify-write)
+    and more than 9 gamma samples (N = 6: accumulating path).  The complex plan, which runs the ring-by-ring kernels
+    checked against the oracle at small sizes, must give the same coefficients and the same synthesis."""
+    torch, api = _api()
+    L = 520
+    flm = inputs.flm_real(L, 900 + N, 1)
+    pr = api.s2wav_plan_create(L, N, 2.0, 7, True, True, 1)
+    pc = api.s2wav_plan_create(L, N, 2.0, 7, True, False, 1)
+    f = pr.harmonic_inverse(torch.from_numpy(flm).cuda())
+    wr = pr.forward(f)
+    wc = pc.forward(f.to(torch.complex128))
+    scale = float(wc.abs().max())
+    assert float(wc.imag.abs().max()) < 1e-12 * scale
+    assert float((wr - wc.real).abs().max()) < 1e-12 * scale
+    br = pr.inverse(wr)
+    bc = pc.inverse(wc)
+    fmax = float(f.abs().max())
+    assert float((br - bc.real).abs().max()) < RT_TOL * fmax
+    assert float((br - f).abs().max()) < RT_TOL * fmax
+    pr.close()
+    pc.close()
