@@ -506,6 +506,111 @@ __global__ void __launch_bounds__(256, 3) so3_inv_pair_kernel(const cplx *__rest
     }
 }
 
+// The analysis counterpart for at most 9 gamma samples: the gamma planes of a ring are read ONCE; the gamma sums of
+// all its rows, Y_n(alpha) = 1/(2N-1) sum_g e^{-i n gamma_g} W(alpha, gamma_g), are formed together, the row n = 0
+// goes straight into the shared-memory buffer (ring t0 real part, ring t0+1 imaginary part) and the rows n > 0 are
+// parked, chirp applied, in the ring's own output rows F_{., n}, F_{., -n} (2L >= 2L-1 entries), from where the fill
+// of that row's convolution takes them back -- each thread its own alpha samples -- before the row is overwritten.
+__device__ __forceinline__ void so3_fwd_pair_few(const double *__restrict__ W, cplx *__restrict__ F, size_t sig_stride,
+                                                 const So3Args &A, const FftTab &T, cplx *buf, const cplx *s_tw,
+                                                 cplx *gph)
+{
+    const int n = T.n, L = T.L, M = T.M;
+    const int t0 = 2 * blockIdx.x, b = blockIdx.y;
+    const bool has1 = t0 + 1 < L;
+    const int ng = 2 * A.N - 1;
+    const double inv_ng = 1.0 / (double)ng, inv_n = 1.0 / (double)n;
+    cplx *Fb = F + (size_t)b * A.nrows * L * L;
+    const double *Wb = W + (size_t)b * sig_stride;
+    const size_t plane = (size_t)L * n;
+    __shared__ int s_rowp[4], s_rowm[4];
+    int q0 = -1, np = 0;
+    for (int q = 0; q < A.nn; ++q) {
+        if (A.n_val[q] == 0) q0 = q;
+        if (A.n_val[q] > 0) {
+            for (int g = threadIdx.x; g < ng; g += blockDim.x) gph[np * ng + g] = cis_2pi_frac(-A.n_val[q] * g, ng);
+            if (threadIdx.x == 0) {
+                s_rowp[np] = A.n_row[q];
+                s_rowm[np] = A.n_rowm[q];
+            }
+            ++np;
+        }
+    }
+    __syncthreads();
+    // gather pass: every gamma plane of both rings once
+    for (int r = 0; r < 2; ++r) {
+        const int t = t0 + r;
+        const bool live = r == 0 || has1;
+        for (int a = threadIdx.x; a < M; a += blockDim.x) {
+            if (a >= n) {
+                if (r == 0) buf[S2W_PAD(a)] = cmake(0.0, 0.0);
+                continue;
+            }
+            const cplx ch = __ldg(&T.chirp[a]);
+            double wv[9];
+#pragma unroll
+            for (int g = 0; g < 9; ++g) wv[g] = (live && g < ng) ? Wb[(size_t)t * n + a + g * plane] : 0.0;
+            double y0 = 0.0;
+#pragma unroll
+            for (int g = 0; g < 9; ++g) y0 += wv[g];
+            if (r == 0) {
+                buf[S2W_PAD(a)] = cmake(y0, 0.0);
+            } else {
+                cplx v = buf[S2W_PAD(a)];
+                v.y = y0;
+                buf[S2W_PAD(a)] = cmul(cscale(v, inv_ng), ch);
+            }
+            if (!live) continue;
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                if (i < np) {
+                    cplx y = cmake(0.0, 0.0);
+#pragma unroll
+                    for (int g = 0; g < 9; ++g) {
+                        const cplx ph = gph[i * ng + (g < ng ? g : 0)];
+                        y.x = fma(ph.x, wv[g], y.x);
+                        y.y = fma(ph.y, wv[g], y.y);
+                    }
+                    y = cmul(cscale(y, inv_ng), ch);
+                    cplx *dst = a < L ? Fb + ((size_t)s_rowp[i] * L + t) * L + a
+                                      : Fb + ((size_t)s_rowm[i] * L + t) * L + (a - L);
+                    *dst = y;
+                }
+        }
+    }
+    __syncthreads();
+    if (q0 >= 0) {
+        fft_convolve(buf, T, s_tw, T.bhat_m);
+        for (int k = threadIdx.x; k < n; k += blockDim.x) buf[S2W_PAD(k)] = cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k]));
+        __syncthreads();
+        cplx *F0 = Fb + ((size_t)A.n_row[q0] * L + t0) * L, *F1 = F0 + L;
+        for (int m = threadIdx.x; m < L; m += blockDim.x) {
+            const cplx a = buf[S2W_PAD(m)], c = cconj(buf[S2W_PAD(m == 0 ? 0 : n - m)]);
+            const cplx sm = cadd(a, c), df = csub(a, c);
+            F0[m] = cscale(sm, 0.5 * inv_n);
+            if (has1) F1[m] = cmake(0.5 * inv_n * df.y, -0.5 * inv_n * df.x);
+        }
+        __syncthreads();
+    }
+    for (int r = 0; r < (has1 ? 2 : 1); ++r) {
+        const int t = t0 + r;
+        for (int i = 0; i < np; ++i) {
+            cplx *Fp = Fb + ((size_t)s_rowp[i] * L + t) * L;
+            cplx *Fm = Fb + ((size_t)s_rowm[i] * L + t) * L;
+            for (int a = threadIdx.x; a < M; a += blockDim.x)
+                buf[S2W_PAD(a)] = a < L ? Fp[a] : (a < n ? Fm[a - L] : cmake(0.0, 0.0));
+            __syncthreads();
+            fft_convolve(buf, T, s_tw, T.bhat_m);
+            for (int m = threadIdx.x; m < L; m += blockDim.x) {
+                Fp[m] = cscale(cmul(buf[S2W_PAD(m)], __ldg(&T.chirp[m])), inv_n);
+                const int k = m == 0 ? 0 : n - m;
+                Fm[m] = cscale(cconj(cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k]))), inv_n);
+            }
+            __syncthreads();
+        }
+    }
+}
+
 __global__ void __launch_bounds__(256, 3) so3_fwd_pair_kernel(const double *__restrict__ W, cplx *__restrict__ F,
                                                              size_t sig_stride, So3Args A, FftTab T)
 {
@@ -521,6 +626,10 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_pair_kernel(const double *__re
     cplx *Fb = F + (size_t)b * A.nrows * L * L;
     const double *Wb = W + (size_t)b * sig_stride;
     const size_t plane = (size_t)L * n;
+    if (ng <= 9) {
+        so3_fwd_pair_few(W, F, sig_stride, A, T, buf, s_tw, gph);
+        return;
+    }
     for (int q = 0; q < A.nn; ++q) {
         const int nv = A.n_val[q];
         if (nv < 0) continue;
