@@ -131,6 +131,8 @@ struct Scale {
 
 using namespace s2w;
 
+#define S2W_LANES 4  // most lanes a captured sphere transform uses (workspace is sized for them)
+
 struct s2w_plan {
     int kind;  // 0 sphere, 1 ball
     int L, N, P, J0, J, J0p, Jp, multires, flags, batch, device;
@@ -168,6 +170,12 @@ struct s2w_plan {
     mutable std::vector<GraphEntry> graphs;
     mutable cudaStream_t capture_stream;
     mutable std::mutex graph_mu;
+    // lanes of a captured sphere transform (sphere_forward / sphere_inverse): the scales are independent, so they are
+    // dealt to S2W_LANES streams of the graph, each with its own F buffers (largest scale first, to the lane with the
+    // least work so far)
+    mutable cudaStream_t lane_stream[S2W_LANES - 1];
+    mutable cudaEvent_t lane_fork, lane_join[S2W_LANES - 1];
+    mutable bool lanes_on;  // set by run_transform while it captures
 };
 
 namespace s2w {
@@ -755,6 +763,66 @@ static Work carve(const s2w_plan *p, void *work)
     return w;
 }
 
+// The lanes of a captured transform: lane 0 is the capture stream with the caller's buffers, lane i > 0 has a stream
+// of the plan and two more F-sized buffers of the workspace.  Only under run_transform's capture (lanes_on):
+// streams and events belong to the plan, and the capture holds the plan's graph mutex.
+struct Lanes {
+    int n;
+    cudaStream_t s[S2W_LANES];
+    Work w[S2W_LANES];
+    double load[S2W_LANES];
+    int pick(double cost)  // the lane with the least work so far
+    {
+        int best = 0;
+        for (int i = 1; i < n; ++i)
+            if (load[i] < load[best]) best = i;
+        load[best] += cost;
+        return best;
+    }
+};
+
+static int lanes_fork(const s2w_plan *p, const Work &w, cplx *spare, cudaStream_t s, bool allow, Lanes *ln)
+{
+    ln->n = 1;
+    ln->s[0] = s;
+    ln->w[0] = w;
+    for (int i = 0; i < S2W_LANES; ++i) ln->load[i] = 0.0;
+    static const int nl = [] {
+        const char *e = getenv("S2W_LANES");
+        const int v = e ? atoi(e) : S2W_LANES;
+        return v < 1 ? 1 : (v > S2W_LANES ? S2W_LANES : v);
+    }();
+    if (!allow || !p->lanes_on || nl == 1) return S2W_OK;
+    const size_t Fsz = ((p->ws_F_elems + 15) / 16) * 16;
+    if (!p->lane_fork) S2W_CUDA_CHECK(cudaEventCreateWithFlags(&p->lane_fork, cudaEventDisableTiming));
+    S2W_CUDA_CHECK(cudaEventRecord(p->lane_fork, s));
+    for (int i = 1; i < nl; ++i) {
+        if (!p->lane_stream[i - 1]) {
+            S2W_CUDA_CHECK(cudaStreamCreateWithFlags(&p->lane_stream[i - 1], cudaStreamNonBlocking));
+            S2W_CUDA_CHECK(cudaEventCreateWithFlags(&p->lane_join[i - 1], cudaEventDisableTiming));
+        }
+        S2W_CUDA_CHECK(cudaStreamWaitEvent(p->lane_stream[i - 1], p->lane_fork, 0));
+        ln->s[i] = p->lane_stream[i - 1];
+        ln->w[i] = w;
+        ln->w[i].F = spare + (size_t)(2 * i - 2) * Fsz;  // `spare`: 2 (S2W_LANES - 1) F-sized buffers
+        ln->w[i].Ft = ln->w[i].F + Fsz;
+        ln->w[i].Ft2 = 0;
+    }
+    ln->n = nl;
+    return S2W_OK;
+}
+
+static int lanes_join(const s2w_plan *p, const Lanes &ln)
+{
+    for (int i = 1; i < ln.n; ++i) {
+        S2W_CUDA_CHECK(cudaEventRecord(p->lane_join[i - 1], ln.s[i]));
+        S2W_CUDA_CHECK(cudaStreamWaitEvent(ln.s[0], p->lane_join[i - 1], 0));
+    }
+    return S2W_OK;
+}
+
+static double scale_cost(const Scale &sc) { return (double)sc.Lj * sc.Lj * sc.Lj * (sc.st.nn + 0.01); }
+
 // pixels [B][L][2L-1] -> flmT
 static int sht_forward_dev(const s2w_plan *p, const Stage &st, const void *f, size_t sig_stride, int B, const Work &w,
                            bool zero_first, cudaStream_t s)
@@ -930,6 +998,9 @@ static int sphere_forward(const s2w_plan *p, const void *in, void *out, void *wo
     int rc;
     if ((rc = sht_forward_dev(p, p->sht, in, p->signal_elems, B, w, true, s))) return rc;
     const int ns = (int)p->scales.size();
+    Lanes ln;
+    if ((rc = lanes_fork(p, w, w.Ft2 + ((p->ws_F_elems + 15) / 16) * 16, s, !hp, &ln))) return rc;
+    const bool lanes = ln.n > 1;
     // the two top scales share one recursion when they can; they go first (their blocks are the big host copies)
     int rest = ns;
     if (ns >= 2 && scales_fusable(p, p->scales[ns - 2], p->scales[ns - 1], B)) {
@@ -940,16 +1011,20 @@ static int sphere_forward(const s2w_plan *p, const void *in, void *out, void *wo
         if (hp && (rc = hp->block_out(b.offset * esz, nn * b.Lj * (2 * b.Lj - 1) * esz, s))) return rc;
         if (hp && (rc = hp->block_out(a.offset * esz, nn * a.Lj * (2 * a.Lj - 1) * esz, s))) return rc;
         rest = ns - 2;
+        ln.load[0] += scale_cost(a) + scale_cost(b);  // the pair ran on lane 0 (the only one with an Ft2 buffer)
     }
-    for (int k = 0; k < rest; ++k) {
-        const Scale &sc = p->scales[hp ? rest - 1 - k : k];
-        if ((rc = scale_analysis(p, sc, B, w, (char *)out + sc.offset * esz, p->coeff_elems, s))) return rc;
+    for (int k = 0; k < rest; ++k) {  // largest first when pipelined: the lanes (or the host copies) stay balanced
+        const Scale &sc = p->scales[(hp || lanes) ? rest - 1 - k : k];
+        const int l = ln.pick(scale_cost(sc));
+        if ((rc = scale_analysis(p, sc, B, ln.w[l], (char *)out + sc.offset * esz, p->coeff_elems, ln.s[l]))) return rc;
         if (hp && (rc = hp->block_out(sc.offset * esz, nn * sc.Lj * (2 * sc.Lj - 1) * esz, s))) return rc;
     }
     // scaling coefficients
-    if ((rc = sht_inverse_dev(p, p->scaling, (char *)out + p->scaling_offset * esz, p->coeff_elems, B, w, s)))
+    const int l = ln.pick(0.0);
+    if ((rc = sht_inverse_dev(p, p->scaling, (char *)out + p->scaling_offset * esz, p->coeff_elems, B, ln.w[l], ln.s[l])))
         return rc;
     if (hp && (rc = hp->block_out(p->scaling_offset * esz, (size_t)p->Ls * (2 * p->Ls - 1) * esz, s))) return rc;
+    if ((rc = lanes_join(p, ln))) return rc;
     S2W_CUDA_CHECK(cudaPeekAtLastError());
     return S2W_OK;
 }
@@ -974,6 +1049,9 @@ static int sphere_inverse(const s2w_plan *p, const void *in, void *out, void *wo
     if ((rc = sht_forward_dev(p, p->scaling, (const char *)in + p->scaling_offset * esz, p->coeff_elems, B, w, true,
                               s)))
         return rc;
+    Lanes ln;
+    if ((rc = lanes_fork(p, w, w.Ft2 + ((p->ws_F_elems + 15) / 16) * 16, s, !hp, &ln))) return rc;
+    const bool lanes = ln.n > 1;
     int rest = ns;
     if (ns >= 2 && scales_fusable(p, p->scales[ns - 2], p->scales[ns - 1], B)) {
         const Scale &a = p->scales[ns - 2], &b = p->scales[ns - 1];
@@ -985,13 +1063,17 @@ static int sphere_inverse(const s2w_plan *p, const void *in, void *out, void *wo
                                        p->coeff_elems, s)))
             return rc;
         rest = ns - 2;
+        ln.load[0] += scale_cost(a) + scale_cost(b);
     }
-    for (int k = 0; k < rest; ++k) {
-        const int i = hp ? rest - 1 - k : k;
+    for (int k = 0; k < rest; ++k) {  // the forward contractions of all scales accumulate into flmT by atomics
+        const int i = (hp || lanes) ? rest - 1 - k : k;
         const Scale &sc = p->scales[i];
         if (hp) S2W_CUDA_CHECK(cudaStreamWaitEvent(s, ready[i], 0));
-        if ((rc = scale_synthesis(p, sc, B, w, (const char *)in + sc.offset * esz, p->coeff_elems, s))) return rc;
+        const int l = ln.pick(scale_cost(sc));
+        if ((rc = scale_synthesis(p, sc, B, ln.w[l], (const char *)in + sc.offset * esz, p->coeff_elems, ln.s[l])))
+            return rc;
     }
+    if ((rc = lanes_join(p, ln))) return rc;
     if ((rc = sht_inverse_dev(p, p->sht, out, p->signal_elems, B, w, s))) return rc;
     S2W_CUDA_CHECK(cudaPeekAtLastError());
     return S2W_OK;
@@ -1020,6 +1102,8 @@ static int ball_forward(const s2w_plan *p, const void *in, void *out, void *work
     w.flmT = bw.flm_sh;
     w.F = bw.F;
     w.Ft = bw.Ft;
+    w.Ft2 = 0;
+    cplx *spare = bw.Ft + ((p->ws_F_elems + 15) / 16) * 16;
     const int P = p->P, L = p->L;
     const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
     const size_t cols = (size_t)(p->real ? L : 2 * L - 1) * L;
@@ -1037,11 +1121,18 @@ static int ball_forward(const s2w_plan *p, const void *in, void *out, void *work
     while (i < p->scales.size()) {
         const Scale &first = p->scales[i];
         if ((rc = launch_radial(first.Kinv, first.Pj, first.Pj, bw.flmp, bw.flm_sh, cols, L, 0, 0, false, s))) return rc;
-        for (; i < p->scales.size() && p->scales[i].jp == first.jp; ++i) {
-            const Scale &sc = p->scales[i];
+        size_t e = i;
+        while (e < p->scales.size() && p->scales[e].jp == first.jp) ++e;
+        Lanes ln;  // the angular scales of one j' read the same flm_sh: dealt to the lanes, largest first
+        if ((rc = lanes_fork(p, w, spare, s, true, &ln))) return rc;
+        for (size_t k = e; k-- > i;) {
+            const Scale &sc = p->scales[k];
             const size_t stride = (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1);
-            if ((rc = scale_analysis(p, sc, sc.Pj, w, (char *)out + sc.offset * esz, stride, s))) return rc;
+            const int l = ln.pick(scale_cost(sc));
+            if ((rc = scale_analysis(p, sc, sc.Pj, ln.w[l], (char *)out + sc.offset * esz, stride, ln.s[l]))) return rc;
         }
+        if ((rc = lanes_join(p, ln))) return rc;
+        i = e;
     }
     S2W_CUDA_CHECK(cudaPeekAtLastError());
     return S2W_OK;
@@ -1054,6 +1145,8 @@ static int ball_inverse(const s2w_plan *p, const void *in, void *out, void *work
     w.flmT = bw.flm_sh;
     w.F = bw.F;
     w.Ft = bw.Ft;
+    w.Ft2 = 0;
+    cplx *spare = bw.Ft + ((p->ws_F_elems + 15) / 16) * 16;
     const int P = p->P, L = p->L;
     const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
     const size_t Mfull = p->real ? L : 2 * L - 1;
@@ -1068,11 +1161,19 @@ static int ball_inverse(const s2w_plan *p, const void *in, void *out, void *work
     while (i < p->scales.size()) {
         const Scale &first = p->scales[i];
         S2W_CUDA_CHECK(cudaMemsetAsync(bw.flm_sh, 0, (size_t)first.Pj * cols * sizeof(cplx), s));
-        for (; i < p->scales.size() && p->scales[i].jp == first.jp; ++i) {
-            const Scale &sc = p->scales[i];
+        size_t e = i;
+        while (e < p->scales.size() && p->scales[e].jp == first.jp) ++e;
+        Lanes ln;  // the angular scales of one j' accumulate into the same flm_sh by atomics
+        if ((rc = lanes_fork(p, w, spare, s, true, &ln))) return rc;
+        for (size_t k = e; k-- > i;) {
+            const Scale &sc = p->scales[k];
             const size_t stride = (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1);
-            if ((rc = scale_synthesis(p, sc, sc.Pj, w, (const char *)in + sc.offset * esz, stride, s))) return rc;
+            const int l = ln.pick(scale_cost(sc));
+            if ((rc = scale_synthesis(p, sc, sc.Pj, ln.w[l], (const char *)in + sc.offset * esz, stride, ln.s[l])))
+                return rc;
         }
+        if ((rc = lanes_join(p, ln))) return rc;
+        i = e;
         if ((rc = launch_radial(first.Kfwd, first.Pj, first.Pj, bw.flm_sh, bw.flmp, cols, L, 0, 0, true, s))) return rc;
     }
     // Z^-1
@@ -1195,6 +1296,12 @@ int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int m
     s2w_plan *p = new s2w_plan();
     p->kind = 0;
     p->capture_stream = 0;
+    for (int i = 0; i < S2W_LANES - 1; ++i) {
+        p->lane_stream[i] = 0;
+        p->lane_join[i] = 0;
+    }
+    p->lane_fork = 0;
+    p->lanes_on = false;
     p->L = L;
     p->N = N;
     p->P = 1;
@@ -1267,7 +1374,7 @@ int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int m
     p->signal_elems = (size_t)L * (2 * L - 1);
     p->ws_flm_elems = (size_t)batch * (p->real ? L : 2 * L - 1) * L;
     p->ws_F_elems = (size_t)batch * maxF;
-    p->ws_bytes = (((p->ws_flm_elems + 15) / 16) * 16 + 3 * (((p->ws_F_elems + 15) / 16) * 16)) * sizeof(cplx) + 256;
+    p->ws_bytes = (((p->ws_flm_elems + 15) / 16) * 16 + (3 + 2 * (S2W_LANES - 1)) * (((p->ws_F_elems + 15) / 16) * 16)) * sizeof(cplx) + 256;
     S2W_PLAN_TRY(cudaDeviceSynchronize() == cudaSuccess ? S2W_OK : S2W_ECUDA);
     *out = p;
     return S2W_OK;
@@ -1295,6 +1402,12 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
     s2w_plan *p = new s2w_plan();
     p->kind = 1;
     p->capture_stream = 0;
+    for (int i = 0; i < S2W_LANES - 1; ++i) {
+        p->lane_stream[i] = 0;
+        p->lane_join[i] = 0;
+    }
+    p->lane_fork = 0;
+    p->lanes_on = false;
     p->L = L;
     p->N = N;
     p->P = P;
@@ -1408,7 +1521,7 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
     p->ws_shell_elems = (size_t)P * (p->real ? L : 2 * L - 1) * L;
     p->ws_flm_elems = 2 * (((p->ws_shell_elems + 15) / 16) * 16);
     p->ws_F_elems = (size_t)P * maxF;
-    p->ws_bytes = (p->ws_flm_elems + 2 * (((p->ws_F_elems + 15) / 16) * 16)) * sizeof(cplx) + 256;
+    p->ws_bytes = (p->ws_flm_elems + (2 + 2 * (S2W_LANES - 1)) * (((p->ws_F_elems + 15) / 16) * 16)) * sizeof(cplx) + 256;
     S2W_PLAN_TRY(cudaDeviceSynchronize() == cudaSuccess ? S2W_OK : S2W_ECUDA);
     *out = p;
     return S2W_OK;
@@ -1419,6 +1532,11 @@ int s2w_plan_destroy(s2w_plan *p)
     if (!p) return S2W_OK;
     for (auto &g : p->graphs) cudaGraphExecDestroy(g.exec);
     if (p->capture_stream) cudaStreamDestroy(p->capture_stream);
+    for (int i = 0; i < S2W_LANES - 1; ++i) {
+        if (p->lane_stream[i]) cudaStreamDestroy(p->lane_stream[i]);
+        if (p->lane_join[i]) cudaEventDestroy(p->lane_join[i]);
+    }
+    if (p->lane_fork) cudaEventDestroy(p->lane_fork);
     p->pool.release();
     delete p;
     return S2W_OK;
@@ -1494,7 +1612,9 @@ static int run_transform(const s2w_plan *p, int dir, const void *in, void *out, 
     if (!p->capture_stream) S2W_CUDA_CHECK(cudaStreamCreateWithFlags(&p->capture_stream, cudaStreamNonBlocking));
     const unsigned long long n0 = g_launches;
     S2W_CUDA_CHECK(cudaStreamBeginCapture(p->capture_stream, cudaStreamCaptureModeThreadLocal));
+    p->lanes_on = true;
     const int rc = direct(p->capture_stream);
+    p->lanes_on = false;
     cudaGraph_t graph = 0;
     const cudaError_t ce = cudaStreamEndCapture(p->capture_stream, &graph);
     const unsigned long long nl = g_launches - n0;
