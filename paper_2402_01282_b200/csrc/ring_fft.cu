@@ -137,6 +137,120 @@ __global__ void __launch_bounds__(256, 3) ring_inv_kernel(const cplx *__restrict
 // Real: rows n >= 0 only: V_n(a) = sum_m F_mn e^{i m alpha_a} with F_{-m,n} = conj(F_{m,-n});
 //       W = sum_{n>=0} c_n Re(e^{i n gamma_g} V_n), c_0 = 1, c_n = 2.
 // ---------------------------------------------------------------------------------------------------------------
+// Few gamma samples (real: 2N-1 <= 9, complex: 2N-1 <= 5): no read-modify-write of the gamma planes.  The transforms
+// V_n(alpha) of all rows but the last are parked in the ring's own output planes (real: row i in planes 2i, 2i+1;
+// complex: row i in plane i), the pass of the last row reads them back -- each thread its own alpha samples, so
+// program order is all the ordering needed -- and writes every plane once.
+template <bool REAL, bool MULTI>
+__device__ __forceinline__ void so3_inv_few(const cplx *__restrict__ F, void *__restrict__ W, size_t sig_stride,
+                                            const So3Args &A, const FftTab &T, int rpb, cplx *buf0, const cplx *s_tw,
+                                            cplx *gph)
+{
+    constexpr int NG = REAL ? 9 : 5;  // most gamma samples
+    constexpr int NP = 4;             // most parked rows
+    const int n = T.n, L = T.L, M = T.M;
+    const int bstride = fft_padded_len(M);
+    const int tpr = MULTI ? blockDim.x / rpb : blockDim.x;
+    const int rl = MULTI ? threadIdx.x / tpr : 0, tl = MULTI ? threadIdx.x - rl * tpr : threadIdx.x;
+    cplx *buf = buf0 + (size_t)rl * bstride;
+    const int t = MULTI ? blockIdx.x * rpb + rl : blockIdx.x, b = blockIdx.y;
+    const bool has = MULTI ? t < L : true;
+    const int Md = REAL ? L : n;
+    const int ng = 2 * A.N - 1;
+    const size_t plane = (size_t)L * n;
+    const cplx *Fb = F + (size_t)b * A.nrows * L * Md;
+    int nproc = 0;
+    for (int q = 0; q < A.nn; ++q) {
+        if (REAL && A.n_val[q] < 0) continue;
+        for (int g = threadIdx.x; g < ng; g += blockDim.x) {
+            cplx ph = cis_2pi_frac(A.n_val[q] * g, ng);
+            if (REAL && A.n_val[q] != 0) ph = cscale(ph, 2.0);  // W = V_0 + 2 Re sum_{n>0} e^{i n gamma} V_n
+            gph[nproc * ng + g] = ph;
+        }
+        ++nproc;
+    }
+    int i = 0;
+    for (int q = 0; q < A.nn; ++q) {
+        const int nv = A.n_val[q];
+        if (REAL && nv < 0) continue;
+        const cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * Md;   // row of n
+        const cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * Md;  // row of -n
+        for (int k = tl; k < M; k += tpr) {
+            cplx v = cmake(0.0, 0.0);
+            if (k < n && has) {
+                if (REAL) {
+                    v = k < L ? Fp[k] : cconj(Fm[n - k]);
+                } else {
+                    int m = k < L ? k : k - n;
+                    v = Fp[m + L - 1];
+                }
+                v = cmulc(v, __ldg(&T.chirp[k]));
+            }
+            buf[S2W_PAD(k)] = v;
+        }
+        __syncthreads();
+        if (MULTI)
+            fft_convolve_b(buf0, T, s_tw, T.bhat_p, rpb, bstride);
+        else
+            fft_convolve(buf, T, s_tw, T.bhat_p);
+        for (int a = tl; a < (has ? n : 0); a += tpr) {
+            const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
+            if (REAL) {
+                double *Wr = (double *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+                if (i + 1 < nproc) {
+                    Wr[(size_t)(2 * i) * plane] = v.x;
+                    Wr[(size_t)(2 * i + 1) * plane] = v.y;
+                } else {
+                    double sc[2 * NP];
+#pragma unroll
+                    for (int k = 0; k < 2 * NP; ++k) sc[k] = k < 2 * i ? Wr[(size_t)k * plane] : 0.0;
+                    double out[NG];
+#pragma unroll
+                    for (int g = 0; g < NG; ++g) {
+                        const cplx ph = gph[i * ng + (g < ng ? g : 0)];
+                        out[g] = ph.x * v.x - ph.y * v.y;
+                    }
+#pragma unroll
+                    for (int j = 0; j < NP; ++j)
+                        if (j < i) {
+#pragma unroll
+                            for (int g = 0; g < NG; ++g) {
+                                const cplx ph = gph[j * ng + (g < ng ? g : 0)];
+                                out[g] += ph.x * sc[2 * j] - ph.y * sc[2 * j + 1];
+                            }
+                        }
+#pragma unroll
+                    for (int g = 0; g < NG; ++g)
+                        if (g < ng) Wr[(size_t)g * plane] = out[g];
+                }
+            } else {
+                cplx *Wc = (cplx *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+                if (i + 1 < nproc) {
+                    Wc[(size_t)i * plane] = v;
+                } else {
+                    cplx sc[NP];
+#pragma unroll
+                    for (int k = 0; k < NP; ++k) sc[k] = k < i ? Wc[(size_t)k * plane] : cmake(0.0, 0.0);
+                    cplx out[NG];
+#pragma unroll
+                    for (int g = 0; g < NG; ++g) out[g] = cmul(gph[i * ng + (g < ng ? g : 0)], v);
+#pragma unroll
+                    for (int j = 0; j < NP; ++j)
+                        if (j < i) {
+#pragma unroll
+                            for (int g = 0; g < NG; ++g) out[g] = cadd(out[g], cmul(gph[j * ng + (g < ng ? g : 0)], sc[j]));
+                        }
+#pragma unroll
+                    for (int g = 0; g < NG; ++g)
+                        if (g < ng) Wc[(size_t)g * plane] = out[g];
+                }
+            }
+        }
+        ++i;
+        __syncthreads();
+    }
+}
+
 // MULTI: rpb rings per block (small grids), tpr = blockDim / rpb threads per ring; otherwise one ring per block.
 template <bool REAL, bool MULTI>
 __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict__ F, void *__restrict__ W, size_t sig_stride,
@@ -156,6 +270,10 @@ __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict_
     const int ng = 2 * A.N - 1;
     const cplx *Fb = F + (size_t)b * A.nrows * L * Md;
     __shared__ cplx gph[2 * S2W_MAX_N];
+    if (ng <= (REAL ? 9 : 5)) {
+        so3_inv_few<REAL, MULTI>(F, W, sig_stride, A, T, rpb, buf0, s_tw, gph);
+        return;
+    }
     bool first = true;
     for (int q = 0; q < A.nn; ++q) {
         const int nv = A.n_val[q];
@@ -223,6 +341,123 @@ __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict_
 // The gamma sum is done first in pixel space, V_n(a) = (1/n_g) sum_g e^{-i n gamma_g} W(g,t,a), then one DFT per row.
 // Real: rows n >= 0; the row of -n follows from F_{m,-n} = conj(F_{-m,n}).
 // ---------------------------------------------------------------------------------------------------------------
+// Few gamma samples (real: 2N-1 <= 9, complex: 2N-1 <= 5): the gamma planes of a ring are read ONCE.  The gamma sums
+// of all rows, Y_n(alpha) = 1/(2N-1) sum_g e^{-i n gamma_g} W(alpha, gamma_g), are formed together; the first row goes
+// straight into the shared-memory buffer, the others are parked, chirp applied, in their own output rows (real:
+// F_{., n} and F_{., -n}, 2L >= 2L-1 slots, which is why a row n = 0 goes first; complex: the row's 2L-1 slots) and
+// fetched back -- each thread its own alpha samples -- when their convolution is due.
+template <bool REAL, bool MULTI>
+__device__ __forceinline__ void so3_fwd_few(const void *__restrict__ W, cplx *__restrict__ F, size_t sig_stride,
+                                            const So3Args &A, const FftTab &T, int rpb, cplx *buf0, const cplx *s_tw,
+                                            cplx *gph)
+{
+    constexpr int NG = REAL ? 9 : 5;
+    constexpr int NR = 5;  // most rows
+    const int n = T.n, L = T.L, M = T.M;
+    const int bstride = fft_padded_len(M);
+    const int tpr = MULTI ? blockDim.x / rpb : blockDim.x;
+    const int rl = MULTI ? threadIdx.x / tpr : 0, tl = MULTI ? threadIdx.x - rl * tpr : threadIdx.x;
+    cplx *buf = buf0 + (size_t)rl * bstride;
+    const int t = MULTI ? blockIdx.x * rpb + rl : blockIdx.x, b = blockIdx.y;
+    const bool has = MULTI ? t < L : true;
+    const int Md = REAL ? L : n;
+    const int ng = 2 * A.N - 1;
+    const size_t plane = (size_t)L * n;
+    const double inv_ng = 1.0 / (double)ng, inv_n = 1.0 / (double)n;
+    cplx *Fb = F + (size_t)b * A.nrows * L * Md;
+    __shared__ int s_nv[NR], s_rowp[NR], s_rowm[NR];
+    int nproc = 0;
+    for (int pass = 0; pass < 2; ++pass)  // a row n = 0 first
+        for (int q = 0; q < A.nn; ++q) {
+            const int nv = A.n_val[q];
+            if ((REAL && nv < 0) || (pass == 0) != (nv == 0)) continue;
+            for (int g = threadIdx.x; g < ng; g += blockDim.x) gph[nproc * ng + g] = cis_2pi_frac(-nv * g, ng);
+            if (threadIdx.x == 0) {
+                s_nv[nproc] = nv;
+                s_rowp[nproc] = A.n_row[q];
+                s_rowm[nproc] = A.n_rowm[q];
+            }
+            ++nproc;
+        }
+    __syncthreads();
+    // gather pass
+    for (int a = tl; a < M; a += tpr) {
+        if (a >= n || !has) {
+            buf[S2W_PAD(a)] = cmake(0.0, 0.0);
+            continue;
+        }
+        const cplx ch = __ldg(&T.chirp[a]);
+        double wr[NG];
+        cplx wc[REAL ? 1 : NG];
+        if (REAL) {
+            const double *Wr = (const double *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+#pragma unroll
+            for (int g = 0; g < NG; ++g) wr[g] = g < ng ? Wr[(size_t)g * plane] : 0.0;
+        } else {
+            const cplx *Wc = (const cplx *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+#pragma unroll
+            for (int g = 0; g < NG; ++g) wc[g] = g < ng ? Wc[(size_t)g * plane] : cmake(0.0, 0.0);
+        }
+#pragma unroll
+        for (int i = 0; i < NR; ++i)
+            if (i < nproc) {
+                cplx y = cmake(0.0, 0.0);
+#pragma unroll
+                for (int g = 0; g < NG; ++g) {
+                    const cplx ph = gph[i * ng + (g < ng ? g : 0)];
+                    if (REAL) {
+                        y.x = fma(ph.x, wr[g], y.x);
+                        y.y = fma(ph.y, wr[g], y.y);
+                    } else {
+                        y = cadd(y, cmul(ph, wc[g]));
+                    }
+                }
+                y = cmul(cscale(y, inv_ng), ch);
+                if (i == 0)
+                    buf[S2W_PAD(a)] = y;
+                else if (REAL)
+                    Fb[((size_t)(a < L ? s_rowp[i] : s_rowm[i]) * L + t) * Md + (a < L ? a : a - L)] = y;
+                else
+                    Fb[((size_t)s_rowp[i] * L + t) * Md + a] = y;
+            }
+    }
+    __syncthreads();
+    for (int i = 0; i < nproc; ++i) {
+        cplx *Fp = Fb + ((size_t)s_rowp[i] * L + t) * Md;
+        cplx *Fm = Fb + ((size_t)s_rowm[i] * L + t) * Md;
+        if (i > 0) {
+            for (int a = tl; a < M; a += tpr) {
+                cplx v = cmake(0.0, 0.0);
+                if (a < n && has) v = REAL ? (a < L ? Fp[a] : Fm[a - L]) : Fp[a];
+                buf[S2W_PAD(a)] = v;
+            }
+            __syncthreads();
+        }
+        if (MULTI)
+            fft_convolve_b(buf0, T, s_tw, T.bhat_m, rpb, bstride);
+        else
+            fft_convolve(buf, T, s_tw, T.bhat_m);
+        if (REAL) {
+            const int nv = s_nv[i];
+            for (int m = tl; m < (has ? L : 0); m += tpr) {
+                Fp[m] = cscale(cmul(buf[S2W_PAD(m)], __ldg(&T.chirp[m])), inv_n);
+                if (nv != 0) {
+                    int k = m == 0 ? 0 : n - m;
+                    Fm[m] = cscale(cconj(cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k]))), inv_n);
+                }
+            }
+        } else {
+            // the row is also this ring's parking slot of the NEXT rows' values only; its own were consumed above
+            for (int mi = tl; mi < (has ? n : 0); mi += tpr) {
+                int m = mi - (L - 1);
+                int k = m < 0 ? m + n : m;
+                Fp[mi] = cscale(cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k])), inv_n);
+            }
+        }
+        __syncthreads();
+    }
+}
+
 template <bool REAL, bool MULTI>
 __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict__ W, cplx *__restrict__ F, size_t sig_stride,
                                                      So3Args A, FftTab T, int rpb)
@@ -242,6 +477,10 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
     const double inv_ng = 1.0 / (double)ng, inv_n = 1.0 / (double)n;
     cplx *Fb = F + (size_t)b * A.nrows * L * Md;
     __shared__ cplx gph[2 * S2W_MAX_N];
+    if (ng <= (REAL ? 9 : 5)) {
+        so3_fwd_few<REAL, MULTI>(W, F, sig_stride, A, T, rpb, buf0, s_tw, gph);
+        return;
+    }
     for (int q = 0; q < A.nn; ++q) {
         const int nv = A.n_val[q];
         if (REAL && nv < 0) continue;
