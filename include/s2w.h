@@ -95,6 +95,16 @@ int s2w_plan_forward(const s2w_plan *plan, const void *in_dev, void *out_dev, vo
 /* Synthesis, Alg. 1 / Alg. 2: in = coefficients, out = signal(s). */
 int s2w_plan_inverse(const s2w_plan *plan, const void *in_dev, void *out_dev, void *work_dev, void *stream);
 
+/* Adjoint transforms (the "differentiable" half of the paper, P:9: the maps are linear, so a
+ * vector-Jacobian product is the adjoint map applied to the cotangent).  With <u, v> = sum conj(u_i) v_i over the stored
+ * samples (pixels / coefficient samples, no quadrature weights):
+ *   <A f, y> = <f, A^H y>    s2w_plan_forward_adjoint: in = coefficient-shaped y, out = signal-shaped A^H y;
+ *   <S w, g> = <w, S^H g>    s2w_plan_inverse_adjoint: in = signal-shaped g,      out = coefficient-shaped S^H g,
+ * A = s2w_plan_forward, S = s2w_plan_inverse.  Same buffers, layouts, workspace and stream semantics as those.
+ * Complex-signal sphere plans only: S2W_EUNSUPPORTED for S2W_REAL and ball plans. */
+int s2w_plan_forward_adjoint(const s2w_plan *plan, const void *in_dev, void *out_dev, void *work_dev, void *stream);
+int s2w_plan_inverse_adjoint(const s2w_plan *plan, const void *in_dev, void *out_dev, void *work_dev, void *stream);
+
 /* Harmonic-space taps used by the parity tests: forward spherical harmonic transform of the plan's signal(s)
  * (steps a1-a3 of DESIGN.md) writing flm [batch][L][2L-1] complex128 at [l][m+L-1] (ball: [P][L][2L-1], after the
  * radial transform: f_{lmp}), and its inverse. */

@@ -36,6 +36,8 @@ SIGNATURES = {
     "s2w_plan_workspace_bytes": (_c_sz, [_c_vp]),
     "s2w_plan_forward": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_vp]),
     "s2w_plan_inverse": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_vp]),
+    "s2w_plan_forward_adjoint": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_vp]),
+    "s2w_plan_inverse_adjoint": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_vp]),
     "s2w_plan_harmonic_forward": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_vp]),
     "s2w_plan_harmonic_inverse": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_vp]),
     "s2wav_forward": (_c_int, [_c_vp, _c_vp, _c_int, _c_int, _c_dbl, _c_int, _c_int, _c_int, _c_int, _c_vp]),
@@ -215,6 +217,26 @@ class Plan:
         _check(lib().s2w_plan_inverse(self._h, w.data_ptr(), out.data_ptr(), self._workspace(w.device).data_ptr(),
                                       _stream_ptr()))
         return out if shape is None else out.view(shape)
+
+    def forward_adjoint(self, y, out=None):
+        """Adjoint of the analysis: coefficient-shaped y -> signal-shaped A^H y (s2w_plan_forward_adjoint)."""
+        torch = _torch()
+        self._check_in(y, self.coeff_elems)
+        if out is None:
+            out = torch.empty((self.batch, self.signal_elems), dtype=self.dtype, device=y.device)
+        _check(lib().s2w_plan_forward_adjoint(self._h, y.data_ptr(), out.data_ptr(),
+                                              self._workspace(y.device).data_ptr(), _stream_ptr()))
+        return out
+
+    def inverse_adjoint(self, g, out=None):
+        """Adjoint of the synthesis: signal-shaped g -> coefficient-shaped S^H g (s2w_plan_inverse_adjoint)."""
+        torch = _torch()
+        self._check_in(g, self.signal_elems)
+        if out is None:
+            out = torch.empty((self.batch, self.coeff_elems), dtype=self.dtype, device=g.device)
+        _check(lib().s2w_plan_inverse_adjoint(self._h, g.data_ptr(), out.data_ptr(),
+                                              self._workspace(g.device).data_ptr(), _stream_ptr()))
+        return out
 
     def harmonic_forward(self, f, flm_elems):
         torch = _torch()

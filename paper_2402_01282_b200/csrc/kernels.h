@@ -80,6 +80,7 @@ int launch_so3_fwd(bool real, const void *W, size_t sig_stride, cplx *F, const S
 // a2: reads F[b][row][t][mi], writes the reweighted columns TRANSPOSED, Ft[b][row][mi][t] (what the forward Wigner
 // contraction reads: ring data of one m contiguous)
 int launch_reweight(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const FftTab &T, cudaStream_t st);
+int launch_transpose(const cplx *src, cplx *dst, int R, int C, int nb, cudaStream_t st);
 int launch_reweight_th(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st);   // L >= 8, L <= 2048
 int launch_fft_forward(cplx *data, const FftTab &T, cudaStream_t st);   // plan-time, in place, digit-reversed out
 

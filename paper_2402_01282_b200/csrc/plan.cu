@@ -115,6 +115,11 @@ struct Stage {  // one Wigner contraction launch: rows, filters
     int n_val[S2W_MAX_ROWS], n_tab[S2W_MAX_ROWS], n_row[S2W_MAX_ROWS], n_rowm[S2W_MAX_ROWS], n_filtm[S2W_MAX_ROWS];
     cplx *filt_ana;  // [nn][Lg]  harmonic -> rings
     cplx *filt_syn;  // [nn][Lg]  rings -> harmonic
+    // adjoint transforms: c conj(filt_ana) for the rings -> harmonic contraction that is the adjoint
+    // of this stage's harmonic -> rings one, conj(filt_syn) / c for the other direction; c = number of (alpha, gamma)
+    // or phi samples per ring, the factor between the unnormalised inverse DFT and the adjoint of the normalised one
+    cplx *filt_ana_adj;
+    cplx *filt_syn_adj;
 };
 
 struct Scale {
@@ -674,11 +679,16 @@ int plan_common(s2w_plan *p)
     return S2W_OK;
 }
 
-int make_stage_filters(s2w_plan *p, Stage &st, const std::vector<cplx> &ana, const std::vector<cplx> &syn)
+int make_stage_filters(s2w_plan *p, Stage &st, const std::vector<cplx> &ana, const std::vector<cplx> &syn, double c)
 {
     int rc;
     if ((rc = p->pool.upload(&st.filt_ana, ana))) return rc;
     if ((rc = p->pool.upload(&st.filt_syn, syn))) return rc;
+    std::vector<cplx> aa(ana.size()), sa(syn.size());
+    for (size_t i = 0; i < ana.size(); ++i) aa[i] = cmake(c * ana[i].x, -c * ana[i].y);
+    for (size_t i = 0; i < syn.size(); ++i) sa[i] = cmake(syn[i].x / c, -syn[i].y / c);
+    if ((rc = p->pool.upload(&st.filt_ana_adj, aa))) return rc;
+    if ((rc = p->pool.upload(&st.filt_syn_adj, sa))) return rc;
     return S2W_OK;
 }
 
@@ -698,7 +708,7 @@ int make_n0_stage(s2w_plan *p, Stage &st, int Lg, const std::vector<double> &a, 
         fa[l] = cmake(a[l], 0.0);
         fs[l] = cmake(s[l], 0.0);
     }
-    return make_stage_filters(p, st, fa, fs);
+    return make_stage_filters(p, st, fa, fs, 2.0 * Lg - 1.0);
 }
 
 // wavelet stage of angular scale j at band-limit sc.Lj: rows n of script-N inside the band-limit, filters
@@ -739,7 +749,7 @@ int make_scale_stage(s2w_plan *p, Scale &sc, const double *kj, const std::vector
             fa[(size_t)q * sc.Lj + l] = cmake(re, -im);
             fs[(size_t)q * sc.Lj + l] = cmake(re * syn_norm, im * syn_norm);
         }
-    return make_stage_filters(p, st, fa, fs);
+    return make_stage_filters(p, st, fa, fs, (2.0 * sc.Lj - 1.0) * nn);
 }
 
 }  // namespace
@@ -1075,6 +1085,96 @@ static int sphere_inverse(const s2w_plan *p, const void *in, void *out, void *wo
     }
     if ((rc = lanes_join(p, ln))) return rc;
     if ((rc = sht_inverse_dev(p, p->sht, out, p->signal_elems, B, w, s))) return rc;
+    S2W_CUDA_CHECK(cudaPeekAtLastError());
+    return S2W_OK;
+}
+
+// ---- adjoint transforms (sphere, complex signals) ------------------------------------
+// With <u, v> = sum conj(u) v over the stored samples, the adjoint of a chain is the reversed chain of adjoints:
+//   (inverse DFT E)^H = n x (normalised forward DFT),   (normalised forward DFT E^H / n)^H = E / n,
+//   (harmonic -> rings contraction D diag(a))^H = diag(conj a) D^T  = the rings -> harmonic contraction, no quadrature,
+//   (rings -> harmonic contraction diag(s) D^T R)^H = R D diag(conj s): the reweighting operator R = E_x^T K E_x
+//   (extension, the real symmetric kernel K of section 6.3, fold) is its own adjoint.
+// The same kernels in the other order; the constants live in filt_ana_adj / filt_syn_adj, and transpose_kernel stands
+// in where the reweighting kernel's transposed output is missing (or has to be undone).
+
+// w.F [B][nrows][t][m]  ->  flmT += c conj(a_l) sum_t d^l_{mn}(theta_t) F
+static int adj_rings_to_harmonic(const s2w_plan *p, const Stage &st, int B, const Work &w, cudaStream_t s)
+{
+    const int Md = 2 * st.Lg - 1;
+    int rc;
+    if ((rc = launch_transpose(w.F, w.Ft, st.Lg, Md, B * st.nrows, s))) return rc;
+    WigArgs A;
+    fill_wig_args(p, st, true, B, w.flmT, w.Ft, A);
+    A.filt = st.filt_ana_adj;
+    return launch_wigner_forward(A, s);
+}
+
+// flmT  ->  w.F [B][nrows][t][m] = R sum_l d^l_{mn}(theta_t) conj(s_l) / c flm
+static int adj_harmonic_to_rings(const s2w_plan *p, const Stage &st, int B, const Work &w, cudaStream_t s)
+{
+    const GridTab &g = p->grids[st.grid];
+    const int Md = 2 * st.Lg - 1;
+    int rc;
+    WigArgs A;
+    fill_wig_args(p, st, false, B, w.flmT, w.F, A);
+    A.filt = st.filt_syn_adj;
+    if ((rc = launch_wigner_inverse(A, s))) return rc;
+    RwArgs R;
+    fill_rw_args(p, st, R);
+    if ((rc = g.rw.L ? launch_reweight_th(w.F, w.Ft, R, B, g.rw, s) : launch_reweight(w.F, w.Ft, R, B, g.fft, s))) return rc;
+    return launch_transpose(w.Ft, w.F, Md, st.Lg, B * st.nrows, s);
+}
+
+// adjoint of the analysis: coefficients -> signal
+static int sphere_forward_adjoint(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s)
+{
+    const Work w = carve(p, work);
+    const int B = p->batch;
+    const cplx *y = (const cplx *)in;
+    int rc;
+    S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * (2 * p->L - 1) * p->L * sizeof(cplx), s));
+    if ((rc = launch_ring_fwd(false, y + p->scaling_offset, w.F, B, p->Ls, p->coeff_elems, p->grids[p->scaling.grid].fft, s)))
+        return rc;
+    if ((rc = adj_rings_to_harmonic(p, p->scaling, B, w, s))) return rc;
+    for (const Scale &sc : p->scales) {
+        if (sc.st.nn == 0) continue;
+        So3Args S;
+        fill_so3_args(p, sc.st, S);
+        if ((rc = launch_so3_fwd(false, y + sc.offset, p->coeff_elems, w.F, S, B, p->grids[sc.st.grid].fft, s))) return rc;
+        if ((rc = adj_rings_to_harmonic(p, sc.st, B, w, s))) return rc;
+    }
+    if ((rc = adj_harmonic_to_rings(p, p->sht, B, w, s))) return rc;
+    if ((rc = launch_ring_inv(false, w.F, out, B, p->L, p->signal_elems, p->grids[p->sht.grid].fft, s))) return rc;
+    S2W_CUDA_CHECK(cudaPeekAtLastError());
+    return S2W_OK;
+}
+
+// adjoint of the synthesis: signal -> coefficients
+static int sphere_inverse_adjoint(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s)
+{
+    const Work w = carve(p, work);
+    const int B = p->batch;
+    cplx *y = (cplx *)out;
+    int rc;
+    S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * (2 * p->L - 1) * p->L * sizeof(cplx), s));
+    if ((rc = launch_ring_fwd(false, in, w.F, B, p->L, p->signal_elems, p->grids[p->sht.grid].fft, s))) return rc;
+    if ((rc = adj_rings_to_harmonic(p, p->sht, B, w, s))) return rc;
+    for (const Scale &sc : p->scales) {
+        if (sc.st.nn == 0) {
+            for (int b = 0; b < B; ++b)
+                S2W_CUDA_CHECK(cudaMemsetAsync(y + (size_t)b * p->coeff_elems + sc.offset, 0,
+                                               (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1) * sizeof(cplx), s));
+            continue;
+        }
+        if ((rc = adj_harmonic_to_rings(p, sc.st, B, w, s))) return rc;
+        So3Args S;
+        fill_so3_args(p, sc.st, S);
+        if ((rc = launch_so3_inv(false, w.F, y + sc.offset, p->coeff_elems, S, B, p->grids[sc.st.grid].fft, s))) return rc;
+    }
+    if ((rc = adj_harmonic_to_rings(p, p->scaling, B, w, s))) return rc;
+    if ((rc = launch_ring_inv(false, w.F, y + p->scaling_offset, B, p->Ls, p->coeff_elems, p->grids[p->scaling.grid].fft, s)))
+        return rc;
     S2W_CUDA_CHECK(cudaPeekAtLastError());
     return S2W_OK;
 }
@@ -1597,6 +1697,8 @@ static void *align256(void *p) { return (void *)(((uintptr_t)p + 255) & ~(uintpt
 static int run_transform(const s2w_plan *p, int dir, const void *in, void *out, void *work, cudaStream_t s)
 {
     auto direct = [&](cudaStream_t st) {
+        if (dir == 2) return sphere_forward_adjoint(p, in, out, work, st);
+        if (dir == 3) return sphere_inverse_adjoint(p, in, out, work, st);
         if (p->kind == 1) return dir == 0 ? ball_forward(p, in, out, work, st) : ball_inverse(p, in, out, work, st);
         return dir == 0 ? sphere_forward(p, in, out, work, st) : sphere_inverse(p, in, out, work, st);
     };
@@ -1663,6 +1765,33 @@ int s2w_plan_inverse(const s2w_plan *p, const void *in, void *out, void *work, v
         return S2W_EINVAL;
     }
     return run_transform(p, 1, in, out, align256(work), (cudaStream_t)stream);
+}
+
+static int adjoint_supported(const s2w_plan *p, const void *in, const void *out, const void *work)
+{
+    if (!p || !in || !out || !work) {
+        set_error("null pointer");
+        return S2W_EINVAL;
+    }
+    if (p->kind != 0 || p->real) {
+        set_error("adjoint transforms: complex-signal sphere plans only");
+        return S2W_EUNSUPPORTED;
+    }
+    return S2W_OK;
+}
+
+int s2w_plan_forward_adjoint(const s2w_plan *p, const void *in, void *out, void *work, void *stream)
+{
+    int rc = adjoint_supported(p, in, out, work);
+    if (rc) return rc;
+    return run_transform(p, 2, in, out, align256(work), (cudaStream_t)stream);
+}
+
+int s2w_plan_inverse_adjoint(const s2w_plan *p, const void *in, void *out, void *work, void *stream)
+{
+    int rc = adjoint_supported(p, in, out, work);
+    if (rc) return rc;
+    return run_transform(p, 3, in, out, align256(work), (cudaStream_t)stream);
 }
 
 int s2w_plan_harmonic_forward(const s2w_plan *p, const void *f, void *flm, void *work, void *stream)

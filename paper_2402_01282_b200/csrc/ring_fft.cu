@@ -1302,6 +1302,26 @@ __global__ void __launch_bounds__(256) kernel_spectrum_kernel(cplx *khat, int ki
     for (int e = threadIdx.x; e < M; e += blockDim.x) khat[e] = buf[S2W_PAD(e)];
 }
 
+// dst[b][c][r] = src[b][r][c] for nb matrices of R x C complex values: the adjoint transforms move
+// between the ring-major layout F[n][t][m] of the FFT kernels and the column-major layout Ft[n][m][t] of the forward
+// contraction without the reweighting kernel that normally does it.  32 x 32 tiles through padded shared memory.
+__global__ void __launch_bounds__(256) transpose_kernel(const cplx *__restrict__ src, cplx *__restrict__ dst, int R, int C)
+{
+    __shared__ cplx tile[32][33];
+    const size_t base = (size_t)blockIdx.z * R * C;
+    const int c0 = blockIdx.x * 32, r0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int k = ty; k < 32; k += 8) {
+        const int r = r0 + k, c = c0 + tx;
+        if (r < R && c < C) tile[k][tx] = src[base + (size_t)r * C + c];
+    }
+    __syncthreads();
+    for (int k = ty; k < 32; k += 8) {
+        const int c = c0 + k, r = r0 + tx;
+        if (r < R && c < C) dst[base + (size_t)c * R + r] = tile[tx][k];
+    }
+}
+
 size_t fft_smem_bytes(const FftTab &T) { return (size_t)fft_padded_len(T.M) * sizeof(cplx); }
 
 // Kernels that may need more than 48 KB of dynamic shared memory are raised to the device's opt-in limit, never to
@@ -1468,6 +1488,17 @@ static int seqs_per_block(int fit, long long total, int cap)
     int s = fit < 1 ? 1 : (fit > cap ? cap : fit);
     while (s > 1 && total / s < 900) s >>= 1;
     return s;
+}
+
+int launch_transpose(const cplx *src, cplx *dst, int R, int C, int nb, cudaStream_t st)
+{
+    if (R <= 0 || C <= 0 || nb <= 0) return S2W_OK;
+    for (int b0 = 0; b0 < nb; b0 += 65535) {  // gridDim.z limit
+        const int nz = nb - b0 < 65535 ? nb - b0 : 65535;
+        dim3 grid((C + 31) / 32, (R + 31) / 32, nz);
+        S2W_LAUNCH(transpose_kernel, grid, 256, 0, st, src + (size_t)b0 * R * C, dst + (size_t)b0 * R * C, R, C);
+    }
+    return S2W_OK;
 }
 
 int launch_reweight_th(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st)
