@@ -1,0 +1,109 @@
+"""GPU parity tests of the adjoint transforms: s2w_plan_forward_adjoint / s2w_plan_inverse_adjoint
+through the C ABI against oracle/adjoint.py (the conjugate transpose of the oracle's own analysis / synthesis matrix)
+element by element on the same seeded inputs, and the defining identity <A x, y> = <x, A^H y> at sizes the oracle's
+matrix cannot reach.  Tolerance as for the forward transforms: 1e-11 relative max per block."""
+import numpy as np
+import pytest
+
+from oracle import adjoint as ADJ
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+def _api():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2402_01282_b200 import api
+    return torch, api
+
+
+def _relmax(a, b):
+    den = np.abs(b).max()
+    num = np.abs(a - b).max()
+    return num if den == 0 else num / den
+
+
+def _rand_c(rng, shape):
+    return rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+
+
+def _pack_for_plan(plan, Y_phi, Y_psi):
+    packed = np.zeros((1, plan.coeff_elems), dtype=np.complex128)
+    nr, ng, nt, npx, off = plan.scale_shape(-1)
+    packed[0, off:off + nt * npx] = np.asarray(Y_phi, dtype=np.complex128).ravel()
+    for j, a in Y_psi.items():
+        nr, ng, nt, npx, off = plan.scale_shape(j)
+        packed[0, off:off + ng * nt * npx] = np.asarray(a, dtype=np.complex128).ravel()
+    return packed
+
+
+CASES = [(8, 2, 2.0, 0, True), (6, 3, 2.0, 1, True), (7, 1, 3.0, 0, False), (10, 4, 2.0, 0, True)]
+
+
+@pytest.mark.parametrize("L,N,lam,J0,mr", CASES)
+def test_adjoints_match_oracle(L, N, lam, J0, mr):
+    torch, api = _api()
+    rng = np.random.default_rng(700 + L)
+    plan = api.s2wav_plan_create(L, N, lam, J0, mr, False, 1)
+    # A^H
+    Y_phi, Y_psi = None, {}
+    for key, shp in ADJ.shapes(L, N, lam, J0, mr):
+        a = _rand_c(rng, shp)
+        if key < 0:
+            Y_phi = a
+        else:
+            Y_psi[key] = a
+    ref = ADJ.analysis_adjoint(Y_phi, Y_psi, L, N, lam, J0, mr, "f80").astype(np.complex128)
+    got = plan.forward_adjoint(torch.from_numpy(_pack_for_plan(plan, Y_phi, Y_psi)).cuda()).cpu().numpy()
+    assert _relmax(got.reshape(L, 2 * L - 1), ref) < TOL
+    # S^H
+    g = _rand_c(rng, (L, 2 * L - 1))
+    Z_phi, Z_psi = ADJ.synthesis_adjoint(g, L, N, lam, J0, mr, "f80")
+    z = plan.inverse_adjoint(torch.from_numpy(np.ascontiguousarray(g.reshape(1, -1))).cuda())
+    scal, scales = plan.split(z)
+    assert _relmax(scal[0].cpu().numpy(), Z_phi.astype(np.complex128)) < TOL
+    for j, refj in Z_psi.items():
+        gotj = scales[(j, 0)][0].cpu().numpy()
+        assert gotj.shape == refj.shape
+        if np.abs(refj).max() == 0:
+            assert np.abs(gotj).max() == 0
+        else:
+            assert _relmax(gotj, refj.astype(np.complex128)) < TOL, j
+    plan.close()
+
+
+@pytest.mark.parametrize("L,N,lam,J0,mr,batch", [(64, 3, 2.0, 1, True, 2), (300, 3, 2.0, 2, True, 1), (130, 5, 2.0, 3, False, 1),
+                                                 (1024, 2, 2.0, 8, True, 1)])
+def test_inner_product_identities_at_larger_sizes(L, N, lam, J0, mr, batch):
+    """<A x, y> = <x, A^H y> and <S y, x> = <y, S^H x> for random (not band-limited) x and y: several ring groups per
+    warp, ragged groups, the Toeplitz/Hankel reweighting and the ring-by-ring kernels of the large grids."""
+    torch, api = _api()
+    gen = torch.Generator(device="cuda").manual_seed(L + N)
+    plan = api.s2wav_plan_create(L, N, lam, J0, mr, False, batch)
+    x = torch.randn(batch, plan.signal_elems, dtype=torch.complex128, device="cuda", generator=gen)
+    y = torch.randn(batch, plan.coeff_elems, dtype=torch.complex128, device="cuda", generator=gen)
+    Ax, Ahy = plan.forward(x), plan.forward_adjoint(y)
+    lhs, rhs = torch.vdot(Ax.flatten(), y.flatten()), torch.vdot(x.flatten(), Ahy.flatten())
+    assert abs(lhs - rhs) < 1e-12 * Ax.norm() * y.norm()
+    Sy, Shx = plan.inverse(y), plan.inverse_adjoint(x)
+    lhs, rhs = torch.vdot(Sy.flatten(), x.flatten()), torch.vdot(y.flatten(), Shx.flatten())
+    assert abs(lhs - rhs) < 1e-12 * Sy.norm() * x.norm()
+    # a second call replays the captured graph (the harmonic sums accumulate by atomics: equal up to rounding order)
+    assert float((plan.inverse_adjoint(x) - Shx).abs().max()) < 1e-13 * float(Shx.abs().max())
+    plan.close()
+
+
+def test_adjoint_is_refused_where_it_is_not_built():
+    torch, api = _api()
+    pr = api.s2wav_plan_create(8, 2, 2.0, 0, True, True, 1)
+    w = torch.zeros(1, pr.coeff_elems, dtype=torch.float64, device="cuda")
+    with pytest.raises(api.S2WError, match="S2W_EUNSUPPORTED"):
+        pr.forward_adjoint(w)
+    pr.close()
+    pb = api.s2ball_plan_create(8, 4, 2, 2.0, 2.0, 0, 1.0)
+    w = torch.zeros(1, pb.coeff_elems, dtype=torch.complex128, device="cuda")
+    with pytest.raises(api.S2WError, match="S2W_EUNSUPPORTED"):
+        pb.forward_adjoint(w)
+    pb.close()
