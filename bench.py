@@ -43,6 +43,9 @@ def parse_args():
     ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--precompute", action="store_true",
                     help="sphere workloads: the precomputed-kernel variant (S2W_PRECOMPUTE, step a9)")
+    ap.add_argument("--adjoint", action="store_true",
+                    help="sphere workloads: time the adjoint pair S^H (signal -> coefficients) + A^H (coefficients -> "
+                         "signal) on a complex-signal plan of the same shape (SURVEY 8(f)-1); no e2e / cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -251,9 +254,10 @@ def run_reference(args, cfg):
 
 
 def workload_config(cfg, args):
-    return {"workload": "%s: sphere L=%d N=%d lambda=%g J0=%d multires=%s %s fp64 batch=%d, forward+inverse"
+    return {"workload": "%s: sphere L=%d N=%d lambda=%g J0=%d multires=%s %s fp64 batch=%d, %s"
                         % (cfg["name"], cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"],
-                           "real" if cfg["real"] else "complex", cfg["batch"]),
+                           "real" if cfg["real"] else "complex", cfg["batch"],
+                           "adjoint pair S^H + A^H" if getattr(args, "adjoint", False) else "forward+inverse"),
             "L": cfg["L"], "N": cfg["N"], "lambda": cfg["lam"], "J0": cfg["J0"], "multiresolution": cfg["multires"],
             "batch_per_gpu": cfg["batch"],
             "mode": "precomputed Wigner-d table (DMMA)" if getattr(args, "precompute", False) else "on-the-fly Wigner recursion",
@@ -308,8 +312,14 @@ def run_ours(args, cfg):
             dist.barrier()
         torch.cuda.synchronize()
 
+    adj = bool(getattr(args, "adjoint", False))
+    if adj:  # the adjoints are built for complex-signal plans: the same signals, stored as complex
+        cfg = dict(cfg, real=False)
+        args.no_e2e = args.no_cpu_baseline = True
     L, N, lam, J0, mr, real, B = cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"], cfg["real"], cfg["batch"]
     f = make_signals(cfg, api, torch, device, seed_offset=replica_seed_offset(rank))     # independent signals per replica
+    if adj and not f.is_complex():
+        f = f.to(torch.complex128)
     plan = api.s2wav_plan_create(L, N, lam, J0, mr, real, B, local,
                                  flags=api.S2W_PRECOMPUTE if args.precompute else 0)
     cfg["coeff_gb"] = plan.coeff_elems * B * (8 if real else 16) / 1e9
@@ -317,13 +327,23 @@ def run_ours(args, cfg):
     back = torch.empty((B, plan.signal_elems), dtype=plan.dtype, device=device)
 
     def step():
-        plan.forward(f, out=w)
-        plan.inverse(w, out=back)
+        if adj:
+            plan.inverse_adjoint(f, out=w)
+            plan.forward_adjoint(w, out=back)
+        else:
+            plan.forward(f, out=w)
+            plan.inverse(w, out=back)
 
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
-    rt_err = float((back.view_as(f) - f).abs().max() / f.abs().max())
+    if adj:  # A^H S^H is not the identity; the check is the defining identity <A f, y> = <f, A^H y> with y = S^H f
+        Af = plan.forward(f)
+        rt_err = float((torch.vdot(Af.flatten(), w.flatten()) - torch.vdot(f.flatten(), back.flatten())).abs()
+                       / (Af.norm() * w.norm()))
+        del Af
+    else:
+        rt_err = float((back.view_as(f) - f).abs().max() / f.abs().max())
 
     # ---- device-resident timing: exactly K steps, CUDA events on the launching (current) stream ----
     sampler = ClockSampler(local)
@@ -418,7 +438,7 @@ def run_ours(args, cfg):
         "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, args),
         "clocks": clocks, "gpu_launches": int(launches),
-        "roundtrip_rel_err": rt_err,
+        ("adjoint_identity_rel_err" if adj else "roundtrip_rel_err"): rt_err,
         "roofline": roofline,
         "kernel_ms_per_step": {k: round(v[0] / ksteps, 4) for k, v in classes.items()},
         "kernel_share": {k: round(v[0] / total_kms, 4) for k, v in classes.items()} if total_kms else None,

@@ -1134,16 +1134,26 @@ static int sphere_forward_adjoint(const s2w_plan *p, const void *in, void *out, 
     const cplx *y = (const cplx *)in;
     int rc;
     S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * (2 * p->L - 1) * p->L * sizeof(cplx), s));
-    if ((rc = launch_ring_fwd(false, y + p->scaling_offset, w.F, B, p->Ls, p->coeff_elems, p->grids[p->scaling.grid].fft, s)))
-        return rc;
-    if ((rc = adj_rings_to_harmonic(p, p->scaling, B, w, s))) return rc;
-    for (const Scale &sc : p->scales) {
+    Lanes ln;  // every block accumulates into flmT by atomics: the blocks are dealt to the lanes, largest first
+    if ((rc = lanes_fork(p, w, w.Ft2 + ((p->ws_F_elems + 15) / 16) * 16, s, true, &ln))) return rc;
+    for (size_t k = p->scales.size(); k-- > 0;) {
+        const Scale &sc = p->scales[k];
         if (sc.st.nn == 0) continue;
+        const int l = ln.pick(scale_cost(sc));
         So3Args S;
         fill_so3_args(p, sc.st, S);
-        if ((rc = launch_so3_fwd(false, y + sc.offset, p->coeff_elems, w.F, S, B, p->grids[sc.st.grid].fft, s))) return rc;
-        if ((rc = adj_rings_to_harmonic(p, sc.st, B, w, s))) return rc;
+        if ((rc = launch_so3_fwd(false, y + sc.offset, p->coeff_elems, ln.w[l].F, S, B, p->grids[sc.st.grid].fft, ln.s[l])))
+            return rc;
+        if ((rc = adj_rings_to_harmonic(p, sc.st, B, ln.w[l], ln.s[l]))) return rc;
     }
+    {
+        const int l = ln.pick(0.0);
+        if ((rc = launch_ring_fwd(false, y + p->scaling_offset, ln.w[l].F, B, p->Ls, p->coeff_elems,
+                                  p->grids[p->scaling.grid].fft, ln.s[l])))
+            return rc;
+        if ((rc = adj_rings_to_harmonic(p, p->scaling, B, ln.w[l], ln.s[l]))) return rc;
+    }
+    if ((rc = lanes_join(p, ln))) return rc;
     if ((rc = adj_harmonic_to_rings(p, p->sht, B, w, s))) return rc;
     if ((rc = launch_ring_inv(false, w.F, out, B, p->L, p->signal_elems, p->grids[p->sht.grid].fft, s))) return rc;
     S2W_CUDA_CHECK(cudaPeekAtLastError());
@@ -1160,21 +1170,31 @@ static int sphere_inverse_adjoint(const s2w_plan *p, const void *in, void *out, 
     S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * (2 * p->L - 1) * p->L * sizeof(cplx), s));
     if ((rc = launch_ring_fwd(false, in, w.F, B, p->L, p->signal_elems, p->grids[p->sht.grid].fft, s))) return rc;
     if ((rc = adj_rings_to_harmonic(p, p->sht, B, w, s))) return rc;
-    for (const Scale &sc : p->scales) {
+    Lanes ln;  // every block reads the same flmT
+    if ((rc = lanes_fork(p, w, w.Ft2 + ((p->ws_F_elems + 15) / 16) * 16, s, true, &ln))) return rc;
+    for (size_t k = p->scales.size(); k-- > 0;) {
+        const Scale &sc = p->scales[k];
         if (sc.st.nn == 0) {
             for (int b = 0; b < B; ++b)
                 S2W_CUDA_CHECK(cudaMemsetAsync(y + (size_t)b * p->coeff_elems + sc.offset, 0,
                                                (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1) * sizeof(cplx), s));
             continue;
         }
-        if ((rc = adj_harmonic_to_rings(p, sc.st, B, w, s))) return rc;
+        const int l = ln.pick(scale_cost(sc));
+        if ((rc = adj_harmonic_to_rings(p, sc.st, B, ln.w[l], ln.s[l]))) return rc;
         So3Args S;
         fill_so3_args(p, sc.st, S);
-        if ((rc = launch_so3_inv(false, w.F, y + sc.offset, p->coeff_elems, S, B, p->grids[sc.st.grid].fft, s))) return rc;
+        if ((rc = launch_so3_inv(false, ln.w[l].F, y + sc.offset, p->coeff_elems, S, B, p->grids[sc.st.grid].fft, ln.s[l])))
+            return rc;
     }
-    if ((rc = adj_harmonic_to_rings(p, p->scaling, B, w, s))) return rc;
-    if ((rc = launch_ring_inv(false, w.F, y + p->scaling_offset, B, p->Ls, p->coeff_elems, p->grids[p->scaling.grid].fft, s)))
-        return rc;
+    {
+        const int l = ln.pick(0.0);
+        if ((rc = adj_harmonic_to_rings(p, p->scaling, B, ln.w[l], ln.s[l]))) return rc;
+        if ((rc = launch_ring_inv(false, ln.w[l].F, y + p->scaling_offset, B, p->Ls, p->coeff_elems,
+                                  p->grids[p->scaling.grid].fft, ln.s[l])))
+            return rc;
+    }
+    if ((rc = lanes_join(p, ln))) return rc;
     S2W_CUDA_CHECK(cudaPeekAtLastError());
     return S2W_OK;
 }
