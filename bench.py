@@ -45,7 +45,7 @@ def parse_args():
                     help="sphere workloads: the precomputed-kernel variant (S2W_PRECOMPUTE, step a9)")
     ap.add_argument("--adjoint", action="store_true",
                     help="sphere workloads: time the adjoint pair S^H (signal -> coefficients) + A^H (coefficients -> "
-                         "signal) on a complex-signal plan of the same shape (SURVEY 8(f)-1); no e2e / cpu_baseline")
+                         "signal) of the workload's plan (SURVEY 8(f)-1); no e2e / cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -313,13 +313,10 @@ def run_ours(args, cfg):
         torch.cuda.synchronize()
 
     adj = bool(getattr(args, "adjoint", False))
-    if adj:  # the adjoints are built for complex-signal plans: the same signals, stored as complex
-        cfg = dict(cfg, real=False)
+    if adj:  # no host-buffer entry point and no timed oracle for the adjoints
         args.no_e2e = args.no_cpu_baseline = True
     L, N, lam, J0, mr, real, B = cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"], cfg["real"], cfg["batch"]
     f = make_signals(cfg, api, torch, device, seed_offset=replica_seed_offset(rank))     # independent signals per replica
-    if adj and not f.is_complex():
-        f = f.to(torch.complex128)
     plan = api.s2wav_plan_create(L, N, lam, J0, mr, real, B, local,
                                  flags=api.S2W_PRECOMPUTE if args.precompute else 0)
     cfg["coeff_gb"] = plan.coeff_elems * B * (8 if real else 16) / 1e9

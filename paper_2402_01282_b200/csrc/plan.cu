@@ -1089,7 +1089,7 @@ static int sphere_inverse(const s2w_plan *p, const void *in, void *out, void *wo
     return S2W_OK;
 }
 
-// ---- adjoint transforms (sphere, complex signals) ------------------------------------
+// ---- adjoint transforms (sphere, real and complex signals) ---------------------------
 // With <u, v> = sum conj(u) v over the stored samples, the adjoint of a chain is the reversed chain of adjoints:
 //   (inverse DFT E)^H = n x (normalised forward DFT),   (normalised forward DFT E^H / n)^H = E / n,
 //   (harmonic -> rings contraction D diag(a))^H = diag(conj a) D^T  = the rings -> harmonic contraction, no quadrature,
@@ -1101,7 +1101,7 @@ static int sphere_inverse(const s2w_plan *p, const void *in, void *out, void *wo
 // w.F [B][nrows][t][m]  ->  flmT += c conj(a_l) sum_t d^l_{mn}(theta_t) F
 static int adj_rings_to_harmonic(const s2w_plan *p, const Stage &st, int B, const Work &w, cudaStream_t s)
 {
-    const int Md = 2 * st.Lg - 1;
+    const int Md = p->real ? st.Lg : 2 * st.Lg - 1;
     int rc;
     if ((rc = launch_transpose(w.F, w.Ft, st.Lg, Md, B * st.nrows, s))) return rc;
     WigArgs A;
@@ -1114,7 +1114,7 @@ static int adj_rings_to_harmonic(const s2w_plan *p, const Stage &st, int B, cons
 static int adj_harmonic_to_rings(const s2w_plan *p, const Stage &st, int B, const Work &w, cudaStream_t s)
 {
     const GridTab &g = p->grids[st.grid];
-    const int Md = 2 * st.Lg - 1;
+    const int Md = p->real ? st.Lg : 2 * st.Lg - 1;
     int rc;
     WigArgs A;
     fill_wig_args(p, st, false, B, w.flmT, w.F, A);
@@ -1131,9 +1131,10 @@ static int sphere_forward_adjoint(const s2w_plan *p, const void *in, void *out, 
 {
     const Work w = carve(p, work);
     const int B = p->batch;
-    const cplx *y = (const cplx *)in;
+    const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
+    const char *y = (const char *)in;
     int rc;
-    S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * (2 * p->L - 1) * p->L * sizeof(cplx), s));
+    S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * (p->real ? p->L : 2 * p->L - 1) * p->L * sizeof(cplx), s));
     Lanes ln;  // every block accumulates into flmT by atomics: the blocks are dealt to the lanes, largest first
     if ((rc = lanes_fork(p, w, w.Ft2 + ((p->ws_F_elems + 15) / 16) * 16, s, true, &ln))) return rc;
     for (size_t k = p->scales.size(); k-- > 0;) {
@@ -1142,20 +1143,20 @@ static int sphere_forward_adjoint(const s2w_plan *p, const void *in, void *out, 
         const int l = ln.pick(scale_cost(sc));
         So3Args S;
         fill_so3_args(p, sc.st, S);
-        if ((rc = launch_so3_fwd(false, y + sc.offset, p->coeff_elems, ln.w[l].F, S, B, p->grids[sc.st.grid].fft, ln.s[l])))
+        if ((rc = launch_so3_fwd(p->real, y + sc.offset * esz, p->coeff_elems, ln.w[l].F, S, B, p->grids[sc.st.grid].fft, ln.s[l])))
             return rc;
         if ((rc = adj_rings_to_harmonic(p, sc.st, B, ln.w[l], ln.s[l]))) return rc;
     }
     {
         const int l = ln.pick(0.0);
-        if ((rc = launch_ring_fwd(false, y + p->scaling_offset, ln.w[l].F, B, p->Ls, p->coeff_elems,
+        if ((rc = launch_ring_fwd(p->real, y + p->scaling_offset * esz, ln.w[l].F, B, p->Ls, p->coeff_elems,
                                   p->grids[p->scaling.grid].fft, ln.s[l])))
             return rc;
         if ((rc = adj_rings_to_harmonic(p, p->scaling, B, ln.w[l], ln.s[l]))) return rc;
     }
     if ((rc = lanes_join(p, ln))) return rc;
     if ((rc = adj_harmonic_to_rings(p, p->sht, B, w, s))) return rc;
-    if ((rc = launch_ring_inv(false, w.F, out, B, p->L, p->signal_elems, p->grids[p->sht.grid].fft, s))) return rc;
+    if ((rc = launch_ring_inv(p->real, w.F, out, B, p->L, p->signal_elems, p->grids[p->sht.grid].fft, s))) return rc;
     S2W_CUDA_CHECK(cudaPeekAtLastError());
     return S2W_OK;
 }
@@ -1165,10 +1166,11 @@ static int sphere_inverse_adjoint(const s2w_plan *p, const void *in, void *out, 
 {
     const Work w = carve(p, work);
     const int B = p->batch;
-    cplx *y = (cplx *)out;
+    const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
+    char *y = (char *)out;
     int rc;
-    S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * (2 * p->L - 1) * p->L * sizeof(cplx), s));
-    if ((rc = launch_ring_fwd(false, in, w.F, B, p->L, p->signal_elems, p->grids[p->sht.grid].fft, s))) return rc;
+    S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * (p->real ? p->L : 2 * p->L - 1) * p->L * sizeof(cplx), s));
+    if ((rc = launch_ring_fwd(p->real, in, w.F, B, p->L, p->signal_elems, p->grids[p->sht.grid].fft, s))) return rc;
     if ((rc = adj_rings_to_harmonic(p, p->sht, B, w, s))) return rc;
     Lanes ln;  // every block reads the same flmT
     if ((rc = lanes_fork(p, w, w.Ft2 + ((p->ws_F_elems + 15) / 16) * 16, s, true, &ln))) return rc;
@@ -1176,21 +1178,21 @@ static int sphere_inverse_adjoint(const s2w_plan *p, const void *in, void *out, 
         const Scale &sc = p->scales[k];
         if (sc.st.nn == 0) {
             for (int b = 0; b < B; ++b)
-                S2W_CUDA_CHECK(cudaMemsetAsync(y + (size_t)b * p->coeff_elems + sc.offset, 0,
-                                               (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1) * sizeof(cplx), s));
+                S2W_CUDA_CHECK(cudaMemsetAsync(y + ((size_t)b * p->coeff_elems + sc.offset) * esz, 0,
+                                               (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1) * esz, s));
             continue;
         }
         const int l = ln.pick(scale_cost(sc));
         if ((rc = adj_harmonic_to_rings(p, sc.st, B, ln.w[l], ln.s[l]))) return rc;
         So3Args S;
         fill_so3_args(p, sc.st, S);
-        if ((rc = launch_so3_inv(false, ln.w[l].F, y + sc.offset, p->coeff_elems, S, B, p->grids[sc.st.grid].fft, ln.s[l])))
+        if ((rc = launch_so3_inv(p->real, ln.w[l].F, y + sc.offset * esz, p->coeff_elems, S, B, p->grids[sc.st.grid].fft, ln.s[l])))
             return rc;
     }
     {
         const int l = ln.pick(0.0);
         if ((rc = adj_harmonic_to_rings(p, p->scaling, B, ln.w[l], ln.s[l]))) return rc;
-        if ((rc = launch_ring_inv(false, ln.w[l].F, y + p->scaling_offset, B, p->Ls, p->coeff_elems,
+        if ((rc = launch_ring_inv(p->real, ln.w[l].F, y + p->scaling_offset * esz, B, p->Ls, p->coeff_elems,
                                   p->grids[p->scaling.grid].fft, ln.s[l])))
             return rc;
     }
@@ -1793,8 +1795,8 @@ static int adjoint_supported(const s2w_plan *p, const void *in, const void *out,
         set_error("null pointer");
         return S2W_EINVAL;
     }
-    if (p->kind != 0 || p->real) {
-        set_error("adjoint transforms: complex-signal sphere plans only");
+    if (p->kind != 0) {
+        set_error("adjoint transforms: sphere plans only");
         return S2W_EUNSUPPORTED;
     }
     return S2W_OK;

@@ -95,13 +95,58 @@ def test_inner_product_identities_at_larger_sizes(L, N, lam, J0, mr, batch):
     plan.close()
 
 
+@pytest.mark.parametrize("L,N,lam,J0,mr", [(8, 2, 2.0, 0, True), (9, 3, 2.0, 1, True), (7, 4, 2.0, 0, False)])
+def test_real_plan_adjoints_match_oracle(L, N, lam, J0, mr):
+    """Real-signal plans (m >= 0 kernels): the matrix of A is real in the pixel basis, so its adjoint on a real
+    cotangent is the oracle's A^H applied to it (imaginary part zero); the same for S."""
+    torch, api = _api()
+    rng = np.random.default_rng(800 + L)
+    plan = api.s2wav_plan_create(L, N, lam, J0, mr, True, 1)
+    Y_phi, Y_psi = None, {}
+    for key, shp in ADJ.shapes(L, N, lam, J0, mr):
+        a = rng.standard_normal(shp)
+        if key < 0:
+            Y_phi = a
+        else:
+            Y_psi[key] = a
+    ref = ADJ.analysis_adjoint(Y_phi, Y_psi, L, N, lam, J0, mr, "f80")
+    assert np.abs(ref.imag).max() < 1e-15 * np.abs(ref).max()
+    packed = _pack_for_plan(plan, Y_phi, Y_psi).real.copy()
+    got = plan.forward_adjoint(torch.from_numpy(packed).cuda()).cpu().numpy()
+    assert _relmax(got.reshape(L, 2 * L - 1), ref.real.astype(np.float64)) < TOL
+    g = rng.standard_normal((L, 2 * L - 1))
+    Z_phi, Z_psi = ADJ.synthesis_adjoint(g, L, N, lam, J0, mr, "f80")
+    z = plan.inverse_adjoint(torch.from_numpy(np.ascontiguousarray(g.reshape(1, -1))).cuda())
+    scal, scales = plan.split(z)
+    assert _relmax(scal[0].cpu().numpy(), Z_phi.real.astype(np.float64)) < TOL
+    for j, refj in Z_psi.items():
+        assert np.abs(refj.imag).max() <= 1e-15 * max(np.abs(refj).max(), 1e-300)
+        gotj = scales[(j, 0)][0].cpu().numpy()
+        if np.abs(refj).max() == 0:
+            assert np.abs(gotj).max() == 0
+        else:
+            assert _relmax(gotj, refj.real.astype(np.float64)) < TOL, j
+    plan.close()
+
+
+@pytest.mark.parametrize("L,N,lam,J0,mr,batch", [(96, 6, 2.0, 3, True, 1), (600, 5, 2.0, 6, True, 2), (1024, 5, 2.0, 9, True, 4)])
+def test_real_plan_inner_product_identities(L, N, lam, J0, mr, batch):
+    """<A x, y> = <x, A^T y>, <S y, x> = <y, S^T x> on real plans: ring-pair (alpha, gamma) kernels, accumulating and
+    parked gamma planes, the metric configuration's top scales (L = 1024, N = 5, batch 4, J0 = 9)."""
+    torch, api = _api()
+    gen = torch.Generator(device="cuda").manual_seed(L + N)
+    plan = api.s2wav_plan_create(L, N, lam, J0, mr, True, batch)
+    x = torch.randn(batch, plan.signal_elems, dtype=torch.float64, device="cuda", generator=gen)
+    y = torch.randn(batch, plan.coeff_elems, dtype=torch.float64, device="cuda", generator=gen)
+    Ax, Aty = plan.forward(x), plan.forward_adjoint(y)
+    assert abs(torch.dot(Ax.flatten(), y.flatten()) - torch.dot(x.flatten(), Aty.flatten())) < 1e-12 * Ax.norm() * y.norm()
+    Sy, Stx = plan.inverse(y), plan.inverse_adjoint(x)
+    assert abs(torch.dot(Sy.flatten(), x.flatten()) - torch.dot(y.flatten(), Stx.flatten())) < 1e-12 * Sy.norm() * x.norm()
+    plan.close()
+
+
 def test_adjoint_is_refused_where_it_is_not_built():
     torch, api = _api()
-    pr = api.s2wav_plan_create(8, 2, 2.0, 0, True, True, 1)
-    w = torch.zeros(1, pr.coeff_elems, dtype=torch.float64, device="cuda")
-    with pytest.raises(api.S2WError, match="S2W_EUNSUPPORTED"):
-        pr.forward_adjoint(w)
-    pr.close()
     pb = api.s2ball_plan_create(8, 4, 2, 2.0, 2.0, 0, 1.0)
     w = torch.zeros(1, pb.coeff_elems, dtype=torch.complex128, device="cuda")
     with pytest.raises(api.S2WError, match="S2W_EUNSUPPORTED"):
