@@ -129,6 +129,7 @@ struct Scale {
     Stage st;
     double *Kinv;   // ball: [Pj nodes][Pj p]   K_p(r_i) kappa^{j'}(p) on the Pj-node grid       (analysis)
     double *Kfwd;   // ball: [Pj p][Pj nodes]   q_i K_p(r_i) kappa^{j'}(p)                       (synthesis)
+    double *KinvT, *KfwdT;  // their transposes (adjoint transforms)
 };
 
 }  // namespace
@@ -160,6 +161,7 @@ struct s2w_plan {
     // ball
     double *Kfull_fwd;  // [P p][P nodes]  q_i K_p(r_i)
     double *Kfull_inv;  // [P nodes][P p]  K_p(r_i)
+    double *Kfull_fwdT, *Kfull_invT;  // their transposes (adjoint transforms)
     double *phi_ball;   // [P][L] sqrt(4pi/(2l+1)) Phi_{l0p}
     size_t ws_shell_elems;  // ball: elements of one [P][Mfull][L] harmonic array
     // CUDA graphs of whole transforms (s2w_plan_forward / s2w_plan_inverse), keyed by direction and buffer addresses:
@@ -1305,6 +1307,114 @@ static int ball_inverse(const s2w_plan *p, const void *in, void *out, void *work
     return S2W_OK;
 }
 
+// ---- adjoint transforms (ball): the chains of ball_forward / ball_inverse reversed, radial matrices transposed ------
+static int ball_forward_adjoint(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s)
+{
+    const BallWork bw = carve_ball(p, work);
+    Work w;
+    w.flmT = bw.flm_sh;
+    w.F = bw.F;
+    w.Ft = bw.Ft;
+    w.Ft2 = 0;
+    cplx *spare = bw.Ft + ((p->ws_F_elems + 15) / 16) * 16;
+    const int P = p->P, L = p->L;
+    const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
+    const size_t cols = (size_t)(p->real ? L : 2 * L - 1) * L;
+    const size_t shell = (size_t)L * (2 * L - 1);
+    const char *y = (const char *)in;
+    int rc;
+    S2W_CUDA_CHECK(cudaMemsetAsync(bw.flmp, 0, (size_t)P * cols * sizeof(cplx), s));
+    // wavelet blocks: per j' the adjoint scale stages accumulate into flm_sh, then K_inv^T onto f_{lmp}
+    size_t i = 0;
+    while (i < p->scales.size()) {
+        const Scale &first = p->scales[i];
+        S2W_CUDA_CHECK(cudaMemsetAsync(bw.flm_sh, 0, (size_t)first.Pj * cols * sizeof(cplx), s));
+        size_t e = i;
+        while (e < p->scales.size() && p->scales[e].jp == first.jp) ++e;
+        Lanes ln;
+        if ((rc = lanes_fork(p, w, spare, s, true, &ln))) return rc;
+        for (size_t k = e; k-- > i;) {
+            const Scale &sc = p->scales[k];
+            if (sc.st.nn == 0) continue;
+            const size_t stride = (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1);
+            const int l = ln.pick(scale_cost(sc));
+            So3Args S;
+            fill_so3_args(p, sc.st, S);
+            if ((rc = launch_so3_fwd(p->real, y + sc.offset * esz, stride, ln.w[l].F, S, sc.Pj, p->grids[sc.st.grid].fft, ln.s[l])))
+                return rc;
+            if ((rc = adj_rings_to_harmonic(p, sc.st, sc.Pj, ln.w[l], ln.s[l]))) return rc;
+        }
+        if ((rc = lanes_join(p, ln))) return rc;
+        i = e;
+        if ((rc = launch_radial(first.KinvT, first.Pj, first.Pj, bw.flm_sh, bw.flmp, cols, L, 0, 0, true, s))) return rc;
+    }
+    // scaling block: (Y^-1)^H per shell, then Phi K_inv^T
+    S2W_CUDA_CHECK(cudaMemsetAsync(bw.flm_sh, 0, (size_t)P * cols * sizeof(cplx), s));
+    if ((rc = launch_ring_fwd(p->real, y + p->scaling_offset * esz, w.F, P, L, shell, p->grids[p->sht.grid].fft, s))) return rc;
+    if ((rc = adj_rings_to_harmonic(p, p->sht, P, w, s))) return rc;
+    if ((rc = launch_radial(p->Kfull_invT, P, P, bw.flm_sh, bw.flmp, cols, L, 0, p->phi_ball, true, s))) return rc;
+    // Z^H: K_fwd^T, then Y^H per shell
+    if ((rc = launch_radial(p->Kfull_fwdT, P, P, bw.flmp, bw.flm_sh, cols, L, 0, 0, false, s))) return rc;
+    if ((rc = adj_harmonic_to_rings(p, p->sht, P, w, s))) return rc;
+    if ((rc = launch_ring_inv(p->real, w.F, out, P, L, shell, p->grids[p->sht.grid].fft, s))) return rc;
+    S2W_CUDA_CHECK(cudaPeekAtLastError());
+    return S2W_OK;
+}
+
+static int ball_inverse_adjoint(const s2w_plan *p, const void *in, void *out, void *work, cudaStream_t s)
+{
+    const BallWork bw = carve_ball(p, work);
+    Work w;
+    w.flmT = bw.flm_sh;
+    w.F = bw.F;
+    w.Ft = bw.Ft;
+    w.Ft2 = 0;
+    cplx *spare = bw.Ft + ((p->ws_F_elems + 15) / 16) * 16;
+    const int P = p->P, L = p->L;
+    const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
+    const size_t cols = (size_t)(p->real ? L : 2 * L - 1) * L;
+    const size_t shell = (size_t)L * (2 * L - 1);
+    char *y = (char *)out;
+    int rc;
+    // (Z^-1)^H: (Y^-1)^H per shell, then K_inv^T
+    S2W_CUDA_CHECK(cudaMemsetAsync(bw.flm_sh, 0, (size_t)P * cols * sizeof(cplx), s));
+    if ((rc = launch_ring_fwd(p->real, in, w.F, P, L, shell, p->grids[p->sht.grid].fft, s))) return rc;
+    if ((rc = adj_rings_to_harmonic(p, p->sht, P, w, s))) return rc;
+    if ((rc = launch_radial(p->Kfull_invT, P, P, bw.flm_sh, bw.flmp, cols, L, 0, 0, false, s))) return rc;
+    // wavelet blocks: K_fwd^T onto the P_j' grid, then the adjoint scale stages
+    size_t i = 0;
+    while (i < p->scales.size()) {
+        const Scale &first = p->scales[i];
+        if ((rc = launch_radial(first.KfwdT, first.Pj, first.Pj, bw.flmp, bw.flm_sh, cols, L, 0, 0, false, s))) return rc;
+        size_t e = i;
+        while (e < p->scales.size() && p->scales[e].jp == first.jp) ++e;
+        Lanes ln;
+        if ((rc = lanes_fork(p, w, spare, s, true, &ln))) return rc;
+        for (size_t k = e; k-- > i;) {
+            const Scale &sc = p->scales[k];
+            const size_t stride = (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1);
+            if (sc.st.nn == 0) {
+                S2W_CUDA_CHECK(cudaMemsetAsync(y + sc.offset * esz, 0, (size_t)sc.Pj * stride * esz, s));
+                continue;
+            }
+            const int l = ln.pick(scale_cost(sc));
+            if ((rc = adj_harmonic_to_rings(p, sc.st, sc.Pj, ln.w[l], ln.s[l]))) return rc;
+            So3Args S;
+            fill_so3_args(p, sc.st, S);
+            if ((rc = launch_so3_inv(p->real, ln.w[l].F, y + sc.offset * esz, stride, S, sc.Pj, p->grids[sc.st.grid].fft, ln.s[l])))
+                return rc;
+        }
+        if ((rc = lanes_join(p, ln))) return rc;
+        i = e;
+    }
+    // scaling block: K_fwd^T Phi, then Y^H per shell
+    if ((rc = launch_radial(p->Kfull_fwdT, P, P, bw.flmp, bw.flm_sh, cols, L, p->phi_ball, 0, false, s))) return rc;
+    if ((rc = adj_harmonic_to_rings(p, p->sht, P, w, s))) return rc;
+    if ((rc = launch_ring_inv(p->real, w.F, y + p->scaling_offset * esz, P, L, shell, p->grids[p->sht.grid].fft, s))) return rc;
+    S2W_CUDA_CHECK(cudaPeekAtLastError());
+    return S2W_OK;
+}
+
 }  // namespace s2w
 
 // =================================================================================================================
@@ -1439,6 +1549,7 @@ int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int m
     p->device = device;
     p->real = (flags & S2W_REAL) != 0;
     p->Kfull_fwd = p->Kfull_inv = 0;
+    p->Kfull_fwdT = p->Kfull_invT = 0;
     p->phi_ball = 0;
 #define S2W_PLAN_TRY(expr)          \
     do {                            \
@@ -1546,6 +1657,7 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
     p->device = device;
     p->real = (flags & S2W_REAL) != 0;
     p->Kfull_fwd = p->Kfull_inv = 0;
+    p->Kfull_fwdT = p->Kfull_invT = 0;
     p->phi_ball = 0;
     S2W_PLAN_TRY(plan_common(p));
 
@@ -1589,6 +1701,16 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
             }
         S2W_PLAN_TRY(p->pool.upload(&p->Kfull_fwd, fwd));
         S2W_PLAN_TRY(p->pool.upload(&p->Kfull_inv, inv));
+        {
+            std::vector<double> fwdT((size_t)P * P), invT((size_t)P * P);
+            for (int a = 0; a < P; ++a)
+                for (int b = 0; b < P; ++b) {
+                    fwdT[(size_t)b * P + a] = fwd[(size_t)a * P + b];
+                    invT[(size_t)b * P + a] = inv[(size_t)a * P + b];
+                }
+            S2W_PLAN_TRY(p->pool.upload(&p->Kfull_fwdT, fwdT));
+            S2W_PLAN_TRY(p->pool.upload(&p->Kfull_invT, invT));
+        }
         S2W_PLAN_TRY(p->pool.upload(&p->phi_ball, phi));
     }
     size_t off = 0;
@@ -1624,15 +1746,27 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
                 kinv[(size_t)i * Pj + pp] = K[(size_t)pp * Pj + i] * kj[pp];
                 kfwd[(size_t)pp * Pj + i] = t3 * qw[i] * K[(size_t)pp * Pj + i] * kj[pp];
             }
-        double *dKinv, *dKfwd;
+        double *dKinv, *dKfwd, *dKinvT, *dKfwdT;
         S2W_PLAN_TRY(p->pool.upload(&dKinv, kinv));
         S2W_PLAN_TRY(p->pool.upload(&dKfwd, kfwd));
+        {
+            std::vector<double> kinvT((size_t)Pj * Pj), kfwdT((size_t)Pj * Pj);
+            for (int a = 0; a < Pj; ++a)
+                for (int b = 0; b < Pj; ++b) {
+                    kinvT[(size_t)b * Pj + a] = kinv[(size_t)a * Pj + b];
+                    kfwdT[(size_t)b * Pj + a] = kfwd[(size_t)a * Pj + b];
+                }
+            S2W_PLAN_TRY(p->pool.upload(&dKinvT, kinvT));
+            S2W_PLAN_TRY(p->pool.upload(&dKfwdT, kfwdT));
+        }
         for (size_t a = 0; a < ang.size(); ++a) {
             Scale sc = ang[a];
             sc.jp = jp;
             sc.Pj = Pj;
             sc.Kinv = dKinv;
             sc.Kfwd = dKfwd;
+            sc.KinvT = dKinvT;
+            sc.KfwdT = dKfwdT;
             sc.offset = off;
             off += (size_t)Pj * nn * sc.Lj * (2 * sc.Lj - 1);
             p->scales.push_back(sc);
@@ -1719,8 +1853,8 @@ static void *align256(void *p) { return (void *)(((uintptr_t)p + 255) & ~(uintpt
 static int run_transform(const s2w_plan *p, int dir, const void *in, void *out, void *work, cudaStream_t s)
 {
     auto direct = [&](cudaStream_t st) {
-        if (dir == 2) return sphere_forward_adjoint(p, in, out, work, st);
-        if (dir == 3) return sphere_inverse_adjoint(p, in, out, work, st);
+        if (dir == 2) return p->kind == 1 ? ball_forward_adjoint(p, in, out, work, st) : sphere_forward_adjoint(p, in, out, work, st);
+        if (dir == 3) return p->kind == 1 ? ball_inverse_adjoint(p, in, out, work, st) : sphere_inverse_adjoint(p, in, out, work, st);
         if (p->kind == 1) return dir == 0 ? ball_forward(p, in, out, work, st) : ball_inverse(p, in, out, work, st);
         return dir == 0 ? sphere_forward(p, in, out, work, st) : sphere_inverse(p, in, out, work, st);
     };
@@ -1794,10 +1928,6 @@ static int adjoint_supported(const s2w_plan *p, const void *in, const void *out,
     if (!p || !in || !out || !work) {
         set_error("null pointer");
         return S2W_EINVAL;
-    }
-    if (p->kind != 0) {
-        set_error("adjoint transforms: sphere plans only");
-        return S2W_EUNSUPPORTED;
     }
     return S2W_OK;
 }
