@@ -491,13 +491,27 @@ def run_ball(args, cfg):
     w = torch.empty((1, plan.coeff_elems), dtype=plan.dtype, device=device)
     back = torch.empty((1, plan.signal_elems), dtype=plan.dtype, device=device)
 
+    adj = bool(getattr(args, "adjoint", False))
+    if adj:
+        args.no_e2e = args.no_cpu_baseline = True
+
     def step():
-        plan.forward(f, out=w)
-        plan.inverse(w, out=back)
+        if adj:
+            plan.inverse_adjoint(f, out=w)
+            plan.forward_adjoint(w, out=back)
+        else:
+            plan.forward(f, out=w)
+            plan.inverse(w, out=back)
     for _ in range(max(args.warmup, 3)):
         step()
     torch.cuda.synchronize()
-    rt_err = float((back - f).abs().max() / f.abs().max())
+    if adj:  # the defining identity <A f, y> = <f, A^H y> with y = S^H f
+        Af = plan.forward(f)
+        rt_err = float((torch.vdot(Af.flatten(), w.flatten()) - torch.vdot(f.flatten(), back.flatten())).abs()
+                       / (Af.norm() * w.norm()))
+        del Af
+    else:
+        rt_err = float((back - f).abs().max() / f.abs().max())
     sampler = ClockSampler(0)
     sampler.start()
     l0 = api.launch_count()
@@ -551,11 +565,12 @@ def run_ball(args, cfg):
         "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "C5: ball L=%d P=%d N=%d lambda_l=%g lambda_p=%g J0=%d tau=%g complex fp64, "
-                               "forward+inverse" % (L, P, N, lam, nu, J0, tau),
+                               "%s" % (L, P, N, lam, nu, J0, tau, "adjoint pair S^H + A^H" if adj else "forward+inverse"),
                    "L": L, "P": P, "N": N, "parallelism": "replicas x1 (no data-path collective)",
                    "l2": "coefficient block per step (%.2f GB) exceeds the 126 MB L2; no explicit flush"
                          % (plan.coeff_elems * 16 / 1e9)},
-        "clocks": clocks, "gpu_launches": int(launches), "roundtrip_rel_err": rt_err,
+        "clocks": clocks, "gpu_launches": int(launches),
+        ("adjoint_identity_rel_err" if adj else "roundtrip_rel_err"): rt_err,
         "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                      "frac": achieved / peak if peak else None, "traffic": None,
                      "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x sm_max_mhz (DESIGN.md)",

@@ -101,8 +101,8 @@ int s2w_plan_inverse(const s2w_plan *plan, const void *in_dev, void *out_dev, vo
  *   <A f, y> = <f, A^H y>    s2w_plan_forward_adjoint: in = coefficient-shaped y, out = signal-shaped A^H y;
  *   <S w, g> = <w, S^H g>    s2w_plan_inverse_adjoint: in = signal-shaped g,      out = coefficient-shaped S^H g,
  * A = s2w_plan_forward, S = s2w_plan_inverse.  Same buffers, layouts, workspace and stream semantics as those.
- * Sphere plans, real or complex (on an S2W_REAL plan cotangents and results are real: the adjoint is the transpose
- * of the real matrix); S2W_EUNSUPPORTED for ball plans. */
+ * Sphere and ball plans, real or complex (on an S2W_REAL plan cotangents and results are real: the adjoint is the
+ * transpose of the real matrix). */
 int s2w_plan_forward_adjoint(const s2w_plan *plan, const void *in_dev, void *out_dev, void *work_dev, void *stream);
 int s2w_plan_inverse_adjoint(const s2w_plan *plan, const void *in_dev, void *out_dev, void *work_dev, void *stream);
 

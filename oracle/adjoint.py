@@ -92,3 +92,52 @@ def synthesis_adjoint(g, L, N, lam, J0, multires, prec="f80", matrix=None):
     M = synthesis_matrix(L, N, lam, J0, multires, prec) if matrix is None else matrix
     v = np.conj(M).T @ np.asarray(g).reshape(-1).astype(M.dtype)
     return unpack(v, L, N, lam, J0, multires)
+
+
+# --------------------------------------------------------------------------
+# ball (oracle/ball.py): the same definition.  A coefficient set is (W_phi [P][L][2L-1],
+# {(j, j'): [P_j'][2N-1][L_j][2L_j-1]}), packed W_phi first, then the blocks in sorted key order.
+# --------------------------------------------------------------------------
+def ball_pack(W_phi, W_psi):
+    return np.concatenate([np.asarray(W_phi).reshape(-1)] + [np.asarray(W_psi[k]).reshape(-1) for k in sorted(W_psi)])
+
+
+def ball_analysis_adjoint_entries(Y_phi, Y_psi, entries, L, P, N, lam, nu, J0, J0p, tau, prec="f80"):
+    """Sampled entries of A^H y on the ball: for each voxel index k (C order of [P][L][2L-1]) in `entries`,
+    <A e_k, y> -- one oracle analysis each."""
+    from . import ball as OB
+    filt = OB.filters(L, P, N, lam, nu, J0, J0p, prec)
+    y = ball_pack(Y_phi, Y_psi).astype(S.CPLX[prec])
+    nvox = P * L * (2 * L - 1)
+    out = []
+    for k in entries:
+        e = np.zeros(nvox, dtype=S.CPLX[prec])
+        e[k] = 1
+        W_phi, W_psi = OB.analysis(e.reshape(P, L, 2 * L - 1), L, P, N, lam, nu, J0, J0p, tau, prec, filt)
+        out.append(np.vdot(ball_pack(W_phi, W_psi), y))
+    return np.array(out)
+
+
+def ball_synthesis_adjoint_entries(g, template, entries, L, P, N, lam, nu, J0, J0p, tau, prec="f80"):
+    """Sampled entries of S^H g on the ball: for each packed coefficient index c in `entries`, <S e_c, g> (one oracle
+    synthesis each).  `template` = (W_phi, W_psi) of the right shapes (values ignored)."""
+    from . import ball as OB
+    filt = OB.filters(L, P, N, lam, nu, J0, J0p, prec)
+    T_phi, T_psi = template
+    keys = sorted(T_psi)
+    sizes = [int(np.asarray(T_phi).size)] + [int(np.asarray(T_psi[k]).size) for k in keys]
+    ncoef = sum(sizes)
+    gv = np.asarray(g).reshape(-1).astype(S.CPLX[prec])
+    out = []
+    for c in entries:
+        e = np.zeros(ncoef, dtype=S.CPLX[prec])
+        e[c] = 1
+        o = sizes[0]
+        W_phi = e[:o].reshape(np.asarray(T_phi).shape)
+        W_psi = {}
+        for k, n in zip(keys, sizes[1:]):
+            W_psi[k] = e[o:o + n].reshape(np.asarray(T_psi[k]).shape)
+            o += n
+        f = OB.synthesis(W_phi, W_psi, L, P, N, lam, nu, J0, J0p, tau, prec, filt)
+        out.append(np.vdot(np.asarray(f).reshape(-1), gv))
+    return np.array(out)

@@ -145,10 +145,69 @@ def test_real_plan_inner_product_identities(L, N, lam, J0, mr, batch):
     plan.close()
 
 
-def test_adjoint_is_refused_where_it_is_not_built():
+@pytest.mark.parametrize("L,P,N,lam,nu,J0,tau", [(6, 4, 2, 2.0, 2.0, 0, 1.0), (8, 5, 3, 2.0, 3.0, 1, 0.5)])
+def test_ball_adjoints_match_oracle_on_sampled_entries(L, P, N, lam, nu, J0, tau):
+    """Ball plans: sampled entries of A^H y and S^H g against the oracle (one oracle transform per entry)."""
+    from oracle import ball as OB
     torch, api = _api()
-    pb = api.s2ball_plan_create(8, 4, 2, 2.0, 2.0, 0, 1.0)
-    w = torch.zeros(1, pb.coeff_elems, dtype=torch.complex128, device="cuda")
-    with pytest.raises(api.S2WError, match="S2W_EUNSUPPORTED"):
-        pb.forward_adjoint(w)
-    pb.close()
+    rng = np.random.default_rng(900 + L)
+    plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau)
+    T_phi, T_psi = OB.analysis(np.zeros((P, L, 2 * L - 1), dtype=np.clongdouble), L, P, N, lam, nu, J0, J0, tau, "f80")
+    Y_phi = _rand_c(rng, T_phi.shape)
+    Y_psi = {k: _rand_c(rng, v.shape) for k, v in T_psi.items()}
+    packed = np.zeros((1, plan.coeff_elems), dtype=np.complex128)
+    index_of = {}            # oracle packing index -> plan packing index, block by block
+    nr, ng, nt, npx, off = plan.scale_shape(-1)
+    packed[0, off:off + nr * nt * npx] = Y_phi.astype(np.complex128).ravel()
+    blocks = [(0, off, T_phi.size)]
+    o = T_phi.size
+    for key in sorted(T_psi):
+        nr, ng, nt, npx, off = plan.scale_shape(*key)
+        assert (nr, ng, nt, npx) == T_psi[key].shape
+        packed[0, off:off + T_psi[key].size] = Y_psi[key].astype(np.complex128).ravel()
+        blocks.append((o, off, T_psi[key].size))
+        o += T_psi[key].size
+    nvox = P * L * (2 * L - 1)
+    vox = sorted(rng.choice(nvox, size=24, replace=False).tolist())
+    ref = ADJ.ball_analysis_adjoint_entries(Y_phi, Y_psi, vox, L, P, N, lam, nu, J0, J0, tau, "f80")
+    got = plan.forward_adjoint(torch.from_numpy(packed).cuda()).cpu().numpy().ravel()
+    assert np.abs(got[vox] - ref.astype(np.complex128)).max() < TOL * np.abs(got).max()
+    g = _rand_c(rng, (P, L, 2 * L - 1))
+    cs = sorted(rng.choice(o, size=40, replace=False).tolist())
+    ref = ADJ.ball_synthesis_adjoint_entries(g, (T_phi, T_psi), cs, L, P, N, lam, nu, J0, J0, tau, "f80")
+    z = plan.inverse_adjoint(torch.from_numpy(np.ascontiguousarray(g.reshape(1, -1))).cuda()).cpu().numpy().ravel()
+
+    def plan_index(c):
+        for o0, off, n in blocks:
+            if o0 <= c < o0 + n:
+                return off + (c - o0)
+        raise AssertionError(c)
+
+    gotc = np.array([z[plan_index(c)] for c in cs])
+    assert np.abs(gotc - ref.astype(np.complex128)).max() < TOL * np.abs(z).max()
+    plan.close()
+
+
+@pytest.mark.parametrize("L,P,N,real", [(20, 16, 3, False), (12, 6, 3, True), (128, 128, 3, False)])
+def test_ball_inner_product_identities(L, P, N, real):
+    """<A x, y> = <x, A^H y>, <S y, x> = <y, S^H x> on ball plans up to BASELINE config 5 (L = P = 128)."""
+    torch, api = _api()
+    gen = torch.Generator(device="cuda").manual_seed(L + P)
+    plan = api.s2ball_plan_create(L, P, N, 2.0, 2.0, 0, 1.0, real=real)
+    dt = torch.float64 if real else torch.complex128
+    x = torch.randn(1, plan.signal_elems, dtype=dt, device="cuda", generator=gen)
+    y = torch.randn(1, plan.coeff_elems, dtype=dt, device="cuda", generator=gen)
+    Ax, Ahy = plan.forward(x), plan.forward_adjoint(y)
+    assert abs(torch.vdot(Ax.flatten(), y.flatten()) - torch.vdot(x.flatten(), Ahy.flatten())) < 1e-12 * Ax.norm() * y.norm()
+    Sy, Shx = plan.inverse(y), plan.inverse_adjoint(x)
+    assert abs(torch.vdot(Sy.flatten(), x.flatten()) - torch.vdot(y.flatten(), Shx.flatten())) < 1e-12 * Sy.norm() * x.norm()
+    plan.close()
+
+
+def test_adjoint_argument_errors():
+    torch, api = _api()
+    plan = api.s2wav_plan_create(8, 2, 2.0, 0, True, False, 1)
+    with pytest.raises(ValueError):
+        plan.forward_adjoint(torch.zeros(1, plan.coeff_elems - 1, dtype=torch.complex128, device="cuda"))
+    assert api.lib().s2w_plan_forward_adjoint(None, None, None, None, None) == -1  # S2W_EINVAL
+    plan.close()

@@ -76,3 +76,35 @@ def test_one_pixel_case_is_complex_conjugation():
     y = ADJ.pack(Y_phi, Y_psi, L, N, lam, J0, mr)
     got = ADJ.analysis_adjoint(Y_phi, Y_psi, L, N, lam, J0, mr, "f80")
     assert abs(got[0, 0] - np.sum(np.conj(a) * y)) < 1e-17 * (1 + abs(got[0, 0])) * 100
+
+
+def test_ball_adjoint_entries_inner_product_identity():
+    """Ball: sampled entries of A^H y and S^H g against <A x, y> and <S w, g> with x / w supported on the sampled
+    entries and A x, S w computed by applying the oracle directly."""
+    from oracle import ball as OB
+    L, P, N, lam, nu, J0, tau = 5, 3, 2, 2.0, 2.0, 0, 1.0
+    rng = np.random.default_rng(3)
+    nvox = P * L * (2 * L - 1)
+    T_phi, T_psi = OB.analysis(np.zeros((P, L, 2 * L - 1), dtype=np.clongdouble), L, P, N, lam, nu, J0, J0, tau, "f80")
+    Y_phi = _rand_c(rng, T_phi.shape)
+    Y_psi = {k: _rand_c(rng, v.shape) for k, v in T_psi.items()}
+    vox = sorted(rng.choice(nvox, size=6, replace=False).tolist())
+    x = np.zeros(nvox, dtype=np.clongdouble)
+    x[vox] = _rand_c(rng, len(vox))
+    W_phi, W_psi = OB.analysis(x.reshape(P, L, 2 * L - 1), L, P, N, lam, nu, J0, J0, tau, "f80")
+    lhs = np.vdot(ADJ.ball_pack(W_phi, W_psi), ADJ.ball_pack(Y_phi, Y_psi))
+    rhs = np.vdot(x[vox], ADJ.ball_analysis_adjoint_entries(Y_phi, Y_psi, vox, L, P, N, lam, nu, J0, J0, tau, "f80"))
+    assert abs(lhs - rhs) < 1e-15 * abs(lhs) * 50
+    ncoef = ADJ.ball_pack(T_phi, T_psi).size
+    cs = sorted(rng.choice(ncoef, size=8, replace=False).tolist())
+    w = np.zeros(ncoef, dtype=np.clongdouble)
+    w[cs] = _rand_c(rng, len(cs))
+    o = T_phi.size
+    V_phi, V_psi = w[:o].reshape(T_phi.shape), {}
+    for k in sorted(T_psi):
+        V_psi[k] = w[o:o + T_psi[k].size].reshape(T_psi[k].shape)
+        o += T_psi[k].size
+    g = _rand_c(rng, (P, L, 2 * L - 1))
+    lhs = np.vdot(OB.synthesis(V_phi, V_psi, L, P, N, lam, nu, J0, J0, tau, "f80"), g)
+    rhs = np.vdot(w[cs], ADJ.ball_synthesis_adjoint_entries(g, (T_phi, T_psi), cs, L, P, N, lam, nu, J0, J0, tau, "f80"))
+    assert abs(lhs - rhs) < 1e-15 * abs(lhs) * 50
