@@ -40,7 +40,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5", "T2"])
     ap.add_argument("--precompute", action="store_true",
                     help="sphere workloads: the precomputed-kernel variant (S2W_PRECOMPUTE, step a9)")
     ap.add_argument("--adjoint", action="store_true",
@@ -486,7 +486,7 @@ def run_ball(args, cfg):
     device = torch.device("cuda", 0)
     L, P, N, lam, nu, J0, tau = cfg["L"], cfg["P"], cfg["N"], cfg["lam"], cfg["nu"], cfg["J0"], cfg["tau"]
     plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau)
-    flmp = inputs.config_coefficients("C5")
+    flmp = inputs.config_coefficients(cfg["name"])
     f = plan.harmonic_inverse(torch.from_numpy(flmp).to(device).reshape(1, -1))
     w = torch.empty((1, plan.coeff_elems), dtype=plan.dtype, device=device)
     back = torch.empty((1, plan.signal_elems), dtype=plan.dtype, device=device)
@@ -564,8 +564,8 @@ def run_ball(args, cfg):
         "metric": METRIC, "value": args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "C5: ball L=%d P=%d N=%d lambda_l=%g lambda_p=%g J0=%d tau=%g complex fp64, "
-                               "%s" % (L, P, N, lam, nu, J0, tau, "adjoint pair S^H + A^H" if adj else "forward+inverse"),
+        "config": {"workload": "%s: ball L=%d P=%d N=%d lambda_l=%g lambda_p=%g J0=%d tau=%g complex fp64, "
+                               "%s" % (cfg["name"], L, P, N, lam, nu, J0, tau, "adjoint pair S^H + A^H" if adj else "forward+inverse"),
                    "L": L, "P": P, "N": N, "parallelism": "replicas x1 (no data-path collective)",
                    "l2": "coefficient block per step (%.2f GB) exceeds the 126 MB L2; no explicit flush"
                          % (plan.coeff_elems * 16 / 1e9)},

@@ -23,6 +23,9 @@ CONFIGS = {
                spectrum="l^-2"),
     "C5": dict(kind="ball", L=128, P=128, N=3, lam=2.0, nu=2.0, J0=0, J0p=0, tau=1.0, real=False, seed=4,
                spectrum="l^-2 p^-1"),
+    # not a BASELINE.json configuration: the shape of the paper's Table 2 (ball, N = 1, P = L) at its largest size
+    "T2": dict(kind="ball", L=256, P=256, N=1, lam=2.0, nu=2.0, J0=0, J0p=0, tau=1.0, real=False, seed=5,
+               spectrum="l^-2 p^-1"),
 }
 
 
