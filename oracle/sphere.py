@@ -303,33 +303,36 @@ def mw_reweight(F, L, sigma, prec):
 
 
 # --------------------------------------------------------------------------
-# O2 / O3: spherical harmonic transforms Y^-1, Y (Eqs. 2-3; spin 0)
+# O2 / O3: spherical harmonic transforms Y^-1, Y (Eqs. 2-3), spin s (Eq. 1):
+#   sY_{lm}(theta, phi) = (-1)^s sqrt((2l+1)/4pi) D^{l*}_{m,-s}(phi, theta, 0)
+#                       = (-1)^s sqrt((2l+1)/4pi) d^l_{m,-s}(theta) e^{i m phi},      zero for l < |s|.
 # --------------------------------------------------------------------------
-def sht_inverse(flm, L, prec="f80", thetas=None):
-    """f(theta_t, phi_p) = sum_{l m} f_{lm} Y_{lm},  Y_{lm} = sqrt((2l+1)/4pi) d^l_{m0}(theta) e^{i m phi}
+def sht_inverse(flm, L, prec="f80", thetas=None, spin=0):
+    """f(theta_t, phi_p) = sum_{l m} f_{lm} sY_{lm}; spin 0: Y_{lm} = sqrt((2l+1)/4pi) d^l_{m0}(theta) e^{i m phi}
     (Eq. 3; R2).  `thetas` overrides the MW rings (used to evaluate single rings)."""
     rt, ct = REAL[prec], CPLX[prec]
     flm = _as(flm, ct)
     ell = np.arange(L).astype(rt)
-    c_l = np.sqrt((2 * ell + 1) / (4 * pi(prec)))
+    c_l = np.sqrt((2 * ell + 1) / (4 * pi(prec))) * (-1 if spin % 2 else 1)
     th = mw_thetas(L, prec) if thetas is None else _as(thetas, rt)
-    Fm = dl_inverse(c_l[:, None] * flm, L, 0, th, prec)          # [mi][t]
+    Fm = dl_inverse(c_l[:, None] * flm, L, -spin, th, prec)      # [mi][t]
     Fm = _centered_to_fft_order(Fm.T, L)                          # [t][m mod n]
     return dft_last_axis(Fm, +1, prec)                            # sum_m F_m e^{+i m phi_p}
 
 
-def sht_forward(f, L, prec="f80"):
-    """f_{lm} = int f Y*_{lm} dOmega, exact on the MW grid for band-limit L (O3, R3)."""
+def sht_forward(f, L, prec="f80", spin=0):
+    """f_{lm} = int f sY*_{lm} dOmega, exact on the MW grid for band-limit L (O3, R3); the integrand's theta
+    dependence has parity (-1)^{m+s} under the extension of R3 (ii)."""
     rt, ct = REAL[prec], CPLX[prec]
     f = _as(f, ct)
     n = 2 * L - 1
     Fm = dft_last_axis(f, -1, prec) / rt(n)                       # (i)  [t][m mod n]
     Fm = _fft_order_to_centered(Fm, L).T                          # [mi][t]
     m = np.arange(-(L - 1), L)
-    H = mw_reweight(Fm, L, np.where(m % 2 == 0, 1, -1), prec)     # (ii)-(vi), parity (-1)^m
-    W = dl_forward(H, L, 0, mw_thetas(L, prec), prec)             # (vii)
+    H = mw_reweight(Fm, L, np.where((m + spin) % 2 == 0, 1, -1), prec)   # (ii)-(vi), parity (-1)^{m+s}
+    W = dl_forward(H, L, -spin, mw_thetas(L, prec), prec)         # (vii)
     ell = np.arange(L).astype(rt)
-    c_l = np.sqrt((2 * ell + 1) / (4 * pi(prec)))
+    c_l = np.sqrt((2 * ell + 1) / (4 * pi(prec))) * (-1 if spin % 2 else 1)
     return (2 * pi(prec) / rt(n)) * c_l[:, None] * W
 
 
@@ -405,7 +408,7 @@ def _pad_lm(a, Lc, L):
     return out
 
 
-def analysis_from_flm(flm, L, N, lam, J0, multires, prec="f80", filt=None, scales=None, rings=None):
+def analysis_from_flm(flm, L, N, lam, J0, multires, prec="f80", filt=None, scales=None, rings=None, spin=0):
     """Algorithm 1 'Analysis' after its first line:
     returns (W_phi, {j: W_psi_j}).  `scales` restricts j; `rings` = {j: ring indices}
     evaluates only those beta rings of scale j (same sums, fewer outputs)."""
@@ -416,7 +419,7 @@ def analysis_from_flm(flm, L, N, lam, J0, multires, prec="f80", filt=None, scale
     # W^Phi_hat = Phi f_hat : einsum("lm,l->lm") with entries sqrt(4pi/(2l+1)) Phi*_{l0}  (Eq. 29/41, R5)
     wphi_hat = np.einsum("lm,l->lm", flm, np.sqrt(4 * pi(prec) / (2 * ell + 1)) * phi)
     Ls = bandlimit_of_scaling(L, lam, J0, multires)
-    W_phi = sht_inverse(_crop_lm(wphi_hat, L, Ls), Ls, prec)      # Y^-1
+    W_phi = sht_inverse(_crop_lm(wphi_hat, L, Ls), Ls, prec, spin=spin)   # Y^-1 (a spin-s field, Eq. 12)
     W_psi = {}
     for j in (range(J0, J + 1) if scales is None else scales):
         Lj = bandlimit_of_scale(j, L, lam, multires)
@@ -430,19 +433,19 @@ def analysis_from_flm(flm, L, N, lam, J0, multires, prec="f80", filt=None, scale
     return W_phi, W_psi
 
 
-def analysis(f, L, N, lam, J0, multires, prec="f80", filt=None):
-    """Algorithm 1 'Analysis wavelet transform'."""
-    flm = sht_forward(f, L, prec)                                 # f_hat <- Y f
-    return analysis_from_flm(flm, L, N, lam, J0, multires, prec, filt)
+def analysis(f, L, N, lam, J0, multires, prec="f80", filt=None, spin=0):
+    """Algorithm 1 'Analysis wavelet transform'; `spin`: the signal's spin number (Eq. 1)."""
+    flm = sht_forward(f, L, prec, spin=spin)                      # f_hat <- Y f
+    return analysis_from_flm(flm, L, N, lam, J0, multires, prec, filt, spin=spin)
 
 
-def synthesis_to_flm(W_phi, W_psi, L, N, lam, J0, multires, prec="f80", filt=None):
+def synthesis_to_flm(W_phi, W_psi, L, N, lam, J0, multires, prec="f80", filt=None, spin=0):
     """Algorithm 1 'Synthesis' up to its last line: returns f_hat."""
     rt, ct = REAL[prec], CPLX[prec]
     psi, phi, J = filters(L, N, lam, J0, prec) if filt is None else filt
     ell = np.arange(L).astype(rt)
     Ls = bandlimit_of_scaling(L, lam, J0, multires)
-    wphi_hat = _pad_lm(sht_forward(W_phi, Ls, prec), Ls, L)       # Y W^Phi
+    wphi_hat = _pad_lm(sht_forward(W_phi, Ls, prec, spin=spin), Ls, L)    # Y W^Phi
     flm = np.einsum("lm,l->lm", wphi_hat, np.sqrt(4 * pi(prec) / (2 * ell + 1)) * phi)
     for j in range(J0, J + 1):
         Lj = bandlimit_of_scale(j, L, lam, multires)
@@ -452,7 +455,7 @@ def synthesis_to_flm(W_phi, W_psi, L, N, lam, J0, multires, prec="f80", filt=Non
     return flm
 
 
-def synthesis(W_phi, W_psi, L, N, lam, J0, multires, prec="f80", filt=None):
+def synthesis(W_phi, W_psi, L, N, lam, J0, multires, prec="f80", filt=None, spin=0):
     """Algorithm 1 'Synthesis wavelet transform'."""
-    flm = synthesis_to_flm(W_phi, W_psi, L, N, lam, J0, multires, prec, filt)
-    return sht_inverse(flm, L, prec)                              # f <- Y^-1 f_hat
+    flm = synthesis_to_flm(W_phi, W_psi, L, N, lam, J0, multires, prec, filt, spin=spin)
+    return sht_inverse(flm, L, prec, spin=spin)                   # f <- Y^-1 f_hat

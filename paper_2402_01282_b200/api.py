@@ -26,6 +26,8 @@ SIGNATURES = {
     "s2ball_radial_nodes": (_c_int, [_c_vp, _c_vp, _c_int, _c_dbl]),
     "s2wav_plan_create": (_c_int, [ctypes.POINTER(_c_vp), _c_int, _c_int, _c_dbl, _c_int, _c_int, _c_int, _c_int,
                                    _c_int]),
+    "s2wav_plan_create_spin": (_c_int, [ctypes.POINTER(_c_vp), _c_int, _c_int, _c_dbl, _c_int, _c_int, _c_int, _c_int,
+                                        _c_int, _c_int]),
     "s2ball_plan_create": (_c_int, [ctypes.POINTER(_c_vp), _c_int, _c_int, _c_int, _c_dbl, _c_dbl, _c_int, _c_dbl,
                                     _c_int, _c_int]),
     "s2w_plan_destroy": (_c_int, [_c_vp]),
@@ -266,11 +268,15 @@ class Plan:
         return scal, out
 
 
-def s2wav_plan_create(L, N, lam, J0, multiresolution=True, real=False, batch=1, device=0, flags=0):
+def s2wav_plan_create(L, N, lam, J0, multiresolution=True, real=False, batch=1, device=0, flags=0, spin=0):
     h = _c_vp()
     fl = int(flags) | (S2W_REAL if real else 0)
-    _check(lib().s2wav_plan_create(ctypes.byref(h), int(L), int(N), float(lam), int(J0), int(bool(multiresolution)),
-                                   fl, int(batch), int(device)))
+    if spin:
+        _check(lib().s2wav_plan_create_spin(ctypes.byref(h), int(L), int(N), float(lam), int(J0),
+                                            int(bool(multiresolution)), fl, int(batch), int(device), int(spin)))
+    else:
+        _check(lib().s2wav_plan_create(ctypes.byref(h), int(L), int(N), float(lam), int(J0),
+                                       int(bool(multiresolution)), fl, int(batch), int(device)))
     return Plan(h, bool(real), int(batch), "sphere")
 
 

@@ -146,7 +146,8 @@ struct s2w_plan {
     bool real;
     DevPool pool;
     std::vector<GridTab> grids;
-    std::vector<int> tabn;  // table values of n: script-N united with {0}
+    int spin;               // spin number s of the signal (Eq. 1): the SHT stages contract with d^l_{m,-s}
+    std::vector<int> tabn;  // table values of n: script-N united with {-spin, +spin}
     double *coef;
     size_t tri;
     cplx *tw;
@@ -667,7 +668,8 @@ int plan_common(s2w_plan *p)
     int rc;
     p->tabn.clear();
     for (int n = -(p->N - 1); n <= p->N - 1; n += 2) p->tabn.push_back(n);
-    if (find_tab(p, 0) < 0) p->tabn.push_back(0);
+    if (find_tab(p, -p->spin) < 0) p->tabn.push_back(-p->spin);
+    if (find_tab(p, p->spin) < 0) p->tabn.push_back(p->spin);  // the mirror columns (-m, -s) run the recursion of +s
     p->tri = (size_t)p->L * (p->L + 1) / 2;
     {
         std::vector<double> coef;
@@ -703,13 +705,29 @@ int make_n0_stage(s2w_plan *p, Stage &st, int Lg, const std::vector<double> &a, 
     st.grid = grid_index(p, Lg);
     st.Lg = Lg;
     st.lmin = 0;
-    std::vector<int> ns(1, 0), rows(1, 0);
-    if ((rc = fill_stage_rows(p, st, ns, rows, 1))) return rc;
-    std::vector<cplx> fa(Lg), fs(Lg);
-    for (int l = 0; l < Lg; ++l) {
-        fa[l] = cmake(a[l], 0.0);
-        fs[l] = cmake(s[l], 0.0);
+    // spin-s harmonics sY_lm = (-1)^s sqrt((2l+1)/4pi) d^l_{m,-s}(theta) e^{i m phi} (Eq. 1): the row n = -s, zero
+    // below l = |s| (the contraction kernels start at max(|m|, |n|)); no row at all when the band-limit is <= |s|.
+    // The kernels pair the column (m, n) with (-m, -n) (one recursion serves both), so for s != 0 the stage carries
+    // the recursions of n = -s (columns m >= 0 of row 0) and n = +s (whose mirror columns are (-m, -s): the m < 0 half of
+    // row 0); the other halves land in / are read from a second, scratch row that the FFT side keeps at zero.
+    const int nspin = -p->spin;
+    std::vector<int> ns, rows;
+    if (std::abs(nspin) < Lg) {
+        ns.push_back(nspin);
+        rows.push_back(0);
+        if (nspin != 0) {
+            ns.push_back(-nspin);
+            rows.push_back(1);
+        }
     }
+    if ((rc = fill_stage_rows(p, st, ns, rows, nspin != 0 ? 2 : 1))) return rc;
+    const double sgn = (p->spin & 1) ? -1.0 : 1.0;
+    std::vector<cplx> fa((size_t)std::max(1, st.nn) * Lg), fs((size_t)std::max(1, st.nn) * Lg);
+    for (int q = 0; q < std::max(1, st.nn); ++q)
+        for (int l = 0; l < Lg; ++l) {
+            fa[(size_t)q * Lg + l] = cmake(sgn * a[l], 0.0);
+            fs[(size_t)q * Lg + l] = cmake(sgn * s[l], 0.0);
+        }
     return make_stage_filters(p, st, fa, fs, 2.0 * Lg - 1.0);
 }
 
@@ -835,13 +853,47 @@ static int lanes_join(const s2w_plan *p, const Lanes &ln)
 
 static double scale_cost(const Scale &sc) { return (double)sc.Lj * sc.Lj * sc.Lj * (sc.st.nn + 0.01); }
 
+// Ring FFTs of an SHT stage (a1).  A spin stage has two rows per signal in F (the second one scratch, kept at zero on
+// the way to the forward contraction), so its signals are transformed one by one into / out of row 0.
+static int stage_ring_fwd(const s2w_plan *p, const Stage &st, const void *f, size_t sig_stride, int B, cplx *F,
+                          cudaStream_t s)
+{
+    const FftTab &T = p->grids[st.grid].fft;
+    if (st.nrows == 1) return launch_ring_fwd(p->real, f, F, B, st.Lg, sig_stride, T, s);
+    const size_t per = (size_t)st.nrows * st.Lg * (2 * st.Lg - 1);
+    S2W_CUDA_CHECK(cudaMemsetAsync(F, 0, (size_t)B * per * sizeof(cplx), s));
+    for (int b = 0; b < B; ++b) {
+        int rc = launch_ring_fwd(false, (const cplx *)f + (size_t)b * sig_stride, F + (size_t)b * per, 1, st.Lg, sig_stride, T, s);
+        if (rc) return rc;
+    }
+    return S2W_OK;
+}
+
+static int stage_ring_inv(const s2w_plan *p, const Stage &st, const cplx *F, void *f, size_t sig_stride, int B,
+                          cudaStream_t s)
+{
+    const FftTab &T = p->grids[st.grid].fft;
+    if (st.nrows == 1) return launch_ring_inv(p->real, F, f, B, st.Lg, sig_stride, T, s);
+    const size_t per = (size_t)st.nrows * st.Lg * (2 * st.Lg - 1);
+    for (int b = 0; b < B; ++b) {
+        int rc = launch_ring_inv(false, F + (size_t)b * per, (cplx *)f + (size_t)b * sig_stride, 1, st.Lg, sig_stride, T, s);
+        if (rc) return rc;
+    }
+    return S2W_OK;
+}
+
 // pixels [B][L][2L-1] -> flmT
 static int sht_forward_dev(const s2w_plan *p, const Stage &st, const void *f, size_t sig_stride, int B, const Work &w,
                            bool zero_first, cudaStream_t s)
 {
     const GridTab &g = p->grids[st.grid];
     int rc;
-    if ((rc = launch_ring_fwd(p->real, f, w.F, B, st.Lg, sig_stride, g.fft, s))) return rc;
+    if (st.nn == 0) {  // band-limit <= |spin|: nothing to project onto
+        if (zero_first)
+            S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * (p->real ? p->L : 2 * p->L - 1) * p->L * sizeof(cplx), s));
+        return S2W_OK;
+    }
+    if ((rc = stage_ring_fwd(p, st, f, sig_stride, B, w.F, s))) return rc;
     RwArgs R;
     fill_rw_args(p, st, R);
     if ((rc = g.rw.L ? launch_reweight_th(w.F, w.Ft, R, B, g.rw, s) : launch_reweight(w.F, w.Ft, R, B, g.fft, s))) return rc;
@@ -859,11 +911,18 @@ static int sht_inverse_dev(const s2w_plan *p, const Stage &st, void *f, size_t s
                            cudaStream_t s)
 {
     const GridTab &g = p->grids[st.grid];
+    if (st.nn == 0) {
+        const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
+        for (int b = 0; b < B; ++b)
+            S2W_CUDA_CHECK(cudaMemsetAsync((char *)f + (size_t)b * sig_stride * esz, 0,
+                                           (size_t)st.Lg * (2 * st.Lg - 1) * esz, s));
+        return S2W_OK;
+    }
     WigArgs A;
     fill_wig_args(p, st, false, B, w.flmT, w.F, A);
     int rc;
     if ((rc = launch_wigner_inverse(A, s))) return rc;
-    return launch_ring_inv(p->real, w.F, f, B, st.Lg, sig_stride, g.fft, s);
+    return stage_ring_inv(p, st, w.F, f, sig_stride, B, s);
 }
 
 // a4 + a5 + a8 for one scale: filter x inverse Wigner contraction at L_j, then the (alpha, gamma) DFT.  B signals whose
@@ -1105,6 +1164,7 @@ static int adj_rings_to_harmonic(const s2w_plan *p, const Stage &st, int B, cons
 {
     const int Md = p->real ? st.Lg : 2 * st.Lg - 1;
     int rc;
+    if (st.nn == 0) return S2W_OK;
     if ((rc = launch_transpose(w.F, w.Ft, st.Lg, Md, B * st.nrows, s))) return rc;
     WigArgs A;
     fill_wig_args(p, st, true, B, w.flmT, w.Ft, A);
@@ -1118,6 +1178,10 @@ static int adj_harmonic_to_rings(const s2w_plan *p, const Stage &st, int B, cons
     const GridTab &g = p->grids[st.grid];
     const int Md = p->real ? st.Lg : 2 * st.Lg - 1;
     int rc;
+    if (st.nn == 0) {
+        S2W_CUDA_CHECK(cudaMemsetAsync(w.F, 0, (size_t)B * st.nrows * st.Lg * Md * sizeof(cplx), s));
+        return S2W_OK;
+    }
     WigArgs A;
     fill_wig_args(p, st, false, B, w.flmT, w.F, A);
     A.filt = st.filt_syn_adj;
@@ -1151,14 +1215,13 @@ static int sphere_forward_adjoint(const s2w_plan *p, const void *in, void *out, 
     }
     {
         const int l = ln.pick(0.0);
-        if ((rc = launch_ring_fwd(p->real, y + p->scaling_offset * esz, ln.w[l].F, B, p->Ls, p->coeff_elems,
-                                  p->grids[p->scaling.grid].fft, ln.s[l])))
+        if ((rc = stage_ring_fwd(p, p->scaling, y + p->scaling_offset * esz, p->coeff_elems, B, ln.w[l].F, ln.s[l])))
             return rc;
         if ((rc = adj_rings_to_harmonic(p, p->scaling, B, ln.w[l], ln.s[l]))) return rc;
     }
     if ((rc = lanes_join(p, ln))) return rc;
     if ((rc = adj_harmonic_to_rings(p, p->sht, B, w, s))) return rc;
-    if ((rc = launch_ring_inv(p->real, w.F, out, B, p->L, p->signal_elems, p->grids[p->sht.grid].fft, s))) return rc;
+    if ((rc = stage_ring_inv(p, p->sht, w.F, out, p->signal_elems, B, s))) return rc;
     S2W_CUDA_CHECK(cudaPeekAtLastError());
     return S2W_OK;
 }
@@ -1172,7 +1235,7 @@ static int sphere_inverse_adjoint(const s2w_plan *p, const void *in, void *out, 
     char *y = (char *)out;
     int rc;
     S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * (p->real ? p->L : 2 * p->L - 1) * p->L * sizeof(cplx), s));
-    if ((rc = launch_ring_fwd(p->real, in, w.F, B, p->L, p->signal_elems, p->grids[p->sht.grid].fft, s))) return rc;
+    if ((rc = stage_ring_fwd(p, p->sht, in, p->signal_elems, B, w.F, s))) return rc;
     if ((rc = adj_rings_to_harmonic(p, p->sht, B, w, s))) return rc;
     Lanes ln;  // every block reads the same flmT
     if ((rc = lanes_fork(p, w, w.Ft2 + ((p->ws_F_elems + 15) / 16) * 16, s, true, &ln))) return rc;
@@ -1194,8 +1257,7 @@ static int sphere_inverse_adjoint(const s2w_plan *p, const void *in, void *out, 
     {
         const int l = ln.pick(0.0);
         if ((rc = adj_harmonic_to_rings(p, p->scaling, B, ln.w[l], ln.s[l]))) return rc;
-        if ((rc = launch_ring_inv(p->real, ln.w[l].F, y + p->scaling_offset * esz, B, p->Ls, p->coeff_elems,
-                                  p->grids[p->scaling.grid].fft, ln.s[l])))
+        if ((rc = stage_ring_inv(p, p->scaling, ln.w[l].F, y + p->scaling_offset * esz, p->coeff_elems, B, ln.s[l])))
             return rc;
     }
     if ((rc = lanes_join(p, ln))) return rc;
@@ -1509,6 +1571,12 @@ int s2ball_radial_nodes(double *r, double *q, int P, double tau)
 int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int multiresolution, int flags, int batch,
                       int device)
 {
+    return s2wav_plan_create_spin(out, L, N, lambda, J0, multiresolution, flags, batch, device, 0);
+}
+
+int s2wav_plan_create_spin(s2w_plan **out, int L, int N, double lambda, int J0, int multiresolution, int flags, int batch,
+                           int device, int spin)
+{
     if (!out) {
         set_error("null plan pointer");
         return S2W_EINVAL;
@@ -1516,6 +1584,10 @@ int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int m
     *out = 0;
     int rc = check_params(L, N, lambda, J0);
     if (rc) return rc;
+    if (spin != 0 && ((flags & S2W_REAL) || std::abs(spin) >= L)) {
+        set_error("invalid argument: a spin signal is complex and needs |spin| < L");
+        return S2W_EINVAL;
+    }
     if (batch < 1) {
         set_error("invalid argument: batch < 1");
         return S2W_EINVAL;
@@ -1527,6 +1599,7 @@ int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int m
     S2W_CUDA_CHECK(cudaSetDevice(device));
     s2w_plan *p = new s2w_plan();
     p->kind = 0;
+    p->spin = spin;
     p->capture_stream = 0;
     for (int i = 0; i < S2W_LANES - 1; ++i) {
         p->lane_stream[i] = 0;
@@ -1589,7 +1662,7 @@ int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int m
     size_t off = 0;
     p->scaling_offset = 0;
     off += (size_t)p->Ls * (2 * p->Ls - 1);
-    size_t maxF = (size_t)L * (p->real ? L : 2 * L - 1);
+    size_t maxF = (size_t)(p->spin ? 2 : 1) * L * (p->real ? L : 2 * L - 1);
     for (int j = J0; j <= p->J; ++j) {
         Scale sc;
         memset(&sc, 0, sizeof(sc));
@@ -1634,6 +1707,7 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
     S2W_CUDA_CHECK(cudaSetDevice(device));
     s2w_plan *p = new s2w_plan();
     p->kind = 1;
+    p->spin = 0;
     p->capture_stream = 0;
     for (int i = 0; i < S2W_LANES - 1; ++i) {
         p->lane_stream[i] = 0;
