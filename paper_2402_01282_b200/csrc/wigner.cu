@@ -432,18 +432,22 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
             gs[r] = g < G ? gsrow[g] : INT_MAX;
             d[r] = 0.0;
             u[r] = 0.0;
+            // branch-free, so that the 8 ring indices and then the 8 values are loaded together (one latency each,
+            // not one per value): invalid rings / columns read element 0 of a valid column and are zeroed afterwards
+            const int row = fci.minus ? A.n_rowm[q] : A.n_row[q];
+            const int mi = A.isReal ? m : (fci.minus ? Lg - 1 - m : Lg - 1 + m);
+            const double *hcol = reinterpret_cast<const double *>(
+                                     Fsrc + (((size_t)(fci.valid ? fci.b : 0) * A.nrows + row) * Md + mi) * Lg) + (fc & 1);
+            const int *ringp = A.ring + (g < G ? g : 0) * 32 + fk;
+            int tq[8];
+#pragma unroll
+            for (int qd = 0; qd < 8; ++qd) tq[qd] = ringp[qd * 4];
+            const double keep = fci.valid ? (fci.minus ? sgn : 1.0) : 0.0;
 #pragma unroll
             for (int qd = 0; qd < 8; ++qd) {
-                double v = 0.0;
-                const int t = g < G ? A.ring[g * 32 + qd * 4 + fk] : -1;
-                if (t >= 0 && fci.valid) {
-                    const int row = fci.minus ? A.n_rowm[q] : A.n_row[q];
-                    const int mi = A.isReal ? m : (fci.minus ? Lg - 1 - m : Lg - 1 + m);
-                    const cplx hv = Fsrc[(((size_t)fci.b * A.nrows + row) * Md + mi) * Lg + t];
-                    v = (fc & 1) ? hv.y : hv.x;
-                    if (fci.minus) v *= sgn;
-                }
-                hA[r][qd] = v;
+                const bool ok = g < G && tq[qd] >= 0;
+                const double v = hcol[2 * (size_t)(ok ? tq[qd] : 0)];
+                hA[r][qd] = ok ? v * keep : 0.0;
             }
         }
         // tiles start at the first group start; tiles wholly below the filter support run the recursion only
