@@ -212,9 +212,9 @@ __device__ __forceinline__ void dif_pass_b(cplx *buf, int M, int logS, const Fft
     const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
     const int s = 1 << logs;
     const int twm = T.twmul << (T.logM - logS);
-    const int per = M / R;
+    const int lper = T.logM - (R == 8 ? 3 : (R == 4 ? 2 : 1)), per = 1 << lper;  // M is a power of two
     for (int it = threadIdx.x; it < nb * per; it += blockDim.x) {
-        const int bi = it / per, idx = it - bi * per;
+        const int bi = it >> lper, idx = it & (per - 1);
         cplx *b = buf + bi * bstride;
         int i = idx & (s - 1);
         int base = ((idx >> logs) << logS) + i;
@@ -237,9 +237,9 @@ __device__ __forceinline__ void dit_pass_b(cplx *buf, int M, int logS, const Fft
     const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
     const int s = 1 << logs;
     const int twm = T.twmul << (T.logM - logS);
-    const int per = M / R;
+    const int lper = T.logM - (R == 8 ? 3 : (R == 4 ? 2 : 1)), per = 1 << lper;  // M is a power of two
     for (int it = threadIdx.x; it < nb * per; it += blockDim.x) {
-        const int bi = it / per, idx = it - bi * per;
+        const int bi = it >> lper, idx = it & (per - 1);
         cplx *b = buf + bi * bstride;
         int i = idx & (s - 1);
         int base = ((idx >> logs) << logS) + i;
@@ -298,9 +298,9 @@ __device__ inline void fft_dit_full_b(cplx *buf, const FftTab &T, const cplx *st
 template <int R>
 __device__ __forceinline__ void mid_pass_b(cplx *buf, int M, const cplx *__restrict__ khat, int nb, int bstride)
 {
-    const int per = M / R;
+    const int lper = __ffs(M) - 1 - (R == 8 ? 3 : (R == 4 ? 2 : 1)), per = 1 << lper;  // M is a power of two
     for (int it = threadIdx.x; it < nb * per; it += blockDim.x) {
-        const int bi = it / per, g = it - bi * per;
+        const int bi = it >> lper, g = it & (per - 1);
         cplx *b = buf + bi * bstride;
         cplx v[R];
 #pragma unroll

@@ -1013,6 +1013,7 @@ __global__ void __launch_bounds__(256) reweight_kernel(const cplx *__restrict__ 
 // accurate (2e-16 at L = 1024).  One block per column; both sequences go through each FFT pass together.
 // ---------------------------------------------------------------------------------------------------------------
 #define RW_MAXPT 8  // ring values a thread keeps in registers (L <= 8 * blockDim)
+template <int PT>  // ring values a thread keeps in registers: L <= PT * blockDim
 __global__ void __launch_bounds__(256, 3) reweight_th_kernel(const cplx *__restrict__ F, cplx *__restrict__ Ft, RwArgs A,
                                                             RwTab R)
 {
@@ -1034,10 +1035,10 @@ __global__ void __launch_bounds__(256, 3) reweight_th_kernel(const cplx *__restr
     cplx *colT = Ft + (((size_t)b * A.nrows + A.n_row[q]) * A.Md + mi) * (size_t)L;  // [b][row][mi][t]: t contiguous
     const double *rp = R.rpole + par * L, *vp = R.vpole + par * L;
 
-    cplx xs[RW_MAXPT];
+    cplx xs[PT];
     cplx dot = cmake(0.0, 0.0);
 #pragma unroll
-    for (int k = 0; k < RW_MAXPT; ++k) {
+    for (int k = 0; k < PT; ++k) {
         const int t = threadIdx.x + k * blockDim.x;
         cplx x = cmake(0.0, 0.0);
         if (t < L) {
@@ -1055,7 +1056,7 @@ __global__ void __launch_bounds__(256, 3) reweight_th_kernel(const cplx *__restr
     }
     __syncthreads();
 #pragma unroll
-    for (int k = 0; k < RW_MAXPT; ++k) {
+    for (int k = 0; k < PT; ++k) {
         const int t = threadIdx.x + k * blockDim.x;
         if (t < Lm) {
             const cplx u1 = (t & 1) ? cscale(xs[k], -1.0) : xs[k];
@@ -1090,7 +1091,7 @@ __global__ void __launch_bounds__(256, 3) reweight_th_kernel(const cplx *__restr
     fft_dit_full_b(buf, T, s_tw, 2, bstride);
     const cplx xpole = s_pole[0];
 #pragma unroll
-    for (int k = 0; k < RW_MAXPT; ++k) {
+    for (int k = 0; k < PT; ++k) {
         const int t = threadIdx.x + k * blockDim.x;
         if (t < Lm) {
             const cplx y1 = b1[S2W_PAD(t)], y2 = b2[S2W_PAD(t)];
@@ -1514,9 +1515,14 @@ int launch_reweight_th(const cplx *F, cplx *Ft, const RwArgs &A, int batch, cons
                      ncol);
         return S2W_OK;
     }
-    if ((rc = set_smem(reweight_th_kernel, sm))) return rc;
     dim3 grid(A.Md, A.nn, batch);
-    S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight_th_kernel, grid, 256, sm, st, F, Ft, A, R);
+    if (R.L <= 4 * 256) {  // four values per thread: no spills under the 80-register cap of three blocks per SM
+        if ((rc = set_smem(reweight_th_kernel<4>, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight_th_kernel<4>, grid, 256, sm, st, F, Ft, A, R);
+        return S2W_OK;
+    }
+    if ((rc = set_smem(reweight_th_kernel<RW_MAXPT>, sm))) return rc;
+    S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight_th_kernel<RW_MAXPT>, grid, 256, sm, st, F, Ft, A, R);
     return S2W_OK;
 }
 
