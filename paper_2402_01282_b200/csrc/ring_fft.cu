@@ -175,18 +175,25 @@ __device__ __forceinline__ void so3_inv_few(const cplx *__restrict__ F, void *__
         if (REAL && nv < 0) continue;
         const cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * Md;   // row of n
         const cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * Md;  // row of -n
-        for (int k = tl; k < M; k += tpr) {
-            cplx v = cmake(0.0, 0.0);
-            if (k < n && has) {
-                if (REAL) {
-                    v = k < L ? Fp[k] : cconj(Fm[n - k]);
-                } else {
-                    int m = k < L ? k : k - n;
-                    v = Fp[m + L - 1];
-                }
-                v = cmulc(v, __ldg(&T.chirp[k]));
+        for (int k0 = tl; k0 < M; k0 += 4 * tpr) {  // four elements at a time, loads first
+            cplx x[4], c[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int k = k0 + j * tpr;
+                const int kk = (k < n && has) ? k : 0;
+                if (REAL)
+                    x[j] = *(kk < L ? Fp + kk : Fm + (n - kk));
+                else
+                    x[j] = Fp[(kk < L ? kk : kk - n) + L - 1];
+                c[j] = __ldg(&T.chirp[kk]);
             }
-            buf[S2W_PAD(k)] = v;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int k = k0 + j * tpr;
+                if (k >= M) continue;
+                const cplx v = (REAL && k >= L) ? cconj(x[j]) : x[j];
+                buf[S2W_PAD(k)] = (k < n && has) ? cmulc(v, c[j]) : cmake(0.0, 0.0);
+            }
         }
         __syncthreads();
         if (MULTI)
@@ -551,6 +558,31 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
 // ring t0+1 in the imaginary part), as in a1; the rows n > 0 are done ring by ring.  5 instead of 6 convolutions per
 // ring pair at N = 5.
 // ---------------------------------------------------------------------------------------------------------------
+// Fill of one Bluestein buffer from a half-stored Hermitian row pair: buf[k] = conj(chirp[k]) x, x = Fp[k] for k < L,
+// conj(Fm[n-k]) for L <= k < n, 0 for k >= n.  Four elements per thread at a time, loads first (one unconditional
+// load each through a selected pointer), so that a thread waits for global memory once per four elements.
+__device__ __forceinline__ void fill_row_pm(cplx *buf, const cplx *__restrict__ Fp, const cplx *__restrict__ Fm,
+                                            const cplx *__restrict__ chirp, int n, int L, int M)
+{
+    for (int k0 = threadIdx.x; k0 < M; k0 += 4 * blockDim.x) {
+        cplx x[4], c[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int k = k0 + j * blockDim.x;
+            const int kk = k < n ? k : 0;
+            x[j] = *(kk < L ? Fp + kk : Fm + (n - kk));
+            c[j] = __ldg(&chirp[kk]);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int k = k0 + j * blockDim.x;
+            if (k >= M) continue;
+            cplx v = k >= L ? cconj(x[j]) : x[j];
+            buf[S2W_PAD(k)] = k < n ? cmulc(v, c[j]) : cmake(0.0, 0.0);
+        }
+    }
+}
+
 // The same for at most 9 gamma samples (N <= 5), without read-modify-write of the gamma planes: the rows are done
 // ring by ring, the transforms V_n(alpha) of all rows but the last are parked in the ring's own output planes (V_0 in
 // plane 0, row i in planes 2i+1, 2i+2: at most 2N-3 of the 2N-1 planes), and the pass of the last row reads them back
@@ -576,19 +608,28 @@ __device__ __forceinline__ void so3_inv_pair_few(const cplx *__restrict__ F, dou
         }
     }
     if (q0 >= 0) {
-        const cplx *X0 = Fb + ((size_t)A.n_row[q0] * L + t0) * L, *X1 = X0 + L;
-        for (int k = threadIdx.x; k < M; k += blockDim.x) {
-            cplx v = cmake(0.0, 0.0);
-            if (k < n) {
-                const int m = k < L ? k : n - k;
-                cplx a = X0[m], c = has1 ? X1[m] : cmake(0.0, 0.0);
+        const cplx *X0 = Fb + ((size_t)A.n_row[q0] * L + t0) * L, *X1 = has1 ? X0 + L : X0;
+        for (int k0 = threadIdx.x; k0 < M; k0 += 4 * blockDim.x) {  // four elements at a time, loads first
+            cplx xa[4], xc[4], ch[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int k = k0 + j * blockDim.x;
+                const int kk = k < n ? k : 0, m = kk < L ? kk : n - kk;
+                xa[j] = X0[m];
+                xc[j] = X1[m];
+                ch[j] = __ldg(&T.chirp[kk]);
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int k = k0 + j * blockDim.x;
+                if (k >= M) continue;
+                cplx a = xa[j], c = has1 ? xc[j] : cmake(0.0, 0.0);
                 if (k >= L) {
                     a = cconj(a);
                     c = cconj(c);
                 }
-                v = cmulc(cmake(a.x - c.y, a.y + c.x), __ldg(&T.chirp[k]));
+                buf[S2W_PAD(k)] = k < n ? cmulc(cmake(a.x - c.y, a.y + c.x), ch[j]) : cmake(0.0, 0.0);
             }
-            buf[S2W_PAD(k)] = v;
         }
         __syncthreads();
         fft_convolve(buf, T, s_tw, T.bhat_p);
@@ -609,11 +650,7 @@ __device__ __forceinline__ void so3_inv_pair_few(const cplx *__restrict__ F, dou
             if (A.n_val[q] <= 0) continue;
             const cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * L;
             const cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * L;
-            for (int k = threadIdx.x; k < M; k += blockDim.x) {
-                cplx v = cmake(0.0, 0.0);
-                if (k < n) v = cmulc(k < L ? Fp[k] : cconj(Fm[n - k]), __ldg(&T.chirp[k]));
-                buf[S2W_PAD(k)] = v;
-            }
+            fill_row_pm(buf, Fp, Fm, T.chirp, n, L, M);
             __syncthreads();
             fft_convolve(buf, T, s_tw, T.bhat_p);
             if (i + 1 < np) {
@@ -776,30 +813,36 @@ __device__ __forceinline__ void so3_fwd_pair_few(const double *__restrict__ W, c
         }
     }
     __syncthreads();
-    // gather pass: every gamma plane of both rings once
-    for (int r = 0; r < 2; ++r) {
-        const int t = t0 + r;
-        const bool live = r == 0 || has1;
-        for (int a = threadIdx.x; a < M; a += blockDim.x) {
-            if (a >= n) {
-                if (r == 0) buf[S2W_PAD(a)] = cmake(0.0, 0.0);
-                continue;
-            }
-            const cplx ch = __ldg(&T.chirp[a]);
-            double wv[9];
+    // gather pass: every gamma plane of both rings once, the 2 x 9 loads of an alpha sample issued together
+    const double *W0 = Wb + (size_t)t0 * n, *W1 = Wb + (size_t)(has1 ? t0 + 1 : t0) * n;
+    for (int a = threadIdx.x; a < M; a += blockDim.x) {
+        if (a >= n) {
+            buf[S2W_PAD(a)] = cmake(0.0, 0.0);
+            continue;
+        }
+        const cplx ch = __ldg(&T.chirp[a]);
+        double wv[2][9];
 #pragma unroll
-            for (int g = 0; g < 9; ++g) wv[g] = (live && g < ng) ? Wb[(size_t)t * n + a + g * plane] : 0.0;
-            double y0 = 0.0;
+        for (int g = 0; g < 9; ++g) {
+            const size_t o = a + (size_t)(g < ng ? g : 0) * plane;
+            wv[0][g] = W0[o];
+            wv[1][g] = W1[o];
+        }
 #pragma unroll
-            for (int g = 0; g < 9; ++g) y0 += wv[g];
-            if (r == 0) {
-                buf[S2W_PAD(a)] = cmake(y0, 0.0);
-            } else {
-                cplx v = buf[S2W_PAD(a)];
-                v.y = y0;
-                buf[S2W_PAD(a)] = cmul(cscale(v, inv_ng), ch);
-            }
-            if (!live) continue;
+        for (int g = 0; g < 9; ++g) {
+            if (g >= ng) wv[0][g] = 0.0;
+            if (g >= ng || !has1) wv[1][g] = 0.0;
+        }
+        double y0 = 0.0, y1 = 0.0;
+#pragma unroll
+        for (int g = 0; g < 9; ++g) {
+            y0 += wv[0][g];
+            y1 += wv[1][g];
+        }
+        buf[S2W_PAD(a)] = cmul(cscale(cmake(y0, y1), inv_ng), ch);
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            if (r == 1 && !has1) continue;
 #pragma unroll
             for (int i = 0; i < 4; ++i)
                 if (i < np) {
@@ -807,12 +850,12 @@ __device__ __forceinline__ void so3_fwd_pair_few(const double *__restrict__ W, c
 #pragma unroll
                     for (int g = 0; g < 9; ++g) {
                         const cplx ph = gph[i * ng + (g < ng ? g : 0)];
-                        y.x = fma(ph.x, wv[g], y.x);
-                        y.y = fma(ph.y, wv[g], y.y);
+                        y.x = fma(ph.x, wv[r][g], y.x);
+                        y.y = fma(ph.y, wv[r][g], y.y);
                     }
                     y = cmul(cscale(y, inv_ng), ch);
-                    cplx *dst = a < L ? Fb + ((size_t)s_rowp[i] * L + t) * L + a
-                                      : Fb + ((size_t)s_rowm[i] * L + t) * L + (a - L);
+                    cplx *dst = a < L ? Fb + ((size_t)s_rowp[i] * L + t0 + r) * L + a
+                                      : Fb + ((size_t)s_rowm[i] * L + t0 + r) * L + (a - L);
                     *dst = y;
                 }
         }
@@ -836,8 +879,20 @@ __device__ __forceinline__ void so3_fwd_pair_few(const double *__restrict__ W, c
         for (int i = 0; i < np; ++i) {
             cplx *Fp = Fb + ((size_t)s_rowp[i] * L + t) * L;
             cplx *Fm = Fb + ((size_t)s_rowm[i] * L + t) * L;
-            for (int a = threadIdx.x; a < M; a += blockDim.x)
-                buf[S2W_PAD(a)] = a < L ? Fp[a] : (a < n ? Fm[a - L] : cmake(0.0, 0.0));
+            for (int a0 = threadIdx.x; a0 < M; a0 += 4 * blockDim.x) {  // four at a time, loads first
+                cplx x[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int a = a0 + j * blockDim.x;
+                    const int aa = a < n ? a : 0;
+                    x[j] = *(aa < L ? Fp + aa : Fm + (aa - L));
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int a = a0 + j * blockDim.x;
+                    if (a < M) buf[S2W_PAD(a)] = a < n ? x[j] : cmake(0.0, 0.0);
+                }
+            }
             __syncthreads();
             fft_convolve(buf, T, s_tw, T.bhat_m);
             for (int m = threadIdx.x; m < L; m += blockDim.x) {
