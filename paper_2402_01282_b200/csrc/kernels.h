@@ -88,6 +88,9 @@ int launch_fft_forward(cplx *data, const FftTab &T, cudaStream_t st);   // plan-
 int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int G,
                         const int *n_vals, int ntab, const double *yv, const int *ring, int *gstart, double2 *dseed,
                         cudaStream_t st);
+int launch_wigner_seed_floor(const double *coef, size_t tri, int Lfull, int Lg, int G, int ntab, const double *yv,
+                             const int *gstart, const double2 *dseed, int lfloor, int *gstart_f, double2 *dseed_f,
+                             cudaStream_t st);
 int launch_wigner_table(const double *coef, size_t tri, int Lfull, int Lg, int G, const int *n_vals, int ntab,
                         const double *yv, const int *gstart, const double2 *dseed, double *dtab, size_t tri_g,
                         cudaStream_t st);

@@ -120,6 +120,10 @@ struct Stage {  // one Wigner contraction launch: rows, filters
     // or phi samples per ring, the factor between the unnormalised inverse DFT and the adjoint of the normalised one
     cplx *filt_ana_adj;
     cplx *filt_syn_adj;
+    // start degrees and seeds of the recursion advanced to lmin (0: the grid's own tables): a stage whose filter
+    // support begins at lmin does not re-run the recursion from each group's start up to lmin at every transform
+    int *gstart_f;
+    double2 *dseed_f;
 };
 
 struct Scale {
@@ -607,8 +611,8 @@ void fill_wig_args(const s2w_plan *p, const Stage &st, bool synthesis, int B, cp
     A.tri = p->tri;
     A.coef = p->coef;
     A.G = g.G;
-    A.gstart = g.gstart;
-    A.dseed = g.dseed;
+    A.gstart = st.gstart_f ? st.gstart_f : g.gstart;
+    A.dseed = st.dseed_f ? st.dseed_f : g.dseed;
     A.yv = g.yv;
     A.ring = g.ring;
     A.dtab = g.dtab;
@@ -759,6 +763,15 @@ int make_scale_stage(s2w_plan *p, Scale &sc, const double *kj, const std::vector
             }
         }
     if ((rc = fill_stage_rows(p, st, ns, rows, N))) return rc;
+    if (st.nn > 0 && st.lmin > 0 && !(p->flags & S2W_PRECOMPUTE)) {
+        const GridTab &g = p->grids[st.grid];
+        const size_t ntab = p->tabn.size();
+        if ((rc = p->pool.alloc(&st.gstart_f, ntab * sc.Lj * g.G))) return rc;
+        if ((rc = p->pool.alloc(&st.dseed_f, ntab * sc.Lj * (size_t)32 * g.G))) return rc;
+        if ((rc = launch_wigner_seed_floor(p->coef, p->tri, p->L, sc.Lj, g.G, (int)ntab, g.yv, g.gstart, g.dseed, st.lmin,
+                                           st.gstart_f, st.dseed_f, 0)))
+            return rc;
+    }
     std::vector<cplx> fa((size_t)st.nn * sc.Lj), fs((size_t)st.nn * sc.Lj);
     const double syn_norm = 4.0 * pi * pi / (2.0 * sc.Lj - 1.0);
     for (int q = 0; q < st.nn; ++q)

@@ -113,6 +113,38 @@ __global__ void __launch_bounds__(32) wigner_seed_kernel(const double *__restric
     }
 }
 
+// plan-time: start degrees and seeds of a stage whose filter support begins at lfloor > 0.  The recursion of a group
+// that would start below lfloor has nothing to contribute there, so it is run once, here, from the group start to
+// lfloor (the same steps the transform kernels would take) and the state is stored as that stage's seed.
+__global__ void __launch_bounds__(32) wigner_seed_floor_kernel(const double *__restrict__ coef, size_t tri, int Lfull, int Lg,
+                                                              int G, const double *__restrict__ yv,
+                                                              const int *__restrict__ gstart,
+                                                              const double2 *__restrict__ dseed, int lfloor,
+                                                              int *__restrict__ gstart_f, double2 *__restrict__ dseed_f)
+{
+    const int g = blockIdx.x, m = blockIdx.y, tab = blockIdx.z, lane = threadIdx.x;
+    const int k = g * 32 + lane;
+    const size_t gidx = ((size_t)tab * Lg + m) * G + g;
+    const size_t sidx = ((size_t)tab * Lg + m) * (size_t)(32 * G) + k;
+    const int gs = gstart[gidx];
+    int target = gs;
+    if (gs < Lg && gs < lfloor) target = lfloor < Lg ? lfloor : Lg;
+    double2 s = dseed[sidx];
+    if (target > gs) {
+        const double *c = coef + ((size_t)tab * tri + tri_off(m, Lfull)) * 4;
+        const double y = yv[k];
+        const bool south = (g & 1) != 0;
+        double d = s.x, u = s.y;
+        for (int l = gs; l < target; ++l) {
+            const double4 q = *reinterpret_cast<const double4 *>(c + 4 * (size_t)l);
+            wig_step(d, u, y, q.x, q.y, south ? q.w : q.z);
+        }
+        s = make_double2(d, u);
+    }
+    dseed_f[sidx] = s;
+    if (lane == 0) gstart_f[gidx] = target;
+}
+
 __global__ void wigner_start_fix_kernel(int *__restrict__ gstart, int G, int count)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -907,6 +939,16 @@ int launch_wigner_seeds(const double *mant, const int *expo, const double *coef,
     const int count = Lg * ntab;
     S2W_LAUNCH(wigner_start_fix_kernel, (count + 127) / 128, 128, 0, st, gstart, G, count);
     S2W_LAUNCH(wigner_seed_kernel, grid, 32, 0, st, mant, expo, coef, tri, Lfull, Lg, G, nl, yv, ring, gstart, dseed, 1);
+    return S2W_OK;
+}
+
+int launch_wigner_seed_floor(const double *coef, size_t tri, int Lfull, int Lg, int G, int ntab, const double *yv,
+                             const int *gstart, const double2 *dseed, int lfloor, int *gstart_f, double2 *dseed_f,
+                             cudaStream_t st)
+{
+    dim3 grid(G, Lg, ntab);
+    S2W_LAUNCH(wigner_seed_floor_kernel, grid, 32, 0, st, coef, tri, Lfull, Lg, G, yv, gstart, dseed, lfloor, gstart_f,
+               dseed_f);
     return S2W_OK;
 }
 
