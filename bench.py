@@ -31,6 +31,10 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "fp64 wavelet fwd+inv transforms/sec"
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel class, summed over the launches of ONE step (like
+# `achieved`, which is flops per step / ms per step), from the `ncu --set full` captures of profiles/r01j_wigner_ncu.md
+# (C3, on-the-fly): (workload, on-the-fly?, class) -> bytes per step.  Other workloads have no capture: traffic = null.
+NCU_TRAFFIC = {("C3", "wigner_forward"): 1.299e9 + 0.070e9, ("C3", "wigner_inverse"): 0.519e9 + 0.679e9}
 UNIT = "transforms/s"
 
 
@@ -413,7 +417,9 @@ def run_ours(args, cfg):
         probe = {"error": str(e)}
     total_kms = sum(v[0] for v in classes.values())
     roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak if peak else None, "traffic": None,
+                "frac": achieved / peak if peak else None,
+                "traffic": NCU_TRAFFIC.get((cfg["name"], dom)) if not (args.precompute or adj) else None,
+                "traffic_unit": "bytes per step (all launches of the class), ncu --set full, profiles/r01j_wigner_ncu.md",
                 "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x sm_max_mhz (DESIGN.md); "
                                "measured DFMA-chain probe beside it",
                 "probe": probe, "tuples_per_step": tup, "flops_per_step": flops,

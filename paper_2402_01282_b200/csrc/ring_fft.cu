@@ -1073,11 +1073,21 @@ __global__ void __launch_bounds__(256, 3) reweight_th_kernel(const cplx *__restr
                                                             RwTab R)
 {
     extern __shared__ cplx buf[];
-    __shared__ cplx s_tw[S2W_TW_SMEM];
-    tw_stage(s_tw, R.fft);
+    // twiddles: a two-level split of W_M^k on the transform's own length (k = 32 hi + lo, M / 32 + 32 entries) instead
+    // of the plan-wide table's split (up to 192 entries): the 1.5 KB are what lets a third block fit on an SM at L = 1024
+    constexpr int TWN = 64 * (PT / 4) + 32;
+    __shared__ cplx s_tw[TWN];
     __shared__ cplx s_part[8];
     __shared__ cplx s_pole[2];
-    const FftTab &T = R.fft;
+    FftTab T = R.fft;
+    {
+        const int nh = T.M >> 5;
+        for (int i = threadIdx.x; i < nh; i += blockDim.x) s_tw[i] = R.fft.tw[(i << 5) * R.fft.twmul];
+        if (threadIdx.x < 32) s_tw[nh + threadIdx.x] = R.fft.tw[threadIdx.x * R.fft.twmul];
+        T.twmul = 1;
+        T.twmask = T.M - 1;
+        T.twlo = 5;
+    }
     const int L = R.L, Lm = L - 1, M = T.M;
     const int bstride = fft_padded_len(M);
     cplx *b1 = buf, *b2 = buf + bstride;
@@ -1085,6 +1095,12 @@ __global__ void __launch_bounds__(256, 3) reweight_th_kernel(const cplx *__restr
     const int m = A.isReal ? mi : mi - (L - 1);
     const int nv = A.n_val[q];
     const int par = ((m + nv) & 1) ? 1 : 0;  // 0: sigma = +1, 1: sigma = -1
+    // M = 512 PT (always, see launch_reweight_th): the outermost radix-8 pass of both transforms has stride
+    // M / 8 = NI * 256, so its butterflies touch exactly the rings t = threadIdx.x + 256 j this thread holds in xs[]
+    // (inputs 4..7 are the zero padding) -- the first forward pass runs straight from the registers, the last inverse
+    // pass feeds the epilogue from them: no zero fill, and 2 writes + 2 reads of the buffers less per column
+    constexpr int NI = PT / 4;
+    const bool fused = M == 512 * PT && blockDim.x == 256;
     const double sigma = par ? -1.0 : 1.0;
     const cplx *col = F + ((size_t)b * A.nrows + A.n_row[q]) * (size_t)L * A.Md + mi;
     cplx *colT = Ft + (((size_t)b * A.nrows + A.n_row[q]) * A.Md + mi) * (size_t)L;  // [b][row][mi][t]: t contiguous
@@ -1105,18 +1121,20 @@ __global__ void __launch_bounds__(256, 3) reweight_th_kernel(const cplx *__restr
         xs[k] = x;
         if (t == Lm) s_pole[0] = x;
     }
-    for (int t = threadIdx.x; t < M; t += blockDim.x) {  // zero padding (and the slots filled below)
-        b1[S2W_PAD(t)] = cmake(0.0, 0.0);
-        b2[S2W_PAD(t)] = cmake(0.0, 0.0);
-    }
-    __syncthreads();
+    if (!fused) {
+        for (int t = threadIdx.x; t < M; t += blockDim.x) {  // zero padding (and the slots filled below)
+            b1[S2W_PAD(t)] = cmake(0.0, 0.0);
+            b2[S2W_PAD(t)] = cmake(0.0, 0.0);
+        }
+        __syncthreads();
 #pragma unroll
-    for (int k = 0; k < PT; ++k) {
-        const int t = threadIdx.x + k * blockDim.x;
-        if (t < Lm) {
-            const cplx u1 = (t & 1) ? cscale(xs[k], -1.0) : xs[k];
-            b1[S2W_PAD(t)] = u1;
-            b2[S2W_PAD(t)] = cscale(u1, R.delta[t]);
+        for (int k = 0; k < PT; ++k) {
+            const int t = threadIdx.x + k * blockDim.x;
+            if (t < Lm) {
+                const cplx u1 = (t & 1) ? cscale(xs[k], -1.0) : xs[k];
+                b1[S2W_PAD(t)] = u1;
+                b2[S2W_PAD(t)] = cscale(u1, R.delta[t]);
+            }
         }
     }
     // pole-ring dot product: warp shuffle, then across warps
@@ -1127,7 +1145,51 @@ __global__ void __launch_bounds__(256, 3) reweight_th_kernel(const cplx *__restr
     }
     if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = dot;
     __syncthreads();
-    fft_dif_full_b(buf, T, s_tw, 2, bstride);
+    if (fused) {
+        const int per = M >> 3;
+#pragma unroll
+        for (int c = 0; c < NI; ++c) {
+            const int idx = threadIdx.x + c * 256;
+            cplx w[8];
+            twiddle_powers<8>(tw_lookup(s_tw, T, idx), w);
+#pragma unroll
+            for (int sq = 0; sq < 2; ++sq) {
+                cplx v[8];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const int t = idx + k * per;  // = threadIdx.x + 256 (c + k NI)
+                    cplx u = cmake(0.0, 0.0);
+                    if (t < Lm) {
+                        u = (t & 1) ? cscale(xs[c + k * NI], -1.0) : xs[c + k * NI];
+                        if (sq) u = cscale(u, R.delta[t]);
+                    }
+                    v[k] = u;
+                }
+#pragma unroll
+                for (int k = 4; k < 8; ++k) v[k] = cmake(0.0, 0.0);
+                Bfly<8, false>::run(v);
+#pragma unroll
+                for (int j = 1; j < 8; ++j) v[j] = cmul(v[j], w[j]);
+                cplx *bq = buf + sq * bstride;
+#pragma unroll
+                for (int k = 0; k < 8; ++k) bq[S2W_PAD(idx + k * per)] = v[k];
+            }
+        }
+        __syncthreads();
+        for (int logS = T.logM - 3; logS >= 3; logS -= 3) {
+            dif_pass_b<8>(buf, M, logS, T, s_tw, 2, bstride);
+            __syncthreads();
+        }
+        if (T.logM % 3 == 2) {
+            dif_pass_b<4>(buf, M, 2, T, s_tw, 2, bstride);
+            __syncthreads();
+        } else if (T.logM % 3 == 1) {
+            dif_pass_b<2>(buf, M, 1, T, s_tw, 2, bstride);
+            __syncthreads();
+        }
+    } else {
+        fft_dif_full_b(buf, T, s_tw, 2, bstride);
+    }
     // spectra of T u -/+ sigma H u: Y(k) = That(k) U(k) -/+ sigma Ghat(k) U(-k)
     for (int i = threadIdx.x; i < R.npairs; i += blockDim.x) {
         const int2 pp = __ldg(&R.pairs[i]);
@@ -1143,8 +1205,63 @@ __global__ void __launch_bounds__(256, 3) reweight_th_kernel(const cplx *__restr
         }
     }
     __syncthreads();
-    fft_dit_full_b(buf, T, s_tw, 2, bstride);
     const cplx xpole = s_pole[0];
+    if (fused) {
+        if (T.logM % 3 == 2) {
+            dit_pass_b<4>(buf, M, 2, T, s_tw, 2, bstride);
+            __syncthreads();
+        } else if (T.logM % 3 == 1) {
+            dit_pass_b<2>(buf, M, 1, T, s_tw, 2, bstride);
+            __syncthreads();
+        }
+        for (int logS = T.logM % 3 + 3; logS < T.logM; logS += 3) {
+            dit_pass_b<8>(buf, M, logS, T, s_tw, 2, bstride);
+            __syncthreads();
+        }
+        const int per = M >> 3;
+#pragma unroll
+        for (int c = 0; c < NI; ++c) {
+            const int idx = threadIdx.x + c * 256;
+            cplx w[8];
+            twiddle_powers<8>(tw_lookup(s_tw, T, idx), w);
+            cplx y1[4];
+            {
+                cplx v[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) v[k] = b1[S2W_PAD(idx + k * per)];
+#pragma unroll
+                for (int j = 1; j < 8; ++j) v[j] = cmulc(v[j], w[j]);
+                Bfly<8, true>::run(v);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) y1[k] = v[k];
+            }
+            cplx v[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] = b2[S2W_PAD(idx + k * per)];
+#pragma unroll
+            for (int j = 1; j < 8; ++j) v[j] = cmulc(v[j], w[j]);
+            Bfly<8, true>::run(v);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int t = idx + k * per;
+                const cplx x = xs[c + k * NI];
+                if (t < Lm) {
+                    const double dl = R.delta[t], ds = R.dsum[t], vv = vp[t];
+                    cplx h = cmake(fma(dl, y1[k].x, -v[k].x), fma(dl, y1[k].y, -v[k].y));
+                    if (t & 1) h = cscale(h, -1.0);
+                    h.x += fma(ds, x.x, vv * xpole.x);
+                    h.y += fma(ds, x.y, vv * xpole.y);
+                    colT[t] = h;
+                } else if (t == Lm) {
+                    cplx acc = cmake(0.0, 0.0);
+                    for (int wi = 0; wi < (int)(blockDim.x >> 5); ++wi) acc = cadd(acc, s_part[wi]);
+                    colT[t] = acc;
+                }
+            }
+        }
+        return;
+    }
+    fft_dit_full_b(buf, T, s_tw, 2, bstride);
 #pragma unroll
     for (int k = 0; k < PT; ++k) {
         const int t = threadIdx.x + k * blockDim.x;
