@@ -141,8 +141,27 @@ __device__ __forceinline__ cplx tw_lookup(const cplx *stw, const FftTab &T, int 
     return cmul(stw[k >> T.twlo], stw[nh + (k & ((1 << T.twlo) - 1))]);
 }
 
+// The same split on the transform's own length M (W_M^k = W^{hi << tl} W^{lo}, tl = ceil(logM / 2)) instead of the
+// plan-wide table's: 2 sqrt(M) entries (2 KB at M = 4096), which is what lets a third block of the one-sequence-per-
+// block kernels fit on an SM.  T is the caller's local copy and is rewritten to index the staged table.
+__host__ __device__ inline int tw_own_entries(int logM)
+{
+    const int tl = (logM + 1) >> 1;
+    return (1 << (logM - tl)) + (1 << tl);
+}
+__device__ __forceinline__ void tw_stage_own(cplx *stw, FftTab &T)
+{
+    const int tl = (T.logM + 1) >> 1, nh = T.M >> tl, nl = 1 << tl;
+    for (int i = threadIdx.x; i < nh; i += blockDim.x) stw[i] = T.tw[(i << tl) * T.twmul];
+    for (int i = threadIdx.x; i < nl; i += blockDim.x) stw[nh + i] = T.tw[i * T.twmul];
+    T.twmul = 1;
+    T.twmask = T.M - 1;
+    T.twlo = tl;
+}
+
 // One decimation-in-frequency pass on sub-transforms of size S (radix R): butterflies, then twiddles W_S^{i j}.
-template <int R>
+// HALF (outermost radix-8 pass only, S = M): the upper half of the buffer is taken as zero without being read.
+template <int R, bool HALF = false>
 __device__ __forceinline__ void dif_pass(cplx *buf, int M, int logS, const FftTab &T, const cplx *stw)
 {
     const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
@@ -153,7 +172,7 @@ __device__ __forceinline__ void dif_pass(cplx *buf, int M, int logS, const FftTa
         int base = ((idx >> logs) << logS) + i;
         cplx v[R];
 #pragma unroll
-        for (int k = 0; k < R; ++k) v[k] = buf[S2W_PAD(base + (k << logs))];
+        for (int k = 0; k < R; ++k) v[k] = (HALF && 2 * k >= R) ? cmake(0.0, 0.0) : buf[S2W_PAD(base + (k << logs))];
         Bfly<R, false>::run(v);
         cplx w[R];
         twiddle_powers<R>(tw_lookup(stw, T, (i * twm) & T.twmask), w);
@@ -165,7 +184,8 @@ __device__ __forceinline__ void dif_pass(cplx *buf, int M, int logS, const FftTa
 }
 
 // The matching decimation-in-time inverse pass: conjugate twiddles, then inverse butterflies.
-template <int R>
+// HALF (outermost radix-8 pass only, S = M): the upper half of the result is neither formed nor stored.
+template <int R, bool HALF = false>
 __device__ __forceinline__ void dit_pass(cplx *buf, int M, int logS, const FftTab &T, const cplx *stw)
 {
     const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
@@ -183,7 +203,8 @@ __device__ __forceinline__ void dit_pass(cplx *buf, int M, int logS, const FftTa
         for (int j = 1; j < R; ++j) v[j] = cmulc(v[j], w[j]);
         Bfly<R, true>::run(v);
 #pragma unroll
-        for (int k = 0; k < R; ++k) buf[S2W_PAD(base + (k << logs))] = v[k];
+        for (int k = 0; k < R; ++k)
+            if (!(HALF && 2 * k >= R)) buf[S2W_PAD(base + (k << logs))] = v[k];
     }
 }
 
@@ -363,12 +384,21 @@ __device__ inline void fft_dif_full(cplx *buf, const FftTab &T, const cplx *stw)
 
 // buf <- circular convolution (length M) of buf with the kernel whose digit-reversed, 1/M-scaled spectrum is khat.
 // Ends with a __syncthreads().  Requires a __syncthreads() after the caller's writes to buf.
+// HALF: the sequence occupies the lower half of the buffer only (Bluestein: n <= M/2 inputs, n outputs wanted): the
+// upper half is taken as zero whatever it holds, and holds garbage afterwards -- the outermost pass of each transform
+// moves half the data.
+template <bool HALF = false>
 __device__ inline void fft_convolve(cplx *buf, const FftTab &T, const cplx *stw, const cplx *__restrict__ khat)
 {
     const int M = T.M;
     const int r = T.logM % 3;
     const int logMid = (r == 0) ? 3 : r;  // innermost group: 8, 2 or 4 elements
     int logS = T.logM;
+    if (HALF && logS > logMid) {
+        dif_pass<8, true>(buf, M, logS, T, stw);
+        __syncthreads();
+        logS -= 3;
+    }
     while (logS > logMid) {
         dif_pass<8>(buf, M, logS, T, stw);
         __syncthreads();
@@ -383,7 +413,10 @@ __device__ inline void fft_convolve(cplx *buf, const FftTab &T, const cplx *stw,
     __syncthreads();
     logS = logMid + 3;
     while (logS <= T.logM) {
-        dit_pass<8>(buf, M, logS, T, stw);
+        if (HALF && logS == T.logM)
+            dit_pass<8, true>(buf, M, logS, T, stw);
+        else
+            dit_pass<8>(buf, M, logS, T, stw);
         __syncthreads();
         logS += 3;
     }

@@ -632,7 +632,7 @@ __device__ __forceinline__ void so3_inv_pair_few(const cplx *__restrict__ F, dou
             }
         }
         __syncthreads();
-        fft_convolve(buf, T, s_tw, T.bhat_p);
+        fft_convolve<true>(buf, T, s_tw, T.bhat_p);
         for (int a = threadIdx.x; a < n; a += blockDim.x) {
             const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));  // V_0 of ring t0 + i V_0 of ring t0+1
             double *Wr = Wb + (size_t)t0 * n + a;
@@ -652,7 +652,7 @@ __device__ __forceinline__ void so3_inv_pair_few(const cplx *__restrict__ F, dou
             const cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * L;
             fill_row_pm(buf, Fp, Fm, T.chirp, n, L, M);
             __syncthreads();
-            fft_convolve(buf, T, s_tw, T.bhat_p);
+            fft_convolve<true>(buf, T, s_tw, T.bhat_p);
             if (i + 1 < np) {
                 for (int a = threadIdx.x; a < n; a += blockDim.x) {
                     const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
@@ -698,12 +698,16 @@ __device__ __forceinline__ void so3_inv_pair_few(const cplx *__restrict__ F, dou
 }
 
 __global__ void __launch_bounds__(256, 3) so3_inv_pair_kernel(const cplx *__restrict__ F, double *__restrict__ W,
-                                                             size_t sig_stride, So3Args A, FftTab T)
+                                                             size_t sig_stride, So3Args A, FftTab Tin)
 {
+    // dynamic shared memory: the Bluestein buffer, the twiddles (own split, tw_own_entries), and for 2N-1 > 9 the gamma
+    // phases; static shared memory stays small enough for three blocks per SM at M = 4096 (so3_launch)
     extern __shared__ cplx buf[];
-    __shared__ cplx s_tw[S2W_TW_SMEM];
-    __shared__ cplx gph[2 * S2W_MAX_N];
-    tw_stage(s_tw, T);
+    FftTab T = Tin;
+    cplx *s_tw = buf + fft_padded_len(T.M);
+    __shared__ cplx s_gph[36];
+    cplx *gph = 2 * A.N - 1 <= 9 ? s_gph : s_tw + tw_own_entries(T.logM);
+    tw_stage_own(s_tw, T);
     const int n = T.n, L = T.L, M = T.M;
     const int t0 = 2 * blockIdx.x, b = blockIdx.y;
     const bool has1 = t0 + 1 < L;
@@ -862,7 +866,7 @@ __device__ __forceinline__ void so3_fwd_pair_few(const double *__restrict__ W, c
     }
     __syncthreads();
     if (q0 >= 0) {
-        fft_convolve(buf, T, s_tw, T.bhat_m);
+        fft_convolve<true>(buf, T, s_tw, T.bhat_m);
         for (int k = threadIdx.x; k < n; k += blockDim.x) buf[S2W_PAD(k)] = cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k]));
         __syncthreads();
         cplx *F0 = Fb + ((size_t)A.n_row[q0] * L + t0) * L, *F1 = F0 + L;
@@ -894,7 +898,7 @@ __device__ __forceinline__ void so3_fwd_pair_few(const double *__restrict__ W, c
                 }
             }
             __syncthreads();
-            fft_convolve(buf, T, s_tw, T.bhat_m);
+            fft_convolve<true>(buf, T, s_tw, T.bhat_m);
             for (int m = threadIdx.x; m < L; m += blockDim.x) {
                 Fp[m] = cscale(cmul(buf[S2W_PAD(m)], __ldg(&T.chirp[m])), inv_n);
                 const int k = m == 0 ? 0 : n - m;
@@ -906,12 +910,16 @@ __device__ __forceinline__ void so3_fwd_pair_few(const double *__restrict__ W, c
 }
 
 __global__ void __launch_bounds__(256, 3) so3_fwd_pair_kernel(const double *__restrict__ W, cplx *__restrict__ F,
-                                                             size_t sig_stride, So3Args A, FftTab T)
+                                                             size_t sig_stride, So3Args A, FftTab Tin)
 {
+    // dynamic shared memory: the Bluestein buffer, the twiddles (own split, tw_own_entries), and for 2N-1 > 9 the gamma
+    // phases; static shared memory stays small enough for three blocks per SM at M = 4096 (so3_launch)
     extern __shared__ cplx buf[];
-    __shared__ cplx s_tw[S2W_TW_SMEM];
-    __shared__ cplx gph[2 * S2W_MAX_N];
-    tw_stage(s_tw, T);
+    FftTab T = Tin;
+    cplx *s_tw = buf + fft_padded_len(T.M);
+    __shared__ cplx s_gph[36];
+    cplx *gph = 2 * A.N - 1 <= 9 ? s_gph : s_tw + tw_own_entries(T.logM);
+    tw_stage_own(s_tw, T);
     const int n = T.n, L = T.L, M = T.M;
     const int t0 = 2 * blockIdx.x, b = blockIdx.y;
     const bool has1 = t0 + 1 < L;
@@ -1612,7 +1620,8 @@ static int so3_launch(bool fwd, bool real, const void *in, void *out, size_t sig
 {
     const int rpb = seqs_per_block(4096 / T.M, (long long)T.L * batch, 32);
     if (rpb == 1 && real) {  // large grids, real signals: ring pairs (the n = 0 row shares one transform)
-        size_t sm = fft_smem_bytes(T);
+        const int ng = 2 * A.N - 1;
+        size_t sm = ((size_t)fft_padded_len(T.M) + tw_own_entries(T.logM) + (ng <= 9 ? 0 : ng)) * sizeof(cplx);
         dim3 grid((T.L + 1) / 2, batch);
         int rc;
         if (fwd) {
