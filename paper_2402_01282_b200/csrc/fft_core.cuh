@@ -227,7 +227,7 @@ __device__ __forceinline__ void mid_pass(cplx *buf, int M, const cplx *__restric
 
 // Batched variants: nb transforms of length M stored bstride elements apart in one shared-memory buffer; one pass
 // works on all of them between two barriers.
-template <int R>
+template <int R, bool HALF = false>
 __device__ __forceinline__ void dif_pass_b(cplx *buf, int M, int logS, const FftTab &T, const cplx *stw, int nb, int bstride)
 {
     const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
@@ -241,7 +241,7 @@ __device__ __forceinline__ void dif_pass_b(cplx *buf, int M, int logS, const Fft
         int base = ((idx >> logs) << logS) + i;
         cplx v[R];
 #pragma unroll
-        for (int k = 0; k < R; ++k) v[k] = b[S2W_PAD(base + (k << logs))];
+        for (int k = 0; k < R; ++k) v[k] = (HALF && 2 * k >= R) ? cmake(0.0, 0.0) : b[S2W_PAD(base + (k << logs))];
         Bfly<R, false>::run(v);
         cplx w[R];
         twiddle_powers<R>(tw_lookup(stw, T, (i * twm) & T.twmask), w);
@@ -252,7 +252,7 @@ __device__ __forceinline__ void dif_pass_b(cplx *buf, int M, int logS, const Fft
     }
 }
 
-template <int R>
+template <int R, bool HALF = false>
 __device__ __forceinline__ void dit_pass_b(cplx *buf, int M, int logS, const FftTab &T, const cplx *stw, int nb, int bstride)
 {
     const int logs = logS - (R == 8 ? 3 : (R == 4 ? 2 : 1));
@@ -273,7 +273,8 @@ __device__ __forceinline__ void dit_pass_b(cplx *buf, int M, int logS, const Fft
         for (int j = 1; j < R; ++j) v[j] = cmulc(v[j], w[j]);
         Bfly<R, true>::run(v);
 #pragma unroll
-        for (int k = 0; k < R; ++k) b[S2W_PAD(base + (k << logs))] = v[k];
+        for (int k = 0; k < R; ++k)
+            if (!(HALF && 2 * k >= R)) b[S2W_PAD(base + (k << logs))] = v[k];
     }
 }
 
@@ -336,6 +337,7 @@ __device__ __forceinline__ void mid_pass_b(cplx *buf, int M, const cplx *__restr
 }
 
 // nb circular convolutions (sequences bstride apart) with the same kernel spectrum; see fft_convolve.
+template <bool HALF = false>
 __device__ inline void fft_convolve_b(cplx *buf, const FftTab &T, const cplx *stw, const cplx *__restrict__ khat,
                                       int nb, int bstride)
 {
@@ -343,6 +345,11 @@ __device__ inline void fft_convolve_b(cplx *buf, const FftTab &T, const cplx *st
     const int r = T.logM % 3;
     const int logMid = (r == 0) ? 3 : r;
     int logS = T.logM;
+    if (HALF && logS > logMid) {
+        dif_pass_b<8, true>(buf, M, logS, T, stw, nb, bstride);
+        __syncthreads();
+        logS -= 3;
+    }
     while (logS > logMid) {
         dif_pass_b<8>(buf, M, logS, T, stw, nb, bstride);
         __syncthreads();
@@ -357,7 +364,10 @@ __device__ inline void fft_convolve_b(cplx *buf, const FftTab &T, const cplx *st
     __syncthreads();
     logS = logMid + 3;
     while (logS <= T.logM) {
-        dit_pass_b<8>(buf, M, logS, T, stw, nb, bstride);
+        if (HALF && logS == T.logM)
+            dit_pass_b<8, true>(buf, M, logS, T, stw, nb, bstride);
+        else
+            dit_pass_b<8>(buf, M, logS, T, stw, nb, bstride);
         __syncthreads();
         logS += 3;
     }

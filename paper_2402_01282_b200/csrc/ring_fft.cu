@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(256, 3) ring_fwd_kernel(const void *__restrict
             buf[S2W_PAD(p)] = v;
         }
         __syncthreads();
-        fft_convolve(buf, T, s_tw, T.bhat_m);
+        fft_convolve<true>(buf, T, s_tw, T.bhat_m);
         for (int k = threadIdx.x; k < n; k += blockDim.x) buf[S2W_PAD(k)] = cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k]));
         __syncthreads();
         for (int m = threadIdx.x; m < L; m += blockDim.x) {
@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(256, 3) ring_fwd_kernel(const void *__restrict
             buf[S2W_PAD(p)] = v;
         }
         __syncthreads();
-        fft_convolve(buf, T, s_tw, T.bhat_m);
+        fft_convolve<true>(buf, T, s_tw, T.bhat_m);
         for (int mi = threadIdx.x; mi < n; mi += blockDim.x) {
             int m = mi - (L - 1);
             int k = m < 0 ? m + n : m;
@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(256, 3) ring_inv_kernel(const cplx *__restrict
             buf[S2W_PAD(k)] = v;
         }
         __syncthreads();
-        fft_convolve(buf, T, s_tw, T.bhat_p);
+        fft_convolve<true>(buf, T, s_tw, T.bhat_p);
         double *y0 = (double *)out + (size_t)(r0 / L) * sig_stride + (size_t)(r0 % L) * n;
         double *y1 = (double *)out + (size_t)(r1 / L) * sig_stride + (size_t)(r1 % L) * n;
         for (int p = threadIdx.x; p < n; p += blockDim.x) {
@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(256, 3) ring_inv_kernel(const cplx *__restrict
             buf[S2W_PAD(k)] = v;
         }
         __syncthreads();
-        fft_convolve(buf, T, s_tw, T.bhat_p);
+        fft_convolve<true>(buf, T, s_tw, T.bhat_p);
         cplx *y0 = (cplx *)out + (size_t)(r0 / L) * sig_stride + (size_t)(r0 % L) * n;
         for (int p = threadIdx.x; p < n; p += blockDim.x) y0[p] = cmulc(buf[S2W_PAD(p)], __ldg(&T.chirp[p]));
     }
@@ -197,9 +197,9 @@ __device__ __forceinline__ void so3_inv_few(const cplx *__restrict__ F, void *__
         }
         __syncthreads();
         if (MULTI)
-            fft_convolve_b(buf0, T, s_tw, T.bhat_p, rpb, bstride);
+            fft_convolve_b<true>(buf0, T, s_tw, T.bhat_p, rpb, bstride);
         else
-            fft_convolve(buf, T, s_tw, T.bhat_p);
+            fft_convolve<true>(buf, T, s_tw, T.bhat_p);
         for (int a = tl; a < (has ? n : 0); a += tpr) {
             const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
             if (REAL) {
@@ -303,9 +303,9 @@ __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict_
         }
         __syncthreads();
         if (MULTI)
-            fft_convolve_b(buf0, T, s_tw, T.bhat_p, rpb, bstride);
+            fft_convolve_b<true>(buf0, T, s_tw, T.bhat_p, rpb, bstride);
         else
-            fft_convolve(buf, T, s_tw, T.bhat_p);
+            fft_convolve<true>(buf, T, s_tw, T.bhat_p);
         // one pass over alpha: the chirp product once, then all gamma planes with their loads issued together
         for (int a = tl; a < (has ? n : 0); a += tpr) {
             const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
@@ -441,9 +441,9 @@ __device__ __forceinline__ void so3_fwd_few(const void *__restrict__ W, cplx *__
             __syncthreads();
         }
         if (MULTI)
-            fft_convolve_b(buf0, T, s_tw, T.bhat_m, rpb, bstride);
+            fft_convolve_b<true>(buf0, T, s_tw, T.bhat_m, rpb, bstride);
         else
-            fft_convolve(buf, T, s_tw, T.bhat_m);
+            fft_convolve<true>(buf, T, s_tw, T.bhat_m);
         if (REAL) {
             const int nv = s_nv[i];
             for (int m = tl; m < (has ? L : 0); m += tpr) {
@@ -528,9 +528,9 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
         }
         __syncthreads();
         if (MULTI)
-            fft_convolve_b(buf0, T, s_tw, T.bhat_m, rpb, bstride);
+            fft_convolve_b<true>(buf0, T, s_tw, T.bhat_m, rpb, bstride);
         else
-            fft_convolve(buf, T, s_tw, T.bhat_m);
+            fft_convolve<true>(buf, T, s_tw, T.bhat_m);
         cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * Md;
         cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * Md;
         if (REAL) {
@@ -739,7 +739,7 @@ __global__ void __launch_bounds__(256, 3) so3_inv_pair_kernel(const cplx *__rest
                 buf[S2W_PAD(k)] = v;
             }
             __syncthreads();
-            fft_convolve(buf, T, s_tw, T.bhat_p);
+            fft_convolve<true>(buf, T, s_tw, T.bhat_p);
             for (int a = threadIdx.x; a < n; a += blockDim.x) {
                 const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));  // V_0 of ring t0 + i V_0 of ring t0+1
                 double *Wr = Wb + (size_t)t0 * n + a;
@@ -763,7 +763,7 @@ __global__ void __launch_bounds__(256, 3) so3_inv_pair_kernel(const cplx *__rest
                 buf[S2W_PAD(k)] = v;
             }
             __syncthreads();
-            fft_convolve(buf, T, s_tw, T.bhat_p);
+            fft_convolve<true>(buf, T, s_tw, T.bhat_p);
             for (int a = threadIdx.x; a < n; a += blockDim.x) {
                 const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
                 double *Wr = Wb + (size_t)t * n + a;
@@ -958,7 +958,7 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_pair_kernel(const double *__re
                 buf[S2W_PAD(a)] = v;
             }
             __syncthreads();
-            fft_convolve(buf, T, s_tw, T.bhat_m);
+            fft_convolve<true>(buf, T, s_tw, T.bhat_m);
             for (int k = threadIdx.x; k < n; k += blockDim.x) buf[S2W_PAD(k)] = cmul(buf[S2W_PAD(k)], __ldg(&T.chirp[k]));
             __syncthreads();
             cplx *F0 = Fb + ((size_t)A.n_row[q] * L + t0) * L, *F1 = F0 + L;
@@ -996,7 +996,7 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_pair_kernel(const double *__re
                 buf[S2W_PAD(a)] = v;
             }
             __syncthreads();
-            fft_convolve(buf, T, s_tw, T.bhat_m);
+            fft_convolve<true>(buf, T, s_tw, T.bhat_m);
             cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * L;
             cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * L;
             for (int m = threadIdx.x; m < L; m += blockDim.x) {
