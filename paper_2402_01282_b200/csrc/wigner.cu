@@ -418,7 +418,11 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
     constexpr int TLF = FWD_TILE(R);
     __shared__ double2 s_ag[TLF];
     __shared__ double2 s_e[TLF];
-    __shared__ double s_red[TLF][NC];  // per-tile sums over all warps (shared-memory atomics), true sign
+    // per-tile sums over all warps (shared-memory atomics), true sign: (degree ll, column c) at SRED(ll, c) -- degree
+    // pairs 20 doubles apart, so that the 16 lanes of a half-warp (4 degree pairs x 4 columns of a D fragment) hit 16
+    // different bank pairs (with rows of 8 the four degree pairs shared one: 4-way conflicts on the load and the CAS)
+#define SRED(ll, c) ((((ll) >> 1) * 20) + (((ll) & 1) * 8) + (c))
+    __shared__ double s_red[(TLF / 2) * 20];
     extern __shared__ double s_dt[];   // the B-fragment tiles [W][R][FWD_GT]
 
     const int m = blockIdx.x, chunk = blockIdx.y;
@@ -489,7 +493,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
 
         for (int lt = first & ~(TLF - 1); lt < Lg; lt += TLF) {
             __syncthreads();
-            for (int i = threadIdx.x; i < TLF * NC; i += T) (&s_red[0][0])[i] = 0.0;
+            for (int i = threadIdx.x; i < (TLF / 2) * 20; i += T) s_red[i] = 0.0;
             if (!PRE) stage_coef<TLF>(crow, lt, l0, Lg, s_ag, s_e);
             __syncthreads();
             const bool want = lt + TLF > lacc;  // this tile has outputs
@@ -583,8 +587,8 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                 // (southern warps: d = (-1)^l d~, and the octet starts at an even degree)
                 if (contributed) {
                     const double v0 = c0 + c2, v1 = c1 + c3;
-                    atomicAdd(&s_red[8 * oc + 2 * fk][fc], v0);
-                    atomicAdd(&s_red[8 * oc + 2 * fk + 1][fc], (!PRE && hemi) ? -v1 : v1);
+                    atomicAdd(&s_red[SRED(8 * oc + 2 * fk, fc)], v0);
+                    atomicAdd(&s_red[SRED(8 * oc + 2 * fk + 1, fc)], (!PRE && hemi) ? -v1 : v1);
                 }
             }
             if (!want) continue;
@@ -600,7 +604,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                 cplx val = cmake(0.0, 0.0);
                 for (int sc = 0; sc < (fuse ? 2 : 1); ++sc) {
                     const int c0i = 2 * k + 4 * sc;
-                    const double re = s_red[ll][c0i], im = s_red[ll][c0i + 1];
+                    const double re = s_red[SRED(ll, c0i)], im = s_red[SRED(ll, c0i + 1)];
                     const cplx Gf = (sc ? A.filt2 : A.filt)[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
                     val = cadd(val, cmul(Gf, cmake(re, im)));
                 }
