@@ -1,0 +1,608 @@
+// fft16_kernels.cu -- rows a8 (alpha, gamma FFT) and a2 (theta reweighting) on the register-fed radix-16 core of
+// fft16_core.cuh, for Bluestein / Toeplitz lengths 1024, 2048 and 4096 (grids with 129 <= L_j <= 1024: every grid that
+// matters for the time of BASELINE configs 2, 3 and 5).  Other lengths stay on the radix-8 kernels of ring_fft.cu.
+//
+//   a8  W(gamma_g, beta_t, alpha_a) = sum_{m,n} F_mn(beta_t) e^{i(m alpha_a + n gamma_g)}            (Eq. 5/47)
+//       F_mn(beta_t) = 1/(n_a n_g) sum_{a,g} W e^{-i(m alpha_a + n gamma_g)}                         (Eq. 48)
+//   a2  h = reweight(F) per (m, n) column along theta, Toeplitz/Hankel form                          (R3)
+//
+// A block works on NB = 4096 / M sequences at a time ("round").  Thread tid owns elements tid + 256 c (c < M/512) of
+// every sequence of a round: it loads them from global memory (coalesced), and gets the same elements of the result
+// back in registers.
+#include "fft16_core.cuh"
+#include "kernels.h"
+#include "smem_attr.cuh"
+
+namespace s2w {
+
+namespace {
+
+__device__ __forceinline__ cplx cis_2pi(int num, int den)  // exp(2 pi i num/den), num reduced mod den
+{
+    int r = num % den;
+    if (r < 0) r += den;
+    double s, c;
+    sincospi(2.0 * (double)r / (double)den, &s, &c);
+    return cmake(c, s);
+}
+
+// rows n = 0 / n > 0 of a real-signal launch, and the gamma phases e^{+- i n gamma_g} of the rows n > 0
+struct RowSet {
+    int q0, np;
+};
+__device__ __forceinline__ RowSet so3_rows(const So3Args &A, int sign, cplx *gph, int *s_rowp, int *s_rowm)
+{
+    const int ng = 2 * A.N - 1;
+    RowSet r;
+    r.q0 = -1;
+    r.np = 0;
+    for (int q = 0; q < A.nn; ++q) {
+        if (A.n_val[q] == 0) r.q0 = q;
+        if (A.n_val[q] > 0 && r.np < 4) {
+            for (int g = threadIdx.x; g < ng; g += blockDim.x) gph[r.np * ng + g] = cis_2pi(sign * A.n_val[q] * g, ng);
+            if (threadIdx.x == 0) {
+                s_rowp[r.np] = A.n_row[q];
+                s_rowm[r.np] = A.n_rowm[q];
+            }
+            ++r.np;
+        }
+    }
+    return r;
+}
+
+// The I/O stages around a round work on the thread's 8 elements e = q HR + c (sequence q, element tid + 256 c) in ROLLED
+// loops over batches of 4 (or 2), loads first: fully unrolled they keep the addresses and loaded values of all 8 elements
+// live at once and spill (ptxas: 0.8-1.6 KB of local memory per thread, as much LSU traffic as the transform itself).
+// XE(h, j) is element 4h + j of the register array x[NB][R1] for a rolled h and an unrolled j: one select per register.
+#define XE_GET(x, HRv, h, j) ((h) ? (x)[(4 + (j)) / (HRv)][(4 + (j)) % (HRv)] : (x)[(j) / (HRv)][(j) % (HRv)])
+#define XE_SET(x, HRv, h, j, val)                                   \
+    do {                                                            \
+        const cplx _v = (val);                                      \
+        if (h)                                                      \
+            (x)[(4 + (j)) / (HRv)][(4 + (j)) % (HRv)] = _v;         \
+        else                                                        \
+            (x)[(j) / (HRv)][(j) % (HRv)] = _v;                     \
+    } while (0)
+
+// the same for batches of 2: element 2h + j, h = 0..3 rolled, j = 0..1 unrolled
+#define X2_AT(x, HRv, e) (x)[(e) / (HRv)][(e) % (HRv)]
+#define X2_GET(x, HRv, h, j) \
+    ((h) == 0 ? X2_AT(x, HRv, j) : (h) == 1 ? X2_AT(x, HRv, 2 + (j)) : (h) == 2 ? X2_AT(x, HRv, 4 + (j)) : X2_AT(x, HRv, 6 + (j)))
+#define X2_SET(x, HRv, h, j, val)                   \
+    do {                                            \
+        const cplx _v = (val);                      \
+        if ((h) == 0) X2_AT(x, HRv, j) = _v;        \
+        if ((h) == 1) X2_AT(x, HRv, 2 + (j)) = _v;  \
+        if ((h) == 2) X2_AT(x, HRv, 4 + (j)) = _v;  \
+        if ((h) == 3) X2_AT(x, HRv, 6 + (j)) = _v;  \
+    } while (0)
+
+// ---------------------------------------------------------------------------------------------------------------
+// a8 analysis, real signals, 2N-1 <= 9: F[b][row][t][m >= 0] -> W[b][g][t][a] (real).  A block owns NB PAIRS of rings.
+// Round 0: the rows n = 0 of a pair's two rings share one transform (X_t0 + i X_t1, Hermitian in m); then one round
+// per row n > 0 and ring parity.  Until a ring's last row the transforms V_n(alpha) are parked in the ring's own output
+// planes (each thread reads back only what it wrote), and every plane is written once in the last round.
+// ---------------------------------------------------------------------------------------------------------------
+template <int R1>
+__global__ void __launch_bounds__(256, 2) so3_inv_pair16_kernel(const cplx *__restrict__ F, double *__restrict__ W,
+                                                               size_t sig_stride, So3Args A, FftTab T)
+{
+    constexpr int NB = 16 / R1, HR = R1 / 2;
+    extern __shared__ cplx buf[];
+    __shared__ cplx gph[36];
+    __shared__ int s_rowp[4], s_rowm[4];
+    const F16Tw tw = f16_twiddles<R1>();
+    const int n = T.n, L = T.L, ng = 2 * A.N - 1;
+    const cplx *Fb = F + (size_t)blockIdx.y * A.nrows * L * L;
+    double *Wb = W + (size_t)blockIdx.y * sig_stride;
+    const size_t plane = (size_t)L * n;
+    const RowSet rs = so3_rows(A, +1, gph, s_rowp, s_rowm);
+    const int q0 = rs.q0, np = rs.np;
+    __syncthreads();
+    cplx x[NB][R1];
+    if (q0 >= 0) {
+        const cplx *Xrow = Fb + (size_t)A.n_row[q0] * L * L;
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+            cplx a[4], cc[4], ch[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int e = 4 * h + j, q = e / HR, c = e % HR;
+                const int t0 = 2 * (blockIdx.x * NB + q), k = threadIdx.x + 256 * c;
+                const int kk = (k < n && t0 < L) ? k : 0, m = kk < L ? kk : n - kk;
+                const cplx *X0 = Xrow + (size_t)(t0 < L ? t0 : 0) * L;
+                a[j] = X0[m];
+                cc[j] = X0[(t0 + 1 < L ? L : 0) + m];
+                ch[j] = __ldg(&T.chirp[kk]);
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int e = 4 * h + j, q = e / HR, c = e % HR;
+                const int t0 = 2 * (blockIdx.x * NB + q), k = threadIdx.x + 256 * c;
+                cplx av = a[j], cv = t0 + 1 < L ? cc[j] : cmake(0.0, 0.0);
+                if (k >= L) {
+                    av = cconj(av);
+                    cv = cconj(cv);
+                }
+                XE_SET(x, HR, h, j, (k < n && t0 < L) ? cmulc(cmake(av.x - cv.y, av.y + cv.x), ch[j]) : cmake(0.0, 0.0));
+            }
+        }
+        f16_convolve_half<R1>(buf, x, T.bhat16_p, tw);
+        const int nplanes = np ? 1 : ng;
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int e = 4 * h + j, q = e / HR, c = e % HR;
+                const int t0 = 2 * (blockIdx.x * NB + q), a = threadIdx.x + 256 * c;
+                if (a < n && t0 < L) {
+                    const cplx v = cmulc(XE_GET(x, HR, h, j), __ldg(&T.chirp[a]));  // V_0 of ring t0 + i V_0 of ring t0+1
+                    double *Wr = Wb + (size_t)t0 * n + a;
+                    for (int g = 0; g < nplanes; ++g) {
+                        Wr[g * plane] = v.x;
+                        if (t0 + 1 < L) Wr[g * plane + n] = v.y;
+                    }
+                }
+            }
+        }
+    }
+#pragma unroll 1
+    for (int ri = 0; ri < 2 * np; ++ri) {
+        const int r = ri / np, i = ri - r * np;
+        const cplx *Fp = Fb + (size_t)s_rowp[i] * L * L, *Fm = Fb + (size_t)s_rowm[i] * L * L;
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+            cplx v[4], ch[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int e = 4 * h + j, q = e / HR, c = e % HR;
+                const int t = 2 * (blockIdx.x * NB + q) + r, k = threadIdx.x + 256 * c;
+                const int kk = (k < n && t < L) ? k : 0;
+                const size_t ro = (size_t)(t < L ? t : 0) * L;
+                v[j] = *(kk < L ? Fp + ro + kk : Fm + ro + (n - kk));
+                ch[j] = __ldg(&T.chirp[kk]);
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int e = 4 * h + j, q = e / HR, c = e % HR;
+                const int t = 2 * (blockIdx.x * NB + q) + r, k = threadIdx.x + 256 * c;
+                const cplx vv = k >= L ? cconj(v[j]) : v[j];
+                XE_SET(x, HR, h, j, (k < n && t < L) ? cmulc(vv, ch[j]) : cmake(0.0, 0.0));
+            }
+        }
+        f16_convolve_half<R1>(buf, x, T.bhat16_p, tw);
+        if (i + 1 < np) {  // park V_n in planes 2i+1, 2i+2 of the ring
+#pragma unroll 1
+            for (int h = 0; h < 2; ++h) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int e = 4 * h + j, q = e / HR, c = e % HR;
+                    const int t = 2 * (blockIdx.x * NB + q) + r, a = threadIdx.x + 256 * c;
+                    if (a < n && t < L) {
+                        const cplx v = cmulc(XE_GET(x, HR, h, j), __ldg(&T.chirp[a]));
+                        double *Wr = Wb + (size_t)t * n + a;
+                        Wr[(2 * i + 1) * plane] = v.x;
+                        Wr[(2 * i + 2) * plane] = v.y;
+                    }
+                }
+            }
+            continue;
+        }
+#pragma unroll 1
+        for (int h = 0; h < 4; ++h) {  // last row of the ring: every gamma plane written once; two elements at a time
+            cplx xv[2];
+            double sc[2][7];
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                xv[j] = X2_GET(x, HR, h, j);
+                const int e = 2 * h + j, q = e / HR, c = e % HR;
+                const int t = 2 * (blockIdx.x * NB + q) + r, a = threadIdx.x + 256 * c;
+                const bool on = a < n && t < L;
+                const double *Wr = Wb + (on ? (size_t)t * n + a : 0);
+#pragma unroll
+                for (int s = 0; s < 7; ++s) sc[j][s] = 0.0;
+                if (q0 >= 0) sc[j][0] = Wr[0];
+#pragma unroll
+                for (int s = 1; s < 7; ++s)
+                    if (s < 2 * np - 1) sc[j][s] = Wr[s * plane];
+            }
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int e = 2 * h + j, q = e / HR, c = e % HR;
+                const int t = 2 * (blockIdx.x * NB + q) + r, a = threadIdx.x + 256 * c;
+                if (a >= n || t >= L) continue;
+                const cplx v = cmulc(xv[j], __ldg(&T.chirp[a]));
+                double *Wr = Wb + (size_t)t * n + a;
+                double out[9];
+#pragma unroll
+                for (int g = 0; g < 9; ++g) {
+                    const cplx ph = gph[(np - 1) * ng + (g < ng ? g : 0)];
+                    out[g] = fma(2.0, ph.x * v.x - ph.y * v.y, sc[j][0]);
+                }
+#pragma unroll
+                for (int jj = 0; jj < 3; ++jj)
+                    if (jj + 1 < np) {
+#pragma unroll
+                        for (int g = 0; g < 9; ++g) {
+                            const cplx ph = gph[jj * ng + (g < ng ? g : 0)];
+                            out[g] = fma(2.0, ph.x * sc[j][2 * jj + 1] - ph.y * sc[j][2 * jj + 2], out[g]);
+                        }
+                    }
+#pragma unroll
+                for (int g = 0; g < 9; ++g)
+                    if (g < ng) Wr[g * plane] = out[g];
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a8 synthesis, real signals, 2N-1 <= 9: W[b][g][t][a] -> F[b][row][t][m >= 0].  The gamma planes of a ring cross the
+// memory system once: the gather forms the gamma sums Y_n(alpha) of all rows, feeds the row n = 0 (ring t0 real part,
+// ring t0+1 imaginary part) straight into round 0 and parks the rows n > 0, chirp applied, in the ring's own output
+// rows F_{., n}, F_{., -n} (2L >= 2L-1 entries), from where that row's round takes them back (same thread).
+// ---------------------------------------------------------------------------------------------------------------
+template <int R1>
+__global__ void __launch_bounds__(256, 2) so3_fwd_pair16_kernel(const double *__restrict__ W, cplx *__restrict__ F,
+                                                               size_t sig_stride, So3Args A, FftTab T)
+{
+    constexpr int NB = 16 / R1, HR = R1 / 2, M = R1 * 256;
+    extern __shared__ cplx buf[];
+    __shared__ cplx gph[36];
+    __shared__ int s_rowp[4], s_rowm[4];
+    const F16Tw tw = f16_twiddles<R1>();
+    const int n = T.n, L = T.L, ng = 2 * A.N - 1;
+    const double inv_ng = 1.0 / (double)ng, inv_n = 1.0 / (double)n;
+    cplx *Fb = F + (size_t)blockIdx.y * A.nrows * L * L;
+    const double *Wb = W + (size_t)blockIdx.y * sig_stride;
+    const size_t plane = (size_t)L * n;
+    const RowSet rs = so3_rows(A, -1, gph, s_rowp, s_rowm);
+    const int q0 = rs.q0, np = rs.np;
+    __syncthreads();
+    cplx x[NB][R1];
+    // gather: every gamma plane of both rings of a pair once, two alpha samples (36 loads) at a time
+#pragma unroll 1
+    for (int h = 0; h < 4; ++h) {
+        double wv[2][2][9];
+        cplx ch[2];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int e = 2 * h + j, q = e / HR, c = e % HR;
+            const int t0 = 2 * (blockIdx.x * NB + q), a = threadIdx.x + 256 * c;
+            const int aa = a < n ? a : 0;
+            const double *W0 = Wb + (size_t)(t0 < L ? t0 : 0) * n + aa, *W1 = Wb + (size_t)(t0 + 1 < L ? t0 + 1 : 0) * n + aa;
+            ch[j] = __ldg(&T.chirp[aa]);
+#pragma unroll
+            for (int g = 0; g < 9; ++g) {
+                const size_t o = (size_t)(g < ng ? g : 0) * plane;
+                wv[j][0][g] = W0[o];
+                wv[j][1][g] = W1[o];
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int e = 2 * h + j, q = e / HR, c = e % HR;
+            const int t0 = 2 * (blockIdx.x * NB + q), a = threadIdx.x + 256 * c;
+            const bool has0 = t0 < L && a < n, has1 = t0 + 1 < L && a < n;
+#pragma unroll
+            for (int g = 0; g < 9; ++g) {
+                if (g >= ng || !has0) wv[j][0][g] = 0.0;
+                if (g >= ng || !has1) wv[j][1][g] = 0.0;
+            }
+            double y0 = 0.0, y1 = 0.0;
+#pragma unroll
+            for (int g = 0; g < 9; ++g) {
+                y0 += wv[j][0][g];
+                y1 += wv[j][1][g];
+            }
+            X2_SET(x, HR, h, j, cmul(cscale(cmake(y0, y1), inv_ng), ch[j]));
+#pragma unroll
+            for (int r = 0; r < 2; ++r) {
+                if (r == 0 ? !has0 : !has1) continue;
+                for (int i = 0; i < np; ++i) {
+                    cplx y = cmake(0.0, 0.0);
+#pragma unroll
+                    for (int g = 0; g < 9; ++g) {
+                        const cplx ph = gph[i * ng + (g < ng ? g : 0)];
+                        y.x = fma(ph.x, wv[j][r][g], y.x);
+                        y.y = fma(ph.y, wv[j][r][g], y.y);
+                    }
+                    y = cmul(cscale(y, inv_ng), ch[j]);
+                    cplx *dst = a < L ? Fb + ((size_t)s_rowp[i] * L + t0 + r) * L + a
+                                      : Fb + ((size_t)s_rowm[i] * L + t0 + r) * L + (a - L);
+                    *dst = y;
+                }
+            }
+        }
+    }
+    if (q0 >= 0) {
+        f16_convolve_half<R1>(buf, x, T.bhat16_m, tw);
+        // u(k) = chirp(k) y(k) back into the thread's own column slots, then F0[m], F1[m] from u(m), u(n - m)
+#pragma unroll
+        for (int q = 0; q < NB; ++q)
+#pragma unroll
+            for (int c = 0; c < HR; ++c) {
+                const int k = threadIdx.x + 256 * c;
+                buf[F16_PAD(q * M + k)] = cmul(x[q][c], __ldg(&T.chirp[k < n ? k : 0]));
+            }
+        __syncthreads();
+#pragma unroll 1
+        for (int q = 0; q < NB; ++q) {
+            const int t0 = 2 * (blockIdx.x * NB + q);
+            if (t0 >= L) continue;
+            const bool has1 = t0 + 1 < L;
+            cplx *F0 = Fb + ((size_t)A.n_row[q0] * L + t0) * L, *F1 = F0 + L;
+            for (int m = threadIdx.x; m < L; m += 256) {
+                const cplx a = buf[F16_PAD(q * M + m)], c = cconj(buf[F16_PAD(q * M + (m == 0 ? 0 : n - m))]);
+                const cplx sm = cadd(a, c), df = csub(a, c);
+                F0[m] = cscale(sm, 0.5 * inv_n);
+                if (has1) F1[m] = cmake(0.5 * inv_n * df.y, -0.5 * inv_n * df.x);
+            }
+        }
+        __syncthreads();
+    }
+#pragma unroll 1
+    for (int ri = 0; ri < 2 * np; ++ri) {
+        const int r = ri / np, i = ri - r * np;
+        cplx *Fp = Fb + (size_t)s_rowp[i] * L * L, *Fm = Fb + (size_t)s_rowm[i] * L * L;
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+            cplx v[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int e = 4 * h + j, q = e / HR, c = e % HR;
+                const int t = 2 * (blockIdx.x * NB + q) + r, a = threadIdx.x + 256 * c;
+                const int aa = (a < n && t < L) ? a : 0;
+                const size_t ro = (size_t)(t < L ? t : 0) * L;
+                v[j] = *(aa < L ? Fp + ro + aa : Fm + ro + (aa - L));
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int e = 4 * h + j, q = e / HR, c = e % HR;
+                const int t = 2 * (blockIdx.x * NB + q) + r, a = threadIdx.x + 256 * c;
+                XE_SET(x, HR, h, j, (a < n && t < L) ? v[j] : cmake(0.0, 0.0));
+            }
+        }
+        f16_convolve_half<R1>(buf, x, T.bhat16_m, tw);
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int e = 4 * h + j, q = e / HR, c = e % HR;
+                const int t = 2 * (blockIdx.x * NB + q) + r, k = threadIdx.x + 256 * c;
+                if (k >= n || t >= L) continue;
+                const cplx u = cscale(cmul(XE_GET(x, HR, h, j), __ldg(&T.chirp[k])), inv_n);
+                const size_t ro = (size_t)t * L;
+                if (k < L) Fp[ro + k] = u;
+                if (k == 0 || k >= L) Fm[ro + (k == 0 ? 0 : n - k)] = cconj(u);
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a2 on the radix-16 core: the Toeplitz/Hankel form of DESIGN.md 6.3 (see reweight_th_kernel in ring_fft.cu for the
+// algebra), M2 = R1 * 256 = 2048 or 1024.  A block owns NC = 8 / R1 columns, two sequences each (u1 = a x, u2 = delta a x);
+// thread tid holds the ring values x_t, t = tid + 256 c, of its columns in registers from the first load to the last
+// store.  The spectra U(k) and U(-k) meet between the innermost forward and inverse passes: position
+// p = j1 256 + j2 16 + j3 holds k = j1 + R1 (j2 + 16 j3), so the partners of a thread's 16 contiguous positions are 16
+// contiguous positions of another thread, in reverse order.
+// ---------------------------------------------------------------------------------------------------------------
+template <int R1>
+__global__ void __launch_bounds__(256, 2) reweight16_kernel(const cplx *__restrict__ F, cplx *__restrict__ Ft, RwArgs A,
+                                                           RwTab R, int ncolumns)
+{
+    constexpr int NB = 16 / R1, NC = NB / 2, HR = R1 / 2, M = R1 * 256;
+    extern __shared__ cplx buf[];
+    __shared__ cplx s_part[NC][8];
+    __shared__ cplx s_pole[NC];
+    const F16Tw tw = f16_twiddles<R1>();
+    const int L = R.L, Lm = L - 1;
+    cplx xs[NC][HR];
+    cplx x[NB][R1];
+    int par_of[NC];
+    cplx *colT_of[NC];
+#pragma unroll
+    for (int ci = 0; ci < NC; ++ci) {
+        const int colid = blockIdx.x * NC + ci;
+        const bool has = colid < ncolumns;
+        const int mi = colid % A.Md, q = (colid / A.Md) % A.nn, b = colid / (A.Md * A.nn);
+        const int m = A.isReal ? mi : mi - (L - 1);
+        const int nv = has ? A.n_val[q] : 0, row = has ? A.n_row[q] : 0;
+        const int par = ((m + nv) & 1) ? 1 : 0;  // 0: sigma = +1, 1: sigma = -1
+        par_of[ci] = par;
+        const cplx *col = F + ((size_t)(has ? b : 0) * A.nrows + row) * (size_t)L * A.Md + (has ? mi : 0);
+        colT_of[ci] = has ? Ft + (((size_t)b * A.nrows + row) * A.Md + mi) * (size_t)L : nullptr;
+        const double *rp = R.rpole + par * L;
+        cplx dot = cmake(0.0, 0.0);
+#pragma unroll
+        for (int c = 0; c < HR; ++c) {
+            const int t = threadIdx.x + 256 * c;
+            cplx xv = cmake(0.0, 0.0);
+            if (t < L && has) {
+                xv = col[(size_t)t * A.Md];
+                const double r = rp[t];
+                dot.x = fma(r, xv.x, dot.x);
+                dot.y = fma(r, xv.y, dot.y);
+            }
+            xs[ci][c] = xv;
+            if (t == Lm) s_pole[ci] = xv;
+            cplx u1 = cmake(0.0, 0.0), u2 = u1;
+            if (t < Lm) {
+                u1 = (t & 1) ? cscale(xv, -1.0) : xv;
+                u2 = cscale(u1, R.delta[t]);
+            }
+            x[2 * ci][c] = u1;
+            x[2 * ci + 1][c] = u2;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            dot.x += __shfl_xor_sync(0xffffffffu, dot.x, o);
+            dot.y += __shfl_xor_sync(0xffffffffu, dot.y, o);
+        }
+        if ((threadIdx.x & 31) == 0) s_part[ci][threadIdx.x >> 5] = dot;
+    }
+#pragma unroll
+    for (int q = 0; q < NB; ++q) f16_pass1_fwd<R1, true>(buf, q, x[q], tw);
+    __syncthreads();
+    f16_pass2_fwd(buf, tw);
+    __syncwarp();
+    f16_pass3_fwd(buf);
+    __syncthreads();
+    {
+        const int hw = threadIdx.x >> 4, j2 = threadIdx.x & 15;
+        const int sq = hw / R1, j1 = hw % R1;                       // sequence, sub-block inside it
+        const int j1p = (R1 - j1) % R1, j2p = j1 ? 15 - j2 : (16 - j2) & 15;
+        const bool shifted = j1 == 0 && j2 == 0;                    // partner of j3 is (16 - j3) % 16, else 15 - j3
+        cplx *own = buf + F16_PAD(hw * 256 + j2 * 16);
+        const cplx *prt = buf + F16_PAD(sq * M + j1p * 256 + j2p * 16);
+        const cplx *tg = R.TG16 + (j1 * 256 + j2);                   // [2][M2] in the storage order F16_TPOS
+        double sg = par_of[0] ? -1.0 : 1.0;
+#pragma unroll
+        for (int ci = 1; ci < NC; ++ci)
+            if ((sq >> 1) == ci) sg = par_of[ci] ? -1.0 : 1.0;
+        if (!(sq & 1)) sg = -sg;                                    // u1: T - sigma H, u2: T + sigma H
+        cplx v[16];
+#pragma unroll
+        for (int j3 = 0; j3 < 16; ++j3) {
+            const cplx u = own[j3], un = prt[shifted ? (16 - j3) & 15 : 15 - j3];
+            const cplx th = __ldg(&tg[16 * j3]), gh = cscale(__ldg(&tg[M + 16 * j3]), sg);
+            v[j3] = cadd(cmul(th, u), cmul(gh, un));
+        }
+        __syncthreads();                                            // every partner value has been read
+        bfly16<true>(v);
+#pragma unroll
+        for (int j3 = 0; j3 < 16; ++j3) own[j3] = v[j3];
+    }
+    __syncwarp();
+    f16_pass2_inv(buf, tw);
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < NB; ++q) f16_pass1_inv<R1, true>(buf, q, x[q], tw);
+#pragma unroll
+    for (int ci = 0; ci < NC; ++ci) {
+        cplx *colT = colT_of[ci];
+        if (!colT) continue;
+        const double *vp = R.vpole + par_of[ci] * L;
+        const cplx xpole = s_pole[ci];
+#pragma unroll
+        for (int c = 0; c < HR; ++c) {
+            const int t = threadIdx.x + 256 * c;
+            if (t < Lm) {
+                const cplx y1 = x[2 * ci][c], y2 = x[2 * ci + 1][c];
+                const double dl = R.delta[t], ds = R.dsum[t], vv = vp[t];
+                cplx h = cmake(fma(dl, y1.x, -y2.x), fma(dl, y1.y, -y2.y));
+                if (t & 1) h = cscale(h, -1.0);
+                h.x += fma(ds, xs[ci][c].x, vv * xpole.x);
+                h.y += fma(ds, xs[ci][c].y, vv * xpole.y);
+                colT[t] = h;
+            } else if (t == Lm) {
+                cplx acc = cmake(0.0, 0.0);
+                for (int w = 0; w < 8; ++w) acc = cadd(acc, s_part[ci][w]);
+                colT[t] = acc;
+            }
+        }
+    }
+}
+
+// ---- plan time: kernel spectra in the core's own order --------------------------------------------------------------
+
+template <int R1>
+__global__ void __launch_bounds__(256) fft16_forward_kernel(cplx *data)
+{
+    extern __shared__ cplx buf[];
+    const F16Tw tw = f16_twiddles<R1>();
+    f16_forward_full<R1, true>(buf, data, data, tw);
+}
+
+// natural-order Bluestein kernels: kind 0: b[d mod M] = exp(+i pi d^2/n)/M, |d| < n (forward DFT); kind 1: conjugate
+__global__ void chirp_wrap_kernel(cplx *khat, int kind, int n, int M)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= M) return;
+    int d = e < n ? e : (e > M - n ? e - M : M);  // M: outside the support
+    cplx v = cmake(0.0, 0.0);
+    if (d != M) {
+        const long long r = ((long long)d * d) % (2LL * n);
+        double s, c;
+        sincospi((double)r / (double)n, &s, &c);
+        v = cscale(cmake(c, kind == 0 ? s : -s), 1.0 / (double)M);
+    }
+    khat[e] = v;
+}
+
+}  // namespace
+
+int launch_fft16_forward(cplx *data, int M, cudaStream_t st)
+{
+    const size_t sm = (size_t)F16_BUF * sizeof(cplx);
+    int rc;
+    if (M == 4096) {
+        if ((rc = set_smem(fft16_forward_kernel<16>, sm))) return rc;
+        S2W_LAUNCH(fft16_forward_kernel<16>, 1, 256, sm, st, data);
+    } else if (M == 2048) {
+        if ((rc = set_smem(fft16_forward_kernel<8>, sm))) return rc;
+        S2W_LAUNCH(fft16_forward_kernel<8>, 1, 256, sm, st, data);
+    } else if (M == 1024) {
+        if ((rc = set_smem(fft16_forward_kernel<4>, sm))) return rc;
+        S2W_LAUNCH(fft16_forward_kernel<4>, 1, 256, sm, st, data);
+    } else {
+        set_error("launch_fft16_forward: unsupported length");
+        return S2W_EINVAL;
+    }
+    return S2W_OK;
+}
+
+int launch_fft16_spectrum(cplx *khat, int kind, int n, int M, cudaStream_t st)
+{
+    S2W_LAUNCH(chirp_wrap_kernel, (M + 255) / 256, 256, 0, st, khat, kind, n, M);
+    return launch_fft16_forward(khat, M, st);
+}
+
+template <int R1>
+static int so3_pair16_t(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch,
+                        const FftTab &T, cudaStream_t st)
+{
+    constexpr int NB = 16 / R1;
+    const size_t sm = (size_t)F16_BUF * sizeof(cplx);
+    const int npairs = (T.L + 1) / 2;
+    dim3 grid((npairs + NB - 1) / NB, batch);
+    int rc;
+    if (fwd) {
+        if ((rc = set_smem(so3_fwd_pair16_kernel<R1>, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_SO3_FFT, so3_fwd_pair16_kernel<R1>, grid, 256, sm, st, (const double *)in, (cplx *)out,
+                     sig_stride, A, T);
+    } else {
+        if ((rc = set_smem(so3_inv_pair16_kernel<R1>, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_SO3_FFT, so3_inv_pair16_kernel<R1>, grid, 256, sm, st, (const cplx *)in, (double *)out,
+                     sig_stride, A, T);
+    }
+    return S2W_OK;
+}
+
+// real signals, 2N-1 <= 9, Bluestein length 1024 / 2048 / 4096 (the caller checks)
+int launch_so3_pair16(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch,
+                      const FftTab &T, cudaStream_t st)
+{
+    if (T.M == 4096) return so3_pair16_t<16>(fwd, in, out, sig_stride, A, batch, T, st);
+    if (T.M == 2048) return so3_pair16_t<8>(fwd, in, out, sig_stride, A, batch, T, st);
+    return so3_pair16_t<4>(fwd, in, out, sig_stride, A, batch, T, st);
+}
+
+// Toeplitz length 2048 / 1024 (the caller checks)
+int launch_reweight16(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st)
+{
+    const int ncol = A.Md * A.nn * batch;
+    const size_t sm = (size_t)F16_BUF * sizeof(cplx);
+    int rc;
+    if (R.fft.M == 2048) {
+        if ((rc = set_smem(reweight16_kernel<8>, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight16_kernel<8>, ncol, 256, sm, st, F, Ft, A, R, ncol);
+    } else {
+        if ((rc = set_smem(reweight16_kernel<4>, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight16_kernel<4>, (ncol + 1) / 2, 256, sm, st, F, Ft, A, R, ncol);
+    }
+    return S2W_OK;
+}
+
+}  // namespace s2w

@@ -15,6 +15,9 @@ namespace s2w {
 #define S2W_PAD(e) ((e) + ((e) >> 3))
 __host__ __device__ inline int fft_padded_len(int M) { return M + (M >> 3) + 1; }
 
+// lengths served by the radix-16 core (fft16_core.cuh)
+__host__ __device__ inline bool f16_supported(int M) { return M == 4096 || M == 2048 || M == 1024; }
+
 struct FftTab {
     int n;              // DFT length (2L-1)
     int L;              // band-limit of the grid
@@ -28,6 +31,7 @@ struct FftTab {
     const cplx *bhat_p; // [M]  same for exp(-i pi d^2/n)                                       (inverse DFT, sign +)
     const cplx *what;   // [M]  digit-reversed FFT of the wrapped quadrature kernel w(q), times 1/M   (reweighting)
     const cplx *rw_in1, *rw_out1, *rw_in3, *rw_out3;  // [n] each: reweighting phase tables (ring_fft.cu)
+    const cplx *bhat16_m, *bhat16_p;  // [M] the same spectra in the order of fft16_core.cuh (M = 1024, 2048, 4096), else null
 };
 
 // Tables of the Toeplitz/Hankel form of the theta reweighting (ring_fft.cu, reweight_th_kernel): length-M2 power-of-two
@@ -43,6 +47,7 @@ struct RwTab {
     const double *dsum;    // [L] (K_tt + K_{n-1-t,n-1-t}) / n
     const double *vpole;   // [2][L] pole column per parity (sigma = +1, -1), / n
     const double *rpole;   // [2][L] pole row per parity, / n
+    const cplx *TG16;      // [2][M2]: That, Ghat in the storage order of fft16_core.cuh's tables (M2 = 1024, 2048), else null
 };
 
 template <bool INV>

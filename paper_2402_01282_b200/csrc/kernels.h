@@ -83,6 +83,12 @@ int launch_reweight(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const F
 int launch_transpose(const cplx *src, cplx *dst, int R, int C, int nb, cudaStream_t st);
 int launch_reweight_th(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st);   // L >= 8, L <= 2048
 int launch_fft_forward(cplx *data, const FftTab &T, cudaStream_t st);   // plan-time, in place, digit-reversed out
+// the radix-16 core (fft16_kernels.cu), lengths 1024 / 2048 / 4096
+int launch_fft16_forward(cplx *data, int M, cudaStream_t st);           // plan-time, in place, the core's own order out
+int launch_fft16_spectrum(cplx *khat, int kind, int n, int M, cudaStream_t st);  // Bluestein kernel spectra (kind 0: -, 1: +)
+int launch_so3_pair16(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch,
+                      const FftTab &T, cudaStream_t st);                // a8, real signals, 2N-1 <= 9
+int launch_reweight16(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st);  // a2
 
 // plan-time: group start degrees and seeds from the range-extended values d^{l0}_{mn}(beta_t) = mant 2^expo ([ntab][Lg m][Lg t])
 int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int G,

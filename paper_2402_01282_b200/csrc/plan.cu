@@ -486,6 +486,43 @@ int build_rw(s2w_plan *p, GridTab &g)
     g.rw.vpole = dv;
     g.rw.rpole = dr;
     g.rw.L = L;
+    if (M2 == 2048 || M2 == 1024) {
+        // the same two spectra in the order of the radix-16 core (fft16_core.cuh), which is read off the transform of e_1
+        std::vector<cplx> h16((size_t)3 * M2, cmake(0.0, 0.0));
+        for (int i = 0; i < M2; ++i) {
+            h16[i] = cmake(H.kT[i], 0.0);
+            h16[(size_t)M2 + i] = cmake(H.kG[i], 0.0);
+        }
+        h16[(size_t)2 * M2 + 1] = cmake(1.0, 0.0);
+        cplx *d16;
+        if ((rc = p->pool.upload(&d16, h16))) return rc;
+        for (int a = 0; a < 3; ++a)
+            if ((rc = launch_fft16_forward(d16 + (size_t)a * M2, M2, 0))) return rc;
+        S2W_CUDA_CHECK(cudaMemcpy(h16.data(), d16, h16.size() * sizeof(cplx), cudaMemcpyDeviceToHost));
+        std::vector<cplx> tg16((size_t)2 * M2);
+        const int R1 = M2 / 256;
+        for (int q = 0; q < M2; ++q) {
+            const cplx v = h16[(size_t)2 * M2 + q];  // exp(-2 pi i k / M2)
+            long long k = llround(-std::atan2(v.y, v.x) * (double)M2 / (2.0 * pi_d()));
+            k %= M2;
+            if (k < 0) k += M2;
+            // launch_fft16_forward stores position p = j1 256 + j2 16 + j3 (frequency j1 + R1 (j2 + 16 j3)) at
+            // q = j1 256 + j3 16 + j2 (F16_TPOS)
+            if (k != (q >> 8) + R1 * ((q & 15) + 16 * ((q >> 4) & 15))) {
+                set_error("internal error: the radix-16 transform's order is not the documented one");
+                return S2W_ECUDA;
+            }
+            const long long j = (k * (Lm - 1)) % M2;  // reversal phase of the Hankel part
+            const ld ang = -2 * PI_L * (ld)j / (ld)M2;
+            const ld pr = cosl(ang), pi_ = sinl(ang);
+            const cplx gq = h16[(size_t)M2 + q];
+            tg16[q] = h16[q];
+            tg16[(size_t)M2 + q] = cmake((double)(gq.x * pr - gq.y * pi_), (double)(gq.x * pi_ + gq.y * pr));
+        }
+        cplx *dtg16;
+        if ((rc = p->pool.upload(&dtg16, tg16))) return rc;
+        g.rw.TG16 = dtg16;
+    }
     return S2W_OK;
 }
 
@@ -523,6 +560,15 @@ int build_grid(s2w_plan *p, int Lg)
     T.bhat_p = bp;
     T.what = wh;
     if ((rc = launch_fft_tables(T, chirp, i1, o1, i3, o3, bm, bp, wh, 0))) return rc;
+    if (f16_supported(T.M)) {  // the Bluestein spectra in the order of the radix-16 core
+        cplx *bm16, *bp16;
+        if ((rc = p->pool.alloc(&bm16, T.M))) return rc;
+        if ((rc = p->pool.alloc(&bp16, T.M))) return rc;
+        if ((rc = launch_fft16_spectrum(bm16, 0, T.n, T.M, 0))) return rc;
+        if ((rc = launch_fft16_spectrum(bp16, 1, T.n, T.M, 0))) return rc;
+        T.bhat16_m = bm16;
+        T.bhat16_p = bp16;
+    }
     if ((rc = build_rw(p, g))) return rc;
 
     std::vector<double> mant, yv;

@@ -8,8 +8,11 @@
 //
 // Real signals: W real  <=>  F_{-m,-n} = conj(F_mn).  The harmonic-side arrays then hold m = 0..L-1 only, two real
 // rings share one complex DFT in a1, and a8 transforms only the rows n >= 0.
+#include <cstdlib>
+
 #include "fft_core.cuh"
 #include "kernels.h"
+#include "smem_attr.cuh"
 
 namespace s2w {
 
@@ -1505,38 +1508,6 @@ __global__ void __launch_bounds__(256) transpose_kernel(const cplx *__restrict__
 
 size_t fft_smem_bytes(const FftTab &T) { return (size_t)fft_padded_len(T.M) * sizeof(cplx); }
 
-// Kernels that may need more than 48 KB of dynamic shared memory are raised to the device's opt-in limit, never to
-// the size of one launch: the attribute belongs to the function, not to the launch, so a per-launch value would be
-// lowered again by the next (smaller) launch -- under a captured graph, or with two host threads, that is a race with
-// the launches that still need the larger size.
-template <typename K>
-int set_smem(K kernel, size_t bytes)
-{
-    if (bytes > 48 * 1024) {
-        static int optin = 0;
-        if (!optin) {
-            int dev = 0;
-            cudaGetDevice(&dev);
-            if (cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) optin = 0;
-        }
-        cudaFuncAttributes fa;
-        if (cudaFuncGetAttributes(&fa, kernel) != cudaSuccess) fa.sharedSizeBytes = 0;
-        const int room = optin - (int)fa.sharedSizeBytes;  // the limit covers static + dynamic
-        if (room < 0 || (size_t)room < bytes) {
-            cudaGetLastError();
-            set_error("shared memory per block: the transform length needs more than the device offers");
-            return S2W_ECUDA;
-        }
-        if (fa.maxDynamicSharedSizeBytes == room) return S2W_OK;
-        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, room);
-        if (e != cudaSuccess) {
-            set_error(std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
-            return S2W_ECUDA;
-        }
-    }
-    return S2W_OK;
-}
-
 }  // namespace
 
 // ---- host launchers -------------------------------------------------------------------------------------------
@@ -1596,6 +1567,16 @@ int launch_ring_inv(bool real, const cplx *in, void *out, int B, int Lg, size_t 
 
 static int seqs_per_block(int fit, long long total, int cap);
 
+// S2W_FFT16=0 in the environment keeps the radix-8 kernels (before / after measurements); read once
+static bool use_fft16()
+{
+    static const bool on = [] {
+        const char *e = getenv("S2W_FFT16");
+        return !(e && e[0] == '0');
+    }();
+    return on;
+}
+
 template <bool REAL, bool MULTI>
 static int so3_launch_t(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch,
                         const FftTab &T, int rpb, cudaStream_t st)
@@ -1618,6 +1599,8 @@ static int so3_launch_t(bool fwd, const void *in, void *out, size_t sig_stride, 
 static int so3_launch(bool fwd, bool real, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch,
                       const FftTab &T, cudaStream_t st)
 {
+    if (real && 2 * A.N - 1 <= 9 && T.bhat16_m && f16_supported(T.M) && use_fft16())
+        return launch_so3_pair16(fwd, in, out, sig_stride, A, batch, T, st);
     const int rpb = seqs_per_block(4096 / T.M, (long long)T.L * batch, 32);
     if (rpb == 1 && real) {  // large grids, real signals: ring pairs (the n = 0 row shares one transform)
         const int ng = 2 * A.N - 1;
@@ -1686,6 +1669,7 @@ int launch_transpose(const cplx *src, cplx *dst, int R, int C, int nb, cudaStrea
 int launch_reweight_th(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st)
 {
     if (A.nn <= 0) return S2W_OK;
+    if (R.TG16 && (R.fft.M == 2048 || R.fft.M == 1024) && use_fft16()) return launch_reweight16(F, Ft, A, batch, R, st);
     const int ncol = A.Md * A.nn * batch;
     const int cpb = seqs_per_block(2048 / R.fft.M, ncol, RW_MAXCPB);
     size_t sm = 2 * (size_t)cpb * fft_padded_len(R.fft.M) * sizeof(cplx);
