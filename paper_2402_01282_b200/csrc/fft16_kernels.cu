@@ -259,7 +259,6 @@ __global__ void __launch_bounds__(256, 2) so3_fwd_pair16_kernel(const double *__
     const RowSet rs = so3_rows(A, -1, gph, s_rowp, s_rowm);
     const int q0 = rs.q0, np = rs.np;
     __syncthreads();
-    cplx x[NB][R1];
     // gather: every gamma plane of both rings of a pair once, two alpha samples (36 loads) at a time
 #pragma unroll 1
     for (int h = 0; h < 4; ++h) {
@@ -295,7 +294,10 @@ __global__ void __launch_bounds__(256, 2) so3_fwd_pair16_kernel(const double *__
                 y0 += wv[j][0][g];
                 y1 += wv[j][1][g];
             }
-            X2_SET(x, HR, h, j, cmul(cscale(cmake(y0, y1), inv_ng), ch[j]));
+            // round 0's input goes through the thread's own column slot of the buffer, not through 32 live registers: with
+            // them the 38 loads of a batch spilled, and a spill store of a just-loaded value waits for that load -- the
+            // batch's loads went out one DRAM round trip after the other (43 % of the kernel's samples sat here)
+            buf[F16_PAD(q * M + a)] = cmul(cscale(cmake(y0, y1), inv_ng), ch[j]);
 #pragma unroll
             for (int r = 0; r < 2; ++r) {
                 if (r == 0 ? !has0 : !has1) continue;
@@ -315,7 +317,12 @@ __global__ void __launch_bounds__(256, 2) so3_fwd_pair16_kernel(const double *__
             }
         }
     }
+    cplx x[NB][R1];
     if (q0 >= 0) {
+#pragma unroll
+        for (int q = 0; q < NB; ++q)
+#pragma unroll
+            for (int c = 0; c < HR; ++c) x[q][c] = buf[F16_PAD(q * M + threadIdx.x + 256 * c)];
         f16_convolve_half<R1>(buf, x, T.bhat16_m, tw);
         // u(k) = chirp(k) y(k) back into the thread's own column slots, then F0[m], F1[m] from u(m), u(n - m)
 #pragma unroll
