@@ -1,6 +1,9 @@
 """bench.py -- throughput of the fp64 directional wavelet transform (forward + inverse) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C3|C2|C1|C4]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C3|C2|C1|C4|C5|T2]
+
+`--gpus N` (N > 1) outside a launcher starts the N ranks itself (torch.distributed.run, one rank per GPU, rendezvous on
+127.0.0.1); under a launcher (WORLD_SIZE set) N must equal WORLD_SIZE.
 
 One "step" = one forward + one inverse transform of one batch of the workload (all hot-path steps a1-a8 of DESIGN.md).
 The default workload is BASELINE.json's metric configuration: L = 1024, N = 5, lambda = 2, J0 = 2, multiresolution,
@@ -50,6 +53,9 @@ def parse_args():
     ap.add_argument("--adjoint", action="store_true",
                     help="sphere workloads: time the adjoint pair S^H (signal -> coefficients) + A^H (coefficients -> "
                          "signal) of the workload's plan (SURVEY 8(f)-1); no e2e / cpu_baseline")
+    ap.add_argument("--dry-run-cpu", action="store_true",
+                    help="launcher check without GPUs: the N ranks rendezvous over gloo, report rank / seed offset / pid, "
+                         "run the MAX-over-ranks exchange on the CPU and rank 0 prints what it gathered")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -174,11 +180,34 @@ def make_signals(cfg, api, torch, device, seed_offset=0):
 # ---------------------------------------------------------------------------------------------------------------
 # CPU baseline: the oracle as it stands (double instance, OpenMP), on a bounded sample of the workload
 # ---------------------------------------------------------------------------------------------------------------
-def oracle_sample(cfg, nrings=None):
-    """Times the oracle's analysis of ONE signal restricted to the top wavelet scale and to `nrings` of its beta
-    rings (same sums, fewer outputs: oracle.sphere.analysis_from_flm(scales=, rings=)), and scales the time to one
-    full forward + inverse transform by the tuple counts of DESIGN.md (forward and inverse visit the same tuples).
-    Returns (transforms/s, cores, description, seconds)."""
+def _scale_stages(cfg):
+    """[(Lg, n_list, lmin)] of the oracle's contraction stages in ONE direction (all m of both signs)."""
+    from oracle import sphere as S
+    L, N, lam, J0, mr = cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"]
+    psi, phi, J = S.filters(L, N, lam, J0, "f64")
+    stages = [(L, [0], 0), (S.bandlimit_of_scaling(L, lam, J0, mr), [0], 0)]
+    for j in range(J0, J + 1):
+        Lj = S.bandlimit_of_scale(j, L, lam, mr)
+        a = np.abs(np.asarray(psi[j - J0][:Lj], dtype=np.complex128))
+        ns = [n for n in range(-(N - 1), N, 2) if abs(n) < Lj and a[:, n + N - 1].any()]
+        nz = np.nonzero(a.any(axis=1))[0]
+        if len(ns) and len(nz):
+            stages.append((Lj, ns, int(nz[0])))
+    return stages
+
+
+def _tuples_per_ring(Lg, ns, lmin):
+    m = np.abs(np.arange(-(Lg - 1), Lg))
+    return sum(int(np.clip(Lg - np.maximum(np.maximum(m, abs(n)), lmin), 0, None).sum()) for n in ns)
+
+
+def cpu_baseline(cfg, budget=1.0):
+    """The oracle as it stands (double instance, OpenMP, all host cores) on a bounded sample of the workload, every
+    O(L^3)-class part of it timed: (1) analysis-side contraction: oracle.sphere.analysis_from_flm of one signal on a
+    subset of the top scale's beta rings; (2) synthesis-side contraction: oracle.sphere.dl_forward of one row n on a
+    subset of rings; (3) the MW reweighting (R3 (ii)-(vi), O(L^2) per column) on a batch of columns of the top grid.
+    Each part is scaled to one full forward + inverse transform -- (1), (2) by (t, m, l, n) tuple count, (3) by column
+    count x (L_j / L_top)^2 -- and the three are added.  `budget` scales the sample sizes (1.0: about 10-30 s)."""
     from oracle import sphere as S
     from paper_2402_01282_b200 import inputs
     L, N, lam, J0, mr, real = cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"], cfg["real"]
@@ -186,70 +215,80 @@ def oracle_sample(cfg, nrings=None):
     flm = gen(L, cfg["seed"], 1, cfg["spectrum"])[0]
     filt = S.filters(L, N, lam, J0, "f64")
     psi, phi, J = filt
-    Lj = S.bandlimit_of_scale(J, L, lam, mr)
-    if nrings is None:
-        nrings = max(1, min(Lj, int(round(6.0e9 / (N * float(Lj) ** 2 * 4.0)))))  # ~10-30 s of CPU work
-    rings = np.unique(np.linspace(0, Lj - 1, nrings).astype(int))
+    stages = _scale_stages(cfg)
+    Lj, ns, lmin = stages[-1]
     S.wigner_d(8, 1, 0, 0.3, "f64")  # loads / builds the library outside the timed region
+    dir_tuples = sum(_tuples_per_ring(Lg, n_, lm_) * Lg for (Lg, n_, lm_) in stages)
+    # (1) analysis-side contraction
+    nr1 = max(1, min(Lj, int(round(budget * 6.0e9 / (N * float(Lj) ** 2 * 4.0)))))
+    rings = np.unique(np.linspace(0, Lj - 1, nr1).astype(int))
     t0 = time.perf_counter()
     S.analysis_from_flm(flm, L, N, lam, J0, mr, "f64", filt, scales=[J], rings={J: rings})
-    dt = time.perf_counter() - t0
-    # tuples of the sample (complex oracle: both signs of m) vs tuples of a full forward + inverse transform
-    a = np.abs(psi[J - J0][:Lj])
-    ns = [n for n in range(-(N - 1), N, 2) if abs(n) < Lj and a[:, n + N - 1].any()]
-    lmin = int(np.nonzero(a.any(axis=1))[0][0])
-    per_ring = 0
-    for n in ns:
-        m = np.abs(np.arange(-(Lj - 1), Lj))
-        per_ring += int(np.clip(Lj - np.maximum(np.maximum(m, abs(n)), lmin), 0, None).sum())
-    sample_tuples = per_ring * len(rings)
-    return dt, sample_tuples, S.num_threads("f64"), ("oracle analysis of 1 signal, top scale j=%d (L_j=%d), %d of %d "
-                                                    "beta rings; scaled by (t,m,l,n) tuple count" % (J, Lj, len(rings), Lj))
+    dt1 = time.perf_counter() - t0
+    tup1 = _tuples_per_ring(Lj, ns, lmin) * len(rings)
+    # (2) synthesis-side contraction: one row n, a subset of rings, all (l, m)
+    rng = np.random.default_rng(0)
+    nr2 = max(1, min(Lj, int(round(budget * 2.0e9 / (float(Lj) ** 2 * 2.0)))))
+    betas = S.mw_thetas(Lj, "f64")[np.unique(np.linspace(0, Lj - 1, nr2).astype(int))]
+    H = rng.standard_normal((2 * Lj - 1, betas.size)) + 1j * rng.standard_normal((2 * Lj - 1, betas.size))
+    t0 = time.perf_counter()
+    S.dl_forward(H, Lj, ns[-1], betas, "f64")
+    dt2 = time.perf_counter() - t0
+    tup2 = _tuples_per_ring(Lj, [ns[-1]], 0) * betas.size
+    # (3) reweighting columns of the top grid
+    nc = max(1, min(2 * Lj - 1, int(round(budget * 1.6e8 / float(Lj) ** 2))))
+    Fc = rng.standard_normal((nc, Lj)) + 1j * rng.standard_normal((nc, Lj))
+    t0 = time.perf_counter()
+    S.mw_reweight(Fc, Lj, np.ones(nc, dtype=np.int32), "f64")
+    dt3 = time.perf_counter() - t0
+    # forward transforms with reweighting: SHT of f at L (analysis), SHT of W^Phi at L_s and every scale (synthesis)
+    col_equiv = sum((2 * Lg - 1) * len(n_) * (Lg / float(Lj)) ** 2 for (Lg, n_, lm_) in stages)
+    est = dt1 * dir_tuples / max(tup1, 1) + dt2 * dir_tuples / max(tup2, 1) + dt3 * col_equiv / nc
+    return {"value": 1.0 / est, "unit": UNIT, "cores": S.num_threads("f64"), "kind": "oracle",
+            "sample": "contraction + reweighting, extrapolated: (1) oracle analysis of 1 signal, top scale j=%d (L_j=%d), "
+                      "%d of %d beta rings, %.1f s; (2) synthesis-side contraction dl_forward, row n=%d, %d rings, %.1f s; "
+                      "(3) MW reweighting of %d of the top grid's columns, %.1f s; scaled to one fwd+inv transform by "
+                      "tuple count (%.3g per direction) and column count -> %.0f s (contraction %.0f + %.0f, "
+                      "reweighting %.0f)"
+                      % (J, Lj, len(rings), Lj, dt1, ns[-1], betas.size, dt2, nc, dt3, dir_tuples, est,
+                         dt1 * dir_tuples / max(tup1, 1), dt2 * dir_tuples / max(tup2, 1), dt3 * col_equiv / nc)}
 
 
-def full_tuples_complex(cfg, api_or_none=None):
-    """(t, m, l, n) tuples of one forward + inverse transform as the oracle visits them (all m of both signs)."""
+def oracle_measured_small():
+    """One un-extrapolated oracle forward + inverse transform (double instance, all cores) of BASELINE config 2
+    (L = 256, N = 3, complex): the measured companion of the extrapolated C3 figure."""
     from oracle import sphere as S
-    L, N, lam, J0, mr = cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"]
-    psi, phi, J = S.filters(L, N, lam, J0, "f64")
-    tot = 0
-
-    def add(Lg, ns, lmin):
-        t = 0
-        m = np.abs(np.arange(-(Lg - 1), Lg))
-        for n in ns:
-            t += int(np.clip(Lg - np.maximum(np.maximum(m, abs(n)), lmin), 0, None).sum()) * Lg
-        return t
-    tot += add(L, [0], 0) + add(S.bandlimit_of_scaling(L, lam, J0, mr), [0], 0)
-    for j in range(J0, J + 1):
-        Lj = S.bandlimit_of_scale(j, L, lam, mr)
-        a = np.abs(np.asarray(psi[j - J0][:Lj], dtype=np.complex128))
-        ns = [n for n in range(-(N - 1), N, 2) if abs(n) < Lj and a[:, n + N - 1].any()]
-        nz = np.nonzero(a.any(axis=1))[0]
-        if len(ns) and len(nz):
-            tot += add(Lj, ns, int(nz[0]))
-    return 2 * tot  # analysis + synthesis
-
-
-def cpu_baseline(cfg):
-    dt, sample_tuples, cores, desc = oracle_sample(cfg)
-    full = full_tuples_complex(cfg)
-    est_seconds = dt * full / max(sample_tuples, 1)
-    return {"value": 1.0 / est_seconds, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": "%s; sample %.1f s = %.3g of the %.3g tuples of one fwd+inv transform (extrapolated)"
-                      % (desc, dt, sample_tuples / full, full)}
+    from paper_2402_01282_b200 import inputs
+    c = inputs.CONFIGS["C2"]
+    L, N, lam, J0 = c["L"], c["N"], c["lam"], c["J0"]
+    flm = inputs.config_coefficients("C2")[0]
+    filt = S.filters(L, N, lam, J0, "f64")
+    f = S.sht_inverse(flm, L, "f64")
+    t0 = time.perf_counter()
+    phi, psi = S.analysis(f, L, N, lam, J0, True, "f64", filt)
+    back = S.synthesis(phi, psi, L, N, lam, J0, True, "f64", filt)
+    dt = time.perf_counter() - t0
+    return {"workload": "C2: sphere L=256 N=3 lambda=2 J0=2 multires complex, forward+inverse, whole transform timed",
+            "value": 1.0 / dt, "unit": UNIT, "seconds": dt, "cores": S.num_threads("f64"),
+            "roundtrip_rel_err": float(np.abs(back - f).max() / np.abs(f).max())}
 
 
 def run_reference(args, cfg):
     """--impl reference: the oracle as it stands on the host cores; each step is one bounded sample."""
+    from paper_2402_01282_b200 import api
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    args.gpus = world
+    cfg["coeff_gb"] = (api._coeff_elems_sphere(cfg["L"], cfg["N"], cfg["lam"], cfg["J0"], cfg["multires"])
+                       * cfg["batch"] * (8 if cfg["real"] else 16) / 1e9)
     vals, base = [], None
     for i in range(args.warmup + args.steps):
-        base = cpu_baseline(cfg)
+        base = cpu_baseline(cfg, budget=0.25)
         if i >= args.warmup:
             vals.append(base["value"])
     v = float(np.mean(vals))
     base["value"] = v
-    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+    base["measured_small"] = oracle_measured_small()
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * cfg["batch"] / v,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": workload_config(cfg, args), "cpu_baseline": base,
@@ -274,7 +313,7 @@ def workload_config(cfg, args):
 # no data-path collective; the only exchange is this MAX over the ranks' device times.
 # ---------------------------------------------------------------------------------------------------------------
 def replica_seed_offset(rank):
-    """Rank r draws its signals from seed + 1000 r: independent signals per replica."""
+    """Seed offset of rank r (make_signals draws its signals from seed + 1000 r): independent signals per replica."""
     return int(rank)
 
 
@@ -451,6 +490,7 @@ def run_ours(args, cfg):
                        "d2h_bytes_per_step": e2e["d2h"], "roundtrip_rel_err": e2e["rt_err"]}
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(cfg)
+        line["cpu_baseline"]["measured_small"] = oracle_measured_small()
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -590,8 +630,55 @@ def run_ball(args, cfg):
 
 
 
+def free_port():
+    import socket
+    with socket.socket(socket.AF_INET, socket.SOCK_STREAM) as sk:
+        sk.bind(("127.0.0.1", 0))
+        return sk.getsockname()[1]
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` outside a launcher: start N ranks of this same command, one per GPU, under
+    torch.distributed.run (what the driver does itself for N > 1) and return its exit code."""
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")            # the communicator log shows the N ranks (stderr)
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd, env=env)
+
+
+def run_dry(args):
+    """--dry-run-cpu: every rank joins a gloo group and reports itself; no transform runs."""
+    import torch
+    import torch.distributed as dist
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    me = {"rank": rank, "local_rank": int(os.environ.get("LOCAL_RANK", "0")), "pid": os.getpid(),
+          "seed_offset": replica_seed_offset(rank)}
+    everyone = [me]
+    if world > 1:
+        everyone = [None] * world
+        dist.all_gather_object(everyone, me)
+    ms, = max_over_ranks([10.0 + rank], world, torch.device("cpu"))
+    if rank == 0:
+        print(json.dumps({"dry_run": True, "n_gpus": world, "ranks": everyone, "ms_max": ms,
+                          "value": whole_job_value(world, 4, args.steps, ms), "unit": UNIT}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     args = parse_args()
+    world_env = os.environ.get("WORLD_SIZE")
+    if world_env is None and args.gpus > 1:
+        raise SystemExit(spawn_ranks(args))
+    if world_env is not None and int(world_env) != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but the launcher started WORLD_SIZE=%s ranks" % (args.gpus, world_env))
+    if args.dry_run_cpu:
+        run_dry(args)
+        return
     from paper_2402_01282_b200 import inputs
     cfg = dict(inputs.CONFIGS[args.workload])
     cfg["name"] = args.workload

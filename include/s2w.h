@@ -73,7 +73,7 @@ int s2ball_radial_nodes(double *r, double *q, int P, double tau);
  * Creation allocates device tables, runs set-up kernels and synchronises. */
 int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int multiresolution,
                       int flags, int batch, int device);
-/* The same for a spin-s signal (Eq. 1; Eq. 12): the signal and the scaling coefficients are expanded
+/* The same for a spin-s signal (spin fields: Eq. 1, Eq. 12; the formula of sY_lm is reading R2, Goldberg et al. 1967 convention -- the paper prints none): the signal and the scaling coefficients are expanded
  * in spin-weighted harmonics sY_lm = (-1)^s sqrt((2l+1)/4pi) d^l_{m,-s}(theta) e^{i m phi} (f_lm = 0 below l = |s|),
  * the wavelet coefficients on SO(3) are as in the scalar case.  spin != 0 needs a complex plan and |spin| < L
  * (S2W_EINVAL otherwise); spin = 0 is s2wav_plan_create. */

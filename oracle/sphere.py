@@ -303,7 +303,7 @@ def mw_reweight(F, L, sigma, prec):
 
 
 # --------------------------------------------------------------------------
-# O2 / O3: spherical harmonic transforms Y^-1, Y (Eqs. 2-3), spin s (Eq. 1):
+# O2 / O3: spherical harmonic transforms Y^-1, Y (Eqs. 2-3), spin s (sY_lm by reading R2, Goldberg et al. 1967 convention; the paper prints no formula):
 #   sY_{lm}(theta, phi) = (-1)^s sqrt((2l+1)/4pi) D^{l*}_{m,-s}(phi, theta, 0)
 #                       = (-1)^s sqrt((2l+1)/4pi) d^l_{m,-s}(theta) e^{i m phi},      zero for l < |s|.
 # --------------------------------------------------------------------------
@@ -434,7 +434,7 @@ def analysis_from_flm(flm, L, N, lam, J0, multires, prec="f80", filt=None, scale
 
 
 def analysis(f, L, N, lam, J0, multires, prec="f80", filt=None, spin=0):
-    """Algorithm 1 'Analysis wavelet transform'; `spin`: the signal's spin number (Eq. 1)."""
+    """Algorithm 1 'Analysis wavelet transform'; `spin`: the signal's spin number (spin fields: Eq. 1; sY_lm: reading R2)."""
     flm = sht_forward(f, L, prec, spin=spin)                      # f_hat <- Y f
     return analysis_from_flm(flm, L, N, lam, J0, multires, prec, filt, spin=spin)
 

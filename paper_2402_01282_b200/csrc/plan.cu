@@ -150,7 +150,7 @@ struct s2w_plan {
     bool real;
     DevPool pool;
     std::vector<GridTab> grids;
-    int spin;               // spin number s of the signal (Eq. 1): the SHT stages contract with d^l_{m,-s}
+    int spin;               // spin number s of the signal (spin fields: Eq. 1): the SHT stages contract with d^l_{m,-s}
     std::vector<int> tabn;  // table values of n: script-N united with {-spin, +spin}
     double *coef;
     size_t tri;
@@ -755,7 +755,7 @@ int make_n0_stage(s2w_plan *p, Stage &st, int Lg, const std::vector<double> &a, 
     st.grid = grid_index(p, Lg);
     st.Lg = Lg;
     st.lmin = 0;
-    // spin-s harmonics sY_lm = (-1)^s sqrt((2l+1)/4pi) d^l_{m,-s}(theta) e^{i m phi} (Eq. 1): the row n = -s, zero
+    // spin-s harmonics sY_lm = (-1)^s sqrt((2l+1)/4pi) d^l_{m,-s}(theta) e^{i m phi} (reading R2, Goldberg convention): the row n = -s, zero
     // below l = |s| (the contraction kernels start at max(|m|, |n|)); no row at all when the band-limit is <= |s|.
     // The kernels pair the column (m, n) with (-m, -n) (one recursion serves both), so for s != 0 the stage carries
     // the recursions of n = -s (columns m >= 0 of row 0) and n = +s (whose mirror columns are (-m, -s): the m < 0 half of

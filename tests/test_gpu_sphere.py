@@ -299,7 +299,10 @@ def test_two_plans_and_a_side_stream():
             wa = pa.forward(fa)
         wb = pb.forward(fb)
         torch.cuda.synchronize()
-        assert torch.equal(wa, ref_a) and torch.equal(wb, ref_b)
+        # by tolerance, not bitwise: the forward SHT adds eight warps' partial sums with shared-memory atomics, in any
+        # order (reading R16)
+        assert float((wa - ref_a).abs().max()) <= 1e-12 * float(ref_a.abs().max())
+        assert float((wb - ref_b).abs().max()) <= 1e-12 * float(ref_b.abs().max())
     back = pa.inverse(wa).cpu().numpy().reshape(f_a.shape)
     assert _relmax(back, f_a) < RT_TOL
     pa.close()

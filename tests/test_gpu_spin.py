@@ -1,4 +1,4 @@
-"""GPU parity tests of spin-s plans (Eq. 1, Eq. 12): s2wav_plan_create_spin through the
+"""GPU parity tests of spin-s plans (spin fields: Eq. 1, Eq. 12; sY_lm by reading R2): s2wav_plan_create_spin through the
 C ABI against the oracle's spin transforms on the same seeded inputs -- harmonic transform, wavelet coefficients,
 round trip, adjoint identity.  Tolerances as for spin 0."""
 import numpy as np

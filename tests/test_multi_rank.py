@@ -64,3 +64,33 @@ def test_single_rank_is_identity():
     import bench
     assert bench.max_over_ranks([3.0, 1.0], 1, torch.device("cpu")) == [3.0, 1.0]
     assert bench.whole_job_value(1, 4, 10, 50.0) == 4 * 10 / 50e-3
+
+
+def test_bench_gpus_n_starts_n_ranks():
+    """`python bench.py --gpus 2` outside a launcher must itself start 2 ranks (it ran one rank and
+    printed n_gpus 1).  --dry-run-cpu: the ranks rendezvous over gloo on 127.0.0.1 and report themselves, no GPU."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR",
+                                                           "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "5", "--dry-run-cpu"],
+                       capture_output=True, text=True, timeout=300, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1                                   # rank 0 alone prints
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2
+    ranks = d["ranks"]
+    assert sorted(x["rank"] for x in ranks) == [0, 1]
+    assert len({x["pid"] for x in ranks}) == 2               # two processes
+    assert len({x["seed_offset"] for x in ranks}) == 2       # distinct seeds per replica
+    assert d["ms_max"] == 11.0                               # MAX over the ranks' times (10 + rank)
+    assert abs(d["value"] - 2 * 4 * 5 / 11.0e-3) < 1e-9
+
+
+def test_bench_rejects_a_world_size_that_contradicts_gpus():
+    import subprocess
+    env = dict(os.environ, WORLD_SIZE="3", RANK="0", LOCAL_RANK="0")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-run-cpu"],
+                       capture_output=True, text=True, timeout=120, env=env)
+    assert r.returncode != 0 and "WORLD_SIZE=3" in (r.stderr + r.stdout)

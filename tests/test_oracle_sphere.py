@@ -103,6 +103,20 @@ def test_wigner_d_unitarity(prec, L, tol):
             assert np.abs(tot[n:] - 1).max() < tol
 
 
+def test_wigner_d_unitarity_at_band_limit_2048():
+    """The same identity on MW rings of the L = 2048 grid for the long-double parity reference ("incl.
+    L=2048 rings -- this one catches the underflow bug"): ring 156 is where the plain double seed of m = 480 is 1e-300
+    (SURVEY 7-1); the polar rings are where the plain three-term recursion loses the most digits."""
+    L = 2048
+    th = S.mw_thetas(L, "f80")
+    for t, tol in ((0, 1e-12), (156, 1e-14), (1024, 1e-14), (2046, 1e-12)):
+        for n in (0, 2):
+            tot = np.zeros(L, dtype=S.REAL["f80"])
+            for m in range(-(L - 1), L):
+                tot += S.wigner_d(L, m, n, th[t], "f80") ** 2
+            assert np.abs(tot[n:] - 1).max() < tol, (t, n)
+
+
 def test_wigner_d_legendre_and_jacobi():
     L, beta = 40, 1.234
     d = S.wigner_d(L, 0, 0, LD(beta)).astype(float)

@@ -1,4 +1,4 @@
-"""CPU pins of the oracle's spin-s harmonic transforms (Eq. 1: sY_lm = (-1)^s sqrt((2l+1)/4pi) D^{l*}_{m,-s}):
+"""CPU pins of the oracle's spin-s harmonic transforms (reading R2, Goldberg et al. 1967 convention -- the paper prints no formula; its Eq. 1, is the transformation law: sY_lm = (-1)^s sqrt((2l+1)/4pi) D^{l*}_{m,-s}):
 textbook closed forms of the spin-weighted harmonics (Goldberg et al. 1967 phase, the one Eq. 1 reproduces), their
 orthonormality through the exact MW quadrature, exact forward o inverse on band-limited spin signals, and exact
 reconstruction of the spin wavelet transform."""
