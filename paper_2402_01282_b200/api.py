@@ -137,9 +137,33 @@ def _torch():
     return torch
 
 
-def _stream_ptr():
+def _stream_ptr(device=None):
+    """The current stream of `device` (a tensor's device; default: the current device)."""
     torch = _torch()
-    return _c_vp(torch.cuda.current_stream().cuda_stream)
+    return _c_vp(torch.cuda.current_stream(device).cuda_stream)
+
+
+def _dtype_real(dt):
+    """True for float64 (S2W_REAL), False for complex128; any other dtype would be read out of bounds by the library."""
+    name = str(dt).replace("torch.", "")
+    if name == "float64":
+        return True
+    if name == "complex128":
+        return False
+    raise ValueError("expected float64 (real signals) or complex128, got %s" % dt)
+
+
+def _whole(n, unit, what):
+    if unit <= 0 or n == 0 or n % unit:
+        raise ValueError("%s: %d elements is not a whole number of blocks of %d" % (what, n, unit))
+    return n // unit
+
+
+def _check_tensor(t, dtype, elems, what):
+    """Argument marshalling guard: the library reads / writes `elems` elements of `dtype` behind the pointer."""
+    if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype and t.numel() == elems):
+        raise ValueError("%s: expected a contiguous CUDA tensor of dtype %s with %d elements, got %s %s with %d"
+                         % (what, dtype, elems, "cuda" if t.is_cuda else "cpu", t.dtype, t.numel()))
 
 
 class Plan:
@@ -194,50 +218,52 @@ class Plan:
             return [(j, 0) for j in range(self.J0, self.J + 1)]
         return [(j, jp) for jp in range(self.J0p, self.Jp + 1) for j in range(self.J0, self.J + 1)]
 
-    def _check_in(self, t, elems):
+    def _check_in(self, t, elems, what="input"):
+        _check_tensor(t, self.dtype, elems * self.batch, what)
+
+    def _out(self, out, elems, like):
         torch = _torch()
-        if not (t.is_cuda and t.is_contiguous() and t.dtype == self.dtype and t.numel() == elems * self.batch):
-            raise ValueError("expected a contiguous CUDA tensor of dtype %s with %d elements"
-                             % (self.dtype, elems * self.batch))
+        if out is None:
+            return torch.empty((self.batch, elems), dtype=self.dtype, device=like.device)
+        self._check_in(out, elems, "out")
+        if out.device != like.device:
+            raise ValueError("out: on %s, the input is on %s" % (out.device, like.device))
+        return out
 
     def forward(self, f, out=None):
         """Analysis: signal(s) -> packed coefficient tensor [batch][coeff_elems]."""
         torch = _torch()
         self._check_in(f, self.signal_elems)
-        if out is None:
-            out = torch.empty((self.batch, self.coeff_elems), dtype=self.dtype, device=f.device)
+        out = self._out(out, self.coeff_elems, f)
         _check(lib().s2w_plan_forward(self._h, f.data_ptr(), out.data_ptr(), self._workspace(f.device).data_ptr(),
-                                      _stream_ptr()))
+                                      _stream_ptr(f.device)))
         return out
 
     def inverse(self, w, out=None, shape=None):
         """Synthesis: packed coefficients -> signal(s)."""
         torch = _torch()
         self._check_in(w, self.coeff_elems)
-        if out is None:
-            out = torch.empty((self.batch, self.signal_elems), dtype=self.dtype, device=w.device)
+        out = self._out(out, self.signal_elems, w)
         _check(lib().s2w_plan_inverse(self._h, w.data_ptr(), out.data_ptr(), self._workspace(w.device).data_ptr(),
-                                      _stream_ptr()))
+                                      _stream_ptr(w.device)))
         return out if shape is None else out.view(shape)
 
     def forward_adjoint(self, y, out=None):
         """Adjoint of the analysis: coefficient-shaped y -> signal-shaped A^H y (s2w_plan_forward_adjoint)."""
         torch = _torch()
         self._check_in(y, self.coeff_elems)
-        if out is None:
-            out = torch.empty((self.batch, self.signal_elems), dtype=self.dtype, device=y.device)
+        out = self._out(out, self.signal_elems, y)
         _check(lib().s2w_plan_forward_adjoint(self._h, y.data_ptr(), out.data_ptr(),
-                                              self._workspace(y.device).data_ptr(), _stream_ptr()))
+                                              self._workspace(y.device).data_ptr(), _stream_ptr(y.device)))
         return out
 
     def inverse_adjoint(self, g, out=None):
         """Adjoint of the synthesis: signal-shaped g -> coefficient-shaped S^H g (s2w_plan_inverse_adjoint)."""
         torch = _torch()
         self._check_in(g, self.signal_elems)
-        if out is None:
-            out = torch.empty((self.batch, self.coeff_elems), dtype=self.dtype, device=g.device)
+        out = self._out(out, self.coeff_elems, g)
         _check(lib().s2w_plan_inverse_adjoint(self._h, g.data_ptr(), out.data_ptr(),
-                                              self._workspace(g.device).data_ptr(), _stream_ptr()))
+                                              self._workspace(g.device).data_ptr(), _stream_ptr(g.device)))
         return out
 
     def harmonic_forward(self, f, flm_elems):
@@ -245,14 +271,16 @@ class Plan:
         self._check_in(f, self.signal_elems)
         out = torch.empty((self.batch, flm_elems), dtype=torch.complex128, device=f.device)
         _check(lib().s2w_plan_harmonic_forward(self._h, f.data_ptr(), out.data_ptr(),
-                                               self._workspace(f.device).data_ptr(), _stream_ptr()))
+                                               self._workspace(f.device).data_ptr(), _stream_ptr(f.device)))
         return out
 
     def harmonic_inverse(self, flm):
         torch = _torch()
+        if flm.numel() % self.batch or not (flm.is_cuda and flm.is_contiguous() and flm.dtype == torch.complex128):
+            raise ValueError("flm: expected a contiguous complex128 CUDA tensor [batch, ...]")
         out = torch.empty((self.batch, self.signal_elems), dtype=self.dtype, device=flm.device)
         _check(lib().s2w_plan_harmonic_inverse(self._h, flm.data_ptr(), out.data_ptr(),
-                                               self._workspace(flm.device).data_ptr(), _stream_ptr()))
+                                               self._workspace(flm.device).data_ptr(), _stream_ptr(flm.device)))
         return out
 
     def split(self, w):
@@ -316,12 +344,12 @@ def s2wav_forward(f, L, N, lam, J0, multiresolution=True):
     """f: CUDA tensor [batch, L, 2L-1] (float64 -> S2W_REAL, complex128 otherwise) -> packed coefficients [batch, K]."""
     torch = _torch()
     f = f.contiguous()
-    batch = f.numel() // (L * (2 * L - 1))
-    real = f.dtype == torch.float64
+    batch = _whole(f.numel(), L * (2 * L - 1), "f")
+    real = _dtype_real(f.dtype)
     K = _coeff_elems_sphere(L, N, lam, J0, multiresolution)
     w = torch.empty((batch, K), dtype=f.dtype, device=f.device)
     _check(lib().s2wav_forward(f.data_ptr(), w.data_ptr(), int(L), int(N), float(lam), int(J0),
-                               int(bool(multiresolution)), S2W_REAL if real else 0, batch, _stream_ptr()))
+                               int(bool(multiresolution)), S2W_REAL if real else 0, batch, _stream_ptr(f.device)))
     return w
 
 
@@ -330,11 +358,11 @@ def s2wav_inverse(w, L, N, lam, J0, multiresolution=True):
     torch = _torch()
     w = w.contiguous()
     K = _coeff_elems_sphere(L, N, lam, J0, multiresolution)
-    batch = w.numel() // K
-    real = w.dtype == torch.float64
+    batch = _whole(w.numel(), K, "w")
+    real = _dtype_real(w.dtype)
     f = torch.empty((batch, L, 2 * L - 1), dtype=w.dtype, device=w.device)
     _check(lib().s2wav_inverse(w.data_ptr(), f.data_ptr(), int(L), int(N), float(lam), int(J0),
-                               int(bool(multiresolution)), S2W_REAL if real else 0, batch, _stream_ptr()))
+                               int(bool(multiresolution)), S2W_REAL if real else 0, batch, _stream_ptr(w.device)))
     return f
 
 
@@ -350,8 +378,8 @@ def _host_out(out, shape, dtype):
 def s2wav_forward_host(f, L, N, lam, J0, multiresolution=True, out=None):
     """numpy in, numpy out; host<->device copies happen inside the library call."""
     f = np.ascontiguousarray(f)
-    real = f.dtype == np.float64
-    batch = f.size // (L * (2 * L - 1))
+    real = _dtype_real(f.dtype)
+    batch = _whole(f.size, L * (2 * L - 1), "f")
     K = _coeff_elems_sphere(L, N, lam, J0, multiresolution)
     w = _host_out(out, (batch, K), f.dtype)
     _check(lib().s2wav_forward_host(_np_ptr(f), _np_ptr(w), int(L), int(N), float(lam), int(J0),
@@ -361,9 +389,9 @@ def s2wav_forward_host(f, L, N, lam, J0, multiresolution=True, out=None):
 
 def s2wav_inverse_host(w, L, N, lam, J0, multiresolution=True, out=None):
     w = np.ascontiguousarray(w)
-    real = w.dtype == np.float64
+    real = _dtype_real(w.dtype)
     K = _coeff_elems_sphere(L, N, lam, J0, multiresolution)
-    batch = w.size // K
+    batch = _whole(w.size, K, "w")
     f = _host_out(out, (batch, L, 2 * L - 1), w.dtype)
     _check(lib().s2wav_inverse_host(_np_ptr(w), _np_ptr(f), int(L), int(N), float(lam), int(J0),
                                     int(bool(multiresolution)), S2W_REAL if real else 0, batch))
@@ -391,26 +419,30 @@ def s2ball_forward(f, L, P, N, lam_l, lam_p, J0, tau=1.0):
     """f: CUDA tensor [P, L, 2L-1] on the Gauss-Laguerre shells -> packed coefficients [K]."""
     torch = _torch()
     f = f.contiguous()
-    real = f.dtype == torch.float64
+    real = _dtype_real(f.dtype)
+    if not f.is_cuda or f.numel() != P * L * (2 * L - 1):
+        raise ValueError("f: expected a CUDA tensor of %d elements [P, L, 2L-1]" % (P * L * (2 * L - 1)))
     w = torch.empty(_coeff_elems_ball(L, P, N, lam_l, lam_p, J0), dtype=f.dtype, device=f.device)
     _check(lib().s2ball_forward(f.data_ptr(), w.data_ptr(), int(L), int(P), int(N), float(lam_l), float(lam_p),
-                                int(J0), float(tau), S2W_REAL if real else 0, _stream_ptr()))
+                                int(J0), float(tau), S2W_REAL if real else 0, _stream_ptr(f.device)))
     return w
 
 
 def s2ball_inverse(w, L, P, N, lam_l, lam_p, J0, tau=1.0):
     torch = _torch()
     w = w.contiguous()
-    real = w.dtype == torch.float64
+    real = _dtype_real(w.dtype)
+    if not w.is_cuda or w.numel() != _coeff_elems_ball(L, P, N, lam_l, lam_p, J0):
+        raise ValueError("w: expected a CUDA tensor of %d elements" % _coeff_elems_ball(L, P, N, lam_l, lam_p, J0))
     f = torch.empty((P, L, 2 * L - 1), dtype=w.dtype, device=w.device)
     _check(lib().s2ball_inverse(w.data_ptr(), f.data_ptr(), int(L), int(P), int(N), float(lam_l), float(lam_p),
-                                int(J0), float(tau), S2W_REAL if real else 0, _stream_ptr()))
+                                int(J0), float(tau), S2W_REAL if real else 0, _stream_ptr(w.device)))
     return f
 
 
 def s2ball_forward_host(f, L, P, N, lam_l, lam_p, J0, tau=1.0, out=None):
     f = np.ascontiguousarray(f)
-    real = f.dtype == np.float64
+    real = _dtype_real(f.dtype)
     w = _host_out(out, (_coeff_elems_ball(L, P, N, lam_l, lam_p, J0),), f.dtype)
     _check(lib().s2ball_forward_host(_np_ptr(f), _np_ptr(w), int(L), int(P), int(N), float(lam_l), float(lam_p),
                                      int(J0), float(tau), S2W_REAL if real else 0))
@@ -419,7 +451,7 @@ def s2ball_forward_host(f, L, P, N, lam_l, lam_p, J0, tau=1.0, out=None):
 
 def s2ball_inverse_host(w, L, P, N, lam_l, lam_p, J0, tau=1.0, out=None):
     w = np.ascontiguousarray(w)
-    real = w.dtype == np.float64
+    real = _dtype_real(w.dtype)
     f = _host_out(out, (P, L, 2 * L - 1), w.dtype)
     _check(lib().s2ball_inverse_host(_np_ptr(w), _np_ptr(f), int(L), int(P), int(N), float(lam_l), float(lam_p),
                                      int(J0), float(tau), S2W_REAL if real else 0))

@@ -25,6 +25,7 @@ __device__ __forceinline__ cplx cscale(cplx a, double s) { return make_double2(a
 
 void set_error(const std::string &msg);
 void count_launch();
+void debug_launch(const char *name);  // S2W_DEBUG_LAUNCH=1: report the first launch that leaves a CUDA error behind
 
 #define S2W_CUDA_CHECK(expr)                                                                       \
     do {                                                                                           \
@@ -48,6 +49,7 @@ void timing_end(cudaStream_t st);
         kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);                                \
         s2w::timing_end((stream));                                                                 \
         s2w::count_launch();                                                                       \
+        s2w::debug_launch(#kernel);                                                                \
     } while (0)
 #define S2W_LAUNCH(kernel, grid, block, smem, stream, ...)                                         \
     S2W_LAUNCH_C(s2w::S2W_K_OTHER, kernel, grid, block, smem, stream, __VA_ARGS__)

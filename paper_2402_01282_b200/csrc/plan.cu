@@ -10,6 +10,7 @@
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
+#include <functional>
 #include <map>
 #include <mutex>
 #include <string>
@@ -25,6 +26,17 @@ static thread_local std::string g_err;
 static unsigned long long g_launches = 0;
 void set_error(const std::string &msg) { g_err = msg; }
 void count_launch() { ++g_launches; }
+void debug_launch(const char *name)
+{
+    static const bool on = getenv("S2W_DEBUG_LAUNCH") != 0;
+    if (!on) return;
+    static bool reported = false;
+    const cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess && !reported) {
+        reported = true;
+        fprintf(stderr, "[s2w] launch of %s left the error: %s\n", name, cudaGetErrorString(e));
+    }
+}
 
 // ---- per-class device timers: cudaEvent pairs around every launch while enabled (s2w_timing_enable/read) ----
 namespace {
@@ -2038,12 +2050,28 @@ static int run_transform(const s2w_plan *p, int dir, const void *in, void *out, 
     return S2W_OK;
 }
 
+// A plan's tables, streams and events live on the device it was created for; its kernels must be launched with that
+// device current (nothing checked this, so a call from another device's context launched on the wrong GPU).
+static int check_device(const s2w_plan *p)
+{
+    int dev = -1;
+    S2W_CUDA_CHECK(cudaGetDevice(&dev));
+    if (dev != p->device) {
+        set_error("the current CUDA device (" + std::to_string(dev) + ") is not the plan's device (" +
+                  std::to_string(p->device) + "): call cudaSetDevice / torch.cuda.set_device first");
+        return S2W_EINVAL;
+    }
+    return S2W_OK;
+}
+
 int s2w_plan_forward(const s2w_plan *p, const void *in, void *out, void *work, void *stream)
 {
     if (!p || !in || !out || !work) {
         set_error("null pointer");
         return S2W_EINVAL;
     }
+    int rc = check_device(p);
+    if (rc) return rc;
     return run_transform(p, 0, in, out, align256(work), (cudaStream_t)stream);
 }
 
@@ -2053,6 +2081,8 @@ int s2w_plan_inverse(const s2w_plan *p, const void *in, void *out, void *work, v
         set_error("null pointer");
         return S2W_EINVAL;
     }
+    int rc = check_device(p);
+    if (rc) return rc;
     return run_transform(p, 1, in, out, align256(work), (cudaStream_t)stream);
 }
 
@@ -2061,6 +2091,10 @@ static int adjoint_supported(const s2w_plan *p, const void *in, const void *out,
     if (!p || !in || !out || !work) {
         set_error("null pointer");
         return S2W_EINVAL;
+    }
+    {
+        int rcd = check_device(p);
+        if (rcd) return rcd;
     }
     return S2W_OK;
 }
@@ -2084,6 +2118,10 @@ int s2w_plan_harmonic_forward(const s2w_plan *p, const void *f, void *flm, void 
     if (!p || !f || !flm || !work) {
         set_error("null pointer");
         return S2W_EINVAL;
+    }
+    {
+        int rcd = check_device(p);
+        if (rcd) return rcd;
     }
     cudaStream_t s = (cudaStream_t)stream;
     int rc;
@@ -2111,6 +2149,10 @@ int s2w_plan_harmonic_inverse(const s2w_plan *p, const void *flm, void *f, void 
     if (!p || !f || !flm || !work) {
         set_error("null pointer");
         return S2W_EINVAL;
+    }
+    {
+        int rcd = check_device(p);
+        if (rcd) return rcd;
     }
     cudaStream_t s = (cudaStream_t)stream;
     int rc;
@@ -2143,11 +2185,32 @@ struct CacheKey {
         return std::memcmp(this, &o, sizeof(CacheKey)) < 0;
     }
 };
+// Users of one cache entry share ONE workspace and one pair of staging buffers: they are serialised.  Host
+// threads take `mu` for the duration of their launches; on the device every use waits for the event the previous use
+// recorded on its own stream, so two calls with the same parameters on different streams run one after the other.
+struct EntrySync {
+    std::mutex mu;
+    cudaEvent_t done;
+    bool used;
+    cudaStream_t copy_stream;  // second stream of the host-buffer pipeline, created on the entry's device
+};
 struct CacheEntry {
     s2w_plan *plan;
     void *work;
     void *d_sig, *d_cof;  // device staging buffers of the host-buffer entry points (allocated on first use)
+    EntrySync *sync;
 };
+
+// run `fn(stream)` as the next user of entry `e` on `stream`
+int entry_serialised(const CacheEntry &e, cudaStream_t stream, const std::function<int(cudaStream_t)> &fn)
+{
+    std::lock_guard<std::mutex> lock(e.sync->mu);
+    if (e.sync->used) S2W_CUDA_CHECK(cudaStreamWaitEvent(stream, e.sync->done, 0));
+    const int rc = fn(stream);
+    S2W_CUDA_CHECK(cudaEventRecord(e.sync->done, stream));
+    e.sync->used = true;
+    return rc;
+}
 std::map<CacheKey, CacheEntry> g_cache;
 std::mutex g_cache_mu;
 
@@ -2177,6 +2240,7 @@ int cached_plan(int kind, int L, int P, int N, double lambda, double nu, double 
         ne.plan = 0;
         ne.work = 0;
         ne.d_sig = ne.d_cof = 0;
+        ne.sync = 0;
         int rc = kind == 0 ? s2wav_plan_create(&ne.plan, L, N, lambda, J0, multires, flags, batch, device)
                            : s2ball_plan_create(&ne.plan, L, P, N, lambda, nu, J0, tau, flags, device);
         if (rc) return rc;
@@ -2186,6 +2250,18 @@ int cached_plan(int kind, int L, int P, int N, double lambda, double nu, double 
             set_error(std::string("cudaMalloc(workspace): ") + cudaGetErrorString(ce));
             cudaGetLastError();
             return S2W_ENOMEM;
+        }
+        ne.sync = new EntrySync();
+        ne.sync->used = false;
+        ne.sync->copy_stream = 0;
+        if (cudaEventCreateWithFlags(&ne.sync->done, cudaEventDisableTiming) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&ne.sync->copy_stream, cudaStreamNonBlocking) != cudaSuccess) {
+            cudaGetLastError();
+            delete ne.sync;
+            cudaFree(ne.work);
+            s2w_plan_destroy(ne.plan);
+            set_error("cudaEventCreate / cudaStreamCreate for a cache entry failed");
+            return S2W_ECUDA;
         }
         it = g_cache.insert(std::make_pair(k, ne)).first;
     }
@@ -2230,10 +2306,12 @@ int host_transform(bool fwd, const CacheEntry &e, const void *in_h, void *out_h)
     const size_t sig = p->signal_elems * p->batch * esz, cof = p->coeff_elems * p->batch * esz;
     void *d_in = fwd ? e.d_sig : e.d_cof, *d_out = fwd ? e.d_cof : e.d_sig;
     int rc = S2W_OK;
+    // one user of the entry's workspace and staging buffers at a time; the call synchronises before it returns
+    std::lock_guard<std::mutex> lock(e.sync->mu);
+    if (e.sync->used) S2W_CUDA_CHECK(cudaEventSynchronize(e.sync->done));
     if (p->kind == 0) {
         // sphere: coefficient blocks pipelined over a second stream (see HostPipe)
-        static cudaStream_t copy_stream = 0;
-        if (!copy_stream) S2W_CUDA_CHECK(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+        cudaStream_t copy_stream = e.sync->copy_stream;
         HostPipe hp;
         hp.copy = copy_stream;
         hp.host = fwd ? (char *)out_h : (char *)const_cast<void *>(in_h);
@@ -2273,7 +2351,7 @@ int s2wav_forward(const void *f, void *w, int L, int N, double lambda, int J0, i
     CacheEntry e;
     int rc = cached_plan(0, L, 1, N, lambda, 0.0, 1.0, J0, multires, flags, batch, &e);
     if (rc) return rc;
-    return s2w_plan_forward(e.plan, f, w, e.work, stream);
+    return entry_serialised(e, (cudaStream_t)stream, [&](cudaStream_t st) { return s2w_plan_forward(e.plan, f, w, e.work, (void *)st); });
 }
 
 int s2wav_inverse(const void *w, void *f, int L, int N, double lambda, int J0, int multires, int flags, int batch,
@@ -2282,7 +2360,7 @@ int s2wav_inverse(const void *w, void *f, int L, int N, double lambda, int J0, i
     CacheEntry e;
     int rc = cached_plan(0, L, 1, N, lambda, 0.0, 1.0, J0, multires, flags, batch, &e);
     if (rc) return rc;
-    return s2w_plan_inverse(e.plan, w, f, e.work, stream);
+    return entry_serialised(e, (cudaStream_t)stream, [&](cudaStream_t st) { return s2w_plan_inverse(e.plan, w, f, e.work, (void *)st); });
 }
 
 int s2wav_forward_host(const void *f, void *w, int L, int N, double lambda, int J0, int multires, int flags, int batch)
@@ -2306,7 +2384,7 @@ int s2ball_forward(const void *f, void *w, int L, int P, int N, double lambda_l,
     CacheEntry e;
     int rc = cached_plan(1, L, P, N, lambda_l, lambda_p, tau, J0, 1, flags, 1, &e);
     if (rc) return rc;
-    return s2w_plan_forward(e.plan, f, w, e.work, stream);
+    return entry_serialised(e, (cudaStream_t)stream, [&](cudaStream_t st) { return s2w_plan_forward(e.plan, f, w, e.work, (void *)st); });
 }
 int s2ball_inverse(const void *w, void *f, int L, int P, int N, double lambda_l, double lambda_p, int J0, double tau,
                    int flags, void *stream)
@@ -2314,7 +2392,7 @@ int s2ball_inverse(const void *w, void *f, int L, int P, int N, double lambda_l,
     CacheEntry e;
     int rc = cached_plan(1, L, P, N, lambda_l, lambda_p, tau, J0, 1, flags, 1, &e);
     if (rc) return rc;
-    return s2w_plan_inverse(e.plan, w, f, e.work, stream);
+    return entry_serialised(e, (cudaStream_t)stream, [&](cudaStream_t st) { return s2w_plan_inverse(e.plan, w, f, e.work, (void *)st); });
 }
 
 int s2ball_forward_host(const void *f, void *w, int L, int P, int N, double lambda_l, double lambda_p, int J0,
@@ -2341,6 +2419,11 @@ int s2w_cache_clear(void)
         cudaFree(kv.second.work);
         cudaFree(kv.second.d_sig);
         cudaFree(kv.second.d_cof);
+        if (kv.second.sync) {
+            cudaEventDestroy(kv.second.sync->done);
+            cudaStreamDestroy(kv.second.sync->copy_stream);
+            delete kv.second.sync;
+        }
         s2w_plan_destroy(kv.second.plan);
     }
     g_cache.clear();

@@ -29,6 +29,7 @@
 #include <climits>
 
 #include "kernels.h"
+#include "smem_attr.cuh"
 
 namespace s2w {
 
@@ -842,15 +843,10 @@ template <int R, int MAXT, bool PRE, bool FUSE>
 int launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
 {
     const size_t smem = PRE ? 0 : (size_t)(T / 32) * R * FWD_GT * sizeof(double);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(wigner_forward_kernel<R, MAXT, PRE, FUSE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)((size_t)(MAXT / 32) * R * FWD_GT * sizeof(double)));
-        if (e != cudaSuccess) {
-            set_error(std::string("cudaFuncSetAttribute(wigner_forward_kernel): ") + cudaGetErrorString(e));
-            return S2W_ECUDA;
-        }
-        configured = true;
+    // the attribute is per device and per function: query and raise it when needed (smem_attr.cuh), no per-process flag
+    {
+        const int rc = set_smem(wigner_forward_kernel<R, MAXT, PRE, FUSE>, (size_t)(MAXT / 32) * R * FWD_GT * sizeof(double));
+        if (rc) return rc;
     }
     dim3 grid(A.Lg, chunks);
     S2W_LAUNCH_C(S2W_K_WIGNER_FWD, (wigner_forward_kernel<R, MAXT, PRE, FUSE>), grid, T, smem, st, A);

@@ -92,3 +92,21 @@ def test_no_cpu_fallback():
     f = np.zeros((1, 8, 15))
     with pytest.raises(api.S2WError, match="S2W_ECUDA"):
         api.s2wav_forward_host(f, 8, 2, 2.0, 0)
+
+
+def test_binding_rejects_dtypes_and_sizes_the_library_would_read_out_of_bounds():
+    """the argument-style wrappers inferred `real` from dtype == float64 and took anything else as
+    complex128; a float32 / complex64 array was then read out of bounds.  The marshalling layer now refuses."""
+    import numpy as np
+    import pytest
+    from paper_2402_01282_b200 import api
+    assert api._dtype_real(np.dtype("float64")) is True and api._dtype_real(np.dtype("complex128")) is False
+    for bad in ("float32", "complex64", "int64"):
+        with pytest.raises(ValueError):
+            api._dtype_real(np.dtype(bad))
+    with pytest.raises(ValueError):
+        api.s2wav_forward_host(np.zeros((1, 8, 15), dtype=np.float32), 8, 2, 2.0, 0)
+    with pytest.raises(ValueError):
+        api.s2wav_forward_host(np.zeros((8, 14)), 8, 2, 2.0, 0)          # not a whole number of L x (2L-1) signals
+    with pytest.raises(ValueError):
+        api.s2wav_inverse_host(np.zeros(17), 8, 2, 2.0, 0)
