@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(256, 2) so3_inv_pair16_kernel(const cplx *__re
     const F16Tw tw = f16_twiddles<R1>();
     const int n = T.n, L = T.L, ng = 2 * A.N - 1;
     const cplx *Fb = F + (size_t)blockIdx.y * A.nrows * L * L;
-    double *Wb = W + (size_t)blockIdx.y * sig_stride;
+    double *Wb = W + so3_base(A, blockIdx.y, sig_stride);
     const size_t plane = (size_t)L * n;
     const RowSet rs = so3_rows(A, +1, gph, s_rowp, s_rowm);
     const int q0 = rs.q0, np = rs.np;
@@ -254,7 +254,7 @@ __global__ void __launch_bounds__(256, 2) so3_fwd_pair16_kernel(const double *__
     const int n = T.n, L = T.L, ng = 2 * A.N - 1;
     const double inv_ng = 1.0 / (double)ng, inv_n = 1.0 / (double)n;
     cplx *Fb = F + (size_t)blockIdx.y * A.nrows * L * L;
-    const double *Wb = W + (size_t)blockIdx.y * sig_stride;
+    const double *Wb = W + so3_base(A, blockIdx.y, sig_stride);
     const size_t plane = (size_t)L * n;
     const RowSet rs = so3_rows(A, -1, gph, s_rowp, s_rowm);
     const int q0 = rs.q0, np = rs.np;

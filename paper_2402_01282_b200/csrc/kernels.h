@@ -21,7 +21,14 @@ struct So3Args {
     int n_val[S2W_MAX_ROWS];     // n
     int n_row[S2W_MAX_ROWS];     // row index of n in F
     int n_rowm[S2W_MAX_ROWS];    // row index of -n in F
+    const size_t *sig_off;       // device array [batch]: element offset of signal b's coefficient block, or null:
+                                 // b * sig_stride (the ball's stacked shells of all radial scales j' are not equidistant)
 };
+// element offset of signal b's block in the pixel-side array
+__host__ __device__ inline size_t so3_base(const So3Args &A, int b, size_t sig_stride)
+{
+    return A.sig_off ? A.sig_off[b] : (size_t)b * sig_stride;
+}
 
 struct RwArgs {
     int nn, nrows, Md, isReal;
@@ -100,8 +107,9 @@ int launch_wigner_seed_floor(const double *coef, size_t tri, int Lfull, int Lg, 
 int launch_wigner_table(const double *coef, size_t tri, int Lfull, int Lg, int G, const int *n_vals, int ntab,
                         const double *yv, const int *gstart, const double2 *dseed, double *dtab, size_t tri_g,
                         cudaStream_t st);
+// krange: device array, one [kbeg, kend) per 64-row tile of A (block-sparse stacked matrices), or null
 int launch_radial(const double *A, int R, int K, const cplx *in, cplx *out, size_t cols, int Lfull, const double *win,
-                  const double *wout, bool accumulate, cudaStream_t st);
+                  const double *wout, bool accumulate, cudaStream_t st, const int2 *krange = 0);
 int launch_wigner_inverse(const WigArgs &A, cudaStream_t st);   // harmonic -> rings   (a5, a7)
 int launch_wigner_forward(const WigArgs &A, cudaStream_t st);   // rings -> harmonic   (a3, a6), accumulates
 

@@ -154,6 +154,7 @@ struct Scale {
 using namespace s2w;
 
 #define S2W_LANES 4  // most lanes a captured sphere transform uses (workspace is sized for them)
+#define S2W_BALL_LANES 2  // streams the angular scales of a stacked ball transform are dealt to
 
 struct s2w_plan {
     int kind;  // 0 sphere, 1 ball
@@ -181,6 +182,16 @@ struct s2w_plan {
     double *Kfull_fwdT, *Kfull_invT;  // their transposes (adjoint transforms)
     double *phi_ball;   // [P][L] sqrt(4pi/(2l+1)) Phi_{l0p}
     size_t ws_shell_elems;  // ball: elements of one [P][Mfull][L] harmonic array
+    // ball, stacked shells: for a fixed angular scale j the radial scales j' differ only in their shell count P_j' and
+    // share grid, filters and tables, so the shells of ALL j' are stacked (PS = sum_j' P_j') and every step of a scale j
+    // is ONE launch over PS shells instead of one per (j, j') (Alg. 2)
+    int PS;                       // stacked shells
+    std::vector<Scale> ang;       // the angular stage of each j (Pj = PS)
+    std::vector<size_t *> ang_off;  // device [PS]: element offset of stacked shell b's block of scale j in a coefficient array
+    double *Kstk_inv;             // [PS nodes][P p]   rows of scale j': K_p(r_i) kappa^{j'}(p), zero for p >= P_j'
+    double *Kstk_fwd;             // [P p][PS nodes]   q_i K_p(r_i) kappa^{j'}(p)
+    int2 *krange_inv, *krange_fwd;  // per 64-row tile of the two matrices: the k range that holds non-zeros
+    size_t ws_stk_elems, ws_stkF_elems, ws_stk_off;  // stacked harmonic array, one F buffer, offset of this part (elements)
     // CUDA graphs of whole transforms (s2w_plan_forward / s2w_plan_inverse), keyed by direction and buffer addresses:
     // a transform is 40 (sphere) to 900 (ball) small launches, replayed as one graph launch after its first call.
     // The only mutable state of a plan; guarded by graph_mu.
@@ -685,6 +696,7 @@ void fill_wig_args(const s2w_plan *p, const Stage &st, bool synthesis, int B, cp
 
 void fill_so3_args(const s2w_plan *p, const Stage &st, So3Args &A)
 {
+    A.sig_off = 0;
     A.N = p->N;
     A.nn = st.nn;
     A.nrows = st.nrows;
@@ -882,7 +894,8 @@ struct Lanes {
     }
 };
 
-static int lanes_fork(const s2w_plan *p, const Work &w, cplx *spare, cudaStream_t s, bool allow, Lanes *ln)
+static int lanes_fork(const s2w_plan *p, const Work &w, cplx *spare, cudaStream_t s, bool allow, Lanes *ln,
+                      size_t Fsz_override = 0, int max_lanes = S2W_LANES)
 {
     ln->n = 1;
     ln->s[0] = s;
@@ -893,11 +906,12 @@ static int lanes_fork(const s2w_plan *p, const Work &w, cplx *spare, cudaStream_
         const int v = e ? atoi(e) : S2W_LANES;
         return v < 1 ? 1 : (v > S2W_LANES ? S2W_LANES : v);
     }();
-    if (!allow || !p->lanes_on || nl == 1) return S2W_OK;
-    const size_t Fsz = ((p->ws_F_elems + 15) / 16) * 16;
+    const int nuse = nl < max_lanes ? nl : max_lanes;
+    if (!allow || !p->lanes_on || nuse == 1) return S2W_OK;
+    const size_t Fsz = Fsz_override ? Fsz_override : ((p->ws_F_elems + 15) / 16) * 16;
     if (!p->lane_fork) S2W_CUDA_CHECK(cudaEventCreateWithFlags(&p->lane_fork, cudaEventDisableTiming));
     S2W_CUDA_CHECK(cudaEventRecord(p->lane_fork, s));
-    for (int i = 1; i < nl; ++i) {
+    for (int i = 1; i < nuse; ++i) {
         if (!p->lane_stream[i - 1]) {
             S2W_CUDA_CHECK(cudaStreamCreateWithFlags(&p->lane_stream[i - 1], cudaStreamNonBlocking));
             S2W_CUDA_CHECK(cudaEventCreateWithFlags(&p->lane_join[i - 1], cudaEventDisableTiming));
@@ -909,7 +923,7 @@ static int lanes_fork(const s2w_plan *p, const Work &w, cplx *spare, cudaStream_
         ln->w[i].Ft = ln->w[i].F + Fsz;
         ln->w[i].Ft2 = 0;
     }
-    ln->n = nl;
+    ln->n = nuse;
     return S2W_OK;
 }
 
@@ -999,7 +1013,7 @@ static int sht_inverse_dev(const s2w_plan *p, const Stage &st, void *f, size_t s
 // a4 + a5 + a8 for one scale: filter x inverse Wigner contraction at L_j, then the (alpha, gamma) DFT.  B signals whose
 // coefficient blocks are sig_stride elements apart.
 static int scale_analysis(const s2w_plan *p, const Scale &sc, int B, const Work &w, void *dst, size_t sig_stride,
-                          cudaStream_t s)
+                          cudaStream_t s, const size_t *sig_off = 0)
 {
     const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
     if (sc.st.nn == 0) {
@@ -1014,18 +1028,20 @@ static int scale_analysis(const s2w_plan *p, const Scale &sc, int B, const Work 
     if ((rc = launch_wigner_inverse(A, s))) return rc;
     So3Args S;
     fill_so3_args(p, sc.st, S);
+    S.sig_off = sig_off;
     return launch_so3_inv(p->real, w.F, dst, sig_stride, S, B, p->grids[sc.st.grid].fft, s);
 }
 
 // a8 + a2 + a6 + a4 for one scale: (alpha, gamma) DFT, reweighting, forward Wigner contraction accumulating into flmT.
 static int scale_synthesis(const s2w_plan *p, const Scale &sc, int B, const Work &w, const void *src, size_t sig_stride,
-                           cudaStream_t s)
+                           cudaStream_t s, const size_t *sig_off = 0)
 {
     if (sc.st.nn == 0) return S2W_OK;
     const GridTab &g = p->grids[sc.st.grid];
     int rc;
     So3Args S;
     fill_so3_args(p, sc.st, S);
+    S.sig_off = sig_off;
     if ((rc = launch_so3_fwd(p->real, src, sig_stride, w.F, S, B, g.fft, s))) return rc;
     RwArgs R;
     fill_rw_args(p, sc.st, R);
@@ -1372,8 +1388,38 @@ static int ball_forward(const s2w_plan *p, const void *in, void *out, void *work
     // scaling coefficients: Phi f, Z^-1 at full resolution (Eq. 35; R9)
     if ((rc = launch_radial(p->Kfull_inv, P, P, bw.flmp, bw.flm_sh, cols, L, p->phi_ball, 0, false, s))) return rc;
     if ((rc = sht_inverse_dev(p, p->sht, (char *)out + p->scaling_offset * esz, shell, P, w, s))) return rc;
-    // wavelet coefficients: per radial scale j' one inverse Laguerre contraction onto the P_j' grid, then the sphere's
-    // scale stage on each of its shells for every angular scale j (Eqs. 33, 43-44)
+    // wavelet coefficients (Eqs. 33, 43-44), stacked shells: ONE inverse Laguerre contraction onto the
+    // node grids of all radial scales j' (stacked matrix, kappa^{j'}(p) folded in), then for every angular scale j the
+    // sphere's scale stage a4 + a5 + a8 over all PS = sum_j' P_j' shells in one launch each
+    static const bool stacked = getenv("S2W_BALL_UNSTACKED") == 0;
+    if (stacked) {
+        cplx *stk = (cplx *)work + p->ws_stk_off;
+        cplx *Fs = stk + p->ws_stk_elems;
+        if ((rc = launch_radial(p->Kstk_inv, p->PS, P, bw.flmp, stk, cols, L, 0, 0, false, s, p->krange_inv))) return rc;
+        Work ws = w;
+        ws.flmT = stk;
+        ws.F = Fs;
+        ws.Ft = Fs + p->ws_stkF_elems;
+        Lanes ln;
+        if ((rc = lanes_fork(p, ws, Fs + 2 * p->ws_stkF_elems, s, true, &ln, p->ws_stkF_elems, S2W_BALL_LANES))) return rc;
+        const size_t nj = p->ang.size();
+        for (size_t k = nj; k-- > 0;) {
+            const Scale &sc = p->ang[k];
+            if (sc.st.nn == 0) {  // empty angular scale: its blocks of every j' are zero
+                for (size_t a = k; a < p->scales.size(); a += nj) {
+                    const Scale &q = p->scales[a];
+                    S2W_CUDA_CHECK(cudaMemsetAsync((char *)out + q.offset * esz, 0,
+                                                   (size_t)q.Pj * (2 * p->N - 1) * q.Lj * (2 * q.Lj - 1) * esz, s));
+                }
+                continue;
+            }
+            const int l = ln.pick(scale_cost(sc));
+            if ((rc = scale_analysis(p, sc, p->PS, ln.w[l], out, 0, ln.s[l], p->ang_off[k]))) return rc;
+        }
+        if ((rc = lanes_join(p, ln))) return rc;
+        S2W_CUDA_CHECK(cudaPeekAtLastError());
+        return S2W_OK;
+    }
     size_t i = 0;
     while (i < p->scales.size()) {
         const Scale &first = p->scales[i];
@@ -1413,7 +1459,31 @@ static int ball_inverse(const s2w_plan *p, const void *in, void *out, void *work
     // scaling part: Z W^Phi, times Phi (Eq. 46)
     if ((rc = sht_forward_dev(p, p->sht, (const char *)in + p->scaling_offset * esz, shell, P, w, true, s))) return rc;
     if ((rc = launch_radial(p->Kfull_fwd, P, P, bw.flm_sh, bw.flmp, cols, L, 0, p->phi_ball, false, s))) return rc;
-    // wavelet part: per j' sum the angular scales shell by shell, then the radial quadrature on the P_j' grid
+    // wavelet part, stacked shells: every angular scale j adds its PS shells into the stacked harmonic array (one launch
+    // per step and scale), then ONE radial quadrature with the stacked matrix
+    static const bool stacked = getenv("S2W_BALL_UNSTACKED") == 0;
+    if (stacked) {
+        cplx *stk = (cplx *)work + p->ws_stk_off;
+        cplx *Fs = stk + p->ws_stk_elems;
+        S2W_CUDA_CHECK(cudaMemsetAsync(stk, 0, (size_t)p->PS * cols * sizeof(cplx), s));
+        Work ws = w;
+        ws.flmT = stk;
+        ws.F = Fs;
+        ws.Ft = Fs + p->ws_stkF_elems;
+        Lanes ln;
+        if ((rc = lanes_fork(p, ws, Fs + 2 * p->ws_stkF_elems, s, true, &ln, p->ws_stkF_elems, S2W_BALL_LANES))) return rc;
+        for (size_t k = p->ang.size(); k-- > 0;) {
+            const Scale &sc = p->ang[k];
+            const int l = ln.pick(scale_cost(sc));
+            if ((rc = scale_synthesis(p, sc, p->PS, ln.w[l], in, 0, ln.s[l], p->ang_off[k]))) return rc;
+        }
+        if ((rc = lanes_join(p, ln))) return rc;
+        if ((rc = launch_radial(p->Kstk_fwd, P, p->PS, stk, bw.flmp, cols, L, 0, 0, true, s, p->krange_fwd))) return rc;
+        if ((rc = launch_radial(p->Kfull_inv, P, P, bw.flmp, bw.flm_sh, cols, L, 0, 0, false, s))) return rc;
+        if ((rc = sht_inverse_dev(p, p->sht, out, shell, P, w, s))) return rc;
+        S2W_CUDA_CHECK(cudaPeekAtLastError());
+        return S2W_OK;
+    }
     size_t i = 0;
     while (i < p->scales.size()) {
         const Scale &first = p->scales[i];
@@ -1922,7 +1992,65 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
     p->ws_shell_elems = (size_t)P * (p->real ? L : 2 * L - 1) * L;
     p->ws_flm_elems = 2 * (((p->ws_shell_elems + 15) / 16) * 16);
     p->ws_F_elems = (size_t)P * maxF;
-    p->ws_bytes = (p->ws_flm_elems + (2 + 2 * (S2W_LANES - 1)) * (((p->ws_F_elems + 15) / 16) * 16)) * sizeof(cplx) + 256;
+    // stacked shells (see the plan's fields): matrices, k ranges per 64-row tile, per-j offset tables
+    {
+        const int njp = p->Jp - p->J0p + 1, nj = (int)ang.size();
+        std::vector<int> base(njp + 1, 0), Pjs(njp);
+        for (int a = 0; a < njp; ++a) {
+            Pjs[a] = p->scales[(size_t)a * nj].Pj;
+            base[a + 1] = base[a] + Pjs[a];
+        }
+        const int PS = base[njp];
+        p->PS = PS;
+        std::vector<double> kinv((size_t)PS * P, 0.0), kfwd((size_t)P * PS, 0.0);
+        for (int a = 0; a < njp; ++a) {
+            const int Pj = Pjs[a];
+            std::vector<double> hi((size_t)Pj * Pj), hf((size_t)Pj * Pj);
+            const Scale &sc = p->scales[(size_t)a * nj];
+            S2W_PLAN_TRY(cudaMemcpy(hi.data(), sc.Kinv, hi.size() * sizeof(double), cudaMemcpyDeviceToHost) == cudaSuccess ? S2W_OK : S2W_ECUDA);
+            S2W_PLAN_TRY(cudaMemcpy(hf.data(), sc.Kfwd, hf.size() * sizeof(double), cudaMemcpyDeviceToHost) == cudaSuccess ? S2W_OK : S2W_ECUDA);
+            for (int i = 0; i < Pj; ++i)
+                for (int pp = 0; pp < Pj; ++pp) {
+                    kinv[(size_t)(base[a] + i) * P + pp] = hi[(size_t)i * Pj + pp];
+                    kfwd[(size_t)pp * PS + base[a] + i] = hf[(size_t)pp * Pj + i];
+                }
+        }
+        S2W_PLAN_TRY(p->pool.upload(&p->Kstk_inv, kinv));
+        S2W_PLAN_TRY(p->pool.upload(&p->Kstk_fwd, kfwd));
+        std::vector<int2> kri((PS + 63) / 64), krf((P + 63) / 64);
+        for (size_t t = 0; t < kri.size(); ++t) {  // rows = stacked nodes, ascending P_j': the last row's P_j' bounds k
+            const int rlast = std::min(PS - 1, (int)t * 64 + 63);
+            int a = 0;
+            while (base[a + 1] <= rlast) ++a;
+            kri[t] = make_int2(0, Pjs[a]);
+        }
+        for (size_t t = 0; t < krf.size(); ++t) {  // rows = p: nodes of the scales with P_j' > first p of the tile
+            int a = 0;
+            while (a < njp - 1 && Pjs[a] <= (int)t * 64) ++a;
+            krf[t] = make_int2(base[a], PS);
+        }
+        S2W_PLAN_TRY(p->pool.upload(&p->krange_inv, kri));
+        S2W_PLAN_TRY(p->pool.upload(&p->krange_fwd, krf));
+        for (int j = 0; j < nj; ++j) {
+            Scale sc = ang[j];
+            sc.Pj = PS;
+            sc.jp = -1;
+            p->ang.push_back(sc);
+            std::vector<size_t> offs(PS);
+            for (int a = 0; a < njp; ++a) {
+                const Scale &q = p->scales[(size_t)a * nj + j];
+                const size_t stride = (size_t)nn * q.Lj * (2 * q.Lj - 1);
+                for (int i = 0; i < Pjs[a]; ++i) offs[base[a] + i] = q.offset + (size_t)i * stride;
+            }
+            size_t *doff;
+            S2W_PLAN_TRY(p->pool.upload(&doff, offs));
+            p->ang_off.push_back(doff);
+        }
+        p->ws_stk_elems = (((size_t)PS * (p->real ? L : 2 * L - 1) * L + 15) / 16) * 16;
+        p->ws_stkF_elems = (((size_t)PS * maxF + 15) / 16) * 16;
+    }
+    p->ws_stk_off = p->ws_flm_elems + (2 + 2 * (S2W_LANES - 1)) * (((p->ws_F_elems + 15) / 16) * 16);
+    p->ws_bytes = (p->ws_stk_off + p->ws_stk_elems + 2 * S2W_BALL_LANES * p->ws_stkF_elems) * sizeof(cplx) + 256;
     S2W_PLAN_TRY(cudaDeviceSynchronize() == cudaSuccess ? S2W_OK : S2W_ECUDA);
     *out = p;
     return S2W_OK;

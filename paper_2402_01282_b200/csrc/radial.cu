@@ -35,7 +35,8 @@ __device__ __forceinline__ void dmma884_r(double &c0, double &c1, double a, doub
 __global__ void __launch_bounds__(256) radial_kernel(const double *__restrict__ A, int R, int K,
                                                     const cplx *__restrict__ in, cplx *__restrict__ out, size_t cols,
                                                     int Lfull, const double *__restrict__ win,
-                                                    const double *__restrict__ wout, int accumulate)
+                                                    const double *__restrict__ wout, int accumulate,
+                                                    const int2 *__restrict__ krange)
 {
     __shared__ double sA[RAD_TR * RAD_SA];
     __shared__ double sB[RAD_TK * RAD_SB];
@@ -51,7 +52,11 @@ __global__ void __launch_bounds__(256) radial_kernel(const double *__restrict__ 
 #pragma unroll
         for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-    for (int k0 = 0; k0 < K; k0 += RAD_TK) {
+    // block-sparse stacked matrices (ball, all radial scales in one launch): only [kbeg, kend) of this row tile holds
+    // non-zeros
+    const int kbeg = krange ? (krange[blockIdx.y].x / RAD_TK) * RAD_TK : 0;
+    const int kend = krange ? min(krange[blockIdx.y].y, K) : K;
+    for (int k0 = kbeg; k0 < kend; k0 += RAD_TK) {
         __syncthreads();
         for (int e = threadIdx.x; e < RAD_TR * RAD_TK; e += 256) {
             const int kk = e & (RAD_TK - 1), rr = e >> 4;
@@ -103,12 +108,12 @@ __global__ void __launch_bounds__(256) radial_kernel(const double *__restrict__ 
 }  // namespace
 
 int launch_radial(const double *A, int R, int K, const cplx *in, cplx *out, size_t cols, int Lfull, const double *win,
-                  const double *wout, bool accumulate, cudaStream_t st)
+                  const double *wout, bool accumulate, cudaStream_t st, const int2 *krange)
 {
     if (R <= 0 || cols == 0) return S2W_OK;
     dim3 grid((unsigned)((2 * cols + RAD_TC - 1) / RAD_TC), (R + RAD_TR - 1) / RAD_TR);
     S2W_LAUNCH_C(S2W_K_RADIAL, radial_kernel, grid, 256, 0, st, A, R, K, in, out, cols, Lfull, win, wout,
-                 accumulate ? 1 : 0);
+                 accumulate ? 1 : 0, krange);
     return S2W_OK;
 }
 

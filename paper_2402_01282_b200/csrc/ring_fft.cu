@@ -206,7 +206,7 @@ __device__ __forceinline__ void so3_inv_few(const cplx *__restrict__ F, void *__
         for (int a = tl; a < (has ? n : 0); a += tpr) {
             const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
             if (REAL) {
-                double *Wr = (double *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+                double *Wr = (double *)W + so3_base(A, b, sig_stride) + (size_t)t * n + a;
                 if (i + 1 < nproc) {
                     Wr[(size_t)(2 * i) * plane] = v.x;
                     Wr[(size_t)(2 * i + 1) * plane] = v.y;
@@ -234,7 +234,7 @@ __device__ __forceinline__ void so3_inv_few(const cplx *__restrict__ F, void *__
                         if (g < ng) Wr[(size_t)g * plane] = out[g];
                 }
             } else {
-                cplx *Wc = (cplx *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+                cplx *Wc = (cplx *)W + so3_base(A, b, sig_stride) + (size_t)t * n + a;
                 if (i + 1 < nproc) {
                     Wc[(size_t)i * plane] = v;
                 } else {
@@ -313,7 +313,7 @@ __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict_
         for (int a = tl; a < (has ? n : 0); a += tpr) {
             const cplx v = cmulc(buf[S2W_PAD(a)], __ldg(&T.chirp[a]));
             if (REAL) {
-                double *Wr = (double *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+                double *Wr = (double *)W + so3_base(A, b, sig_stride) + (size_t)t * n + a;
                 const double cn = nv == 0 ? 1.0 : 2.0;
                 const double vx = cn * v.x, vy = cn * v.y;
                 for (int g0 = 0; g0 < ng; g0 += 9) {
@@ -329,7 +329,7 @@ __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict_
                         }
                 }
             } else {
-                cplx *Wc = (cplx *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+                cplx *Wc = (cplx *)W + so3_base(A, b, sig_stride) + (size_t)t * n + a;
                 for (int g0 = 0; g0 < ng; g0 += 5) {
                     cplx old[5];
 #pragma unroll
@@ -400,11 +400,11 @@ __device__ __forceinline__ void so3_fwd_few(const void *__restrict__ W, cplx *__
         double wr[NG];
         cplx wc[REAL ? 1 : NG];
         if (REAL) {
-            const double *Wr = (const double *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+            const double *Wr = (const double *)W + so3_base(A, b, sig_stride) + (size_t)t * n + a;
 #pragma unroll
             for (int g = 0; g < NG; ++g) wr[g] = g < ng ? Wr[(size_t)g * plane] : 0.0;
         } else {
-            const cplx *Wc = (const cplx *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+            const cplx *Wc = (const cplx *)W + so3_base(A, b, sig_stride) + (size_t)t * n + a;
 #pragma unroll
             for (int g = 0; g < NG; ++g) wc[g] = g < ng ? Wc[(size_t)g * plane] : cmake(0.0, 0.0);
         }
@@ -500,7 +500,7 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
             cplx v = cmake(0.0, 0.0);
             if (a < n && has) {
                 if (REAL) {
-                    const double *Wr = (const double *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+                    const double *Wr = (const double *)W + so3_base(A, b, sig_stride) + (size_t)t * n + a;
                     for (int g0 = 0; g0 < ng; g0 += 9) {
                         double wv[9];
 #pragma unroll
@@ -514,7 +514,7 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
                             }
                     }
                 } else {
-                    const cplx *Wc = (const cplx *)W + (size_t)b * sig_stride + (size_t)t * n + a;
+                    const cplx *Wc = (const cplx *)W + so3_base(A, b, sig_stride) + (size_t)t * n + a;
                     for (int g0 = 0; g0 < ng; g0 += 5) {
                         cplx wv[5];
 #pragma unroll
@@ -600,7 +600,7 @@ __device__ __forceinline__ void so3_inv_pair_few(const cplx *__restrict__ F, dou
     const bool has1 = t0 + 1 < L;
     const int ng = 2 * A.N - 1;
     const cplx *Fb = F + (size_t)b * A.nrows * L * L;
-    double *Wb = W + (size_t)b * sig_stride;
+    double *Wb = W + so3_base(A, b, sig_stride);
     const size_t plane = (size_t)L * n;
     int q0 = -1, np = 0;  // the row n = 0 and the number of rows n > 0
     for (int q = 0; q < A.nn; ++q) {
@@ -716,7 +716,7 @@ __global__ void __launch_bounds__(256, 3) so3_inv_pair_kernel(const cplx *__rest
     const bool has1 = t0 + 1 < L;
     const int ng = 2 * A.N - 1;
     const cplx *Fb = F + (size_t)b * A.nrows * L * L;
-    double *Wb = W + (size_t)b * sig_stride;
+    double *Wb = W + so3_base(A, b, sig_stride);
     const size_t plane = (size_t)L * n;
     if (ng <= 9) {
         so3_inv_pair_few(F, W, sig_stride, A, T, buf, s_tw, gph);
@@ -804,7 +804,7 @@ __device__ __forceinline__ void so3_fwd_pair_few(const double *__restrict__ W, c
     const int ng = 2 * A.N - 1;
     const double inv_ng = 1.0 / (double)ng, inv_n = 1.0 / (double)n;
     cplx *Fb = F + (size_t)b * A.nrows * L * L;
-    const double *Wb = W + (size_t)b * sig_stride;
+    const double *Wb = W + so3_base(A, b, sig_stride);
     const size_t plane = (size_t)L * n;
     __shared__ int s_rowp[4], s_rowm[4];
     int q0 = -1, np = 0;
@@ -929,7 +929,7 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_pair_kernel(const double *__re
     const int ng = 2 * A.N - 1;
     const double inv_ng = 1.0 / (double)ng, inv_n = 1.0 / (double)n;
     cplx *Fb = F + (size_t)b * A.nrows * L * L;
-    const double *Wb = W + (size_t)b * sig_stride;
+    const double *Wb = W + so3_base(A, b, sig_stride);
     const size_t plane = (size_t)L * n;
     if (ng <= 9) {
         so3_fwd_pair_few(W, F, sig_stride, A, T, buf, s_tw, gph);
