@@ -1,5 +1,5 @@
 // fft16_core.cuh -- the second-generation block FFT of the path (rows a1, a2, a8): circular convolutions of length
-// M = R1 * 256 (R1 = 16, 8, 4: M = 4096, 2048, 1024) on a 4096-element shared-memory buffer holding NB = 16 / R1
+// M = R1 * 256 (R1 = 16, 8, 4, 2, 1: M = 4096 ... 256) on a 4096-element shared-memory buffer holding NB = 16 / R1
 // sequences, by 256 threads.
 //
 // Why a second core (profiles/r01k_notes.md): the radix-8 core of fft_core.cuh moves every sequence through shared
@@ -149,8 +149,14 @@ __device__ __forceinline__ void bfly_r(cplx (&v)[R])
         bfly16<INV, HIN, HOUT>(v);
     else if constexpr (R == 8)
         bfly8<INV, HIN, HOUT>(v);
-    else
+    else if constexpr (R == 4)
         bfly4a<INV, HIN, HOUT>(v);
+    else if constexpr (R == 2) {  // HIN: v[1] = 0; HOUT: only v[0] is formed
+        const cplx a = v[0], b = HIN ? cmake(0.0, 0.0) : v[1];
+        v[0] = HIN ? a : cadd(a, b);
+        if (!HOUT) v[1] = HIN ? a : csub(a, b);
+    }
+    // R == 1: nothing to do
 }
 
 __device__ __forceinline__ cplx csqr(cplx a) { return cmake(fma(a.x, a.x, -a.y * a.y), 2.0 * a.x * a.y); }
@@ -159,16 +165,21 @@ __device__ __forceinline__ cplx csqr(cplx a) { return cmake(fma(a.x, a.x, -a.y *
 template <int R, bool CONJ>
 __device__ __forceinline__ void twiddle_apply(cplx (&v)[R], cplx w1)
 {
+    if constexpr (R == 1) return;
+    if constexpr (R == 2) {
+        v[1] = CONJ ? cmulc(v[1], w1) : cmul(v[1], w1);
+        return;
+    }
     // opaque to the optimiser: otherwise the powers are hoisted out of the caller's loop over convolutions (loop-invariant)
     // or shared between a forward and an inverse pass, i.e. 15-30 complex values kept live -- in local memory (ptxas
     // spilled 0.85 KB per thread, one LDL.128 per twiddle: as much LSU traffic as half the transform's own)
     asm volatile("" : "+d"(w1.x), "+d"(w1.y));
     if (CONJ) w1 = cconj(w1);
     const cplx w2 = csqr(w1);
-    v[1] = cmul(v[1], w1);
-    v[2] = cmul(v[2], w2);
+    v[1 % R] = cmul(v[1 % R], w1);
+    v[2 % R] = cmul(v[2 % R], w2);
     const cplx w3 = cmul(w2, w1);
-    v[3] = cmul(v[3], w3);
+    v[3 % R] = cmul(v[3 % R], w3);
     if constexpr (R >= 8) {
         const cplx w4 = csqr(w2);
         v[4] = cmul(v[4], w4);
@@ -308,12 +319,12 @@ __device__ __forceinline__ void f16_convolve_half(cplx *buf, cplx (&x)[16 / R1][
                                                   const F16Tw &tw)
 {
 #pragma unroll
-    for (int q = 0; q < 16 / R1; ++q) f16_pass1_fwd<R1, true>(buf, q, x[q], tw);
+    for (int q = 0; q < 16 / R1; ++q) f16_pass1_fwd<R1, (R1 > 1)>(buf, q, x[q], tw);
     __syncthreads();
     f16_middle<R1>(buf, khat, tw);
     __syncthreads();
 #pragma unroll
-    for (int q = 0; q < 16 / R1; ++q) f16_pass1_inv<R1, true>(buf, q, x[q], tw);
+    for (int q = 0; q < 16 / R1; ++q) f16_pass1_inv<R1, (R1 > 1)>(buf, q, x[q], tw);
 }
 
 // plan time: full forward transform of one length-M sequence (natural order in, the core's own order out; TPOSE: in the
@@ -326,7 +337,7 @@ __device__ __forceinline__ void f16_forward_full(cplx *buf, const cplx *in, cplx
     for (int k = 0; k < R1; ++k) x[k] = in[threadIdx.x + 256 * k];
     f16_pass1_fwd<R1, false>(buf, 0, x, tw);
     __syncthreads();
-    if ((int)(threadIdx.x >> 4) < R1) {
+    if ((int)(threadIdx.x >> 5) < (R1 + 1) / 2) {  // whole warps (a lone half-warp cannot __syncwarp)
         f16_pass2_fwd(buf, tw);
         __syncwarp();
         f16_pass3_fwd(buf);

@@ -399,7 +399,7 @@ template <int R1>
 __global__ void __launch_bounds__(256, 2) reweight16_kernel(const cplx *__restrict__ F, cplx *__restrict__ Ft, RwArgs A,
                                                            RwTab R, int ncolumns)
 {
-    constexpr int NB = 16 / R1, NC = NB / 2, HR = R1 / 2, M = R1 * 256;
+    constexpr int NB = 16 / R1, NC = NB / 2, HR = R1 >= 2 ? R1 / 2 : 1, M = R1 * 256;
     extern __shared__ cplx buf[];
     __shared__ cplx s_part[NC][8];
     __shared__ cplx s_pole[NC];
@@ -450,7 +450,7 @@ __global__ void __launch_bounds__(256, 2) reweight16_kernel(const cplx *__restri
         if ((threadIdx.x & 31) == 0) s_part[ci][threadIdx.x >> 5] = dot;
     }
 #pragma unroll
-    for (int q = 0; q < NB; ++q) f16_pass1_fwd<R1, true>(buf, q, x[q], tw);
+    for (int q = 0; q < NB; ++q) f16_pass1_fwd<R1, (R1 > 1)>(buf, q, x[q], tw);
     __syncthreads();
     f16_pass2_fwd(buf, tw);
     __syncwarp();
@@ -485,7 +485,7 @@ __global__ void __launch_bounds__(256, 2) reweight16_kernel(const cplx *__restri
     f16_pass2_inv(buf, tw);
     __syncthreads();
 #pragma unroll
-    for (int q = 0; q < NB; ++q) f16_pass1_inv<R1, true>(buf, q, x[q], tw);
+    for (int q = 0; q < NB; ++q) f16_pass1_inv<R1, (R1 > 1)>(buf, q, x[q], tw);
 #pragma unroll
     for (int ci = 0; ci < NC; ++ci) {
         cplx *colT = colT_of[ci];
@@ -508,6 +508,124 @@ __global__ void __launch_bounds__(256, 2) reweight16_kernel(const cplx *__restri
                 for (int w = 0; w < 8; ++w) acc = cadd(acc, s_part[ci][w]);
                 colT[t] = acc;
             }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a8 for complex signals (sphere configs 2, the ball), NN <= 3 active rows n, Bluestein lengths 256 ... 1024 (R1 = 1, 2,
+// 4): a round holds the NN rows of RB = NB / NN rings, so the gamma DFT of a ring (Eq. 48) is done in registers
+// right after / before the transforms -- nothing is parked.  F[b][row][t][m + L-1], W[b][g][t][a] complex.
+// ---------------------------------------------------------------------------------------------------------------
+template <int R1, int NN>
+__global__ void __launch_bounds__(256, 2) so3_inv_c16_kernel(const cplx *__restrict__ F, cplx *__restrict__ W,
+                                                            size_t sig_stride, So3Args A, FftTab T)
+{
+    constexpr int NB = 16 / R1, HR = R1 >= 2 ? R1 / 2 : 1, RB = NB / NN;
+    static_assert(RB >= 1, "more rows than sequences in a round");
+    extern __shared__ cplx buf[];
+    __shared__ cplx gph[NN * 64];
+    const F16Tw tw = f16_twiddles<R1>();
+    const int n = T.n, L = T.L, ng = 2 * A.N - 1;
+    const cplx *Fb = F + (size_t)blockIdx.y * A.nrows * L * n;
+    cplx *Wb = W + so3_base(A, blockIdx.y, sig_stride);
+    const size_t plane = (size_t)L * n;
+    for (int e = threadIdx.x; e < NN * ng; e += 256) gph[e] = cis_2pi(A.n_val[e / ng] * (e % ng), ng);
+    cplx x[NB][R1];
+#pragma unroll
+    for (int q = 0; q < NB; ++q) {
+        const int r = q / NN, i = q % NN;
+        const int t = blockIdx.x * RB + r;
+        const bool on = r < RB && t < L;
+        const cplx *Fp = Fb + ((size_t)A.n_row[i] * L + (on ? t : 0)) * n + (L - 1);
+#pragma unroll
+        for (int c = 0; c < HR; ++c) {
+            const int k = threadIdx.x + 256 * c;
+            const int kk = (k < n && on) ? k : 0;
+            const cplx v = Fp[kk < L ? kk : kk - n], ch = __ldg(&T.chirp[kk]);
+            x[q][c] = (k < n && on) ? cmulc(v, ch) : cmake(0.0, 0.0);
+        }
+    }
+    __syncthreads();  // gph
+    f16_convolve_half<R1>(buf, x, T.bhat16_p, tw);
+#pragma unroll
+    for (int r = 0; r < RB; ++r) {
+        const int t = blockIdx.x * RB + r;
+        if (t >= L) continue;
+#pragma unroll
+        for (int c = 0; c < HR; ++c) {
+            const int a = threadIdx.x + 256 * c;
+            if (a >= n) continue;
+            const cplx ch = __ldg(&T.chirp[a]);
+            cplx v[NN];
+#pragma unroll
+            for (int i = 0; i < NN; ++i) v[i] = cmulc(x[r * NN + i][c], ch);
+            cplx *Wr = Wb + (size_t)t * n + a;
+            for (int g = 0; g < ng; ++g) {
+                cplx o = cmul(gph[g], v[0]);
+#pragma unroll
+                for (int i = 1; i < NN; ++i) o = cadd(o, cmul(gph[i * ng + g], v[i]));
+                Wr[(size_t)g * plane] = o;
+            }
+        }
+    }
+}
+
+template <int R1, int NN>
+__global__ void __launch_bounds__(256, 2) so3_fwd_c16_kernel(const cplx *__restrict__ W, cplx *__restrict__ F,
+                                                            size_t sig_stride, So3Args A, FftTab T)
+{
+    constexpr int NB = 16 / R1, HR = R1 >= 2 ? R1 / 2 : 1, RB = NB / NN;
+    static_assert(RB >= 1, "more rows than sequences in a round");
+    extern __shared__ cplx buf[];
+    __shared__ cplx gph[NN * 64];
+    const F16Tw tw = f16_twiddles<R1>();
+    const int n = T.n, L = T.L, ng = 2 * A.N - 1;
+    const double inv_ng = 1.0 / (double)ng, inv_n = 1.0 / (double)n;
+    cplx *Fb = F + (size_t)blockIdx.y * A.nrows * L * n;
+    const cplx *Wb = W + so3_base(A, blockIdx.y, sig_stride);
+    const size_t plane = (size_t)L * n;
+    for (int e = threadIdx.x; e < NN * ng; e += 256) gph[e] = cis_2pi(-A.n_val[e / ng] * (e % ng), ng);
+    __syncthreads();
+    cplx x[NB][R1];
+#pragma unroll
+    for (int q = 0; q < NB; ++q)
+#pragma unroll
+        for (int c = 0; c < HR; ++c) x[q][c] = cmake(0.0, 0.0);
+#pragma unroll
+    for (int r = 0; r < RB; ++r) {
+        const int t = blockIdx.x * RB + r;
+        if (t >= L) continue;
+#pragma unroll
+        for (int c = 0; c < HR; ++c) {
+            const int a = threadIdx.x + 256 * c;
+            if (a >= n) continue;
+            const cplx *Wr = Wb + (size_t)t * n + a;
+            cplx y[NN];
+#pragma unroll
+            for (int i = 0; i < NN; ++i) y[i] = cmake(0.0, 0.0);
+            for (int g = 0; g < ng; ++g) {
+                const cplx wv = Wr[(size_t)g * plane];
+#pragma unroll
+                for (int i = 0; i < NN; ++i) y[i] = cadd(y[i], cmul(gph[i * ng + g], wv));
+            }
+            const cplx ch = cscale(__ldg(&T.chirp[a]), inv_ng);
+#pragma unroll
+            for (int i = 0; i < NN; ++i) x[r * NN + i][c] = cmul(y[i], ch);
+        }
+    }
+    f16_convolve_half<R1>(buf, x, T.bhat16_m, tw);
+#pragma unroll
+    for (int q = 0; q < NB; ++q) {
+        const int r = q / NN, i = q % NN;
+        const int t = blockIdx.x * RB + r;
+        if (r >= RB || t >= L) continue;
+        cplx *Fp = Fb + ((size_t)A.n_row[i] * L + t) * n + (L - 1);
+#pragma unroll
+        for (int c = 0; c < HR; ++c) {
+            const int k = threadIdx.x + 256 * c;
+            if (k >= n) continue;
+            Fp[k < L ? k : k - n] = cscale(cmul(x[q][c], __ldg(&T.chirp[k])), inv_n);
         }
     }
 }
@@ -553,6 +671,12 @@ int launch_fft16_forward(cplx *data, int M, cudaStream_t st)
     } else if (M == 1024) {
         if ((rc = set_smem(fft16_forward_kernel<4>, sm))) return rc;
         S2W_LAUNCH(fft16_forward_kernel<4>, 1, 256, sm, st, data);
+    } else if (M == 512) {
+        if ((rc = set_smem(fft16_forward_kernel<2>, sm))) return rc;
+        S2W_LAUNCH(fft16_forward_kernel<2>, 1, 256, sm, st, data);
+    } else if (M == 256) {
+        if ((rc = set_smem(fft16_forward_kernel<1>, sm))) return rc;
+        S2W_LAUNCH(fft16_forward_kernel<1>, 1, 256, sm, st, data);
     } else {
         set_error("launch_fft16_forward: unsupported length");
         return S2W_EINVAL;
@@ -596,20 +720,72 @@ int launch_so3_pair16(bool fwd, const void *in, void *out, size_t sig_stride, co
     return so3_pair16_t<4>(fwd, in, out, sig_stride, A, batch, T, st);
 }
 
-// Toeplitz length 2048 / 1024 (the caller checks)
-int launch_reweight16(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st)
+template <int R1, int NN>
+static int so3_c16_t(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
+                     cudaStream_t st)
 {
+    constexpr int RB = (16 / R1) / NN;
+    const size_t sm = (size_t)F16_BUF * sizeof(cplx);
+    dim3 grid((T.L + RB - 1) / RB, batch);
+    int rc;
+    if (fwd) {
+        if ((rc = set_smem(so3_fwd_c16_kernel<R1, NN>, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_SO3_FFT, (so3_fwd_c16_kernel<R1, NN>), grid, 256, sm, st, (const cplx *)in, (cplx *)out,
+                     sig_stride, A, T);
+    } else {
+        if ((rc = set_smem(so3_inv_c16_kernel<R1, NN>, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_SO3_FFT, (so3_inv_c16_kernel<R1, NN>), grid, 256, sm, st, (const cplx *)in, (cplx *)out,
+                     sig_stride, A, T);
+    }
+    return S2W_OK;
+}
+
+bool so3_c16_supported(const So3Args &A, const FftTab &T)
+{
+    return T.bhat16_m && (T.M == 256 || T.M == 512 || T.M == 1024) && A.nn >= 1 && A.nn <= 3;
+}
+
+// complex signals; the caller checks so3_c16_supported
+int launch_so3_c16(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
+                   cudaStream_t st)
+{
+#define S2W_C16_CASE(MM, RR)                                                                          \
+    if (T.M == MM) {                                                                                  \
+        if (A.nn == 1) return so3_c16_t<RR, 1>(fwd, in, out, sig_stride, A, batch, T, st);            \
+        if (A.nn == 2) return so3_c16_t<RR, 2>(fwd, in, out, sig_stride, A, batch, T, st);            \
+        return so3_c16_t<RR, 3>(fwd, in, out, sig_stride, A, batch, T, st);                           \
+    }
+    S2W_C16_CASE(256, 1)
+    S2W_C16_CASE(512, 2)
+    S2W_C16_CASE(1024, 4)
+#undef S2W_C16_CASE
+    set_error("launch_so3_c16: unsupported length");
+    return S2W_EINVAL;
+}
+
+// Toeplitz length 2048 ... 256 (the caller checks)
+template <int R1>
+static int reweight16_t(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st)
+{
+    constexpr int NC = 8 / R1;
     const int ncol = A.Md * A.nn * batch;
     const size_t sm = (size_t)F16_BUF * sizeof(cplx);
     int rc;
-    if (R.fft.M == 2048) {
-        if ((rc = set_smem(reweight16_kernel<8>, sm))) return rc;
-        S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight16_kernel<8>, ncol, 256, sm, st, F, Ft, A, R, ncol);
-    } else {
-        if ((rc = set_smem(reweight16_kernel<4>, sm))) return rc;
-        S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight16_kernel<4>, (ncol + 1) / 2, 256, sm, st, F, Ft, A, R, ncol);
-    }
+    if ((rc = set_smem(reweight16_kernel<R1>, sm))) return rc;
+    S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight16_kernel<R1>, (ncol + NC - 1) / NC, 256, sm, st, F, Ft, A, R, ncol);
     return S2W_OK;
+}
+
+int launch_reweight16(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st)
+{
+    switch (R.fft.M) {
+    case 2048: return reweight16_t<8>(F, Ft, A, batch, R, st);
+    case 1024: return reweight16_t<4>(F, Ft, A, batch, R, st);
+    case 512: return reweight16_t<2>(F, Ft, A, batch, R, st);
+    case 256: return reweight16_t<1>(F, Ft, A, batch, R, st);
+    }
+    set_error("launch_reweight16: unsupported length");
+    return S2W_EINVAL;
 }
 
 }  // namespace s2w

@@ -16,7 +16,7 @@ namespace s2w {
 __host__ __device__ inline int fft_padded_len(int M) { return M + (M >> 3) + 1; }
 
 // lengths served by the radix-16 core (fft16_core.cuh)
-__host__ __device__ inline bool f16_supported(int M) { return M == 4096 || M == 2048 || M == 1024; }
+__host__ __device__ inline bool f16_supported(int M) { return M == 4096 || M == 2048 || M == 1024 || M == 512 || M == 256; }
 
 struct FftTab {
     int n;              // DFT length (2L-1)

@@ -96,6 +96,9 @@ int launch_fft16_spectrum(cplx *khat, int kind, int n, int M, cudaStream_t st); 
 int launch_so3_pair16(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch,
                       const FftTab &T, cudaStream_t st);                // a8, real signals, 2N-1 <= 9
 int launch_reweight16(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st);  // a2
+bool so3_c16_supported(const So3Args &A, const FftTab &T);            // a8, complex signals, <= 3 rows, M = 256 ... 1024
+int launch_so3_c16(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
+                   cudaStream_t st);
 
 // plan-time: group start degrees and seeds from the range-extended values d^{l0}_{mn}(beta_t) = mant 2^expo ([ntab][Lg m][Lg t])
 int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int G,

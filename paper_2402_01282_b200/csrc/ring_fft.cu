@@ -1599,8 +1599,9 @@ static int so3_launch_t(bool fwd, const void *in, void *out, size_t sig_stride, 
 static int so3_launch(bool fwd, bool real, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch,
                       const FftTab &T, cudaStream_t st)
 {
-    if (real && 2 * A.N - 1 <= 9 && T.bhat16_m && f16_supported(T.M) && use_fft16())
+    if (real && 2 * A.N - 1 <= 9 && T.bhat16_m && T.M >= 1024 && f16_supported(T.M) && use_fft16())
         return launch_so3_pair16(fwd, in, out, sig_stride, A, batch, T, st);
+    if (!real && so3_c16_supported(A, T) && use_fft16()) return launch_so3_c16(fwd, in, out, sig_stride, A, batch, T, st);
     const int rpb = seqs_per_block(4096 / T.M, (long long)T.L * batch, 32);
     if (rpb == 1 && real) {  // large grids, real signals: ring pairs (the n = 0 row shares one transform)
         const int ng = 2 * A.N - 1;
@@ -1669,7 +1670,7 @@ int launch_transpose(const cplx *src, cplx *dst, int R, int C, int nb, cudaStrea
 int launch_reweight_th(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st)
 {
     if (A.nn <= 0) return S2W_OK;
-    if (R.TG16 && (R.fft.M == 2048 || R.fft.M == 1024) && use_fft16()) return launch_reweight16(F, Ft, A, batch, R, st);
+    if (R.TG16 && R.fft.M >= 256 && R.fft.M <= 2048 && use_fft16()) return launch_reweight16(F, Ft, A, batch, R, st);
     const int ncol = A.Md * A.nn * batch;
     const int cpb = seqs_per_block(2048 / R.fft.M, ncol, RW_MAXCPB);
     size_t sm = 2 * (size_t)cpb * fft_padded_len(R.fft.M) * sizeof(cplx);
