@@ -27,6 +27,7 @@
 // tensor pipe (mma.sync.m8n8k4.f64: D[col][l] += h^T[col][ring] d[ring][l]), the d values of an l-octet passing
 // through a warp-private shared-memory transpose.
 #include <climits>
+#include <cstdlib>
 
 #include "kernels.h"
 #include "smem_attr.cuh"
@@ -746,6 +747,215 @@ __global__ void __launch_bounds__(MAXT) precomp_inverse_kernel(WigArgs A)
     }
 }
 
+// ---- bulk-asynchronous (TMA) staging of the table: cp.async.bulk global -> shared with mbarrier completion ----------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+// 1-D bulk copy (bytes: a multiple of 16, both addresses 16-byte aligned); completes on the mbarrier
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// The inverse direction from the table with TMA-staged tiles (north_star: "batched dense contraction on the fp64 tensor
+// pipe (DMMA), with TMA-staged tiles").  Same contraction as precomp_inverse_kernel, but the A operand --
+// 4 degrees x 32 ring slots of each of the warp's R groups per step, 256-byte runs of the table -- reaches shared memory
+// by cp.async.bulk (SASS UBLKCP) into a ring of PRE_STAGES stages PER WARP, completion signalled on a per-stage
+// mbarrier, PRE_STAGES - 1 steps ahead of the DMMA that consumes it.  A warp produces and consumes only its own
+// stages (its lane 0 issues the copies after __syncwarp), so there is no cross-warp synchronisation on the table stream;
+// the per-lane 8-byte __ldg gathers of the plain kernel kept at most 4 loads per lane in flight (0.56 of the HBM roof).
+// A warp owns R CONTIGUOUS groups here (ring slots 32 R warp ...), so a degree's row for the warp is one contiguous run
+// of up to 256 R bytes: one bulk copy per degree.  Stage layout: [degree of the quad][32 R ring slots + 4 pad doubles],
+// so that the A-fragment reads (ring lane/4 of an octet, degree lane%4) of a half-warp fall into 16 different bank pairs.
+template <int R>
+struct PreStage {
+    static constexpr int row = 32 * R + 4;        // one degree: the warp's R contiguous groups + 4 pad doubles
+    static constexpr int doubles = 4 * row;
+};
+template <int R, int MAXT, int STAGES>
+__global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) precomp_inverse_tma_kernel(WigArgs A)
+{
+    constexpr int NC = 8;
+    __shared__ double s_X[WIG_TL * NC];
+    extern __shared__ __align__(16) double s_dyn[];   // [W][STAGES][4 degrees][32 R + 4] then the mbarriers [W][STAGES]
+
+    const int m = blockIdx.x, chunk = blockIdx.y;
+    const int Lg = A.Lg, Lfull = A.Lfull, G = A.G;
+    const int Md = A.isReal ? Lg : 2 * Lg - 1;
+    const int Mfull = A.isReal ? Lfull : 2 * Lfull - 1;
+    const int T = blockDim.x, W = T >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int fr = lane >> 2, fk = lane & 3;
+    double *wst = s_dyn + (size_t)warp * STAGES * PreStage<R>::doubles;
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(s_dyn + (size_t)W * STAGES * PreStage<R>::doubles) +
+                               warp * STAGES;
+    if (lane == 0) {
+#pragma unroll
+        for (int sgi = 0; sgi < STAGES; ++sgi) mbar_init(&bars[sgi], 1);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the barriers are visible to the async proxy
+    }
+    __syncwarp();
+    unsigned it_prod = 0, it_cons = 0;  // steps issued / consumed by this warp since kernel start (stage and parity)
+
+    for (int q = 0; q < A.nn; ++q) {
+        const int n = A.n_val[q], an = n < 0 ? -n : n;
+        const int l0 = m > an ? m : an;
+        if (l0 >= Lg) continue;
+        const int tab = A.n_tab[q];
+        const int *gsrow = A.gstart + ((size_t)tab * Lg + m) * G;
+        const double sgn = ((m + n) & 1) ? -1.0 : 1.0;
+        const int lacc = l0 > A.lmin ? l0 : A.lmin;
+        const double *tbase = A.dtab + ((size_t)tab * A.tri_g + tri_off(m, Lg)) * (size_t)(32 * G);
+
+        int gs[R];
+        double acc[R][4][2];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int g = warp * R + r;
+            gs[r] = g < G ? gsrow[g] : INT_MAX;
+#pragma unroll
+            for (int o = 0; o < 4; ++o) acc[r][o][0] = acc[r][o][1] = 0.0;
+        }
+        int first = gsrow[0];
+        if (G > 1 && gsrow[1] < first) first = gsrow[1];
+        if (first < lacc) first = lacc;
+        const int lt0 = first & ~(WIG_TL - 1);
+
+        // a step = one degree quad lo..lo+3; `live` steps are those the plain kernel does not skip
+        auto live = [&](int lo) { return !(lo + 4 <= lacc || lo >= Lg || gs[0] >= lo + 4); };
+        auto issue = [&](int lo) {  // lane 0: bulk copies of the quad's rows for the warp's started groups
+            const unsigned sgi = it_prod % STAGES;
+            double *dst = wst + (size_t)sgi * PreStage<R>::doubles;
+            unsigned bytes = 0;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                if (gs[r] >= lo + 4) continue;
+                bytes = (r + 1) * 256;
+            }
+            {
+                int rows = 0;
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (lo + k >= l0 && lo + k < Lg) ++rows;
+                bytes *= rows;
+            }
+            mbar_arrive_expect_tx(&bars[sgi], bytes);
+            // the warp's started groups are a prefix of its R contiguous groups (starts are monotone within a hemisphere
+            // and the two hemispheres of a pair start together or the northern one first): one copy per degree
+            int nact = 0;
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+                if (gs[r] < lo + 4) nact = r + 1;
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (lo + k >= l0 && lo + k < Lg)
+                    bulk_g2s(dst + k * PreStage<R>::row, tbase + (size_t)(lo + k) * (32 * G) + (size_t)warp * R * 32, nact * 256,
+                             &bars[sgi]);
+            ++it_prod;
+        };
+        // prologue: up to STAGES - 1 live steps ahead
+        int lo_prod = lt0;
+        {
+            int ahead = 0;
+            while (lo_prod < Lg && ahead < STAGES - 1) {
+                if (live(lo_prod)) {
+                    if (lane == 0) issue(lo_prod);
+                    ++ahead;
+                }
+                lo_prod += 4;
+            }
+        }
+        it_prod = __shfl_sync(0xffffffffu, it_prod, 0);
+
+        for (int lt = lt0; lt < Lg; lt += WIG_TL) {
+            __syncthreads();
+            for (int i = threadIdx.x; i < WIG_TL * (NC / 2); i += T) {
+                const int k = i / WIG_TL, ll = i % WIG_TL;
+                const int l = lt + ll;
+                const ColInfo ci = col_info(A, chunk * (NC / 2) + k);
+                cplx X = cmake(0.0, 0.0);
+                if (l >= lacc && l < Lg && ci.valid) {
+                    const int mi = A.isReal ? m : (ci.minus ? Lfull - 1 - m : Lfull - 1 + m);
+                    const cplx f = A.flmT[((size_t)ci.b * Mfull + mi) * Lfull + l];
+                    const cplx Gf = A.filt[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
+                    X = cmul(Gf, f);
+                    if (ci.minus) X = cscale(X, sgn);
+                }
+                s_X[ll * NC + 2 * k] = X.x;
+                s_X[ll * NC + 2 * k + 1] = X.y;
+            }
+            __syncthreads();
+            for (int lq = 0; lq < WIG_TL; lq += 4) {
+                const int lo = lt + lq;
+                if (!live(lo)) continue;
+                // keep the pipeline full: the next live step not yet issued (its stage was released by the __syncwarp
+                // that ended the step STAGES - 1 steps ago)
+                while (lo_prod < Lg && !live(lo_prod)) lo_prod += 4;
+                if (lo_prod < Lg) {
+                    if (lane == 0) issue(lo_prod);
+                    it_prod = __shfl_sync(0xffffffffu, it_prod, 0);
+                    lo_prod += 4;
+                }
+                const unsigned sgi = it_cons % STAGES;
+                mbar_wait(&bars[sgi], (it_cons / STAGES) & 1);
+                ++it_cons;
+                const double *src = wst + (size_t)sgi * PreStage<R>::doubles + fk * PreStage<R>::row + fr;
+                const double bv = s_X[(lq + fk) * NC + fr];
+                const int lrow = lo + fk;
+                const bool ok = lrow >= l0 && lrow < Lg;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    if (gs[r] >= lo + 4) continue;
+                    double av[4];
+#pragma unroll
+                    for (int o = 0; o < 4; ++o) av[o] = ok ? src[r * 32 + 8 * o] : 0.0;
+#pragma unroll
+                    for (int o = 0; o < 4; ++o) dmma884(acc[r][o][0], acc[r][o][1], av[o], bv);
+                }
+                __syncwarp();  // every lane has read the stage before lane 0 refills it
+            }
+        }
+
+        const ColInfo ci = col_info(A, chunk * (NC / 2) + fk);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int g = warp * R + r;
+            if (g >= G || !ci.valid) continue;
+            if (ci.minus && m == 0) continue;
+            const int row = ci.minus ? A.n_rowm[q] : A.n_row[q];
+            const int mi = A.isReal ? m : (ci.minus ? Lg - 1 - m : Lg - 1 + m);
+#pragma unroll
+            for (int o = 0; o < 4; ++o) {
+                const int t = A.ring[g * 32 + o * 8 + fr];
+                if (t < 0) continue;
+                A.F[(((size_t)ci.b * A.nrows + row) * Lg + t) * Md + mi] = cmake(acc[r][o][0], acc[r][o][1]);
+            }
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // layout conversion between the user's flm[b][l][m+L-1] and the internal m-major flmT[b][mi][l]
 // ---------------------------------------------------------------------------------------------------------------
@@ -888,8 +1098,36 @@ int dispatch_fwd(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t st)
     return S2W_EINVAL;
 }
 
+// the TMA-staged inverse kernel: 3 stages per warp at 8 warps (two blocks per SM), 2 at 16 warps
+template <int R, int MAXT>
+int launch_inv_pre_tma(const WigArgs &A, int T, int chunks, cudaStream_t st)
+{
+    constexpr int STAGES = MAXT <= 256 ? 3 : 2;
+    const size_t smem = (size_t)(MAXT / 32) * STAGES * (PreStage<R>::doubles * sizeof(double) + sizeof(unsigned long long));
+    int rc = set_smem(precomp_inverse_tma_kernel<R, MAXT, STAGES>, smem);
+    if (rc) return rc;
+    dim3 grid(A.Lg, chunks);
+    S2W_LAUNCH_C(S2W_K_WIGNER_INV, (precomp_inverse_tma_kernel<R, MAXT, STAGES>), grid, T, smem, st, A);
+    return S2W_OK;
+}
+
 int dispatch_inv_pre(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t st)
 {
+    static const bool tma = [] {
+        const char *e = getenv("S2W_PRE_TMA");
+        return !(e && e[0] == '0');
+    }();
+    if (tma) {
+#define S2W_WIG_CASE(RR, MT) \
+    if (c.R == RR && c.MAXT == MT) return launch_inv_pre_tma<RR, MT>(A, 32 * c.W, chunks, st);
+        S2W_WIG_CASE(1, 256)
+        S2W_WIG_CASE(2, 256)
+        S2W_WIG_CASE(3, 256)
+        S2W_WIG_CASE(4, 256)
+        S2W_WIG_CASE(3, 512)
+        S2W_WIG_CASE(4, 512)
+#undef S2W_WIG_CASE
+    }
 #define S2W_WIG_CASE(RR, MT)                                                                                  \
     if (c.R == RR && c.MAXT == MT) {                                                                          \
         dim3 grid(A.Lg, chunks);                                                                              \
