@@ -91,6 +91,36 @@ def z_inverse(flmp, L, P, tau, prec="f80"):
 
 
 # --------------------------------------------------------------------------
+# Q, Q^-1: Wigner-Laguerre transforms on H^4 = R+ x SO(3) (Eqs. 24-25): Q = K D, with
+# D of Eq. 4 (no conjugate, reading R6) and K of Eq. 7.  Reading R18: Eq. 24 prints Q^* in the analysis integral, which
+# contradicts P:424 ("Q = K D", D as in Eq. 4) and Eqs. 4-5; the basis function is Q^l_{mnp}(h) = K_p(r) D^l_{mn}(rho),
+# analysis  f^l_{mnp} = int f Q^l_{mnp} r^2 dr dOmega(rho),  synthesis  f = sum (2l+1)/(8 pi^2) f^l_{mnp} K_p D^{l*}_{mn}.
+#   f      [P][2N-1][L][2L-1]   samples f(r_i, gamma_g, beta_t, alpha_a) on the Gauss-Laguerre shells x the MW grid
+#   fhat   [2N-1][P][L][2L-1]   f^l_{mnp} at [n+N-1][p][l][m+L-1], |n| <= min(N-1, l)
+# --------------------------------------------------------------------------
+def q_forward(f, L, P, N, tau, prec="f80"):
+    ct = CPLX[prec]
+    per_shell = np.stack([S.wigner_forward(f[i], L, N, prec) for i in range(P)])      # [i][n][l][m]: D, Eq. 4
+    out = np.empty((2 * N - 1, P, L, 2 * L - 1), dtype=ct)
+    for ni in range(2 * N - 1):
+        out[ni] = laguerre_forward(per_shell[:, ni], P, tau, prec)                   # K, Eq. 7
+    return out
+
+
+def q_inverse(fhat, L, P, N, tau, prec="f80"):
+    rt, ct = REAL[prec], CPLX[prec]
+    fhat = fhat.astype(ct)
+    ell = np.arange(L).astype(rt)
+    w = (2 * ell + 1) / (8 * S.pi(prec) ** 2)                                          # Eq. 5 / Eq. 25
+    shells = np.stack([laguerre_inverse(fhat[ni], P, tau, prec) for ni in range(2 * N - 1)])   # [n][i][l][m]: K^-1
+    out = np.empty((P, 2 * N - 1, L, 2 * L - 1), dtype=ct)
+    for i in range(P):
+        X = shells[:, i] * w[None, :, None]
+        out[i] = S.wigner_inverse(X, L, N, prec)                                      # D^-1, Eq. 5 with Eq. 47
+    return out
+
+
+# --------------------------------------------------------------------------
 # filters (Appendix A.3-A.4)
 # --------------------------------------------------------------------------
 def filters(L, P, N, lam, nu, J0, J0p, prec="f80"):

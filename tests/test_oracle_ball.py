@@ -111,3 +111,65 @@ def test_ball_round_trip(L, P, N, J0, J0p):
     for (j, jp), W in W_psi.items():
         assert W.shape == (S.bandlimit_of_scale(jp, P, 2, True), 2 * N - 1,
                            S.bandlimit_of_scale(j, L, 2, True), 2 * S.bandlimit_of_scale(j, L, 2, True) - 1)
+
+
+# ---- Wigner-Laguerre transform Q = K D (Eqs. 24-25; reading R18) ----
+def _random_fhat(L, P, N, seed):
+    """Band-limited coefficients f^l_{mnp}: |m| <= l, |n| <= min(N-1, l)."""
+    rng = np.random.default_rng(seed)
+    fh = rng.standard_normal((2 * N - 1, P, L, 2 * L - 1)) + 1j * rng.standard_normal((2 * N - 1, P, L, 2 * L - 1))
+    ell = np.arange(L)[:, None]
+    m = np.arange(-(L - 1), L)[None, :]
+    fh *= (np.abs(m) <= ell)[None, None]
+    for ni in range(2 * N - 1):
+        fh[ni] *= (abs(ni - (N - 1)) <= np.arange(L))[None, :, None]
+    return fh
+
+
+def test_wigner_laguerre_inverse_is_the_literal_sum_of_eq_25():
+    """q_inverse at sampled points h = (r_i, alpha, beta, gamma) against Eq. 25 written out: sum over (l, m, n, p) of
+    (2l+1)/(8 pi^2) f^l_{mnp} K_p(r) d^l_{mn}(beta) e^{i(m alpha + n gamma)} (D^* of Eq. 47), with K_p from its own
+    closed form (scipy genlaguerre) and d^l_{mn} from the long-double recursion pinned in test_oracle_sphere."""
+    from scipy.special import eval_genlaguerre, gammaln
+    L, P, N, tau = 5, 4, 3, 1.3
+    fh = _random_fhat(L, P, N, 3)
+    f = B.q_inverse(fh, L, P, N, tau, "f80")
+    r, _ = B.radial_nodes(P, tau, "f80")
+    th = S.mw_thetas(L, "f80").astype(float)
+    ph = S.mw_phis(L, "f80").astype(float)
+    for (i, g, t, a) in [(0, 0, 0, 0), (1, 3, 2, 5), (3, 4, 4, 8), (2, 1, 3, 2)]:
+        gam = 2 * np.pi * g / (2 * N - 1)
+        tot = 0
+        for p in range(P):
+            x = float(r[i]) / tau
+            Kp = np.exp(0.5 * (gammaln(p + 1) - gammaln(p + 3))) * tau ** -1.5 * np.exp(-x / 2) * eval_genlaguerre(p, 2, x)
+            for n in range(-(N - 1), N):
+                for m in range(-(L - 1), L):
+                    d = S.wigner_d(L, m, n, LD(th[t]), "f80").astype(float)
+                    for l in range(max(abs(m), abs(n)), L):
+                        tot += (2 * l + 1) / (8 * np.pi ** 2) * fh[n + N - 1, p, l, m + L - 1] * Kp * d[l] \
+                            * np.exp(1j * (m * ph[a] + n * gam))
+        assert abs(complex(f[i, g, t, a]) - tot) < 1e-12 * max(1.0, abs(tot))
+
+
+def test_wigner_laguerre_forward_inverts_the_inverse():
+    """Q Q^-1 = identity on band-limited coefficients (orthogonality and completeness behind Eq. 25), odd and even N."""
+    for (L, P, N, tau) in ((6, 5, 3, 1.0), (5, 3, 2, 0.7), (4, 6, 4, 2.0)):
+        fh = _random_fhat(L, P, N, L + P + N)
+        back = B.q_forward(B.q_inverse(fh, L, P, N, tau, "f80"), L, P, N, tau, "f80")
+        assert np.abs(back - fh).max() < 1e-13 * np.abs(fh).max()
+
+
+def test_wigner_laguerre_reduces_to_its_factors():
+    """N = 1: Q is the spherical-Laguerre transform Z (D with n = 0 is the SHT up to the 2 pi of the gamma integral and
+    sqrt(4pi/(2l+1)): D^l_{m0} = sqrt(4pi/(2l+1)) Y*_{lm}); a radially constant-in-p input reduces K to one column."""
+    L, P, tau = 6, 4, 1.0
+    rng = np.random.default_rng(5)
+    flmp = rng.standard_normal((P, L, 2 * L - 1)) + 1j * rng.standard_normal((P, L, 2 * L - 1))
+    flmp *= (np.abs(np.arange(-(L - 1), L))[None, :] <= np.arange(L)[:, None])[None]
+    f = B.z_inverse(flmp, L, P, tau, "f80")                     # [P][L][2L-1], a function on the ball
+    qh = B.q_forward(f[:, None], L, P, 1, tau, "f80")[0]         # the same function, constant in gamma
+    ell = np.arange(L)
+    expect = 2 * np.pi * np.sqrt(4 * np.pi / (2 * ell + 1))[None, :, None] * flmp
+    # int f D^l_{m0} = 2 pi sqrt(4pi/(2l+1)) int f Y*_{lm}: Y*_{lm} = (-1)^m Y_{l,-m} is what D^l_{m0} = d^l_{m0} e^{-i m alpha} gives
+    assert np.abs(qh - expect).max() < 1e-12 * np.abs(expect).max()
