@@ -142,6 +142,24 @@ int s2ball_inverse_host(const void *w_host, void *f_host, int L, int P, int N, d
                         int J0, double tau, int flags);
 
 /* Drop every cached plan and workspace. */
+/* ---- the generalised Fourier transforms on B^3 and H^4 as stand-alone calls ----
+ * Z = K Y, the spherical-Laguerre transform (Eqs. 9-11): f [P][L][2L-1] samples on the P Gauss-Laguerre shells
+ * r_i = tau x_i (s2ball_radial_nodes) x the MW grid  <->  f_{lmp} [P][L][2L-1] at [p][l][m+L-1]; double with S2W_REAL
+ * in flags (the coefficients are complex128 either way), complex128 otherwise.
+ * Q = K D, the Wigner-Laguerre transform on H^4 = R+ x SO(3) (Eqs. 24-25; "Q = K D"; reading R18: the
+ * basis function is Q^l_{mnp} = K_p(r) D^l_{mn}(rho) with Eq. 4 unconjugated and Eq. 5 conjugated, as printed there):
+ *   forward  f^l_{mnp} = int f(h) K_p(r) D^l_{mn}(rho) r^2 dr dOmega(rho)
+ *   inverse  f(h) = sum_{l,m,n,p} (2l+1)/(8 pi^2) f^l_{mnp} K_p(r) D^{l*}_{mn}(rho)
+ * f [P][2N-1][L][2L-1] complex128 = f(r_i, gamma_g, beta_t, alpha_a), gamma_g = 2 pi g/(2N-1), (beta_t, alpha_a) the MW
+ * grid; fhat [2N-1][P][L][2L-1] complex128 at [n+N-1][p][l][m+L-1], |n| <= min(N-1, l), |m| <= l.  Exact for functions
+ * band-limited at (L, N, P).  All pointers are device pointers owned by the caller; the calls are asynchronous on
+ * `stream` after the first call with given parameters (which builds and caches the plan; calls that share a cached plan
+ * are serialised).  Errors: S2W_EINVAL for L < 1, N < 1, N > L, N > 32, P < 1, tau <= 0, null pointers. */
+int s2ball_z_forward(const void *f_dev, void *flmp_dev, int L, int P, double tau, int flags, void *stream);
+int s2ball_z_inverse(const void *flmp_dev, void *f_dev, int L, int P, double tau, int flags, void *stream);
+int s2ball_q_forward(const void *f_dev, void *fhat_dev, int L, int P, int N, double tau, void *stream);
+int s2ball_q_inverse(const void *fhat_dev, void *f_dev, int L, int P, int N, double tau, void *stream);
+
 int s2w_cache_clear(void);
 
 /* FP64 pipe probe: runs a register-resident DFMA chain (kind 0) or an mma.sync m8n8k4 f64 chain (kind 1) on

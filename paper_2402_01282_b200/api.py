@@ -50,6 +50,10 @@ SIGNATURES = {
     "s2wav_inverse_host": (_c_int, [_c_vp, _c_vp, _c_int, _c_int, _c_dbl, _c_int, _c_int, _c_int, _c_int]),
     "s2ball_forward_host": (_c_int, [_c_vp, _c_vp, _c_int, _c_int, _c_int, _c_dbl, _c_dbl, _c_int, _c_dbl, _c_int]),
     "s2ball_inverse_host": (_c_int, [_c_vp, _c_vp, _c_int, _c_int, _c_int, _c_dbl, _c_dbl, _c_int, _c_dbl, _c_int]),
+    "s2ball_z_forward": (_c_int, [_c_vp, _c_vp, _c_int, _c_int, _c_dbl, _c_int, _c_vp]),
+    "s2ball_z_inverse": (_c_int, [_c_vp, _c_vp, _c_int, _c_int, _c_dbl, _c_int, _c_vp]),
+    "s2ball_q_forward": (_c_int, [_c_vp, _c_vp, _c_int, _c_int, _c_int, _c_dbl, _c_vp]),
+    "s2ball_q_inverse": (_c_int, [_c_vp, _c_vp, _c_int, _c_int, _c_int, _c_dbl, _c_vp]),
     "s2w_cache_clear": (_c_int, []),
     "s2w_probe_fp64": (_c_int, [_c_int, _c_int, ctypes.POINTER(_c_dbl)]),
     "s2w_timing_enable": (_c_int, [_c_int]),
@@ -456,6 +460,55 @@ def s2ball_inverse_host(w, L, P, N, lam_l, lam_p, J0, tau=1.0, out=None):
     _check(lib().s2ball_inverse_host(_np_ptr(w), _np_ptr(f), int(L), int(P), int(N), float(lam_l), float(lam_p),
                                      int(J0), float(tau), S2W_REAL if real else 0))
     return f
+
+
+# ------------------------------------------------------------------------------------------------
+# the generalised Fourier transforms on B^3 and H^4 as stand-alone calls (include/s2w.h)
+# ------------------------------------------------------------------------------------------------
+def s2ball_z_forward(f, L, P, tau=1.0):
+    """Spherical-Laguerre transform Z (Eq. 10): f CUDA tensor [P, L, 2L-1] (float64 or complex128) -> f_lmp [P, L, 2L-1]."""
+    torch = _torch()
+    f = f.contiguous()
+    real = _dtype_real(f.dtype)
+    if not f.is_cuda or f.numel() != P * L * (2 * L - 1):
+        raise ValueError("f: expected a CUDA tensor of %d elements [P, L, 2L-1]" % (P * L * (2 * L - 1)))
+    out = torch.empty((P, L, 2 * L - 1), dtype=torch.complex128, device=f.device)
+    _check(lib().s2ball_z_forward(f.data_ptr(), out.data_ptr(), int(L), int(P), float(tau), S2W_REAL if real else 0,
+                                  _stream_ptr(f.device)))
+    return out
+
+
+def s2ball_z_inverse(flmp, L, P, tau=1.0, real=False):
+    """Z^-1 (Eq. 11): f_lmp [P, L, 2L-1] complex128 -> f [P, L, 2L-1] (float64 if real)."""
+    torch = _torch()
+    flmp = flmp.contiguous()
+    _check_tensor(flmp, torch.complex128, P * L * (2 * L - 1), "flmp")
+    out = torch.empty((P, L, 2 * L - 1), dtype=torch.float64 if real else torch.complex128, device=flmp.device)
+    _check(lib().s2ball_z_inverse(flmp.data_ptr(), out.data_ptr(), int(L), int(P), float(tau), S2W_REAL if real else 0,
+                                  _stream_ptr(flmp.device)))
+    return out
+
+
+def s2ball_q_forward(f, L, P, N, tau=1.0):
+    """Wigner-Laguerre transform Q = K D (Eq. 24): f [P, 2N-1, L, 2L-1] complex128 -> fhat [2N-1, P, L, 2L-1]."""
+    torch = _torch()
+    f = f.contiguous()
+    _check_tensor(f, torch.complex128, P * (2 * N - 1) * L * (2 * L - 1), "f")
+    out = torch.empty((2 * N - 1, P, L, 2 * L - 1), dtype=torch.complex128, device=f.device)
+    _check(lib().s2ball_q_forward(f.data_ptr(), out.data_ptr(), int(L), int(P), int(N), float(tau),
+                                  _stream_ptr(f.device)))
+    return out
+
+
+def s2ball_q_inverse(fhat, L, P, N, tau=1.0):
+    """Q^-1 (Eq. 25): fhat [2N-1, P, L, 2L-1] complex128 -> f [P, 2N-1, L, 2L-1]."""
+    torch = _torch()
+    fhat = fhat.contiguous()
+    _check_tensor(fhat, torch.complex128, P * (2 * N - 1) * L * (2 * L - 1), "fhat")
+    out = torch.empty((P, 2 * N - 1, L, 2 * L - 1), dtype=torch.complex128, device=fhat.device)
+    _check(lib().s2ball_q_inverse(fhat.data_ptr(), out.data_ptr(), int(L), int(P), int(N), float(tau),
+                                  _stream_ptr(fhat.device)))
+    return out
 
 
 def probe_fp64(kind, device=0):

@@ -118,6 +118,8 @@ int launch_wigner_forward(const WigArgs &A, cudaStream_t st);   // rings -> harm
 
 int launch_flm_pack(const cplx *flm_user, cplx *flmT, int B, int L, bool real, cudaStream_t st);
 int launch_flm_unpack(const cplx *flmT, cplx *flm_user, int B, int L, bool real, cudaStream_t st);
+int launch_flm_pack_pm(const cplx *pos, const cplx *neg, cplx *flmT, int B, int L, cudaStream_t st);
+int launch_flm_unpack_pm(const cplx *flmT, cplx *pos, cplx *neg, int B, int L, cudaStream_t st);
 
 int probe_fp64(int kind, double *tflops);
 

@@ -185,6 +185,10 @@ struct s2w_plan {
     // ball, stacked shells: for a fixed angular scale j the radial scales j' differ only in their shell count P_j' and
     // share grid, filters and tables, so the shells of ALL j' are stacked (PS = sum_j' P_j') and every step of a scale j
     // is ONE launch over PS shells instead of one per (j, j') (Alg. 2)
+    // kind 2: Wigner-Laguerre plan (Q = K D on H^4 = R+ x SO(3), Eqs. 24-25): one single-row stage per signed n whose
+    // mirror columns land in the row of -n, and a stage listing all rows for the (alpha, gamma) FFT and the reweighting
+    std::vector<Stage> qst;
+    Stage qall;
     int PS;                       // stacked shells
     std::vector<Scale> ang;       // the angular stage of each j (Pj = PS)
     std::vector<size_t *> ang_off;  // device [PS]: element offset of stacked shell b's block of scale j in a coefficient array
@@ -741,7 +745,7 @@ int plan_common(s2w_plan *p)
 {
     int rc;
     p->tabn.clear();
-    for (int n = -(p->N - 1); n <= p->N - 1; n += 2) p->tabn.push_back(n);
+    for (int n = -(p->N - 1); n <= p->N - 1; n += (p->kind == 2 ? 1 : 2)) p->tabn.push_back(n);
     if (find_tab(p, -p->spin) < 0) p->tabn.push_back(-p->spin);
     if (find_tab(p, p->spin) < 0) p->tabn.push_back(p->spin);  // the mirror columns (-m, -s) run the recursion of +s
     p->tri = (size_t)p->L * (p->L + 1) / 2;
@@ -2303,6 +2307,158 @@ int s2w_plan_harmonic_inverse(const s2w_plan *p, const void *flm, void *f, void 
     return S2W_OK;
 }
 
+// ---- Wigner-Laguerre (Q) and spherical-Laguerre (Z) transforms as stand-alone calls (Eqs. 10-11, 24-25) ----------
+static int qplan_create(s2w_plan **out, int L, int P, int N, double tau, int device)
+{
+    *out = 0;
+    if (L < 1 || P < 1 || N < 1 || N > L || N > S2W_MAX_N || L > 2048 || !(tau > 0)) {
+        set_error("invalid argument: need 1 <= N <= L <= 2048, N <= 32, P >= 1, tau > 0");
+        return S2W_EINVAL;
+    }
+    S2W_CUDA_CHECK(cudaSetDevice(device));
+    s2w_plan *p = new s2w_plan();
+    int rc;
+    p->kind = 2;
+    p->spin = 0;
+    p->capture_stream = 0;
+    for (int i = 0; i < S2W_LANES - 1; ++i) {
+        p->lane_stream[i] = 0;
+        p->lane_join[i] = 0;
+    }
+    p->lane_fork = 0;
+    p->lanes_on = false;
+    p->L = L;
+    p->N = N;
+    p->P = P;
+    p->lambda = p->nu = 2.0;
+    p->tau = tau;
+    p->J0 = p->J = p->J0p = p->Jp = 0;
+    p->multires = 0;
+    p->flags = 0;
+    p->batch = 1;
+    p->device = device;
+    p->real = false;
+    p->Kfull_fwd = p->Kfull_inv = p->Kfull_fwdT = p->Kfull_invT = 0;
+    p->phi_ball = 0;
+    p->PS = 0;
+    S2W_PLAN_TRY(plan_common(p));
+    S2W_PLAN_TRY(build_grid(p, L));
+    const double pi = pi_d();
+    const int nn = 2 * N - 1;
+    std::vector<cplx> fa(L), fs(L);
+    for (int l = 0; l < L; ++l) {
+        fa[l] = cmake((2.0 * l + 1.0) / (8.0 * pi * pi), 0.0);        // Eq. 5 / Eq. 25
+        fs[l] = cmake(4.0 * pi * pi / (2.0 * L - 1.0), 0.0);          // Eq. 4 on the MW x gamma grid
+    }
+    std::vector<int> all_n, all_rows;
+    for (int n = -(N - 1); n <= N - 1; ++n) {
+        Stage st;
+        memset(&st, 0, sizeof(st));
+        st.grid = grid_index(p, L);
+        st.Lg = L;
+        st.lmin = 0;
+        st.nn = 1;
+        st.nrows = nn;
+        st.n_val[0] = n;
+        st.n_tab[0] = find_tab(p, n);
+        st.n_row[0] = n + N - 1;
+        st.n_rowm[0] = -n + N - 1;   // the mirror columns (-m, -n) belong to the row of -n
+        st.n_filtm[0] = 0;
+        S2W_PLAN_TRY(make_stage_filters(p, st, fa, fs, (2.0 * L - 1.0) * nn));
+        p->qst.push_back(st);
+        all_n.push_back(n);
+        all_rows.push_back(n + N - 1);
+    }
+    memset(&p->qall, 0, sizeof(p->qall));
+    p->qall.grid = grid_index(p, L);
+    p->qall.Lg = L;
+    S2W_PLAN_TRY(fill_stage_rows(p, p->qall, all_n, all_rows, nn));
+    {
+        std::vector<double> x, qw, K;
+        gauss_laguerre2(P, x, qw);
+        if ((int)x.size() != P) {
+            set_error("Gauss-Laguerre root search failed");
+            s2w_plan_destroy(p);
+            return S2W_EUNSUPPORTED;
+        }
+        laguerre_basis(P, x, tau, K);
+        const double t3 = tau * tau * tau;
+        std::vector<double> fwd((size_t)P * P), inv((size_t)P * P);
+        for (int pp = 0; pp < P; ++pp)
+            for (int i = 0; i < P; ++i) {
+                fwd[(size_t)pp * P + i] = t3 * qw[i] * K[(size_t)pp * P + i];
+                inv[(size_t)i * P + pp] = K[(size_t)pp * P + i];
+            }
+        S2W_PLAN_TRY(p->pool.upload(&p->Kfull_fwd, fwd));
+        S2W_PLAN_TRY(p->pool.upload(&p->Kfull_inv, inv));
+    }
+    p->signal_elems = p->coeff_elems = (size_t)P * nn * L * (2 * L - 1);
+    p->ws_shell_elems = (((size_t)P * (2 * L - 1) * L + 15) / 16) * 16;      // one internal [P][Mfull][L] array
+    p->ws_F_elems = (((size_t)P * nn * L * (2 * L - 1) + 15) / 16) * 16;     // F and Ft
+    p->ws_flm_elems = 2 * (size_t)nn * p->ws_shell_elems;                   // H_n and G_n for every signed n
+    p->ws_bytes = (p->ws_flm_elems + 2 * p->ws_F_elems) * sizeof(cplx) + 256;
+    S2W_PLAN_TRY(cudaDeviceSynchronize() == cudaSuccess ? S2W_OK : S2W_ECUDA);
+    *out = p;
+    return S2W_OK;
+}
+
+// f [P][2N-1][L][2L-1] -> fhat [2N-1][P][L][2L-1]
+static int q_forward_dev(const s2w_plan *p, const void *f, void *fhat, void *work, cudaStream_t s)
+{
+    const int L = p->L, P = p->P, nn = 2 * p->N - 1;
+    cplx *H = (cplx *)align256(work), *Gb = H + (size_t)nn * p->ws_shell_elems;
+    cplx *F = Gb + (size_t)nn * p->ws_shell_elems, *Ft = F + p->ws_F_elems;
+    const GridTab &g = p->grids[p->qall.grid];
+    const size_t cols = (size_t)(2 * L - 1) * L, blk = (size_t)P * L * (2 * L - 1);
+    int rc;
+    So3Args S;
+    fill_so3_args(p, p->qall, S);
+    if ((rc = launch_so3_fwd(false, f, (size_t)nn * L * (2 * L - 1), F, S, P, g.fft, s))) return rc;
+    RwArgs R;
+    fill_rw_args(p, p->qall, R);
+    if ((rc = g.rw.L ? launch_reweight_th(F, Ft, R, P, g.rw, s) : launch_reweight(F, Ft, R, P, g.fft, s))) return rc;
+    S2W_CUDA_CHECK(cudaMemsetAsync(H, 0, (size_t)nn * p->ws_shell_elems * sizeof(cplx), s));
+    for (int q = 0; q < nn; ++q) {
+        WigArgs A;
+        fill_wig_args(p, p->qst[q], true, P, H + (size_t)q * p->ws_shell_elems, Ft, A);
+        if ((rc = launch_wigner_forward(A, s))) return rc;
+        if ((rc = launch_radial(p->Kfull_fwd, P, P, H + (size_t)q * p->ws_shell_elems, Gb + (size_t)q * p->ws_shell_elems, cols,
+                                L, 0, 0, false, s)))
+            return rc;
+    }
+    for (int q = 0; q < nn; ++q)
+        if ((rc = launch_flm_unpack_pm(Gb + (size_t)q * p->ws_shell_elems, (cplx *)fhat + (size_t)q * blk,
+                                       (cplx *)fhat + (size_t)(nn - 1 - q) * blk, P, L, s)))
+            return rc;
+    S2W_CUDA_CHECK(cudaPeekAtLastError());
+    return S2W_OK;
+}
+
+static int q_inverse_dev(const s2w_plan *p, const void *fhat, void *f, void *work, cudaStream_t s)
+{
+    const int L = p->L, P = p->P, nn = 2 * p->N - 1;
+    cplx *H = (cplx *)align256(work), *Gb = H + (size_t)nn * p->ws_shell_elems;
+    cplx *F = Gb + (size_t)nn * p->ws_shell_elems;
+    const GridTab &g = p->grids[p->qall.grid];
+    const size_t cols = (size_t)(2 * L - 1) * L, blk = (size_t)P * L * (2 * L - 1);
+    int rc;
+    for (int q = 0; q < nn; ++q) {
+        cplx *Gq = Gb + (size_t)q * p->ws_shell_elems, *Hq = H + (size_t)q * p->ws_shell_elems;
+        if ((rc = launch_flm_pack_pm((const cplx *)fhat + (size_t)q * blk, (const cplx *)fhat + (size_t)(nn - 1 - q) * blk, Gq, P,
+                                     L, s)))
+            return rc;
+        if ((rc = launch_radial(p->Kfull_inv, P, P, Gq, Hq, cols, L, 0, 0, false, s))) return rc;
+        WigArgs A;
+        fill_wig_args(p, p->qst[q], false, P, Hq, F, A);
+        if ((rc = launch_wigner_inverse(A, s))) return rc;
+    }
+    So3Args S;
+    fill_so3_args(p, p->qall, S);
+    if ((rc = launch_so3_inv(false, F, f, (size_t)nn * L * (2 * L - 1), S, P, g.fft, s))) return rc;
+    S2W_CUDA_CHECK(cudaPeekAtLastError());
+    return S2W_OK;
+}
+
 // ---- plan cache behind the argument-style entry points ----
 namespace {
 struct CacheKey {
@@ -2369,8 +2525,9 @@ int cached_plan(int kind, int L, int P, int N, double lambda, double nu, double 
         ne.work = 0;
         ne.d_sig = ne.d_cof = 0;
         ne.sync = 0;
-        int rc = kind == 0 ? s2wav_plan_create(&ne.plan, L, N, lambda, J0, multires, flags, batch, device)
-                           : s2ball_plan_create(&ne.plan, L, P, N, lambda, nu, J0, tau, flags, device);
+        int rc = kind == 0   ? s2wav_plan_create(&ne.plan, L, N, lambda, J0, multires, flags, batch, device)
+                 : kind == 1 ? s2ball_plan_create(&ne.plan, L, P, N, lambda, nu, J0, tau, flags, device)
+                             : qplan_create(&ne.plan, L, P, N, tau, device);
         if (rc) return rc;
         cudaError_t ce = cudaMalloc(&ne.work, s2w_plan_workspace_bytes(ne.plan));
         if (ce != cudaSuccess) {
@@ -2538,6 +2695,49 @@ int s2ball_inverse_host(const void *w, void *f, int L, int P, int N, double lamb
     int rc = cached_plan_staged(1, L, P, N, lambda_l, lambda_p, tau, J0, 1, flags, 1, &e);
     if (rc) return rc;
     return host_transform(false, e, w, f);
+}
+
+// Z = K Y, Z^-1 (Eqs. 10-11): the harmonic taps of a cached ball plan
+int s2ball_z_forward(const void *f, void *flmp, int L, int P, double tau, int flags, void *stream)
+{
+    CacheEntry e;
+    int rc = cached_plan(1, L, P, 1, 2.0, 2.0, tau, 0, 1, flags, 1, &e);
+    if (rc) return rc;
+    return entry_serialised(e, (cudaStream_t)stream,
+                            [&](cudaStream_t st) { return s2w_plan_harmonic_forward(e.plan, f, flmp, e.work, (void *)st); });
+}
+int s2ball_z_inverse(const void *flmp, void *f, int L, int P, double tau, int flags, void *stream)
+{
+    CacheEntry e;
+    int rc = cached_plan(1, L, P, 1, 2.0, 2.0, tau, 0, 1, flags, 1, &e);
+    if (rc) return rc;
+    return entry_serialised(e, (cudaStream_t)stream,
+                            [&](cudaStream_t st) { return s2w_plan_harmonic_inverse(e.plan, flmp, f, e.work, (void *)st); });
+}
+// Q = K D, Q^-1 (Eqs. 24-25)
+int s2ball_q_forward(const void *f, void *fhat, int L, int P, int N, double tau, void *stream)
+{
+    if (!f || !fhat) {
+        set_error("null pointer");
+        return S2W_EINVAL;
+    }
+    CacheEntry e;
+    int rc = cached_plan(2, L, P, N, 2.0, 2.0, tau, 0, 0, 0, 1, &e);
+    if (rc) return rc;
+    return entry_serialised(e, (cudaStream_t)stream,
+                            [&](cudaStream_t st) { return q_forward_dev(e.plan, f, fhat, e.work, st); });
+}
+int s2ball_q_inverse(const void *fhat, void *f, int L, int P, int N, double tau, void *stream)
+{
+    if (!f || !fhat) {
+        set_error("null pointer");
+        return S2W_EINVAL;
+    }
+    CacheEntry e;
+    int rc = cached_plan(2, L, P, N, 2.0, 2.0, tau, 0, 0, 0, 1, &e);
+    if (rc) return rc;
+    return entry_serialised(e, (cudaStream_t)stream,
+                            [&](cudaStream_t st) { return q_inverse_dev(e.plan, fhat, f, e.work, st); });
 }
 
 int s2w_cache_clear(void)

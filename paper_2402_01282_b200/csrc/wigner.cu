@@ -992,6 +992,25 @@ __global__ void flm_unpack_kernel(const cplx *__restrict__ flmT, cplx *__restric
     flm[((size_t)b * L + l) * (2 * L - 1) + mi] = v;
 }
 
+__global__ void flm_pack_pm_kernel(const cplx *__restrict__ pos, const cplx *__restrict__ neg, cplx *__restrict__ flmT, int L)
+{
+    const int l = blockIdx.x * blockDim.x + threadIdx.x, mi = blockIdx.y, b = blockIdx.z;
+    if (l >= L) return;
+    const int m = mi - (L - 1), am = m < 0 ? -m : m;
+    cplx v = cmake(0.0, 0.0);
+    if (am <= l) v = (m >= 0 ? pos : neg)[((size_t)b * L + l) * (2 * L - 1) + mi];
+    flmT[((size_t)b * (2 * L - 1) + mi) * L + l] = v;
+}
+
+__global__ void flm_unpack_pm_kernel(const cplx *__restrict__ flmT, cplx *__restrict__ pos, cplx *__restrict__ neg, int L)
+{
+    const int l = blockIdx.x * blockDim.x + threadIdx.x, mi = blockIdx.y, b = blockIdx.z;
+    if (l >= L) return;
+    const int m = mi - (L - 1), am = m < 0 ? -m : m;
+    const cplx v = am <= l ? flmT[((size_t)b * (2 * L - 1) + mi) * L + l] : cmake(0.0, 0.0);
+    (m >= 0 ? pos : neg)[((size_t)b * L + l) * (2 * L - 1) + mi] = v;
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // FP64 pipe probes
 // ---------------------------------------------------------------------------------------------------------------
@@ -1203,6 +1222,21 @@ int launch_wigner_table(const double *coef, size_t tri, int Lfull, int Lg, int G
 
 int launch_wigner_inverse(const WigArgs &A, cudaStream_t st) { return launch_wigner(false, A, st); }
 int launch_wigner_forward(const WigArgs &A, cudaStream_t st) { return launch_wigner(true, A, st); }
+
+// Wigner-Laguerre transform: the internal array of the signed row n holds f_{m,n} for m >= 0 and f_{m,-n} for m < 0 (the
+// contraction kernels pair the column (m, n) with (-m, -n)); pos / neg are the user arrays [b][l][m+L-1] of n and -n.
+int launch_flm_pack_pm(const cplx *pos, const cplx *neg, cplx *flmT, int B, int L, cudaStream_t st)
+{
+    dim3 grid((L + 127) / 128, 2 * L - 1, B);
+    S2W_LAUNCH(flm_pack_pm_kernel, grid, 128, 0, st, pos, neg, flmT, L);
+    return S2W_OK;
+}
+int launch_flm_unpack_pm(const cplx *flmT, cplx *pos, cplx *neg, int B, int L, cudaStream_t st)
+{
+    dim3 grid((L + 127) / 128, 2 * L - 1, B);
+    S2W_LAUNCH(flm_unpack_pm_kernel, grid, 128, 0, st, flmT, pos, neg, L);
+    return S2W_OK;
+}
 
 int launch_flm_pack(const cplx *flm_user, cplx *flmT, int B, int L, bool real, cudaStream_t st)
 {

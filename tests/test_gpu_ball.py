@@ -181,3 +181,55 @@ def test_table2_shape_full_size():
     back = plan.inverse(w)
     assert float((back - f).abs().max() / f.abs().max()) < RT_TOL
     plan.close()
+
+
+# ---- stand-alone generalised Fourier transforms on B^3 and H^4 ----
+def _band_limited_fhat(L, P, N, seed):
+    rng = np.random.default_rng(seed)
+    fh = rng.standard_normal((2 * N - 1, P, L, 2 * L - 1)) + 1j * rng.standard_normal((2 * N - 1, P, L, 2 * L - 1))
+    ell = np.arange(L)[:, None]
+    m = np.arange(-(L - 1), L)[None, :]
+    fh *= (np.abs(m) <= ell)[None, None]
+    for ni in range(2 * N - 1):
+        fh[ni] *= (abs(ni - (N - 1)) <= np.arange(L))[None, :, None]
+    return fh
+
+
+@pytest.mark.parametrize("L,P,N,tau", [(8, 6, 3, 1.0), (12, 5, 2, 0.7), (20, 9, 4, 1.5), (33, 16, 1, 1.0)])
+def test_wigner_laguerre_transform_matches_oracle(L, P, N, tau):
+    """s2ball_q_inverse / s2ball_q_forward (Q = K D, Eqs. 24-25) element by element against oracle.ball.q_inverse /
+    q_forward, odd and even N, and Q Q^-1 = identity on the GPU."""
+    import torch
+    from paper_2402_01282_b200 import api
+    from oracle import ball as B
+    fh = _band_limited_fhat(L, P, N, 40 + L)
+    f_ref = B.q_inverse(fh, L, P, N, tau, "f80").astype(np.complex128)
+    f_gpu = api.s2ball_q_inverse(torch.from_numpy(fh).cuda(), L, P, N, tau)
+    assert np.abs(f_gpu.cpu().numpy() - f_ref).max() < 1e-11 * np.abs(f_ref).max()
+    fh_ref = B.q_forward(f_ref, L, P, N, tau, "f80").astype(np.complex128)
+    fh_gpu = api.s2ball_q_forward(torch.from_numpy(np.ascontiguousarray(f_ref)).cuda(), L, P, N, tau)
+    assert np.abs(fh_gpu.cpu().numpy() - fh_ref).max() < 1e-11 * np.abs(fh_ref).max()
+    back = api.s2ball_q_forward(f_gpu, L, P, N, tau).cpu().numpy()
+    assert np.abs(back - fh).max() < 1e-12 * np.abs(fh).max()
+
+
+@pytest.mark.parametrize("L,P,tau,real", [(10, 7, 1.0, False), (16, 12, 1.3, True)])
+def test_spherical_laguerre_entry_points_match_oracle(L, P, tau, real):
+    """s2ball_z_forward / s2ball_z_inverse (Z = K Y, Eqs. 10-11) against oracle.ball.z_forward / z_inverse."""
+    import torch
+    from paper_2402_01282_b200 import api, inputs
+    from oracle import ball as B
+    flmp = inputs.flmp_complex(L, P, 77)
+    if real:
+        m = np.arange(-(L - 1), L)
+        flmp = 0.5 * (flmp + ((-1.0) ** np.abs(m))[None, None, :] * np.conj(flmp[:, :, ::-1]))
+    f_ref = B.z_inverse(flmp, L, P, tau, "f80")
+    if real:
+        assert np.abs(f_ref.imag).max() < 1e-14 * np.abs(f_ref).max()
+    f_gpu = api.s2ball_z_inverse(torch.from_numpy(flmp).cuda(), L, P, tau, real=real).cpu().numpy()
+    ref = f_ref.real.astype(np.float64) if real else f_ref.astype(np.complex128)
+    assert np.abs(f_gpu - ref).max() < 1e-11 * np.abs(ref).max()
+    back = api.s2ball_z_forward(torch.from_numpy(np.ascontiguousarray(ref)).cuda(), L, P, tau).cpu().numpy()
+    assert np.abs(back - flmp).max() < 1e-12 * np.abs(flmp).max()
+    z_ref = B.z_forward(f_ref, L, P, tau, "f80").astype(np.complex128)
+    assert np.abs(back - z_ref).max() < 1e-11 * np.abs(z_ref).max()
