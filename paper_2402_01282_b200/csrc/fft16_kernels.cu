@@ -630,6 +630,135 @@ __global__ void __launch_bounds__(256, 2) so3_fwd_c16_kernel(const cplx *__restr
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// a1 ring FFTs (Eqs. 2-3) on the radix-16 core: a block works on NB sequences, each a pair of real rings (one
+// complex DFT, split by Hermitian symmetry) or one complex ring.  Layouts as in ring_fwd_kernel / ring_inv_kernel.
+// ---------------------------------------------------------------------------------------------------------------
+template <int R1, bool REAL>
+__global__ void __launch_bounds__(256, 2) ring_fwd16_kernel(const void *__restrict__ in, cplx *__restrict__ out, int nrows,
+                                                           size_t sig_stride, FftTab T)
+{
+    constexpr int NB = 16 / R1, HR = R1 >= 2 ? R1 / 2 : 1, M = R1 * 256;
+    extern __shared__ cplx buf[];
+    const F16Tw tw = f16_twiddles<R1>();
+    const int n = T.n, L = T.L;
+    const double inv_n = 1.0 / (double)n;
+    cplx x[NB][R1];
+#pragma unroll
+    for (int q = 0; q < NB; ++q) {
+        const int s = blockIdx.x * NB + q;
+        const int r0 = REAL ? 2 * s : s, r1 = r0 + 1;
+        const bool on0 = r0 < nrows, on1 = REAL && r1 < nrows;
+        const size_t o0 = (size_t)((on0 ? r0 : 0) / L) * sig_stride + (size_t)((on0 ? r0 : 0) % L) * n;
+        const size_t o1 = (size_t)((on1 ? r1 : 0) / L) * sig_stride + (size_t)((on1 ? r1 : 0) % L) * n;
+#pragma unroll
+        for (int c = 0; c < HR; ++c) {
+            const int pp = threadIdx.x + 256 * c;
+            const int pk = (pp < n && on0) ? pp : 0;
+            cplx v;
+            if (REAL) {
+                const double a = ((const double *)in)[o0 + pk], b = ((const double *)in)[o1 + pk];
+                v = cmake(a, on1 ? b : 0.0);
+            } else {
+                v = ((const cplx *)in)[o0 + pk];
+            }
+            x[q][c] = (pp < n && on0) ? cmul(v, __ldg(&T.chirp[pk])) : cmake(0.0, 0.0);
+        }
+    }
+    f16_convolve_half<R1>(buf, x, T.bhat16_m, tw);
+    if (REAL) {
+#pragma unroll
+        for (int q = 0; q < NB; ++q)
+#pragma unroll
+            for (int c = 0; c < HR; ++c) {
+                const int k = threadIdx.x + 256 * c;
+                buf[F16_PAD(q * M + k)] = cmul(x[q][c], __ldg(&T.chirp[k < n ? k : 0]));
+            }
+        __syncthreads();
+#pragma unroll 1
+        for (int q = 0; q < NB; ++q) {
+            const int r0 = 2 * (blockIdx.x * NB + q), r1 = r0 + 1;
+            if (r0 >= nrows) continue;
+            for (int m = threadIdx.x; m < L; m += 256) {
+                const cplx a = buf[F16_PAD(q * M + m)], b = cconj(buf[F16_PAD(q * M + (m == 0 ? 0 : n - m))]);
+                const cplx sm = cadd(a, b), d = csub(a, b);
+                out[(size_t)r0 * L + m] = cscale(sm, 0.5 * inv_n);
+                if (r1 < nrows) out[(size_t)r1 * L + m] = cmake(0.5 * inv_n * d.y, -0.5 * inv_n * d.x);
+            }
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < NB; ++q) {
+            const int r0 = blockIdx.x * NB + q;
+            if (r0 >= nrows) continue;
+#pragma unroll
+            for (int c = 0; c < HR; ++c) {
+                const int k = threadIdx.x + 256 * c;
+                if (k >= n) continue;
+                out[(size_t)r0 * n + (k < L ? k : k - n) + (L - 1)] = cscale(cmul(x[q][c], __ldg(&T.chirp[k])), inv_n);
+            }
+        }
+    }
+}
+
+template <int R1, bool REAL>
+__global__ void __launch_bounds__(256, 2) ring_inv16_kernel(const cplx *__restrict__ in, void *__restrict__ out, int nrows,
+                                                           size_t sig_stride, FftTab T)
+{
+    constexpr int NB = 16 / R1, HR = R1 >= 2 ? R1 / 2 : 1;
+    extern __shared__ cplx buf[];
+    const F16Tw tw = f16_twiddles<R1>();
+    const int n = T.n, L = T.L;
+    cplx x[NB][R1];
+#pragma unroll
+    for (int q = 0; q < NB; ++q) {
+        const int s = blockIdx.x * NB + q;
+        const int r0 = REAL ? 2 * s : s, r1 = r0 + 1;
+        const bool on0 = r0 < nrows, on1 = REAL && r1 < nrows;
+        const cplx *X0 = in + (size_t)(on0 ? r0 : 0) * (REAL ? L : n), *X1 = in + (size_t)(on1 ? r1 : 0) * L;
+#pragma unroll
+        for (int c = 0; c < HR; ++c) {
+            const int k = threadIdx.x + 256 * c;
+            const int kk = (k < n && on0) ? k : 0;
+            cplx v;
+            if (REAL) {
+                const int m = kk < L ? kk : n - kk;
+                cplx a = X0[m], b = X1[m];
+                if (!on1) b = cmake(0.0, 0.0);
+                if (kk >= L) {
+                    a = cconj(a);
+                    b = cconj(b);
+                }
+                v = cmake(a.x - b.y, a.y + b.x);  // Z_k = A_k + i B_k
+            } else {
+                v = X0[(kk < L ? kk : kk - n) + (L - 1)];
+            }
+            x[q][c] = (k < n && on0) ? cmulc(v, __ldg(&T.chirp[kk])) : cmake(0.0, 0.0);
+        }
+    }
+    f16_convolve_half<R1>(buf, x, T.bhat16_p, tw);
+#pragma unroll
+    for (int q = 0; q < NB; ++q) {
+        const int s = blockIdx.x * NB + q;
+        const int r0 = REAL ? 2 * s : s, r1 = r0 + 1;
+        if (r0 >= nrows) continue;
+        const size_t o0 = (size_t)(r0 / L) * sig_stride + (size_t)(r0 % L) * n;
+        const size_t o1 = (size_t)((r1 < nrows ? r1 : r0) / L) * sig_stride + (size_t)((r1 < nrows ? r1 : r0) % L) * n;
+#pragma unroll
+        for (int c = 0; c < HR; ++c) {
+            const int pp = threadIdx.x + 256 * c;
+            if (pp >= n) continue;
+            const cplx z = cmulc(x[q][c], __ldg(&T.chirp[pp]));
+            if (REAL) {
+                ((double *)out)[o0 + pp] = z.x;
+                if (r1 < nrows) ((double *)out)[o1 + pp] = z.y;
+            } else {
+                ((cplx *)out)[o0 + pp] = z;
+            }
+        }
+    }
+}
+
 // ---- plan time: kernel spectra in the core's own order --------------------------------------------------------------
 
 template <int R1>
@@ -760,6 +889,43 @@ int launch_so3_c16(bool fwd, const void *in, void *out, size_t sig_stride, const
     S2W_C16_CASE(1024, 4)
 #undef S2W_C16_CASE
     set_error("launch_so3_c16: unsupported length");
+    return S2W_EINVAL;
+}
+
+template <int R1, bool REAL>
+static int ring16_t(bool fwd, const void *in, void *out, int nrows, size_t sig_stride, const FftTab &T, cudaStream_t st)
+{
+    constexpr int NB = 16 / R1;
+    const size_t sm = (size_t)F16_BUF * sizeof(cplx);
+    const int nseq = REAL ? (nrows + 1) / 2 : nrows;
+    const int grid = (nseq + NB - 1) / NB;
+    int rc;
+    if (fwd) {
+        if ((rc = set_smem(ring_fwd16_kernel<R1, REAL>, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_RING_FFT, (ring_fwd16_kernel<R1, REAL>), grid, 256, sm, st, in, (cplx *)out, nrows, sig_stride, T);
+    } else {
+        if ((rc = set_smem(ring_inv16_kernel<R1, REAL>, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_RING_FFT, (ring_inv16_kernel<R1, REAL>), grid, 256, sm, st, (const cplx *)in, out, nrows,
+                     sig_stride, T);
+    }
+    return S2W_OK;
+}
+
+// a1 on the radix-16 core; the caller checks T.bhat16_m and f16_supported(T.M)
+int launch_ring16(bool fwd, bool real, const void *in, void *out, int nrows, size_t sig_stride, const FftTab &T,
+                  cudaStream_t st)
+{
+#define S2W_R16_CASE(MM, RR)                                                                   \
+    if (T.M == MM)                                                                             \
+        return real ? ring16_t<RR, true>(fwd, in, out, nrows, sig_stride, T, st)               \
+                    : ring16_t<RR, false>(fwd, in, out, nrows, sig_stride, T, st);
+    S2W_R16_CASE(4096, 16)
+    S2W_R16_CASE(2048, 8)
+    S2W_R16_CASE(1024, 4)
+    S2W_R16_CASE(512, 2)
+    S2W_R16_CASE(256, 1)
+#undef S2W_R16_CASE
+    set_error("launch_ring16: unsupported length");
     return S2W_EINVAL;
 }
 

@@ -96,6 +96,8 @@ int launch_fft16_spectrum(cplx *khat, int kind, int n, int M, cudaStream_t st); 
 int launch_so3_pair16(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch,
                       const FftTab &T, cudaStream_t st);                // a8, real signals, 2N-1 <= 9
 int launch_reweight16(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st);  // a2
+int launch_ring16(bool fwd, bool real, const void *in, void *out, int nrows, size_t sig_stride, const FftTab &T,
+                  cudaStream_t st);                                     // a1, M = 256 ... 4096
 bool so3_c16_supported(const So3Args &A, const FftTab &T);            // a8, complex signals, <= 3 rows, M = 256 ... 1024
 int launch_so3_c16(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
                    cudaStream_t st);

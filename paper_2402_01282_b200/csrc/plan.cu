@@ -28,10 +28,11 @@ void set_error(const std::string &msg) { g_err = msg; }
 void count_launch() { ++g_launches; }
 void debug_launch(const char *name)
 {
-    static const bool on = getenv("S2W_DEBUG_LAUNCH") != 0;
-    if (!on) return;
+    static const char *env = getenv("S2W_DEBUG_LAUNCH");
+    if (!env) return;
     static bool reported = false;
-    const cudaError_t e = cudaPeekAtLastError();
+    // "2": wait for the kernel, so that a fault is attributed to the launch that caused it (never under stream capture)
+    const cudaError_t e = env[0] == '2' ? cudaDeviceSynchronize() : cudaPeekAtLastError();
     if (e != cudaSuccess && !reported) {
         reported = true;
         fprintf(stderr, "[s2w] launch of %s left the error: %s\n", name, cudaGetErrorString(e));
@@ -2136,6 +2137,14 @@ static int run_transform(const s2w_plan *p, int dir, const void *in, void *out, 
         return dir == 0 ? sphere_forward(p, in, out, work, st) : sphere_inverse(p, in, out, work, st);
     };
     static const bool no_graph = getenv("S2W_NO_GRAPH") != 0;
+    static const bool lanes_direct = getenv("S2W_LANES_DIRECT") != 0;  // debugging: the lanes without a graph
+    if (no_graph && lanes_direct && !g_timing) {
+        std::lock_guard<std::mutex> lock(p->graph_mu);
+        p->lanes_on = true;
+        const int rc = direct(s);
+        p->lanes_on = false;
+        return rc;
+    }
     if (no_graph || g_timing) return direct(s);
     std::lock_guard<std::mutex> lock(p->graph_mu);
     for (auto &g : p->graphs)

@@ -1094,7 +1094,9 @@ __global__ void __launch_bounds__(256, 3) reweight_th_kernel(const cplx *__restr
     {
         const int nh = T.M >> 5;
         for (int i = threadIdx.x; i < nh; i += blockDim.x) s_tw[i] = R.fft.tw[(i << 5) * R.fft.twmul];
-        if (threadIdx.x < 32) s_tw[nh + threadIdx.x] = R.fft.tw[threadIdx.x * R.fft.twmul];
+        // (M < 32: only the first M entries exist -- reading on ran past the end of the plan's twiddle table, a fault that
+        // showed or not with the neighbouring allocations; entry 0 = 1 then also serves as the single "high" entry)
+        if (threadIdx.x < 32 && (int)threadIdx.x < T.M) s_tw[nh + threadIdx.x] = R.fft.tw[threadIdx.x * R.fft.twmul];
         T.twmul = 1;
         T.twmask = T.M - 1;
         T.twlo = 5;
@@ -1512,6 +1514,16 @@ size_t fft_smem_bytes(const FftTab &T) { return (size_t)fft_padded_len(T.M) * si
 
 // ---- host launchers -------------------------------------------------------------------------------------------
 
+// S2W_FFT16=0 in the environment keeps the radix-8 kernels (before / after measurements); read once
+static bool use_fft16()
+{
+    static const bool on = [] {
+        const char *e = getenv("S2W_FFT16");
+        return !(e && e[0] == '0');
+    }();
+    return on;
+}
+
 int launch_twiddles(cplx *tw, int Mtab, cudaStream_t st)
 {
     S2W_LAUNCH(twiddle_kernel, (Mtab + 255) / 256, 256, 0, st, tw, Mtab);
@@ -1536,6 +1548,7 @@ int launch_ring_fwd(bool real, const void *in, cplx *out, int B, int Lg, size_t 
 {
     const int nrows = B * Lg;
     if (nrows <= 0) return S2W_OK;
+    if (T.bhat16_m && f16_supported(T.M) && use_fft16()) return launch_ring16(true, real, in, out, nrows, sig_stride, T, st);
     size_t sm = fft_smem_bytes(T);
     int rc;
     if (real) {
@@ -1553,6 +1566,7 @@ int launch_ring_inv(bool real, const cplx *in, void *out, int B, int Lg, size_t 
 {
     const int nrows = B * Lg;
     if (nrows <= 0) return S2W_OK;
+    if (T.bhat16_m && f16_supported(T.M) && use_fft16()) return launch_ring16(false, real, in, out, nrows, sig_stride, T, st);
     size_t sm = fft_smem_bytes(T);
     int rc;
     if (real) {
@@ -1567,15 +1581,6 @@ int launch_ring_inv(bool real, const cplx *in, void *out, int B, int Lg, size_t 
 
 static int seqs_per_block(int fit, long long total, int cap);
 
-// S2W_FFT16=0 in the environment keeps the radix-8 kernels (before / after measurements); read once
-static bool use_fft16()
-{
-    static const bool on = [] {
-        const char *e = getenv("S2W_FFT16");
-        return !(e && e[0] == '0');
-    }();
-    return on;
-}
 
 template <bool REAL, bool MULTI>
 static int so3_launch_t(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch,
