@@ -458,7 +458,8 @@ def run_ours(args, cfg):
     roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak if peak else None,
                 "traffic": NCU_TRAFFIC.get((cfg["name"], dom)) if not (args.precompute or adj) else None,
-                "traffic_unit": "bytes per step (all launches of the class), ncu --set full, profiles/r01j_wigner_ncu.md",
+                "traffic_unit": "bytes per step (all launches of the class), ncu --set full, profiles/r01j_wigner_ncu.md "
+                                "(the Wigner kernels are unchanged since that capture)",
                 "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x sm_max_mhz (DESIGN.md); "
                                "measured DFMA-chain probe beside it",
                 "probe": probe, "tuples_per_step": tup, "flops_per_step": flops,
@@ -489,7 +490,7 @@ def run_ours(args, cfg):
         line["e2e"] = {"value": world * B / e2e_dt, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"],
                        "d2h_bytes_per_step": e2e["d2h"], "roundtrip_rel_err": e2e["rt_err"]}
     if not args.no_cpu_baseline and world == 1:
-        line["cpu_baseline"] = cpu_baseline(cfg)
+        line["cpu_baseline"] = cpu_baseline(cfg, budget=3.0)   # about 10-30 s of host work
         line["cpu_baseline"]["measured_small"] = oracle_measured_small()
     print(json.dumps(line))
     if world > 1:
