@@ -512,6 +512,132 @@ __global__ void __launch_bounds__(256, 2) reweight16_kernel(const cplx *__restri
     }
 }
 
+// a2 at Toeplitz length 256 (grids with 65 <= L_j <= 128: the two top angular scales of BASELINE config 5, over all
+// stacked shells).  A sequence is one half-warp's 256-point problem, so nothing crosses a warp: warp = column, its two
+// half-warps carry u1 = a x and u2 = delta a x; lane l holds the ring values x_t, t = l + 16 k (k < 8), feeds the
+// radix-16 pass straight from registers (upper half zero) and gets y(t) back from the last inverse pass -- no pass over
+// stride 256, no block barrier, and the partner spectrum U(-k) of the Hankel term lives in the same half-warp.
+__global__ void __launch_bounds__(256, 2) reweight16s_kernel(const cplx *__restrict__ F, cplx *__restrict__ Ft, RwArgs A,
+                                                            RwTab R, int ncolumns)
+{
+    extern __shared__ cplx buf[];
+    const int L = R.L, Lm = L - 1;
+    const int lane = threadIdx.x & 31, l = lane & 15, half = lane >> 4, warp = threadIdx.x >> 5;
+    const int colid = blockIdx.x * 8 + warp;
+    const bool has = colid < ncolumns;
+    const int mi = colid % A.Md, q = (colid / A.Md) % A.nn, b = colid / (A.Md * A.nn);
+    const int m = A.isReal ? mi : mi - (L - 1);
+    const int nv = has ? A.n_val[q] : 0, row = has ? A.n_row[q] : 0;
+    const int par = ((m + nv) & 1) ? 1 : 0;  // 0: sigma = +1, 1: sigma = -1
+    const cplx *col = F + ((size_t)(has ? b : 0) * A.nrows + row) * (size_t)L * A.Md + (has ? mi : 0);
+    cplx *colT = Ft + (((size_t)(has ? b : 0) * A.nrows + row) * A.Md + (has ? mi : 0)) * (size_t)L;
+    const double *rp = R.rpole + par * L, *vp = R.vpole + par * L;
+    double s, c;
+    sincospi(-2.0 * (double)l / 256.0, &s, &c);
+    const cplx w2 = cmake(c, s);
+
+    cplx xs[8];
+    cplx dot = cmake(0.0, 0.0), xpole = cmake(0.0, 0.0);
+    cplx v[16];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int t = l + 16 * k;
+        cplx xv = cmake(0.0, 0.0);
+        if (t < L && has) {
+            xv = col[(size_t)t * A.Md];
+            const double r = rp[t];
+            dot.x = fma(r, xv.x, dot.x);
+            dot.y = fma(r, xv.y, dot.y);
+        }
+        xs[k] = xv;
+        if (t == Lm) xpole = xv;
+        cplx u = cmake(0.0, 0.0);
+        if (t < Lm) {
+            u = (t & 1) ? cscale(xv, -1.0) : xv;
+            if (half) u = cscale(u, R.delta[t]);
+        }
+        v[k] = u;
+    }
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) {  // over the 16 lanes of the half-warp (both halves hold the same column)
+        dot.x += __shfl_xor_sync(0xffffffffu, dot.x, o);
+        dot.y += __shfl_xor_sync(0xffffffffu, dot.y, o);
+        xpole.x += __shfl_xor_sync(0xffffffffu, xpole.x, o);
+        xpole.y += __shfl_xor_sync(0xffffffffu, xpole.y, o);
+    }
+    cplx *seq = buf + F16_PAD((threadIdx.x >> 4) * 256);      // this half-warp's 256 elements (272 slots)
+    {   // radix-16 pass over stride 16 from registers
+        bfly16<false, true, false>(v);
+        twiddle_apply<16, false>(v, w2);
+        cplx *bq = seq + l;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) bq[17 * k] = v[k];
+    }
+    __syncwarp();
+    {   // innermost forward pass on 16 contiguous elements
+        cplx *bq = seq + 17 * l;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) v[k] = bq[k];
+        bfly16<false>(v);
+#pragma unroll
+        for (int k = 0; k < 16; ++k) bq[k] = v[k];
+    }
+    __syncwarp();
+    {   // Y(p) = That(p) U(p) -/+ sigma Ghat(p) U(p'), p = 16 j2 + j3 <-> k = j2 + 16 j3; p' = (16 - j2) % 16 * 16 + ...
+        const int j2 = l, j2p = (16 - j2) & 15;
+        const cplx *prt = seq + 17 * j2p;
+        const cplx *tg = R.TG16 + j2;                             // [2][256] in the storage order F16_TPOS
+        double sg = par ? -1.0 : 1.0;
+        if (!half) sg = -sg;                                      // u1: T - sigma H, u2: T + sigma H
+#pragma unroll
+        for (int j3 = 0; j3 < 16; ++j3) {
+            const cplx un = prt[j2 ? 15 - j3 : (16 - j3) & 15];
+            const cplx th = __ldg(&tg[16 * j3]), gh = cscale(__ldg(&tg[256 + 16 * j3]), sg);
+            v[j3] = cadd(cmul(th, v[j3]), cmul(gh, un));
+        }
+        __syncwarp();                                             // every partner value has been read
+        bfly16<true>(v);
+        cplx *bq = seq + 17 * l;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) bq[k] = v[k];
+    }
+    __syncwarp();
+    {   // inverse radix-16 pass over stride 16; only y(t), t = l + 16 k < 128, is formed
+        const cplx *bq = seq + l;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) v[k] = bq[17 * k];
+        twiddle_apply<16, true>(v, w2);
+        bfly16<true, false, true>(v);
+    }
+    // half 0 holds y1 = (T - sigma H) u1, half 1 holds y2 = (T + sigma H) u2: half 0 finishes k < 4, half 1 k >= 4
+    cplx other[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const cplx snd = half ? v[k] : v[k + 4];
+        other[k].x = __shfl_xor_sync(0xffffffffu, snd.x, 16);
+        other[k].y = __shfl_xor_sync(0xffffffffu, snd.y, 16);
+    }
+    if (!has) return;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int kk = half ? k + 4 : k;
+        const int t = l + 16 * kk;
+        const cplx mine = half ? v[k + 4] : v[k];
+        const cplx y1 = half ? other[k] : mine, y2 = half ? mine : other[k];
+        const cplx xv = half ? xs[k + 4] : xs[k];
+        if (t < Lm) {
+            const double dl = R.delta[t], ds = R.dsum[t], vv = vp[t];
+            cplx h = cmake(fma(dl, y1.x, -y2.x), fma(dl, y1.y, -y2.y));
+            if (t & 1) h = cscale(h, -1.0);
+            h.x += fma(ds, xv.x, vv * xpole.x);
+            h.y += fma(ds, xv.y, vv * xpole.y);
+            colT[t] = h;
+        } else if (t == Lm) {
+            colT[t] = dot;
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // a8 for complex signals (sphere configs 2, the ball), NN <= 3 active rows n, Bluestein lengths 256 ... 1024 (R1 = 1, 2,
 // 4): a round holds the NN rows of RB = NB / NN rings, so the gamma DFT of a ring (Eq. 48) is done in registers
@@ -948,7 +1074,14 @@ int launch_reweight16(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const
     case 2048: return reweight16_t<8>(F, Ft, A, batch, R, st);
     case 1024: return reweight16_t<4>(F, Ft, A, batch, R, st);
     case 512: return reweight16_t<2>(F, Ft, A, batch, R, st);
-    case 256: return reweight16_t<1>(F, Ft, A, batch, R, st);
+    case 256: {
+        const int ncol = A.Md * A.nn * batch;
+        const size_t sm = (size_t)F16_BUF * sizeof(cplx);
+        int rc = set_smem(reweight16s_kernel, sm);
+        if (rc) return rc;
+        S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight16s_kernel, (ncol + 7) / 8, 256, sm, st, F, Ft, A, R, ncol);
+        return S2W_OK;
+    }
     }
     set_error("launch_reweight16: unsupported length");
     return S2W_EINVAL;
