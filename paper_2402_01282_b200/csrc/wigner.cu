@@ -1136,10 +1136,11 @@ int dispatch_inv_pre(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t
         const char *e = getenv("S2W_PRE_TMA");
         return !(e && e[0] == '0');
     }();
-    if (tma) {
+    // small grids (one ring group per warp: L_j <= 256) keep the __ldg kernel: their 256-byte copies cost more than
+    // they hide (ball, L = P = 128, precompute: 3.15 ms with TMA against 1.99 ms)
+    if (tma && c.R >= 2) {
 #define S2W_WIG_CASE(RR, MT) \
     if (c.R == RR && c.MAXT == MT) return launch_inv_pre_tma<RR, MT>(A, 32 * c.W, chunks, st);
-        S2W_WIG_CASE(1, 256)
         S2W_WIG_CASE(2, 256)
         S2W_WIG_CASE(3, 256)
         S2W_WIG_CASE(4, 256)
