@@ -70,6 +70,35 @@ def mw_phis(L, prec="f80"):
 
 
 # --------------------------------------------------------------------------
+# Driscoll-Healy sampling ("sampling agnostic").  Reading R19: the paper names the sampling
+# schemes of S2FFT without formulas; the equiangular Driscoll & Healy (1994) grid with 2L rings is taken,
+#   theta_t = pi (2t+1)/(4L), t = 0..2L-1,   phi_p = 2 pi p/(2L-1), p = 0..2L-2,
+# with the quadrature weights of their Theorem 3 on it,
+#   q_t = (2/L) sin(theta_t) sum_{k<L} sin((2k+1) theta_t)/(2k+1):   sum_t q_t g(theta_t) = int_0^pi g sin(theta) dtheta
+# for every g that is a cosine polynomial of degree < 2L (so the product of two band-limited functions is integrated
+# exactly and no reweighting operator is needed).
+# --------------------------------------------------------------------------
+def dh_thetas(L, prec="f80"):
+    rt = REAL[prec]
+    return pi(prec) * (2 * np.arange(2 * L).astype(rt) + 1) / rt(4 * L)
+
+
+def dh_weights(L, prec="f80"):
+    rt = REAL[prec]
+    th = dh_thetas(L, prec)
+    k = np.arange(L).astype(rt)
+    return (rt(2) / rt(L)) * np.sin(th) * (np.sin((2 * k[None, :] + 1) * th[:, None]) / (2 * k[None, :] + 1)).sum(axis=1)
+
+
+def thetas_of(L, sampling, prec="f80"):
+    if sampling == "mw":
+        return mw_thetas(L, prec)
+    if sampling == "dh":
+        return dh_thetas(L, prec)
+    raise ValueError("sampling must be 'mw' or 'dh'")
+
+
+# --------------------------------------------------------------------------
 # O1 filters (Appendix A)
 # --------------------------------------------------------------------------
 def _gauss_legendre(n, prec):
@@ -307,27 +336,33 @@ def mw_reweight(F, L, sigma, prec):
 #   sY_{lm}(theta, phi) = (-1)^s sqrt((2l+1)/4pi) D^{l*}_{m,-s}(phi, theta, 0)
 #                       = (-1)^s sqrt((2l+1)/4pi) d^l_{m,-s}(theta) e^{i m phi},      zero for l < |s|.
 # --------------------------------------------------------------------------
-def sht_inverse(flm, L, prec="f80", thetas=None, spin=0):
+def sht_inverse(flm, L, prec="f80", thetas=None, spin=0, sampling="mw"):
     """f(theta_t, phi_p) = sum_{l m} f_{lm} sY_{lm}; spin 0: Y_{lm} = sqrt((2l+1)/4pi) d^l_{m0}(theta) e^{i m phi}
     (Eq. 3; R2).  `thetas` overrides the MW rings (used to evaluate single rings)."""
     rt, ct = REAL[prec], CPLX[prec]
     flm = _as(flm, ct)
     ell = np.arange(L).astype(rt)
     c_l = np.sqrt((2 * ell + 1) / (4 * pi(prec))) * (-1 if spin % 2 else 1)
-    th = mw_thetas(L, prec) if thetas is None else _as(thetas, rt)
+    th = thetas_of(L, sampling, prec) if thetas is None else _as(thetas, rt)
     Fm = dl_inverse(c_l[:, None] * flm, L, -spin, th, prec)      # [mi][t]
     Fm = _centered_to_fft_order(Fm.T, L)                          # [t][m mod n]
     return dft_last_axis(Fm, +1, prec)                            # sum_m F_m e^{+i m phi_p}
 
 
-def sht_forward(f, L, prec="f80", spin=0):
+def sht_forward(f, L, prec="f80", spin=0, sampling="mw"):
     """f_{lm} = int f sY*_{lm} dOmega, exact on the MW grid for band-limit L (O3, R3); the integrand's theta
-    dependence has parity (-1)^{m+s} under the extension of R3 (ii)."""
+    dependence has parity (-1)^{m+s} under the extension of R3 (ii).  sampling="dh": the same integral by the
+    Driscoll-Healy quadrature on 2L rings, f_{lm} = 2 pi c_l sum_t q_t d^l_{m,-s}(theta_t) F_m(theta_t)."""
     rt, ct = REAL[prec], CPLX[prec]
     f = _as(f, ct)
     n = 2 * L - 1
     Fm = dft_last_axis(f, -1, prec) / rt(n)                       # (i)  [t][m mod n]
     Fm = _fft_order_to_centered(Fm, L).T                          # [mi][t]
+    if sampling == "dh":
+        W = dl_forward(Fm * dh_weights(L, prec)[None, :], L, -spin, dh_thetas(L, prec), prec)
+        ell = np.arange(L).astype(rt)
+        c_l = np.sqrt((2 * ell + 1) / (4 * pi(prec))) * (-1 if spin % 2 else 1)
+        return 2 * pi(prec) * c_l[:, None] * W
     m = np.arange(-(L - 1), L)
     H = mw_reweight(Fm, L, np.where((m + spin) % 2 == 0, 1, -1), prec)   # (ii)-(vi), parity (-1)^{m+s}
     W = dl_forward(H, L, -spin, mw_thetas(L, prec), prec)         # (vii)
@@ -350,13 +385,13 @@ def _gamma_phases(N, sign, prec):
     return (np.cos(ang) + sign * 1j * np.sin(ang)).astype(ct)
 
 
-def wigner_inverse(X, L, N, prec="f80", n_list=None, thetas=None):
+def wigner_inverse(X, L, N, prec="f80", n_list=None, thetas=None, sampling="mw"):
     """W(gamma_g, beta_t, alpha_a) = sum_{l m n} X[n][l][m] d^l_{mn}(beta_t) e^{i(m alpha_a + n gamma_g)}
     i.e. Eq. 5 with f^l_{mn} (2l+1)/(8 pi^2) = X and D^{l*}_{mn} from Eq. 47.
     n outside n_list is treated as identically zero."""
     rt, ct = REAL[prec], CPLX[prec]
     X = _as(X, ct)
-    th = mw_thetas(L, prec) if thetas is None else _as(thetas, rt)
+    th = thetas_of(L, sampling, prec) if thetas is None else _as(thetas, rt)
     ns = range(-(N - 1), N) if n_list is None else n_list
     Fmn = np.zeros((2 * N - 1, th.size, 2 * L - 1), dtype=ct)     # [ni][t][mi]
     for n in ns:
@@ -367,7 +402,7 @@ def wigner_inverse(X, L, N, prec="f80", n_list=None, thetas=None):
     return dft_last_axis(A, +1, prec)                             # sum over m
 
 
-def wigner_forward(W, L, N, prec="f80", n_list=None):
+def wigner_forward(W, L, N, prec="f80", n_list=None, sampling="mw"):
     """f^l_{mn} = int_{SO(3)} W D^l_{mn} dOmega(rho) (Eq. 4; R6) on the MW x gamma grid:
     2-D DFT over (alpha, gamma) (Eq. 48), MW reweighting in beta, projection on d^l_{mn}."""
     rt, ct = REAL[prec], CPLX[prec]
@@ -382,6 +417,10 @@ def wigner_forward(W, L, N, prec="f80", n_list=None):
     m = np.arange(-(L - 1), L)
     p = pi(prec)
     for n in ns:
+        if sampling == "dh":                                      # Driscoll-Healy quadrature in beta, no reweighting
+            H = Fmn[n + N - 1].T * dh_weights(L, prec)[None, :]
+            out[n + N - 1] = (2 * p) ** 2 * dl_forward(H, L, n, dh_thetas(L, prec), prec)
+            continue
         sigma = np.where((m + n) % 2 == 0, 1, -1)
         H = mw_reweight(Fmn[n + N - 1].T, L, sigma, prec)         # [mi][t]
         out[n + N - 1] = ((2 * p) ** 2 / rt(n_a)) * dl_forward(H, L, n, mw_thetas(L, prec), prec)
@@ -408,7 +447,8 @@ def _pad_lm(a, Lc, L):
     return out
 
 
-def analysis_from_flm(flm, L, N, lam, J0, multires, prec="f80", filt=None, scales=None, rings=None, spin=0):
+def analysis_from_flm(flm, L, N, lam, J0, multires, prec="f80", filt=None, scales=None, rings=None, spin=0,
+                      sampling="mw"):
     """Algorithm 1 'Analysis' after its first line:
     returns (W_phi, {j: W_psi_j}).  `scales` restricts j; `rings` = {j: ring indices}
     evaluates only those beta rings of scale j (same sums, fewer outputs)."""
@@ -419,7 +459,7 @@ def analysis_from_flm(flm, L, N, lam, J0, multires, prec="f80", filt=None, scale
     # W^Phi_hat = Phi f_hat : einsum("lm,l->lm") with entries sqrt(4pi/(2l+1)) Phi*_{l0}  (Eq. 29/41, R5)
     wphi_hat = np.einsum("lm,l->lm", flm, np.sqrt(4 * pi(prec) / (2 * ell + 1)) * phi)
     Ls = bandlimit_of_scaling(L, lam, J0, multires)
-    W_phi = sht_inverse(_crop_lm(wphi_hat, L, Ls), Ls, prec, spin=spin)   # Y^-1 (a spin-s field, Eq. 12)
+    W_phi = sht_inverse(_crop_lm(wphi_hat, L, Ls), Ls, prec, spin=spin, sampling=sampling)   # Y^-1 (Eq. 12)
     W_psi = {}
     for j in (range(J0, J + 1) if scales is None else scales):
         Lj = bandlimit_of_scale(j, L, lam, multires)
@@ -428,34 +468,34 @@ def analysis_from_flm(flm, L, N, lam, J0, multires, prec="f80", filt=None, scale
         X = np.einsum("lm,ln->nlm", flm, np.conj(psi[j - J0]))
         th = None
         if rings is not None and j in rings:
-            th = mw_thetas(Lj, prec)[np.asarray(rings[j])]
-        W_psi[j] = wigner_inverse(_crop_lm(X, L, Lj), Lj, N, prec, _active_n(psi[j - J0]), th)  # D^-1
+            th = thetas_of(Lj, sampling, prec)[np.asarray(rings[j])]
+        W_psi[j] = wigner_inverse(_crop_lm(X, L, Lj), Lj, N, prec, _active_n(psi[j - J0]), th, sampling=sampling)  # D^-1
     return W_phi, W_psi
 
 
-def analysis(f, L, N, lam, J0, multires, prec="f80", filt=None, spin=0):
+def analysis(f, L, N, lam, J0, multires, prec="f80", filt=None, spin=0, sampling="mw"):
     """Algorithm 1 'Analysis wavelet transform'; `spin`: the signal's spin number (spin fields: Eq. 1; sY_lm: reading R2)."""
-    flm = sht_forward(f, L, prec, spin=spin)                      # f_hat <- Y f
-    return analysis_from_flm(flm, L, N, lam, J0, multires, prec, filt, spin=spin)
+    flm = sht_forward(f, L, prec, spin=spin, sampling=sampling)   # f_hat <- Y f
+    return analysis_from_flm(flm, L, N, lam, J0, multires, prec, filt, spin=spin, sampling=sampling)
 
 
-def synthesis_to_flm(W_phi, W_psi, L, N, lam, J0, multires, prec="f80", filt=None, spin=0):
+def synthesis_to_flm(W_phi, W_psi, L, N, lam, J0, multires, prec="f80", filt=None, spin=0, sampling="mw"):
     """Algorithm 1 'Synthesis' up to its last line: returns f_hat."""
     rt, ct = REAL[prec], CPLX[prec]
     psi, phi, J = filters(L, N, lam, J0, prec) if filt is None else filt
     ell = np.arange(L).astype(rt)
     Ls = bandlimit_of_scaling(L, lam, J0, multires)
-    wphi_hat = _pad_lm(sht_forward(W_phi, Ls, prec, spin=spin), Ls, L)    # Y W^Phi
+    wphi_hat = _pad_lm(sht_forward(W_phi, Ls, prec, spin=spin, sampling=sampling), Ls, L)    # Y W^Phi
     flm = np.einsum("lm,l->lm", wphi_hat, np.sqrt(4 * pi(prec) / (2 * ell + 1)) * phi)
     for j in range(J0, J + 1):
         Lj = bandlimit_of_scale(j, L, lam, multires)
-        what = wigner_forward(W_psi[j], Lj, N, prec, _active_n(psi[j - J0]))     # D W^{Psi j}
+        what = wigner_forward(W_psi[j], Lj, N, prec, _active_n(psi[j - J0]), sampling=sampling)     # D W^{Psi j}
         # f_hat += Psi^dagger W_hat: einsum("nlm,ln->lm")  (Eq. 42, P:307; no extra normalisation, P:309)
         flm = flm + np.einsum("nlm,ln->lm", _pad_lm(what, Lj, L), psi[j - J0])
     return flm
 
 
-def synthesis(W_phi, W_psi, L, N, lam, J0, multires, prec="f80", filt=None, spin=0):
+def synthesis(W_phi, W_psi, L, N, lam, J0, multires, prec="f80", filt=None, spin=0, sampling="mw"):
     """Algorithm 1 'Synthesis wavelet transform'."""
-    flm = synthesis_to_flm(W_phi, W_psi, L, N, lam, J0, multires, prec, filt, spin=spin)
-    return sht_inverse(flm, L, prec, spin=spin)                   # f <- Y^-1 f_hat
+    flm = synthesis_to_flm(W_phi, W_psi, L, N, lam, J0, multires, prec, filt, spin=spin, sampling=sampling)
+    return sht_inverse(flm, L, prec, spin=spin, sampling=sampling)   # f <- Y^-1 f_hat
