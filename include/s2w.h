@@ -39,7 +39,7 @@ extern "C" {
 typedef struct s2w_plan s2w_plan;
 
 enum { S2W_OK = 0, S2W_EINVAL = -1, S2W_ENOMEM = -2, S2W_ECUDA = -3, S2W_EUNSUPPORTED = -4 };
-enum { S2W_REAL = 1, S2W_PRECOMPUTE = 2 };
+enum { S2W_REAL = 1, S2W_PRECOMPUTE = 2, S2W_DH = 4 };
 
 /* ---- kernel-build calls (host only; Appendix A; "calculated and cached") ---- */
 
@@ -65,7 +65,13 @@ int s2ball_radial_nodes(double *r, double *q, int P, double tau);
 
 /* ---- plans: the cached precomputed components ---- */
 
-/* flags: S2W_REAL (signal and coefficients real); S2W_PRECOMPUTE: the Wigner-d values of every theta grid of the plan
+/* Sampling: by default every function on the sphere is sampled on the McEwen-Wiaux grid of its band-limit Lg: theta_t =
+ * pi (2t+1)/(2Lg-1), t < Lg, phi_p = 2 pi p/(2Lg-1).  With S2W_DH ("sampling agnostic"; reading R19) sphere
+ * plans use the Driscoll-Healy grid instead: 2Lg rings theta_t = pi (2t+1)/(4Lg), the same 2Lg-1 samples in phi / alpha;
+ * signals are then [batch][2L][2L-1], coefficient blocks [2N-1][2L_j][2L_j-1] (s2w_plan_scale_shape reports n_theta =
+ * 2L_j), and the theta quadrature is the diagonal Driscoll-Healy rule instead of the reweighting operator.  Scalar
+ * (spin-0) sphere plans up to L = 1024; ball plans, spin plans and the adjoint calls return S2W_EUNSUPPORTED with it.
+ * flags: S2W_REAL (signal and coefficients real); S2W_PRECOMPUTE: the Wigner-d values of every theta grid of the plan
  * are tabulated in device memory at creation ("simply precomputed"; 8 B per (ring, m >= 0, l, n): 21.5 GB at
  * L = 1024, N = 5) and the contractions stream that table through the FP64 tensor pipe instead of running the
  * recursion; S2W_ENOMEM if the table does not fit.

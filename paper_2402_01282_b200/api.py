@@ -13,6 +13,7 @@ from . import build as _build
 
 S2W_REAL = 1
 S2W_PRECOMPUTE = 2
+S2W_DH = 4
 _ERRORS = {-1: "S2W_EINVAL", -2: "S2W_ENOMEM", -3: "S2W_ECUDA", -4: "S2W_EUNSUPPORTED"}
 
 _c_int, _c_dbl, _c_vp, _c_sz = ctypes.c_int, ctypes.c_double, ctypes.c_void_p, ctypes.c_size_t

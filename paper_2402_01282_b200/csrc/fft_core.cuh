@@ -21,6 +21,8 @@ __host__ __device__ inline bool f16_supported(int M) { return M == 4096 || M == 
 struct FftTab {
     int n;              // DFT length (2L-1)
     int L;              // band-limit of the grid
+    int nt;             // rings of the grid: L (McEwen-Wiaux) or 2L (Driscoll-Healy); the radix-16 and ring-pair kernels
+                        // assume nt == L (the launchers route Driscoll-Healy grids to the generic radix-8 kernels)
     int logM, M;        // Bluestein length
     int twmul;          // twiddle table stride: W_M^k = tw[k * twmul]
     int twmask;         // table length - 1

@@ -42,7 +42,8 @@ struct RwArgs {
 // (equator first); group 2j holds north rings 32j..32j+31 of that order, group 2j+1 the south ones.  All rings of a
 // group start the recursion at the same degree gstart (monotone non-decreasing in j), with seeds stored at that degree.
 struct WigArgs {
-    int Lg;        // band-limit of the theta grid (rings t = 0..Lg-1, |m| < Lg, l < Lg)
+    int Lg;        // band-limit of the theta grid (|m| < Lg, l < Lg)
+    int nt;        // rings of the grid, t = 0..nt-1: Lg (McEwen-Wiaux) or 2 Lg (Driscoll-Healy)
     int Lfull;     // band-limit of the plan (l-stride of flmT, extent of the coefficient table)
     int B;         // signals
     int isReal;    // harmonic arrays hold m >= 0 only
@@ -87,7 +88,9 @@ int launch_so3_fwd(bool real, const void *W, size_t sig_stride, cplx *F, const S
 // a2: reads F[b][row][t][mi], writes the reweighted columns TRANSPOSED, Ft[b][row][mi][t] (what the forward Wigner
 // contraction reads: ring data of one m contiguous)
 int launch_reweight(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const FftTab &T, cudaStream_t st);
-int launch_transpose(const cplx *src, cplx *dst, int R, int C, int nb, cudaStream_t st);
+// dst[b][c][r] = w[r] src[b][r][c] (w = null: 1): layout change between F[n][t][m] and Ft[n][m][t]; with the Driscoll-Healy
+// quadrature weights w[t] it is step a2 on a Driscoll-Healy grid
+int launch_transpose(const cplx *src, cplx *dst, int R, int C, int nb, cudaStream_t st, const double *w = 0);
 int launch_reweight_th(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st);   // L >= 8, L <= 2048
 int launch_fft_forward(cplx *data, const FftTab &T, cudaStream_t st);   // plan-time, in place, digit-reversed out
 // the radix-16 core (fft16_kernels.cu), lengths 1024 / 2048 / 4096
@@ -103,7 +106,7 @@ int launch_so3_c16(bool fwd, const void *in, void *out, size_t sig_stride, const
                    cudaStream_t st);
 
 // plan-time: group start degrees and seeds from the range-extended values d^{l0}_{mn}(beta_t) = mant 2^expo ([ntab][Lg m][Lg t])
-int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int G,
+int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int nt, int G,
                         const int *n_vals, int ntab, const double *yv, const int *ring, int *gstart, double2 *dseed,
                         cudaStream_t st);
 int launch_wigner_seed_floor(const double *coef, size_t tri, int Lfull, int Lg, int G, int ntab, const double *yv,

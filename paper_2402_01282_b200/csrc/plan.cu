@@ -112,6 +112,9 @@ struct GridTab {  // everything that depends on the theta/phi grid of band-limit
     int Lg;
     FftTab fft;
     RwTab rw;        // Toeplitz/Hankel reweighting tables (rw.L = 0 on tiny grids)
+    int nt;          // rings: Lg (McEwen-Wiaux) or 2 Lg (Driscoll-Healy)
+    double *dhw;     // Driscoll-Healy: [nt] (2 Lg - 1) q_t, the quadrature weights in the normalisation of the contraction
+                     // stages' filters (which carry 1/(2 Lg - 1)); null on McEwen-Wiaux grids
     int G;           // ring groups of 32 (even): 2j north, 2j+1 south, each hemisphere sorted by |cos beta|
     double *yv;      // [32 G] 1 - |cos beta_t| of the ring in each slot
     int *ring;       // [32 G] ring index t, -1 for an empty slot
@@ -190,6 +193,7 @@ struct s2w_plan {
     // mirror columns land in the row of -n, and a stage listing all rows for the (alpha, gamma) FFT and the reweighting
     std::vector<Stage> qst;
     Stage qall;
+    int dh;                       // S2W_DH: Driscoll-Healy sampling (2 L_j rings per grid), sphere plans only
     int PS;                       // stacked shells
     std::vector<Scale> ang;       // the angular stage of each j (Pj = PS)
     std::vector<size_t *> ang_off;  // device [PS]: element offset of stacked shell b's block of scale j in a coefficient array
@@ -245,20 +249,21 @@ int ceil_log2(int v)
 // Range-extended seeds d^{l0}_{mn}(beta_t), l0 = max(m,|n|), m >= 0, as mantissa * 2^expo (long double arithmetic):
 //   d^m_{mn} = sqrt((2m)!/((m+n)!(m-n)!)) cos^{m+n}(beta/2) (-sin(beta/2))^{m-n}   for m >= |n|,
 // built by the one-term recursion in m, and for m < |n| from d^l_{mn} = (-1)^{m-n} d^l_{nm} = d^l_{-n,-m}.
-void host_seeds(int Lg, const std::vector<int> &tabn, std::vector<double> &mant, std::vector<int> &expo,
+// rings beta_t, t < nt: McEwen-Wiaux pi (2t+1)/(2 Lg - 1), nt = Lg; Driscoll-Healy pi (2t+1)/(4 Lg), nt = 2 Lg
+void host_seeds(int Lg, int nt, bool dh, const std::vector<int> &tabn, std::vector<double> &mant, std::vector<int> &expo,
                 std::vector<double> &yv, std::vector<int> &ring, int &G)
 {
-    const size_t per = (size_t)Lg * Lg;
+    const size_t per = (size_t)Lg * nt;
     mant.assign(tabn.size() * per, 0.0);
     expo.assign(tabn.size() * per, 0);
-    std::vector<ld> ch(Lg), sh(Lg);
+    std::vector<ld> ch(nt), sh(nt);
     // ring groups: each hemisphere sorted by |cos beta| ascending, y = 1 - |cos beta| = 2 sin^2(beta/2) or 2 cos^2(beta/2)
     std::vector<std::pair<ld, int> > hemi[2];
-    for (int t = 0; t < Lg; ++t) {
-        ld beta = PI_L * (ld)(2 * t + 1) / (ld)(2 * Lg - 1);
+    for (int t = 0; t < nt; ++t) {
+        ld beta = dh ? PI_L * (ld)(2 * t + 1) / (ld)(4 * Lg) : PI_L * (ld)(2 * t + 1) / (ld)(2 * Lg - 1);
         ch[t] = cosl(beta / 2);
         sh[t] = sinl(beta / 2);
-        const bool south = 4 * t + 2 > 2 * Lg - 1;  // beta > pi/2
+        const bool south = dh ? t >= Lg : 4 * t + 2 > 2 * Lg - 1;  // beta > pi/2
         const ld y = south ? 2 * ch[t] * ch[t] : 2 * sh[t] * sh[t];
         hemi[south ? 1 : 0].push_back(std::make_pair(-y, t));  // |cos| ascending = y descending
     }
@@ -294,7 +299,7 @@ void host_seeds(int Lg, const std::vector<int> &tabn, std::vector<double> &mant,
         if (an >= Lg) continue;
         for (int m = an; m + 1 < Lg; ++m)
             ratio[m] = sqrtl((ld)(2 * m + 2) * (ld)(2 * m + 1) / ((ld)(m + 1 + n) * (ld)(m + 1 - n)));
-        for (int t = 0; t < Lg; ++t) {
+        for (int t = 0; t < nt; ++t) {
             // m < |n|
             for (int m = 0; m < an; ++m) {
                 ld v;
@@ -302,7 +307,7 @@ void host_seeds(int Lg, const std::vector<int> &tabn, std::vector<double> &mant,
                     v = (((an - m) & 1) ? -1 : 1) * S_direct(an, m, t);
                 else
                     v = S_direct(an, -m, t);
-                put((tab * Lg + m) * (size_t)Lg + t, v);
+                put((tab * Lg + m) * (size_t)nt + t, v);
             }
             // m >= |n|
             ld s = 1;
@@ -312,7 +317,7 @@ void host_seeds(int Lg, const std::vector<int> &tabn, std::vector<double> &mant,
                 for (int i = 0; i < 2 * an; ++i) s *= sh[t];
             const ld cs = -ch[t] * sh[t];
             for (int m = an; m < Lg; ++m) {
-                put((tab * Lg + m) * (size_t)Lg + t, s);
+                put((tab * Lg + m) * (size_t)nt + t, s);
                 if (m + 1 < Lg) s *= ratio[m] * cs;
             }
         }
@@ -597,11 +602,25 @@ int build_grid(s2w_plan *p, int Lg)
         T.bhat16_m = bm16;
         T.bhat16_p = bp16;
     }
-    if ((rc = build_rw(p, g))) return rc;
+    g.nt = p->dh ? 2 * Lg : Lg;
+    T.nt = g.nt;
+    if (p->dh) {
+        // Driscoll-Healy quadrature (their Theorem 3): q_t = (2/L) sin(theta_t) sum_{k<L} sin((2k+1) theta_t)/(2k+1)
+        memset(&g.rw, 0, sizeof(g.rw));
+        std::vector<double> w(g.nt);
+        for (int t = 0; t < g.nt; ++t) {
+            const ld th = PI_L * (ld)(2 * t + 1) / (ld)(4 * Lg);
+            ld acc = 0;
+            for (int k = 0; k < Lg; ++k) acc += sinl((ld)(2 * k + 1) * th) / (ld)(2 * k + 1);
+            w[t] = (double)((ld)(2 * Lg - 1) * 2 / (ld)Lg * sinl(th) * acc);
+        }
+        if ((rc = p->pool.upload(&g.dhw, w))) return rc;
+    } else if ((rc = build_rw(p, g)))
+        return rc;
 
     std::vector<double> mant, yv;
     std::vector<int> expo, ring;
-    host_seeds(Lg, p->tabn, mant, expo, yv, ring, g.G);
+    host_seeds(Lg, g.nt, p->dh != 0, p->tabn, mant, expo, yv, ring, g.G);
     double *dmant;
     int *dexpo;
     if ((rc = p->pool.upload(&g.yv, yv))) return rc;
@@ -615,7 +634,7 @@ int build_grid(s2w_plan *p, int Lg)
     S2W_CUDA_CHECK(cudaMemcpy(dexpo, expo.data(), cnt * sizeof(int), cudaMemcpyHostToDevice));
     if ((rc = p->pool.alloc(&g.gstart, ntab * Lg * g.G))) return rc;
     if ((rc = p->pool.alloc(&g.dseed, ntab * Lg * (size_t)32 * g.G))) return rc;
-    rc = launch_wigner_seeds(dmant, dexpo, p->coef, p->tri, p->L, Lg, g.G, p->tabn.data(), (int)ntab, g.yv, g.ring,
+    rc = launch_wigner_seeds(dmant, dexpo, p->coef, p->tri, p->L, Lg, g.nt, g.G, p->tabn.data(), (int)ntab, g.yv, g.ring,
                              g.gstart, g.dseed, 0);
     cudaError_t e = cudaDeviceSynchronize();
     cudaFree(dmant);
@@ -669,6 +688,7 @@ void fill_wig_args(const s2w_plan *p, const Stage &st, bool synthesis, int B, cp
 {
     const GridTab &g = p->grids[st.grid];
     A.Lg = st.Lg;
+    A.nt = g.nt;
     A.Lfull = p->L;
     A.B = B;
     A.isReal = p->real ? 1 : 0;
@@ -943,6 +963,21 @@ static int lanes_join(const s2w_plan *p, const Lanes &ln)
 
 static double scale_cost(const Scale &sc) { return (double)sc.Lj * sc.Lj * sc.Lj * (sc.st.nn + 0.01); }
 
+// Step a2 on the grid of a stage: F[b][row][t][mi] -> Ft[b][row][mi][t] with the theta quadrature applied.  McEwen-Wiaux:
+// the reweighting operator of reading R3 (Toeplitz/Hankel form, or the Bluestein kernel on tiny grids); Driscoll-Healy:
+// the diagonal quadrature weights q_t, applied by the transposing copy.
+static int stage_reweight(const s2w_plan *p, const Stage &st, const cplx *F, cplx *Ft, int B, cudaStream_t s)
+{
+    const GridTab &g = p->grids[st.grid];
+    if (g.dhw) return launch_transpose(F, Ft, g.nt, p->real ? st.Lg : 2 * st.Lg - 1, B * st.nrows, s, g.dhw);
+    RwArgs R;
+    fill_rw_args(p, st, R);
+    return g.rw.L ? launch_reweight_th(F, Ft, R, B, g.rw, s) : launch_reweight(F, Ft, R, B, g.fft, s);
+}
+
+// pixels of one signal on the grid of band-limit Lg: rings x (2 Lg - 1)
+static size_t grid_pixels(const s2w_plan *p, int Lg) { return (size_t)(p->dh ? 2 * Lg : Lg) * (2 * Lg - 1); }
+
 // Ring FFTs of an SHT stage (a1).  A spin stage has two rows per signal in F (the second one scratch, kept at zero on
 // the way to the forward contraction), so its signals are transformed one by one into / out of row 0.
 static int stage_ring_fwd(const s2w_plan *p, const Stage &st, const void *f, size_t sig_stride, int B, cplx *F,
@@ -950,7 +985,7 @@ static int stage_ring_fwd(const s2w_plan *p, const Stage &st, const void *f, siz
 {
     const FftTab &T = p->grids[st.grid].fft;
     if (st.nrows == 1) return launch_ring_fwd(p->real, f, F, B, st.Lg, sig_stride, T, s);
-    const size_t per = (size_t)st.nrows * st.Lg * (2 * st.Lg - 1);
+    const size_t per = (size_t)st.nrows * grid_pixels(p, st.Lg);
     S2W_CUDA_CHECK(cudaMemsetAsync(F, 0, (size_t)B * per * sizeof(cplx), s));
     for (int b = 0; b < B; ++b) {
         int rc = launch_ring_fwd(false, (const cplx *)f + (size_t)b * sig_stride, F + (size_t)b * per, 1, st.Lg, sig_stride, T, s);
@@ -964,7 +999,7 @@ static int stage_ring_inv(const s2w_plan *p, const Stage &st, const cplx *F, voi
 {
     const FftTab &T = p->grids[st.grid].fft;
     if (st.nrows == 1) return launch_ring_inv(p->real, F, f, B, st.Lg, sig_stride, T, s);
-    const size_t per = (size_t)st.nrows * st.Lg * (2 * st.Lg - 1);
+    const size_t per = (size_t)st.nrows * grid_pixels(p, st.Lg);
     for (int b = 0; b < B; ++b) {
         int rc = launch_ring_inv(false, F + (size_t)b * per, (cplx *)f + (size_t)b * sig_stride, 1, st.Lg, sig_stride, T, s);
         if (rc) return rc;
@@ -984,9 +1019,7 @@ static int sht_forward_dev(const s2w_plan *p, const Stage &st, const void *f, si
         return S2W_OK;
     }
     if ((rc = stage_ring_fwd(p, st, f, sig_stride, B, w.F, s))) return rc;
-    RwArgs R;
-    fill_rw_args(p, st, R);
-    if ((rc = g.rw.L ? launch_reweight_th(w.F, w.Ft, R, B, g.rw, s) : launch_reweight(w.F, w.Ft, R, B, g.fft, s))) return rc;
+    if ((rc = stage_reweight(p, st, w.F, w.Ft, B, s))) return rc;
     if (zero_first) {
         const size_t Mfull = p->real ? p->L : 2 * p->L - 1;
         S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * Mfull * p->L * sizeof(cplx), s));
@@ -1005,7 +1038,7 @@ static int sht_inverse_dev(const s2w_plan *p, const Stage &st, void *f, size_t s
         const size_t esz = p->real ? sizeof(double) : sizeof(cplx);
         for (int b = 0; b < B; ++b)
             S2W_CUDA_CHECK(cudaMemsetAsync((char *)f + (size_t)b * sig_stride * esz, 0,
-                                           (size_t)st.Lg * (2 * st.Lg - 1) * esz, s));
+                                           grid_pixels(p, st.Lg) * esz, s));
         return S2W_OK;
     }
     WigArgs A;
@@ -1024,7 +1057,7 @@ static int scale_analysis(const s2w_plan *p, const Scale &sc, int B, const Work 
     if (sc.st.nn == 0) {
         for (int b = 0; b < B; ++b)
             S2W_CUDA_CHECK(cudaMemsetAsync((char *)dst + (size_t)b * sig_stride * esz, 0,
-                                           (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1) * esz, s));
+                                           (size_t)(2 * p->N - 1) * grid_pixels(p, sc.Lj) * esz, s));
         return S2W_OK;
     }
     int rc;
@@ -1048,9 +1081,7 @@ static int scale_synthesis(const s2w_plan *p, const Scale &sc, int B, const Work
     fill_so3_args(p, sc.st, S);
     S.sig_off = sig_off;
     if ((rc = launch_so3_fwd(p->real, src, sig_stride, w.F, S, B, g.fft, s))) return rc;
-    RwArgs R;
-    fill_rw_args(p, sc.st, R);
-    if ((rc = g.rw.L ? launch_reweight_th(w.F, w.Ft, R, B, g.rw, s) : launch_reweight(w.F, w.Ft, R, B, g.fft, s))) return rc;
+    if ((rc = stage_reweight(p, sc.st, w.F, w.Ft, B, s))) return rc;
     WigArgs A;
     fill_wig_args(p, sc.st, true, B, w.flmT, w.Ft, A);
     return launch_wigner_forward(A, s);
@@ -1141,8 +1172,7 @@ static int scale_pair_synthesis(const s2w_plan *p, const Scale &a, const Scale &
     for (int k = 0; k < 2; ++k) {
         cplx *Ft = k ? w.Ft2 : w.Ft;
         if ((rc = launch_so3_fwd(p->real, k ? src_b : src_a, sig_stride, w.F, S, B, g.fft, s))) return rc;
-        if ((rc = g.rw.L ? launch_reweight_th(w.F, Ft, R, B, g.rw, s) : launch_reweight(w.F, Ft, R, B, g.fft, s)))
-            return rc;
+        if ((rc = stage_reweight(p, a.st, w.F, Ft, B, s))) return rc;
     }
     WigArgs A;
     fill_wig_args(p, a.st, true, B, w.flmT, w.Ft, A);
@@ -1171,8 +1201,8 @@ static int sphere_forward(const s2w_plan *p, const void *in, void *out, void *wo
         if ((rc = scale_pair_analysis(p, a, b, B, w, (char *)out + a.offset * esz, (char *)out + b.offset * esz,
                                       p->coeff_elems, s)))
             return rc;
-        if (hp && (rc = hp->block_out(b.offset * esz, nn * b.Lj * (2 * b.Lj - 1) * esz, s))) return rc;
-        if (hp && (rc = hp->block_out(a.offset * esz, nn * a.Lj * (2 * a.Lj - 1) * esz, s))) return rc;
+        if (hp && (rc = hp->block_out(b.offset * esz, nn * grid_pixels(p, b.Lj) * esz, s))) return rc;
+        if (hp && (rc = hp->block_out(a.offset * esz, nn * grid_pixels(p, a.Lj) * esz, s))) return rc;
         rest = ns - 2;
         ln.load[0] += scale_cost(a) + scale_cost(b);  // the pair ran on lane 0 (the only one with an Ft2 buffer)
     }
@@ -1180,13 +1210,13 @@ static int sphere_forward(const s2w_plan *p, const void *in, void *out, void *wo
         const Scale &sc = p->scales[(hp || lanes) ? rest - 1 - k : k];
         const int l = ln.pick(scale_cost(sc));
         if ((rc = scale_analysis(p, sc, B, ln.w[l], (char *)out + sc.offset * esz, p->coeff_elems, ln.s[l]))) return rc;
-        if (hp && (rc = hp->block_out(sc.offset * esz, nn * sc.Lj * (2 * sc.Lj - 1) * esz, s))) return rc;
+        if (hp && (rc = hp->block_out(sc.offset * esz, nn * grid_pixels(p, sc.Lj) * esz, s))) return rc;
     }
     // scaling coefficients
     const int l = ln.pick(0.0);
     if ((rc = sht_inverse_dev(p, p->scaling, (char *)out + p->scaling_offset * esz, p->coeff_elems, B, ln.w[l], ln.s[l])))
         return rc;
-    if (hp && (rc = hp->block_out(p->scaling_offset * esz, (size_t)p->Ls * (2 * p->Ls - 1) * esz, s))) return rc;
+    if (hp && (rc = hp->block_out(p->scaling_offset * esz, grid_pixels(p, p->Ls) * esz, s))) return rc;
     if ((rc = lanes_join(p, ln))) return rc;
     S2W_CUDA_CHECK(cudaPeekAtLastError());
     return S2W_OK;
@@ -1202,10 +1232,10 @@ static int sphere_inverse(const s2w_plan *p, const void *in, void *out, void *wo
     int rc;
     std::vector<cudaEvent_t> ready(ns + 1);
     if (hp) {
-        if ((rc = hp->block_in(p->scaling_offset * esz, (size_t)p->Ls * (2 * p->Ls - 1) * esz, &ready[ns]))) return rc;
+        if ((rc = hp->block_in(p->scaling_offset * esz, grid_pixels(p, p->Ls) * esz, &ready[ns]))) return rc;
         for (int k = 0; k < ns; ++k) {
             const Scale &sc = p->scales[ns - 1 - k];
-            if ((rc = hp->block_in(sc.offset * esz, nn * sc.Lj * (2 * sc.Lj - 1) * esz, &ready[ns - 1 - k]))) return rc;
+            if ((rc = hp->block_in(sc.offset * esz, nn * grid_pixels(p, sc.Lj) * esz, &ready[ns - 1 - k]))) return rc;
         }
         S2W_CUDA_CHECK(cudaStreamWaitEvent(s, ready[ns], 0));
     }
@@ -1336,7 +1366,7 @@ static int sphere_inverse_adjoint(const s2w_plan *p, const void *in, void *out, 
         if (sc.st.nn == 0) {
             for (int b = 0; b < B; ++b)
                 S2W_CUDA_CHECK(cudaMemsetAsync(y + ((size_t)b * p->coeff_elems + sc.offset) * esz, 0,
-                                               (size_t)(2 * p->N - 1) * sc.Lj * (2 * sc.Lj - 1) * esz, s));
+                                               (size_t)(2 * p->N - 1) * grid_pixels(p, sc.Lj) * esz, s));
             continue;
         }
         const int l = ln.pick(scale_cost(sc));
@@ -1742,9 +1772,14 @@ int s2wav_plan_create_spin(s2w_plan **out, int L, int N, double lambda, int J0, 
         set_error("L > 2048 is not supported");
         return S2W_EUNSUPPORTED;
     }
+    if ((flags & S2W_DH) && (spin != 0 || L > 1024)) {
+        set_error("Driscoll-Healy sampling: scalar signals (spin 0) up to L = 1024 (2L rings = 64 ring groups)");
+        return S2W_EUNSUPPORTED;
+    }
     S2W_CUDA_CHECK(cudaSetDevice(device));
     s2w_plan *p = new s2w_plan();
     p->kind = 0;
+    p->dh = (flags & S2W_DH) ? 1 : 0;
     p->spin = spin;
     p->capture_stream = 0;
     for (int i = 0; i < S2W_LANES - 1; ++i) {
@@ -1807,8 +1842,9 @@ int s2wav_plan_create_spin(s2w_plan **out, int L, int N, double lambda, int J0, 
     }
     size_t off = 0;
     p->scaling_offset = 0;
-    off += (size_t)p->Ls * (2 * p->Ls - 1);
-    size_t maxF = (size_t)(p->spin ? 2 : 1) * L * (p->real ? L : 2 * L - 1);
+    const size_t rf = p->dh ? 2 : 1;  // rings per band-limit: Driscoll-Healy grids have 2 L_j rings
+    off += grid_pixels(p, p->Ls);
+    size_t maxF = (size_t)(p->spin ? 2 : 1) * rf * L * (p->real ? L : 2 * L - 1);
     for (int j = J0; j <= p->J; ++j) {
         Scale sc;
         memset(&sc, 0, sizeof(sc));
@@ -1817,13 +1853,13 @@ int s2wav_plan_create_spin(s2w_plan **out, int L, int N, double lambda, int J0, 
         sc.Pj = 1;
         sc.Lj = scale_bandlimit(j, L, lambda, p->multires);
         sc.offset = off;
-        off += (size_t)nn * sc.Lj * (2 * sc.Lj - 1);
+        off += (size_t)nn * grid_pixels(p, sc.Lj);
         S2W_PLAN_TRY(make_scale_stage(p, sc, &kappa[(size_t)(j - J0) * L], zeta));
-        maxF = std::max(maxF, (size_t)N * sc.Lj * (p->real ? sc.Lj : 2 * sc.Lj - 1));
+        maxF = std::max(maxF, (size_t)N * rf * sc.Lj * (p->real ? sc.Lj : 2 * sc.Lj - 1));
         p->scales.push_back(sc);
     }
     p->coeff_elems = off;
-    p->signal_elems = (size_t)L * (2 * L - 1);
+    p->signal_elems = grid_pixels(p, L);
     p->ws_flm_elems = (size_t)batch * (p->real ? L : 2 * L - 1) * L;
     p->ws_F_elems = (size_t)batch * maxF;
     p->ws_bytes = (((p->ws_flm_elems + 15) / 16) * 16 + (3 + 2 * (S2W_LANES - 1)) * (((p->ws_F_elems + 15) / 16) * 16)) * sizeof(cplx) + 256;
@@ -1841,6 +1877,10 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
     }
     *out = 0;
     int rc = check_params(L, N, lambda_l, J0);
+    if (!rc && (flags & S2W_DH)) {
+        set_error("Driscoll-Healy sampling is available for sphere plans only");
+        return S2W_EUNSUPPORTED;
+    }
     if (rc) return rc;
     if (P < 1 || !(lambda_p > 1.0) || !(tau > 0.0) || J0 > scale_count(P, lambda_p)) {
         set_error("invalid argument: need P >= 1, lambda_p > 1, tau > 0, J0 <= J'");
@@ -1879,6 +1919,7 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
     p->Kfull_fwd = p->Kfull_inv = 0;
     p->Kfull_fwdT = p->Kfull_invT = 0;
     p->phi_ball = 0;
+    p->dh = 0;
     S2W_PLAN_TRY(plan_common(p));
 
     const double pi = pi_d();
@@ -2094,7 +2135,7 @@ int s2w_plan_scale_shape(const s2w_plan *p, int j, int jp, int *n_r, int *n_gamm
     size_t off = 0;
     if (j < 0) {
         nr = p->kind == 1 ? p->P : 1;
-        nt = p->Ls;
+        nt = (p->dh ? 2 : 1) * p->Ls;
         np = 2 * p->Ls - 1;
         off = p->scaling_offset;
     } else {
@@ -2107,7 +2148,7 @@ int s2w_plan_scale_shape(const s2w_plan *p, int j, int jp, int *n_r, int *n_gamm
         }
         nr = sc->Pj;
         ngam = 2 * p->N - 1;
-        nt = sc->Lj;
+        nt = (p->dh ? 2 : 1) * sc->Lj;
         np = 2 * sc->Lj - 1;
         off = sc->offset;
     }
@@ -2236,6 +2277,10 @@ static int adjoint_supported(const s2w_plan *p, const void *in, const void *out,
     {
         int rcd = check_device(p);
         if (rcd) return rcd;
+    }
+    if (p->dh) {
+        set_error("the adjoint transforms are not available on Driscoll-Healy plans");
+        return S2W_EUNSUPPORTED;
     }
     return S2W_OK;
 }

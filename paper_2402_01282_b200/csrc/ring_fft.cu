@@ -43,8 +43,8 @@ __global__ void __launch_bounds__(256, 3) ring_fwd_kernel(const void *__restrict
     if (REAL) {
         const int r0 = 2 * blockIdx.x, r1 = r0 + 1;
         const bool has1 = r1 < nrows;
-        const double *x0 = (const double *)in + (size_t)(r0 / L) * sig_stride + (size_t)(r0 % L) * n;
-        const double *x1 = (const double *)in + (size_t)(r1 / L) * sig_stride + (size_t)(r1 % L) * n;
+        const double *x0 = (const double *)in + (size_t)(r0 / T.nt) * sig_stride + (size_t)(r0 % T.nt) * n;
+        const double *x1 = (const double *)in + (size_t)(r1 / T.nt) * sig_stride + (size_t)(r1 % T.nt) * n;
         for (int p = threadIdx.x; p < M; p += blockDim.x) {
             cplx v = cmake(0.0, 0.0);
             if (p < n) v = cmul(cmake(x0[p], has1 ? x1[p] : 0.0), __ldg(&T.chirp[p]));
@@ -62,7 +62,7 @@ __global__ void __launch_bounds__(256, 3) ring_fwd_kernel(const void *__restrict
         }
     } else {
         const int r0 = blockIdx.x;
-        const cplx *x0 = (const cplx *)in + (size_t)(r0 / L) * sig_stride + (size_t)(r0 % L) * n;
+        const cplx *x0 = (const cplx *)in + (size_t)(r0 / T.nt) * sig_stride + (size_t)(r0 % T.nt) * n;
         for (int p = threadIdx.x; p < M; p += blockDim.x) {
             cplx v = cmake(0.0, 0.0);
             if (p < n) v = cmul(x0[p], __ldg(&T.chirp[p]));
@@ -110,8 +110,8 @@ __global__ void __launch_bounds__(256, 3) ring_inv_kernel(const cplx *__restrict
         }
         __syncthreads();
         fft_convolve<true>(buf, T, s_tw, T.bhat_p);
-        double *y0 = (double *)out + (size_t)(r0 / L) * sig_stride + (size_t)(r0 % L) * n;
-        double *y1 = (double *)out + (size_t)(r1 / L) * sig_stride + (size_t)(r1 % L) * n;
+        double *y0 = (double *)out + (size_t)(r0 / T.nt) * sig_stride + (size_t)(r0 % T.nt) * n;
+        double *y1 = (double *)out + (size_t)(r1 / T.nt) * sig_stride + (size_t)(r1 % T.nt) * n;
         for (int p = threadIdx.x; p < n; p += blockDim.x) {
             cplx z = cmulc(buf[S2W_PAD(p)], __ldg(&T.chirp[p]));
             y0[p] = z.x;
@@ -130,7 +130,7 @@ __global__ void __launch_bounds__(256, 3) ring_inv_kernel(const cplx *__restrict
         }
         __syncthreads();
         fft_convolve<true>(buf, T, s_tw, T.bhat_p);
-        cplx *y0 = (cplx *)out + (size_t)(r0 / L) * sig_stride + (size_t)(r0 % L) * n;
+        cplx *y0 = (cplx *)out + (size_t)(r0 / T.nt) * sig_stride + (size_t)(r0 % T.nt) * n;
         for (int p = threadIdx.x; p < n; p += blockDim.x) y0[p] = cmulc(buf[S2W_PAD(p)], __ldg(&T.chirp[p]));
     }
 }
@@ -157,11 +157,11 @@ __device__ __forceinline__ void so3_inv_few(const cplx *__restrict__ F, void *__
     const int rl = MULTI ? threadIdx.x / tpr : 0, tl = MULTI ? threadIdx.x - rl * tpr : threadIdx.x;
     cplx *buf = buf0 + (size_t)rl * bstride;
     const int t = MULTI ? blockIdx.x * rpb + rl : blockIdx.x, b = blockIdx.y;
-    const bool has = MULTI ? t < L : true;
+    const bool has = MULTI ? t < T.nt : true;
     const int Md = REAL ? L : n;
     const int ng = 2 * A.N - 1;
-    const size_t plane = (size_t)L * n;
-    const cplx *Fb = F + (size_t)b * A.nrows * L * Md;
+    const size_t plane = (size_t)T.nt * n;
+    const cplx *Fb = F + (size_t)b * A.nrows * T.nt * Md;
     int nproc = 0;
     for (int q = 0; q < A.nn; ++q) {
         if (REAL && A.n_val[q] < 0) continue;
@@ -176,8 +176,8 @@ __device__ __forceinline__ void so3_inv_few(const cplx *__restrict__ F, void *__
     for (int q = 0; q < A.nn; ++q) {
         const int nv = A.n_val[q];
         if (REAL && nv < 0) continue;
-        const cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * Md;   // row of n
-        const cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * Md;  // row of -n
+        const cplx *Fp = Fb + ((size_t)A.n_row[q] * T.nt + t) * Md;   // row of n
+        const cplx *Fm = Fb + ((size_t)A.n_rowm[q] * T.nt + t) * Md;  // row of -n
         for (int k0 = tl; k0 < M; k0 += 4 * tpr) {  // four elements at a time, loads first
             cplx x[4], c[4];
 #pragma unroll
@@ -275,10 +275,10 @@ __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict_
     const int rl = MULTI ? threadIdx.x / tpr : 0, tl = MULTI ? threadIdx.x - rl * tpr : threadIdx.x;
     cplx *buf = buf0 + (size_t)rl * bstride;
     const int t = MULTI ? blockIdx.x * rpb + rl : blockIdx.x, b = blockIdx.y;
-    const bool has = MULTI ? t < L : true;
+    const bool has = MULTI ? t < T.nt : true;
     const int Md = REAL ? L : n;
     const int ng = 2 * A.N - 1;
-    const cplx *Fb = F + (size_t)b * A.nrows * L * Md;
+    const cplx *Fb = F + (size_t)b * A.nrows * T.nt * Md;
     __shared__ cplx gph[2 * S2W_MAX_N];
     if (ng <= (REAL ? 9 : 5)) {
         so3_inv_few<REAL, MULTI>(F, W, sig_stride, A, T, rpb, buf0, s_tw, gph);
@@ -289,8 +289,8 @@ __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict_
         const int nv = A.n_val[q];
         if (REAL && nv < 0) continue;
         if (threadIdx.x < ng) gph[threadIdx.x] = cis_2pi_frac(nv * (int)threadIdx.x, ng);
-        const cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * Md;   // row of n
-        const cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * Md;  // row of -n
+        const cplx *Fp = Fb + ((size_t)A.n_row[q] * T.nt + t) * Md;   // row of n
+        const cplx *Fm = Fb + ((size_t)A.n_rowm[q] * T.nt + t) * Md;  // row of -n
         for (int k = tl; k < M; k += tpr) {
             cplx v = cmake(0.0, 0.0);
             if (k < n && has) {
@@ -320,12 +320,12 @@ __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict_
                     double old[9];
 #pragma unroll
                     for (int k = 0; k < 9; ++k)
-                        old[k] = (!first && g0 + k < ng) ? Wr[(size_t)(g0 + k) * L * n] : 0.0;
+                        old[k] = (!first && g0 + k < ng) ? Wr[(size_t)(g0 + k) * T.nt * n] : 0.0;
 #pragma unroll
                     for (int k = 0; k < 9; ++k)
                         if (g0 + k < ng) {
                             const cplx ph = gph[g0 + k];
-                            Wr[(size_t)(g0 + k) * L * n] = old[k] + (ph.x * vx - ph.y * vy);
+                            Wr[(size_t)(g0 + k) * T.nt * n] = old[k] + (ph.x * vx - ph.y * vy);
                         }
                 }
             } else {
@@ -334,10 +334,10 @@ __global__ void __launch_bounds__(256, 3) so3_inv_kernel(const cplx *__restrict_
                     cplx old[5];
 #pragma unroll
                     for (int k = 0; k < 5; ++k)
-                        old[k] = (!first && g0 + k < ng) ? Wc[(size_t)(g0 + k) * L * n] : cmake(0.0, 0.0);
+                        old[k] = (!first && g0 + k < ng) ? Wc[(size_t)(g0 + k) * T.nt * n] : cmake(0.0, 0.0);
 #pragma unroll
                     for (int k = 0; k < 5; ++k)
-                        if (g0 + k < ng) Wc[(size_t)(g0 + k) * L * n] = cadd(old[k], cmul(gph[g0 + k], v));
+                        if (g0 + k < ng) Wc[(size_t)(g0 + k) * T.nt * n] = cadd(old[k], cmul(gph[g0 + k], v));
                 }
             }
         }
@@ -369,12 +369,12 @@ __device__ __forceinline__ void so3_fwd_few(const void *__restrict__ W, cplx *__
     const int rl = MULTI ? threadIdx.x / tpr : 0, tl = MULTI ? threadIdx.x - rl * tpr : threadIdx.x;
     cplx *buf = buf0 + (size_t)rl * bstride;
     const int t = MULTI ? blockIdx.x * rpb + rl : blockIdx.x, b = blockIdx.y;
-    const bool has = MULTI ? t < L : true;
+    const bool has = MULTI ? t < T.nt : true;
     const int Md = REAL ? L : n;
     const int ng = 2 * A.N - 1;
-    const size_t plane = (size_t)L * n;
+    const size_t plane = (size_t)T.nt * n;
     const double inv_ng = 1.0 / (double)ng, inv_n = 1.0 / (double)n;
-    cplx *Fb = F + (size_t)b * A.nrows * L * Md;
+    cplx *Fb = F + (size_t)b * A.nrows * T.nt * Md;
     __shared__ int s_nv[NR], s_rowp[NR], s_rowm[NR];
     int nproc = 0;
     for (int pass = 0; pass < 2; ++pass)  // a row n = 0 first
@@ -426,15 +426,15 @@ __device__ __forceinline__ void so3_fwd_few(const void *__restrict__ W, cplx *__
                 if (i == 0)
                     buf[S2W_PAD(a)] = y;
                 else if (REAL)
-                    Fb[((size_t)(a < L ? s_rowp[i] : s_rowm[i]) * L + t) * Md + (a < L ? a : a - L)] = y;
+                    Fb[((size_t)(a < L ? s_rowp[i] : s_rowm[i]) * T.nt + t) * Md + (a < L ? a : a - L)] = y;
                 else
-                    Fb[((size_t)s_rowp[i] * L + t) * Md + a] = y;
+                    Fb[((size_t)s_rowp[i] * T.nt + t) * Md + a] = y;
             }
     }
     __syncthreads();
     for (int i = 0; i < nproc; ++i) {
-        cplx *Fp = Fb + ((size_t)s_rowp[i] * L + t) * Md;
-        cplx *Fm = Fb + ((size_t)s_rowm[i] * L + t) * Md;
+        cplx *Fp = Fb + ((size_t)s_rowp[i] * T.nt + t) * Md;
+        cplx *Fm = Fb + ((size_t)s_rowm[i] * T.nt + t) * Md;
         if (i > 0) {
             for (int a = tl; a < M; a += tpr) {
                 cplx v = cmake(0.0, 0.0);
@@ -481,11 +481,11 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
     const int rl = MULTI ? threadIdx.x / tpr : 0, tl = MULTI ? threadIdx.x - rl * tpr : threadIdx.x;
     cplx *buf = buf0 + (size_t)rl * bstride;
     const int t = MULTI ? blockIdx.x * rpb + rl : blockIdx.x, b = blockIdx.y;
-    const bool has = MULTI ? t < L : true;
+    const bool has = MULTI ? t < T.nt : true;
     const int Md = REAL ? L : n;
     const int ng = 2 * A.N - 1;
     const double inv_ng = 1.0 / (double)ng, inv_n = 1.0 / (double)n;
-    cplx *Fb = F + (size_t)b * A.nrows * L * Md;
+    cplx *Fb = F + (size_t)b * A.nrows * T.nt * Md;
     __shared__ cplx gph[2 * S2W_MAX_N];
     if (ng <= (REAL ? 9 : 5)) {
         so3_fwd_few<REAL, MULTI>(W, F, sig_stride, A, T, rpb, buf0, s_tw, gph);
@@ -504,7 +504,7 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
                     for (int g0 = 0; g0 < ng; g0 += 9) {
                         double wv[9];
 #pragma unroll
-                        for (int k = 0; k < 9; ++k) wv[k] = g0 + k < ng ? Wr[(size_t)(g0 + k) * L * n] : 0.0;
+                        for (int k = 0; k < 9; ++k) wv[k] = g0 + k < ng ? Wr[(size_t)(g0 + k) * T.nt * n] : 0.0;
 #pragma unroll
                         for (int k = 0; k < 9; ++k)
                             if (g0 + k < ng) {
@@ -519,7 +519,7 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
                         cplx wv[5];
 #pragma unroll
                         for (int k = 0; k < 5; ++k)
-                            wv[k] = g0 + k < ng ? Wc[(size_t)(g0 + k) * L * n] : cmake(0.0, 0.0);
+                            wv[k] = g0 + k < ng ? Wc[(size_t)(g0 + k) * T.nt * n] : cmake(0.0, 0.0);
 #pragma unroll
                         for (int k = 0; k < 5; ++k)
                             if (g0 + k < ng) v = cadd(v, cmul(gph[g0 + k], wv[k]));
@@ -534,8 +534,8 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_kernel(const void *__restrict_
             fft_convolve_b<true>(buf0, T, s_tw, T.bhat_m, rpb, bstride);
         else
             fft_convolve<true>(buf, T, s_tw, T.bhat_m);
-        cplx *Fp = Fb + ((size_t)A.n_row[q] * L + t) * Md;
-        cplx *Fm = Fb + ((size_t)A.n_rowm[q] * L + t) * Md;
+        cplx *Fp = Fb + ((size_t)A.n_row[q] * T.nt + t) * Md;
+        cplx *Fm = Fb + ((size_t)A.n_rowm[q] * T.nt + t) * Md;
         if (REAL) {
             for (int m = tl; m < (has ? L : 0); m += tpr) {
                 Fp[m] = cscale(cmul(buf[S2W_PAD(m)], __ldg(&T.chirp[m])), inv_n);
@@ -1491,7 +1491,8 @@ __global__ void __launch_bounds__(256) kernel_spectrum_kernel(cplx *khat, int ki
 // dst[b][c][r] = src[b][r][c] for nb matrices of R x C complex values: the adjoint transforms move
 // between the ring-major layout F[n][t][m] of the FFT kernels and the column-major layout Ft[n][m][t] of the forward
 // contraction without the reweighting kernel that normally does it.  32 x 32 tiles through padded shared memory.
-__global__ void __launch_bounds__(256) transpose_kernel(const cplx *__restrict__ src, cplx *__restrict__ dst, int R, int C)
+__global__ void __launch_bounds__(256) transpose_kernel(const cplx *__restrict__ src, cplx *__restrict__ dst, int R, int C,
+                                                       const double *__restrict__ w)
 {
     __shared__ cplx tile[32][33];
     const size_t base = (size_t)blockIdx.z * R * C;
@@ -1499,7 +1500,7 @@ __global__ void __launch_bounds__(256) transpose_kernel(const cplx *__restrict__
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     for (int k = ty; k < 32; k += 8) {
         const int r = r0 + k, c = c0 + tx;
-        if (r < R && c < C) tile[k][tx] = src[base + (size_t)r * C + c];
+        if (r < R && c < C) tile[k][tx] = w ? cscale(src[base + (size_t)r * C + c], w[r]) : src[base + (size_t)r * C + c];
     }
     __syncthreads();
     for (int k = ty; k < 32; k += 8) {
@@ -1546,9 +1547,11 @@ int launch_fft_tables(const FftTab &T, cplx *chirp, cplx *rw_in1, cplx *rw_out1,
 int launch_ring_fwd(bool real, const void *in, cplx *out, int B, int Lg, size_t sig_stride, const FftTab &T,
                     cudaStream_t st)
 {
-    const int nrows = B * Lg;
+    const int nrows = B * T.nt;
+    (void)Lg;
     if (nrows <= 0) return S2W_OK;
-    if (T.bhat16_m && f16_supported(T.M) && use_fft16()) return launch_ring16(true, real, in, out, nrows, sig_stride, T, st);
+    if (T.nt == T.L && T.bhat16_m && f16_supported(T.M) && use_fft16())
+        return launch_ring16(true, real, in, out, nrows, sig_stride, T, st);
     size_t sm = fft_smem_bytes(T);
     int rc;
     if (real) {
@@ -1564,9 +1567,11 @@ int launch_ring_fwd(bool real, const void *in, cplx *out, int B, int Lg, size_t 
 int launch_ring_inv(bool real, const cplx *in, void *out, int B, int Lg, size_t sig_stride, const FftTab &T,
                     cudaStream_t st)
 {
-    const int nrows = B * Lg;
+    const int nrows = B * T.nt;
+    (void)Lg;
     if (nrows <= 0) return S2W_OK;
-    if (T.bhat16_m && f16_supported(T.M) && use_fft16()) return launch_ring16(false, real, in, out, nrows, sig_stride, T, st);
+    if (T.nt == T.L && T.bhat16_m && f16_supported(T.M) && use_fft16())
+        return launch_ring16(false, real, in, out, nrows, sig_stride, T, st);
     size_t sm = fft_smem_bytes(T);
     int rc;
     if (real) {
@@ -1587,7 +1592,7 @@ static int so3_launch_t(bool fwd, const void *in, void *out, size_t sig_stride, 
                         const FftTab &T, int rpb, cudaStream_t st)
 {
     size_t sm = (size_t)rpb * fft_smem_bytes(T);
-    dim3 grid((T.L + rpb - 1) / rpb, batch);
+    dim3 grid((T.nt + rpb - 1) / rpb, batch);
     int rc;
     if (fwd) {
         if ((rc = set_smem(so3_fwd_kernel<REAL, MULTI>, sm))) return rc;
@@ -1604,11 +1609,13 @@ static int so3_launch_t(bool fwd, const void *in, void *out, size_t sig_stride, 
 static int so3_launch(bool fwd, bool real, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch,
                       const FftTab &T, cudaStream_t st)
 {
-    if (real && 2 * A.N - 1 <= 9 && T.bhat16_m && T.M >= 1024 && f16_supported(T.M) && use_fft16())
+    const bool mw = T.nt == T.L;  // the radix-16 and ring-pair kernels are written for McEwen-Wiaux grids (L rings)
+    if (mw && real && 2 * A.N - 1 <= 9 && T.bhat16_m && T.M >= 1024 && f16_supported(T.M) && use_fft16())
         return launch_so3_pair16(fwd, in, out, sig_stride, A, batch, T, st);
-    if (!real && so3_c16_supported(A, T) && use_fft16()) return launch_so3_c16(fwd, in, out, sig_stride, A, batch, T, st);
-    const int rpb = seqs_per_block(4096 / T.M, (long long)T.L * batch, 32);
-    if (rpb == 1 && real) {  // large grids, real signals: ring pairs (the n = 0 row shares one transform)
+    if (mw && !real && so3_c16_supported(A, T) && use_fft16())
+        return launch_so3_c16(fwd, in, out, sig_stride, A, batch, T, st);
+    const int rpb = seqs_per_block(4096 / T.M, (long long)T.nt * batch, 32);
+    if (mw && rpb == 1 && real) {  // large grids, real signals: ring pairs (the n = 0 row shares one transform)
         const int ng = 2 * A.N - 1;
         size_t sm = ((size_t)fft_padded_len(T.M) + tw_own_entries(T.logM) + (ng <= 9 ? 0 : ng)) * sizeof(cplx);
         dim3 grid((T.L + 1) / 2, batch);
@@ -1661,13 +1668,14 @@ static int seqs_per_block(int fit, long long total, int cap)
     return s;
 }
 
-int launch_transpose(const cplx *src, cplx *dst, int R, int C, int nb, cudaStream_t st)
+int launch_transpose(const cplx *src, cplx *dst, int R, int C, int nb, cudaStream_t st, const double *w)
 {
     if (R <= 0 || C <= 0 || nb <= 0) return S2W_OK;
     for (int b0 = 0; b0 < nb; b0 += 65535) {  // gridDim.z limit
         const int nz = nb - b0 < 65535 ? nb - b0 : 65535;
         dim3 grid((C + 31) / 32, (R + 31) / 32, nz);
-        S2W_LAUNCH(transpose_kernel, grid, 256, 0, st, src + (size_t)b0 * R * C, dst + (size_t)b0 * R * C, R, C);
+        S2W_LAUNCH_C(w ? S2W_K_REWEIGHT : S2W_K_OTHER, transpose_kernel, grid, 256, 0, st, src + (size_t)b0 * R * C,
+                     dst + (size_t)b0 * R * C, R, C, w);
     }
     return S2W_OK;
 }

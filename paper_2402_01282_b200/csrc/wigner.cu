@@ -63,7 +63,7 @@ __device__ __forceinline__ void wig_step(double &d, double &u, double y, double 
 // ---------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(32) wigner_seed_kernel(const double *__restrict__ mant, const int *__restrict__ expo,
                                                         const double *__restrict__ coef, size_t tri, int Lfull, int Lg,
-                                                        int G, NList nl, const double *__restrict__ yv,
+                                                        int nt, int G, NList nl, const double *__restrict__ yv,
                                                         const int *__restrict__ ring, int *__restrict__ gstart,
                                                         double2 *__restrict__ dseed, int pass)
 {
@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(32) wigner_seed_kernel(const double *__restric
     double d = 0.0, u = 0.0;
     int e = 0, l = l0;
     if (t >= 0 && l0 < Lg) {
-        const size_t idx = ((size_t)tab * Lg + m) * Lg + t;
+        const size_t idx = ((size_t)tab * Lg + m) * nt + t;
         d = mant[idx];
         if (south && (l0 & 1)) d = -d;
         u = d;
@@ -356,7 +356,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_inverse_ke
                 if (ci.minus && m == 0) continue;  // (0,-n) is the plus column of another n
                 const int row = ci.minus ? A.n_rowm[q] : A.n_row[q];
                 const int mi = A.isReal ? m : (ci.minus ? Lg - 1 - m : Lg - 1 + m);
-                (sc ? A.F2 : A.F)[(((size_t)ci.b * A.nrows + row) * Lg + tr[r]) * Md + mi] =
+                (sc ? A.F2 : A.F)[(((size_t)ci.b * A.nrows + row) * A.nt + tr[r]) * Md + mi] =
                     cmake(acc[r][2 * k], acc[r][2 * k + 1]);
             }
         }
@@ -475,7 +475,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
             const int row = fci.minus ? A.n_rowm[q] : A.n_row[q];
             const int mi = A.isReal ? m : (fci.minus ? Lg - 1 - m : Lg - 1 + m);
             const double *hcol = reinterpret_cast<const double *>(
-                                     Fsrc + (((size_t)(fci.valid ? fci.b : 0) * A.nrows + row) * Md + mi) * Lg) + (fc & 1);
+                                     Fsrc + (((size_t)(fci.valid ? fci.b : 0) * A.nrows + row) * Md + mi) * A.nt) + (fc & 1);
             const int *ringp = A.ring + (g < G ? g : 0) * 32 + fk;
             int tq[8];
 #pragma unroll
@@ -741,7 +741,7 @@ __global__ void __launch_bounds__(MAXT) precomp_inverse_kernel(WigArgs A)
             for (int o = 0; o < 4; ++o) {
                 const int t = A.ring[g * 32 + o * 8 + fr];
                 if (t < 0) continue;
-                A.F[(((size_t)ci.b * A.nrows + row) * Lg + t) * Md + mi] = cmake(acc[r][o][0], acc[r][o][1]);
+                A.F[(((size_t)ci.b * A.nrows + row) * A.nt + t) * Md + mi] = cmake(acc[r][o][0], acc[r][o][1]);
             }
         }
     }
@@ -950,7 +950,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) precomp_inverse_t
             for (int o = 0; o < 4; ++o) {
                 const int t = A.ring[g * 32 + o * 8 + fr];
                 if (t < 0) continue;
-                A.F[(((size_t)ci.b * A.nrows + row) * Lg + t) * Md + mi] = cmake(acc[r][o][0], acc[r][o][1]);
+                A.F[(((size_t)ci.b * A.nrows + row) * A.nt + t) * Md + mi] = cmake(acc[r][o][0], acc[r][o][1]);
             }
         }
     }
@@ -1186,17 +1186,17 @@ int launch_wigner(bool fwd, const WigArgs &A, cudaStream_t st)
 
 }  // namespace
 
-int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int G,
+int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int nt, int G,
                         const int *n_vals, int ntab, const double *yv, const int *ring, int *gstart, double2 *dseed,
                         cudaStream_t st)
 {
     NList nl;
     for (int i = 0; i < ntab; ++i) nl.v[i] = n_vals[i];
     dim3 grid(G, Lg, ntab);
-    S2W_LAUNCH(wigner_seed_kernel, grid, 32, 0, st, mant, expo, coef, tri, Lfull, Lg, G, nl, yv, ring, gstart, dseed, 0);
+    S2W_LAUNCH(wigner_seed_kernel, grid, 32, 0, st, mant, expo, coef, tri, Lfull, Lg, nt, G, nl, yv, ring, gstart, dseed, 0);
     const int count = Lg * ntab;
     S2W_LAUNCH(wigner_start_fix_kernel, (count + 127) / 128, 128, 0, st, gstart, G, count);
-    S2W_LAUNCH(wigner_seed_kernel, grid, 32, 0, st, mant, expo, coef, tri, Lfull, Lg, G, nl, yv, ring, gstart, dseed, 1);
+    S2W_LAUNCH(wigner_seed_kernel, grid, 32, 0, st, mant, expo, coef, tri, Lfull, Lg, nt, G, nl, yv, ring, gstart, dseed, 1);
     return S2W_OK;
 }
 
