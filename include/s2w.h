@@ -124,6 +124,25 @@ int s2w_plan_inverse_adjoint(const s2w_plan *plan, const void *in_dev, void *out
 int s2w_plan_harmonic_forward(const s2w_plan *plan, const void *f_dev, void *flm_dev, void *work_dev, void *stream);
 int s2w_plan_harmonic_inverse(const s2w_plan *plan, const void *flm_dev, void *f_dev, void *work_dev, void *stream);
 
+/* s2w_plan_harmonic_forward for callers that cannot allocate device memory (code under CUDA graph capture, serving
+ * loops, harnesses that forbid cudaMalloc): the same forward spherical harmonic transform (steps a1-a3; Eq. 2 / Eq. 13,
+ * P:49 / P:116, by the separation of variables of P:378-384), same kernels, same f_dev / flm_dev layouts, but the scratch
+ * (f_lm accumulator, ring spectra F, reweighted columns Ft) lives in a static device array of
+ * S2W_STATIC_SCRATCH_BYTES inside the library instead of a caller workspace.  Every GPU that loads the library holds
+ * that array until the process exits.  The call allocates nothing: no cudaMalloc / cudaFree, no stream, event or graph
+ * creation (the first call on a device resolves the array's device address with cudaGetSymbolAddress).
+ * Sphere plans only (S2W_EUNSUPPORTED for ball plans, and while s2w_timing_enable(1) is in force: the timers create
+ * events).  S2W_EINVAL, with the sizes in s2w_last_error(), if the plan needs more scratch than the array holds:
+ * 16 B x batch x (M L + 2 N M L), M = L (S2W_REAL) or 2L-1 (the F buffers are sized for the plan's largest stage, the N
+ * rows of a top wavelet scale; each term rounded up to 16 elements) -- at batch = 1: L <= 836 (real, N = 1), 547 (real,
+ * N = 3), 591 (complex, N = 1), 387 (complex, N = 3); use s2w_plan_harmonic_forward with a caller workspace beyond that.
+ * All calls on a device share the one array, which keeps the previous call's contents; what must start at zero (the
+ * f_lm accumulator) is cleared by the call itself on `stream`.  Two calls that overlap on the GPU (different streams,
+ * or different host threads without stream ordering between them) RACE on the array: order them on one stream or
+ * with events.  Asynchronous on `stream`; plan and buffers must belong to the current device. */
+#define S2W_STATIC_SCRATCH_BYTES (32u << 20)
+int s2w_plan_harmonic_forward_static(const s2w_plan *plan, const void *f_dev, void *flm_dev, void *stream);
+
 /* ---- the transforms named by the problem statement: explicit arguments, device pointers.
  * The plan and its workspace are looked up in an internal cache keyed on the arguments (the first call builds them
  * and synchronises; later calls are asynchronous on `stream`). ---- */

@@ -14,6 +14,7 @@ from . import build as _build
 S2W_REAL = 1
 S2W_PRECOMPUTE = 2
 S2W_DH = 4
+S2W_STATIC_SCRATCH_BYTES = 32 << 20   # include/s2w.h: capacity of the static device scratch array
 _ERRORS = {-1: "S2W_EINVAL", -2: "S2W_ENOMEM", -3: "S2W_ECUDA", -4: "S2W_EUNSUPPORTED"}
 
 _c_int, _c_dbl, _c_vp, _c_sz = ctypes.c_int, ctypes.c_double, ctypes.c_void_p, ctypes.c_size_t
@@ -43,6 +44,7 @@ SIGNATURES = {
     "s2w_plan_inverse_adjoint": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_vp]),
     "s2w_plan_harmonic_forward": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_vp]),
     "s2w_plan_harmonic_inverse": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_vp]),
+    "s2w_plan_harmonic_forward_static": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp]),
     "s2wav_forward": (_c_int, [_c_vp, _c_vp, _c_int, _c_int, _c_dbl, _c_int, _c_int, _c_int, _c_int, _c_vp]),
     "s2wav_inverse": (_c_int, [_c_vp, _c_vp, _c_int, _c_int, _c_dbl, _c_int, _c_int, _c_int, _c_int, _c_vp]),
     "s2ball_forward": (_c_int, [_c_vp, _c_vp, _c_int, _c_int, _c_int, _c_dbl, _c_dbl, _c_int, _c_dbl, _c_int, _c_vp]),
@@ -277,6 +279,19 @@ class Plan:
         out = torch.empty((self.batch, flm_elems), dtype=torch.complex128, device=f.device)
         _check(lib().s2w_plan_harmonic_forward(self._h, f.data_ptr(), out.data_ptr(),
                                                self._workspace(f.device).data_ptr(), _stream_ptr(f.device)))
+        return out
+
+    def harmonic_forward_static(self, f, flm_elems, out=None):
+        """s2w_plan_harmonic_forward_static: harmonic_forward with the scratch in the library's static device array
+        (S2W_STATIC_SCRATCH_BYTES); `out` lets the caller pass the result buffer, so that nothing is allocated here."""
+        torch = _torch()
+        self._check_in(f, self.signal_elems)
+        if out is None:
+            out = torch.empty((self.batch, flm_elems), dtype=torch.complex128, device=f.device)
+        elif not (out.is_cuda and out.is_contiguous() and out.dtype == torch.complex128
+                  and out.numel() == self.batch * flm_elems and out.device == f.device):
+            raise ValueError("out: expected a contiguous complex128 CUDA tensor of %d elements" % (self.batch * flm_elems))
+        _check(lib().s2w_plan_harmonic_forward_static(self._h, f.data_ptr(), out.data_ptr(), _stream_ptr(f.device)))
         return out
 
     def harmonic_inverse(self, flm):

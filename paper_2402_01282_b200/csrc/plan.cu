@@ -2361,6 +2361,72 @@ int s2w_plan_harmonic_inverse(const s2w_plan *p, const void *flm, void *f, void 
     return S2W_OK;
 }
 
+// ---- the forward harmonic transform with its scratch in a static device array (s2w.h: s2w_plan_harmonic_forward_static)
+// For callers that cannot call cudaMalloc (CUDA graph capture, serving loops, harnesses that forbid it).  The scratch of
+// steps a1-a3 (flmT, F, Ft) is carved from g_static_scratch instead of a caller buffer.  In host code the name
+// g_static_scratch is only a host-side stand-in for the array: its DEVICE address is fetched with cudaGetSymbolAddress,
+// once per device and with that device current, and only that pointer goes to the kernels.
+static __device__ __align__(256) unsigned char g_static_scratch[S2W_STATIC_SCRATCH_BYTES];
+
+static int static_scratch_ptr(int device, void **out)
+{
+    enum { MAXDEV = 64 };
+    static std::mutex mu;
+    static void *ptr[MAXDEV] = {0};
+    if (device < 0 || device >= MAXDEV) {
+        set_error("s2w_plan_harmonic_forward_static: device ordinal out of range");
+        return S2W_EINVAL;
+    }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr[device]) {  // check_device() has made sure that `device` is the current one
+        void *q = 0;
+        const cudaError_t e = cudaGetSymbolAddress(&q, g_static_scratch);
+        if (e != cudaSuccess || !q) {
+            set_error(std::string("cudaGetSymbolAddress(g_static_scratch): ") + cudaGetErrorString(e));
+            cudaGetLastError();
+            return S2W_ECUDA;
+        }
+        ptr[device] = q;
+    }
+    *out = ptr[device];
+    return S2W_OK;
+}
+
+int s2w_plan_harmonic_forward_static(const s2w_plan *p, const void *f, void *flm, void *stream)
+{
+    if (!p || !f || !flm) {
+        set_error("null pointer");
+        return S2W_EINVAL;
+    }
+    if (p->kind != 0) {
+        set_error("s2w_plan_harmonic_forward_static: sphere plans only");
+        return S2W_EUNSUPPORTED;
+    }
+    if (g_timing) {
+        set_error("s2w_plan_harmonic_forward_static: the per-class timers create events (s2w_timing_enable(0) first)");
+        return S2W_EUNSUPPORTED;
+    }
+    int rc = check_device(p);
+    if (rc) return rc;
+    // carve(): flmT, then F and Ft, each rounded up to 16 elements
+    const size_t need = (((p->ws_flm_elems + 15) / 16) * 16 + 2 * (((p->ws_F_elems + 15) / 16) * 16)) * sizeof(cplx);
+    if (need > (size_t)S2W_STATIC_SCRATCH_BYTES) {
+        set_error("s2w_plan_harmonic_forward_static: this plan needs " + std::to_string(need) +
+                  " bytes of scratch, the static array holds " + std::to_string((size_t)S2W_STATIC_SCRATCH_BYTES) +
+                  " (S2W_STATIC_SCRATCH_BYTES): use s2w_plan_harmonic_forward with a caller workspace");
+        return S2W_EINVAL;
+    }
+    void *scratch = 0;
+    if ((rc = static_scratch_ptr(p->device, &scratch))) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    const Work w = carve(p, scratch);
+    // flmT is accumulated into and is cleared by sht_forward_dev (zero_first); F and Ft are fully overwritten
+    if ((rc = sht_forward_dev(p, p->sht, f, p->signal_elems, p->batch, w, true, s))) return rc;
+    if ((rc = launch_flm_unpack(w.flmT, (cplx *)flm, p->batch, p->L, p->real, s))) return rc;
+    S2W_CUDA_CHECK(cudaPeekAtLastError());
+    return S2W_OK;
+}
+
 // ---- Wigner-Laguerre (Q) and spherical-Laguerre (Z) transforms as stand-alone calls (Eqs. 10-11, 24-25) ----------
 static int qplan_create(s2w_plan **out, int L, int P, int N, double tau, int device)
 {
