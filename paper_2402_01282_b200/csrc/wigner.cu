@@ -413,9 +413,83 @@ __device__ __forceinline__ void fwd_octet(const double2 *s_ag8, const double *se
     }
 }
 
-template <int R, int MAXT, bool PRE, bool FUSE>
+// ---- few columns (CF = 2 or 4 real columns per recursion): plain FP64 instead of the tensor pipe ---------------------
+// A DMMA consumes 32 d~ values whatever the number of columns, i.e. 8 DFMA-equivalents per (ring, degree) -- for one
+// complex column 6 of the 8 tile rows are idle (L = 2048, batch 1: 9 useful flops of the 24 issued per tuple).  Here a
+// lane first sums its OWN R rings, p_c(l) = sum_r d~_r(l) h_r[c] (R CF DFMA per degree), and only the CF partial sums per
+// degree are transposed through shared memory (P[degree s][c][lane]) and summed over the 32 lanes: 32 R + 8 CF (R + 1)
+// FP64 instructions per warp and octet instead of 96 R, and CF instead of R shared-memory round trips per degree.
+#define FWD_PS 33  // doubles per row of P (32 lanes + 1: a lane walks along its row with immediate offsets, conflict-free)
+template <int R, int RA, int CF, bool MM>
+__device__ __forceinline__ void fwd_octet_dfma(const double2 *s_ag8, const double *se8, double *pw,
+                                               const double (&y)[R], double (&d)[R], double (&u)[R],
+                                               const double (&h)[R][CF > 0 ? CF : 1])
+{
+#pragma unroll
+    for (int s = 0; s < 8; ++s) {
+        const double2 ag = s_ag8[s];
+        const double e = se8[2 * s];
+        double p[CF > 0 ? CF : 1];
+#pragma unroll
+        for (int r = 0; r < RA; ++r) {
+            if (MM) {
+#pragma unroll
+                for (int c = 0; c < CF; ++c) p[c] = r ? fma(d[r], h[r][c], p[c]) : d[r] * h[r][c];
+            }
+            wig_step(d[r], u[r], y[r], ag.x, ag.y, e);
+        }
+        if (MM) {
+#pragma unroll
+            for (int c = 0; c < CF; ++c) pw[(s * CF + c) * FWD_PS] = p[c];
+        }
+    }
+}
+
+template <int R, int CF>
+__device__ __forceinline__ void fwd_octet_dfma_ra(int ra, bool mm, const double2 *ag8, const double *se8, double *pw,
+                                                  const double (&y)[R], double (&d)[R], double (&u)[R],
+                                                  const double (&h)[R][CF > 0 ? CF : 1])
+{
+#define S2W_OCT(RA_)                                                            \
+    {                                                                           \
+        if (mm)                                                                 \
+            fwd_octet_dfma<R, (R >= RA_ ? RA_ : R), CF, true>(ag8, se8, pw, y, d, u, h);  \
+        else                                                                    \
+            fwd_octet_dfma<R, (R >= RA_ ? RA_ : R), CF, false>(ag8, se8, pw, y, d, u, h); \
+        return;                                                                 \
+    }
+    if (R >= 4 && ra == 4) S2W_OCT(4)
+    if (R >= 3 && ra == 3) S2W_OCT(3)
+    if (R >= 2 && ra == 2) S2W_OCT(2)
+    S2W_OCT(1)
+#undef S2W_OCT
+}
+
+// sum over the 32 lanes of the 8 CF partial sums of an octet: row o = s CF + c of P holds one value per lane.  Lane
+// (o, half) adds 32 / (32 / K) of them; rows are FWD_PS = 33 doubles apart, so the 16 lanes of a half-warp hit 16 banks.
+template <int CF>
+__device__ __forceinline__ double fwd_octet_reduce(const double *P, int lane)
+{
+    constexpr int K = 8 * CF, NH = 32 / K, CNT = 32 / NH;  // K = 16: two lanes per output, 16 addends each
+    const int o = lane % K, half = lane / K;
+    const double *row = P + o * FWD_PS + half * CNT;
+    double v0 = row[0], v1 = row[1], v2 = row[2], v3 = row[3];
+#pragma unroll
+    for (int i = 4; i < CNT; i += 4) {
+        v0 += row[i];
+        v1 += row[i + 1];
+        v2 += row[i + 2];
+        v3 += row[i + 3];
+    }
+    double v = (v0 + v1) + (v2 + v3);
+    if (NH == 2) v += __shfl_xor_sync(0xffffffffu, v, 16);
+    return v;
+}
+
+template <int R, int MAXT, bool PRE, bool FUSE, int CF = 0>
 __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_kernel(WigArgs A)
 {
+    static_assert(CF == 0 || (!PRE && (CF == 2 || CF == 4)), "CF: 0 (tensor pipe), 2 or 4 real columns (FP64 pipe)");
     constexpr int NC = 8;
     constexpr int TLF = FWD_TILE(R);
     __shared__ double2 s_ag[TLF];
@@ -433,13 +507,21 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
     const int Mfull = A.isReal ? Lfull : 2 * Lfull - 1;
     const int T = blockDim.x, W = T >> 5;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, hemi = warp & 1;
-    double *dt = s_dt + (size_t)warp * R * FWD_GT;
+    // per warp: R B-fragment tiles, or (CF > 0) the 8 CF x 32 partial sums of an octet
+    constexpr int DT_WARP = R * FWD_GT > 8 * CF * FWD_PS ? R * FWD_GT : 8 * CF * FWD_PS;
+    double *dt = s_dt + (size_t)warp * DT_WARP;
+    // gridDim.z > 1: the ring groups of the grid are dealt out to gridDim.z blocks per (m, chunk), 8 warps each, instead
+    // of one block of 16 warps (grids with more than 32 groups): two blocks per SM, so that one block's barriers and
+    // epilogue overlap the other's recursion.  Slot r of warp w is group (r gridDim.z + blockIdx.z) W + w; each block
+    // adds its partial sums into f_lm with the atomics the epilogue uses anyway.
+    const int gz = gridDim.z, bz = blockIdx.z;
+#define FWD_GRP(r) (((r) * gz + bz) * W + warp)
     const int wr_off = (lane >> 2) * FWD_QS + (lane & 3);  // + 4 * (l & 7): store slot of this lane's ring
 
     double y[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const int g = r * W + warp;
+        const int g = FWD_GRP(r);
         y[r] = g < G ? A.yv[g * 32 + lane] : 0.0;
     }
     // A-fragment coordinates of this lane: column c = lane / 4, ring quad member lane % 4
@@ -463,13 +545,32 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
 
         // ring data as A-fragments: hA[r][quad] = h[ring (r, quad, fk)][column fc]
         int gs[R];
-        double d[R], u[R], hA[R][8];
+        double d[R], u[R], hA[R][8], h[R][CF > 0 ? CF : 1];  // hA: tensor-pipe path, h: CF > 0
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const int g = r * W + warp;
+            const int g = FWD_GRP(r);
             gs[r] = g < G ? gsrow[g] : INT_MAX;
             d[r] = 0.0;
             u[r] = 0.0;
+            if constexpr (CF > 0) {
+                // ring data of this lane's own ring: (re, im) of complex column k (not fused: CF / 2 columns of A.F;
+                // fused: column 0 of scale A, then of scale B), zero for padding slots
+                const int t = g < G ? A.ring[g * 32 + lane] : -1;
+#pragma unroll
+                for (int k = 0; k < CF / 2; ++k) {
+                    const ColInfo ci = col_info(A, FUSE ? 0 : k);
+                    const int row = ci.minus ? A.n_rowm[q] : A.n_row[q];
+                    const int mi = A.isReal ? m : (ci.minus ? Lg - 1 - m : Lg - 1 + m);
+                    const bool ok = t >= 0 && ci.valid;
+                    const cplx *src = ((FUSE && k) ? A.F2 : A.F) +
+                                      (((size_t)(ci.valid ? ci.b : 0) * A.nrows + row) * Md + mi) * A.nt + (ok ? t : 0);
+                    const cplx v = *src;
+                    const double keep = ok ? (ci.minus ? sgn : 1.0) : 0.0;
+                    h[r][2 * k] = ok ? v.x * keep : 0.0;
+                    h[r][2 * k + 1] = ok ? v.y * keep : 0.0;
+                }
+                continue;
+            }
             // branch-free, so that the 8 ring indices and then the 8 values are loaded together (one latency each,
             // not one per value): invalid rings / columns read element 0 of a valid column and are zeroed afterwards
             const int row = fci.minus ? A.n_rowm[q] : A.n_row[q];
@@ -516,7 +617,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
 #pragma unroll
                         for (int r = 0; r < R; ++r) {
                             if (gs[r] >= lo + 8) continue;
-                            const double *src = trow + (r * W + warp) * 32;
+                            const double *src = trow + FWD_GRP(r) * 32;
                             double bv[8];
 #pragma unroll
                             for (int qd = 0; qd < 8; ++qd) bv[qd] = ok ? __ldg(src + 4 * qd) : 0.0;
@@ -541,7 +642,49 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                     }
                     double *dst = dt + wr_off;
                     const double *src = dt + lane;
-                    if (!starting) {
+                    if (CF > 0) {
+                        double *pw = dt + lane;
+                        if (!starting) {
+                            fwd_octet_dfma_ra<R, CF>(ra, mm, s_ag + 8 * oc, se + 16 * oc, pw, y, d, u, h);
+                        } else {
+#pragma unroll 1
+                            for (int s = 0; s < 8; ++s) {
+                                const double2 ag = s_ag[8 * oc + s];
+                                const double e = se[2 * (8 * oc + s)];
+                                double pp[CF > 0 ? CF : 1];
+#pragma unroll
+                                for (int c = 0; c < CF; ++c) pp[c] = 0.0;
+#pragma unroll
+                                for (int r = 0; r < R; ++r) {
+                                    if (r < ra) {
+                                        if (gs[r] == lo + s) {  // the group starts here (warp-uniform)
+                                            const double2 sd = seedrow[FWD_GRP(r) * 32 + lane];
+                                            d[r] = sd.x;
+                                            u[r] = sd.y;
+                                        }
+#pragma unroll
+                                        for (int c = 0; c < CF; ++c) pp[c] = fma(d[r], h[r][c], pp[c]);
+                                        wig_step(d[r], u[r], y[r], ag.x, ag.y, e);
+                                    }
+                                }
+#pragma unroll
+                                for (int c = 0; c < CF; ++c) pw[(s * CF + c) * FWD_PS] = pp[c];
+                            }
+                        }
+                        if (mm) {
+                            __syncwarp();
+                            double v = fwd_octet_reduce<(CF > 0 ? CF : 2)>(dt, lane);
+                            constexpr int K = 8 * (CF > 0 ? CF : 2);
+                            if (lane < K) {
+                                const int sdeg = lane / (CF > 0 ? CF : 2), c = lane % (CF > 0 ? CF : 2);
+                                // southern warps: d = (-1)^l d~, and the octet starts at an even degree
+                                if (hemi && (sdeg & 1)) v = -v;
+                                atomicAdd(&s_red[SRED(8 * oc + sdeg, FUSE ? ((c >> 1) * 4 + (c & 1)) : c)], v);
+                            }
+                            __syncwarp();
+                        }
+                        contributed = false;  // the sums of this octet are in s_red already
+                    } else if (!starting) {
                         const double2 *ag8 = s_ag + 8 * oc;
                         const double *se8 = se + 16 * oc;
                         if (R >= 4 && ra == 4)
@@ -561,7 +704,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                             for (int r = 0; r < R; ++r) {
                                 if (r < ra) {
                                     if (gs[r] == lo + s) {  // the group starts here (warp-uniform)
-                                        const double2 sd = seedrow[(r * W + warp) * 32 + lane];
+                                        const double2 sd = seedrow[FWD_GRP(r) * 32 + lane];
                                         d[r] = sd.x;
                                         u[r] = sd.y;
                                     }
@@ -1068,17 +1211,19 @@ void launch_inv_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
     S2W_LAUNCH_C(S2W_K_WIGNER_INV, (wigner_inverse_kernel<NC, R, MAXT, NS>), grid, T, 0, st, A);
 }
 
-template <int R, int MAXT, bool PRE, bool FUSE>
-int launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
+template <int R, int MAXT, bool PRE, bool FUSE, int CF = 0>
+int launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st, int gz = 1)
 {
-    const size_t smem = PRE ? 0 : (size_t)(T / 32) * R * FWD_GT * sizeof(double);
+    // per warp: R B-fragment tiles (tensor pipe) or the 8 CF x 32 partial sums of an octet (CF > 0)
+    constexpr size_t per_warp = ((size_t)R * FWD_GT > (size_t)8 * CF * FWD_PS ? (size_t)R * FWD_GT : (size_t)8 * CF * FWD_PS) * sizeof(double);
+    const size_t smem = PRE ? 0 : (size_t)(T / 32) * per_warp;
     // the attribute is per device and per function: query and raise it when needed (smem_attr.cuh), no per-process flag
     {
-        const int rc = set_smem(wigner_forward_kernel<R, MAXT, PRE, FUSE>, (size_t)(MAXT / 32) * R * FWD_GT * sizeof(double));
+        const int rc = set_smem(wigner_forward_kernel<R, MAXT, PRE, FUSE, CF>, (size_t)(MAXT / 32) * per_warp);
         if (rc) return rc;
     }
-    dim3 grid(A.Lg, chunks);
-    S2W_LAUNCH_C(S2W_K_WIGNER_FWD, (wigner_forward_kernel<R, MAXT, PRE, FUSE>), grid, T, smem, st, A);
+    dim3 grid(A.Lg, chunks, gz);
+    S2W_LAUNCH_C(S2W_K_WIGNER_FWD, (wigner_forward_kernel<R, MAXT, PRE, FUSE, CF>), grid, T, smem, st, A);
     return S2W_OK;
 }
 
@@ -1100,8 +1245,57 @@ int dispatch_inv(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t st)
     return S2W_EINVAL;
 }
 
+static bool split_on()
+{
+    static const bool split = [] {
+        const char *e = getenv("S2W_FWD_SPLIT");
+        return !(e && e[0] == '0');
+    }();
+    return split;
+}
+
 int dispatch_fwd(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t st)
 {
+    // grids with more than 32 ring groups (L_j > 1024): two 8-warp blocks per (m, chunk), each with half of the groups
+    // (wigner_forward_kernel, gridDim.z), instead of one 16-warp block
+    const bool split = split_on();
+    // few columns: the FP64-pipe variant (fwd_octet_dfma).  CF = real columns per recursion: 2 CT, twice that when two
+    // scales share the recursion.  S2W_FWD_DFMA = 0: never, 2: only CF = 2, 4 (default): CF = 2 and CF = 4
+    static const int dfma_max = [] {
+        const char *e = getenv("S2W_FWD_DFMA");
+        return e ? atoi(e) : 4;
+    }();
+    const int CT = A.isReal ? A.B : 2 * A.B;
+    const int cf = (A.F2 ? 4 : 2) * CT;
+    const int gz = (split_on() && c.W == 16) ? 2 : 1;
+    // CF = 4 pays from three ring groups per warp on (FP64 instructions per warp and octet: 64 R + 32 against 96 R)
+    static const int dfma4_minR = [] {
+        const char *e = getenv("S2W_FWD_DFMA4_MINR");
+        return e ? atoi(e) : 3;
+    }();
+    if (!A.dtab && cf <= dfma_max && (cf == 2 || c.R >= dfma4_minR) && (c.MAXT == 256 || gz == 2)) {
+#define S2W_WIG_CASE(RR)                                                                                   \
+    if (c.R == RR) {                                                                                       \
+        if (A.F2) return launch_fwd_t<RR, 256, false, true, 4>(A, gz == 2 ? 256 : 32 * c.W, 1, st, gz);    \
+        return cf == 2 ? launch_fwd_t<RR, 256, false, false, 2>(A, gz == 2 ? 256 : 32 * c.W, 1, st, gz)    \
+                       : launch_fwd_t<RR, 256, false, false, 4>(A, gz == 2 ? 256 : 32 * c.W, 1, st, gz);   \
+    }
+        S2W_WIG_CASE(1)
+        S2W_WIG_CASE(2)
+        S2W_WIG_CASE(3)
+        S2W_WIG_CASE(4)
+#undef S2W_WIG_CASE
+    }
+    if (split && c.W == 16) {
+#define S2W_WIG_CASE(RR)                                                                \
+    if (c.R == RR)                                                                      \
+        return A.dtab ? launch_fwd_t<RR, 256, true, false>(A, 256, chunks, st, 2)       \
+                      : (A.F2 ? launch_fwd_t<RR, 256, false, true>(A, 256, chunks, st, 2) \
+                              : launch_fwd_t<RR, 256, false, false>(A, 256, chunks, st, 2));
+        S2W_WIG_CASE(3)
+        S2W_WIG_CASE(4)
+#undef S2W_WIG_CASE
+    }
 #define S2W_WIG_CASE(RR, MT)                                                              \
     if (c.R == RR && c.MAXT == MT)                                                        \
         return A.dtab ? launch_fwd_t<RR, MT, true, false>(A, 32 * c.W, chunks, st)        \
