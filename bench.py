@@ -532,7 +532,7 @@ def run_ball(args, cfg):
     torch.cuda.set_device(0)
     device = torch.device("cuda", 0)
     L, P, N, lam, nu, J0, tau = cfg["L"], cfg["P"], cfg["N"], cfg["lam"], cfg["nu"], cfg["J0"], cfg["tau"]
-    plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau)
+    plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau, flags=api.S2W_PRECOMPUTE if getattr(args, "precompute", False) else 0)
     flmp = inputs.config_coefficients(cfg["name"])
     f = plan.harmonic_inverse(torch.from_numpy(flmp).to(device).reshape(1, -1))
     w = torch.empty((1, plan.coeff_elems), dtype=plan.dtype, device=device)

@@ -676,10 +676,12 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                             double v = fwd_octet_reduce<(CF > 0 ? CF : 2)>(dt, lane);
                             constexpr int K = 8 * (CF > 0 ? CF : 2);
                             if (lane < K) {
-                                const int sdeg = lane / (CF > 0 ? CF : 2), c = lane % (CF > 0 ? CF : 2);
+                                const int sdeg = lane / (CF > 0 ? CF : 2);
                                 // southern warps: d = (-1)^l d~, and the octet starts at an even degree
                                 if (hemi && (sdeg & 1)) v = -v;
-                                atomicAdd(&s_red[SRED(8 * oc + sdeg, FUSE ? ((c >> 1) * 4 + (c & 1)) : c)], v);
+                                // CF > 0 layout of s_red: [degree][CF], the K lanes hit K consecutive doubles (the SRED
+                                // layout of the tensor-pipe path would put them four to a bank)
+                                atomicAdd(&s_red[(8 * oc) * (CF > 0 ? CF : 2) + lane], v);
                             }
                             __syncwarp();
                         }
@@ -749,7 +751,9 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                 cplx val = cmake(0.0, 0.0);
                 for (int sc = 0; sc < (fuse ? 2 : 1); ++sc) {
                     const int c0i = 2 * k + 4 * sc;
-                    const double re = s_red[SRED(ll, c0i)], im = s_red[SRED(ll, c0i + 1)];
+                    const int cp = FUSE ? 2 * sc : 2 * k;  // CF > 0: column pair of (scale sc | complex column k)
+                    const double re = CF > 0 ? s_red[ll * (CF > 0 ? CF : 2) + cp] : s_red[SRED(ll, c0i)];
+                    const double im = CF > 0 ? s_red[ll * (CF > 0 ? CF : 2) + cp + 1] : s_red[SRED(ll, c0i + 1)];
                     const cplx Gf = (sc ? A.filt2 : A.filt)[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
                     val = cadd(val, cmul(Gf, cmake(re, im)));
                 }
