@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5", "T2"])
     ap.add_argument("--precompute", action="store_true",
                     help="sphere workloads: the precomputed-kernel variant (S2W_PRECOMPUTE, step a9)")
+    ap.add_argument("--recursion", action="store_true",
+                    help="ball workloads: S2W_RECURSION, the on-the-fly Wigner recursion where the plan would precompute")
     ap.add_argument("--adjoint", action="store_true",
                     help="sphere workloads: time the adjoint pair S^H (signal -> coefficients) + A^H (coefficients -> "
                          "signal) of the workload's plan (SURVEY 8(f)-1); no e2e / cpu_baseline")
@@ -532,7 +534,11 @@ def run_ball(args, cfg):
     torch.cuda.set_device(0)
     device = torch.device("cuda", 0)
     L, P, N, lam, nu, J0, tau = cfg["L"], cfg["P"], cfg["N"], cfg["lam"], cfg["nu"], cfg["J0"], cfg["tau"]
-    plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau, flags=api.S2W_PRECOMPUTE if getattr(args, "precompute", False) else 0)
+    flags = api.S2W_PRECOMPUTE if getattr(args, "precompute", False) else (api.S2W_RECURSION if getattr(args, "recursion", False) else 0)
+    plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau, flags=flags)
+    pre = bool(flags & api.S2W_PRECOMPUTE) or (not (flags & api.S2W_RECURSION) and L <= 128)
+    if flags:
+        args.no_e2e = True                          # the host-buffer entry points build their plan with flags = 0
     flmp = inputs.config_coefficients(cfg["name"])
     f = plan.harmonic_inverse(torch.from_numpy(flmp).to(device).reshape(1, -1))
     w = torch.empty((1, plan.coeff_elems), dtype=plan.dtype, device=device)
@@ -614,6 +620,8 @@ def run_ball(args, cfg):
         "config": {"workload": "%s: ball L=%d P=%d N=%d lambda_l=%g lambda_p=%g J0=%d tau=%g complex fp64, "
                                "%s" % (cfg["name"], L, P, N, lam, nu, J0, tau, "adjoint pair S^H + A^H" if adj else "forward+inverse"),
                    "L": L, "P": P, "N": N, "parallelism": "replicas x1 (no data-path collective)",
+                   "mode": ("precomputed Wigner-d tables, theta quadrature folded into the table on grids with L_j <= 128 "
+                            "(the default of ball plans with L <= 128)" if pre else "on-the-fly Wigner recursion"),
                    "l2": "coefficient block per step (%.2f GB) exceeds the 126 MB L2; no explicit flush"
                          % (plan.coeff_elems * 16 / 1e9)},
         "clocks": clocks, "gpu_launches": int(launches),

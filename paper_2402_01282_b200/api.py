@@ -14,6 +14,7 @@ from . import build as _build
 S2W_REAL = 1
 S2W_PRECOMPUTE = 2
 S2W_DH = 4
+S2W_RECURSION = 8
 S2W_STATIC_SCRATCH_BYTES = 32 << 20   # include/s2w.h: capacity of the static device scratch array
 _ERRORS = {-1: "S2W_EINVAL", -2: "S2W_ENOMEM", -3: "S2W_ECUDA", -4: "S2W_EUNSUPPORTED"}
 

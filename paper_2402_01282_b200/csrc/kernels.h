@@ -60,6 +60,8 @@ struct WigArgs {
     const int *ring;            // [32 G] ring index t of the slot, -1 if empty
     const double *dtab;         // precomputed-kernel variant: [ntab][tri_g][32 G] d^l_mn(beta) per ring slot, else null
     size_t tri_g;               // Lg (Lg + 1) / 2
+    int dense;                  // forward direction, dtab = the quadrature-folded table (launch_wigner_table_fold): every ring
+                                // group is active from l = max(m, |n|) on (no group starts), the input is F transposed, NOT reweighted
     const cplx *filt;           // [nn][Lg] filter applied to row q at degree l
     // two scales sharing one recursion (same grid, same rows n; at most 2 complex columns): the second scale's filter,
     // support start (>= lmin) and array; null / unused otherwise
@@ -73,6 +75,13 @@ struct WigArgs {
 
 void set_error(const std::string &msg);
 
+// S2W_PRECOMPUTE on small grids: fold the theta quadrature (the reweighting operator R_sigma of DESIGN.md 6.3, real and
+// symmetric) into the table of one n: X[l][t][m] = d^l_mn(theta_t) (gather), Y = R X per column by the reweighting kernels,
+// dtab_rw = Y in the table's layout (scatter).  sum_t d(theta_t) (R F)(theta_t) = sum_t (R d)(theta_t) F(theta_t).
+int launch_wigner_table_gather(const double *dtab, size_t tri_g, int tab, int n, int Lg, int nt, int G, const int *ring, cplx *X,
+                               cudaStream_t st);
+int launch_wigner_table_scatter(const cplx *Y, double *dtab_rw, size_t tri_g, int tab, int n, int Lg, int nt, int G,
+                                const int *ring, cudaStream_t st);
 int launch_twiddles(cplx *tw, int Mtab, cudaStream_t st);
 int launch_fft_tables(const FftTab &T, cplx *chirp, cplx *rw_in1, cplx *rw_out1, cplx *rw_in3, cplx *rw_out3,
                       cplx *bhat_m, cplx *bhat_p, cplx *what, cudaStream_t st);

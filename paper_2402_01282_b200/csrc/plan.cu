@@ -121,6 +121,9 @@ struct GridTab {  // everything that depends on the theta/phi grid of band-limit
     int *gstart;     // [ntab][Lg][G]
     double2 *dseed;  // [ntab][Lg][32 G]
     double *dtab;    // S2W_PRECOMPUTE: [ntab][Lg (Lg+1)/2][32 G] d^l_mn(beta) per ring slot (else null)
+    double *dtab_rw; // S2W_PRECOMPUTE, McEwen-Wiaux grids with Lg <= S2W_FOLD_MAX_L: the same table with the theta quadrature
+                     // folded in, (R_sigma d^l_mn)(theta_t): the rings -> harmonic contraction then takes F transposed, and
+                     // the reweighting step (a2) disappears from the transform (else null)
 };
 
 struct Stage {  // one Wigner contraction launch: rows, filters
@@ -559,6 +562,17 @@ int build_rw(s2w_plan *p, GridTab &g)
     return S2W_OK;
 }
 
+// largest band-limit of a grid whose precomputed table also gets the quadrature-folded copy (GridTab::dtab_rw): small
+// grids, where the reweighting kernels cost more than the contraction saves by skipping the rings below a group start
+static int fold_max_l()
+{
+    static const int v = [] {
+        const char *e = getenv("S2W_FOLD_MAX_L");
+        return e ? atoi(e) : 128;
+    }();
+    return v;
+}
+
 int build_grid(s2w_plan *p, int Lg)
 {
     if (grid_index(p, Lg) >= 0) return S2W_OK;
@@ -656,6 +670,42 @@ int build_grid(s2w_plan *p, int Lg)
                                       g.dtab, tri_g, 0)))
             return rc;
         S2W_CUDA_CHECK(cudaDeviceSynchronize());
+        if (!p->dh && g.rw.L && Lg <= fold_max_l()) {
+            // sum_t d(theta_t) (R F)(theta_t) = sum_t (R d)(theta_t) F(theta_t), R real symmetric: run the
+            // reweighting kernels once over the table's columns (ring index t at fixed (l, m, n)) instead of over every
+            // transform's columns
+            if ((rc = p->pool.alloc(&g.dtab_rw, elems))) return rc;
+            S2W_CUDA_CHECK(cudaMemsetAsync(g.dtab_rw, 0, elems * sizeof(double), 0));
+            cplx *X = 0, *Y = 0;
+            const size_t slab = (size_t)Lg * g.nt * Lg;
+            if (cudaMalloc((void **)&X, slab * sizeof(cplx)) != cudaSuccess || cudaMalloc((void **)&Y, slab * sizeof(cplx)) != cudaSuccess) {
+                cudaFree(X);
+                cudaGetLastError();
+                set_error("no device memory for the set-up buffers of the quadrature-folded table");
+                return S2W_ENOMEM;
+            }
+            for (size_t tab = 0; tab < ntab && !rc; ++tab) {
+                RwArgs R;
+                memset(&R, 0, sizeof(R));
+                R.nn = 1;
+                R.nrows = 1;
+                R.Md = Lg;
+                R.isReal = 1;
+                R.n_val[0] = p->tabn[tab];
+                R.n_row[0] = 0;
+                rc = launch_wigner_table_gather(g.dtab, tri_g, (int)tab, p->tabn[tab], Lg, g.nt, g.G, g.ring, X, 0);
+                if (!rc) rc = launch_reweight_th(X, Y, R, Lg, g.rw, 0);
+                if (!rc) rc = launch_wigner_table_scatter(Y, g.dtab_rw, tri_g, (int)tab, p->tabn[tab], Lg, g.nt, g.G, g.ring, 0);
+            }
+            const cudaError_t ce = cudaDeviceSynchronize();
+            cudaFree(X);
+            cudaFree(Y);
+            if (rc) return rc;
+            if (ce != cudaSuccess) {
+                set_error(std::string("quadrature-folded table: ") + cudaGetErrorString(ce));
+                return S2W_ECUDA;
+            }
+        }
     }
     p->grids.push_back(g);
     return S2W_OK;
@@ -710,6 +760,7 @@ void fill_wig_args(const s2w_plan *p, const Stage &st, bool synthesis, int B, cp
     A.yv = g.yv;
     A.ring = g.ring;
     A.dtab = g.dtab;
+    A.dense = 0;
     A.tri_g = (size_t)st.Lg * (st.Lg + 1) / 2;
     A.filt = synthesis ? st.filt_syn : st.filt_ana;
     A.filt2 = 0;
@@ -966,13 +1017,29 @@ static double scale_cost(const Scale &sc) { return (double)sc.Lj * sc.Lj * sc.Lj
 // Step a2 on the grid of a stage: F[b][row][t][mi] -> Ft[b][row][mi][t] with the theta quadrature applied.  McEwen-Wiaux:
 // the reweighting operator of reading R3 (Toeplitz/Hankel form, or the Bluestein kernel on tiny grids); Driscoll-Healy:
 // the diagonal quadrature weights q_t, applied by the transposing copy.
-static int stage_reweight(const s2w_plan *p, const Stage &st, const cplx *F, cplx *Ft, int B, cudaStream_t s)
+// `folded`: the caller contracts with the quadrature-folded table (GridTab::dtab_rw, see use_folded): transposing copy only.
+static int stage_reweight(const s2w_plan *p, const Stage &st, const cplx *F, cplx *Ft, int B, cudaStream_t s,
+                          bool folded = false)
 {
     const GridTab &g = p->grids[st.grid];
+    if (folded) return launch_transpose(F, Ft, g.nt, p->real ? st.Lg : 2 * st.Lg - 1, B * st.nrows, s, 0);
     if (g.dhw) return launch_transpose(F, Ft, g.nt, p->real ? st.Lg : 2 * st.Lg - 1, B * st.nrows, s, g.dhw);
     RwArgs R;
     fill_rw_args(p, st, R);
     return g.rw.L ? launch_reweight_th(F, Ft, R, B, g.rw, s) : launch_reweight(F, Ft, R, B, g.fft, s);
+}
+
+// rings -> harmonic contraction of a stage with the quadrature-folded table (transforms only; the adjoint calls and the
+// stand-alone Q transform keep the plain table and the explicit reweighting)
+static bool use_folded(const s2w_plan *p, const Stage &st, WigArgs *A)
+{
+    const GridTab &g = p->grids[st.grid];
+    if (!g.dtab_rw) return false;
+    if (A) {
+        A->dtab = g.dtab_rw;
+        A->dense = 1;
+    }
+    return true;
 }
 
 // pixels of one signal on the grid of band-limit Lg: rings x (2 Lg - 1)
@@ -1019,13 +1086,14 @@ static int sht_forward_dev(const s2w_plan *p, const Stage &st, const void *f, si
         return S2W_OK;
     }
     if ((rc = stage_ring_fwd(p, st, f, sig_stride, B, w.F, s))) return rc;
-    if ((rc = stage_reweight(p, st, w.F, w.Ft, B, s))) return rc;
+    if ((rc = stage_reweight(p, st, w.F, w.Ft, B, s, use_folded(p, st, 0)))) return rc;
     if (zero_first) {
         const size_t Mfull = p->real ? p->L : 2 * p->L - 1;
         S2W_CUDA_CHECK(cudaMemsetAsync(w.flmT, 0, (size_t)B * Mfull * p->L * sizeof(cplx), s));
     }
     WigArgs A;
     fill_wig_args(p, st, true, B, w.flmT, w.Ft, A);
+    use_folded(p, st, &A);
     return launch_wigner_forward(A, s);
 }
 
@@ -1081,9 +1149,10 @@ static int scale_synthesis(const s2w_plan *p, const Scale &sc, int B, const Work
     fill_so3_args(p, sc.st, S);
     S.sig_off = sig_off;
     if ((rc = launch_so3_fwd(p->real, src, sig_stride, w.F, S, B, g.fft, s))) return rc;
-    if ((rc = stage_reweight(p, sc.st, w.F, w.Ft, B, s))) return rc;
+    if ((rc = stage_reweight(p, sc.st, w.F, w.Ft, B, s, use_folded(p, sc.st, 0)))) return rc;
     WigArgs A;
     fill_wig_args(p, sc.st, true, B, w.flmT, w.Ft, A);
+    use_folded(p, sc.st, &A);
     return launch_wigner_forward(A, s);
 }
 
@@ -1890,6 +1959,11 @@ int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, dou
         set_error("L > 2048 is not supported");
         return S2W_EUNSUPPORTED;
     }
+    // Small angular band-limits: a ball plan contracts hundreds of columns (shells x signed columns) with every Wigner-d
+    // value, and the tables of all its grids are a few tens of MB (L2-resident): the precomputed-kernel variant with the
+    // theta quadrature folded into the table (GridTab::dtab_rw) is the default there ("simply precomputed" below
+    // L ~ 256); S2W_RECURSION keeps the on-the-fly recursion.
+    if (!(flags & (S2W_PRECOMPUTE | S2W_RECURSION)) && L <= fold_max_l()) flags |= S2W_PRECOMPUTE;
     S2W_CUDA_CHECK(cudaSetDevice(device));
     s2w_plan *p = new s2w_plan();
     p->kind = 1;

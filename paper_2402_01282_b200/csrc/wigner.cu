@@ -549,7 +549,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int g = FWD_GRP(r);
-            gs[r] = g < G ? gsrow[g] : INT_MAX;
+            gs[r] = g < G ? ((PRE && A.dense) ? l0 : gsrow[g]) : INT_MAX;
             d[r] = 0.0;
             u[r] = 0.0;
             if constexpr (CF > 0) {
@@ -592,7 +592,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
         // tiles start at the first group start; tiles wholly below the filter support run the recursion only
         int first = gsrow[0];
         if (G > 1 && gsrow[1] < first) first = gsrow[1];
-        if (first < l0) first = l0;
+        if (first < l0 || (PRE && A.dense)) first = l0;
 
         for (int lt = first & ~(TLF - 1); lt < Lg; lt += TLF) {
             __syncthreads();
@@ -794,6 +794,33 @@ __global__ void __launch_bounds__(32) wigner_table_kernel(const double *__restri
         out[(size_t)l * (32 * G)] = (south && (l & 1)) ? -d : d;
         const double4 q = *reinterpret_cast<const double4 *>(c + 4 * (size_t)l);
         wig_step(d, u, y, q.x, q.y, south ? q.w : q.z);
+    }
+}
+
+// the table of one n as reweighting input X[l][t][m] (complex, imaginary part zero) and back (kernels.h)
+__global__ void wigner_table_gather_kernel(const double *__restrict__ dtab, size_t tri_g, int tab, int n, int Lg, int nt,
+                                           int G, const int *__restrict__ ring, cplx *__restrict__ X)
+{
+    const int l = blockIdx.x, m = blockIdx.y;
+    const int an = n < 0 ? -n : n;
+    const bool in = l >= m && l >= an;
+    const double *row = dtab + ((size_t)tab * tri_g + tri_off(m, Lg) + (in ? l : m)) * (size_t)(32 * G);
+    for (int k = threadIdx.x; k < 32 * G; k += blockDim.x) {
+        const int t = ring[k];
+        if (t >= 0 && t < nt) X[((size_t)l * nt + t) * Lg + m] = cmake(in ? row[k] : 0.0, 0.0);
+    }
+}
+
+__global__ void wigner_table_scatter_kernel(const cplx *__restrict__ Y, double *__restrict__ dtab_rw, size_t tri_g, int tab,
+                                            int n, int Lg, int nt, int G, const int *__restrict__ ring)
+{
+    const int l = blockIdx.x, m = blockIdx.y;
+    const int an = n < 0 ? -n : n;
+    if (l < m || l < an) return;
+    double *row = dtab_rw + ((size_t)tab * tri_g + tri_off(m, Lg) + l) * (size_t)(32 * G);
+    for (int k = threadIdx.x; k < 32 * G; k += blockDim.x) {
+        const int t = ring[k];
+        row[k] = (t >= 0 && t < nt) ? Y[((size_t)l * Lg + m) * nt + t].x : 0.0;
     }
 }
 
@@ -1416,6 +1443,22 @@ int launch_wigner_table(const double *coef, size_t tri, int Lfull, int Lg, int G
     for (int i = 0; i < ntab; ++i) nl.v[i] = n_vals[i];
     dim3 grid(G, Lg, ntab);
     S2W_LAUNCH(wigner_table_kernel, grid, 32, 0, st, coef, tri, Lfull, Lg, G, nl, yv, gstart, dseed, dtab, tri_g);
+    return S2W_OK;
+}
+
+int launch_wigner_table_gather(const double *dtab, size_t tri_g, int tab, int n, int Lg, int nt, int G, const int *ring, cplx *X,
+                               cudaStream_t st)
+{
+    dim3 grid(Lg, Lg);
+    S2W_LAUNCH(wigner_table_gather_kernel, grid, 128, 0, st, dtab, tri_g, tab, n, Lg, nt, G, ring, X);
+    return S2W_OK;
+}
+
+int launch_wigner_table_scatter(const cplx *Y, double *dtab_rw, size_t tri_g, int tab, int n, int Lg, int nt, int G,
+                                const int *ring, cudaStream_t st)
+{
+    dim3 grid(Lg, Lg);
+    S2W_LAUNCH(wigner_table_scatter_kernel, grid, 128, 0, st, Y, dtab_rw, tri_g, tab, n, Lg, nt, G, ring);
     return S2W_OK;
 }
 

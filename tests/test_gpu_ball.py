@@ -57,11 +57,14 @@ CASES = [
 ]
 
 
+@pytest.mark.parametrize("mode", ["default", "recursion"])
 @pytest.mark.parametrize("L,P,N,lam,nu,J0,tau", CASES)
-def test_ball_forward_inverse_parity(L, P, N, lam, nu, J0, tau):
+def test_ball_forward_inverse_parity(L, P, N, lam, nu, J0, tau, mode):
+    """Both modes of a small ball plan against the oracle: the default (L <= 128: precomputed Wigner-d tables with the
+    theta quadrature folded in, step a2 a transposing copy) and S2W_RECURSION (on-the-fly recursion, explicit step a2)."""
     torch, api = _api()
     flmp, f = _voxels(L, P, tau, 70 + L + N)
-    plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau)
+    plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau, flags=api.S2W_RECURSION if mode == "recursion" else 0)
     fd = torch.from_numpy(f).cuda().reshape(1, -1)
     w = plan.forward(fd)
     scal, scales = plan.split(w)
@@ -122,14 +125,16 @@ def test_ball_real_signal_gives_real_coefficients():
     pc.close()
 
 
-def test_config5_full_size():
-    """BASELINE config 5 at full size (L = P = 128, N = 3, complex, 64 (j, j') scales): round trip on all voxels,
+@pytest.mark.parametrize("mode", ["default", "recursion"])
+def test_config5_full_size(mode):
+    """BASELINE config 5 at full size (L = P = 128, N = 3, complex, 64 (j, j') scales), in the configuration bench.py times
+    (default: precomputed tables with the folded quadrature) and with S2W_RECURSION: round trip on all voxels,
     recovered f_lmp against the seeded truth, and two whole (j, j') coefficient blocks against the oracle."""
     torch, api = _api()
     c = inputs.CONFIGS["C5"]
     L, P, N, lam, nu, J0, tau = c["L"], c["P"], c["N"], c["lam"], c["nu"], c["J0"], c["tau"]
     flmp = inputs.config_coefficients("C5")
-    plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau)
+    plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau, flags=api.S2W_RECURSION if mode == "recursion" else 0)
     f = plan.harmonic_inverse(torch.from_numpy(flmp).cuda().reshape(1, -1))
     got = plan.harmonic_forward(f, P * L * (2 * L - 1)).cpu().numpy().reshape(P, L, 2 * L - 1)
     assert _relmax(got, flmp) < FWD_TOL
@@ -154,7 +159,7 @@ def test_ball_precomputed_kernel_variant_matches_on_the_fly():
     L, P, N, lam, nu, J0, tau = 20, 8, 3, 2.0, 2.0, 0, 1.0
     flmp, f = _voxels(L, P, tau, 77)
     fd = torch.from_numpy(f).cuda().reshape(1, -1)
-    otf = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau)
+    otf = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau, flags=api.S2W_RECURSION)
     pre = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau, flags=api.S2W_PRECOMPUTE)
     w0, w1 = otf.forward(fd), pre.forward(fd)
     assert float((w0 - w1).abs().max()) < 1e-12 * float(w0.abs().max())
