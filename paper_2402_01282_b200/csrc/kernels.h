@@ -113,6 +113,10 @@ int launch_ring16(bool fwd, bool real, const void *in, void *out, int nrows, siz
 bool so3_c16_supported(const So3Args &A, const FftTab &T);            // a8, complex signals, <= 3 rows, M = 256 ... 1024
 int launch_so3_c16(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
                    cudaStream_t st);
+// a8, complex signals, <= 3 rows, 2 L_j - 1 = 255 = 3 x 5 x 17: prime-factor transform without twiddles (pfa255_kernels.cu)
+bool so3_pfa255_supported(const So3Args &A, const FftTab &T);
+int launch_so3_pfa255(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
+                      cudaStream_t st);
 
 // plan-time: group start degrees and seeds from the range-extended values d^{l0}_{mn}(beta_t) = mant 2^expo ([ntab][Lg m][Lg t])
 int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int nt, int G,
