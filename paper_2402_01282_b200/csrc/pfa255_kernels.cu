@@ -127,7 +127,7 @@ __device__ __forceinline__ void pfa_round(cplx *buf)
 
 // analysis side: F -> W(gamma_g, beta_t, alpha_a) = sum_{m,n} F_mn(beta_t) e^{i(m alpha_a + n gamma_g)}
 template <int NN>
-__global__ void __launch_bounds__(256, 2) so3_inv_pfa255_kernel(const cplx *__restrict__ F, cplx *__restrict__ W,
+__global__ void __launch_bounds__(256, 3) so3_inv_pfa255_kernel(const cplx *__restrict__ F, cplx *__restrict__ W,
                                                                size_t sig_stride, So3Args A, int L)
 {
     constexpr int RB = PFA_SEQS / NN;
@@ -171,7 +171,7 @@ __global__ void __launch_bounds__(256, 2) so3_inv_pfa255_kernel(const cplx *__re
 
 // synthesis side: F_mn(beta_t) = 1/(n_a n_g) sum_{a,g} W e^{-i(m alpha_a + n gamma_g)}
 template <int NN>
-__global__ void __launch_bounds__(256, 2) so3_fwd_pfa255_kernel(const cplx *__restrict__ W, cplx *__restrict__ F,
+__global__ void __launch_bounds__(256, 3) so3_fwd_pfa255_kernel(const cplx *__restrict__ W, cplx *__restrict__ F,
                                                                size_t sig_stride, So3Args A, int L)
 {
     constexpr int RB = PFA_SEQS / NN;

@@ -173,3 +173,22 @@ def test_real_ring_pair_kernels_against_the_oracle(N):
     back = plan.inverse(w)
     assert float((back - f).abs().max()) < RT_TOL * float(f.abs().max())
     plan.close()
+
+
+@pytest.mark.parametrize("N", [1, 2, 3])
+def test_alpha_gamma_prime_factor_255(N):
+    """Row a8 on grids with 2 L_j - 1 = 255 = 3 x 5 x 17 alpha samples (complex signals, 1 to 3 rows n): the prime-factor
+    kernels of pfa255_kernels.cu.  L = 128, complex, two signals: sampled rings (poles, equator, ragged last block of 15 / nn
+    rings) of the two scales with L_j = 128 against the oracle; synthesis through the round trip."""
+    torch, api = _api()
+    L, lam, J0, batch = 128, 2.0, 5, 2
+    flm = inputs.flm_complex(L, 1300 + N, batch)
+    plan = api.s2wav_plan_create(L, N, lam, J0, True, False, batch)
+    f = plan.harmonic_inverse(torch.from_numpy(flm).cuda())
+    w = plan.forward(f)
+    picks = [(plan.J, [0, 1, 4, 5, 63, 64, 120, 124, 125, 126, 127]), (plan.J - 1, [0, 2, 77, 127])]
+    for b in range(batch):
+        _check_sampled_rings(plan, w, flm[b], b, L, N, lam, J0, False, picks)
+    back = plan.inverse(w)
+    assert float((back - f).abs().max()) < RT_TOL * float(f.abs().max())
+    plan.close()
