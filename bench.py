@@ -536,7 +536,7 @@ def run_ball(args, cfg):
     L, P, N, lam, nu, J0, tau = cfg["L"], cfg["P"], cfg["N"], cfg["lam"], cfg["nu"], cfg["J0"], cfg["tau"]
     flags = api.S2W_PRECOMPUTE if getattr(args, "precompute", False) else (api.S2W_RECURSION if getattr(args, "recursion", False) else 0)
     plan = api.s2ball_plan_create(L, P, N, lam, nu, J0, tau, flags=flags)
-    pre = bool(flags & api.S2W_PRECOMPUTE) or (not (flags & api.S2W_RECURSION) and L <= 128)
+    pre = bool(flags & api.S2W_PRECOMPUTE) or (not (flags & api.S2W_RECURSION) and L <= 256)
     if flags:
         args.no_e2e = True                          # the host-buffer entry points build their plan with flags = 0
     flmp = inputs.config_coefficients(cfg["name"])
@@ -620,8 +620,8 @@ def run_ball(args, cfg):
         "config": {"workload": "%s: ball L=%d P=%d N=%d lambda_l=%g lambda_p=%g J0=%d tau=%g complex fp64, "
                                "%s" % (cfg["name"], L, P, N, lam, nu, J0, tau, "adjoint pair S^H + A^H" if adj else "forward+inverse"),
                    "L": L, "P": P, "N": N, "parallelism": "replicas x1 (no data-path collective)",
-                   "mode": ("precomputed Wigner-d tables, theta quadrature folded into the table on grids with L_j <= 128 "
-                            "(the default of ball plans with L <= 128)" if pre else "on-the-fly Wigner recursion"),
+                   "mode": ("precomputed Wigner-d tables, theta quadrature folded into the table on grids with L_j <= 256 "
+                            "(the default of ball plans with L <= 256)" if pre else "on-the-fly Wigner recursion"),
                    "l2": "coefficient block per step (%.2f GB) exceeds the 126 MB L2; no explicit flush"
                          % (plan.coeff_elems * 16 / 1e9)},
         "clocks": clocks, "gpu_launches": int(launches),

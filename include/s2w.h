@@ -74,10 +74,10 @@ int s2ball_radial_nodes(double *r, double *q, int P, double tau);
  * flags: S2W_REAL (signal and coefficients real); S2W_PRECOMPUTE: the Wigner-d values of every theta grid of the plan
  * are tabulated in device memory at creation ("simply precomputed"; 8 B per (ring, m >= 0, l, n): 21.5 GB at
  * L = 1024, N = 5) and the contractions stream that table through the FP64 tensor pipe instead of running the
- * recursion; S2W_ENOMEM if the table does not fit.  On McEwen-Wiaux grids with L_j <= 128 the table of the rings -> harmonic
+ * recursion; S2W_ENOMEM if the table does not fit.  On McEwen-Wiaux grids with L_j <= 256 the table of the rings -> harmonic
  * direction carries the theta quadrature as well ((R d^l_mn)(theta_t), R the real symmetric reweighting operator of step
- * a2), so that step a2 is a plain transposing copy there.  Ball plans with L <= 128 take S2W_PRECOMPUTE by default (a few
- * tens of MB of tables shared by hundreds of shell columns); S2W_RECURSION: never precompute (on-the-fly recursion).
+ * a2), so that step a2 is a plain transposing copy there.  Ball plans with L <= 256 take S2W_PRECOMPUTE by default (tens
+ * of MB of tables shared by hundreds of shell columns); S2W_RECURSION: never precompute (on-the-fly recursion).
  * batch = number of independent signals per call (>= 1).  device = CUDA device ordinal.
  * Creation allocates device tables, runs set-up kernels and synchronises. */
 int s2wav_plan_create(s2w_plan **out, int L, int N, double lambda, int J0, int multiresolution,

@@ -568,7 +568,7 @@ static int fold_max_l()
 {
     static const int v = [] {
         const char *e = getenv("S2W_FOLD_MAX_L");
-        return e ? atoi(e) : 128;
+        return e ? atoi(e) : 256;
     }();
     return v;
 }

@@ -60,7 +60,7 @@ CASES = [
 @pytest.mark.parametrize("mode", ["default", "recursion"])
 @pytest.mark.parametrize("L,P,N,lam,nu,J0,tau", CASES)
 def test_ball_forward_inverse_parity(L, P, N, lam, nu, J0, tau, mode):
-    """Both modes of a small ball plan against the oracle: the default (L <= 128: precomputed Wigner-d tables with the
+    """Both modes of a small ball plan against the oracle: the default (L <= 256: precomputed Wigner-d tables with the
     theta quadrature folded in, step a2 a transposing copy) and S2W_RECURSION (on-the-fly recursion, explicit step a2)."""
     torch, api = _api()
     flmp, f = _voxels(L, P, tau, 70 + L + N)
