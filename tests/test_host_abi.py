@@ -36,6 +36,21 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
     assert api.lib() is not None
 
 
+def test_binding_constants_match_the_header():
+    """The flag bits and the static-scratch capacity of the binding are the header's."""
+    text = open(os.path.join(ROOT, "include", "s2w.h")).read()
+    enum = re.search(r"enum\s*\{\s*S2W_REAL[^}]*\}", text).group(0)
+    flags = {k: int(v) for k, v in re.findall(r"(S2W_[A-Z_]+)\s*=\s*(\d+)", enum)}
+    assert flags == {"S2W_REAL": api.S2W_REAL, "S2W_PRECOMPUTE": api.S2W_PRECOMPUTE, "S2W_DH": api.S2W_DH,
+                     "S2W_RECURSION": api.S2W_RECURSION}
+    assert len(set(flags.values())) == 4 and all(v & (v - 1) == 0 for v in flags.values())   # distinct single bits
+    m = re.search(r"#define\s+S2W_STATIC_SCRATCH_BYTES\s+\((\d+)u\s*<<\s*(\d+)\)", text)
+    assert int(m.group(1)) << int(m.group(2)) == api.S2W_STATIC_SCRATCH_BYTES
+    errs = re.search(r"enum\s*\{\s*S2W_OK[^}]*\}", text).group(0)
+    codes = {k: int(v) for k, v in re.findall(r"(S2W_E[A-Z]+)\s*=\s*(-?\d+)", errs)}
+    assert codes == {v: k for k, v in api._ERRORS.items()}
+
+
 def test_scale_count_and_error_codes_without_a_device():
     assert api.s2w_scale_count(1024, 2.0) == 10
     assert api.s2w_scale_count(9, 2.0) == 4
