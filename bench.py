@@ -36,8 +36,11 @@ if ROOT not in sys.path:
 METRIC = "fp64 wavelet fwd+inv transforms/sec"
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel class, summed over the launches of ONE step (like
 # `achieved`, which is flops per step / ms per step), from the `ncu --set full` captures of profiles/r01j_wigner_ncu.md
-# (C3, on-the-fly): (workload, on-the-fly?, class) -> bytes per step.  Other workloads have no capture: traffic = null.
-NCU_TRAFFIC = {("C3", "wigner_forward"): 1.299e9 + 0.070e9, ("C3", "wigner_inverse"): 0.519e9 + 0.679e9}
+# (C3, on-the-fly) and profiles/r02d_* (C4): (workload, class) -> bytes per step.  Other workloads have no capture: traffic = null.
+NCU_TRAFFIC = {("C3", "wigner_forward"): 1.299e9 + 0.070e9, ("C3", "wigner_inverse"): 0.519e9 + 0.679e9,
+               ("C4", "wigner_forward"): 1.618e9}   # C4: the nine forward launches of a step, profiles/r02d_*.md
+NCU_TRAFFIC_SOURCE = {"C3": "profiles/r01j_wigner_ncu.md (the C3 Wigner kernels are unchanged since that capture)",
+                      "C4": "profiles/r02d_wigner_forward_few_columns.md"}
 UNIT = "transforms/s"
 
 
@@ -460,8 +463,8 @@ def run_ours(args, cfg):
     roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak if peak else None,
                 "traffic": NCU_TRAFFIC.get((cfg["name"], dom)) if not (args.precompute or adj) else None,
-                "traffic_unit": "bytes per step (all launches of the class), ncu --set full, profiles/r01j_wigner_ncu.md "
-                                "(the Wigner kernels are unchanged since that capture)",
+                "traffic_unit": "bytes per step (all launches of the class), ncu --set full, "
+                                + NCU_TRAFFIC_SOURCE.get(cfg["name"], "no capture for this workload"),
                 "peak_source": "derived: 148 SMs x 64 FP64 lanes x 2 flop x sm_max_mhz (DESIGN.md); "
                                "measured DFMA-chain probe beside it",
                 "probe": probe, "tuples_per_step": tup, "flops_per_step": flops,

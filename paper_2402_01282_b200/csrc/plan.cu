@@ -1937,8 +1937,23 @@ int s2wav_plan_create_spin(s2w_plan **out, int L, int N, double lambda, int J0, 
     return S2W_OK;
 }
 
+static int ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, double lambda_p, int J0, double tau,
+                            int flags, int device);
+
 int s2ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, double lambda_p, int J0, double tau,
                        int flags, int device)
+{
+    int rc = ball_plan_create(out, L, P, N, lambda_l, lambda_p, J0, tau, flags, device);
+    // the precomputed tables are a default here, not a request: without room for them the plan runs the recursion
+    if (rc == S2W_ENOMEM && !(flags & (S2W_PRECOMPUTE | S2W_RECURSION))) {
+        cudaGetLastError();
+        rc = ball_plan_create(out, L, P, N, lambda_l, lambda_p, J0, tau, flags | S2W_RECURSION, device);
+    }
+    return rc;
+}
+
+static int ball_plan_create(s2w_plan **out, int L, int P, int N, double lambda_l, double lambda_p, int J0, double tau,
+                            int flags, int device)
 {
     if (!out) {
         set_error("null plan pointer");
