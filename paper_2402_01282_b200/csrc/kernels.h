@@ -118,6 +118,11 @@ bool so3_pfa255_supported(const So3Args &A, const FftTab &T);
 int launch_so3_pfa255(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
                       cudaStream_t st);
 
+// a8, real signals, 2N-1 <= 9, 2 L_j - 1 = 4095 = 9 x 5 x 7 x 13: prime-factor transform without twiddles (pfa4095_kernels.cu)
+bool so3_pfa4095_supported(const So3Args &A, const FftTab &T);
+int launch_so3_pfa4095(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
+                       cudaStream_t st);
+
 // plan-time: group start degrees and seeds from the range-extended values d^{l0}_{mn}(beta_t) = mant 2^expo ([ntab][Lg m][Lg t])
 int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int nt, int G,
                         const int *n_vals, int ntab, const double *yv, const int *ring, int *gstart, double2 *dseed,

@@ -1610,6 +1610,7 @@ static int so3_launch(bool fwd, bool real, const void *in, void *out, size_t sig
                       const FftTab &T, cudaStream_t st)
 {
     const bool mw = T.nt == T.L;  // the radix-16 and ring-pair kernels are written for McEwen-Wiaux grids (L rings)
+    if (mw && real && so3_pfa4095_supported(A, T)) return launch_so3_pfa4095(fwd, in, out, sig_stride, A, batch, T, st);
     if (mw && real && 2 * A.N - 1 <= 9 && T.bhat16_m && T.M >= 1024 && f16_supported(T.M) && use_fft16())
         return launch_so3_pair16(fwd, in, out, sig_stride, A, batch, T, st);
     if (mw && !real && so3_pfa255_supported(A, T)) return launch_so3_pfa255(fwd, in, out, sig_stride, A, batch, T, st);

@@ -192,3 +192,22 @@ def test_alpha_gamma_prime_factor_255(N):
     back = plan.inverse(w)
     assert float((back - f).abs().max()) < RT_TOL * float(f.abs().max())
     plan.close()
+
+
+@pytest.mark.parametrize("N", [1, 2, 4, 5])
+def test_alpha_gamma_prime_factor_4095(N):
+    """Row a8 for real signals on the grid of L_j = 2048 (4095 = 9 x 5 x 7 x 13 alpha samples): the prime-factor kernels of
+    pfa4095_kernels.cu with no row n > 0 (N = 1), without a row n = 0 (even N), with parked rows (N = 4, 5); N = 3 is
+    test_config4_fused_top_scales_against_the_oracle.  Sampled rings (both rings of a pair, the last pair) of the top scale
+    against the oracle; synthesis through the round trip."""
+    torch, api = _api()
+    L, lam, J0 = 2048, 2.0, 10
+    flm = inputs.flm_real(L, 1400 + N, 1)
+    plan = api.s2wav_plan_create(L, N, lam, J0, True, True, 1)
+    f = plan.harmonic_inverse(torch.from_numpy(flm).cuda())
+    w = plan.forward(f)
+    picks = [(plan.J, [0, 1, 1026, 1027, 2046, 2047])]
+    _check_sampled_rings(plan, w, flm[0], 0, L, N, lam, J0, True, picks)
+    back = plan.inverse(w)
+    assert float((back - f).abs().max()) < RT_TOL * float(f.abs().max())
+    plan.close()
