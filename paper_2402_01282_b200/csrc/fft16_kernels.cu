@@ -512,6 +512,117 @@ __global__ void __launch_bounds__(256, 2) reweight16_kernel(const cplx *__restri
     }
 }
 
+// a2 at Toeplitz length 4096 (the grid of L_j = 2048, BASELINE config 4): one column per block; its two sequences
+// u1 = a x and u2 = delta a x go through the one 4096-element buffer one after the other (y1 waits in registers), the
+// thread keeps the ring values x_t, t = tid + 256 c (c < 8), in registers throughout.  Same algebra and tables as above.
+__global__ void __launch_bounds__(256, 2) reweight16w_kernel(const cplx *__restrict__ F, cplx *__restrict__ Ft, RwArgs A,
+                                                            RwTab R, int ncolumns)
+{
+    constexpr int R1 = 16, HR = 8, M = R1 * 256;
+    extern __shared__ cplx buf[];
+    __shared__ cplx s_part[8];
+    __shared__ cplx s_pole;
+    const F16Tw tw = f16_twiddles<R1>();
+    const int L = R.L, Lm = L - 1;
+    const int colid = blockIdx.x;
+    if (colid >= ncolumns) return;
+    const int mi = colid % A.Md, q = (colid / A.Md) % A.nn, b = colid / (A.Md * A.nn);
+    const int m = A.isReal ? mi : mi - (L - 1);
+    const int par = ((m + A.n_val[q]) & 1) ? 1 : 0;  // 0: sigma = +1, 1: sigma = -1
+    const cplx *col = F + ((size_t)b * A.nrows + A.n_row[q]) * (size_t)L * A.Md + mi;
+    cplx *colT = Ft + (((size_t)b * A.nrows + A.n_row[q]) * A.Md + mi) * (size_t)L;
+    const double *rp = R.rpole + par * L, *vp = R.vpole + par * L;
+    cplx xs[HR], x[1][R1];
+    cplx *sy1 = buf + F16_BUF + threadIdx.x;  // y1 of the first sequence waits here (own slots: element tid + 256 c)
+    cplx dot = cmake(0.0, 0.0);
+#pragma unroll
+    for (int c = 0; c < HR; ++c) {
+        const int t = threadIdx.x + 256 * c;
+        cplx xv = cmake(0.0, 0.0);
+        if (t < L) {
+            xv = col[(size_t)t * A.Md];
+            const double r = rp[t];
+            dot.x = fma(r, xv.x, dot.x);
+            dot.y = fma(r, xv.y, dot.y);
+        }
+        xs[c] = xv;
+        if (t == Lm) s_pole = xv;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        dot.x += __shfl_xor_sync(0xffffffffu, dot.x, o);
+        dot.y += __shfl_xor_sync(0xffffffffu, dot.y, o);
+    }
+    if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = dot;
+#pragma unroll 1
+    for (int sq = 0; sq < 2; ++sq) {
+#pragma unroll
+        for (int c = 0; c < HR; ++c) {
+            const int t = threadIdx.x + 256 * c;
+            cplx u = cmake(0.0, 0.0);
+            if (t < Lm) {
+                u = (t & 1) ? cscale(xs[c], -1.0) : xs[c];
+                if (sq) u = cscale(u, R.delta[t]);
+            }
+            x[0][c] = u;
+        }
+        f16_pass1_fwd<R1, true>(buf, 0, x[0], tw);
+        __syncthreads();
+        f16_pass2_fwd(buf, tw);
+        __syncwarp();
+        f16_pass3_fwd(buf);
+        __syncthreads();
+        {
+            const int j1 = threadIdx.x >> 4, j2 = threadIdx.x & 15;
+            const int j1p = (R1 - j1) % R1, j2p = j1 ? 15 - j2 : (16 - j2) & 15;
+            const bool shifted = j1 == 0 && j2 == 0;                    // partner of j3 is (16 - j3) % 16, else 15 - j3
+            cplx *own = buf + F16_PAD(j1 * 256 + j2 * 16);
+            const cplx *prt = buf + F16_PAD(j1p * 256 + j2p * 16);
+            const cplx *tg = R.TG16 + (j1 * 256 + j2);                   // [2][M2] in the storage order F16_TPOS
+            double sg = par ? -1.0 : 1.0;
+            if (!sq) sg = -sg;                                          // u1: T - sigma H, u2: T + sigma H
+            cplx v[16];
+#pragma unroll
+            for (int j3 = 0; j3 < 16; ++j3) {
+                const cplx u = own[j3], un = prt[shifted ? (16 - j3) & 15 : 15 - j3];
+                const cplx th = __ldg(&tg[16 * j3]), gh = cscale(__ldg(&tg[M + 16 * j3]), sg);
+                v[j3] = cadd(cmul(th, u), cmul(gh, un));
+            }
+            __syncthreads();                                            // every partner value has been read
+            bfly16<true>(v);
+#pragma unroll
+            for (int j3 = 0; j3 < 16; ++j3) own[j3] = v[j3];
+        }
+        __syncwarp();
+        f16_pass2_inv(buf, tw);
+        __syncthreads();
+        f16_pass1_inv<R1, true>(buf, 0, x[0], tw);
+        if (!sq) {
+#pragma unroll
+            for (int c = 0; c < HR; ++c) sy1[256 * c] = x[0][c];
+            __syncthreads();                                            // buf is refilled by the second sequence
+        }
+    }
+    const cplx xpole = s_pole;
+#pragma unroll
+    for (int c = 0; c < HR; ++c) {
+        const int t = threadIdx.x + 256 * c;
+        if (t < Lm) {
+            const cplx y2 = x[0][c], y1 = sy1[256 * c];
+            const double dl = R.delta[t], ds = R.dsum[t], vv = vp[t];
+            cplx h = cmake(fma(dl, y1.x, -y2.x), fma(dl, y1.y, -y2.y));
+            if (t & 1) h = cscale(h, -1.0);
+            h.x += fma(ds, xs[c].x, vv * xpole.x);
+            h.y += fma(ds, xs[c].y, vv * xpole.y);
+            colT[t] = h;
+        } else if (t == Lm) {
+            cplx acc = cmake(0.0, 0.0);
+            for (int w = 0; w < 8; ++w) acc = cadd(acc, s_part[w]);
+            colT[t] = acc;
+        }
+    }
+}
+
 // a2 at Toeplitz length 256 (grids with 65 <= L_j <= 128: the two top angular scales of BASELINE config 5, over all
 // stacked shells).  A sequence is one half-warp's 256-point problem, so nothing crosses a warp: warp = column, its two
 // half-warps carry u1 = a x and u2 = delta a x; lane l holds the ring values x_t, t = l + 16 k (k < 8), feeds the
@@ -1071,6 +1182,14 @@ static int reweight16_t(const cplx *F, cplx *Ft, const RwArgs &A, int batch, con
 int launch_reweight16(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st)
 {
     switch (R.fft.M) {
+    case 4096: {
+        const int ncol = A.Md * A.nn * batch;
+        const size_t sm = (size_t)(F16_BUF + 2048) * sizeof(cplx);
+        int rc = set_smem(reweight16w_kernel, sm);
+        if (rc) return rc;
+        S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight16w_kernel, ncol, 256, sm, st, F, Ft, A, R, ncol);
+        return S2W_OK;
+    }
     case 2048: return reweight16_t<8>(F, Ft, A, batch, R, st);
     case 1024: return reweight16_t<4>(F, Ft, A, batch, R, st);
     case 512: return reweight16_t<2>(F, Ft, A, batch, R, st);

@@ -522,7 +522,7 @@ int build_rw(s2w_plan *p, GridTab &g)
     g.rw.vpole = dv;
     g.rw.rpole = dr;
     g.rw.L = L;
-    if (M2 == 2048 || M2 == 1024 || M2 == 512 || M2 == 256) {
+    if (M2 == 4096 || M2 == 2048 || M2 == 1024 || M2 == 512 || M2 == 256) {
         // the same two spectra in the order of the radix-16 core (fft16_core.cuh), which is read off the transform of e_1
         std::vector<cplx> h16((size_t)3 * M2, cmake(0.0, 0.0));
         for (int i = 0; i < M2; ++i) {

@@ -1685,7 +1685,7 @@ int launch_transpose(const cplx *src, cplx *dst, int R, int C, int nb, cudaStrea
 int launch_reweight_th(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const RwTab &R, cudaStream_t st)
 {
     if (A.nn <= 0) return S2W_OK;
-    if (R.TG16 && R.fft.M >= 256 && R.fft.M <= 2048 && use_fft16()) return launch_reweight16(F, Ft, A, batch, R, st);
+    if (R.TG16 && R.fft.M >= 256 && R.fft.M <= 4096 && use_fft16()) return launch_reweight16(F, Ft, A, batch, R, st);
     const int ncol = A.Md * A.nn * batch;
     const int cpb = seqs_per_block(2048 / R.fft.M, ncol, RW_MAXCPB);
     size_t sm = 2 * (size_t)cpb * fft_padded_len(R.fft.M) * sizeof(cplx);
