@@ -123,6 +123,9 @@ bool so3_pfa4095_supported(const So3Args &A, const FftTab &T);
 int launch_so3_pfa4095(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
                        cudaStream_t st);
 
+bool ring_pfa4095_supported(bool real, const FftTab &T);             // a1, real signals, the same grid
+int launch_ring_pfa4095(bool fwd, const void *in, void *out, int nrows, size_t sig_stride, const FftTab &T, cudaStream_t st);
+
 // plan-time: group start degrees and seeds from the range-extended values d^{l0}_{mn}(beta_t) = mant 2^expo ([ntab][Lg m][Lg t])
 int launch_wigner_seeds(const double *mant, const int *expo, const double *coef, size_t tri, int Lfull, int Lg, int nt, int G,
                         const int *n_vals, int ntab, const double *yv, const int *ring, int *gstart, double2 *dseed,
