@@ -123,7 +123,9 @@ bool so3_pfa4095_supported(const So3Args &A, const FftTab &T);
 int launch_so3_pfa4095(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
                        cudaStream_t st);
 
-bool ring_pfa4095_supported(bool real, const FftTab &T);             // a1, real signals, the same grid
+bool ring_pfa255_supported(bool real, const FftTab &T);              // a1, complex signals, the 255-sample grid
+int launch_ring_pfa255(bool fwd, const void *in, void *out, int nrows, size_t sig_stride, const FftTab &T, cudaStream_t st);
+bool ring_pfa4095_supported(bool real, const FftTab &T);             // a1, real signals, the 4095-sample grid
 int launch_ring_pfa4095(bool fwd, const void *in, void *out, int nrows, size_t sig_stride, const FftTab &T, cudaStream_t st);
 
 // plan-time: group start degrees and seeds from the range-extended values d^{l0}_{mn}(beta_t) = mant 2^expo ([ntab][Lg m][Lg t])

@@ -217,6 +217,57 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_pfa255_kernel(const cplx *__re
     }
 }
 
+// a1 ring FFTs (Eqs. 2-3) of complex signals on the 255-sample grids (the ball's shells): 15 rings per block;
+// layouts and normalisation as ring_fwd16_kernel / ring_inv16_kernel (fft16_kernels.cu): pixel rows [batch][L][n], row r of
+// the spectrum array holds F_m at [m + L-1]
+__global__ void __launch_bounds__(256, 3) ring_fwd_pfa255_kernel(const cplx *__restrict__ in, cplx *__restrict__ out, int nrows,
+                                                                size_t sig_stride, int L)
+{
+    extern __shared__ cplx buf[];
+    const int n = PFA_N, tid = threadIdx.x;
+    const double inv_n = 1.0 / (double)n;
+    if (tid < n) {
+#pragma unroll
+        for (int q = 0; q < PFA_SEQS; ++q) {
+            const int r = blockIdx.x * PFA_SEQS + q;
+            buf[q * PFA_STRIDE + tid] =
+                r < nrows ? in[(size_t)(r / L) * sig_stride + (size_t)(r % L) * n + tid] : cmake(0.0, 0.0);
+        }
+    }
+    pfa_round<false>(buf);
+    if (tid < n) {
+        const int mo = (L - 1) + (tid < L ? tid : tid - n);
+#pragma unroll
+        for (int q = 0; q < PFA_SEQS; ++q) {
+            const int r = blockIdx.x * PFA_SEQS + q;
+            if (r < nrows) out[(size_t)r * n + mo] = cscale(buf[q * PFA_STRIDE + tid], inv_n);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256, 3) ring_inv_pfa255_kernel(const cplx *__restrict__ in, cplx *__restrict__ out, int nrows,
+                                                                size_t sig_stride, int L)
+{
+    extern __shared__ cplx buf[];
+    const int n = PFA_N, tid = threadIdx.x;
+    if (tid < n) {
+        const int mo = (L - 1) + (tid < L ? tid : tid - n);
+#pragma unroll
+        for (int q = 0; q < PFA_SEQS; ++q) {
+            const int r = blockIdx.x * PFA_SEQS + q;
+            buf[q * PFA_STRIDE + tid] = r < nrows ? in[(size_t)r * n + mo] : cmake(0.0, 0.0);
+        }
+    }
+    pfa_round<true>(buf);
+    if (tid < n) {
+#pragma unroll
+        for (int q = 0; q < PFA_SEQS; ++q) {
+            const int r = blockIdx.x * PFA_SEQS + q;
+            if (r < nrows) out[(size_t)(r / L) * sig_stride + (size_t)(r % L) * n + tid] = buf[q * PFA_STRIDE + tid];
+        }
+    }
+}
+
 template <int NN>
 int so3_pfa255_t(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch, int L, cudaStream_t st)
 {
@@ -252,6 +303,33 @@ bool so3_pfa255_supported(const So3Args &A, const FftTab &T)
         return !(e && e[0] == '0');
     }();
     return on && T.n == PFA_N && T.L == 128 && T.nt == T.L && A.nn >= 1 && A.nn <= 3 && 2 * A.N - 1 <= 64;
+}
+
+bool ring_pfa255_supported(bool real, const FftTab &T)
+{
+    static const bool on = [] {
+        const char *e = getenv("S2W_PFA");
+        return !(e && e[0] == '0');
+    }();
+    return on && !real && T.n == PFA_N && T.L == 128 && T.nt == T.L;
+}
+
+// complex signals, nrows = batch x L rings of 255 samples; the caller checks ring_pfa255_supported
+int launch_ring_pfa255(bool fwd, const void *in, void *out, int nrows, size_t sig_stride, const FftTab &T, cudaStream_t st)
+{
+    const size_t sm = (size_t)PFA_SEQS * PFA_STRIDE * sizeof(cplx);
+    const int grid = (nrows + PFA_SEQS - 1) / PFA_SEQS;
+    int rc;
+    if (fwd) {
+        if ((rc = set_smem(ring_fwd_pfa255_kernel, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_RING_FFT, ring_fwd_pfa255_kernel, grid, 256, sm, st, (const cplx *)in, (cplx *)out, nrows, sig_stride,
+                     T.L);
+    } else {
+        if ((rc = set_smem(ring_inv_pfa255_kernel, sm))) return rc;
+        S2W_LAUNCH_C(S2W_K_RING_FFT, ring_inv_pfa255_kernel, grid, 256, sm, st, (const cplx *)in, (cplx *)out, nrows, sig_stride,
+                     T.L);
+    }
+    return S2W_OK;
 }
 
 // complex signals on the McEwen-Wiaux grid of L_j = 128; the caller checks so3_pfa255_supported

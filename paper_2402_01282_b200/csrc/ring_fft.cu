@@ -1551,6 +1551,7 @@ int launch_ring_fwd(bool real, const void *in, cplx *out, int B, int Lg, size_t 
     (void)Lg;
     if (nrows <= 0) return S2W_OK;
     if (ring_pfa4095_supported(real, T)) return launch_ring_pfa4095(true, in, out, nrows, sig_stride, T, st);
+    if (ring_pfa255_supported(real, T)) return launch_ring_pfa255(true, in, out, nrows, sig_stride, T, st);
     if (T.nt == T.L && T.bhat16_m && f16_supported(T.M) && use_fft16())
         return launch_ring16(true, real, in, out, nrows, sig_stride, T, st);
     size_t sm = fft_smem_bytes(T);
@@ -1572,6 +1573,7 @@ int launch_ring_inv(bool real, const cplx *in, void *out, int B, int Lg, size_t 
     (void)Lg;
     if (nrows <= 0) return S2W_OK;
     if (ring_pfa4095_supported(real, T)) return launch_ring_pfa4095(false, in, out, nrows, sig_stride, T, st);
+    if (ring_pfa255_supported(real, T)) return launch_ring_pfa255(false, in, out, nrows, sig_stride, T, st);
     if (T.nt == T.L && T.bhat16_m && f16_supported(T.M) && use_fft16())
         return launch_ring16(false, real, in, out, nrows, sig_stride, T, st);
     size_t sm = fft_smem_bytes(T);
