@@ -34,11 +34,13 @@ def _spin_flm(L, seed, spin):
 
 @pytest.mark.parametrize("L,N,lam,J0,mr,spin", [(8, 2, 2.0, 0, True, 2), (16, 3, 2.0, 1, True, -1), (20, 4, 2.0, 0, False, 1),
                                                 (12, 3, 2.0, 0, True, 3), (33, 5, 2.0, 2, True, -2)])
-def test_spin_transforms_match_oracle(L, N, lam, J0, mr, spin):
+@pytest.mark.parametrize("pre", [False, True])
+def test_spin_transforms_match_oracle(L, N, lam, J0, mr, spin, pre):
+    """pre: S2W_PRECOMPUTE -- the table kernels, with the theta quadrature folded into the table of the rows n = -s, +s."""
     torch, api = _api()
     flm = _spin_flm(L, 60 + L, spin)
     f = np.ascontiguousarray(S.sht_inverse(flm, L, "f80", spin=spin).astype(np.complex128))
-    plan = api.s2wav_plan_create(L, N, lam, J0, mr, False, 1, spin=spin)
+    plan = api.s2wav_plan_create(L, N, lam, J0, mr, False, 1, spin=spin, flags=api.S2W_PRECOMPUTE if pre else 0)
     fd = torch.from_numpy(f).cuda().reshape(1, -1)
     got = plan.harmonic_forward(fd, L * (2 * L - 1)).cpu().numpy().reshape(L, 2 * L - 1)
     assert _relmax(got, flm) < FWD_TOL
