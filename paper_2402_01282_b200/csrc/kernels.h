@@ -23,6 +23,8 @@ struct So3Args {
     int n_rowm[S2W_MAX_ROWS];    // row index of -n in F
     const size_t *sig_off;       // device array [batch]: element offset of signal b's coefficient block, or null:
                                  // b * sig_stride (the ball's stacked shells of all radial scales j' are not equidistant)
+    int f_transposed;            // synthesis side only, where so3_fwd_writes_transposed() says so: F is written as
+                                 // [b][row][m][t] (the forward contraction's input layout) instead of [b][row][t][m]
 };
 // element offset of signal b's block in the pixel-side array
 __host__ __device__ inline size_t so3_base(const So3Args &A, int b, size_t sig_stride)
@@ -92,6 +94,9 @@ int launch_ring_inv(bool real, const cplx *in, void *out, int B, int Lg, size_t 
                     cudaStream_t st);
 int launch_so3_inv(bool real, const cplx *F, void *W, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
                    cudaStream_t st);
+// whether launch_so3_fwd honours So3Args::f_transposed for these arguments (only the prime-factor kernels of the 255-sample
+// grids do: the quadrature-folded table path of small grids then needs no transposing copy at all)
+bool so3_fwd_writes_transposed(bool real, const So3Args &A, const FftTab &T);
 int launch_so3_fwd(bool real, const void *W, size_t sig_stride, cplx *F, const So3Args &A, int batch, const FftTab &T,
                    cudaStream_t st);
 // a2: reads F[b][row][t][mi], writes the reweighted columns TRANSPOSED, Ft[b][row][mi][t] (what the forward Wigner

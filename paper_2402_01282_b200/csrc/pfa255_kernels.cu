@@ -211,8 +211,13 @@ __global__ void __launch_bounds__(256, 3) so3_fwd_pfa255_kernel(const cplx *__re
             const int t = blockIdx.x * RB + r;
             if (t >= L) continue;
 #pragma unroll
-            for (int i = 0; i < NN; ++i)
-                Fb[((size_t)A.n_row[i] * L + t) * n + mo] = buf[(r * NN + i) * PFA_STRIDE + tid];
+            for (int i = 0; i < NN; ++i) {
+                const cplx v = buf[(r * NN + i) * PFA_STRIDE + tid];
+                if (A.f_transposed)
+                    Fb[((size_t)A.n_row[i] * n + mo) * L + t] = v;   // [row][m][t]: runs of RB rings per (row, m)
+                else
+                    Fb[((size_t)A.n_row[i] * L + t) * n + mo] = v;
+            }
         }
     }
 }

@@ -772,6 +772,7 @@ void fill_wig_args(const s2w_plan *p, const Stage &st, bool synthesis, int B, cp
 
 void fill_so3_args(const s2w_plan *p, const Stage &st, So3Args &A)
 {
+    A.f_transposed = 0;
     A.sig_off = 0;
     A.N = p->N;
     A.nn = st.nn;
@@ -1148,8 +1149,13 @@ static int scale_synthesis(const s2w_plan *p, const Scale &sc, int B, const Work
     So3Args S;
     fill_so3_args(p, sc.st, S);
     S.sig_off = sig_off;
-    if ((rc = launch_so3_fwd(p->real, src, sig_stride, w.F, S, B, g.fft, s))) return rc;
-    if ((rc = stage_reweight(p, sc.st, w.F, w.Ft, B, s, use_folded(p, sc.st, 0)))) return rc;
+    if (use_folded(p, sc.st, 0) && so3_fwd_writes_transposed(p->real, S, g.fft)) {
+        S.f_transposed = 1;  // folded quadrature: a2 would be a transposing copy; the (alpha, gamma) kernel writes Ft itself
+        if ((rc = launch_so3_fwd(p->real, src, sig_stride, w.Ft, S, B, g.fft, s))) return rc;
+    } else {
+        if ((rc = launch_so3_fwd(p->real, src, sig_stride, w.F, S, B, g.fft, s))) return rc;
+        if ((rc = stage_reweight(p, sc.st, w.F, w.Ft, B, s, use_folded(p, sc.st, 0)))) return rc;
+    }
     WigArgs A;
     fill_wig_args(p, sc.st, true, B, w.flmT, w.Ft, A);
     use_folded(p, sc.st, &A);

@@ -1650,9 +1650,18 @@ int launch_so3_inv(bool real, const cplx *F, void *W, size_t sig_stride, const S
     return so3_launch(false, real, F, W, sig_stride, A, batch, T, st);
 }
 
+bool so3_fwd_writes_transposed(bool real, const So3Args &A, const FftTab &T)
+{
+    return T.nt == T.L && !real && so3_pfa255_supported(A, T);  // the first branch of so3_launch
+}
+
 int launch_so3_fwd(bool real, const void *W, size_t sig_stride, cplx *F, const So3Args &A, int batch, const FftTab &T,
                    cudaStream_t st)
 {
+    if (A.f_transposed && !so3_fwd_writes_transposed(real, A, T)) {
+        set_error("launch_so3_fwd: transposed output is not available for this grid");
+        return S2W_EINVAL;
+    }
     return so3_launch(true, real, W, F, sig_stride, A, batch, T, st);
 }
 
