@@ -826,13 +826,19 @@ __global__ void wigner_table_scatter_kernel(const cplx *__restrict__ Y, double *
 
 // inverse direction from the table: D[ring][col] += A[ring][l] B[l][col], A-fragments (8 rings x 4 degrees) gathered
 // from the table, B = filter x f_lm from shared memory, accumulators 8 rings x 8 columns per ring octet.
-template <int R, int MAXT>
+// NCH > 1 (small grids with many columns: the stacked shells of a ball plan): a block owns NCH chunks of 4 complex columns,
+// so that one gathered A-fragment (an 8-byte load per lane over four 64-byte runs of the table; knocking these loads out
+// took 0.6 of the 2.0 ms of the class at C5) feeds NCH DMMAs.  Rows of s_X are NCB + 4 doubles apart: the B-fragment reads
+// (degree lane % 4, column lane / 4) of a half-warp then fall into 16 different banks.
+template <int R, int MAXT, int NCH = 1>
 __global__ void __launch_bounds__(MAXT) precomp_inverse_kernel(WigArgs A)
 {
     constexpr int NC = 8;
-    __shared__ double s_X[WIG_TL * NC];
+    constexpr int NCB = NC * NCH;                 // real columns of the block
+    constexpr int XS = NCB + 4;                   // row stride of s_X
+    __shared__ double s_X[WIG_TL * XS];
 
-    const int m = blockIdx.x, chunk = blockIdx.y;
+    const int m = blockIdx.x, chunk = blockIdx.y * NCH;
     const int Lg = A.Lg, Lfull = A.Lfull, G = A.G;
     const int Md = A.isReal ? Lg : 2 * Lg - 1;
     const int Mfull = A.isReal ? Lfull : 2 * Lfull - 1;
@@ -851,13 +857,15 @@ __global__ void __launch_bounds__(MAXT) precomp_inverse_kernel(WigArgs A)
         const double *tbase = A.dtab + ((size_t)tab * A.tri_g + tri_off(m, Lg)) * (size_t)(32 * G);
 
         int gs[R];
-        double acc[R][4][2];
+        double acc[R][NCH][4][2];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int g = r * W + warp;
             gs[r] = g < G ? gsrow[g] : INT_MAX;
 #pragma unroll
-            for (int o = 0; o < 4; ++o) acc[r][o][0] = acc[r][o][1] = 0.0;
+            for (int ch = 0; ch < NCH; ++ch)
+#pragma unroll
+                for (int o = 0; o < 4; ++o) acc[r][ch][o][0] = acc[r][ch][o][1] = 0.0;
         }
         int first = gsrow[0];
         if (G > 1 && gsrow[1] < first) first = gsrow[1];
@@ -865,7 +873,7 @@ __global__ void __launch_bounds__(MAXT) precomp_inverse_kernel(WigArgs A)
 
         for (int lt = first & ~(WIG_TL - 1); lt < Lg; lt += WIG_TL) {
             __syncthreads();
-            for (int i = threadIdx.x; i < WIG_TL * (NC / 2); i += T) {
+            for (int i = threadIdx.x; i < WIG_TL * (NCB / 2); i += T) {
                 const int k = i / WIG_TL, ll = i % WIG_TL;
                 const int l = lt + ll;
                 const ColInfo ci = col_info(A, chunk * (NC / 2) + k);
@@ -877,15 +885,17 @@ __global__ void __launch_bounds__(MAXT) precomp_inverse_kernel(WigArgs A)
                     X = cmul(Gf, f);
                     if (ci.minus) X = cscale(X, sgn);
                 }
-                s_X[ll * NC + 2 * k] = X.x;
-                s_X[ll * NC + 2 * k + 1] = X.y;
+                s_X[ll * XS + 2 * k] = X.x;
+                s_X[ll * XS + 2 * k + 1] = X.y;
             }
             __syncthreads();
 #pragma unroll 2
             for (int lq = 0; lq < WIG_TL; lq += 4) {
                 const int lo = lt + lq;
                 if (lo + 4 <= lacc || lo >= Lg || gs[0] >= lo + 4) continue;
-                const double bv = s_X[(lq + fk) * NC + fr];
+                double bv[NCH];
+#pragma unroll
+                for (int ch = 0; ch < NCH; ++ch) bv[ch] = s_X[(lq + fk) * XS + ch * NC + fr];
                 const int lrow = lo + fk;
                 const bool ok = lrow >= l0 && lrow < Lg;
                 const double *trow = tbase + (size_t)(ok ? lrow : l0) * (32 * G) + fr;
@@ -897,25 +907,30 @@ __global__ void __launch_bounds__(MAXT) precomp_inverse_kernel(WigArgs A)
 #pragma unroll
                     for (int o = 0; o < 4; ++o) av[o] = ok ? __ldg(src + 8 * o) : 0.0;
 #pragma unroll
-                    for (int o = 0; o < 4; ++o) dmma884(acc[r][o][0], acc[r][o][1], av[o], bv);
+                    for (int ch = 0; ch < NCH; ++ch)
+#pragma unroll
+                        for (int o = 0; o < 4; ++o) dmma884(acc[r][ch][o][0], acc[r][ch][o][1], av[o], bv[ch]);
                 }
             }
         }
 
         // D fragment: ring lane / 4 of the octet, real columns 2 (lane % 4) + {0, 1} = complex column lane % 4
-        const ColInfo ci = col_info(A, chunk * (NC / 2) + fk);
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const int g = r * W + warp;
-            if (g >= G || !ci.valid) continue;
-            if (ci.minus && m == 0) continue;
-            const int row = ci.minus ? A.n_rowm[q] : A.n_row[q];
-            const int mi = A.isReal ? m : (ci.minus ? Lg - 1 - m : Lg - 1 + m);
+        for (int ch = 0; ch < NCH; ++ch) {
+            const ColInfo ci = col_info(A, (chunk + ch) * (NC / 2) + fk);
 #pragma unroll
-            for (int o = 0; o < 4; ++o) {
-                const int t = A.ring[g * 32 + o * 8 + fr];
-                if (t < 0) continue;
-                A.F[(((size_t)ci.b * A.nrows + row) * A.nt + t) * Md + mi] = cmake(acc[r][o][0], acc[r][o][1]);
+            for (int r = 0; r < R; ++r) {
+                const int g = r * W + warp;
+                if (g >= G || !ci.valid) continue;
+                if (ci.minus && m == 0) continue;
+                const int row = ci.minus ? A.n_rowm[q] : A.n_row[q];
+                const int mi = A.isReal ? m : (ci.minus ? Lg - 1 - m : Lg - 1 + m);
+#pragma unroll
+                for (int o = 0; o < 4; ++o) {
+                    const int t = A.ring[g * 32 + o * 8 + fr];
+                    if (t < 0) continue;
+                    A.F[(((size_t)ci.b * A.nrows + row) * A.nt + t) * Md + mi] = cmake(acc[r][ch][o][0], acc[r][ch][o][1]);
+                }
             }
         }
     }
@@ -1372,6 +1387,20 @@ int dispatch_inv_pre(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t
         S2W_WIG_CASE(3, 512)
         S2W_WIG_CASE(4, 512)
 #undef S2W_WIG_CASE
+    }
+    static const int pre_nch = [] {
+        const char *e = getenv("S2W_PRE_NCH");
+        return e ? atoi(e) : 2;
+    }();
+    if (c.R == 1 && chunks >= 8 && pre_nch > 1) {  // one ring group per warp, many columns: several chunks per block
+        if (pre_nch == 2) {
+            dim3 grid(A.Lg, (chunks + 1) / 2);
+            S2W_LAUNCH_C(S2W_K_WIGNER_INV, (precomp_inverse_kernel<1, 256, 2>), grid, 32 * c.W, 0, st, A);
+        } else {
+            dim3 grid(A.Lg, (chunks + 3) / 4);
+            S2W_LAUNCH_C(S2W_K_WIGNER_INV, (precomp_inverse_kernel<1, 256, 4>), grid, 32 * c.W, 0, st, A);
+        }
+        return S2W_OK;
     }
 #define S2W_WIG_CASE(RR, MT)                                                                                  \
     if (c.R == RR && c.MAXT == MT) {                                                                          \
