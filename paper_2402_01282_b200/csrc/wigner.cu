@@ -987,7 +987,8 @@ template <int R, int MAXT, int STAGES>
 __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) precomp_inverse_tma_kernel(WigArgs A)
 {
     constexpr int NC = 8;
-    __shared__ double s_X[WIG_TL * NC];
+    constexpr int XS = NC + 4;  // row stride of s_X: conflict-free B-fragment reads (see precomp_inverse_kernel)
+    __shared__ double s_X[WIG_TL * XS];
     extern __shared__ __align__(16) double s_dyn[];   // [W][STAGES][4 degrees][32 R + 4] then the mbarriers [W][STAGES]
 
     const int m = blockIdx.x, chunk = blockIdx.y;
@@ -1092,8 +1093,8 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) precomp_inverse_t
                     X = cmul(Gf, f);
                     if (ci.minus) X = cscale(X, sgn);
                 }
-                s_X[ll * NC + 2 * k] = X.x;
-                s_X[ll * NC + 2 * k + 1] = X.y;
+                s_X[ll * XS + 2 * k] = X.x;
+                s_X[ll * XS + 2 * k + 1] = X.y;
             }
             __syncthreads();
             for (int lq = 0; lq < WIG_TL; lq += 4) {
@@ -1111,7 +1112,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) precomp_inverse_t
                 mbar_wait(&bars[sgi], (it_cons / STAGES) & 1);
                 ++it_cons;
                 const double *src = wst + (size_t)sgi * PreStage<R>::doubles + fk * PreStage<R>::row + fr;
-                const double bv = s_X[(lq + fk) * NC + fr];
+                const double bv = s_X[(lq + fk) * XS + fr];
                 const int lrow = lo + fk;
                 const bool ok = lrow >= l0 && lrow < Lg;
 #pragma unroll
