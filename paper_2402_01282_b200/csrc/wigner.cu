@@ -486,10 +486,14 @@ __device__ __forceinline__ double fwd_octet_reduce(const double *P, int lane)
     return v;
 }
 
-template <int R, int MAXT, bool PRE, bool FUSE, int CF = 0>
+// NCH = 2 (table kernel on grids with one ring group per warp and many columns: the stacked shells of a ball plan): a
+// block owns two chunks of 4 complex columns, so that one gathered B-fragment of the table feeds two DMMAs (the gathers,
+// eight 32-byte runs per 8-byte load instruction, are what the L1 pipe of these launches is busy with)
+template <int R, int MAXT, bool PRE, bool FUSE, int CF = 0, int NCH = 1>
 __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_kernel(WigArgs A)
 {
     static_assert(CF == 0 || (!PRE && (CF == 2 || CF == 4)), "CF: 0 (tensor pipe), 2 or 4 real columns (FP64 pipe)");
+    static_assert(NCH == 1 || (NCH == 2 && PRE && !FUSE && CF == 0), "NCH = 2: table kernel only");
     constexpr int NC = 8;
     constexpr int TLF = FWD_TILE(R);
     __shared__ double2 s_ag[TLF];
@@ -499,9 +503,10 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
     // different bank pairs (with rows of 8 the four degree pairs shared one: 4-way conflicts on the load and the CAS)
 #define SRED(ll, c) ((((ll) >> 1) * 20) + (((ll) & 1) * 8) + (c))
     __shared__ double s_red[(TLF / 2) * 20];
+    __shared__ double s_red2[NCH == 2 ? (TLF / 2) * 20 : 1];  // the second chunk's sums
     extern __shared__ double s_dt[];   // the B-fragment tiles [W][R][FWD_GT]
 
-    const int m = blockIdx.x, chunk = blockIdx.y;
+    const int m = blockIdx.x, chunk = blockIdx.y * NCH;
     const int Lg = A.Lg, Lfull = A.Lfull, G = A.G;
     const int Md = A.isReal ? Lg : 2 * Lg - 1;
     const int Mfull = A.isReal ? Lfull : 2 * Lfull - 1;
@@ -530,6 +535,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
     // recursion (same grid, same rows n): rows 0..3 = columns of scale A (A.F, A.filt), rows 4..7 = scale B (A.F2, A.filt2)
     constexpr bool fuse = FUSE;
     const ColInfo fci = col_info(A, fuse ? ((fc & 3) >> 1) : chunk * (NC / 2) + (fc >> 1));
+    const ColInfo fci2 = col_info(A, (chunk + 1) * (NC / 2) + (fc >> 1));  // NCH = 2
     const cplx *Fsrc = (fuse && fc >= 4) ? A.F2 : A.F;
 
     for (int q = 0; q < A.nn; ++q) {
@@ -546,6 +552,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
         // ring data as A-fragments: hA[r][quad] = h[ring (r, quad, fk)][column fc]
         int gs[R];
         double d[R], u[R], hA[R][8], h[R][CF > 0 ? CF : 1];  // hA: tensor-pipe path, h: CF > 0
+        double hA2[R][NCH == 2 ? 8 : 1];                     // second chunk (NCH = 2)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int g = FWD_GRP(r);
@@ -588,6 +595,19 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                 const double v = hcol[2 * (size_t)(ok ? tq[qd] : 0)];
                 hA[r][qd] = ok ? v * keep : 0.0;
             }
+            if constexpr (NCH == 2) {
+                const int row2 = fci2.minus ? A.n_rowm[q] : A.n_row[q];
+                const int mi2 = A.isReal ? m : (fci2.minus ? Lg - 1 - m : Lg - 1 + m);
+                const double *hcol2 = reinterpret_cast<const double *>(
+                                          A.F + (((size_t)(fci2.valid ? fci2.b : 0) * A.nrows + row2) * Md + mi2) * A.nt) + (fc & 1);
+                const double keep2 = fci2.valid ? (fci2.minus ? sgn : 1.0) : 0.0;
+#pragma unroll
+                for (int qd = 0; qd < 8; ++qd) {
+                    const bool ok = g < G && tq[qd] >= 0;
+                    const double v = hcol2[2 * (size_t)(ok ? tq[qd] : 0)];
+                    hA2[r][qd] = ok ? v * keep2 : 0.0;
+                }
+            }
         }
         // tiles start at the first group start; tiles wholly below the filter support run the recursion only
         int first = gsrow[0];
@@ -596,7 +616,10 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
 
         for (int lt = first & ~(TLF - 1); lt < Lg; lt += TLF) {
             __syncthreads();
-            for (int i = threadIdx.x; i < (TLF / 2) * 20; i += T) s_red[i] = 0.0;
+            for (int i = threadIdx.x; i < (TLF / 2) * 20; i += T) {
+                s_red[i] = 0.0;
+                if (NCH == 2) s_red2[i] = 0.0;
+            }
             if (!PRE) stage_coef<TLF>(crow, lt, l0, Lg, s_ag, s_e);
             __syncthreads();
             const bool want = lt + TLF > lacc;  // this tile has outputs
@@ -605,6 +628,7 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
             for (int oc = 0; oc < TLF / 8; ++oc) {
                 const int lo = lt + 8 * oc;
                 double c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
+                double e0 = 0.0, e1 = 0.0, e2 = 0.0, e3 = 0.0;  // second chunk (NCH = 2)
                 bool contributed = false;
                 if (PRE) {
                     // precomputed-kernel variant (a9): B-fragments straight from the d-table in HBM
@@ -625,6 +649,10 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                             for (int qd = 0; qd < 8; qd += 2) {
                                 dmma884(c0, c1, hA[r][qd], bv[qd]);
                                 dmma884(c2, c3, hA[r][qd + 1], bv[qd + 1]);
+                                if constexpr (NCH == 2) {
+                                    dmma884(e0, e1, hA2[r][qd], bv[qd]);
+                                    dmma884(e2, e3, hA2[r][qd + 1], bv[qd + 1]);
+                                }
                             }
                         }
                     }
@@ -736,24 +764,29 @@ __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1)) wigner_forward_ke
                     const double v0 = c0 + c2, v1 = c1 + c3;
                     atomicAdd(&s_red[SRED(8 * oc + 2 * fk, fc)], v0);
                     atomicAdd(&s_red[SRED(8 * oc + 2 * fk + 1, fc)], (!PRE && hemi) ? -v1 : v1);
+                    if constexpr (NCH == 2) {
+                        atomicAdd(&s_red2[SRED(8 * oc + 2 * fk, fc)], e0 + e2);
+                        atomicAdd(&s_red2[SRED(8 * oc + 2 * fk + 1, fc)], e1 + e3);
+                    }
                 }
             }
             if (!want) continue;
             __syncthreads();
             // cross-warp sum, output filter, accumulate into f_lm
-            for (int i = threadIdx.x; i < TLF * (NC / 2); i += T) {
-                const int k = i / TLF, ll = i % TLF;
+            for (int i = threadIdx.x; i < TLF * (NC / 2) * NCH; i += T) {
+                const int ch = i / (TLF * (NC / 2)), k = (i / TLF) % (NC / 2), ll = i % TLF;
+                const double *sred = (NCH == 2 && ch) ? s_red2 : s_red;
                 const int l = lt + ll;
                 if (fuse && k >= 2) continue;  // fused: k = complex column, both scales summed below
-                const ColInfo ci = col_info(A, fuse ? k : chunk * (NC / 2) + k);
+                const ColInfo ci = col_info(A, fuse ? k : (chunk + ch) * (NC / 2) + k);
                 if (l < lacc || l >= Lg || !ci.valid) continue;
                 if (ci.minus && m == 0) continue;
                 cplx val = cmake(0.0, 0.0);
                 for (int sc = 0; sc < (fuse ? 2 : 1); ++sc) {
                     const int c0i = 2 * k + 4 * sc;
                     const int cp = FUSE ? 2 * sc : 2 * k;  // CF > 0: column pair of (scale sc | complex column k)
-                    const double re = CF > 0 ? s_red[ll * (CF > 0 ? CF : 2) + cp] : s_red[SRED(ll, c0i)];
-                    const double im = CF > 0 ? s_red[ll * (CF > 0 ? CF : 2) + cp + 1] : s_red[SRED(ll, c0i + 1)];
+                    const double re = CF > 0 ? s_red[ll * (CF > 0 ? CF : 2) + cp] : sred[SRED(ll, c0i)];
+                    const double im = CF > 0 ? s_red[ll * (CF > 0 ? CF : 2) + cp + 1] : sred[SRED(ll, c0i + 1)];
                     const cplx Gf = (sc ? A.filt2 : A.filt)[(size_t)(ci.minus ? A.n_filtm[q] : q) * Lg + l];
                     val = cadd(val, cmul(Gf, cmake(re, im)));
                 }
@@ -1258,7 +1291,7 @@ void launch_inv_t(const WigArgs &A, int T, int chunks, cudaStream_t st)
     S2W_LAUNCH_C(S2W_K_WIGNER_INV, (wigner_inverse_kernel<NC, R, MAXT, NS>), grid, T, 0, st, A);
 }
 
-template <int R, int MAXT, bool PRE, bool FUSE, int CF = 0>
+template <int R, int MAXT, bool PRE, bool FUSE, int CF = 0, int NCH = 1>
 int launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st, int gz = 1)
 {
     // per warp: R B-fragment tiles (tensor pipe) or the 8 CF x 32 partial sums of an octet (CF > 0)
@@ -1266,11 +1299,11 @@ int launch_fwd_t(const WigArgs &A, int T, int chunks, cudaStream_t st, int gz = 
     const size_t smem = PRE ? 0 : (size_t)(T / 32) * per_warp;
     // the attribute is per device and per function: query and raise it when needed (smem_attr.cuh), no per-process flag
     {
-        const int rc = set_smem(wigner_forward_kernel<R, MAXT, PRE, FUSE, CF>, (size_t)(MAXT / 32) * per_warp);
+        const int rc = set_smem(wigner_forward_kernel<R, MAXT, PRE, FUSE, CF, NCH>, (size_t)(MAXT / 32) * per_warp);
         if (rc) return rc;
     }
     dim3 grid(A.Lg, chunks, gz);
-    S2W_LAUNCH_C(S2W_K_WIGNER_FWD, (wigner_forward_kernel<R, MAXT, PRE, FUSE, CF>), grid, T, smem, st, A);
+    S2W_LAUNCH_C(S2W_K_WIGNER_FWD, (wigner_forward_kernel<R, MAXT, PRE, FUSE, CF, NCH>), grid, T, smem, st, A);
     return S2W_OK;
 }
 
@@ -1312,6 +1345,13 @@ int dispatch_fwd(const WigArgs &A, const WigCfg &c, int chunks, cudaStream_t st)
         const char *e = getenv("S2W_FWD_DFMA");
         return e ? atoi(e) : 4;
     }();
+    static const int pre_nch = [] {
+        const char *e = getenv("S2W_PRE_NCH");
+        return e ? atoi(e) : 2;
+    }();
+    // table kernel, one ring group per warp, many columns: two column chunks per block (wigner_forward_kernel, NCH)
+    if (A.dtab && c.R == 1 && chunks >= 8 && pre_nch > 1)
+        return launch_fwd_t<1, 256, true, false, 0, 2>(A, 32 * c.W, (chunks + 1) / 2, st);
     const int CT = A.isReal ? A.B : 2 * A.B;
     const int cf = (A.F2 ? 4 : 2) * CT;
     const int gz = (split_on() && c.W == 16) ? 2 : 1;
