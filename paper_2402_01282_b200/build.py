@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libs2w.so")
 SOURCES = ["plan.cu", "wigner.cu", "ring_fft.cu", "fft16_kernels.cu", "pfa255_kernels.cu", "pfa4095_kernels.cu", "radial.cu", "filters.cpp"]
-HEADERS = ["common.cuh", "fft_core.cuh", "fft16_core.cuh", "smem_attr.cuh", "pfa255_dft17.inc", "pfa4095_dft.inc", "kernels.h", "host_math.h", os.path.join("..", "..", "include", "s2w.h")]
+HEADERS = ["common.cuh", "fft_core.cuh", "fft16_core.cuh", "smem_attr.cuh", "pfa255_dft17.inc", "pfa4095_dft.inc", "pfa2047_dft.inc", "kernels.h", "host_math.h", os.path.join("..", "..", "include", "s2w.h")]
 
 
 def _stale():

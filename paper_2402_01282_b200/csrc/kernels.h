@@ -128,6 +128,9 @@ bool so3_pfa4095_supported(const So3Args &A, const FftTab &T);
 int launch_so3_pfa4095(bool fwd, const void *in, void *out, size_t sig_stride, const So3Args &A, int batch, const FftTab &T,
                        cudaStream_t st);
 
+// plan creation on the grid of L_j = 1024 (2047 = 23 x 89 samples): fills the device table of the Rader spectra the
+// prime-factor kernels of that grid use; until it has run on a device the grid stays on the Bluestein kernels there
+int pfa2047_init(cudaStream_t st);
 bool ring_pfa255_supported(bool real, const FftTab &T);              // a1, complex signals, the 255-sample grid
 int launch_ring_pfa255(bool fwd, const void *in, void *out, int nrows, size_t sig_stride, const FftTab &T, cudaStream_t st);
 bool ring_pfa4095_supported(bool real, const FftTab &T);             // a1, real signals, the 4095-sample grid

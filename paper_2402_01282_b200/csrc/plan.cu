@@ -618,6 +618,7 @@ int build_grid(s2w_plan *p, int Lg)
     }
     g.nt = p->dh ? 2 * Lg : Lg;
     T.nt = g.nt;
+    if (Lg == 1024 && !p->dh && (rc = pfa2047_init(0))) return rc;  // Rader spectra of the 2047-sample prime-factor kernels
     if (p->dh) {
         // Driscoll-Healy quadrature (their Theorem 3): q_t = (2/L) sin(theta_t) sum_{k<L} sin((2k+1) theta_t)/(2k+1)
         memset(&g.rw, 0, sizeof(g.rw));

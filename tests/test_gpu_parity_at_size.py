@@ -211,3 +211,24 @@ def test_alpha_gamma_prime_factor_4095(N):
     back = plan.inverse(w)
     assert float((back - f).abs().max()) < RT_TOL * float(f.abs().max())
     plan.close()
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 4])
+def test_alpha_gamma_prime_factor_2047(N):
+    """Row a8 (and a1) for real signals on the grid of L_j = 1024 (2047 = 23 x 89 alpha samples): the prime-factor kernels with
+    the Rader 89-point stage (pfa4095_kernels.cu), with no row n > 0 (N = 1), without a row n = 0 (even N), with a parked
+    row (N = 4); N = 5 is test_config3_full_size_sampled_parity.  Recovered f_lm against the seeded truth (ring FFTs),
+    sampled rings (both rings of a pair, the last pair) of the top scale against the oracle, synthesis through the round trip."""
+    torch, api = _api()
+    L, lam, J0 = 1024, 2.0, 9
+    flm = inputs.flm_real(L, 1500 + N, 2)
+    plan = api.s2wav_plan_create(L, N, lam, J0, True, True, 2)
+    f = plan.harmonic_inverse(torch.from_numpy(flm).cuda())
+    got = plan.harmonic_forward(f, L * (2 * L - 1)).cpu().numpy().reshape(2, L, 2 * L - 1)
+    assert np.abs(got - flm).max() / np.abs(flm).max() < FWD_TOL
+    w = plan.forward(f)
+    picks = [(plan.J, [0, 1, 514, 515, 1022, 1023])]
+    _check_sampled_rings(plan, w, flm[1], 1, L, N, lam, J0, True, picks)
+    back = plan.inverse(w)
+    assert float((back - f).abs().max()) < RT_TOL * float(f.abs().max())
+    plan.close()
