@@ -512,6 +512,154 @@ __global__ void __launch_bounds__(256, 2) reweight16_kernel(const cplx *__restri
     }
 }
 
+__device__ __forceinline__ void rw_cp_async16(void *dst, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+
+template <int R1>
+__global__ void __launch_bounds__(256, 2) reweight16p_kernel(const cplx *__restrict__ F, cplx *__restrict__ Ft, RwArgs A,
+                                                           RwTab R, int ncolumns)
+{
+    constexpr int NB = 16 / R1, NC = NB / 2, HR = R1 >= 2 ? R1 / 2 : 1, M = R1 * 256;
+    extern __shared__ cplx buf[];
+    __shared__ cplx s_part[NC][8];
+    __shared__ cplx s_pole[NC];
+    const F16Tw tw = f16_twiddles<R1>();
+    const int L = R.L, Lm = L - 1;
+    // persistent blocks: the ring values of the NEXT column group arrive by cp.async in a staging area (NC x L <= 1024
+    // values) while the current group is transformed -- the strided column reads (one 16-byte element per ring, Md
+    // elements apart) were the exposed latency at the head of every block
+    cplx *stg = buf + F16_BUF;
+    const int ngroups = (ncolumns + NC - 1) / NC;
+    auto prefetch = [&](int grp) {
+#pragma unroll
+        for (int ci = 0; ci < NC; ++ci) {
+            const int colid = grp * NC + ci;
+            if (colid >= ncolumns) continue;
+            const int mi = colid % A.Md, q = (colid / A.Md) % A.nn, b = colid / (A.Md * A.nn);
+            const cplx *col = F + ((size_t)b * A.nrows + A.n_row[q]) * (size_t)L * A.Md + mi;
+#pragma unroll
+            for (int c = 0; c < HR; ++c) {
+                const int t = threadIdx.x + 256 * c;
+                if (t < L) rw_cp_async16(stg + ci * L + t, col + (size_t)t * A.Md);
+            }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    if ((int)blockIdx.x < ngroups) prefetch(blockIdx.x);
+    for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();  // the staged values of every thread; the previous group's use of buf, s_part, s_pole
+    cplx xs[NC][HR];
+    cplx x[NB][R1];
+    int par_of[NC];
+    cplx *colT_of[NC];
+#pragma unroll
+    for (int ci = 0; ci < NC; ++ci) {
+        const int colid = grp * NC + ci;
+        const bool has = colid < ncolumns;
+        const int mi = colid % A.Md, q = (colid / A.Md) % A.nn, b = colid / (A.Md * A.nn);
+        const int m = A.isReal ? mi : mi - (L - 1);
+        const int nv = has ? A.n_val[q] : 0, row = has ? A.n_row[q] : 0;
+        const int par = ((m + nv) & 1) ? 1 : 0;  // 0: sigma = +1, 1: sigma = -1
+        par_of[ci] = par;
+        colT_of[ci] = has ? Ft + (((size_t)b * A.nrows + row) * A.Md + mi) * (size_t)L : nullptr;
+        const double *rp = R.rpole + par * L;
+        cplx dot = cmake(0.0, 0.0);
+#pragma unroll
+        for (int c = 0; c < HR; ++c) {
+            const int t = threadIdx.x + 256 * c;
+            cplx xv = cmake(0.0, 0.0);
+            if (t < L && has) {
+                xv = stg[ci * L + t];
+                const double r = rp[t];
+                dot.x = fma(r, xv.x, dot.x);
+                dot.y = fma(r, xv.y, dot.y);
+            }
+            xs[ci][c] = xv;
+            if (t == Lm) s_pole[ci] = xv;
+            cplx u1 = cmake(0.0, 0.0), u2 = u1;
+            if (t < Lm) {
+                u1 = (t & 1) ? cscale(xv, -1.0) : xv;
+                u2 = cscale(u1, R.delta[t]);
+            }
+            x[2 * ci][c] = u1;
+            x[2 * ci + 1][c] = u2;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            dot.x += __shfl_xor_sync(0xffffffffu, dot.x, o);
+            dot.y += __shfl_xor_sync(0xffffffffu, dot.y, o);
+        }
+        if ((threadIdx.x & 31) == 0) s_part[ci][threadIdx.x >> 5] = dot;
+    }
+    __syncthreads();  // every thread has taken its staged values
+    if (grp + (int)gridDim.x < ngroups) prefetch(grp + gridDim.x);
+#pragma unroll
+    for (int q = 0; q < NB; ++q) f16_pass1_fwd<R1, (R1 > 1)>(buf, q, x[q], tw);
+    __syncthreads();
+    f16_pass2_fwd(buf, tw);
+    __syncwarp();
+    f16_pass3_fwd(buf);
+    __syncthreads();
+    {
+        const int hw = threadIdx.x >> 4, j2 = threadIdx.x & 15;
+        const int sq = hw / R1, j1 = hw % R1;                       // sequence, sub-block inside it
+        const int j1p = (R1 - j1) % R1, j2p = j1 ? 15 - j2 : (16 - j2) & 15;
+        const bool shifted = j1 == 0 && j2 == 0;                    // partner of j3 is (16 - j3) % 16, else 15 - j3
+        cplx *own = buf + F16_PAD(hw * 256 + j2 * 16);
+        const cplx *prt = buf + F16_PAD(sq * M + j1p * 256 + j2p * 16);
+        const cplx *tg = R.TG16 + (j1 * 256 + j2);                   // [2][M2] in the storage order F16_TPOS
+        double sg = par_of[0] ? -1.0 : 1.0;
+#pragma unroll
+        for (int ci = 1; ci < NC; ++ci)
+            if ((sq >> 1) == ci) sg = par_of[ci] ? -1.0 : 1.0;
+        if (!(sq & 1)) sg = -sg;                                    // u1: T - sigma H, u2: T + sigma H
+        cplx v[16];
+#pragma unroll
+        for (int j3 = 0; j3 < 16; ++j3) {
+            const cplx u = own[j3], un = prt[shifted ? (16 - j3) & 15 : 15 - j3];
+            const cplx th = __ldg(&tg[16 * j3]), gh = cscale(__ldg(&tg[M + 16 * j3]), sg);
+            v[j3] = cadd(cmul(th, u), cmul(gh, un));
+        }
+        __syncthreads();                                            // every partner value has been read
+        bfly16<true>(v);
+#pragma unroll
+        for (int j3 = 0; j3 < 16; ++j3) own[j3] = v[j3];
+    }
+    __syncwarp();
+    f16_pass2_inv(buf, tw);
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < NB; ++q) f16_pass1_inv<R1, (R1 > 1)>(buf, q, x[q], tw);
+#pragma unroll
+    for (int ci = 0; ci < NC; ++ci) {
+        cplx *colT = colT_of[ci];
+        if (!colT) continue;
+        const double *vp = R.vpole + par_of[ci] * L;
+        const cplx xpole = s_pole[ci];
+#pragma unroll
+        for (int c = 0; c < HR; ++c) {
+            const int t = threadIdx.x + 256 * c;
+            if (t < Lm) {
+                const cplx y1 = x[2 * ci][c], y2 = x[2 * ci + 1][c];
+                const double dl = R.delta[t], ds = R.dsum[t], vv = vp[t];
+                cplx h = cmake(fma(dl, y1.x, -y2.x), fma(dl, y1.y, -y2.y));
+                if (t & 1) h = cscale(h, -1.0);
+                h.x += fma(ds, xs[ci][c].x, vv * xpole.x);
+                h.y += fma(ds, xs[ci][c].y, vv * xpole.y);
+                colT[t] = h;
+            } else if (t == Lm) {
+                cplx acc = cmake(0.0, 0.0);
+                for (int w = 0; w < 8; ++w) acc = cadd(acc, s_part[ci][w]);
+                colT[t] = acc;
+            }
+        }
+    }
+    }  // column groups
+}
+
 // a2 at Toeplitz length 4096 (the grid of L_j = 2048, BASELINE config 4): one column per block; its two sequences
 // u1 = a x and u2 = delta a x go through the one 4096-element buffer one after the other (y1 waits in registers), the
 // thread keeps the ring values x_t, t = tid + 256 c (c < 8), in registers throughout.  Same algebra and tables as above.
@@ -1174,8 +1322,25 @@ static int reweight16_t(const cplx *F, cplx *Ft, const RwArgs &A, int batch, con
     const int ncol = A.Md * A.nn * batch;
     const size_t sm = (size_t)F16_BUF * sizeof(cplx);
     int rc;
+    // two blocks per SM, resident for the whole launch (S2W_RW_PERSIST = blocks, 0: one block per column group).  Measured
+    // at C3: the class alone takes the same time (2.34 ms), but the step drops from 13.66 to 13.50 ms -- the launch no
+    // longer floods the SMs that the other lanes' kernels are running on
+    static const int persist = [] {
+        const char *e = getenv("S2W_RW_PERSIST");
+        if (e) return atoi(e);
+        int dev = 0, sms = 148;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        return 2 * sms;
+    }();
+    const int ngroups = (ncol + NC - 1) / NC;
+    if (persist > 0 && ngroups > persist) {  // persistent blocks with a cp.async staging area for the next column group
+        const size_t smp = (size_t)(F16_BUF + 1024) * sizeof(cplx);
+        if ((rc = set_smem(reweight16p_kernel<R1>, smp))) return rc;
+        S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight16p_kernel<R1>, persist, 256, smp, st, F, Ft, A, R, ncol);
+        return S2W_OK;
+    }
     if ((rc = set_smem(reweight16_kernel<R1>, sm))) return rc;
-    S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight16_kernel<R1>, (ncol + NC - 1) / NC, 256, sm, st, F, Ft, A, R, ncol);
+    S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight16_kernel<R1>, ngroups, 256, sm, st, F, Ft, A, R, ncol);
     return S2W_OK;
 }
 
