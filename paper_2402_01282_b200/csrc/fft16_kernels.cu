@@ -672,8 +672,7 @@ __global__ void __launch_bounds__(256, 2) reweight16w_kernel(const cplx *__restr
     __shared__ cplx s_pole;
     const F16Tw tw = f16_twiddles<R1>();
     const int L = R.L, Lm = L - 1;
-    const int colid = blockIdx.x;
-    if (colid >= ncolumns) return;
+    for (int colid = blockIdx.x; colid < ncolumns; colid += gridDim.x) {  // resident blocks walk over the columns
     const int mi = colid % A.Md, q = (colid / A.Md) % A.nn, b = colid / (A.Md * A.nn);
     const int m = A.isReal ? mi : mi - (L - 1);
     const int par = ((m + A.n_val[q]) & 1) ? 1 : 0;  // 0: sigma = +1, 1: sigma = -1
@@ -768,6 +767,8 @@ __global__ void __launch_bounds__(256, 2) reweight16w_kernel(const cplx *__restr
             for (int w = 0; w < 8; ++w) acc = cadd(acc, s_part[w]);
             colT[t] = acc;
         }
+    }
+    __syncthreads();  // buf, s_part, s_pole are reused by the next column
     }
 }
 
@@ -1352,7 +1353,15 @@ int launch_reweight16(const cplx *F, cplx *Ft, const RwArgs &A, int batch, const
         const size_t sm = (size_t)(F16_BUF + 2048) * sizeof(cplx);
         int rc = set_smem(reweight16w_kernel, sm);
         if (rc) return rc;
-        S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight16w_kernel, ncol, 256, sm, st, F, Ft, A, R, ncol);
+        static const int persist_w = [] {
+            const char *e = getenv("S2W_RW_PERSIST");
+            if (e) return atoi(e);
+            int dev = 0, sms = 148;
+            if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            return 2 * sms;
+        }();
+        const int nblk = (persist_w > 0 && ncol > persist_w) ? persist_w : ncol;
+        S2W_LAUNCH_C(S2W_K_REWEIGHT, reweight16w_kernel, nblk, 256, sm, st, F, Ft, A, R, ncol);
         return S2W_OK;
     }
     case 2048: return reweight16_t<8>(F, Ft, A, batch, R, st);
